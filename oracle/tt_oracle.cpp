@@ -1,0 +1,461 @@
+// oracle/tt_oracle.cpp -- TEST INFRASTRUCTURE, NOT THE PRODUCT.
+//
+// Plain, slow, fp64 CPU oracle for the triangle-triangle intersection energy of
+// arXiv 2606.06511.  It follows the paper's Appendix A listing
+// step by step, in the listing's order and notation, with its own
+// forward-mode dual numbers (value + 18 partials) -- the same technique the listing uses
+// (PAPER.md L51, L59).  It shares no code with the CUDA path (which differentiates the
+// end-points analytically) and is only ever imported by tests/, __graft_entry__.smoke()
+// and bench.py's cpu_baseline / --impl reference legs.
+//
+// Every function is pinned by tests/test_oracle_*.py (-m "not gpu") against hand-worked
+// examples, closed forms, invariants, finite differences and brute force; nothing here is
+// "parity unpinned".  Readings of garbled/ambiguous passages (A1..A15) are listed in DESIGN.md.
+//
+// Build: g++ -O2 -ffp-contract=off -fopenmp -shared -fPIC  (no -ffast-math; A14).
+
+#include <algorithm>
+#include <cmath>
+#include <cstdint>
+#include <cstring>
+#include <vector>
+#ifdef _OPENMP
+#include <omp.h>
+#endif
+
+namespace {
+
+constexpr int NDOF = 18;  // x = [a0,a1,a2,b0,b1,b2], 6 vertices x 3 (`loc`)
+
+// ---- forward-mode dual number: value + 18 partials (stands in for autodiff::dual, L59) ----
+struct Dual {
+  double val;
+  double d[NDOF];
+};
+
+inline Dual constant(double c) {
+  Dual r;
+  r.val = c;
+  for (int i = 0; i < NDOF; ++i) r.d[i] = 0.0;
+  return r;
+}
+inline Dual variable(double c, int idx) {
+  Dual r = constant(c);
+  r.d[idx] = 1.0;
+  return r;
+}
+inline Dual operator+(const Dual& a, const Dual& b) {
+  Dual r;
+  r.val = a.val + b.val;
+  for (int i = 0; i < NDOF; ++i) r.d[i] = a.d[i] + b.d[i];
+  return r;
+}
+inline Dual operator-(const Dual& a, const Dual& b) {
+  Dual r;
+  r.val = a.val - b.val;
+  for (int i = 0; i < NDOF; ++i) r.d[i] = a.d[i] - b.d[i];
+  return r;
+}
+inline Dual operator*(const Dual& a, const Dual& b) {
+  Dual r;
+  r.val = a.val * b.val;
+  for (int i = 0; i < NDOF; ++i) r.d[i] = a.d[i] * b.val + a.val * b.d[i];
+  return r;
+}
+inline Dual operator*(double s, const Dual& a) {
+  Dual r;
+  r.val = s * a.val;
+  for (int i = 0; i < NDOF; ++i) r.d[i] = s * a.d[i];
+  return r;
+}
+inline Dual operator/(const Dual& a, const Dual& b) {
+  Dual r;
+  r.val = a.val / b.val;
+  for (int i = 0; i < NDOF; ++i) r.d[i] = (a.d[i] - r.val * b.d[i]) / b.val;
+  return r;
+}
+inline Dual dsqrt(const Dual& a) {
+  Dual r;
+  r.val = std::sqrt(a.val);
+  for (int i = 0; i < NDOF; ++i) r.d[i] = a.d[i] / (2.0 * r.val);
+  return r;
+}
+// min/max on duals select value AND partials of the selected argument (App. A).
+inline Dual dmin(const Dual& a, const Dual& b) { return (b.val < a.val) ? b : a; }
+inline Dual dmax(const Dual& a, const Dual& b) { return (b.val > a.val) ? b : a; }
+
+struct Vec3 {
+  Dual x, y, z;
+};
+inline Vec3 operator+(const Vec3& a, const Vec3& b) { return {a.x + b.x, a.y + b.y, a.z + b.z}; }
+inline Vec3 operator-(const Vec3& a, const Vec3& b) { return {a.x - b.x, a.y - b.y, a.z - b.z}; }
+inline Vec3 operator*(const Dual& s, const Vec3& a) { return {s * a.x, s * a.y, s * a.z}; }
+inline Vec3 operator*(double s, const Vec3& a) { return {s * a.x, s * a.y, s * a.z}; }
+inline Vec3 operator/(const Vec3& a, const Dual& s) { return {a.x / s, a.y / s, a.z / s}; }
+inline Dual dot(const Vec3& a, const Vec3& b) { return a.x * b.x + a.y * b.y + a.z * b.z; }
+inline Vec3 cross(const Vec3& a, const Vec3& b) {
+  return {a.y * b.z - a.z * b.y, a.z * b.x - a.x * b.z, a.x * b.y - a.y * b.x};
+}
+inline Vec3 normalized(const Vec3& a) {  // Vector3dual::normalize()
+  Dual n = dsqrt(dot(a, a));
+  return a / n;
+}
+
+// ---- App. A `intersects` -----------------------------------------------
+// Plane triangle (U0,U1,U2) cuts triangle (V0,V1,V2); on success segment0/1 are the two
+// end-points of the cut.  Readings A1-A4 of DESIGN.md.
+bool intersects(const Vec3& U0, const Vec3& U1, const Vec3& U2, const Vec3& V0, const Vec3& V1,
+                const Vec3& V2, Vec3& segment0, Vec3& segment1) {
+  Vec3 edge1 = U1 - U0;                  // L78
+  Vec3 edge2 = U2 - U0;                  // L79
+  Vec3 normal = cross(edge1, edge2);     // L80
+  // A degenerate plane triangle has no normal: "not coplanar" precondition (L11) fails.
+  if (!(dot(normal, normal).val > 0.0)) return false;
+  normal = normalized(normal);           // L81
+  Dual d[3];
+  int positive = 0, negative = 0, zero = 0;  // L83
+  d[0] = dot(normal, V0 - U0);           // L84
+  d[1] = dot(normal, V1 - U1);           // L85 (as printed: U1; n.(U1-U0) == 0 identically, A1)
+  d[2] = dot(normal, V2 - U2);           // L86 (as printed: U2)
+  for (int i = 0; i < 3; ++i) {          // L87-93 (A2)
+    if (d[i].val > 0.0) ++positive;
+    else if (d[i].val < 0.0) ++negative;
+    else ++zero;
+  }
+  const Vec3* V[3] = {&V0, &V1, &V2};
+  // crossing point of edge (V_i, V_k): (d_i V_k - d_k V_i) / (d_i - d_k)  (L100-101, L104-105)
+  auto crossing = [&](int i, int k) -> Vec3 {
+    return (d[i] * (*V[k]) - d[k] * (*V[i])) / (d[i] - d[k]);
+  };
+  if (positive > 0 && negative > 0) {    // L95
+    if (positive == 2 || negative == 2) {  // L96 / L102: two on one side, one alone (A3)
+      int k;                               // the lone vertex
+      if (positive == 2) k = (d[0].val < 0.0) ? 0 : (d[1].val < 0.0) ? 1 : 2;
+      else               k = (d[0].val > 0.0) ? 0 : (d[1].val > 0.0) ? 1 : 2;
+      int i = (k + 1) % 3, j = (k + 2) % 3;
+      // printed instances: k=1 -> (0,1),(2,1) at L100-101;  k=2 -> (0,2),(1,2) at L104-105.
+      if (i > j) std::swap(i, j);
+      segment0 = crossing(i, k);
+      segment1 = crossing(j, k);
+    } else {                              // L106: positive == 1, negative == 1, zero == 1 (A4)
+      int z = (d[0].val == 0.0) ? 0 : (d[1].val == 0.0) ? 1 : 2;
+      int i = (z + 1) % 3, j = (z + 2) % 3;
+      segment0 = *V[z];                   // L109 / L112: the vertex lying on the plane
+      segment1 = crossing(j, i);          // L110 prints (d2 V1 - d1 V2)/(d2 - d1) for z = 0
+    }
+    return true;                          // L117
+  }
+  return false;                           // L120
+}
+
+struct PairResult {
+  bool active;
+  double tc[2];
+  double g[2][NDOF];  // g[0] = d tc0 / dx, g[1] = d tc1 / dx   (x = [a0,a1,a2,b0,b1,b2])
+};
+
+// ---- App. A `3DTTIT` + Eq. 1 ------------------------------------------
+// x holds T_a = (a0,a1,a2) then T_b = (b0,b1,b2).  The listing names the triangle whose
+// segment is S00/S01 (interval I_a) `U` and the other `V`; so U := T_a, V := T_b, and the dual
+// seeds are placed so that partial index 3m+c is a_m[c] and 9+3m+c is b_m[c].
+PairResult pair_3dttit(const double x[NDOF], double sigma) {
+  PairResult r;
+  r.active = false;
+  r.tc[0] = r.tc[1] = 0.0;
+  std::memset(r.g, 0, sizeof(r.g));
+  Vec3 U[3], V[3];
+  for (int m = 0; m < 3; ++m) {
+    U[m] = {variable(x[3 * m + 0], 3 * m + 0), variable(x[3 * m + 1], 3 * m + 1),
+            variable(x[3 * m + 2], 3 * m + 2)};
+    V[m] = {variable(x[9 + 3 * m + 0], 9 + 3 * m + 0), variable(x[9 + 3 * m + 1], 9 + 3 * m + 1),
+            variable(x[9 + 3 * m + 2], 9 + 3 * m + 2)};
+  }
+  Vec3 S00, S01, S10, S11;
+  if (intersects(V[0], V[1], V[2], U[0], U[1], U[2], S00, S01) &&   // L134: plane(V) cuts U
+      intersects(U[0], U[1], U[2], V[0], V[1], V[2], S10, S11)) {   // L135: plane(U) cuts V
+    Vec3 uNormal = cross(U[1] - U[0], U[2] - U[0]);                  // L137
+    Vec3 vNormal = cross(V[1] - V[0], V[2] - V[0]);                  // L139
+    Vec3 D = cross(uNormal, vNormal);                                // L141
+    if (!(dot(D, D).val > 0.0)) return r;  // parallel planes: excluded by L11 ("not coplanar")
+    D = normalized(D);                                               // L142
+    Vec3 A = 0.25 * (S00 + S01 + S10 + S11);                         // L144
+    Dual t00 = dot(D, S00 - A);                                      // L145
+    Dual t01 = dot(D, S01 - A);
+    Dual t10 = dot(D, S10 - A);
+    Dual t11 = dot(D, S11 - A);
+    Dual ta0 = dmin(t00, t01);                                       // L149
+    Dual ta1 = dmax(t00, t01);
+    Dual tb0 = dmin(t10, t11);
+    Dual tb1 = dmax(t10, t11);
+    bool intersected = (ta1.val > tb0.val && ta0.val < tb1.val);     // L153
+    if (!intersected) return r;                                      // A11: tc := (0,0)
+    Dual tc0 = sigma * (ta0 - tb1);  // Eq. 1 (L13) with sigma = 1; L154 prints sigma = 0.5 (A6)
+    Dual tc1 = sigma * (ta1 - tb0);  // L155
+    r.active = true;
+    r.tc[0] = tc0.val;
+    r.tc[1] = tc1.val;
+    for (int i = 0; i < NDOF; ++i) {
+      r.g[0][i] = tc0.d[i];
+      r.g[1][i] = tc1.d[i];
+    }
+  }
+  return r;
+}
+
+// Eq. 2 (L17)
+inline double energy_of(const double tc[2]) {
+  double p = tc[0] * tc[1];
+  return p * p;
+}
+
+// Eq. 3 coefficients (L21-24): grad = cg[0] g0 + cg[1] g1
+inline void grad_coeffs(const double tc[2], double cg[2]) {
+  cg[0] = 2.0 * tc[0] * (tc[1] * tc[1]);
+  cg[1] = 2.0 * tc[1] * (tc[0] * tc[0]);
+}
+
+// Eq. 4 coefficients (L26-33) + eigenanalysis reading A7 (L47):
+// H = c00 g0 g0^T + c11 g1 g1^T + c01 (g1 g0^T + g0 g1^T)
+//   mode 0 EQ4    : all three parts verbatim
+//   mode 1 FILTER : third part kept iff L47's quantity 8 tc0 tc1 (g0.g1) >= 0
+//   mode 2 PSD2   : parts one and two only
+inline void hess_coeffs(const double tc[2], const double g0[NDOF], const double g1[NDOF], int mode,
+                        double c[3], double lam[3]) {
+  double n0 = 0.0, n1 = 0.0, g01 = 0.0;
+  for (int i = 0; i < NDOF; ++i) {
+    n0 += g0[i] * g0[i];
+    n1 += g1[i] * g1[i];
+    g01 += g0[i] * g1[i];
+  }
+  lam[0] = 2.0 * (tc[1] * tc[1]) * n0;   // L47, first part
+  lam[1] = 2.0 * (tc[0] * tc[0]) * n1;   // L47, second part
+  lam[2] = 8.0 * tc[0] * tc[1] * g01;    // L47, third part ("might be negative")
+  c[0] = 2.0 * (tc[1] * tc[1]);
+  c[1] = 2.0 * (tc[0] * tc[0]);
+  double keep = 1.0;
+  if (mode == 1) keep = (lam[2] >= 0.0) ? 1.0 : 0.0;
+  if (mode == 2) keep = 0.0;
+  c[2] = 4.0 * tc[0] * tc[1] * keep;
+}
+
+inline bool share_vertex(const int32_t* ta, const int32_t* tb) {
+  for (int i = 0; i < 3; ++i)
+    for (int j = 0; j < 3; ++j)
+      if (ta[i] == tb[j]) return true;
+  return false;
+}
+
+inline void gather_x(const double* pos, const int32_t* tris, const int32_t* pr, double x[NDOF],
+                     int32_t vid[6]) {
+  const int32_t* ta = tris + 3 * (int64_t)pr[0];
+  const int32_t* tb = tris + 3 * (int64_t)pr[1];
+  for (int m = 0; m < 3; ++m) {
+    vid[m] = ta[m];
+    vid[3 + m] = tb[m];
+  }
+  for (int v = 0; v < 6; ++v)
+    for (int c = 0; c < 3; ++c) x[3 * v + c] = pos[3 * (int64_t)vid[v] + c];
+}
+
+// Neumaier-compensated accumulation (oracle step 12)
+struct Neumaier {
+  double s = 0.0, c = 0.0;
+  void add(double v) {
+    double t = s + v;
+    if (std::fabs(s) >= std::fabs(v)) c += (s - t) + v;
+    else c += (v - t) + s;
+    s = t;
+  }
+  double value() const { return s + c; }
+};
+
+}  // namespace
+
+extern "C" {
+
+// One pair given as 18 coordinates x = [a0,a1,a2,b0,b1,b2].  Any output pointer may be NULL.
+// H is dense 18x18 row-major; lam = L47's three printed quantities.
+void tt_oracle_pair(const double* x, double sigma, int hess_mode, int* active, double* tc,
+                    double* energy, double* g0, double* g1, double* grad, double* H, double* lam) {
+  PairResult r = pair_3dttit(x, sigma);
+  if (active) *active = r.active ? 1 : 0;
+  if (tc) { tc[0] = r.tc[0]; tc[1] = r.tc[1]; }
+  double T = r.active ? energy_of(r.tc) : 0.0;
+  if (energy) *energy = T;
+  if (g0) std::memcpy(g0, r.g[0], sizeof(double) * NDOF);
+  if (g1) std::memcpy(g1, r.g[1], sizeof(double) * NDOF);
+  double cg[2] = {0, 0}, c[3] = {0, 0, 0}, l[3] = {0, 0, 0};
+  if (r.active) {
+    grad_coeffs(r.tc, cg);
+    hess_coeffs(r.tc, r.g[0], r.g[1], hess_mode, c, l);
+  }
+  if (grad)
+    for (int i = 0; i < NDOF; ++i) grad[i] = cg[0] * r.g[0][i] + cg[1] * r.g[1][i];
+  if (H)
+    for (int i = 0; i < NDOF; ++i)
+      for (int j = 0; j < NDOF; ++j)
+        H[i * NDOF + j] = c[0] * r.g[0][i] * r.g[0][j] + c[1] * r.g[1][i] * r.g[1][j] +
+                          c[2] * (r.g[1][i] * r.g[0][j] + r.g[0][i] * r.g[1][j]);
+  if (lam) { lam[0] = l[0]; lam[1] = l[1]; lam[2] = l[2]; }
+}
+
+// Steps 1-9 for every candidate pair.  Outputs (each may be NULL): active[P] (0/1), tc[P,2],
+// T[P], J[P,2,18] (zero rows for inactive pairs).  Returns sum of T (Neumaier, ascending order).
+// Pairs sharing a vertex index are "topologically adjacent" (L11, A9) -> inactive.
+double tt_oracle_pairs(const double* pos, int64_t n_verts, const int32_t* tris, int64_t n_tris,
+                       const int32_t* pairs, int64_t n_pairs, double sigma, uint8_t* active,
+                       double* tc, double* T, double* J, int n_threads) {
+  (void)n_verts; (void)n_tris;
+  std::vector<double> Tloc((size_t)n_pairs, 0.0);
+#ifdef _OPENMP
+  if (n_threads > 0) omp_set_num_threads(n_threads);
+#endif
+#pragma omp parallel for schedule(static)
+  for (int64_t k = 0; k < n_pairs; ++k) {
+    const int32_t* pr = pairs + 2 * k;
+    PairResult r;
+    r.active = false;
+    if (!share_vertex(tris + 3 * (int64_t)pr[0], tris + 3 * (int64_t)pr[1])) {
+      double x[NDOF];
+      int32_t vid[6];
+      gather_x(pos, tris, pr, x, vid);
+      r = pair_3dttit(x, sigma);
+    }
+    if (active) active[k] = r.active ? 1 : 0;
+    if (tc) { tc[2 * k] = r.active ? r.tc[0] : 0.0; tc[2 * k + 1] = r.active ? r.tc[1] : 0.0; }
+    Tloc[k] = r.active ? energy_of(r.tc) : 0.0;
+    if (J) {
+      if (r.active) {
+        std::memcpy(J + 36 * k, r.g[0], sizeof(double) * NDOF);
+        std::memcpy(J + 36 * k + 18, r.g[1], sizeof(double) * NDOF);
+      } else {
+        std::memset(J + 36 * k, 0, sizeof(double) * 36);
+      }
+    }
+  }
+  Neumaier acc;
+  for (int64_t k = 0; k < n_pairs; ++k) acc.add(Tloc[k]);
+  if (T) std::memcpy(T, Tloc.data(), sizeof(double) * (size_t)n_pairs);
+  return acc.value();
+}
+
+// Step 12, pattern: sorted-unique (p,q) over the 6x6 vertex pairs of every active pair.
+// Writes rowptr[nV+1]; if colind != NULL (capacity >= returned nnzb) also writes colind.
+int64_t tt_oracle_bsr_pattern(int64_t n_verts, const int32_t* tris, const int32_t* pairs,
+                              int64_t n_pairs, const uint8_t* active, int32_t* rowptr,
+                              int32_t* colind) {
+  std::vector<uint64_t> keys;
+  for (int64_t k = 0; k < n_pairs; ++k) {
+    if (!active[k]) continue;
+    int32_t vid[6];
+    for (int m = 0; m < 3; ++m) {
+      vid[m] = tris[3 * (int64_t)pairs[2 * k] + m];
+      vid[3 + m] = tris[3 * (int64_t)pairs[2 * k + 1] + m];
+    }
+    for (int i = 0; i < 6; ++i)
+      for (int j = 0; j < 6; ++j) keys.push_back(((uint64_t)(uint32_t)vid[i] << 32) | (uint32_t)vid[j]);
+  }
+  std::sort(keys.begin(), keys.end());
+  keys.erase(std::unique(keys.begin(), keys.end()), keys.end());
+  for (int64_t v = 0; v <= n_verts; ++v) rowptr[v] = 0;
+  for (uint64_t key : keys) rowptr[(key >> 32) + 1] += 1;
+  for (int64_t v = 0; v < n_verts; ++v) rowptr[v + 1] += rowptr[v];
+  if (colind)
+    for (size_t i = 0; i < keys.size(); ++i) colind[i] = (int32_t)(keys[i] & 0xffffffffu);
+  return (int64_t)keys.size();
+}
+
+// Steps 10-12, numeric: grad[nV,3] and vals[nnzb,3,3] (row-major blocks) accumulated in
+// ASCENDING PAIR ORDER from the per-pair J = [g0; g1] and tc produced by tt_oracle_pairs.
+// rowptr/colind are the pattern from tt_oracle_bsr_pattern.  grad / vals may be NULL.
+void tt_oracle_assemble(int64_t n_verts, const int32_t* tris, const int32_t* pairs, int64_t n_pairs,
+                        const uint8_t* active, const double* tc, const double* J, int hess_mode,
+                        const int32_t* rowptr, const int32_t* colind, double* grad, double* vals) {
+  if (grad) std::memset(grad, 0, sizeof(double) * 3 * (size_t)n_verts);
+  if (vals) std::memset(vals, 0, sizeof(double) * 9 * (size_t)rowptr[n_verts]);
+  for (int64_t k = 0; k < n_pairs; ++k) {
+    if (!active[k]) continue;
+    int32_t vid[6];
+    for (int m = 0; m < 3; ++m) {
+      vid[m] = tris[3 * (int64_t)pairs[2 * k] + m];
+      vid[3 + m] = tris[3 * (int64_t)pairs[2 * k + 1] + m];
+    }
+    const double* g0 = J + 36 * k;
+    const double* g1 = g0 + 18;
+    double cg[2], c[3], lam[3];
+    grad_coeffs(tc + 2 * k, cg);
+    hess_coeffs(tc + 2 * k, g0, g1, hess_mode, c, lam);
+    if (grad)
+      for (int v = 0; v < 6; ++v)
+        for (int a = 0; a < 3; ++a)
+          grad[3 * (int64_t)vid[v] + a] += cg[0] * g0[3 * v + a] + cg[1] * g1[3 * v + a];
+    if (vals)
+      for (int p = 0; p < 6; ++p)
+        for (int q = 0; q < 6; ++q) {
+          const int32_t* lo = colind + rowptr[vid[p]];
+          const int32_t* hi = colind + rowptr[vid[p] + 1];
+          const int32_t* it = std::lower_bound(lo, hi, vid[q]);
+          double* blk = vals + 9 * (int64_t)(it - colind);
+          for (int a = 0; a < 3; ++a)
+            for (int b = 0; b < 3; ++b) {
+              int i = 3 * p + a, j = 3 * q + b;
+              blk[3 * a + b] += c[0] * g0[i] * g0[j] + c[1] * g1[i] * g1[j] +
+                                c[2] * (g1[i] * g0[j] + g0[i] * g1[j]);
+            }
+        }
+  }
+}
+
+// H.p, way one: per active pair y_loc = J^T M (J p_loc), scattered in ascending pair order.
+void tt_oracle_hess_vec_pairs(int64_t n_verts, const int32_t* tris, const int32_t* pairs,
+                              int64_t n_pairs, const uint8_t* active, const double* tc,
+                              const double* J, int hess_mode, const double* p, double* y) {
+  std::memset(y, 0, sizeof(double) * 3 * (size_t)n_verts);
+  for (int64_t k = 0; k < n_pairs; ++k) {
+    if (!active[k]) continue;
+    int32_t vid[6];
+    for (int m = 0; m < 3; ++m) {
+      vid[m] = tris[3 * (int64_t)pairs[2 * k] + m];
+      vid[3 + m] = tris[3 * (int64_t)pairs[2 * k + 1] + m];
+    }
+    const double* g0 = J + 36 * k;
+    const double* g1 = g0 + 18;
+    double c[3], lam[3];
+    hess_coeffs(tc + 2 * k, g0, g1, hess_mode, c, lam);
+    double s0 = 0.0, s1 = 0.0;   // J p_loc
+    for (int v = 0; v < 6; ++v)
+      for (int a = 0; a < 3; ++a) {
+        s0 += g0[3 * v + a] * p[3 * (int64_t)vid[v] + a];
+        s1 += g1[3 * v + a] * p[3 * (int64_t)vid[v] + a];
+      }
+    double u0 = c[0] * s0 + c[2] * s1;   // M (J p_loc),  M = [[c00, c01], [c01, c11]]
+    double u1 = c[2] * s0 + c[1] * s1;
+    for (int v = 0; v < 6; ++v)
+      for (int a = 0; a < 3; ++a) y[3 * (int64_t)vid[v] + a] += u0 * g0[3 * v + a] + u1 * g1[3 * v + a];
+  }
+}
+
+// H.p, way two: plain BSR (3x3 row-major blocks) times vector.
+void tt_oracle_bsr_matvec(int64_t n_verts, const int32_t* rowptr, const int32_t* colind,
+                          const double* vals, const double* p, double* y) {
+  for (int64_t r = 0; r < n_verts; ++r) {
+    double acc[3] = {0, 0, 0};
+    for (int32_t e = rowptr[r]; e < rowptr[r + 1]; ++e) {
+      const double* blk = vals + 9 * (int64_t)e;
+      const double* pv = p + 3 * (int64_t)colind[e];
+      for (int a = 0; a < 3; ++a)
+        for (int b = 0; b < 3; ++b) acc[a] += blk[3 * a + b] * pv[b];
+    }
+    for (int a = 0; a < 3; ++a) y[3 * r + a] = acc[a];
+  }
+}
+
+int tt_oracle_max_threads(void) {
+#ifdef _OPENMP
+  return omp_get_max_threads();
+#else
+  return 1;
+#endif
+}
+
+}  // extern "C"
