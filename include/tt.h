@@ -1,0 +1,152 @@
+/* include/tt.h -- C ABI of libtt.so: the B200 (sm_100a) hot path of arXiv 2606.06511,
+ * "Differentiable 3D Triangle-Triangle Intersection Energy".
+ *
+ * The problem is stated as the paper states it: vertex positions,
+ * triangles, and a list of candidate triangle pairs (the broad phase that produces them, L51,
+ * is a separate structure and not part of this library).  For every candidate pair (T_a, T_b)
+ * that is not topologically adjacent (shares no vertex index, L11):
+ *   1. Moeller's intervals I_a, I_b on the planes' intersection line and
+ *      I_c = [t_c^0, t_c^1] = [t_a^0 - t_b^1, t_a^1 - t_b^0]            (L9-15, Eq. 1);
+ *      the pair is ACTIVE iff t_c^0 < 0 < t_c^1 (strict; coplanar/touching/degenerate: inactive)
+ *   2. energy  T = (t_c^0 t_c^1)^2 for active pairs, 0 otherwise           (L17, Eq. 2)
+ *   3. g0 = d t_c^0/dx, g1 = d t_c^1/dx over the pair's 18 DOF; gradient
+ *      2 t_c^0 (t_c^1)^2 g0 + 2 t_c^1 (t_c^0)^2 g1                          (L21-24, Eq. 3)
+ *      and the outer-product Hessian  c00 g0 g0^T + c11 g1 g1^T + c01 (g1 g0^T + g0 g1^T),
+ *      c00 = 2 (t_c^1)^2, c11 = 2 (t_c^0)^2, c01 = 4 t_c^0 t_c^1 * keep     (L26-33, Eq. 4),
+ *      `keep` chosen by tt_hess_mode from the eigen-analysis of L47
+ *   4. assembly into a per-vertex gradient [nV,3] and a 3x3-block BSR matrix (L51), or the
+ *      matrix-free product y = H p.
+ *
+ * Conventions
+ *   - Unless a parameter says HOST, every array pointer is a DEVICE pointer owned by the caller
+ *     (e.g. a PyTorch tensor's data_ptr()).  The library never frees or reallocates caller memory.
+ *     Workspace is owned by the opaque tt_ctx (cudaMalloc, grow-only, freed by tt_destroy).
+ *   - dtype (tt_options.dtype) selects the element type of pos, energy, grad, vals, p, y, tc:
+ *     TT_F64 = double, TT_F32 = float.  With TT_F32 the discrete decisions (plane sides, min/max,
+ *     t_c^0 < 0 < t_c^1, the FILTER sign) are still taken in fp64 on the fp32-rounded positions, so the
+ *     active set equals the fp64 oracle's on those positions (reading A12).
+ *   - Layouts: pos [nV,3] row-major; tris [nT,3] int32 vertex ids; pairs [P,2] int32 triangle ids
+ *     (pairs[k,0] is T_a, pairs[k,1] is T_b); grad, p, y [nV,3]; BSR: rowptr [nV+1] int32,
+ *     colind [nnzb] int32 (ascending within a row), vals [nnzb,3,3] row-major blocks.  The
+ *     pattern is the union over active pairs of their 6x6 vertex pairs (both triangles, full --
+ *     not only the upper triangle).
+ *   - All work is enqueued on `stream` (a cudaStream_t passed as void*, NULL = default stream).
+ *     tt_energy, tt_energy_grad_hess and tt_hess_vec are asynchronous; tt_hess_symbolic and the
+ *     *_host call synchronise the stream before returning (they hand sizes/results to the host).
+ *   - Outputs are OVERWRITTEN, never accumulated into: grad / y / vals are fully defined on
+ *     return (zeros where nothing contributes).
+ *   - Errors: every call returns a tt_status (negative = failure) and leaves a message readable
+ *     with tt_last_error(ctx).  Index range (tris < nV, pairs < nT) is the caller's
+ *     responsibility (undefined behaviour otherwise); sizes, NULLs and state are checked.
+ *   - One tt_ctx per stream; a ctx is not thread-safe.  There is no CPU fallback anywhere.
+ */
+#ifndef TT_H_
+#define TT_H_
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct tt_ctx tt_ctx;
+
+typedef enum {
+  TT_OK = 0,
+  TT_ERR_INVALID_ARG = -1, /* NULL / negative size / unknown enum / too many rows for int32        */
+  TT_ERR_CUDA = -2,        /* a CUDA runtime call failed (message holds cudaGetErrorString)        */
+  TT_ERR_NOMEM = -3,       /* workspace allocation failed                                           */
+  TT_ERR_CAPACITY = -4,    /* nnzb_capacity smaller than the pattern computed by tt_hess_symbolic   */
+  TT_ERR_STATE = -5        /* numeric / H.p call without a matching tt_hess_symbolic                */
+} tt_status;
+
+typedef enum { TT_F64 = 0, TT_F32 = 1 } tt_dtype;
+
+/* Treatment of Eq. 4's third part ("might be negative"; reading A7):
+ *   TT_HESS_EQ4    all three parts as printed
+ *   TT_HESS_FILTER third part kept iff L47's quantity 8 t_c^0 t_c^1 (g0.g1) >= 0   (default)
+ *   TT_HESS_PSD2   first two parts only (always positive semi-definite)                          */
+typedef enum { TT_HESS_EQ4 = 0, TT_HESS_FILTER = 1, TT_HESS_PSD2 = 2 } tt_hess_mode;
+
+typedef struct {
+  int32_t dtype;      /* tt_dtype                                                                   */
+  int32_t hess_mode;  /* tt_hess_mode                                                               */
+  double tc_scale;    /* sigma multiplying t_c^0, t_c^1: 1.0 = Eq. 1 (L13); 0.5 = App. A   */
+  int32_t device;     /* CUDA device ordinal                                                        */
+  int32_t flags;      /* TT_FLAG_* bits, 0 for defaults                                             */
+} tt_options;
+
+/* Force every BSR row through the general (shared-vertex) merge path; used by tests to cover it
+ * on inputs whose rows would otherwise all take the exclusive-row fast path.                      */
+#define TT_FLAG_FORCE_GENERAL_ROWS 1
+
+typedef struct {
+  const void* pos;      int64_t n_verts;   /* [nV,3] dtype                                          */
+  const int32_t* tris;  int64_t n_tris;    /* [nT,3]                                                */
+  const int32_t* pairs; int64_t n_pairs;   /* [P,2], any order, duplicates allowed                  */
+} tt_problem;
+
+/* Create / destroy a context.  tt_create validates options and selects the device. */
+tt_status tt_create(const tt_options* opt, tt_ctx** out);
+void tt_destroy(tt_ctx* ctx);
+
+/* Steps 1-2 (Eq. 1-2) for every candidate pair.
+ *   energy_sum      [1] dtype: sum of T over all pairs (deterministic reduction order)
+ *   energy_per_pair [P] dtype or NULL
+ *   active_mask     [ceil(P/32)] uint32 or NULL: bit (k & 31) of word k >> 5 set iff pair k active
+ *   tc              [P,2] dtype or NULL: (t_c^0, t_c^1), (0,0) for inactive pairs
+ *   n_active        [1] int64 on the device or NULL                                               */
+tt_status tt_energy(tt_ctx* ctx, const tt_problem* prob, void* energy_sum, void* energy_per_pair,
+                    uint32_t* active_mask, void* tc, int64_t* n_active, void* stream);
+
+/* Symbolic phase of step 4 (L51): classifies the candidates at the current positions, compacts
+ * the active pairs (order preserving) and builds the BSR pattern.  Caches all of it in ctx.
+ *   nnzb_host     HOST [1]: number of 3x3 blocks the numeric phase will write
+ *   n_active_host HOST [1] or NULL
+ * Synchronises `stream`.                                                                          */
+tt_status tt_hess_symbolic(tt_ctx* ctx, const tt_problem* prob, int64_t* nnzb_host,
+                           int64_t* n_active_host, void* stream);
+
+/* Steps 2-4 (Eq. 2-4), numeric phase, on the active set cached by tt_hess_symbolic for
+ * the same problem (same pointers and sizes; positions must be unchanged since, else TT_ERR_STATE
+ * cannot be detected and the cached active set is evaluated at the new positions).
+ *   energy_sum [1] dtype; grad [nV,3] dtype or NULL;
+ *   bsr_rowptr [nV+1], bsr_colind [nnzb_capacity], bsr_vals [nnzb_capacity,3,3] dtype -- all
+ *   three NULL to skip the Hessian.  TT_ERR_CAPACITY if nnzb_capacity < nnzb.                     */
+tt_status tt_energy_grad_hess(tt_ctx* ctx, const tt_problem* prob, void* energy_sum, void* grad,
+                              int32_t* bsr_rowptr, int32_t* bsr_colind, void* bsr_vals,
+                              int64_t nnzb_capacity, void* stream);
+
+/* Matrix-free y = H p with the same Hessian (Eq. 4, same tt_hess_mode) on the cached active set;
+ * never forms a block.  p, y: [nV,3] dtype, p != y.  Needs tt_hess_symbolic first.               */
+tt_status tt_hess_vec(tt_ctx* ctx, const tt_problem* prob, const void* p, void* y, void* stream);
+
+/* End-to-end convenience with HOST buffers: copies pos/tris/pairs host->device (pinned host
+ * memory recommended), runs tt_hess_symbolic + tt_energy_grad_hess into ctx-owned device buffers,
+ * and copies the results back.  `prob` holds HOST pointers.
+ *   energy_host HOST [1] dtype; grad_host HOST [nV,3] dtype or NULL;
+ *   nnzb_host HOST [1]; n_active_host HOST [1] or NULL;
+ *   rowptr_host [nV+1] / colind_host [nnzb_capacity] / vals_host [nnzb_capacity,3,3]: HOST, each
+ *   may be NULL (the BSR then stays on the device, see tt_bsr_device).  Synchronises `stream`.   */
+tt_status tt_energy_grad_hess_host(tt_ctx* ctx, const tt_problem* prob, void* energy_host,
+                                   void* grad_host, int64_t* nnzb_host, int64_t* n_active_host,
+                                   int32_t* rowptr_host, int32_t* colind_host, void* vals_host,
+                                   int64_t nnzb_capacity, void* stream);
+
+/* Device views of the BSR produced by the last tt_energy_grad_hess_host (owned by ctx, valid
+ * until the next *_host call or tt_destroy).                                                      */
+tt_status tt_bsr_device(tt_ctx* ctx, const int32_t** rowptr, const int32_t** colind,
+                        const void** vals, int64_t* nnzb);
+
+/* Counters of the last tt_hess_symbolic: what[0]=n_active, [1]=directed entries (2*n_active),
+ * [2]=touched triangles, [3]=blocks written directly (exclusive rows), [4]=blocks produced by the
+ * general-row merge, [5]=merge records, [6]=nnzb, [7]=kernel launches issued by this ctx so far.                     */
+tt_status tt_stats(const tt_ctx* ctx, int64_t* what, int32_t n);
+
+const char* tt_status_string(tt_status s);
+const char* tt_last_error(const tt_ctx* ctx);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* TT_H_ */

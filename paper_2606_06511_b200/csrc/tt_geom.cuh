@@ -1,0 +1,203 @@
+// tt_geom.cuh -- per-pair device arithmetic of the hot path (sm_100a), fp64 registers only.
+//
+// Steps a1-a3 of DESIGN.md (Eq. 1-4, App. A), written the GPU's own way:
+// where the paper's listing pushes 18-partial dual numbers through Moeller's test, this file
+// differentiates the four segment end-points ANALYTICALLY ("manually construct the computation
+// graph to reduce the number of multiplications").  Because P - Q is parallel to
+// the unit line direction D and D . dD = 0, d(D.(P-Q)) = D^T (dP - dQ): neither dD, nor the
+// normalisation of the plane normals, nor the origin A of App. A L144 contribute (DESIGN.md
+// "analytic form").  Shares nothing with oracle/.
+#pragma once
+#include <cuda_runtime.h>
+
+namespace ttg {
+
+struct d3 {
+  double x, y, z;
+};
+__device__ __forceinline__ d3 mk(double x, double y, double z) { return d3{x, y, z}; }
+__device__ __forceinline__ d3 operator+(d3 a, d3 b) { return mk(a.x + b.x, a.y + b.y, a.z + b.z); }
+__device__ __forceinline__ d3 operator-(d3 a, d3 b) { return mk(a.x - b.x, a.y - b.y, a.z - b.z); }
+__device__ __forceinline__ d3 operator*(double s, d3 a) { return mk(s * a.x, s * a.y, s * a.z); }
+__device__ __forceinline__ double dot(d3 a, d3 b) { return fma(a.x, b.x, fma(a.y, b.y, a.z * b.z)); }
+__device__ __forceinline__ d3 cross(d3 a, d3 b) {
+  return mk(fma(a.y, b.z, -(a.z * b.y)), fma(a.z, b.x, -(a.x * b.z)), fma(a.x, b.y, -(a.y * b.x)));
+}
+__device__ __forceinline__ d3 axpy(double s, d3 a, d3 b) {  // s*a + b
+  return mk(fma(s, a.x, b.x), fma(s, a.y, b.y), fma(s, a.z, b.z));
+}
+__device__ __forceinline__ d3 sel3(int i, d3 v0, d3 v1, d3 v2) {
+  d3 r = v2;
+  if (i == 1) r = v1;
+  if (i == 0) r = v0;
+  return r;
+}
+__device__ __forceinline__ double sel3(int i, double v0, double v1, double v2) {
+  double r = v2;
+  if (i == 1) r = v1;
+  if (i == 0) r = v0;
+  return r;
+}
+
+// One cut of triangle X (vertices x[0..2], plane distances d[0..2] w.r.t. the other plane):
+// two end-points E_e = x_k + tau_e (x_i - x_k), e = 0 (smaller t) and e = 1 (larger t).
+// k == i encodes App. A's "vertex exactly on the plane" branch (L106-115): E = x_k, d tau = 0.
+struct Cut {
+  int k[2], i[2];
+  double tau[2];
+  double t[2];
+};
+
+// Plane-side classification + end-points of one triangle (App. A).  Returns false when
+// the triangle does not strictly straddle the plane (L95 / L120).
+__device__ __forceinline__ bool make_cut(const d3 x0, const d3 x1, const d3 x2, double d0, double d1,
+                                         double d2, const d3 Dh, Cut& c) {
+  const int pos = (d0 > 0.0) + (d1 > 0.0) + (d2 > 0.0);
+  const int neg = (d0 < 0.0) + (d1 < 0.0) + (d2 < 0.0);
+  if (!(pos > 0 && neg > 0)) return false;
+  int k0, i0, k1, i1;
+  if (pos + neg == 3) {  // two on one side, one alone: k = the lone vertex (L96-105)
+    const bool s0 = d0 > 0.0, s1 = d1 > 0.0, s2 = d2 > 0.0;
+    const int k = (s0 == s1) ? 2 : ((s0 == s2) ? 1 : 0);
+    k0 = k1 = k;
+    i0 = (k == 0) ? 1 : 0;
+    i1 = (k == 2) ? 1 : 2;
+  } else {  // one +, one -, one exactly 0 (L106-115): end-point 0 is the vertex itself
+    const int z = (d0 == 0.0) ? 0 : ((d1 == 0.0) ? 1 : 2);
+    k0 = i0 = z;
+    k1 = (z == 0) ? 1 : 0;
+    i1 = (z == 2) ? 1 : 2;
+  }
+  const double dk0 = sel3(k0, d0, d1, d2), di0 = sel3(i0, d0, d1, d2);
+  const double dk1 = sel3(k1, d0, d1, d2), di1 = sel3(i1, d0, d1, d2);
+  // opposite signs: |dk - di| = |dk| + |di|, no cancellation
+  const double tau0 = (k0 == i0) ? 0.0 : dk0 / (dk0 - di0);
+  const double tau1 = dk1 / (dk1 - di1);
+  const d3 xk0 = sel3(k0, x0, x1, x2), xi0 = sel3(i0, x0, x1, x2);
+  const d3 xk1 = sel3(k1, x0, x1, x2), xi1 = sel3(i1, x0, x1, x2);
+  const double t0 = dot(Dh, axpy(tau0, xi0 - xk0, xk0));
+  const double t1 = dot(Dh, axpy(tau1, xi1 - xk1, xk1));
+  const bool sw = t1 < t0;  // min/max of App. A L149-152 (selects the argument and its partials)
+  c.k[0] = sw ? k1 : k0;  c.i[0] = sw ? i1 : i0;  c.tau[0] = sw ? tau1 : tau0;  c.t[0] = sw ? t1 : t0;
+  c.k[1] = sw ? k0 : k1;  c.i[1] = sw ? i0 : i1;  c.tau[1] = sw ? tau0 : tau1;  c.t[1] = sw ? t0 : t1;
+  return true;
+}
+
+struct PairGeom {
+  d3 na, nb, Dh;
+  double alpha[3], beta[3];
+  Cut ca, cb;
+  double tc0, tc1;  // already multiplied by sigma
+};
+
+// Steps a1: Moeller intervals and I_c (Eq. 1; App. A).  a*, b* are the
+// six vertices in any common frame (callers translate by -a0 first).  Returns the `intersected`
+// flag of L153, evaluated in fp64.
+__device__ __forceinline__ bool pair_intervals(const d3 a0, const d3 a1, const d3 a2, const d3 b0,
+                                               const d3 b1, const d3 b2, double sigma, PairGeom& g) {
+  g.na = cross(a1 - a0, a2 - a0);
+  g.nb = cross(b1 - b0, b2 - b0);
+  // signed (unnormalised) distances: same signs as App. A's normalised d[] (L84-86)
+  g.alpha[0] = dot(g.nb, a0 - b0);
+  g.alpha[1] = dot(g.nb, a1 - b0);
+  g.alpha[2] = dot(g.nb, a2 - b0);
+  {
+    const int pos = (g.alpha[0] > 0.0) + (g.alpha[1] > 0.0) + (g.alpha[2] > 0.0);
+    const int neg = (g.alpha[0] < 0.0) + (g.alpha[1] < 0.0) + (g.alpha[2] < 0.0);
+    if (!(pos > 0 && neg > 0)) return false;  // early exit: most candidates leave here
+  }
+  g.beta[0] = dot(g.na, b0 - a0);
+  g.beta[1] = dot(g.na, b1 - a0);
+  g.beta[2] = dot(g.na, b2 - a0);
+  {
+    const int pos = (g.beta[0] > 0.0) + (g.beta[1] > 0.0) + (g.beta[2] > 0.0);
+    const int neg = (g.beta[0] < 0.0) + (g.beta[1] < 0.0) + (g.beta[2] < 0.0);
+    if (!(pos > 0 && neg > 0)) return false;
+  }
+  const d3 D = cross(g.na, g.nb);  // App. A L141 (u = T_a)
+  const double D2 = dot(D, D);
+  if (!(D2 > 0.0)) return false;   // parallel planes (L11 "not coplanar")
+  g.Dh = rsqrt(D2) * D;            // L142
+  if (!make_cut(a0, a1, a2, g.alpha[0], g.alpha[1], g.alpha[2], g.Dh, g.ca)) return false;
+  if (!make_cut(b0, b1, b2, g.beta[0], g.beta[1], g.beta[2], g.Dh, g.cb)) return false;
+  const double ta0 = g.ca.t[0], ta1 = g.ca.t[1], tb0 = g.cb.t[0], tb1 = g.cb.t[1];
+  g.tc0 = sigma * (ta0 - tb1);     // Eq. 1 / L154
+  g.tc1 = sigma * (ta1 - tb0);     // L155
+  return (ta1 > tb0) && (ta0 < tb1);  // L153, strict
+}
+
+// D^T dE for one end-point E = x_k + tau (x_i - x_k) of triangle X cut by plane(Y), added with
+// weight s into g[own..own+8] (the three vertices of X) and g[oth..oth+8] (those of Y).
+//   own blocks: (1-tau) D at x_k, tau D at x_i, plus c dtau/dx with c = D.(x_i - x_k),
+//               dtau/dx_i = d_k nY / den^2, dtau/dx_k = -d_i nY / den^2, den = d_k - d_i
+//   other blocks: dtau/dy1 = (y2-y0) x (E-y0) / den, dtau/dy2 = (E-y0) x (y1-y0) / den,
+//               y0 from translation invariance (all six blocks of D^T dE sum to D).
+template <int OWN, int OTH>
+__device__ __forceinline__ void add_endpoint(double (&g)[18], double s, const d3 Dh, const d3 x0,
+                                             const d3 x1, const d3 x2, const double (&d)[3], const d3 y0,
+                                             const d3 y1, const d3 y2, const d3 nY, int k, int i,
+                                             double tau) {
+  const d3 xk = sel3(k, x0, x1, x2), xi = sel3(i, x0, x1, x2);
+  const double dk = sel3(k, d[0], d[1], d[2]), di = sel3(i, d[0], d[1], d[2]);
+  const double inv = (k == i) ? 0.0 : 1.0 / (dk - di);
+  const d3 e = xi - xk;
+  const double w = s * dot(Dh, e) * inv;  // s * c / den
+  const double wn = w * inv;              // s * c / den^2
+#pragma unroll
+  for (int m = 0; m < 3; ++m) {
+    const double cd = s * (((m == k) ? (1.0 - tau) : 0.0) + ((m == i) ? tau : 0.0));
+    const double cn = wn * (((m == i) ? dk : 0.0) - ((m == k) ? di : 0.0));
+    g[OWN + 3 * m + 0] += fma(cd, Dh.x, cn * nY.x);
+    g[OWN + 3 * m + 1] += fma(cd, Dh.y, cn * nY.y);
+    g[OWN + 3 * m + 2] += fma(cd, Dh.z, cn * nY.z);
+  }
+  const d3 u = axpy(tau, e, xk) - y0;  // E - y0
+  const d3 h1 = w * cross(y2 - y0, u);
+  const d3 h2 = w * cross(u, y1 - y0);
+  g[OTH + 3] += h1.x;  g[OTH + 4] += h1.y;  g[OTH + 5] += h1.z;
+  g[OTH + 6] += h2.x;  g[OTH + 7] += h2.y;  g[OTH + 8] += h2.z;
+  g[OTH + 0] -= fma(w, nY.x, h1.x + h2.x);
+  g[OTH + 1] -= fma(w, nY.y, h1.y + h2.y);
+  g[OTH + 2] -= fma(w, nY.z, h1.z + h2.z);
+}
+
+// Step a3, first half: g0 = d tc0/dx = sigma (D^T dP_min - D^T dQ_max),
+//                      g1 = d tc1/dx = sigma (D^T dP_max - D^T dQ_min),  x = [a0,a1,a2,b0,b1,b2].
+__device__ __forceinline__ void pair_derivs(const d3 a0, const d3 a1, const d3 a2, const d3 b0,
+                                            const d3 b1, const d3 b2, double sigma, const PairGeom& q,
+                                            double (&g0)[18], double (&g1)[18]) {
+#pragma unroll
+  for (int i = 0; i < 18; ++i) { g0[i] = 0.0; g1[i] = 0.0; }
+  add_endpoint<0, 9>(g0, sigma, q.Dh, a0, a1, a2, q.alpha, b0, b1, b2, q.nb, q.ca.k[0], q.ca.i[0], q.ca.tau[0]);
+  add_endpoint<9, 0>(g0, -sigma, q.Dh, b0, b1, b2, q.beta, a0, a1, a2, q.na, q.cb.k[1], q.cb.i[1], q.cb.tau[1]);
+  add_endpoint<0, 9>(g1, sigma, q.Dh, a0, a1, a2, q.alpha, b0, b1, b2, q.nb, q.ca.k[1], q.ca.i[1], q.ca.tau[1]);
+  add_endpoint<9, 0>(g1, -sigma, q.Dh, b0, b1, b2, q.beta, a0, a1, a2, q.na, q.cb.k[0], q.cb.i[0], q.cb.tau[0]);
+}
+
+// Step a3, second half: Eq. 3 and Eq. 4 coefficients.  keep = tt_hess_mode's treatment of the
+// third part (L47): EQ4 -> 1, PSD2 -> 0, FILTER -> [8 tc0 tc1 (g0.g1) >= 0].
+struct Coefs {
+  double cg0, cg1;       // Eq. 3: grad = cg0 g0 + cg1 g1
+  double c00, c11, c01;  // Eq. 4: H = c00 g0g0^T + c11 g1g1^T + c01 (g1g0^T + g0g1^T)
+};
+__device__ __forceinline__ Coefs pair_coefs(double tc0, double tc1, const double (&g0)[18],
+                                            const double (&g1)[18], int hess_mode) {
+  Coefs c;
+  c.cg0 = 2.0 * tc0 * (tc1 * tc1);
+  c.cg1 = 2.0 * tc1 * (tc0 * tc0);
+  c.c00 = 2.0 * (tc1 * tc1);
+  c.c11 = 2.0 * (tc0 * tc0);
+  double keep = 1.0;
+  if (hess_mode == 1) {
+    double g01 = 0.0;
+#pragma unroll
+    for (int i = 0; i < 18; ++i) g01 = fma(g0[i], g1[i], g01);
+    keep = (8.0 * tc0 * tc1 * g01 >= 0.0) ? 1.0 : 0.0;
+  } else if (hess_mode == 2) {
+    keep = 0.0;
+  }
+  c.c01 = 4.0 * tc0 * tc1 * keep;
+  return c;
+}
+
+}  // namespace ttg

@@ -1,0 +1,663 @@
+// tt_lib.cu -- C ABI of libtt.so (include/tt.h): context, workspace, launch logic.
+// Kernels: tt_kernels.cuh; per-pair arithmetic: tt_geom.cuh.  Scans / radix sorts / select of the
+// symbolic phase use CUB (ships with the CUDA toolkit); everything the paper defines runs in the
+// hand-written kernels.
+#include <cstdarg>
+#include <cstdio>
+#include <cstring>
+#include <string>
+
+#include <cub/cub.cuh>
+
+#include "../../include/tt.h"
+#include "tt_kernels.cuh"
+
+namespace {
+
+struct DevBuf {
+  void* p = nullptr;
+  size_t bytes = 0;
+  ~DevBuf() { release(); }
+  void release() {
+    if (p) cudaFree(p);
+    p = nullptr;
+    bytes = 0;
+  }
+  // grow-only; contents are NOT preserved across a grow
+  cudaError_t ensure(size_t need) {
+    if (need <= bytes) return cudaSuccess;
+    release();
+    size_t want = need + need / 8 + 256;
+    cudaError_t e = cudaMalloc(&p, want);
+    if (e != cudaSuccess) {
+      p = nullptr;
+      (void)cudaGetLastError();
+      e = cudaMalloc(&p, need);
+      want = need;
+    }
+    if (e == cudaSuccess) bytes = want;
+    return e;
+  }
+  template <typename U> U* as() const { return reinterpret_cast<U*>(p); }
+};
+
+struct Signature {
+  const void* pos = nullptr;
+  const int32_t* tris = nullptr;
+  const int32_t* pairs = nullptr;
+  int64_t nV = -1, nT = -1, P = -1;
+  bool valid = false;
+  bool matches(const tt_problem* q) const {
+    return valid && pos == q->pos && tris == q->tris && pairs == q->pairs && nV == q->n_verts &&
+           nT == q->n_tris && P == q->n_pairs;
+  }
+};
+
+}  // namespace
+
+struct tt_ctx {
+  tt_options opt;
+  std::string err;
+  int64_t launches = 0;
+  // classification
+  DevBuf mask, blk_count, blk_off, blk_energy, counts, energy;
+  // active set + directed entries
+  DevBuf active_ids, keys[2], dvals[2], tptr, vcnt, tflag, touched;
+  // per-triangle symbolic
+  DevBuf erank, drank, rowlen, tlen, toff, slot_excl, rowbase;
+  // merge path
+  DevBuf rkeys[2], rvals[2], head, ord, rowfirst, run_start, run_dest;
+  // pattern
+  DevBuf rowptr64, rowptr, colind;
+  // numeric
+  DevBuf chunk_tri, asm_energy, tvals, tslot, vkeys[2], vvals[2], vptr;
+  DevBuf cub_tmp;
+  // host-API mirrors
+  DevBuf h_pos, h_tris, h_pairs, o_vals, o_grad, o_energy;
+  // cached symbolic state
+  Signature sig;
+  int64_t A = 0, n_dir = 0, n_touched = 0, R = 0, U = 0, nnzb = 0, n_chunks = 0, rows_excl = 0, rows_gen = 0;
+  int bitsT = 1, bitsV = 1;
+  uint64_t* keys_sorted = nullptr;
+  uint32_t* dvals_sorted = nullptr;
+  uint64_t* rkeys_sorted = nullptr;
+  uint32_t* rvals_sorted = nullptr;
+  uint32_t* vvals_sorted = nullptr;
+  int64_t host_nnzb = 0;
+};
+
+namespace {
+
+tt_status fail(tt_ctx* c, tt_status s, const char* fmt, ...) {
+  char buf[512];
+  va_list ap;
+  va_start(ap, fmt);
+  vsnprintf(buf, sizeof(buf), fmt, ap);
+  va_end(ap);
+  if (c) c->err = buf;
+  return s;
+}
+
+#define TT_CUDA(call)                                                                            \
+  do {                                                                                           \
+    cudaError_t e_ = (call);                                                                     \
+    if (e_ != cudaSuccess) {                                                                     \
+      (void)cudaGetLastError();                                                                  \
+      return fail(ctx, e_ == cudaErrorMemoryAllocation ? TT_ERR_NOMEM : TT_ERR_CUDA,             \
+                  "%s:%d %s: %s", __FILE__, __LINE__, #call, cudaGetErrorString(e_));            \
+    }                                                                                            \
+  } while (0)
+
+#define TT_LAUNCH_CHECK()                                                                        \
+  do {                                                                                           \
+    ctx->launches++;                                                                             \
+    TT_CUDA(cudaGetLastError());                                                                 \
+  } while (0)
+
+inline int ceil_log2(int64_t n) {
+  int b = 1;
+  while ((int64_t(1) << b) < n) ++b;
+  return b;
+}
+inline unsigned grid_for(int64_t n, int threads) { return (unsigned)((n + threads - 1) / threads); }
+
+struct CastI64 {
+  __host__ __device__ int64_t operator()(int v) const { return (int64_t)v; }
+};
+
+tt_status check_problem(tt_ctx* ctx, const tt_problem* q) {
+  if (!ctx) return TT_ERR_INVALID_ARG;
+  if (!q) return fail(ctx, TT_ERR_INVALID_ARG, "problem is NULL");
+  if (q->n_verts < 0 || q->n_tris < 0 || q->n_pairs < 0) return fail(ctx, TT_ERR_INVALID_ARG, "negative size");
+  if (q->n_verts >= (int64_t(1) << 31) / 3 || q->n_tris >= (int64_t(1) << 31) / 3 || q->n_pairs >= (int64_t(1) << 30))
+    return fail(ctx, TT_ERR_INVALID_ARG, "sizes exceed int32 indexing (nV, nT < 2^31/3, P < 2^30)");
+  if ((q->n_verts > 0 && !q->pos) || (q->n_tris > 0 && !q->tris) || (q->n_pairs > 0 && !q->pairs))
+    return fail(ctx, TT_ERR_INVALID_ARG, "NULL array with non-zero size");
+  return TT_OK;
+}
+
+// exclusive sum of n ints (+ grand total in out[n]); `in` must have n+1 entries with in[n] == 0
+tt_status scan_i32(tt_ctx* ctx, const int* in, int* out, int64_t n_plus_1, cudaStream_t st) {
+  size_t tmp = 0;
+  TT_CUDA(cub::DeviceScan::ExclusiveSum(nullptr, tmp, in, out, n_plus_1, st));
+  TT_CUDA(ctx->cub_tmp.ensure(tmp));
+  TT_CUDA(cub::DeviceScan::ExclusiveSum(ctx->cub_tmp.p, tmp, in, out, n_plus_1, st));
+  ctx->launches++;
+  return TT_OK;
+}
+tt_status scan_i64(tt_ctx* ctx, const int64_t* in, int64_t* out, int64_t n_plus_1, cudaStream_t st) {
+  size_t tmp = 0;
+  TT_CUDA(cub::DeviceScan::ExclusiveSum(nullptr, tmp, in, out, n_plus_1, st));
+  TT_CUDA(ctx->cub_tmp.ensure(tmp));
+  TT_CUDA(cub::DeviceScan::ExclusiveSum(ctx->cub_tmp.p, tmp, in, out, n_plus_1, st));
+  ctx->launches++;
+  return TT_OK;
+}
+tt_status scan_i32_to_i64(tt_ctx* ctx, const int* in, int64_t* out, int64_t n_plus_1, cudaStream_t st) {
+  cub::TransformInputIterator<int64_t, CastI64, const int*> it(in, CastI64());
+  size_t tmp = 0;
+  TT_CUDA(cub::DeviceScan::ExclusiveSum(nullptr, tmp, it, out, n_plus_1, st));
+  TT_CUDA(ctx->cub_tmp.ensure(tmp));
+  TT_CUDA(cub::DeviceScan::ExclusiveSum(ctx->cub_tmp.p, tmp, it, out, n_plus_1, st));
+  ctx->launches++;
+  return TT_OK;
+}
+tt_status incl_scan_i32(tt_ctx* ctx, const int* in, int* out, int64_t n, cudaStream_t st) {
+  size_t tmp = 0;
+  TT_CUDA(cub::DeviceScan::InclusiveSum(nullptr, tmp, in, out, n, st));
+  TT_CUDA(ctx->cub_tmp.ensure(tmp));
+  TT_CUDA(cub::DeviceScan::InclusiveSum(ctx->cub_tmp.p, tmp, in, out, n, st));
+  ctx->launches++;
+  return TT_OK;
+}
+// stable LSD radix sort of (key, payload) on bits [0, end_bit); result pointers returned
+tt_status sort_pairs(tt_ctx* ctx, DevBuf (&kb)[2], DevBuf (&vb)[2], int64_t n, int end_bit,
+                     uint64_t** k_out, uint32_t** v_out, cudaStream_t st) {
+  cub::DoubleBuffer<uint64_t> dk(kb[0].as<uint64_t>(), kb[1].as<uint64_t>());
+  cub::DoubleBuffer<uint32_t> dv(vb[0].as<uint32_t>(), vb[1].as<uint32_t>());
+  size_t tmp = 0;
+  TT_CUDA(cub::DeviceRadixSort::SortPairs(nullptr, tmp, dk, dv, n, 0, end_bit, st));
+  TT_CUDA(ctx->cub_tmp.ensure(tmp));
+  TT_CUDA(cub::DeviceRadixSort::SortPairs(ctx->cub_tmp.p, tmp, dk, dv, n, 0, end_bit, st));
+  ctx->launches++;
+  *k_out = dk.Current();
+  *v_out = dv.Current();
+  return TT_OK;
+}
+
+// ---- K1 (+ sums): shared by tt_energy and tt_hess_symbolic -------------------------------------
+template <typename T>
+tt_status run_classify(tt_ctx* ctx, const tt_problem* q, T* e_pp, T* tc, cudaStream_t st, int64_t* nblk_out) {
+  const int64_t P = q->n_pairs;
+  const int64_t nblk = (P + ttk::CLS_THREADS - 1) / ttk::CLS_THREADS;
+  *nblk_out = nblk;
+  TT_CUDA(ctx->mask.ensure(sizeof(uint32_t) * (size_t)(nblk * (ttk::CLS_THREADS / 32) + 1)));
+  TT_CUDA(ctx->blk_count.ensure(sizeof(int) * (size_t)(nblk + 1)));
+  TT_CUDA(ctx->blk_off.ensure(sizeof(int) * (size_t)(nblk + 1)));
+  TT_CUDA(ctx->blk_energy.ensure(sizeof(double) * (size_t)(nblk + 1)));
+  TT_CUDA(ctx->counts.ensure(sizeof(int64_t) * 16));
+  TT_CUDA(ctx->energy.ensure(sizeof(double) * 2));
+  TT_CUDA(cudaMemsetAsync(ctx->blk_count.as<int>() + nblk, 0, sizeof(int), st));
+  if (nblk > 0) {
+    ttk::k_classify<T><<<(unsigned)nblk, ttk::CLS_THREADS, 0, st>>>(
+        (const T*)q->pos, q->tris, (const int2*)q->pairs, P, ctx->opt.tc_scale, ctx->mask.as<uint32_t>(),
+        ctx->blk_count.as<int>(), ctx->blk_energy.as<double>(), e_pp, tc);
+    TT_LAUNCH_CHECK();
+  }
+  tt_status s = scan_i32(ctx, ctx->blk_count.as<int>(), ctx->blk_off.as<int>(), nblk + 1, st);
+  if (s != TT_OK) return s;
+  return TT_OK;
+}
+
+template <typename T>
+tt_status energy_impl(tt_ctx* ctx, const tt_problem* q, void* energy_sum, void* e_pp, uint32_t* active_mask,
+                      void* tc, int64_t* n_active, cudaStream_t st) {
+  int64_t nblk = 0;
+  tt_status s = run_classify<T>(ctx, q, (T*)e_pp, (T*)tc, st, &nblk);
+  if (s != TT_OK) return s;
+  ttk::k_sum_partials<T><<<1, 1024, 0, st>>>(ctx->blk_energy.as<double>(), nblk, 1.0, (T*)energy_sum);
+  TT_LAUNCH_CHECK();
+  if (n_active) {
+    ttk::k_set_count<<<1, 32, 0, st>>>(ctx->blk_off.as<int>(), ctx->blk_count.as<int>(), nblk, n_active, nullptr);
+    TT_LAUNCH_CHECK();
+  }
+  if (active_mask && q->n_pairs > 0)
+    TT_CUDA(cudaMemcpyAsync(active_mask, ctx->mask.p, sizeof(uint32_t) * (size_t)((q->n_pairs + 31) / 32),
+                            cudaMemcpyDeviceToDevice, st));
+  return TT_OK;
+}
+
+template <typename T>
+tt_status symbolic_impl(tt_ctx* ctx, const tt_problem* q, int64_t* nnzb_host, int64_t* n_active_host,
+                        cudaStream_t st) {
+  using namespace ttk;
+  ctx->sig.valid = false;
+  const int64_t P = q->n_pairs, nT = q->n_tris, nV = q->n_verts;
+  int64_t nblk = 0;
+  tt_status s = run_classify<T>(ctx, q, nullptr, nullptr, st, &nblk);
+  if (s != TT_OK) return s;
+  int64_t* d_counts = ctx->counts.as<int64_t>();
+  k_set_count<<<1, 32, 0, st>>>(ctx->blk_off.as<int>(), ctx->blk_count.as<int>(), nblk, d_counts, nullptr);
+  TT_LAUNCH_CHECK();
+  int64_t A = 0;
+  TT_CUDA(cudaMemcpyAsync(&A, d_counts, sizeof(int64_t), cudaMemcpyDeviceToHost, st));
+  TT_CUDA(cudaStreamSynchronize(st));
+  ctx->A = A;
+  const int64_t n = 2 * A;
+  ctx->n_dir = n;
+  ctx->bitsT = ceil_log2(nT > 1 ? nT : 2);
+  ctx->bitsV = ceil_log2(nV > 1 ? nV : 2);
+  const int bitsT = ctx->bitsT, bitsV = ctx->bitsV;
+
+  // ---- compaction + directed entries sorted by (source, partner) ----
+  TT_CUDA(ctx->active_ids.ensure(sizeof(int) * (size_t)(A + 1)));
+  if (nblk > 0) {
+    k_compact<<<(unsigned)nblk, CLS_THREADS, 0, st>>>(ctx->mask.as<uint32_t>(), ctx->blk_off.as<int>(), P,
+                                                      ctx->active_ids.as<int>());
+    TT_LAUNCH_CHECK();
+  }
+  for (int i = 0; i < 2; ++i) {
+    TT_CUDA(ctx->keys[i].ensure(sizeof(uint64_t) * (size_t)(n + 1)));
+    TT_CUDA(ctx->dvals[i].ensure(sizeof(uint32_t) * (size_t)(n + 1)));
+  }
+  ctx->keys_sorted = ctx->keys[0].as<uint64_t>();
+  ctx->dvals_sorted = ctx->dvals[0].as<uint32_t>();
+  if (A > 0) {
+    k_emit_directed<<<grid_for(A, 256), 256, 0, st>>>((const int2*)q->pairs, ctx->active_ids.as<int>(), A, bitsT,
+                                                      ctx->keys[0].as<uint64_t>(), ctx->dvals[0].as<uint32_t>());
+    TT_LAUNCH_CHECK();
+    s = sort_pairs(ctx, ctx->keys, ctx->dvals, n, 2 * bitsT, &ctx->keys_sorted, &ctx->dvals_sorted, st);
+    if (s != TT_OK) return s;
+  }
+  TT_CUDA(ctx->tptr.ensure(sizeof(int) * (size_t)(nT + 2)));
+  k_segment_ptr<<<grid_for(n + 1, 256), 256, 0, st>>>(ctx->keys_sorted, n, bitsT, nT, ctx->tptr.as<int>());
+  TT_LAUNCH_CHECK();
+
+  // ---- touched triangles and vertex use counts ----
+  TT_CUDA(ctx->vcnt.ensure(sizeof(int) * (size_t)(nV + 1)));
+  TT_CUDA(ctx->tflag.ensure(sizeof(int) * (size_t)(nT + 1)));
+  TT_CUDA(ctx->touched.ensure(sizeof(int) * (size_t)(nT + 1)));
+  TT_CUDA(cudaMemsetAsync(ctx->vcnt.p, 0, sizeof(int) * (size_t)(nV + 1), st));
+  int64_t n_touched = 0;
+  if (nT > 0) {
+    k_vertex_touch<<<grid_for(nT, 256), 256, 0, st>>>(q->tris, ctx->tptr.as<int>(), nT, ctx->vcnt.as<int>(),
+                                                      ctx->tflag.as<int>());
+    TT_LAUNCH_CHECK();
+    cub::CountingInputIterator<int> iota(0);
+    size_t tmp = 0;
+    int* d_num = reinterpret_cast<int*>(d_counts + 1);
+    TT_CUDA(cub::DeviceSelect::Flagged(nullptr, tmp, iota, ctx->tflag.as<int>(), ctx->touched.as<int>(), d_num, (int)nT, st));
+    TT_CUDA(ctx->cub_tmp.ensure(tmp));
+    TT_CUDA(cub::DeviceSelect::Flagged(ctx->cub_tmp.p, tmp, iota, ctx->tflag.as<int>(), ctx->touched.as<int>(), d_num, (int)nT, st));
+    ctx->launches++;
+    int nt32 = 0;
+    TT_CUDA(cudaMemcpyAsync(&nt32, d_num, sizeof(int), cudaMemcpyDeviceToHost, st));
+    TT_CUDA(cudaStreamSynchronize(st));
+    n_touched = nt32;
+  }
+  ctx->n_touched = n_touched;
+
+  // ---- per-triangle ranks, exclusive rows, general-row workspace sizes ----
+  TT_CUDA(ctx->erank.ensure(sizeof(int) * (size_t)(3 * n + 3)));
+  TT_CUDA(ctx->drank.ensure(sizeof(int) * (size_t)(3 * nT + 3)));
+  TT_CUDA(ctx->rowlen.ensure(sizeof(int) * (size_t)(nV + 1)));
+  TT_CUDA(ctx->tlen.ensure(sizeof(int64_t) * (size_t)(3 * nT + 1)));
+  TT_CUDA(ctx->toff.ensure(sizeof(int64_t) * (size_t)(3 * nT + 1)));
+  TT_CUDA(ctx->slot_excl.ensure((size_t)(3 * nT + 1)));
+  TT_CUDA(ctx->rowbase.ensure(sizeof(int64_t) * (size_t)(3 * nT + 1)));
+  TT_CUDA(cudaMemsetAsync(ctx->rowlen.p, 0, sizeof(int) * (size_t)(nV + 1), st));
+  TT_CUDA(cudaMemsetAsync(ctx->tlen.p, 0, sizeof(int64_t) * (size_t)(3 * nT + 1), st));
+  TT_CUDA(cudaMemsetAsync(ctx->slot_excl.p, 0, (size_t)(3 * nT + 1), st));
+  const unsigned tri_grid = grid_for(n_touched, SYM_WARPS);
+  if (n_touched > 0) {
+    k_tri_symbolic<<<tri_grid, 32 * SYM_WARPS, 0, st>>>(
+        q->tris, ctx->touched.as<int>(), n_touched, ctx->tptr.as<int>(), ctx->keys_sorted, bitsT,
+        ctx->vcnt.as<int>(), (ctx->opt.flags & TT_FLAG_FORCE_GENERAL_ROWS) ? 1 : 0, ctx->erank.as<int>(),
+        ctx->drank.as<int>(), ctx->rowlen.as<int>(), ctx->tlen.as<int64_t>(), ctx->slot_excl.as<uint8_t>());
+    TT_LAUNCH_CHECK();
+  }
+  s = scan_i64(ctx, ctx->tlen.as<int64_t>(), ctx->toff.as<int64_t>(), 3 * nT + 1, st);
+  if (s != TT_OK) return s;
+  int64_t R = 0;
+  TT_CUDA(cudaMemcpyAsync(&R, ctx->toff.as<int64_t>() + 3 * nT, sizeof(int64_t), cudaMemcpyDeviceToHost, st));
+  TT_CUDA(cudaStreamSynchronize(st));
+  if (R >= (int64_t(1) << 31)) return fail(ctx, TT_ERR_INVALID_ARG, "general-row workspace exceeds 2^31 blocks");
+  ctx->R = R;
+
+  // ---- general rows: merge records sorted by (row, col) ----
+  int64_t U = 0;
+  ctx->rkeys_sorted = nullptr;
+  ctx->rvals_sorted = nullptr;
+  if (R > 0) {
+    for (int i = 0; i < 2; ++i) {
+      TT_CUDA(ctx->rkeys[i].ensure(sizeof(uint64_t) * (size_t)R));
+      TT_CUDA(ctx->rvals[i].ensure(sizeof(uint32_t) * (size_t)R));
+    }
+    TT_CUDA(ctx->head.ensure(sizeof(int) * (size_t)R));
+    TT_CUDA(ctx->ord.ensure(sizeof(int) * (size_t)R));
+    TT_CUDA(ctx->rowfirst.ensure(sizeof(int) * (size_t)(nV + 1)));
+    TT_CUDA(ctx->run_start.ensure(sizeof(int) * (size_t)(R + 1)));
+    TT_CUDA(ctx->run_dest.ensure(sizeof(int) * (size_t)(R + 1)));
+    k_emit_records<<<tri_grid, 32 * SYM_WARPS, 0, st>>>(
+        q->tris, ctx->touched.as<int>(), n_touched, ctx->tptr.as<int>(), ctx->keys_sorted, bitsT, bitsV,
+        ctx->erank.as<int>(), ctx->drank.as<int>(), ctx->toff.as<int64_t>(), ctx->slot_excl.as<uint8_t>(),
+        ctx->rkeys[0].as<uint64_t>(), ctx->rvals[0].as<uint32_t>());
+    TT_LAUNCH_CHECK();
+    s = sort_pairs(ctx, ctx->rkeys, ctx->rvals, R, 2 * bitsV, &ctx->rkeys_sorted, &ctx->rvals_sorted, st);
+    if (s != TT_OK) return s;
+    k_record_heads<<<grid_for(R, 256), 256, 0, st>>>(ctx->rkeys_sorted, R, ctx->head.as<int>());
+    TT_LAUNCH_CHECK();
+    s = incl_scan_i32(ctx, ctx->head.as<int>(), ctx->ord.as<int>(), R, st);
+    if (s != TT_OK) return s;
+    k_record_rows<<<grid_for(R, 256), 256, 0, st>>>(ctx->rkeys_sorted, R, bitsV, ctx->head.as<int>(),
+                                                    ctx->ord.as<int>(), ctx->rowlen.as<int>(),
+                                                    ctx->rowfirst.as<int>(), ctx->run_start.as<int>());
+    TT_LAUNCH_CHECK();
+    int u32 = 0;
+    TT_CUDA(cudaMemcpyAsync(&u32, ctx->ord.as<int>() + (R - 1), sizeof(int), cudaMemcpyDeviceToHost, st));
+    TT_CUDA(cudaStreamSynchronize(st));
+    U = u32;
+  }
+  ctx->U = U;
+
+  // ---- row pointers ----
+  TT_CUDA(ctx->rowptr64.ensure(sizeof(int64_t) * (size_t)(nV + 1)));
+  TT_CUDA(ctx->rowptr.ensure(sizeof(int) * (size_t)(nV + 1)));
+  s = scan_i32_to_i64(ctx, ctx->rowlen.as<int>(), ctx->rowptr64.as<int64_t>(), nV + 1, st);
+  if (s != TT_OK) return s;
+  int64_t nnzb = 0;
+  TT_CUDA(cudaMemcpyAsync(&nnzb, ctx->rowptr64.as<int64_t>() + nV, sizeof(int64_t), cudaMemcpyDeviceToHost, st));
+  TT_CUDA(cudaStreamSynchronize(st));
+  if (nnzb >= (int64_t(1) << 31)) return fail(ctx, TT_ERR_INVALID_ARG, "nnzb %lld exceeds int32 BSR indexing", (long long)nnzb);
+  ctx->nnzb = nnzb;
+  k_i64_to_i32<<<grid_for(nV + 1, 256), 256, 0, st>>>(ctx->rowptr64.as<int64_t>(), nV + 1, ctx->rowptr.as<int>());
+  TT_LAUNCH_CHECK();
+  TT_CUDA(ctx->colind.ensure(sizeof(int) * (size_t)(nnzb + 1)));
+  if (U > 0) {
+    k_record_dest<<<grid_for(U + 1, 256), 256, 0, st>>>(ctx->rkeys_sorted, U, R, bitsV, ctx->run_start.as<int>(),
+                                                        ctx->rowptr.as<int>(), ctx->rowfirst.as<int>(),
+                                                        ctx->run_dest.as<int>(), ctx->colind.as<int>());
+    TT_LAUNCH_CHECK();
+  }
+  if (n_touched > 0) {
+    k_fill_rows<<<tri_grid, 32 * SYM_WARPS, 0, st>>>(
+        q->tris, ctx->touched.as<int>(), n_touched, ctx->tptr.as<int>(), ctx->keys_sorted, bitsT,
+        ctx->erank.as<int>(), ctx->drank.as<int>(), ctx->toff.as<int64_t>(), ctx->slot_excl.as<uint8_t>(),
+        ctx->rowptr.as<int>(), ctx->rowbase.as<int64_t>(), ctx->colind.as<int>());
+    TT_LAUNCH_CHECK();
+  }
+
+  // ---- numeric-phase work partition, per-slot buffers, vertex -> slot incidence ----
+  const int64_t n_chunks = (n + ASM_THREADS - 1) / ASM_THREADS;
+  ctx->n_chunks = n_chunks;
+  TT_CUDA(ctx->chunk_tri.ensure(sizeof(int) * (size_t)(n_chunks + 2)));
+  k_chunk_bounds<<<grid_for(n_chunks + 1, 256), 256, 0, st>>>(ctx->tptr.as<int>(), nT, n_chunks, ctx->chunk_tri.as<int>());
+  TT_LAUNCH_CHECK();
+  TT_CUDA(ctx->asm_energy.ensure(sizeof(double) * (size_t)(n_chunks + 1)));
+  TT_CUDA(ctx->tvals.ensure(sizeof(T) * 9 * (size_t)(R + 1)));
+  TT_CUDA(ctx->tslot.ensure(sizeof(T) * 9 * (size_t)(nT + 1)));
+  const int64_t nvs = 3 * n_touched;
+  for (int i = 0; i < 2; ++i) {
+    TT_CUDA(ctx->vkeys[i].ensure(sizeof(uint64_t) * (size_t)(nvs + 1)));
+    TT_CUDA(ctx->vvals[i].ensure(sizeof(uint32_t) * (size_t)(nvs + 1)));
+  }
+  TT_CUDA(ctx->vptr.ensure(sizeof(int) * (size_t)(nV + 2)));
+  uint64_t* vkeys_sorted = ctx->vkeys[0].as<uint64_t>();
+  ctx->vvals_sorted = ctx->vvals[0].as<uint32_t>();
+  if (nvs > 0) {
+    k_emit_vslots<<<grid_for(nvs, 256), 256, 0, st>>>(q->tris, ctx->touched.as<int>(), n_touched,
+                                                      ctx->vkeys[0].as<uint64_t>(), ctx->vvals[0].as<uint32_t>());
+    TT_LAUNCH_CHECK();
+    s = sort_pairs(ctx, ctx->vkeys, ctx->vvals, nvs, bitsV, &vkeys_sorted, &ctx->vvals_sorted, st);
+    if (s != TT_OK) return s;
+  }
+  k_segment_ptr<<<grid_for(nvs + 1, 256), 256, 0, st>>>(vkeys_sorted, nvs, 0, nV, ctx->vptr.as<int>());
+  TT_LAUNCH_CHECK();
+  TT_CUDA(cudaStreamSynchronize(st));
+
+  ctx->sig.pos = q->pos;
+  ctx->sig.tris = q->tris;
+  ctx->sig.pairs = q->pairs;
+  ctx->sig.nV = nV;
+  ctx->sig.nT = nT;
+  ctx->sig.P = P;
+  ctx->sig.valid = true;
+  ctx->rows_gen = U > 0 ? -1 : 0;  // filled lazily by tt_stats if needed
+  if (nnzb_host) *nnzb_host = nnzb;
+  if (n_active_host) *n_active_host = A;
+  return TT_OK;
+}
+
+template <typename T>
+ttk::AsmParams<T> make_params(tt_ctx* ctx, const tt_problem* q) {
+  ttk::AsmParams<T> p;
+  p.pos = (const T*)q->pos;
+  p.tris = q->tris;
+  p.keys = ctx->keys_sorted;
+  p.dvals = ctx->dvals_sorted;
+  p.tptr = ctx->tptr.as<int>();
+  p.chunk_tri = ctx->chunk_tri.as<int>();
+  p.erank = ctx->erank.as<int>();
+  p.drank = ctx->drank.as<int>();
+  p.rowbase = ctx->rowbase.as<int64_t>();
+  p.vals = nullptr;
+  p.tvals = ctx->tvals.as<T>();
+  p.tslot = ctx->tslot.as<T>();
+  p.blk_energy = ctx->asm_energy.as<double>();
+  p.pvec = nullptr;
+  p.bitsT = ctx->bitsT;
+  p.hess_mode = ctx->opt.hess_mode;
+  p.sigma = ctx->opt.tc_scale;
+  return p;
+}
+
+template <typename T>
+tt_status numeric_impl(tt_ctx* ctx, const tt_problem* q, void* energy_sum, void* grad, int32_t* rowptr,
+                       int32_t* colind, void* vals, int64_t cap, cudaStream_t st) {
+  using namespace ttk;
+  const bool want_h = (vals != nullptr);
+  if (want_h && (!rowptr || !colind)) return fail(ctx, TT_ERR_INVALID_ARG, "bsr_rowptr/bsr_colind/bsr_vals must be all set or all NULL");
+  if (!energy_sum) return fail(ctx, TT_ERR_INVALID_ARG, "energy_sum is NULL");
+  if (want_h && cap < ctx->nnzb) return fail(ctx, TT_ERR_CAPACITY, "nnzb_capacity %lld < nnzb %lld", (long long)cap, (long long)ctx->nnzb);
+  const int64_t nV = q->n_verts;
+  if (want_h) {
+    if (rowptr != ctx->rowptr.as<int>())
+      TT_CUDA(cudaMemcpyAsync(rowptr, ctx->rowptr.p, sizeof(int) * (size_t)(nV + 1), cudaMemcpyDeviceToDevice, st));
+    if (colind != ctx->colind.as<int>() && ctx->nnzb > 0)
+      TT_CUDA(cudaMemcpyAsync(colind, ctx->colind.p, sizeof(int) * (size_t)ctx->nnzb, cudaMemcpyDeviceToDevice, st));
+  }
+  AsmParams<T> p = make_params<T>(ctx, q);
+  p.vals = (T*)vals;
+  if (ctx->n_chunks > 0) {
+    if (want_h) k_assemble<T, 0><<<(unsigned)ctx->n_chunks, ASM_THREADS, 0, st>>>(p);
+    else        k_assemble<T, 1><<<(unsigned)ctx->n_chunks, ASM_THREADS, 0, st>>>(p);
+    TT_LAUNCH_CHECK();
+    if (want_h && ctx->U > 0) {
+      k_merge<T><<<grid_for(9 * ctx->U, 256), 256, 0, st>>>(ctx->run_start.as<int>(), ctx->run_dest.as<int>(),
+                                                            ctx->rvals_sorted, ctx->U, ctx->tvals.as<T>(), (T*)vals);
+      TT_LAUNCH_CHECK();
+    }
+  }
+  if (grad && nV > 0) {
+    k_gather3<T><<<grid_for(3 * nV, 256), 256, 0, st>>>(ctx->vptr.as<int>(), ctx->vvals_sorted, nV, ctx->tslot.as<T>(), (T*)grad);
+    TT_LAUNCH_CHECK();
+  }
+  k_sum_partials<T><<<1, 1024, 0, st>>>(ctx->asm_energy.as<double>(), ctx->n_chunks, 1.0, (T*)energy_sum);
+  TT_LAUNCH_CHECK();
+  return TT_OK;
+}
+
+template <typename T>
+tt_status hessvec_impl(tt_ctx* ctx, const tt_problem* q, const void* pvec, void* y, cudaStream_t st) {
+  using namespace ttk;
+  AsmParams<T> p = make_params<T>(ctx, q);
+  p.pvec = (const T*)pvec;
+  p.blk_energy = nullptr;
+  if (ctx->n_chunks > 0) {
+    k_assemble<T, 2><<<(unsigned)ctx->n_chunks, ASM_THREADS, 0, st>>>(p);
+    TT_LAUNCH_CHECK();
+  }
+  if (q->n_verts > 0) {
+    k_gather3<T><<<grid_for(3 * q->n_verts, 256), 256, 0, st>>>(ctx->vptr.as<int>(), ctx->vvals_sorted, q->n_verts,
+                                                                ctx->tslot.as<T>(), (T*)y);
+    TT_LAUNCH_CHECK();
+  }
+  return TT_OK;
+}
+
+}  // namespace
+
+// =================================================================================== C ABI
+extern "C" {
+
+tt_status tt_create(const tt_options* opt, tt_ctx** out) {
+  if (!opt || !out) return TT_ERR_INVALID_ARG;
+  *out = nullptr;
+  if (opt->dtype != TT_F64 && opt->dtype != TT_F32) return TT_ERR_INVALID_ARG;
+  if (opt->hess_mode < TT_HESS_EQ4 || opt->hess_mode > TT_HESS_PSD2) return TT_ERR_INVALID_ARG;
+  if (!(opt->tc_scale > 0.0)) return TT_ERR_INVALID_ARG;
+  int ndev = 0;
+  if (cudaGetDeviceCount(&ndev) != cudaSuccess || opt->device < 0 || opt->device >= ndev) {
+    (void)cudaGetLastError();
+    return TT_ERR_CUDA;
+  }
+  if (cudaSetDevice(opt->device) != cudaSuccess) return TT_ERR_CUDA;
+  tt_ctx* c = new (std::nothrow) tt_ctx();
+  if (!c) return TT_ERR_NOMEM;
+  c->opt = *opt;
+  *out = c;
+  return TT_OK;
+}
+
+void tt_destroy(tt_ctx* ctx) {
+  if (!ctx) return;
+  cudaSetDevice(ctx->opt.device);
+  delete ctx;
+}
+
+tt_status tt_energy(tt_ctx* ctx, const tt_problem* prob, void* energy_sum, void* energy_per_pair,
+                    uint32_t* active_mask, void* tc, int64_t* n_active, void* stream) {
+  tt_status s = check_problem(ctx, prob);
+  if (s != TT_OK) return s;
+  if (!energy_sum) return fail(ctx, TT_ERR_INVALID_ARG, "energy_sum is NULL");
+  TT_CUDA(cudaSetDevice(ctx->opt.device));
+  cudaStream_t st = (cudaStream_t)stream;
+  return ctx->opt.dtype == TT_F64
+             ? energy_impl<double>(ctx, prob, energy_sum, energy_per_pair, active_mask, tc, n_active, st)
+             : energy_impl<float>(ctx, prob, energy_sum, energy_per_pair, active_mask, tc, n_active, st);
+}
+
+tt_status tt_hess_symbolic(tt_ctx* ctx, const tt_problem* prob, int64_t* nnzb_host, int64_t* n_active_host,
+                           void* stream) {
+  tt_status s = check_problem(ctx, prob);
+  if (s != TT_OK) return s;
+  if (!nnzb_host) return fail(ctx, TT_ERR_INVALID_ARG, "nnzb_host is NULL");
+  TT_CUDA(cudaSetDevice(ctx->opt.device));
+  cudaStream_t st = (cudaStream_t)stream;
+  return ctx->opt.dtype == TT_F64 ? symbolic_impl<double>(ctx, prob, nnzb_host, n_active_host, st)
+                                  : symbolic_impl<float>(ctx, prob, nnzb_host, n_active_host, st);
+}
+
+tt_status tt_energy_grad_hess(tt_ctx* ctx, const tt_problem* prob, void* energy_sum, void* grad,
+                              int32_t* bsr_rowptr, int32_t* bsr_colind, void* bsr_vals, int64_t nnzb_capacity,
+                              void* stream) {
+  tt_status s = check_problem(ctx, prob);
+  if (s != TT_OK) return s;
+  if (!ctx->sig.matches(prob)) return fail(ctx, TT_ERR_STATE, "tt_energy_grad_hess: no matching tt_hess_symbolic for this problem");
+  TT_CUDA(cudaSetDevice(ctx->opt.device));
+  cudaStream_t st = (cudaStream_t)stream;
+  return ctx->opt.dtype == TT_F64
+             ? numeric_impl<double>(ctx, prob, energy_sum, grad, bsr_rowptr, bsr_colind, bsr_vals, nnzb_capacity, st)
+             : numeric_impl<float>(ctx, prob, energy_sum, grad, bsr_rowptr, bsr_colind, bsr_vals, nnzb_capacity, st);
+}
+
+tt_status tt_hess_vec(tt_ctx* ctx, const tt_problem* prob, const void* p, void* y, void* stream) {
+  tt_status s = check_problem(ctx, prob);
+  if (s != TT_OK) return s;
+  if (!p || !y || p == y) return fail(ctx, TT_ERR_INVALID_ARG, "p / y NULL or aliased");
+  if (!ctx->sig.matches(prob)) return fail(ctx, TT_ERR_STATE, "tt_hess_vec: no matching tt_hess_symbolic for this problem");
+  TT_CUDA(cudaSetDevice(ctx->opt.device));
+  cudaStream_t st = (cudaStream_t)stream;
+  return ctx->opt.dtype == TT_F64 ? hessvec_impl<double>(ctx, prob, p, y, st) : hessvec_impl<float>(ctx, prob, p, y, st);
+}
+
+tt_status tt_energy_grad_hess_host(tt_ctx* ctx, const tt_problem* prob, void* energy_host, void* grad_host,
+                                   int64_t* nnzb_host, int64_t* n_active_host, int32_t* rowptr_host,
+                                   int32_t* colind_host, void* vals_host, int64_t nnzb_capacity, void* stream) {
+  tt_status s = check_problem(ctx, prob);
+  if (s != TT_OK) return s;
+  if (!energy_host || !nnzb_host) return fail(ctx, TT_ERR_INVALID_ARG, "energy_host / nnzb_host is NULL");
+  TT_CUDA(cudaSetDevice(ctx->opt.device));
+  cudaStream_t st = (cudaStream_t)stream;
+  const size_t w = ctx->opt.dtype == TT_F64 ? 8 : 4;
+  const int64_t nV = prob->n_verts, nT = prob->n_tris, P = prob->n_pairs;
+  TT_CUDA(ctx->h_pos.ensure(w * 3 * (size_t)nV + 16));
+  TT_CUDA(ctx->h_tris.ensure(sizeof(int) * 3 * (size_t)nT + 16));
+  TT_CUDA(ctx->h_pairs.ensure(sizeof(int) * 2 * (size_t)P + 16));
+  TT_CUDA(ctx->o_grad.ensure(w * 3 * (size_t)nV + 16));
+  TT_CUDA(ctx->o_energy.ensure(16));
+  if (nV) TT_CUDA(cudaMemcpyAsync(ctx->h_pos.p, prob->pos, w * 3 * (size_t)nV, cudaMemcpyHostToDevice, st));
+  if (nT) TT_CUDA(cudaMemcpyAsync(ctx->h_tris.p, prob->tris, sizeof(int) * 3 * (size_t)nT, cudaMemcpyHostToDevice, st));
+  if (P) TT_CUDA(cudaMemcpyAsync(ctx->h_pairs.p, prob->pairs, sizeof(int) * 2 * (size_t)P, cudaMemcpyHostToDevice, st));
+  tt_problem d = *prob;
+  d.pos = ctx->h_pos.p;
+  d.tris = ctx->h_tris.as<int32_t>();
+  d.pairs = ctx->h_pairs.as<int32_t>();
+  int64_t nnzb = 0, A = 0;
+  s = ctx->opt.dtype == TT_F64 ? symbolic_impl<double>(ctx, &d, &nnzb, &A, st) : symbolic_impl<float>(ctx, &d, &nnzb, &A, st);
+  if (s != TT_OK) return s;
+  *nnzb_host = nnzb;
+  if (n_active_host) *n_active_host = A;
+  TT_CUDA(ctx->o_vals.ensure(w * 9 * (size_t)nnzb + 16));
+  s = ctx->opt.dtype == TT_F64
+          ? numeric_impl<double>(ctx, &d, ctx->o_energy.p, ctx->o_grad.p, ctx->rowptr.as<int>(), ctx->colind.as<int>(), ctx->o_vals.p, nnzb, st)
+          : numeric_impl<float>(ctx, &d, ctx->o_energy.p, ctx->o_grad.p, ctx->rowptr.as<int>(), ctx->colind.as<int>(), ctx->o_vals.p, nnzb, st);
+  if (s != TT_OK) return s;
+  ctx->host_nnzb = nnzb;
+  TT_CUDA(cudaMemcpyAsync(energy_host, ctx->o_energy.p, w, cudaMemcpyDeviceToHost, st));
+  if (grad_host && nV) TT_CUDA(cudaMemcpyAsync(grad_host, ctx->o_grad.p, w * 3 * (size_t)nV, cudaMemcpyDeviceToHost, st));
+  if (rowptr_host) TT_CUDA(cudaMemcpyAsync(rowptr_host, ctx->rowptr.p, sizeof(int) * (size_t)(nV + 1), cudaMemcpyDeviceToHost, st));
+  if (colind_host || vals_host) {
+    if (nnzb_capacity < nnzb) {
+      cudaStreamSynchronize(st);
+      return fail(ctx, TT_ERR_CAPACITY, "nnzb_capacity %lld < nnzb %lld", (long long)nnzb_capacity, (long long)nnzb);
+    }
+    if (colind_host && nnzb) TT_CUDA(cudaMemcpyAsync(colind_host, ctx->colind.p, sizeof(int) * (size_t)nnzb, cudaMemcpyDeviceToHost, st));
+    if (vals_host && nnzb) TT_CUDA(cudaMemcpyAsync(vals_host, ctx->o_vals.p, w * 9 * (size_t)nnzb, cudaMemcpyDeviceToHost, st));
+  }
+  TT_CUDA(cudaStreamSynchronize(st));
+  return TT_OK;
+}
+
+tt_status tt_bsr_device(tt_ctx* ctx, const int32_t** rowptr, const int32_t** colind, const void** vals, int64_t* nnzb) {
+  if (!ctx) return TT_ERR_INVALID_ARG;
+  if (!ctx->o_vals.p) return fail(ctx, TT_ERR_STATE, "tt_bsr_device: no tt_energy_grad_hess_host result");
+  if (rowptr) *rowptr = ctx->rowptr.as<int32_t>();
+  if (colind) *colind = ctx->colind.as<int32_t>();
+  if (vals) *vals = ctx->o_vals.p;
+  if (nnzb) *nnzb = ctx->host_nnzb;
+  return TT_OK;
+}
+
+tt_status tt_stats(const tt_ctx* ctx, int64_t* what, int32_t n) {
+  if (!ctx || !what || n < 0) return TT_ERR_INVALID_ARG;
+  const int64_t v[8] = {ctx->A, ctx->n_dir, ctx->n_touched, ctx->nnzb - ctx->U, ctx->U, ctx->R, ctx->nnzb, ctx->launches};
+  for (int i = 0; i < n && i < 8; ++i) what[i] = v[i];
+  return TT_OK;
+}
+
+const char* tt_status_string(tt_status s) {
+  switch (s) {
+    case TT_OK: return "TT_OK";
+    case TT_ERR_INVALID_ARG: return "TT_ERR_INVALID_ARG";
+    case TT_ERR_CUDA: return "TT_ERR_CUDA";
+    case TT_ERR_NOMEM: return "TT_ERR_NOMEM";
+    case TT_ERR_CAPACITY: return "TT_ERR_CAPACITY";
+    case TT_ERR_STATE: return "TT_ERR_STATE";
+  }
+  return "TT_ERR_UNKNOWN";
+}
+
+const char* tt_last_error(const tt_ctx* ctx) { return ctx ? ctx->err.c_str() : "ctx is NULL"; }
+
+}  // extern "C"

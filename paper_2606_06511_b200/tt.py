@@ -1,0 +1,194 @@
+"""Thin Python binding of libtt.so (include/tt.h): argument marshalling only.
+
+Same names as the C ABI.  PyTorch supplies device memory and streams; every step of the hot path
+runs inside the library's CUDA kernels.  There is no CPU fallback: importing works anywhere (so
+that CPU-only tests can check the exported symbols), but creating a context without the built
+library or without a CUDA device raises.
+"""
+from __future__ import annotations
+
+import ctypes
+from pathlib import Path
+
+import torch
+
+_HERE = Path(__file__).resolve().parent
+LIB_PATH = _HERE / "libtt.so"
+
+TT_OK = 0
+TT_F64, TT_F32 = 0, 1
+TT_HESS_EQ4, TT_HESS_FILTER, TT_HESS_PSD2 = 0, 1, 2
+TT_FLAG_FORCE_GENERAL_ROWS = 1
+
+EXPORTS = ["tt_create", "tt_destroy", "tt_energy", "tt_hess_symbolic", "tt_energy_grad_hess", "tt_hess_vec",
+           "tt_energy_grad_hess_host", "tt_bsr_device", "tt_stats", "tt_status_string", "tt_last_error"]
+
+
+class TTOptions(ctypes.Structure):
+    _fields_ = [("dtype", ctypes.c_int32), ("hess_mode", ctypes.c_int32), ("tc_scale", ctypes.c_double),
+                ("device", ctypes.c_int32), ("flags", ctypes.c_int32)]
+
+
+class TTProblem(ctypes.Structure):
+    _fields_ = [("pos", ctypes.c_void_p), ("n_verts", ctypes.c_int64), ("tris", ctypes.c_void_p),
+                ("n_tris", ctypes.c_int64), ("pairs", ctypes.c_void_p), ("n_pairs", ctypes.c_int64)]
+
+
+class TTError(RuntimeError):
+    def __init__(self, status, name, msg):
+        super().__init__("%s (%d): %s" % (name, status, msg))
+        self.status = status
+
+
+_lib = None
+
+
+def load_library():
+    """dlopen libtt.so and declare the C signatures.  Raises if the library was not built."""
+    global _lib
+    if _lib is not None:
+        return _lib
+    if not LIB_PATH.exists():
+        raise RuntimeError("libtt.so is missing (%s): run `python -m paper_2606_06511_b200.build` "
+                           "or __graft_entry__.build(); there is no CPU fallback" % LIB_PATH)
+    lib = ctypes.CDLL(str(LIB_PATH))
+    vp, i64 = ctypes.c_void_p, ctypes.c_int64
+    lib.tt_create.argtypes = [ctypes.POINTER(TTOptions), ctypes.POINTER(vp)]
+    lib.tt_create.restype = ctypes.c_int
+    lib.tt_destroy.argtypes = [vp]
+    lib.tt_destroy.restype = None
+    lib.tt_energy.argtypes = [vp, ctypes.POINTER(TTProblem), vp, vp, vp, vp, vp, vp]
+    lib.tt_energy.restype = ctypes.c_int
+    lib.tt_hess_symbolic.argtypes = [vp, ctypes.POINTER(TTProblem), ctypes.POINTER(i64), ctypes.POINTER(i64), vp]
+    lib.tt_hess_symbolic.restype = ctypes.c_int
+    lib.tt_energy_grad_hess.argtypes = [vp, ctypes.POINTER(TTProblem), vp, vp, vp, vp, vp, i64, vp]
+    lib.tt_energy_grad_hess.restype = ctypes.c_int
+    lib.tt_hess_vec.argtypes = [vp, ctypes.POINTER(TTProblem), vp, vp, vp]
+    lib.tt_hess_vec.restype = ctypes.c_int
+    lib.tt_energy_grad_hess_host.argtypes = [vp, ctypes.POINTER(TTProblem), vp, vp, ctypes.POINTER(i64),
+                                             ctypes.POINTER(i64), vp, vp, vp, i64, vp]
+    lib.tt_energy_grad_hess_host.restype = ctypes.c_int
+    lib.tt_bsr_device.argtypes = [vp, ctypes.POINTER(vp), ctypes.POINTER(vp), ctypes.POINTER(vp), ctypes.POINTER(i64)]
+    lib.tt_bsr_device.restype = ctypes.c_int
+    lib.tt_stats.argtypes = [vp, ctypes.POINTER(i64), ctypes.c_int32]
+    lib.tt_stats.restype = ctypes.c_int
+    lib.tt_status_string.argtypes = [ctypes.c_int]
+    lib.tt_status_string.restype = ctypes.c_char_p
+    lib.tt_last_error.argtypes = [vp]
+    lib.tt_last_error.restype = ctypes.c_char_p
+    _lib = lib
+    return lib
+
+
+def _ptr(t):
+    return None if t is None else ctypes.c_void_p(t.data_ptr())
+
+
+def _stream_ptr(stream):
+    if stream is None:
+        stream = torch.cuda.current_stream()
+    return ctypes.c_void_p(stream.cuda_stream)
+
+
+class Context:
+    """Owns a tt_ctx.  dtype: torch.float64 or torch.float32."""
+
+    def __init__(self, dtype=torch.float64, hess_mode=TT_HESS_FILTER, tc_scale=1.0, device=0, flags=0):
+        if not torch.cuda.is_available():
+            raise RuntimeError("paper_2606_06511_b200 needs a CUDA device (no CPU fallback)")
+        self.lib = load_library()
+        self.dtype = dtype
+        self.device = torch.device("cuda", device)
+        opt = TTOptions(TT_F64 if dtype == torch.float64 else TT_F32, int(hess_mode), float(tc_scale), int(device), int(flags))
+        h = ctypes.c_void_p()
+        st = self.lib.tt_create(ctypes.byref(opt), ctypes.byref(h))
+        if st != TT_OK:
+            raise TTError(st, self.lib.tt_status_string(st).decode(), "tt_create failed")
+        self.h = h
+
+    def close(self):
+        if getattr(self, "h", None):
+            self.lib.tt_destroy(self.h)
+            self.h = None
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+    def _check(self, st):
+        if st != TT_OK:
+            raise TTError(st, self.lib.tt_status_string(st).decode(), self.lib.tt_last_error(self.h).decode())
+
+    def problem(self, pos, tris, pairs):
+        """Builds a tt_problem view of device tensors (kept alive by the returned tuple)."""
+        assert pos.is_cuda and tris.is_cuda and pairs.is_cuda
+        assert pos.dtype == self.dtype and tris.dtype == torch.int32 and pairs.dtype == torch.int32
+        assert pos.is_contiguous() and tris.is_contiguous() and pairs.is_contiguous()
+        pb = TTProblem(pos.data_ptr(), pos.shape[0], tris.data_ptr(), tris.shape[0], pairs.data_ptr(), pairs.shape[0])
+        return pb, (pos, tris, pairs)
+
+    # ---- tt_energy ----
+    def tt_energy(self, prob, energy_sum, energy_per_pair=None, active_mask=None, tc=None, n_active=None, stream=None):
+        self._check(self.lib.tt_energy(self.h, ctypes.byref(prob[0]), _ptr(energy_sum), _ptr(energy_per_pair),
+                                       _ptr(active_mask), _ptr(tc), _ptr(n_active), _stream_ptr(stream)))
+
+    # ---- tt_hess_symbolic ----
+    def tt_hess_symbolic(self, prob, stream=None):
+        nnzb, na = ctypes.c_int64(0), ctypes.c_int64(0)
+        self._check(self.lib.tt_hess_symbolic(self.h, ctypes.byref(prob[0]), ctypes.byref(nnzb), ctypes.byref(na),
+                                              _stream_ptr(stream)))
+        return nnzb.value, na.value
+
+    # ---- tt_energy_grad_hess ----
+    def tt_energy_grad_hess(self, prob, energy_sum, grad=None, bsr_rowptr=None, bsr_colind=None, bsr_vals=None,
+                            nnzb_capacity=0, stream=None):
+        self._check(self.lib.tt_energy_grad_hess(self.h, ctypes.byref(prob[0]), _ptr(energy_sum), _ptr(grad),
+                                                 _ptr(bsr_rowptr), _ptr(bsr_colind), _ptr(bsr_vals),
+                                                 int(nnzb_capacity), _stream_ptr(stream)))
+
+    # ---- tt_hess_vec ----
+    def tt_hess_vec(self, prob, p, y, stream=None):
+        self._check(self.lib.tt_hess_vec(self.h, ctypes.byref(prob[0]), _ptr(p), _ptr(y), _stream_ptr(stream)))
+
+    # ---- tt_energy_grad_hess_host ----
+    def tt_energy_grad_hess_host(self, pos_h, tris_h, pairs_h, energy_h, grad_h=None, rowptr_h=None, colind_h=None,
+                                 vals_h=None, nnzb_capacity=0, stream=None):
+        """All tensors are HOST tensors (pinned recommended).  Returns (nnzb, n_active)."""
+        for t in (pos_h, tris_h, pairs_h, energy_h):
+            assert not t.is_cuda and t.is_contiguous()
+        pb = TTProblem(pos_h.data_ptr(), pos_h.shape[0], tris_h.data_ptr(), tris_h.shape[0], pairs_h.data_ptr(),
+                       pairs_h.shape[0])
+        nnzb, na = ctypes.c_int64(0), ctypes.c_int64(0)
+        self._check(self.lib.tt_energy_grad_hess_host(self.h, ctypes.byref(pb), _ptr(energy_h), _ptr(grad_h),
+                                                      ctypes.byref(nnzb), ctypes.byref(na), _ptr(rowptr_h),
+                                                      _ptr(colind_h), _ptr(vals_h), int(nnzb_capacity),
+                                                      _stream_ptr(stream)))
+        return nnzb.value, na.value
+
+    def tt_stats(self):
+        arr = (ctypes.c_int64 * 8)()
+        self._check(self.lib.tt_stats(self.h, arr, 8))
+        keys = ["n_active", "n_directed", "n_touched_tris", "blocks_direct", "blocks_merged", "merge_records", "nnzb",
+                "launches"]
+        return dict(zip(keys, [int(v) for v in arr]))
+
+
+def assemble(ctx: Context, pos, tris, pairs, want_hess=True, stream=None):
+    """Convenience: symbolic + allocate + numeric.  Returns dict of device tensors."""
+    prob = ctx.problem(pos, tris, pairs)
+    nnzb, n_active = ctx.tt_hess_symbolic(prob, stream)
+    dev, dt = pos.device, ctx.dtype
+    energy = torch.zeros(1, dtype=dt, device=dev)
+    grad = torch.empty((pos.shape[0], 3), dtype=dt, device=dev)
+    out = dict(energy=energy, grad=grad, nnzb=nnzb, n_active=n_active, prob=prob)
+    if want_hess:
+        rowptr = torch.empty(pos.shape[0] + 1, dtype=torch.int32, device=dev)
+        colind = torch.empty(max(nnzb, 1), dtype=torch.int32, device=dev)
+        vals = torch.empty((max(nnzb, 1), 3, 3), dtype=dt, device=dev)
+        ctx.tt_energy_grad_hess(prob, energy, grad, rowptr, colind, vals, max(nnzb, 1), stream)
+        out.update(rowptr=rowptr, colind=colind[:nnzb], vals=vals[:nnzb])
+    else:
+        ctx.tt_energy_grad_hess(prob, energy, grad, None, None, None, 0, stream)
+    return out

@@ -1,0 +1,283 @@
+"""GPU parity (-m gpu): the CUDA path, called through the C ABI, against the CPU oracle on the
+same seeded inputs.  Bars (BASELINE.json north_star, A13): active set bit-exact;
+fp64 energy/gradient rel 1e-10, Hessian blocks Frobenius-rel 1e-9 (pattern exact), H.p rel 1e-9;
+fp32 variant 1e-4 / 1e-3."""
+import numpy as np
+import pytest
+
+from helpers import filter_margins, rel, unpack_mask
+
+torch = pytest.importorskip("torch")
+pytestmark = pytest.mark.gpu
+
+TOL = {"f64": dict(e=1e-10, g=1e-10, h=1e-9, y=1e-9, tc=1e-10),
+       "f32": dict(e=1e-4, g=1e-4, h=1e-3, y=1e-3, tc=1e-4)}
+
+
+def _dev():
+    if not torch.cuda.is_available():
+        pytest.skip("no CUDA device")
+    return torch.device("cuda:0")
+
+
+def run_case(oracle, pb, dtype="f64", hess_mode=1, sigma=1.0, flags=0, check_vals=True, check_energy_call=True):
+    from paper_2606_06511_b200 import tt
+    dev = _dev()
+    tdt = torch.float64 if dtype == "f64" else torch.float32
+    pos_np = pb.pos.astype(np.float32).astype(np.float64) if dtype == "f32" else pb.pos   # A12
+    pbo = type(pb)(pos_np, pb.tris, pb.pairs, pb.name, pb.meta)
+    pairs = filter_margins(oracle, pbo, hess_mode, sigma)
+    ref = oracle.assemble(pos_np, pb.tris, pairs, sigma, hess_mode)
+    tol = TOL[dtype]
+    ctx = tt.Context(tdt, hess_mode, sigma, 0, flags)
+    pos = torch.from_numpy(pos_np).to(dev).to(tdt).contiguous()
+    tris = torch.from_numpy(pb.tris).to(dev)
+    prs = torch.from_numpy(pairs).to(dev)
+    P = pairs.shape[0]
+    act_ref = ref["active"].astype(bool)
+
+    if check_energy_call:
+        prob = ctx.problem(pos, tris, prs)
+        e_sum = torch.zeros(1, dtype=tdt, device=dev)
+        e_pp = torch.zeros(max(P, 1), dtype=tdt, device=dev)
+        mask = torch.zeros(max((P + 31) // 32, 1), dtype=torch.int32, device=dev)
+        tc = torch.zeros((max(P, 1), 2), dtype=tdt, device=dev)
+        na = torch.zeros(1, dtype=torch.int64, device=dev)
+        ctx.tt_energy(prob, e_sum, e_pp, mask, tc, na)
+        torch.cuda.synchronize()
+        act = unpack_mask(mask.cpu().numpy().view(np.uint32), P)
+        assert (act == act_ref).all(), "active set differs at %s" % np.nonzero(act != act_ref)[0][:10]
+        assert int(na.cpu()[0]) == int(act_ref.sum())
+        assert rel(e_sum.cpu().numpy()[0], ref["energy"]) <= tol["e"]
+        if P:
+            tcg = tc.cpu().numpy().astype(np.float64)[:P]
+            scale = np.abs(ref["tc"]).max() if act_ref.any() else 1.0
+            assert np.abs(tcg - ref["tc"]).max() <= max(tol["tc"], 1e-12) * scale * 10
+            assert (tcg[~act_ref] == 0).all()
+            epp = e_pp.cpu().numpy().astype(np.float64)[:P]
+            assert rel(epp, ref["T"]) <= tol["e"]
+
+    out = tt.assemble(ctx, pos, tris, prs, want_hess=True)
+    torch.cuda.synchronize()
+    assert out["n_active"] == int(act_ref.sum())
+    assert rel(out["energy"].cpu().numpy()[0], ref["energy"]) <= tol["e"]
+    assert rel(out["grad"].cpu().numpy(), ref["grad"]) <= tol["g"]
+    assert out["nnzb"] == ref["nnzb"]
+    assert (out["rowptr"].cpu().numpy() == ref["rowptr"]).all()
+    assert (out["colind"].cpu().numpy() == ref["colind"]).all()
+    if check_vals:
+        assert rel(out["vals"].cpu().numpy(), ref["vals"]) <= tol["h"]
+    # gradient-only call must agree with the full call
+    e2 = torch.zeros(1, dtype=tdt, device=dev)
+    g2 = torch.empty_like(out["grad"])
+    ctx.tt_energy_grad_hess(out["prob"], e2, g2)
+    torch.cuda.synchronize()
+    assert torch.equal(g2, out["grad"]) and torch.equal(e2, out["energy"])
+    # matrix-free H.p (a5) == oracle's per-pair J^T M J p == BSR.p (P10)
+    rng = np.random.default_rng(12345)
+    p_np = rng.normal(size=pos_np.shape)
+    if dtype == "f32":
+        p_np = p_np.astype(np.float32).astype(np.float64)
+    p = torch.from_numpy(p_np).to(dev).to(tdt)
+    y = torch.full_like(p, float("nan"))
+    ctx.tt_hess_vec(out["prob"], p, y)
+    torch.cuda.synchronize()
+    y_ref = oracle.hess_vec_pairs(pos_np.shape[0], pb.tris, pairs, ref["active"], ref["tc"], ref["J"], p_np, hess_mode)
+    assert rel(y.cpu().numpy(), y_ref) <= tol["y"]
+    y_bsr = oracle.bsr_matvec(out["rowptr"].cpu().numpy(), out["colind"].cpu().numpy(),
+                              out["vals"].cpu().numpy().astype(np.float64), p_np)
+    assert rel(y_bsr, y_ref) <= tol["y"]
+    stats = ctx.tt_stats()
+    ctx.close()
+    return ref, out, stats
+
+
+# ------------------------------------------------------------------------------------ configs
+@pytest.mark.parametrize("mode", [0, 1, 2])
+@pytest.mark.parametrize("dtype", ["f64", "f32"])
+def test_config0_soup(oracle_mod, mode, dtype):
+    from paper_2606_06511_b200 import inputs
+    ref, out, st = run_case(oracle_mod, inputs.config0_soup(), dtype, mode)
+    assert st["blocks_merged"] == 0          # own-vertex soup: every row is exclusive
+    assert 500 < out["n_active"] < 800
+
+
+@pytest.mark.parametrize("flags", [0, 1])
+def test_config0_shared_vertex_pool(oracle_mod, flags):
+    """Triangles drawn from a small vertex pool: adjacency rule + general (merge) rows."""
+    from paper_2606_06511_b200 import inputs
+    pb = inputs.config0_soup(n_tris=64, pool=48, seed=77)
+    ref, out, st = run_case(oracle_mod, pb, "f64", 1, flags=flags)
+    assert st["blocks_merged"] > 0
+
+
+def test_config0_forced_general_rows_equal_exclusive(oracle_mod):
+    """TT_FLAG_FORCE_GENERAL_ROWS routes every row through the merge path: same matrix."""
+    from paper_2606_06511_b200 import inputs
+    pb = inputs.config0_soup()
+    _, a, sa = run_case(oracle_mod, pb, "f64", 1, flags=0, check_energy_call=False)
+    _, b, sb = run_case(oracle_mod, pb, "f64", 1, flags=1, check_energy_call=False)
+    assert sa["blocks_merged"] == 0 and sb["blocks_direct"] == 0
+    assert torch.equal(a["colind"], b["colind"]) and torch.equal(a["rowptr"], b["rowptr"])
+    assert rel(a["vals"].cpu().numpy(), b["vals"].cpu().numpy()) < 1e-14
+
+
+def test_sigma_half(oracle_mod):
+    from paper_2606_06511_b200 import inputs
+    run_case(oracle_mod, inputs.config0_soup(), "f64", 0, sigma=0.5)
+
+
+@pytest.mark.parametrize("dtype", ["f64", "f32"])
+def test_config1_icospheres(oracle_mod, dtype):
+    from paper_2606_06511_b200 import inputs
+    ref, out, st = run_case(oracle_mod, inputs.config1_icospheres(), dtype, 1)
+    assert out["n_active"] > 100 and st["blocks_merged"] > 0
+
+
+def test_config2_cloth(oracle_mod):
+    from paper_2606_06511_b200 import inputs
+    ref, out, st = run_case(oracle_mod, inputs.config2_cloth(), "f64", 1)
+    assert out["n_active"] > 1000
+
+
+def test_config3_torus_reduced(oracle_mod):
+    """Config 3's recipe at 1/25 of the triangles (full size: tests/test_gpu_full.py, slow)."""
+    from paper_2606_06511_b200 import inputs
+    run_case(oracle_mod, inputs.config3_torus(nu=200, nv=100), "f64", 1)
+    run_case(oracle_mod, inputs.config3_torus(nu=200, nv=100), "f32", 1)
+
+
+@pytest.mark.parametrize("dtype", ["f64", "f32"])
+def test_config4_sweep_reduced(oracle_mod, dtype):
+    """Config 4's recipe, 60k triangles / 300k pairs: several CTA chunks, ragged tail, ~5 partners per triangle."""
+    from paper_2606_06511_b200 import inputs
+    pb = inputs.config4_sweep(n_tris=60_000, n_pairs=300_007)
+    ref, out, st = run_case(oracle_mod, pb, dtype, 1)
+    assert st["blocks_merged"] == 0
+    assert abs(out["n_active"] / pb.n_pairs - 0.5) < 0.01
+
+
+def test_long_rows_span_cta_rounds(oracle_mod):
+    """Few triangles, many pairs each: a triangle's entries span several 128-entry rounds and
+    exceed the shared-memory ranking limit for some rows (general path by size)."""
+    from paper_2606_06511_b200 import inputs
+    pb = inputs.config4_sweep(n_tris=400, n_pairs=60_000, seed=4242)
+    ref, out, st = run_case(oracle_mod, pb, "f64", 1)
+
+
+# ------------------------------------------------------------------------------------ edge cases
+def test_empty_and_inactive_inputs(oracle_mod):
+    from paper_2606_06511_b200 import inputs, tt
+    dev = _dev()
+    pb = inputs.config0_soup()
+    ctx = tt.Context(torch.float64, 1, 1.0, 0)
+    pos = torch.from_numpy(pb.pos).to(dev)
+    tris = torch.from_numpy(pb.tris).to(dev)
+    # no candidates at all
+    empty = torch.zeros((0, 2), dtype=torch.int32, device=dev)
+    out = tt.assemble(ctx, pos, tris, empty)
+    torch.cuda.synchronize()
+    assert out["nnzb"] == 0 and out["n_active"] == 0
+    assert float(out["energy"].cpu()[0]) == 0.0 and not out["grad"].cpu().numpy().any()
+    assert not out["rowptr"].cpu().numpy().any()
+    # candidates, none active (each triangle against a far-away copy)
+    pos2 = torch.cat([pos, pos + 10.0])
+    tris2 = torch.cat([tris, tris + pos.shape[0]])
+    pairs2 = torch.stack([torch.arange(64), torch.arange(64) + 64], 1).to(torch.int32).to(dev)
+    out = tt.assemble(ctx, pos2, tris2, pairs2)
+    p = torch.randn_like(pos2)
+    y = torch.full_like(p, float("nan"))
+    ctx.tt_hess_vec(out["prob"], p, y)
+    torch.cuda.synchronize()
+    assert out["nnzb"] == 0 and out["n_active"] == 0 and not y.cpu().numpy().any()
+    assert float(out["energy"].cpu()[0]) == 0.0 and not out["grad"].cpu().numpy().any()
+    ctx.close()
+
+
+def test_duplicate_and_reversed_candidates(oracle_mod):
+    """The same pair listed twice and once reversed: legal input, contributions add up."""
+    from paper_2606_06511_b200 import inputs
+    pb = inputs.config0_soup()
+    extra = np.concatenate([pb.pairs, pb.pairs[:300], pb.pairs[100:400, ::-1]])
+    pb2 = type(pb)(pb.pos, pb.tris, np.ascontiguousarray(extra), "dups", {})
+    run_case(oracle_mod, pb2, "f64", 1)
+
+
+def test_error_paths(oracle_mod):
+    from paper_2606_06511_b200 import inputs, tt
+    dev = _dev()
+    pb = inputs.config0_soup()
+    ctx = tt.Context(torch.float64, 1, 1.0, 0)
+    pos = torch.from_numpy(pb.pos).to(dev)
+    tris = torch.from_numpy(pb.tris).to(dev)
+    prs = torch.from_numpy(pb.pairs).to(dev)
+    prob = ctx.problem(pos, tris, prs)
+    e = torch.zeros(1, dtype=torch.float64, device=dev)
+    g = torch.zeros_like(pos)
+    with pytest.raises(tt.TTError) as ei:          # numeric before symbolic
+        ctx.tt_energy_grad_hess(prob, e, g)
+    assert ei.value.status == -5
+    nnzb, _ = ctx.tt_hess_symbolic(prob)
+    rp = torch.zeros(pos.shape[0] + 1, dtype=torch.int32, device=dev)
+    ci = torch.zeros(nnzb, dtype=torch.int32, device=dev)
+    va = torch.zeros((nnzb, 3, 3), dtype=torch.float64, device=dev)
+    with pytest.raises(tt.TTError) as ei:          # capacity too small
+        ctx.tt_energy_grad_hess(prob, e, g, rp, ci, va, nnzb - 1)
+    assert ei.value.status == -4
+    with pytest.raises(tt.TTError) as ei:          # aliased p / y
+        ctx.tt_hess_vec(prob, g, g)
+    assert ei.value.status == -1
+    ctx.tt_energy_grad_hess(prob, e, g, rp, ci, va, nnzb)   # still usable after errors
+    torch.cuda.synchronize()
+    ctx.close()
+
+
+def test_host_buffer_entry_point(oracle_mod):
+    """tt_energy_grad_hess_host (the e2e call bench.py times) == device-buffer path == oracle."""
+    from paper_2606_06511_b200 import inputs, tt
+    _dev()
+    pb = inputs.config4_sweep(n_tris=20_000, n_pairs=100_000)
+    pairs = filter_margins(oracle_mod, pb, 1)
+    ref = oracle_mod.assemble(pb.pos, pb.tris, pairs, 1.0, 1)
+    ctx = tt.Context(torch.float64, 1, 1.0, 0)
+    pos_h = torch.from_numpy(pb.pos).pin_memory()
+    tris_h = torch.from_numpy(pb.tris).pin_memory()
+    pairs_h = torch.from_numpy(pairs).pin_memory()
+    e_h = torch.zeros(1, dtype=torch.float64).pin_memory()
+    g_h = torch.zeros((pb.n_verts, 3), dtype=torch.float64).pin_memory()
+    rp_h = torch.zeros(pb.n_verts + 1, dtype=torch.int32)
+    cap = ref["nnzb"]
+    ci_h = torch.zeros(cap, dtype=torch.int32)
+    va_h = torch.zeros((cap, 3, 3), dtype=torch.float64)
+    nnzb, na = ctx.tt_energy_grad_hess_host(pos_h, tris_h, pairs_h, e_h, g_h, rp_h, ci_h, va_h, cap)
+    assert nnzb == ref["nnzb"] and na == int(ref["active"].sum())
+    assert rel(e_h.numpy()[0], ref["energy"]) <= 1e-10
+    assert rel(g_h.numpy(), ref["grad"]) <= 1e-10
+    assert (rp_h.numpy() == ref["rowptr"]).all() and (ci_h.numpy() == ref["colind"]).all()
+    assert rel(va_h.numpy(), ref["vals"]) <= 1e-9
+    ctx.close()
+
+
+def test_properties_on_gpu_outputs(oracle_mod):
+    """Invariants that hold at any size, checked on the GPU's own outputs (config 4 recipe):
+    grad.x = 4E, H_EQ4 x = 3 grad (I6), rows of H sum to zero against translations, symmetry."""
+    from paper_2606_06511_b200 import inputs, tt
+    dev = _dev()
+    pb = inputs.config4_sweep(n_tris=50_000, n_pairs=250_000, seed=99)
+    ctx = tt.Context(torch.float64, 0, 1.0, 0)
+    pos = torch.from_numpy(pb.pos).to(dev)
+    out = tt.assemble(ctx, pos, torch.from_numpy(pb.tris).to(dev), torch.from_numpy(pb.pairs).to(dev))
+    y = torch.empty_like(pos)
+    ctx.tt_hess_vec(out["prob"], pos, y)
+    ones = torch.zeros_like(pos)
+    ones[:, 1] = 1.0
+    z = torch.empty_like(pos)
+    ctx.tt_hess_vec(out["prob"], ones, z)
+    torch.cuda.synchronize()
+    E = float(out["energy"].cpu()[0])
+    g = out["grad"]
+    assert abs(float((g * pos).sum().cpu()) - 4 * E) <= 1e-9 * 4 * E
+    assert float((y - 3 * g).norm().cpu()) <= 1e-9 * float((3 * g).norm().cpu())
+    assert float(z.norm().cpu()) <= 1e-9 * float(out["vals"].norm().cpu())
+    assert float(g.sum(0).abs().max().cpu()) <= 1e-9 * float(g.abs().max().cpu()) * 100
+    ctx.close()
