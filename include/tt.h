@@ -127,11 +127,14 @@ tt_status tt_hess_vec(tt_ctx* ctx, const tt_problem* prob, const void* p, void* 
  *   energy_host HOST [1] dtype; grad_host HOST [nV,3] dtype or NULL;
  *   nnzb_host HOST [1]; n_active_host HOST [1] or NULL;
  *   rowptr_host [nV+1] / colind_host [nnzb_capacity] / vals_host [nnzb_capacity,3,3]: HOST, each
- *   may be NULL (the BSR then stays on the device, see tt_bsr_device).  Synchronises `stream`.   */
+ *   may be NULL (the BSR then stays on the device, see tt_bsr_device);
+ *   p_host / y_host HOST [nV,3] dtype, both set or both NULL: additionally y = H p (tt_hess_vec).
+ * Synchronises `stream`.                                                                          */
 tt_status tt_energy_grad_hess_host(tt_ctx* ctx, const tt_problem* prob, void* energy_host,
                                    void* grad_host, int64_t* nnzb_host, int64_t* n_active_host,
                                    int32_t* rowptr_host, int32_t* colind_host, void* vals_host,
-                                   int64_t nnzb_capacity, void* stream);
+                                   int64_t nnzb_capacity, const void* p_host, void* y_host,
+                                   void* stream);
 
 /* Device views of the BSR produced by the last tt_energy_grad_hess_host (owned by ctx, valid
  * until the next *_host call or tt_destroy).                                                      */
@@ -142,6 +145,11 @@ tt_status tt_bsr_device(tt_ctx* ctx, const int32_t** rowptr, const int32_t** col
  * [2]=touched triangles, [3]=blocks written directly (exclusive rows), [4]=blocks produced by the
  * general-row merge, [5]=merge records, [6]=nnzb, [7]=kernel launches issued by this ctx so far.                     */
 tt_status tt_stats(const tt_ctx* ctx, int64_t* what, int32_t n);
+
+/* Device durations (CUDA events on the caller's stream) of the most recent launch of the three
+ * large kernels: ms[0] = classification (K1), ms[1] = assembly (K4), ms[2] = H.p (K6); -1 if the
+ * kernel has not run.  Blocks until those launches have finished.                                 */
+tt_status tt_kernel_ms(tt_ctx* ctx, float* ms, int32_t n);
 
 const char* tt_status_string(tt_status s);
 const char* tt_last_error(const tt_ctx* ctx);

@@ -21,7 +21,8 @@ namespace ttk {
 using ttg::d3;
 
 constexpr int CLS_THREADS = 256;   // K1 / K2 CTA size (8 warps -> 8 mask words per CTA)
-constexpr int ASM_THREADS = 128;   // K4 / K6 CTA size = directed entries per round
+constexpr int ASM_THREADS = 128;   // K4 / K6 CTA size: 4 independent warps
+constexpr int ASM_CHUNK = 32;      // directed entries per warp chunk (snapped to triangle boundaries)
 constexpr int SYM_WARPS = 4;       // warps per CTA in the per-triangle symbolic kernels
 constexpr int SYM_LMAX = 1536;     // longest row (in blocks) ranked in shared memory
 
@@ -354,12 +355,12 @@ k_fill_rows(const int* __restrict__ tris, const int* __restrict__ touched, int64
 }
 
 // Work partition of K4/K6: chunk c owns the triangles whose first directed entry lies in
-// [c*ASM_THREADS, (c+1)*ASM_THREADS): chunk_tri[c] = first such triangle (binary search in tptr).
+// [c*ASM_CHUNK, (c+1)*ASM_CHUNK): chunk_tri[c] = first such triangle (binary search in tptr).
 __global__ void k_chunk_bounds(const int* __restrict__ tptr, int64_t nT, int64_t n_chunks,
                                int* __restrict__ chunk_tri) {
   const int64_t c = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
   if (c > n_chunks) return;
-  const int64_t target = c * ASM_THREADS;
+  const int64_t target = c * ASM_CHUNK;
   int64_t lo = 0, hi = nT;  // first s in [0,nT] with tptr[s] >= target
   while (lo < hi) {
     const int64_t mid = (lo + hi) >> 1;
@@ -382,18 +383,23 @@ __global__ void k_emit_vslots(const int* __restrict__ tris, const int* __restric
 
 // ------------------------------------------------------------------------------------------ K4
 // Triangle-centric numeric phase.  MODE 0: energy + gradient + Hessian blocks.  MODE 1: energy +
-// gradient only.  MODE 2: H.p (K6).  One thread per directed entry e = (source s -> partner t).
+// gradient only.  MODE 2: H.p (K6).  One LANE per directed entry e = (source s -> partner t); one
+// WARP per chunk of ~32 entries that starts and ends on a triangle boundary, so a warp owns every
+// entry of the triangles it touches and needs no block-level barrier and no atomics.
 // The pair is always evaluated in its canonical order (T_a = pairs[k,0]) so that both directed
 // copies of a pair compute bit-identical J and take the same FILTER decision.
 //
-// Per row slot m of the source triangle the thread forms
-//   off-diagonal blocks  H[p_m, q_n] = g0_pm w0_qn^T + g1_pm w1_qn^T   (q_n = partner vertices)
-//   diagonal contribution H[p_m, p_n], and the gradient / H.p contribution of p_m,
-// with w0 = c00 g0 + c01 g1, w1 = c01 g0 + c11 g1.  Off-diagonal blocks have exactly one
-// contribution and are stored straight to their final place; diagonal blocks and the per-slot
-// 3-vectors are summed over the triangle's entries through shared memory in entry order.
-constexpr int RED_W = 30;       // doubles per entry per row round: 27 diagonal + 3 gradient
-constexpr int RED_STRIDE = 31;  // odd stride: conflict-free column reads
+// Per entry the lane forms, with w0 = c00 g0 + c01 g1 and w1 = c01 g0 + c11 g1,
+//   off-diagonal blocks  H[p_m, q_n] = g0_pm w0_qn^T + g1_pm w1_qn^T   (q_n = partner vertices):
+//     exactly one contribution each -> staged through shared memory row by row and written out
+//     by the whole warp in address order (coalesced) to their final place;
+//   the diagonal 9x9 contribution (symmetric: 45 unique values) and the 9 gradient / H.p values:
+//     staged in shared memory, then summed over the triangle's entries with lane = component,
+//     entries in order (deterministic), accumulators carried in registers across rounds.
+constexpr int NDIAG = 45;                 // upper triangle of the symmetric 9x9 diagonal block
+constexpr int NRED_FULL = NDIAG + 9;      // + gradient of the three own vertices
+constexpr int RED_STRIDE = 55;            // odd: conflict-free lane = entry writes
+constexpr int OUT_STRIDE = 27;            // odd: conflict-free lane = entry writes
 
 template <typename T>
 struct AsmParams {
@@ -409,38 +415,81 @@ struct AsmParams {
   T* vals;                  // final BSR values
   T* tvals;                 // merge workspace values
   T* tslot;                 // [3nT][3] per-slot gradient (MODE 0/1) or H.p (MODE 2) partials
-  double* blk_energy;       // [n_chunks]
+  double* chunk_energy;     // [n_chunks]
   const T* pvec;            // MODE 2: p [nV,3]
+  int64_t n_chunks;
   int bitsT;
   int hess_mode;
   double sigma;
 };
 
+struct AsmWarpSmem {
+  double red[32 * RED_STRIDE];
+  double out[32 * OUT_STRIDE];
+  unsigned long long rowp[3][32];   // destination row base (element pointer) per entry and row
+  int er[32][3];
+  int src[32];
+};
+
 template <typename T, int MODE>
 __global__ void __launch_bounds__(ASM_THREADS)
 k_assemble(const AsmParams<T> P) {
-  __shared__ double s_red[ASM_THREADS * RED_STRIDE];
-  __shared__ double s_carry[2][3][RED_W];  // [round parity][row][component]
-  __shared__ int s_src[ASM_THREADS];
-  __shared__ int s_seg_begin[ASM_THREADS + 1];
-  __shared__ int s_nseg;
-  __shared__ double s_e[ASM_THREADS / 32];
-  __shared__ int s_wcnt[ASM_THREADS / 32];
-
-  const int tid = threadIdx.x;
-  const int c = blockIdx.x;
+  extern __shared__ __align__(16) unsigned char s_raw[];
+  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+  AsmWarpSmem& S = reinterpret_cast<AsmWarpSmem*>(s_raw)[warp];
+  const int64_t c = (int64_t)blockIdx.x * (ASM_THREADS / 32) + warp;
+  if (c >= P.n_chunks) return;  // warps are independent: no __syncthreads below
   const int tri_lo = P.chunk_tri[c], tri_hi = P.chunk_tri[c + 1];
   const int e_lo = P.tptr[tri_lo], e_hi = P.tptr[tri_hi];
   const uint64_t tmask = (1ull << P.bitsT) - 1ull;
-  double e_acc = 0.0;
-  constexpr int NRED = (MODE == 0) ? RED_W : 3;  // values reduced per row round
-  constexpr int ROFF = (MODE == 0) ? 0 : 27;     // first used column of s_red
+  constexpr int NRED = (MODE == 0) ? NRED_FULL : 9;
+  constexpr int GOFF = (MODE == 0) ? NDIAG : 0;  // first gradient / H.p component
 
-  int parity = 0;
-  for (int base = e_lo; base < e_hi; base += ASM_THREADS, parity ^= 1) {
-    const int e = base + tid;
+  // lane = component bookkeeping for the reduction: comp0 = lane, comp1 = lane + 32
+  int al0 = 0, be0 = 0, al1 = 0, be1 = 0;  // (alpha, beta) of the diagonal components
+  if (MODE == 0) {
+    int k = 0;
+    for (int a = 0; a < 9; ++a)
+      for (int b = a; b < 9; ++b, ++k) {
+        if (k == lane) { al0 = a; be0 = b; }
+        if (k == lane + 32) { al1 = a; be1 = b; }
+      }
+  }
+  double acc0 = 0.0, acc1 = 0.0, e_acc = 0.0;
+  int cur = -1;
+
+  auto flush = [&](int s) {
+    if (MODE == 0) {
+      const int64_t rb0 = P.rowbase[3 * (int64_t)s], rb1 = P.rowbase[3 * (int64_t)s + 1], rb2 = P.rowbase[3 * (int64_t)s + 2];
+      const int dr0 = P.drank[3 * (int64_t)s], dr1 = P.drank[3 * (int64_t)s + 1], dr2 = P.drank[3 * (int64_t)s + 2];
+      auto put = [&](int a, int b, double v) {  // D[a][b] and its mirror D[b][a]
+        const int m = a / 3, i = a - 3 * m, n = b / 3, j = b - 3 * n;
+        {
+          const int64_t rb = (m == 0) ? rb0 : (m == 1) ? rb1 : rb2;
+          const int dr = (n == 0) ? dr0 : (n == 1) ? dr1 : dr2;
+          T* rowp = (rb >= 0) ? (P.vals + 9 * rb) : (P.tvals + 9 * (-rb - 1));
+          rowp[9 * (int64_t)dr + 3 * i + j] = (T)v;
+        }
+        if (a != b) {
+          const int64_t rb = (n == 0) ? rb0 : (n == 1) ? rb1 : rb2;
+          const int dr = (m == 0) ? dr0 : (m == 1) ? dr1 : dr2;
+          T* rowp = (rb >= 0) ? (P.vals + 9 * rb) : (P.tvals + 9 * (-rb - 1));
+          rowp[9 * (int64_t)dr + 3 * j + i] = (T)v;
+        }
+      };
+      put(al0, be0, acc0);
+      if (lane + 32 < NDIAG) put(al1, be1, acc1);
+      else if (lane + 32 < NRED_FULL) P.tslot[9 * (int64_t)s + (lane + 32 - NDIAG)] = (T)acc1;
+    } else {
+      if (lane < 9) P.tslot[9 * (int64_t)s + lane] = (T)acc0;
+    }
+  };
+
+  for (int base = e_lo; base < e_hi; base += 32) {
+    const int e = base + lane;
     const bool valid = e < e_hi;
-    int s = -1, side = 0;
+    const int nvalid = min(32, e_hi - base);
+    int s = -1;
     double g0[18], g1[18];
     ttg::Coefs cf = {0, 0, 0, 0, 0};
     double hp0 = 0.0, hp1 = 0.0;  // MODE 2: M (J p_loc)
@@ -449,8 +498,7 @@ k_assemble(const AsmParams<T> P) {
     if (valid) {
       const uint64_t key = P.keys[e];
       s = (int)(key >> P.bitsT);
-      const uint32_t dv = P.dvals[e];
-      side = (int)(dv & 1u);
+      const int side = (int)(P.dvals[e] & 1u);
       const int t = (int)(key & tmask);
       const int2 pr = side ? make_int2(t, s) : make_int2(s, t);  // canonical (pairs[k,0], pairs[k,1])
       int va[3], vb[3];
@@ -461,8 +509,8 @@ k_assemble(const AsmParams<T> P) {
       ttg::pair_derivs(a[0], a[1], a[2], b[0], b[1], b[2], P.sigma, q, g0, g1);
       cf = ttg::pair_coefs(q.tc0, q.tc1, g0, g1, P.hess_mode);
       if (side == 0) {
-        const double t = q.tc0 * q.tc1;
-        e_acc += t * t;  // Eq. 2, counted once per pair
+        const double tt = q.tc0 * q.tc1;
+        e_acc += tt * tt;  // Eq. 2, counted once per pair
       }
       if (MODE == 2) {
         double j0 = 0.0, j1 = 0.0;
@@ -486,108 +534,90 @@ k_assemble(const AsmParams<T> P) {
         }
       }
     }
-    // ---- segment table of this round (entries of one source triangle are consecutive) ----
-    s_src[tid] = s;
-    __syncthreads();
-    const bool head = valid && (tid == 0 || s_src[tid - 1] != s);
-    const uint32_t hb = __ballot_sync(0xffffffffu, head);
-    const int w = tid >> 5, l = tid & 31;
-    if (l == 0) s_wcnt[w] = __popc(hb);
-    __syncthreads();
-    int segbase = 0;
-#pragma unroll
-    for (int i = 0; i < ASM_THREADS / 32; ++i) segbase += (i < w) ? s_wcnt[i] : 0;
-    if (head) s_seg_begin[segbase + __popc(hb & ((1u << l) - 1u))] = tid;
-    if (tid == 0) {
-      int n = 0;
-#pragma unroll
-      for (int i = 0; i < ASM_THREADS / 32; ++i) n += s_wcnt[i];
-      s_nseg = n;
-      const int nvalid = min(ASM_THREADS, e_hi - base);
-      s_seg_begin[n] = nvalid;
-    }
-    __syncthreads();
-    const int nseg = s_nseg;
-
-    // ---- three row rounds ----
-#pragma unroll 1
-    for (int m = 0; m < 3; ++m) {
-      double gm0[3], gm1[3];  // g0, g1 at the row vertex p_m (own slot m)
-#pragma unroll
-      for (int i = 0; i < 3; ++i) {
-        gm0[i] = ttg::sel3(m, g0[i], g0[3 + i], g0[6 + i]);
-        gm1[i] = ttg::sel3(m, g1[i], g1[3 + i], g1[6 + i]);
-      }
-      double* red = s_red + tid * RED_STRIDE;
+    // ---- stage the values to be reduced over the triangle: lane = entry ----
+    S.src[lane] = s;
+    {
+      double* red = S.red + lane * RED_STRIDE;
       if (MODE == 0) {
-        int64_t rb = 0;
-        int er[3] = {0, 0, 0};
-        if (valid) {
-          rb = P.rowbase[3 * (int64_t)s + m];
+        double d0[9], d1[9];
 #pragma unroll
-          for (int n = 0; n < 3; ++n) er[n] = P.erank[3 * (int64_t)e + n];
+        for (int i = 0; i < 9; ++i) {
+          d0[i] = cf.c00 * g0[i] + cf.c01 * g1[i];
+          d1[i] = cf.c01 * g0[i] + cf.c11 * g1[i];
         }
-        T* rowp = (rb >= 0) ? (P.vals + 9 * rb) : (P.tvals + 9 * (-rb - 1));
+        int k = 0;
 #pragma unroll
-        for (int n = 0; n < 3; ++n) {
-          // off-diagonal block (p_m, partner vertex n): partner occupies entries 9..17
-          double w0[3], w1[3], d0[3], d1[3];
+        for (int a = 0; a < 9; ++a)
 #pragma unroll
-          for (int j = 0; j < 3; ++j) {
-            const double a0 = g0[9 + 3 * n + j], a1 = g1[9 + 3 * n + j];
-            w0[j] = cf.c00 * a0 + cf.c01 * a1;
-            w1[j] = cf.c01 * a0 + cf.c11 * a1;
-            const double b0 = g0[3 * n + j], b1 = g1[3 * n + j];
-            d0[j] = cf.c00 * b0 + cf.c01 * b1;
-            d1[j] = cf.c01 * b0 + cf.c11 * b1;
-          }
-          if (valid) {
-            T* blk = rowp + 9 * (int64_t)er[n];
+          for (int b = a; b < 9; ++b, ++k) red[k] = g0[a] * d0[b] + g1[a] * d1[b];
+      }
 #pragma unroll
-            for (int i = 0; i < 3; ++i)
+      for (int i = 0; i < 9; ++i)
+        red[GOFF + i] = (MODE == 2) ? (hp0 * g0[i] + hp1 * g1[i]) : (cf.cg0 * g0[i] + cf.cg1 * g1[i]);
+    }
+    if (MODE == 0) {
 #pragma unroll
-              for (int j = 0; j < 3; ++j) blk[3 * i + j] = (T)(gm0[i] * w0[j] + gm1[i] * w1[j]);
-          }
+      for (int m = 0; m < 3; ++m) {
+        unsigned long long ptr = 0ull;
+        if (valid) {
+          const int64_t rb = P.rowbase[3 * (int64_t)s + m];
+          ptr = (unsigned long long)((rb >= 0) ? (P.vals + 9 * rb) : (P.tvals + 9 * (-rb - 1)));
+          S.er[lane][m] = P.erank[3 * (int64_t)e + m];
+        }
+        S.rowp[m][lane] = ptr;
+      }
+    }
+    __syncwarp();
+    // ---- reduction over entries, lane = component, fixed order ----
+    for (int i = 0; i < nvalid; ++i) {
+      const int si = S.src[i];
+      if (si != cur) {  // warp-uniform
+        if (cur >= 0) flush(cur);
+        acc0 = 0.0;
+        acc1 = 0.0;
+        cur = si;
+      }
+      if (lane < NRED) acc0 += S.red[i * RED_STRIDE + lane];
+      if (NRED > 32 && lane + 32 < NRED) acc1 += S.red[i * RED_STRIDE + lane + 32];
+    }
+    // ---- off-diagonal blocks, one row of the source triangle at a time ----
+    if (MODE == 0) {
+      double w0[9], w1[9];  // partner side: entries 9..17
+#pragma unroll
+      for (int i = 0; i < 9; ++i) {
+        w0[i] = cf.c00 * g0[9 + i] + cf.c01 * g1[9 + i];
+        w1[i] = cf.c01 * g0[9 + i] + cf.c11 * g1[9 + i];
+      }
+#pragma unroll
+      for (int m = 0; m < 3; ++m) {
+        double* o = S.out + lane * OUT_STRIDE;
+#pragma unroll
+        for (int n = 0; n < 3; ++n)
 #pragma unroll
           for (int i = 0; i < 3; ++i)
 #pragma unroll
-            for (int j = 0; j < 3; ++j) red[9 * n + 3 * i + j] = gm0[i] * d0[j] + gm1[i] * d1[j];
+            for (int j = 0; j < 3; ++j)
+              o[9 * n + 3 * i + j] = g0[3 * m + i] * w0[3 * n + j] + g1[3 * m + i] * w1[3 * n + j];
+        __syncwarp();
+        const int total = nvalid * 27;
+        for (int f = lane; f < total; f += 32) {
+          const int ee = f / 27, r = f - 27 * ee;
+          const int n = r / 9, q = r - 9 * n;
+          T* rowp = reinterpret_cast<T*>(S.rowp[m][ee]);
+          rowp[9 * (int64_t)S.er[ee][n] + q] = (T)S.out[f];
         }
+        __syncwarp();
       }
-      if (MODE == 2) {
-#pragma unroll
-        for (int i = 0; i < 3; ++i) red[27 + i] = hp0 * gm0[i] + hp1 * gm1[i];
-      } else {
-#pragma unroll
-        for (int i = 0; i < 3; ++i) red[27 + i] = cf.cg0 * gm0[i] + cf.cg1 * gm1[i];
-      }
-      __syncthreads();
-      // ---- fixed-order segmented reduction: task = (segment, component) ----
-      for (int task = tid; task < nseg * NRED; task += ASM_THREADS) {
-        const int seg = task / NRED, comp = ROFF + (task - seg * NRED);
-        const int i0 = s_seg_begin[seg], i1 = s_seg_begin[seg + 1];
-        const int ss = s_src[i0];
-        // a triangle can span rounds of this CTA: carry in from / out to s_carry
-        const bool cont_in = (seg == 0) && (base > e_lo) && (P.tptr[ss] < base);
-        const bool cont_out = (seg == nseg - 1) && (base + ASM_THREADS < e_hi) && (P.tptr[ss + 1] > base + ASM_THREADS);
-        double acc = cont_in ? s_carry[parity][m][comp - ROFF] : 0.0;
-        for (int i = i0; i < i1; ++i) acc += s_red[i * RED_STRIDE + comp];
-        if (cont_out) {
-          s_carry[parity ^ 1][m][comp - ROFF] = acc;
-        } else if (comp < 27) {
-          const int64_t rb = P.rowbase[3 * (int64_t)ss + m];
-          T* rowp = (rb >= 0) ? (P.vals + 9 * rb) : (P.tvals + 9 * (-rb - 1));
-          const int n = comp / 9;
-          rowp[9 * (int64_t)P.drank[3 * (int64_t)ss + n] + (comp - 9 * n)] = (T)acc;
-        } else {
-          P.tslot[3 * (3 * (int64_t)ss + m) + (comp - 27)] = (T)acc;
-        }
-      }
-      __syncthreads();
+    } else {
+      __syncwarp();
     }
   }
-  const double e = block_sum<ASM_THREADS>(e_acc, s_e);
-  if (tid == 0 && P.blk_energy) P.blk_energy[c] = e;
+  if (cur >= 0) flush(cur);
+  if (MODE != 2) {
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) e_acc += __shfl_down_sync(0xffffffffu, e_acc, o);
+    if (lane == 0) P.chunk_energy[c] = e_acc;
+  }
 }
 
 // ------------------------------------------------------------------------------------------ K5

@@ -73,7 +73,7 @@ struct tt_ctx {
   DevBuf chunk_tri, asm_energy, tvals, tslot, vkeys[2], vvals[2], vptr;
   DevBuf cub_tmp;
   // host-API mirrors
-  DevBuf h_pos, h_tris, h_pairs, o_vals, o_grad, o_energy;
+  DevBuf h_pos, h_tris, h_pairs, h_p, o_vals, o_grad, o_energy, o_y;
   // cached symbolic state
   Signature sig;
   int64_t A = 0, n_dir = 0, n_touched = 0, R = 0, U = 0, nnzb = 0, n_chunks = 0, rows_excl = 0, rows_gen = 0;
@@ -84,6 +84,9 @@ struct tt_ctx {
   uint32_t* rvals_sorted = nullptr;
   uint32_t* vvals_sorted = nullptr;
   int64_t host_nnzb = 0;
+  // device-side timing of the three big kernels (events recorded on the caller's stream)
+  cudaEvent_t ev[3][2] = {{nullptr, nullptr}, {nullptr, nullptr}, {nullptr, nullptr}};
+  bool ev_used[3] = {false, false, false};
 };
 
 namespace {
@@ -199,10 +202,13 @@ tt_status run_classify(tt_ctx* ctx, const tt_problem* q, T* e_pp, T* tc, cudaStr
   TT_CUDA(ctx->energy.ensure(sizeof(double) * 2));
   TT_CUDA(cudaMemsetAsync(ctx->blk_count.as<int>() + nblk, 0, sizeof(int), st));
   if (nblk > 0) {
+    TT_CUDA(cudaEventRecord(ctx->ev[0][0], st));
     ttk::k_classify<T><<<(unsigned)nblk, ttk::CLS_THREADS, 0, st>>>(
         (const T*)q->pos, q->tris, (const int2*)q->pairs, P, ctx->opt.tc_scale, ctx->mask.as<uint32_t>(),
         ctx->blk_count.as<int>(), ctx->blk_energy.as<double>(), e_pp, tc);
     TT_LAUNCH_CHECK();
+    TT_CUDA(cudaEventRecord(ctx->ev[0][1], st));
+    ctx->ev_used[0] = true;
   }
   tt_status s = scan_i32(ctx, ctx->blk_count.as<int>(), ctx->blk_off.as<int>(), nblk + 1, st);
   if (s != TT_OK) return s;
@@ -388,7 +394,7 @@ tt_status symbolic_impl(tt_ctx* ctx, const tt_problem* q, int64_t* nnzb_host, in
   }
 
   // ---- numeric-phase work partition, per-slot buffers, vertex -> slot incidence ----
-  const int64_t n_chunks = (n + ASM_THREADS - 1) / ASM_THREADS;
+  const int64_t n_chunks = (n + ASM_CHUNK - 1) / ASM_CHUNK;
   ctx->n_chunks = n_chunks;
   TT_CUDA(ctx->chunk_tri.ensure(sizeof(int) * (size_t)(n_chunks + 2)));
   k_chunk_bounds<<<grid_for(n_chunks + 1, 256), 256, 0, st>>>(ctx->tptr.as<int>(), nT, n_chunks, ctx->chunk_tri.as<int>());
@@ -443,7 +449,8 @@ ttk::AsmParams<T> make_params(tt_ctx* ctx, const tt_problem* q) {
   p.vals = nullptr;
   p.tvals = ctx->tvals.as<T>();
   p.tslot = ctx->tslot.as<T>();
-  p.blk_energy = ctx->asm_energy.as<double>();
+  p.chunk_energy = ctx->asm_energy.as<double>();
+  p.n_chunks = ctx->n_chunks;
   p.pvec = nullptr;
   p.bitsT = ctx->bitsT;
   p.hess_mode = ctx->opt.hess_mode;
@@ -469,9 +476,14 @@ tt_status numeric_impl(tt_ctx* ctx, const tt_problem* q, void* energy_sum, void*
   AsmParams<T> p = make_params<T>(ctx, q);
   p.vals = (T*)vals;
   if (ctx->n_chunks > 0) {
-    if (want_h) k_assemble<T, 0><<<(unsigned)ctx->n_chunks, ASM_THREADS, 0, st>>>(p);
-    else        k_assemble<T, 1><<<(unsigned)ctx->n_chunks, ASM_THREADS, 0, st>>>(p);
+    TT_CUDA(cudaEventRecord(ctx->ev[1][0], st));
+    const unsigned grid = grid_for(ctx->n_chunks, ASM_THREADS / 32);
+    const size_t smem = sizeof(AsmWarpSmem) * (ASM_THREADS / 32);
+    if (want_h) k_assemble<T, 0><<<grid, ASM_THREADS, smem, st>>>(p);
+    else        k_assemble<T, 1><<<grid, ASM_THREADS, smem, st>>>(p);
     TT_LAUNCH_CHECK();
+    TT_CUDA(cudaEventRecord(ctx->ev[1][1], st));
+    ctx->ev_used[1] = true;
     if (want_h && ctx->U > 0) {
       k_merge<T><<<grid_for(9 * ctx->U, 256), 256, 0, st>>>(ctx->run_start.as<int>(), ctx->run_dest.as<int>(),
                                                             ctx->rvals_sorted, ctx->U, ctx->tvals.as<T>(), (T*)vals);
@@ -492,10 +504,13 @@ tt_status hessvec_impl(tt_ctx* ctx, const tt_problem* q, const void* pvec, void*
   using namespace ttk;
   AsmParams<T> p = make_params<T>(ctx, q);
   p.pvec = (const T*)pvec;
-  p.blk_energy = nullptr;
+  p.chunk_energy = nullptr;
   if (ctx->n_chunks > 0) {
-    k_assemble<T, 2><<<(unsigned)ctx->n_chunks, ASM_THREADS, 0, st>>>(p);
+    TT_CUDA(cudaEventRecord(ctx->ev[2][0], st));
+    k_assemble<T, 2><<<grid_for(ctx->n_chunks, ASM_THREADS / 32), ASM_THREADS, sizeof(AsmWarpSmem) * (ASM_THREADS / 32), st>>>(p);
     TT_LAUNCH_CHECK();
+    TT_CUDA(cudaEventRecord(ctx->ev[2][1], st));
+    ctx->ev_used[2] = true;
   }
   if (q->n_verts > 0) {
     k_gather3<T><<<grid_for(3 * q->n_verts, 256), 256, 0, st>>>(ctx->vptr.as<int>(), ctx->vvals_sorted, q->n_verts,
@@ -525,6 +540,17 @@ tt_status tt_create(const tt_options* opt, tt_ctx** out) {
   tt_ctx* c = new (std::nothrow) tt_ctx();
   if (!c) return TT_ERR_NOMEM;
   c->opt = *opt;
+  for (int i = 0; i < 3; ++i)
+    for (int j = 0; j < 2; ++j)
+      if (cudaEventCreate(&c->ev[i][j]) != cudaSuccess) { delete c; return TT_ERR_CUDA; }
+  {
+    const int smem = (int)(sizeof(ttk::AsmWarpSmem) * (ttk::ASM_THREADS / 32));
+    cudaError_t e = cudaSuccess;
+    auto opt_in = [&](const void* f) { if (e == cudaSuccess) e = cudaFuncSetAttribute(f, cudaFuncAttributeMaxDynamicSharedMemorySize, smem); };
+    opt_in((const void*)ttk::k_assemble<double, 0>); opt_in((const void*)ttk::k_assemble<double, 1>); opt_in((const void*)ttk::k_assemble<double, 2>);
+    opt_in((const void*)ttk::k_assemble<float, 0>);  opt_in((const void*)ttk::k_assemble<float, 1>);  opt_in((const void*)ttk::k_assemble<float, 2>);
+    if (e != cudaSuccess) { (void)cudaGetLastError(); delete c; return TT_ERR_CUDA; }
+  }
   *out = c;
   return TT_OK;
 }
@@ -532,6 +558,9 @@ tt_status tt_create(const tt_options* opt, tt_ctx** out) {
 void tt_destroy(tt_ctx* ctx) {
   if (!ctx) return;
   cudaSetDevice(ctx->opt.device);
+  for (int i = 0; i < 3; ++i)
+    for (int j = 0; j < 2; ++j)
+      if (ctx->ev[i][j]) cudaEventDestroy(ctx->ev[i][j]);
   delete ctx;
 }
 
@@ -583,8 +612,10 @@ tt_status tt_hess_vec(tt_ctx* ctx, const tt_problem* prob, const void* p, void* 
 
 tt_status tt_energy_grad_hess_host(tt_ctx* ctx, const tt_problem* prob, void* energy_host, void* grad_host,
                                    int64_t* nnzb_host, int64_t* n_active_host, int32_t* rowptr_host,
-                                   int32_t* colind_host, void* vals_host, int64_t nnzb_capacity, void* stream) {
+                                   int32_t* colind_host, void* vals_host, int64_t nnzb_capacity,
+                                   const void* p_host, void* y_host, void* stream) {
   tt_status s = check_problem(ctx, prob);
+  if ((p_host == nullptr) != (y_host == nullptr)) return fail(ctx, TT_ERR_INVALID_ARG, "p_host and y_host must both be set or both NULL");
   if (s != TT_OK) return s;
   if (!energy_host || !nnzb_host) return fail(ctx, TT_ERR_INVALID_ARG, "energy_host / nnzb_host is NULL");
   TT_CUDA(cudaSetDevice(ctx->opt.device));
@@ -614,6 +645,15 @@ tt_status tt_energy_grad_hess_host(tt_ctx* ctx, const tt_problem* prob, void* en
           : numeric_impl<float>(ctx, &d, ctx->o_energy.p, ctx->o_grad.p, ctx->rowptr.as<int>(), ctx->colind.as<int>(), ctx->o_vals.p, nnzb, st);
   if (s != TT_OK) return s;
   ctx->host_nnzb = nnzb;
+  if (p_host && nV) {
+    TT_CUDA(ctx->h_p.ensure(w * 3 * (size_t)nV + 16));
+    TT_CUDA(ctx->o_y.ensure(w * 3 * (size_t)nV + 16));
+    TT_CUDA(cudaMemcpyAsync(ctx->h_p.p, p_host, w * 3 * (size_t)nV, cudaMemcpyHostToDevice, st));
+    s = ctx->opt.dtype == TT_F64 ? hessvec_impl<double>(ctx, &d, ctx->h_p.p, ctx->o_y.p, st)
+                                 : hessvec_impl<float>(ctx, &d, ctx->h_p.p, ctx->o_y.p, st);
+    if (s != TT_OK) return s;
+    TT_CUDA(cudaMemcpyAsync(y_host, ctx->o_y.p, w * 3 * (size_t)nV, cudaMemcpyDeviceToHost, st));
+  }
   TT_CUDA(cudaMemcpyAsync(energy_host, ctx->o_energy.p, w, cudaMemcpyDeviceToHost, st));
   if (grad_host && nV) TT_CUDA(cudaMemcpyAsync(grad_host, ctx->o_grad.p, w * 3 * (size_t)nV, cudaMemcpyDeviceToHost, st));
   if (rowptr_host) TT_CUDA(cudaMemcpyAsync(rowptr_host, ctx->rowptr.p, sizeof(int) * (size_t)(nV + 1), cudaMemcpyDeviceToHost, st));
@@ -643,6 +683,17 @@ tt_status tt_stats(const tt_ctx* ctx, int64_t* what, int32_t n) {
   if (!ctx || !what || n < 0) return TT_ERR_INVALID_ARG;
   const int64_t v[8] = {ctx->A, ctx->n_dir, ctx->n_touched, ctx->nnzb - ctx->U, ctx->U, ctx->R, ctx->nnzb, ctx->launches};
   for (int i = 0; i < n && i < 8; ++i) what[i] = v[i];
+  return TT_OK;
+}
+
+tt_status tt_kernel_ms(tt_ctx* ctx, float* ms, int32_t n) {
+  if (!ctx || !ms || n < 0) return TT_ERR_INVALID_ARG;
+  for (int i = 0; i < n && i < 3; ++i) {
+    ms[i] = -1.0f;
+    if (!ctx->ev_used[i]) continue;
+    TT_CUDA(cudaEventSynchronize(ctx->ev[i][1]));
+    TT_CUDA(cudaEventElapsedTime(&ms[i], ctx->ev[i][0], ctx->ev[i][1]));
+  }
   return TT_OK;
 }
 

@@ -45,82 +45,126 @@ class Problem:
 # --------------------------------------------------------------------------------------------
 # orientation determinants (textbook geometry; NOT the method)
 # --------------------------------------------------------------------------------------------
-def _cross(a, b):
-    return np.stack([a[..., 1] * b[..., 2] - a[..., 2] * b[..., 1],
+class _NP:
+    """numpy backend of the orientation classifier."""
+    @staticmethod
+    def asarray(a, like=None):
+        return np.asarray(a)
+
+    stack = staticmethod(lambda xs: np.stack(xs, axis=-1))
+    norm = staticmethod(lambda a: np.linalg.norm(a, axis=-1))
+    maximum = staticmethod(np.maximum)
+    abs = staticmethod(np.abs)
+    to_numpy = staticmethod(lambda a: np.asarray(a))
+
+    @staticmethod
+    def zeros_bool(n, like=None):
+        return np.zeros(n, dtype=bool)
+
+
+def _torch_backend(device):
+    import torch
+
+    class _TH:
+        """torch backend (same arithmetic, any device) -- used by bench.py to shape 10M+ pair
+        workloads in seconds on the GPU box; the pairs it keeps are then copied to the host."""
+        @staticmethod
+        def asarray(a, like=None):
+            return torch.as_tensor(a, device=device)
+
+        stack = staticmethod(lambda xs: torch.stack(xs, dim=-1))
+        norm = staticmethod(lambda a: torch.linalg.norm(a, dim=-1))
+        maximum = staticmethod(lambda a, b: torch.clamp(a, min=b))
+        abs = staticmethod(torch.abs)
+        to_numpy = staticmethod(lambda a: a.cpu().numpy())
+
+        @staticmethod
+        def zeros_bool(n, like=None):
+            return torch.zeros(n, dtype=torch.bool, device=device)
+
+    return _TH
+
+
+def _cross(xp, a, b):
+    return xp.stack([a[..., 1] * b[..., 2] - a[..., 2] * b[..., 1],
                      a[..., 2] * b[..., 0] - a[..., 0] * b[..., 2],
-                     a[..., 0] * b[..., 1] - a[..., 1] * b[..., 0]], axis=-1)
+                     a[..., 0] * b[..., 1] - a[..., 1] * b[..., 0]])
 
 
 def _dot(a, b):
     return (a * b).sum(-1)
 
 
-def _orient(p, q, r, s):
+def _orient(xp, p, q, r, s):
     """Signed volume (x6) of tetrahedron (p,q,r,s)."""
-    return _dot(_cross(q - p, r - p), s - p)
+    return _dot(_cross(xp, q - p, r - p), s - p)
 
 
-def _segment_pierces(p, q, t0, t1, t2):
+def _segment_pierces(xp, p, q, t0, t1, t2):
     """Closed segment pq crosses the interior of triangle (t0,t1,t2) (strict)."""
-    dp = _orient(t0, t1, t2, p)
-    dq = _orient(t0, t1, t2, q)
-    s0 = _orient(p, q, t0, t1)
-    s1 = _orient(p, q, t1, t2)
-    s2 = _orient(p, q, t2, t0)
+    dp = _orient(xp, t0, t1, t2, p)
+    dq = _orient(xp, t0, t1, t2, q)
+    s0 = _orient(xp, p, q, t0, t1)
+    s1 = _orient(xp, p, q, t1, t2)
+    s2 = _orient(xp, p, q, t2, t0)
     opposite = ((dp > 0) & (dq < 0)) | ((dp < 0) & (dq > 0))
     inside = ((s0 > 0) & (s1 > 0) & (s2 > 0)) | ((s0 < 0) & (s1 < 0) & (s2 < 0))
     return opposite & inside
 
 
-def classify_pairs(pos, tris, pairs, eps=1e-6, chunk=1 << 20):
+def classify_pairs(pos, tris, pairs, eps=1e-6, chunk=1 << 20, device=None):
     """Returns (intersects[P] bool, degenerate[P] bool) from orientation determinants only.
 
-    intersects: some edge of one triangle pierces the other (6+... = 6 edge/triangle tests).
+    intersects: some edge of one triangle pierces the other (6 edge/triangle tests).
     degenerate: any vertex-plane distance, edge-line/edge-line distance or plane angle within
     eps (relative to the pair's mean edge length) of zero, or the pair shares a vertex index.
+    device=None: numpy; otherwise a torch device string (same arithmetic in fp64).
     """
+    xp = _NP if device is None else _torch_backend(device)
     P = pairs.shape[0]
     hit = np.zeros(P, dtype=bool)
     deg = np.zeros(P, dtype=bool)
+    pos_x = xp.asarray(pos)
+    tris_x = xp.asarray(tris if device is None else tris.astype(np.int64))
+    tiny = float(np.finfo(np.float64).tiny)
     for lo in range(0, P, chunk):
-        pr = pairs[lo:lo + chunk]
-        ta = tris[pr[:, 0]]
-        tb = tris[pr[:, 1]]
-        A = pos[ta]  # [n,3,3]
-        B = pos[tb]
+        pr = xp.asarray(pairs[lo:lo + chunk] if device is None else pairs[lo:lo + chunk].astype(np.int64))
+        ta = tris_x[pr[:, 0]]
+        tb = tris_x[pr[:, 1]]
+        A = pos_x[ta]  # [n,3,3]
+        B = pos_x[tb]
         a = [A[:, 0], A[:, 1], A[:, 2]]
         b = [B[:, 0], B[:, 1], B[:, 2]]
-        h = np.zeros(pr.shape[0], dtype=bool)
+        h = xp.zeros_bool(pr.shape[0])
         for i in range(3):
-            h |= _segment_pierces(a[i], a[(i + 1) % 3], b[0], b[1], b[2])
-            h |= _segment_pierces(b[i], b[(i + 1) % 3], a[0], a[1], a[2])
+            h = h | _segment_pierces(xp, a[i], a[(i + 1) % 3], b[0], b[1], b[2])
+            h = h | _segment_pierces(xp, b[i], b[(i + 1) % 3], a[0], a[1], a[2])
         # degeneracy measures
         ea = [a[1] - a[0], a[2] - a[1], a[0] - a[2]]
         eb = [b[1] - b[0], b[2] - b[1], b[0] - b[2]]
-        L = sum(np.linalg.norm(e, axis=-1) for e in ea + eb) / 6.0
-        na = _cross(a[1] - a[0], a[2] - a[0])
-        nb = _cross(b[1] - b[0], b[2] - b[0])
-        lna = np.linalg.norm(na, axis=-1)
-        lnb = np.linalg.norm(nb, axis=-1)
-        tiny = np.finfo(np.float64).tiny
+        L = sum(xp.norm(e) for e in ea + eb) / 6.0
+        na = _cross(xp, a[1] - a[0], a[2] - a[0])
+        nb = _cross(xp, b[1] - b[0], b[2] - b[0])
+        lna = xp.norm(na)
+        lnb = xp.norm(nb)
         d = (lna <= tiny) | (lnb <= tiny)
-        lna = np.maximum(lna, tiny)
-        lnb = np.maximum(lnb, tiny)
+        lna = xp.maximum(lna, tiny)
+        lnb = xp.maximum(lnb, tiny)
         for m in range(3):
-            d |= np.abs(_dot(nb, a[m] - b[0])) / lnb < eps * L
-            d |= np.abs(_dot(na, b[m] - a[0])) / lna < eps * L
-        d |= np.linalg.norm(_cross(na, nb), axis=-1) < eps * lna * lnb
+            d = d | (xp.abs(_dot(nb, a[m] - b[0])) / lnb < eps * L)
+            d = d | (xp.abs(_dot(na, b[m] - a[0])) / lna < eps * L)
+        d = d | (xp.norm(_cross(xp, na, nb)) < eps * lna * lnb)
         for i in range(3):
             for j in range(3):
-                c = _cross(ea[i], eb[j])
-                lc = np.linalg.norm(c, axis=-1)
-                lei = np.linalg.norm(ea[i], axis=-1) * np.linalg.norm(eb[j], axis=-1)
+                c = _cross(xp, ea[i], eb[j])
+                lc = xp.norm(c)
+                lei = xp.norm(ea[i]) * xp.norm(eb[j])
                 par = lc < eps * lei                       # near-parallel edges: no line distance
-                dist = np.abs(_dot(c, b[j] - a[i])) / np.maximum(lc, tiny)
-                d |= (~par) & (dist < eps * L)
-        shared = (ta[:, :, None] == tb[:, None, :]).any(axis=(1, 2))
-        hit[lo:lo + chunk] = h & ~shared
-        deg[lo:lo + chunk] = d | shared
+                dist = xp.abs(_dot(c, b[j] - a[i])) / xp.maximum(lc, tiny)
+                d = d | ((~par) & (dist < eps * L))
+        shared = (ta[:, :, None] == tb[:, None, :]).any(-1).any(-1)
+        hit[lo:lo + chunk] = xp.to_numpy(h & ~shared)
+        deg[lo:lo + chunk] = xp.to_numpy(d | shared)
     return hit, deg
 
 
@@ -323,10 +367,12 @@ def config3_torus(nu=1000, nv=500, seed=BASE_SEED + 3, R=1.0, r=0.3, amp=0.25, i
     return _finish(pos, tris, pairs, "torus%dx%d" % (nu, nv), eps, dict(seed=seed, inflate=inflate))
 
 
-def config4_sweep(n_tris=2_000_000, n_pairs=10_000_000, seed=BASE_SEED + 4, frac_active=0.5, eps=1e-6):
+def config4_sweep(n_tris=2_000_000, n_pairs=10_000_000, seed=BASE_SEED + 4, frac_active=0.5, eps=1e-6,
+                  device=None):
     """Random soup (own vertices, uniform [0,1]^3) with seeded random distinct non-adjacent
     candidate pairs, accepted/rejected with the orientation classifier to `frac_active`
-    intersecting (the raw rate for uniform triangles is ~27.6 %).  Pair order is random."""
+    intersecting (the raw rate for uniform triangles is ~27.6 %).  Pair order is random.
+    device: None = numpy classifier; a torch device string runs the same classifier there."""
     rng = np.random.default_rng(seed)
     pos = rng.random((3 * n_tris, 3))
     tris = np.arange(3 * n_tris, dtype=np.int32).reshape(-1, 3)
@@ -341,7 +387,7 @@ def config4_sweep(n_tris=2_000_000, n_pairs=10_000_000, seed=BASE_SEED + 4, frac
         j = rng.integers(0, n_tris, n, dtype=np.int64)
         ok = i != j
         pr = np.stack([i[ok], j[ok]], 1).astype(np.int32)
-        h, d = classify_pairs(pos, tris, pr, eps)
+        h, d = classify_pairs(pos, tris, pr, eps, device=device)
         good = ~d
         ph = pr[good & h][:max(0, want_hit - nh)]
         pm = pr[good & ~h][:max(0, want_miss - nm)]

@@ -21,7 +21,7 @@ TT_HESS_EQ4, TT_HESS_FILTER, TT_HESS_PSD2 = 0, 1, 2
 TT_FLAG_FORCE_GENERAL_ROWS = 1
 
 EXPORTS = ["tt_create", "tt_destroy", "tt_energy", "tt_hess_symbolic", "tt_energy_grad_hess", "tt_hess_vec",
-           "tt_energy_grad_hess_host", "tt_bsr_device", "tt_stats", "tt_status_string", "tt_last_error"]
+           "tt_energy_grad_hess_host", "tt_bsr_device", "tt_stats", "tt_kernel_ms", "tt_status_string", "tt_last_error"]
 
 
 class TTOptions(ctypes.Structure):
@@ -66,12 +66,14 @@ def load_library():
     lib.tt_hess_vec.argtypes = [vp, ctypes.POINTER(TTProblem), vp, vp, vp]
     lib.tt_hess_vec.restype = ctypes.c_int
     lib.tt_energy_grad_hess_host.argtypes = [vp, ctypes.POINTER(TTProblem), vp, vp, ctypes.POINTER(i64),
-                                             ctypes.POINTER(i64), vp, vp, vp, i64, vp]
+                                             ctypes.POINTER(i64), vp, vp, vp, i64, vp, vp, vp]
     lib.tt_energy_grad_hess_host.restype = ctypes.c_int
     lib.tt_bsr_device.argtypes = [vp, ctypes.POINTER(vp), ctypes.POINTER(vp), ctypes.POINTER(vp), ctypes.POINTER(i64)]
     lib.tt_bsr_device.restype = ctypes.c_int
     lib.tt_stats.argtypes = [vp, ctypes.POINTER(i64), ctypes.c_int32]
     lib.tt_stats.restype = ctypes.c_int
+    lib.tt_kernel_ms.argtypes = [vp, ctypes.POINTER(ctypes.c_float), ctypes.c_int32]
+    lib.tt_kernel_ms.restype = ctypes.c_int
     lib.tt_status_string.argtypes = [ctypes.c_int]
     lib.tt_status_string.restype = ctypes.c_char_p
     lib.tt_last_error.argtypes = [vp]
@@ -154,7 +156,7 @@ class Context:
 
     # ---- tt_energy_grad_hess_host ----
     def tt_energy_grad_hess_host(self, pos_h, tris_h, pairs_h, energy_h, grad_h=None, rowptr_h=None, colind_h=None,
-                                 vals_h=None, nnzb_capacity=0, stream=None):
+                                 vals_h=None, nnzb_capacity=0, p_h=None, y_h=None, stream=None):
         """All tensors are HOST tensors (pinned recommended).  Returns (nnzb, n_active)."""
         for t in (pos_h, tris_h, pairs_h, energy_h):
             assert not t.is_cuda and t.is_contiguous()
@@ -164,8 +166,13 @@ class Context:
         self._check(self.lib.tt_energy_grad_hess_host(self.h, ctypes.byref(pb), _ptr(energy_h), _ptr(grad_h),
                                                       ctypes.byref(nnzb), ctypes.byref(na), _ptr(rowptr_h),
                                                       _ptr(colind_h), _ptr(vals_h), int(nnzb_capacity),
-                                                      _stream_ptr(stream)))
+                                                      _ptr(p_h), _ptr(y_h), _stream_ptr(stream)))
         return nnzb.value, na.value
+
+    def tt_kernel_ms(self):
+        arr = (ctypes.c_float * 3)()
+        self._check(self.lib.tt_kernel_ms(self.h, arr, 3))
+        return dict(classify=float(arr[0]), assemble=float(arr[1]), hess_vec=float(arr[2]))
 
     def tt_stats(self):
         arr = (ctypes.c_int64 * 8)()
