@@ -151,6 +151,12 @@ tt_status tt_stats(const tt_ctx* ctx, int64_t* what, int32_t n);
  * kernel has not run.  Blocks until those launches have finished.                                 */
 tt_status tt_kernel_ms(tt_ctx* ctx, float* ms, int32_t n);
 
+/* Diagnostic (not on the hot path): measured vector-FMA issue rate of `device`, FMA = 2 flop.
+ *   tflops HOST [2]: [0] = fp64 (DFMA), [1] = fp32 (FFMA).  Runs ~10 ms of register-only FMA
+ *   chains on the default stream and blocks until done.  bench.py reports it beside the derived
+ *   ALU peak.                                                              */
+tt_status tt_probe_peaks(int32_t device, double* tflops);
+
 const char* tt_status_string(tt_status s);
 const char* tt_last_error(const tt_ctx* ctx);
 

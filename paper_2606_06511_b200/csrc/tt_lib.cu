@@ -11,6 +11,7 @@
 
 #include "../../include/tt.h"
 #include "tt_kernels.cuh"
+#include "tt_probe.cuh"
 
 namespace {
 
@@ -695,6 +696,14 @@ tt_status tt_kernel_ms(tt_ctx* ctx, float* ms, int32_t n) {
     TT_CUDA(cudaEventElapsedTime(&ms[i], ctx->ev[i][0], ctx->ev[i][1]));
   }
   return TT_OK;
+}
+
+tt_status tt_probe_peaks(int32_t device, double* tflops) {
+  if (!tflops) return TT_ERR_INVALID_ARG;
+  if (cudaSetDevice(device) != cudaSuccess) { (void)cudaGetLastError(); return TT_ERR_CUDA; }
+  tflops[0] = ttp::fma_tflops<double>(nullptr);
+  tflops[1] = ttp::fma_tflops<float>(nullptr);
+  return (tflops[0] > 0.0 && tflops[1] > 0.0) ? TT_OK : TT_ERR_CUDA;
 }
 
 const char* tt_status_string(tt_status s) {

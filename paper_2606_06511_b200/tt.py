@@ -21,7 +21,7 @@ TT_HESS_EQ4, TT_HESS_FILTER, TT_HESS_PSD2 = 0, 1, 2
 TT_FLAG_FORCE_GENERAL_ROWS = 1
 
 EXPORTS = ["tt_create", "tt_destroy", "tt_energy", "tt_hess_symbolic", "tt_energy_grad_hess", "tt_hess_vec",
-           "tt_energy_grad_hess_host", "tt_bsr_device", "tt_stats", "tt_kernel_ms", "tt_status_string", "tt_last_error"]
+           "tt_energy_grad_hess_host", "tt_bsr_device", "tt_stats", "tt_kernel_ms", "tt_probe_peaks", "tt_status_string", "tt_last_error"]
 
 
 class TTOptions(ctypes.Structure):
@@ -74,6 +74,8 @@ def load_library():
     lib.tt_stats.restype = ctypes.c_int
     lib.tt_kernel_ms.argtypes = [vp, ctypes.POINTER(ctypes.c_float), ctypes.c_int32]
     lib.tt_kernel_ms.restype = ctypes.c_int
+    lib.tt_probe_peaks.argtypes = [ctypes.c_int32, ctypes.POINTER(ctypes.c_double)]
+    lib.tt_probe_peaks.restype = ctypes.c_int
     lib.tt_status_string.argtypes = [ctypes.c_int]
     lib.tt_status_string.restype = ctypes.c_char_p
     lib.tt_last_error.argtypes = [vp]
@@ -180,6 +182,18 @@ class Context:
         keys = ["n_active", "n_directed", "n_touched_tris", "blocks_direct", "blocks_merged", "merge_records", "nnzb",
                 "launches"]
         return dict(zip(keys, [int(v) for v in arr]))
+
+
+def tt_probe_peaks(device=0):
+    """Measured DFMA / FFMA rate of `device` in TFLOP/s (diagnostic)."""
+    if not torch.cuda.is_available():
+        raise RuntimeError("paper_2606_06511_b200 needs a CUDA device (no CPU fallback)")
+    lib = load_library()
+    arr = (ctypes.c_double * 2)()
+    st = lib.tt_probe_peaks(int(device), arr)
+    if st != TT_OK:
+        raise TTError(st, lib.tt_status_string(st).decode(), "tt_probe_peaks failed")
+    return dict(fp64_tflops=float(arr[0]), fp32_tflops=float(arr[1]))
 
 
 def assemble(ctx: Context, pos, tris, pairs, want_hess=True, stream=None):
