@@ -5,12 +5,14 @@
 //   K2  k_compact       a2'    : order-preserving compaction of active pair ids (ballot/popc)
 //   K3* symbolic kernels a4    : directed (triangle -> partner) entries, per-triangle column
 //                                ranks, exclusive-row detection, general-row merge records
-//   K4  k_assemble      a3+a4  : triangle-centric numeric phase, one thread per directed entry:
-//                                recompute J analytically, write the 9 off-diagonal 3x3 blocks
-//                                once, reduce diagonal blocks + gradient inside the CTA in fixed
-//                                order (no atomics)
+//   K4  k_assemble_tile a3+a4  : triangle-centric numeric phase, one lane per directed entry, one
+//                                warp per round of whole triangles: recompute J analytically,
+//                                build each row's run of 3x3 blocks in a shared-memory tile,
+//                                sum diagonal rows + gradient in fixed order (no atomics), write
+//                                the runs out with TMA bulk copies (k_assemble_long: triangles
+//                                with more than 32 partners)
 //   K5  k_merge / k_gather3    : general rows (vertices shared by several touched triangles)
-//   K6  k_hessvec       a5     : matrix-free H.p with the same decomposition
+//   K6  k_entry_reduce  a5     : matrix-free H.p (and the gradient-only call), same rounds
 #pragma once
 #include <cstdint>
 #include <cuda_runtime.h>
@@ -21,8 +23,6 @@ namespace ttk {
 using ttg::d3;
 
 constexpr int CLS_THREADS = 256;   // K1 / K2 CTA size (8 warps -> 8 mask words per CTA)
-constexpr int ASM_THREADS = 128;   // K4 / K6 CTA size: 4 independent warps
-constexpr int ASM_CHUNK = 32;      // directed entries per warp chunk (snapped to triangle boundaries)
 constexpr int SYM_WARPS = 4;       // warps per CTA in the per-triangle symbolic kernels
 constexpr int SYM_LMAX = 1536;     // longest row (in blocks) ranked in shared memory
 
@@ -354,19 +354,61 @@ k_fill_rows(const int* __restrict__ tris, const int* __restrict__ touched, int64
   }
 }
 
-// Work partition of K4/K6: chunk c owns the triangles whose first directed entry lies in
-// [c*ASM_CHUNK, (c+1)*ASM_CHUNK): chunk_tri[c] = first such triangle (binary search in tptr).
-__global__ void k_chunk_bounds(const int* __restrict__ tptr, int64_t nT, int64_t n_chunks,
-                               int* __restrict__ chunk_tri) {
-  const int64_t c = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
-  if (c > n_chunks) return;
-  const int64_t target = c * ASM_CHUNK;
-  int64_t lo = 0, hi = nT;  // first s in [0,nT] with tptr[s] >= target
-  while (lo < hi) {
-    const int64_t mid = (lo + hi) >> 1;
-    if (tptr[mid] >= target) hi = mid; else lo = mid + 1;
+// Work partition of K4/K6.  A ROUND is a run of consecutive touched triangles, kept whole, with at
+// most RND_MAX_ENT directed entries (one lane each) and RND_MAX_TRI triangles; one warp owns one
+// round.  A triangle with more than RND_MAX_ENT partners is a round of its own ("long": no smem
+// tile can hold its rows; K4 hands it to k_assemble_long).  Packing is greedy in touched order,
+// restarted at every bucket of CHK_BUCKET touched triangles so that buckets pack in parallel
+// (one thread per bucket; count pass, scan, fill pass).
+constexpr int RND_MAX_ENT = 32;
+constexpr int RND_MAX_TRI = 16;
+constexpr int CHK_BUCKET = 128;
+
+// tfirst[i] = first directed entry of touched triangle i; tfirst[n_touched] = n_dir
+__global__ void k_touched_first(const int* __restrict__ touched, int64_t n_touched, const int* __restrict__ tptr,
+                                int64_t n_dir, int* __restrict__ tfirst) {
+  const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (i < n_touched) tfirst[i] = tptr[touched[i]];
+  if (i == n_touched) tfirst[i] = (int)n_dir;
+}
+
+// FILL = false: bucket_cnt[b] = rounds of bucket b (+ long_cnt[b] = long triangles).
+// FILL = true : chunk_start[bucket_off[b] + k] = first touched index of the k-th round of bucket b,
+//               long_list[long_off[b] + k] = round id of the k-th long triangle.
+template <bool FILL>
+__global__ void k_chunk_pack(const int* __restrict__ tfirst, int64_t n_touched, int64_t n_buckets,
+                             int* __restrict__ bucket_cnt, int* __restrict__ long_cnt,
+                             const int* __restrict__ bucket_off, const int* __restrict__ long_off,
+                             int* __restrict__ chunk_start, int* __restrict__ long_list) {
+  const int64_t b = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (b >= n_buckets) return;
+  const int64_t i0 = b * CHK_BUCKET, i1 = min(i0 + (int64_t)CHK_BUCKET, n_touched);
+  int nch = 0, nlong = 0, ent = 0, tri = 0;
+  const int cbase = FILL ? bucket_off[b] : 0, lbase = FILL ? long_off[b] : 0;
+  int e_prev = tfirst[i0];
+  for (int64_t i = i0; i < i1; ++i) {
+    const int e_next = tfirst[i + 1];
+    const int d = e_next - e_prev;
+    e_prev = e_next;
+    const bool is_long = d > RND_MAX_ENT;
+    if (tri == 0 || is_long || ent + d > RND_MAX_ENT || tri + 1 > RND_MAX_TRI) {  // open a new round at i
+      if (FILL) chunk_start[cbase + nch] = (int)i;
+      if (is_long) {
+        if (FILL) long_list[lbase + nlong] = cbase + nch;
+        ++nlong;
+      }
+      ++nch;
+      ent = 0;
+      tri = 0;
+    }
+    ent += d;
+    tri += 1;
+    if (is_long) tri = RND_MAX_TRI;  // closes the round: the next triangle opens a new one
   }
-  chunk_tri[c] = (int)lo;
+  if (!FILL) {
+    bucket_cnt[b] = nch;
+    long_cnt[b] = nlong;
+  }
 }
 
 // vertex -> touched (triangle, slot) incidence keys: key = vertex, payload = 3s+m
@@ -382,24 +424,29 @@ __global__ void k_emit_vslots(const int* __restrict__ tris, const int* __restric
 }
 
 // ------------------------------------------------------------------------------------------ K4
-// Triangle-centric numeric phase.  MODE 0: energy + gradient + Hessian blocks.  MODE 1: energy +
-// gradient only.  MODE 2: H.p (K6).  One LANE per directed entry e = (source s -> partner t); one
-// WARP per chunk of ~32 entries that starts and ends on a triangle boundary, so a warp owns every
-// entry of the triangles it touches and needs no block-level barrier and no atomics.
-// The pair is always evaluated in its canonical order (T_a = pairs[k,0]) so that both directed
-// copies of a pair compute bit-identical J and take the same FILTER decision.
+// Triangle-centric numeric phase.  One LANE per directed entry e = (source s -> partner t); one
+// WARP per round (whole triangles, <= 32 entries), warps fully independent (no __syncthreads, no
+// atomics).  The pair is always evaluated in its canonical order (T_a = pairs[k,0]) so that both
+// directed copies of a pair compute bit-identical J and take the same FILTER decision.
 //
-// Per entry the lane forms, with w0 = c00 g0 + c01 g1 and w1 = c01 g0 + c11 g1,
-//   off-diagonal blocks  H[p_m, q_n] = g0_pm w0_qn^T + g1_pm w1_qn^T   (q_n = partner vertices):
-//     exactly one contribution each -> staged through shared memory row by row and written out
-//     by the whole warp in address order (coalesced) to their final place;
-//   the diagonal 9x9 contribution (symmetric: 45 unique values) and the 9 gradient / H.p values:
-//     staged in shared memory, then summed over the triangle's entries with lane = component,
-//     entries in order (deterministic), accumulators carried in registers across rounds.
-constexpr int NDIAG = 45;                 // upper triangle of the symmetric 9x9 diagonal block
-constexpr int NRED_FULL = NDIAG + 9;      // + gradient of the three own vertices
-constexpr int RED_STRIDE = 55;            // odd: conflict-free lane = entry writes
-constexpr int OUT_STRIDE = 27;            // odd: conflict-free lane = entry writes
+// k_assemble_tile (energy + gradient + Hessian blocks).  Row m of triangle s (vertex p_m) owns ONE
+// contiguous run of L = 3 (deg + 1) blocks in its destination (vals for exclusive rows, the merge
+// workspace otherwise).  For m = 0, 1, 2 the warp builds the runs of all its triangles for that
+// row in a shared-memory tile laid out exactly like global memory,
+//   off-diagonal block (p_m, q_n), one contribution:  a g0_q^T + b g1_q^T,
+//       a = c00 g0_pm + c01 g1_pm,  b = c01 g0_pm + c11 g1_pm            (M symmetric),
+//   diagonal-row blocks (p_m, p_n) and the gradient of p_m: staged per entry, summed over the
+//       triangle's entries with lane = component in entry order (deterministic),
+// and hands every run to the TMA engine (cp.async.bulk shared -> global, 16-byte aligned body;
+// the <= 15 unaligned head / tail bytes by plain stores).  Address generation and full-line
+// writes are the copy engine's; the SM issues ~60 shared stores per entry and row.
+struct Entry {
+  double g0[18], g1[18];   // own triangle's 9 DOF first, partner's 9 after
+  ttg::Coefs cf;
+  double en;               // Eq. 2 energy if this is the canonical copy (side 0), else 0
+  int s;                   // source triangle
+  int va[3], vb[3];        // vertex ids of (own, partner)
+};
 
 template <typename T>
 struct AsmParams {
@@ -407,215 +454,374 @@ struct AsmParams {
   const int* tris;
   const uint64_t* keys;     // sorted directed keys (source << bitsT | partner)
   const uint32_t* dvals;    // 2k + side
-  const int* tptr;          // [nT+1]
-  const int* chunk_tri;     // [n_chunks+1]
+  const int* touched;       // [n_touched]
+  const int* tfirst;        // [n_touched+1]
+  const int* chunk_start;   // [n_chunks+1] first touched index of every round
+  const int* long_list;     // [n_long] round ids of the long triangles
   const int* erank;         // [2A][3]
   const int* drank;         // [nT][3]
   const int64_t* rowbase;   // [3nT]
   T* vals;                  // final BSR values
   T* tvals;                 // merge workspace values
-  T* tslot;                 // [3nT][3] per-slot gradient (MODE 0/1) or H.p (MODE 2) partials
+  T* tslot;                 // [3nT][3] per-slot gradient (K4) or H.p (K6) partials
   double* chunk_energy;     // [n_chunks]
-  const T* pvec;            // MODE 2: p [nV,3]
+  const T* pvec;            // K6: p [nV,3]
   int64_t n_chunks;
+  int64_t n_long;
   int bitsT;
   int hess_mode;
   double sigma;
 };
 
-struct AsmWarpSmem {
-  double red[32 * RED_STRIDE];
-  double out[32 * OUT_STRIDE];
-  unsigned long long rowp[3][32];   // destination row base (element pointer) per entry and row
-  int er[32][3];
-  int src[32];
+// Evaluates directed entry e: canonical pair, J, coefficients; swaps halves so that "own" is first.
+template <typename T>
+__device__ __forceinline__ void eval_entry(const AsmParams<T>& P, int e, Entry& E) {
+  const uint64_t key = __ldg(P.keys + e);
+  const uint64_t tmask = (1ull << P.bitsT) - 1ull;
+  E.s = (int)(key >> P.bitsT);
+  const int t = (int)(key & tmask);
+  const int side = (int)(__ldg(P.dvals + e) & 1u);
+  const int2 pr = side ? make_int2(t, E.s) : make_int2(E.s, t);  // canonical (pairs[k,0], pairs[k,1])
+  int va[3], vb[3];
+  d3 a[3], b[3];
+  gather_pair(P.pos, P.tris, pr.x, pr.y, va, vb, a, b);
+  ttg::PairGeom q;
+  ttg::pair_intervals(a[0], a[1], a[2], b[0], b[1], b[2], P.sigma, q);  // active by construction
+  ttg::pair_derivs(a[0], a[1], a[2], b[0], b[1], b[2], P.sigma, q, E.g0, E.g1);
+  E.cf = ttg::pair_coefs(q.tc0, q.tc1, E.g0, E.g1, P.hess_mode);
+  const double tt = q.tc0 * q.tc1;
+  E.en = side ? 0.0 : tt * tt;  // Eq. 2, counted once per pair
+#pragma unroll
+  for (int m = 0; m < 3; ++m) {
+    E.va[m] = side ? vb[m] : va[m];
+    E.vb[m] = side ? va[m] : vb[m];
+  }
+  if (side) {
+#pragma unroll
+    for (int i = 0; i < 9; ++i) {
+      const double t0 = E.g0[i]; E.g0[i] = E.g0[9 + i]; E.g0[9 + i] = t0;
+      const double t1 = E.g1[i]; E.g1[i] = E.g1[9 + i]; E.g1[9 + i] = t1;
+    }
+  }
+}
+
+__device__ __forceinline__ void bulk_s2g(void* gdst, const void* ssrc, uint32_t bytes) {
+  asm volatile("cp.async.bulk.global.shared::cta.bulk_group [%0], [%1], %2;" ::"l"(gdst),
+               "r"((uint32_t)__cvta_generic_to_shared(ssrc)), "r"(bytes)
+               : "memory");
+}
+__device__ __forceinline__ void bulk_commit() { asm volatile("cp.async.bulk.commit_group;" ::: "memory"); }
+__device__ __forceinline__ void bulk_wait_read() { asm volatile("cp.async.bulk.wait_group.read 0;" ::: "memory"); }
+__device__ __forceinline__ void bulk_wait_all() { asm volatile("cp.async.bulk.wait_group 0;" ::: "memory"); }
+__device__ __forceinline__ void fence_async_smem() { asm volatile("fence.proxy.async.shared::cta;" ::: "memory"); }
+
+constexpr int TILE_WARPS = 2;             // warps per CTA (independent; sized by shared memory)
+constexpr int STG_STRIDE = 31;            // odd: lane = entry writes and lane = component reads conflict-free
+constexpr int NSTG = 30;                  // 27 diagonal-row values + 3 gradient values per entry and row
+
+template <typename T>
+struct TileCfg {
+  static constexpr int RUN_UNIT = 27 * (int)sizeof(T);  // bytes one entry (or the diagonal) adds to a row run
+  static constexpr int TILE_BYTES = RUN_UNIT * (RND_MAX_ENT + RND_MAX_TRI) + 32 * RND_MAX_TRI;
 };
 
-template <typename T, int MODE>
-__global__ void __launch_bounds__(ASM_THREADS)
-k_assemble(const AsmParams<T> P) {
+template <typename T>
+struct alignas(16) TileWarpSmem {
+  unsigned char tile[TileCfg<T>::TILE_BYTES];
+  double stage[32 * STG_STRIDE];
+  unsigned long long run_g[RND_MAX_TRI];  // global byte address of the triangle's run (current row)
+  int run_off[RND_MAX_TRI];               // its byte offset in the tile (same address mod 16)
+  int tri_first[RND_MAX_TRI + 1];         // first entry (lane) of every triangle of the round
+  int tri_id[RND_MAX_TRI];
+  int dr[RND_MAX_TRI][3];
+};
+
+template <typename T>
+__global__ void __launch_bounds__(32 * TILE_WARPS)
+k_assemble_tile(const AsmParams<T> P) {
   extern __shared__ __align__(16) unsigned char s_raw[];
+  constexpr unsigned FULL = 0xffffffffu;
+  constexpr int RUN_UNIT = TileCfg<T>::RUN_UNIT;
   const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-  AsmWarpSmem& S = reinterpret_cast<AsmWarpSmem*>(s_raw)[warp];
-  const int64_t c = (int64_t)blockIdx.x * (ASM_THREADS / 32) + warp;
-  if (c >= P.n_chunks) return;  // warps are independent: no __syncthreads below
-  const int tri_lo = P.chunk_tri[c], tri_hi = P.chunk_tri[c + 1];
-  const int e_lo = P.tptr[tri_lo], e_hi = P.tptr[tri_hi];
-  const uint64_t tmask = (1ull << P.bitsT) - 1ull;
-  constexpr int NRED = (MODE == 0) ? NRED_FULL : 9;
-  constexpr int GOFF = (MODE == 0) ? NDIAG : 0;  // first gradient / H.p component
+  TileWarpSmem<T>& S = reinterpret_cast<TileWarpSmem<T>*>(s_raw)[warp];
+  const int64_t c = (int64_t)blockIdx.x * TILE_WARPS + warp;
+  if (c >= P.n_chunks) return;
+  const int t_lo = __ldg(P.chunk_start + c), ntri = __ldg(P.chunk_start + c + 1) - t_lo;
 
-  // lane = component bookkeeping for the reduction: comp0 = lane, comp1 = lane + 32
-  int al0 = 0, be0 = 0, al1 = 0, be1 = 0;  // (alpha, beta) of the diagonal components
-  if (MODE == 0) {
-    int k = 0;
-    for (int a = 0; a < 9; ++a)
-      for (int b = a; b < 9; ++b, ++k) {
-        if (k == lane) { al0 = a; be0 = b; }
-        if (k == lane + 32) { al1 = a; be1 = b; }
-      }
+  // ---- lane = triangle: ids, entry ranges, row destinations, tile slots ----
+  int my_s = 0, my_e0 = 0, my_e1 = 0;
+  if (lane < ntri) {
+    my_s = __ldg(P.touched + t_lo + lane);
+    my_e0 = __ldg(P.tfirst + t_lo + lane);
+    my_e1 = __ldg(P.tfirst + t_lo + lane + 1);
   }
-  double acc0 = 0.0, acc1 = 0.0, e_acc = 0.0;
-  int cur = -1;
+  const int e_lo = __shfl_sync(FULL, my_e0, 0);
+  const int nent = __shfl_sync(FULL, my_e1, ntri - 1) - e_lo;
+  if (nent > RND_MAX_ENT) {  // long triangle: k_assemble_long's
+    if (lane == 0) P.chunk_energy[c] = 0.0;
+    return;
+  }
+  const int run_bytes = RUN_UNIT * (my_e1 - my_e0 + 1);
+  int slot_off = 0;
+  unsigned long long my_g[3] = {0ull, 0ull, 0ull};
+  {
+    int incl = (lane < ntri) ? (((run_bytes + 15) & ~15) + 16) : 0;
+    const int mine = incl;
+#pragma unroll
+    for (int o = 1; o < 32; o <<= 1) {
+      const int v = __shfl_up_sync(FULL, incl, o);
+      if (lane >= o) incl += v;
+    }
+    slot_off = incl - mine;
+  }
+  if (lane < ntri) {
+#pragma unroll
+    for (int m = 0; m < 3; ++m) {
+      const int64_t rb = __ldg(P.rowbase + 3 * (int64_t)my_s + m);
+      my_g[m] = (unsigned long long)((rb >= 0) ? (P.vals + 9 * rb) : (P.tvals + 9 * (-rb - 1)));
+      S.dr[lane][m] = __ldg(P.drank + 3 * (int64_t)my_s + m);
+    }
+    S.tri_first[lane] = my_e0 - e_lo;
+    S.tri_id[lane] = my_s;
+  }
+  if (lane == 0) S.tri_first[ntri] = nent;
 
-  auto flush = [&](int s) {
-    if (MODE == 0) {
-      const int64_t rb0 = P.rowbase[3 * (int64_t)s], rb1 = P.rowbase[3 * (int64_t)s + 1], rb2 = P.rowbase[3 * (int64_t)s + 2];
-      const int dr0 = P.drank[3 * (int64_t)s], dr1 = P.drank[3 * (int64_t)s + 1], dr2 = P.drank[3 * (int64_t)s + 2];
-      auto put = [&](int a, int b, double v) {  // D[a][b] and its mirror D[b][a]
-        const int m = a / 3, i = a - 3 * m, n = b / 3, j = b - 3 * n;
-        {
-          const int64_t rb = (m == 0) ? rb0 : (m == 1) ? rb1 : rb2;
-          const int dr = (n == 0) ? dr0 : (n == 1) ? dr1 : dr2;
-          T* rowp = (rb >= 0) ? (P.vals + 9 * rb) : (P.tvals + 9 * (-rb - 1));
-          rowp[9 * (int64_t)dr + 3 * i + j] = (T)v;
-        }
-        if (a != b) {
-          const int64_t rb = (n == 0) ? rb0 : (n == 1) ? rb1 : rb2;
-          const int dr = (m == 0) ? dr0 : (m == 1) ? dr1 : dr2;
-          T* rowp = (rb >= 0) ? (P.vals + 9 * rb) : (P.tvals + 9 * (-rb - 1));
-          rowp[9 * (int64_t)dr + 3 * j + i] = (T)v;
-        }
-      };
-      put(al0, be0, acc0);
-      if (lane + 32 < NDIAG) put(al1, be1, acc1);
-      else if (lane + 32 < NRED_FULL) P.tslot[9 * (int64_t)s + (lane + 32 - NDIAG)] = (T)acc1;
-    } else {
-      if (lane < 9) P.tslot[9 * (int64_t)s + lane] = (T)acc0;
-    }
-  };
+  // ---- lane = entry: J, coefficients ----
+  const bool valid = lane < nent;
+  Entry E;
+#pragma unroll
+  for (int i = 0; i < 18; ++i) { E.g0[i] = 0.0; E.g1[i] = 0.0; }
+  E.cf = {0, 0, 0, 0, 0};
+  E.en = 0.0;
+  E.s = -1;
+  int er[3] = {0, 0, 0};
+  if (valid) {
+    eval_entry(P, e_lo + lane, E);
+#pragma unroll
+    for (int n = 0; n < 3; ++n) er[n] = __ldg(P.erank + 3 * (int64_t)(e_lo + lane) + n);
+  }
+  int ti;
+  {
+    const int s_prev = __shfl_up_sync(FULL, E.s, 1);
+    const unsigned heads = __ballot_sync(FULL, valid && (lane == 0 || E.s != s_prev));
+    ti = __popc(heads & (0xffffffffu >> (31 - lane))) - 1;
+  }
+  const int cn = (lane < 27) ? lane / 9 : 0, cq = (lane < 27) ? lane % 9 : 0;
 
-  for (int base = e_lo; base < e_hi; base += 32) {
-    const int e = base + lane;
-    const bool valid = e < e_hi;
-    const int nvalid = min(32, e_hi - base);
-    int s = -1;
-    double g0[18], g1[18];
-    ttg::Coefs cf = {0, 0, 0, 0, 0};
-    double hp0 = 0.0, hp1 = 0.0;  // MODE 2: M (J p_loc)
 #pragma unroll
-    for (int i = 0; i < 18; ++i) { g0[i] = 0.0; g1[i] = 0.0; }
-    if (valid) {
-      const uint64_t key = P.keys[e];
-      s = (int)(key >> P.bitsT);
-      const int side = (int)(P.dvals[e] & 1u);
-      const int t = (int)(key & tmask);
-      const int2 pr = side ? make_int2(t, s) : make_int2(s, t);  // canonical (pairs[k,0], pairs[k,1])
-      int va[3], vb[3];
-      d3 a[3], b[3];
-      gather_pair(P.pos, P.tris, pr.x, pr.y, va, vb, a, b);
-      ttg::PairGeom q;
-      ttg::pair_intervals(a[0], a[1], a[2], b[0], b[1], b[2], P.sigma, q);  // active by construction
-      ttg::pair_derivs(a[0], a[1], a[2], b[0], b[1], b[2], P.sigma, q, g0, g1);
-      cf = ttg::pair_coefs(q.tc0, q.tc1, g0, g1, P.hess_mode);
-      if (side == 0) {
-        const double tt = q.tc0 * q.tc1;
-        e_acc += tt * tt;  // Eq. 2, counted once per pair
-      }
-      if (MODE == 2) {
-        double j0 = 0.0, j1 = 0.0;
-#pragma unroll
-        for (int v = 0; v < 3; ++v) {
-          const d3 pa = load_vertex(P.pvec, va[v]);
-          const d3 pb = load_vertex(P.pvec, vb[v]);
-          j0 += g0[3 * v] * pa.x + g0[3 * v + 1] * pa.y + g0[3 * v + 2] * pa.z;
-          j0 += g0[9 + 3 * v] * pb.x + g0[9 + 3 * v + 1] * pb.y + g0[9 + 3 * v + 2] * pb.z;
-          j1 += g1[3 * v] * pa.x + g1[3 * v + 1] * pa.y + g1[3 * v + 2] * pa.z;
-          j1 += g1[9 + 3 * v] * pb.x + g1[9 + 3 * v + 1] * pb.y + g1[9 + 3 * v + 2] * pb.z;
-        }
-        hp0 = cf.c00 * j0 + cf.c01 * j1;
-        hp1 = cf.c01 * j0 + cf.c11 * j1;
-      }
-      if (side) {  // make "own" = first nine entries: swap the halves of g0, g1
-#pragma unroll
-        for (int i = 0; i < 9; ++i) {
-          double t0 = g0[i]; g0[i] = g0[9 + i]; g0[9 + i] = t0;
-          double t1 = g1[i]; g1[i] = g1[9 + i]; g1[9 + i] = t1;
-        }
-      }
-    }
-    // ---- stage the values to be reduced over the triangle: lane = entry ----
-    S.src[lane] = s;
-    {
-      double* red = S.red + lane * RED_STRIDE;
-      if (MODE == 0) {
-        double d0[9], d1[9];
-#pragma unroll
-        for (int i = 0; i < 9; ++i) {
-          d0[i] = cf.c00 * g0[i] + cf.c01 * g1[i];
-          d1[i] = cf.c01 * g0[i] + cf.c11 * g1[i];
-        }
-        int k = 0;
-#pragma unroll
-        for (int a = 0; a < 9; ++a)
-#pragma unroll
-          for (int b = a; b < 9; ++b, ++k) red[k] = g0[a] * d0[b] + g1[a] * d1[b];
-      }
-#pragma unroll
-      for (int i = 0; i < 9; ++i)
-        red[GOFF + i] = (MODE == 2) ? (hp0 * g0[i] + hp1 * g1[i]) : (cf.cg0 * g0[i] + cf.cg1 * g1[i]);
-    }
-    if (MODE == 0) {
-#pragma unroll
-      for (int m = 0; m < 3; ++m) {
-        unsigned long long ptr = 0ull;
-        if (valid) {
-          const int64_t rb = P.rowbase[3 * (int64_t)s + m];
-          ptr = (unsigned long long)((rb >= 0) ? (P.vals + 9 * rb) : (P.tvals + 9 * (-rb - 1)));
-          S.er[lane][m] = P.erank[3 * (int64_t)e + m];
-        }
-        S.rowp[m][lane] = ptr;
-      }
+  for (int m = 0; m < 3; ++m) {
+    // the tile is single-buffered: the copy engine must have read the previous row's runs
+    bulk_wait_read();
+    __syncwarp();
+    if (lane < ntri) {
+      S.run_g[lane] = my_g[m];
+      S.run_off[lane] = slot_off + (int)(my_g[m] & 15ull);
     }
     __syncwarp();
-    // ---- reduction over entries, lane = component, fixed order ----
-    for (int i = 0; i < nvalid; ++i) {
-      const int si = S.src[i];
-      if (si != cur) {  // warp-uniform
-        if (cur >= 0) flush(cur);
-        acc0 = 0.0;
-        acc1 = 0.0;
-        cur = si;
+    if (valid) {
+      const double g0m[3] = {E.g0[3 * m], E.g0[3 * m + 1], E.g0[3 * m + 2]};
+      const double g1m[3] = {E.g1[3 * m], E.g1[3 * m + 1], E.g1[3 * m + 2]};
+      double a[3], b[3];
+#pragma unroll
+      for (int i = 0; i < 3; ++i) {
+        a[i] = E.cf.c00 * g0m[i] + E.cf.c01 * g1m[i];
+        b[i] = E.cf.c01 * g0m[i] + E.cf.c11 * g1m[i];
       }
-      if (lane < NRED) acc0 += S.red[i * RED_STRIDE + lane];
-      if (NRED > 32 && lane + 32 < NRED) acc1 += S.red[i * RED_STRIDE + lane + 32];
+      T* run = reinterpret_cast<T*>(S.tile + S.run_off[ti]);
+#pragma unroll
+      for (int n = 0; n < 3; ++n) {
+        T* blk = run + 9 * er[n];
+#pragma unroll
+        for (int i = 0; i < 3; ++i)
+#pragma unroll
+          for (int j = 0; j < 3; ++j) blk[3 * i + j] = (T)(a[i] * E.g0[9 + 3 * n + j] + b[i] * E.g1[9 + 3 * n + j]);
+      }
+      double* st = S.stage + lane * STG_STRIDE;
+#pragma unroll
+      for (int n = 0; n < 3; ++n)
+#pragma unroll
+        for (int i = 0; i < 3; ++i)
+#pragma unroll
+          for (int j = 0; j < 3; ++j) st[9 * n + 3 * i + j] = a[i] * E.g0[3 * n + j] + b[i] * E.g1[3 * n + j];
+#pragma unroll
+      for (int i = 0; i < 3; ++i) st[27 + i] = E.cf.cg0 * g0m[i] + E.cf.cg1 * g1m[i];
     }
-    // ---- off-diagonal blocks, one row of the source triangle at a time ----
-    if (MODE == 0) {
-      double w0[9], w1[9];  // partner side: entries 9..17
-#pragma unroll
-      for (int i = 0; i < 9; ++i) {
-        w0[i] = cf.c00 * g0[9 + i] + cf.c01 * g1[9 + i];
-        w1[i] = cf.c01 * g0[9 + i] + cf.c11 * g1[9 + i];
+    __syncwarp();
+    // ---- sum over each triangle's entries, lane = component, entry order ----
+    if (lane < NSTG) {
+      for (int tt = 0; tt < ntri; ++tt) {
+        const int i0 = S.tri_first[tt], i1 = S.tri_first[tt + 1];
+        double acc = 0.0;
+        for (int i = i0; i < i1; ++i) acc += S.stage[i * STG_STRIDE + lane];
+        if (lane < 27) reinterpret_cast<T*>(S.tile + S.run_off[tt])[9 * S.dr[tt][cn] + cq] = (T)acc;
+        else P.tslot[9 * (int64_t)S.tri_id[tt] + 3 * m + (lane - 27)] = (T)acc;
       }
+    }
+    fence_async_smem();
+    __syncwarp();
+    // ---- lane = triangle: hand the run to the copy engine ----
+    if (lane < ntri) {
+      const unsigned long long g = my_g[m];
+      const unsigned char* src = S.tile + slot_off + (int)(g & 15ull);
+      int head = (int)((16ull - (g & 15ull)) & 15ull);
+      head = min(head, run_bytes);
+      const int body = (run_bytes - head) & ~15;
+      for (int o = 0; o < head; o += (int)sizeof(T)) *reinterpret_cast<T*>(g + o) = *reinterpret_cast<const T*>(src + o);
+      if (body > 0) bulk_s2g(reinterpret_cast<void*>(g + head), src + head, (uint32_t)body);
+      for (int o = head + body; o < run_bytes; o += (int)sizeof(T))
+        *reinterpret_cast<T*>(g + o) = *reinterpret_cast<const T*>(src + o);
+      bulk_commit();
+    }
+  }
+  double e_acc = E.en;
 #pragma unroll
-      for (int m = 0; m < 3; ++m) {
-        double* o = S.out + lane * OUT_STRIDE;
+  for (int o = 16; o > 0; o >>= 1) e_acc += __shfl_down_sync(FULL, e_acc, o);
+  if (lane == 0) P.chunk_energy[c] = e_acc;
+  bulk_wait_all();  // shared memory must outlive the engine's reads
+}
+
+// Long triangles (more than RND_MAX_ENT partners): one warp per triangle, entries in groups of 32,
+// off-diagonal blocks stored directly, diagonal rows and gradient carried across groups.
+template <typename T>
+__global__ void __launch_bounds__(32 * TILE_WARPS)
+k_assemble_long(const AsmParams<T> P) {
+  extern __shared__ __align__(16) unsigned char s_raw[];
+  constexpr unsigned FULL = 0xffffffffu;
+  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+  TileWarpSmem<T>& S = reinterpret_cast<TileWarpSmem<T>*>(s_raw)[warp];
+  const int64_t li = (int64_t)blockIdx.x * TILE_WARPS + warp;
+  if (li >= P.n_long) return;
+  const int c = __ldg(P.long_list + li);
+  const int ti = __ldg(P.chunk_start + c);
+  const int s = __ldg(P.touched + ti);
+  const int e_lo = __ldg(P.tfirst + ti), e_hi = __ldg(P.tfirst + ti + 1);
+  T* rowp[3];
+  int dr[3];
+#pragma unroll
+  for (int m = 0; m < 3; ++m) {
+    const int64_t rb = __ldg(P.rowbase + 3 * (int64_t)s + m);
+    rowp[m] = (rb >= 0) ? (P.vals + 9 * rb) : (P.tvals + 9 * (-rb - 1));
+    dr[m] = __ldg(P.drank + 3 * (int64_t)s + m);
+  }
+  const int cn = (lane < 27) ? lane / 9 : 0, cq = (lane < 27) ? lane % 9 : 0;
+  double acc[3] = {0.0, 0.0, 0.0}, e_acc = 0.0;
+  for (int base = e_lo; base < e_hi; base += 32) {
+    const int nvalid = min(32, e_hi - base);
+    const bool valid = lane < nvalid;
+    Entry E;
+    int er[3] = {0, 0, 0};
+    if (valid) {
+      eval_entry(P, base + lane, E);
+      e_acc += E.en;
+#pragma unroll
+      for (int n = 0; n < 3; ++n) er[n] = __ldg(P.erank + 3 * (int64_t)(base + lane) + n);
+    }
+#pragma unroll
+    for (int m = 0; m < 3; ++m) {
+      if (valid) {
+        double a[3], b[3];
+#pragma unroll
+        for (int i = 0; i < 3; ++i) {
+          a[i] = E.cf.c00 * E.g0[3 * m + i] + E.cf.c01 * E.g1[3 * m + i];
+          b[i] = E.cf.c01 * E.g0[3 * m + i] + E.cf.c11 * E.g1[3 * m + i];
+        }
+#pragma unroll
+        for (int n = 0; n < 3; ++n) {
+          T* blk = rowp[m] + 9 * (int64_t)er[n];
+#pragma unroll
+          for (int i = 0; i < 3; ++i)
+#pragma unroll
+            for (int j = 0; j < 3; ++j) blk[3 * i + j] = (T)(a[i] * E.g0[9 + 3 * n + j] + b[i] * E.g1[9 + 3 * n + j]);
+        }
+        double* st = S.stage + lane * STG_STRIDE;
 #pragma unroll
         for (int n = 0; n < 3; ++n)
 #pragma unroll
           for (int i = 0; i < 3; ++i)
 #pragma unroll
-            for (int j = 0; j < 3; ++j)
-              o[9 * n + 3 * i + j] = g0[3 * m + i] * w0[3 * n + j] + g1[3 * m + i] * w1[3 * n + j];
-        __syncwarp();
-        const int total = nvalid * 27;
-        for (int f = lane; f < total; f += 32) {
-          const int ee = f / 27, r = f - 27 * ee;
-          const int n = r / 9, q = r - 9 * n;
-          T* rowp = reinterpret_cast<T*>(S.rowp[m][ee]);
-          rowp[9 * (int64_t)S.er[ee][n] + q] = (T)S.out[f];
-        }
-        __syncwarp();
+            for (int j = 0; j < 3; ++j) st[9 * n + 3 * i + j] = a[i] * E.g0[3 * n + j] + b[i] * E.g1[3 * n + j];
+#pragma unroll
+        for (int i = 0; i < 3; ++i) st[27 + i] = E.cf.cg0 * E.g0[3 * m + i] + E.cf.cg1 * E.g1[3 * m + i];
       }
-    } else {
+      __syncwarp();
+      if (lane < NSTG)
+        for (int i = 0; i < nvalid; ++i) acc[m] += S.stage[i * STG_STRIDE + lane];
       __syncwarp();
     }
   }
-  if (cur >= 0) flush(cur);
-  if (MODE != 2) {
 #pragma unroll
-    for (int o = 16; o > 0; o >>= 1) e_acc += __shfl_down_sync(0xffffffffu, e_acc, o);
+  for (int m = 0; m < 3; ++m) {
+    if (lane < 27) rowp[m][9 * (int64_t)dr[cn] + cq] = (T)acc[m];
+    else if (lane < NSTG) P.tslot[9 * (int64_t)s + 3 * m + (lane - 27)] = (T)acc[m];
+  }
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) e_acc += __shfl_down_sync(FULL, e_acc, o);
+  if (lane == 0) P.chunk_energy[c] = e_acc;
+}
+
+// ------------------------------------------------------------------------------------------ K6
+// MODE 1: energy + gradient only.  MODE 2: matrix-free H.p:  y_s = sum_j (J^T M (J p_loc))_own.
+// Same rounds; a lane stages 9 values per entry, lane = component sums them per triangle in entry
+// order.  Long triangles simply take several groups of 32 entries.
+constexpr int RED_THREADS = 128;
+template <typename T, int MODE>
+__global__ void __launch_bounds__(RED_THREADS)
+k_entry_reduce(const AsmParams<T> P) {
+  __shared__ double s_stage[RED_THREADS / 32][32 * 9];
+  __shared__ int s_src[RED_THREADS / 32][32];
+  constexpr unsigned FULL = 0xffffffffu;
+  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+  const int64_t c = (int64_t)blockIdx.x * (RED_THREADS / 32) + warp;
+  if (c >= P.n_chunks) return;
+  const int t_lo = __ldg(P.chunk_start + c), t_hi = __ldg(P.chunk_start + c + 1);
+  const int e_lo = __ldg(P.tfirst + t_lo), e_hi = __ldg(P.tfirst + t_hi);
+  double* stage = s_stage[warp];
+  int* src = s_src[warp];
+  double acc = 0.0, e_acc = 0.0;
+  int cur = -1;
+  for (int base = e_lo; base < e_hi; base += 32) {
+    const int nvalid = min(32, e_hi - base);
+    int s = -1;
+    if (lane < nvalid) {
+      Entry E;
+      eval_entry(P, base + lane, E);
+      s = E.s;
+      e_acc += E.en;
+      double u0 = E.cf.cg0, u1 = E.cf.cg1;  // MODE 1: Eq. 3
+      if (MODE == 2) {
+        double j0 = 0.0, j1 = 0.0;
+#pragma unroll
+        for (int v = 0; v < 3; ++v) {
+          const d3 pa = load_vertex(P.pvec, E.va[v]);
+          const d3 pb = load_vertex(P.pvec, E.vb[v]);
+          j0 += E.g0[3 * v] * pa.x + E.g0[3 * v + 1] * pa.y + E.g0[3 * v + 2] * pa.z;
+          j0 += E.g0[9 + 3 * v] * pb.x + E.g0[9 + 3 * v + 1] * pb.y + E.g0[9 + 3 * v + 2] * pb.z;
+          j1 += E.g1[3 * v] * pa.x + E.g1[3 * v + 1] * pa.y + E.g1[3 * v + 2] * pa.z;
+          j1 += E.g1[9 + 3 * v] * pb.x + E.g1[9 + 3 * v + 1] * pb.y + E.g1[9 + 3 * v + 2] * pb.z;
+        }
+        u0 = E.cf.c00 * j0 + E.cf.c01 * j1;  // M (J p_loc)
+        u1 = E.cf.c01 * j0 + E.cf.c11 * j1;
+      }
+#pragma unroll
+      for (int i = 0; i < 9; ++i) stage[lane * 9 + i] = u0 * E.g0[i] + u1 * E.g1[i];
+    }
+    src[lane] = s;
+    __syncwarp();
+    for (int i = 0; i < nvalid; ++i) {
+      const int si = src[i];
+      if (si != cur) {  // warp-uniform
+        if (cur >= 0 && lane < 9) P.tslot[9 * (int64_t)cur + lane] = (T)acc;
+        acc = 0.0;
+        cur = si;
+      }
+      if (lane < 9) acc += stage[i * 9 + lane];
+    }
+    __syncwarp();
+  }
+  if (cur >= 0 && lane < 9) P.tslot[9 * (int64_t)cur + lane] = (T)acc;
+  if (MODE == 1) {
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) e_acc += __shfl_down_sync(FULL, e_acc, o);
     if (lane == 0) P.chunk_energy[c] = e_acc;
   }
 }

@@ -71,13 +71,13 @@ struct tt_ctx {
   // pattern
   DevBuf rowptr64, rowptr, colind;
   // numeric
-  DevBuf chunk_tri, asm_energy, tvals, tslot, vkeys[2], vvals[2], vptr;
+  DevBuf tfirst, bucket_cnt, bucket_off, long_cnt, long_off, chunk_start, long_list, asm_energy, tvals, tslot, vkeys[2], vvals[2], vptr;
   DevBuf cub_tmp;
   // host-API mirrors
   DevBuf h_pos, h_tris, h_pairs, h_p, o_vals, o_grad, o_energy, o_y;
   // cached symbolic state
   Signature sig;
-  int64_t A = 0, n_dir = 0, n_touched = 0, R = 0, U = 0, nnzb = 0, n_chunks = 0, rows_excl = 0, rows_gen = 0;
+  int64_t A = 0, n_dir = 0, n_touched = 0, R = 0, U = 0, nnzb = 0, n_chunks = 0, n_long = 0, rows_excl = 0, rows_gen = 0;
   int bitsT = 1, bitsV = 1;
   uint64_t* keys_sorted = nullptr;
   uint32_t* dvals_sorted = nullptr;
@@ -395,11 +395,46 @@ tt_status symbolic_impl(tt_ctx* ctx, const tt_problem* q, int64_t* nnzb_host, in
   }
 
   // ---- numeric-phase work partition, per-slot buffers, vertex -> slot incidence ----
-  const int64_t n_chunks = (n + ASM_CHUNK - 1) / ASM_CHUNK;
+  // rounds: greedy packing of whole touched triangles (<= 32 entries, <= 16 triangles per round)
+  int64_t n_chunks = 0, n_long = 0;
+  TT_CUDA(ctx->tfirst.ensure(sizeof(int) * (size_t)(n_touched + 2)));
+  TT_CUDA(ctx->chunk_start.ensure(sizeof(int) * (size_t)(n_touched + 2)));
+  TT_CUDA(ctx->long_list.ensure(sizeof(int) * (size_t)(n / (RND_MAX_ENT + 1) + 2)));
+  if (n_touched > 0) {
+    const int64_t n_buckets = (n_touched + CHK_BUCKET - 1) / CHK_BUCKET;
+    TT_CUDA(ctx->bucket_cnt.ensure(sizeof(int) * (size_t)(n_buckets + 1)));
+    TT_CUDA(ctx->bucket_off.ensure(sizeof(int) * (size_t)(n_buckets + 1)));
+    TT_CUDA(ctx->long_cnt.ensure(sizeof(int) * (size_t)(n_buckets + 1)));
+    TT_CUDA(ctx->long_off.ensure(sizeof(int) * (size_t)(n_buckets + 1)));
+    k_touched_first<<<grid_for(n_touched + 1, 256), 256, 0, st>>>(ctx->touched.as<int>(), n_touched, ctx->tptr.as<int>(), n,
+                                                                  ctx->tfirst.as<int>());
+    TT_LAUNCH_CHECK();
+    TT_CUDA(cudaMemsetAsync(ctx->bucket_cnt.as<int>() + n_buckets, 0, sizeof(int), st));
+    TT_CUDA(cudaMemsetAsync(ctx->long_cnt.as<int>() + n_buckets, 0, sizeof(int), st));
+    k_chunk_pack<false><<<grid_for(n_buckets, 128), 128, 0, st>>>(ctx->tfirst.as<int>(), n_touched, n_buckets,
+                                                                 ctx->bucket_cnt.as<int>(), ctx->long_cnt.as<int>(), nullptr,
+                                                                 nullptr, nullptr, nullptr);
+    TT_LAUNCH_CHECK();
+    s = scan_i32(ctx, ctx->bucket_cnt.as<int>(), ctx->bucket_off.as<int>(), n_buckets + 1, st);
+    if (s != TT_OK) return s;
+    s = scan_i32(ctx, ctx->long_cnt.as<int>(), ctx->long_off.as<int>(), n_buckets + 1, st);
+    if (s != TT_OK) return s;
+    k_chunk_pack<true><<<grid_for(n_buckets, 128), 128, 0, st>>>(ctx->tfirst.as<int>(), n_touched, n_buckets, nullptr, nullptr,
+                                                                ctx->bucket_off.as<int>(), ctx->long_off.as<int>(),
+                                                                ctx->chunk_start.as<int>(), ctx->long_list.as<int>());
+    TT_LAUNCH_CHECK();
+    int nc32[2] = {0, 0};
+    TT_CUDA(cudaMemcpyAsync(&nc32[0], ctx->bucket_off.as<int>() + n_buckets, sizeof(int), cudaMemcpyDeviceToHost, st));
+    TT_CUDA(cudaMemcpyAsync(&nc32[1], ctx->long_off.as<int>() + n_buckets, sizeof(int), cudaMemcpyDeviceToHost, st));
+    TT_CUDA(cudaStreamSynchronize(st));
+    n_chunks = nc32[0];
+    n_long = nc32[1];
+    const int nt32 = (int)n_touched;
+    TT_CUDA(cudaMemcpyAsync(ctx->chunk_start.as<int>() + n_chunks, &nt32, sizeof(int), cudaMemcpyHostToDevice, st));
+    TT_CUDA(cudaStreamSynchronize(st));  // nt32 lives on this stack frame
+  }
   ctx->n_chunks = n_chunks;
-  TT_CUDA(ctx->chunk_tri.ensure(sizeof(int) * (size_t)(n_chunks + 2)));
-  k_chunk_bounds<<<grid_for(n_chunks + 1, 256), 256, 0, st>>>(ctx->tptr.as<int>(), nT, n_chunks, ctx->chunk_tri.as<int>());
-  TT_LAUNCH_CHECK();
+  ctx->n_long = n_long;
   TT_CUDA(ctx->asm_energy.ensure(sizeof(double) * (size_t)(n_chunks + 1)));
   TT_CUDA(ctx->tvals.ensure(sizeof(T) * 9 * (size_t)(R + 1)));
   TT_CUDA(ctx->tslot.ensure(sizeof(T) * 9 * (size_t)(nT + 1)));
@@ -442,8 +477,10 @@ ttk::AsmParams<T> make_params(tt_ctx* ctx, const tt_problem* q) {
   p.tris = q->tris;
   p.keys = ctx->keys_sorted;
   p.dvals = ctx->dvals_sorted;
-  p.tptr = ctx->tptr.as<int>();
-  p.chunk_tri = ctx->chunk_tri.as<int>();
+  p.touched = ctx->touched.as<int>();
+  p.tfirst = ctx->tfirst.as<int>();
+  p.chunk_start = ctx->chunk_start.as<int>();
+  p.long_list = ctx->long_list.as<int>();
   p.erank = ctx->erank.as<int>();
   p.drank = ctx->drank.as<int>();
   p.rowbase = ctx->rowbase.as<int64_t>();
@@ -452,6 +489,7 @@ ttk::AsmParams<T> make_params(tt_ctx* ctx, const tt_problem* q) {
   p.tslot = ctx->tslot.as<T>();
   p.chunk_energy = ctx->asm_energy.as<double>();
   p.n_chunks = ctx->n_chunks;
+  p.n_long = ctx->n_long;
   p.pvec = nullptr;
   p.bitsT = ctx->bitsT;
   p.hess_mode = ctx->opt.hess_mode;
@@ -478,10 +516,16 @@ tt_status numeric_impl(tt_ctx* ctx, const tt_problem* q, void* energy_sum, void*
   p.vals = (T*)vals;
   if (ctx->n_chunks > 0) {
     TT_CUDA(cudaEventRecord(ctx->ev[1][0], st));
-    const unsigned grid = grid_for(ctx->n_chunks, ASM_THREADS / 32);
-    const size_t smem = sizeof(AsmWarpSmem) * (ASM_THREADS / 32);
-    if (want_h) k_assemble<T, 0><<<grid, ASM_THREADS, smem, st>>>(p);
-    else        k_assemble<T, 1><<<grid, ASM_THREADS, smem, st>>>(p);
+    if (want_h) {
+      const size_t smem = sizeof(TileWarpSmem<T>) * TILE_WARPS;
+      k_assemble_tile<T><<<grid_for(ctx->n_chunks, TILE_WARPS), 32 * TILE_WARPS, smem, st>>>(p);
+      if (ctx->n_long > 0) {
+        TT_LAUNCH_CHECK();
+        k_assemble_long<T><<<grid_for(ctx->n_long, TILE_WARPS), 32 * TILE_WARPS, smem, st>>>(p);
+      }
+    } else {
+      k_entry_reduce<T, 1><<<grid_for(ctx->n_chunks, RED_THREADS / 32), RED_THREADS, 0, st>>>(p);
+    }
     TT_LAUNCH_CHECK();
     TT_CUDA(cudaEventRecord(ctx->ev[1][1], st));
     ctx->ev_used[1] = true;
@@ -508,7 +552,7 @@ tt_status hessvec_impl(tt_ctx* ctx, const tt_problem* q, const void* pvec, void*
   p.chunk_energy = nullptr;
   if (ctx->n_chunks > 0) {
     TT_CUDA(cudaEventRecord(ctx->ev[2][0], st));
-    k_assemble<T, 2><<<grid_for(ctx->n_chunks, ASM_THREADS / 32), ASM_THREADS, sizeof(AsmWarpSmem) * (ASM_THREADS / 32), st>>>(p);
+    k_entry_reduce<T, 2><<<grid_for(ctx->n_chunks, RED_THREADS / 32), RED_THREADS, 0, st>>>(p);
     TT_LAUNCH_CHECK();
     TT_CUDA(cudaEventRecord(ctx->ev[2][1], st));
     ctx->ev_used[2] = true;
@@ -545,11 +589,12 @@ tt_status tt_create(const tt_options* opt, tt_ctx** out) {
     for (int j = 0; j < 2; ++j)
       if (cudaEventCreate(&c->ev[i][j]) != cudaSuccess) { delete c; return TT_ERR_CUDA; }
   {
-    const int smem = (int)(sizeof(ttk::AsmWarpSmem) * (ttk::ASM_THREADS / 32));
     cudaError_t e = cudaSuccess;
-    auto opt_in = [&](const void* f) { if (e == cudaSuccess) e = cudaFuncSetAttribute(f, cudaFuncAttributeMaxDynamicSharedMemorySize, smem); };
-    opt_in((const void*)ttk::k_assemble<double, 0>); opt_in((const void*)ttk::k_assemble<double, 1>); opt_in((const void*)ttk::k_assemble<double, 2>);
-    opt_in((const void*)ttk::k_assemble<float, 0>);  opt_in((const void*)ttk::k_assemble<float, 1>);  opt_in((const void*)ttk::k_assemble<float, 2>);
+    auto opt_in = [&](const void* f, size_t smem) { if (e == cudaSuccess) e = cudaFuncSetAttribute(f, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem); };
+    opt_in((const void*)ttk::k_assemble_tile<double>, sizeof(ttk::TileWarpSmem<double>) * ttk::TILE_WARPS);
+    opt_in((const void*)ttk::k_assemble_long<double>, sizeof(ttk::TileWarpSmem<double>) * ttk::TILE_WARPS);
+    opt_in((const void*)ttk::k_assemble_tile<float>, sizeof(ttk::TileWarpSmem<float>) * ttk::TILE_WARPS);
+    opt_in((const void*)ttk::k_assemble_long<float>, sizeof(ttk::TileWarpSmem<float>) * ttk::TILE_WARPS);
     if (e != cudaSuccess) { (void)cudaGetLastError(); delete c; return TT_ERR_CUDA; }
   }
   *out = c;
