@@ -126,52 +126,91 @@ __device__ __forceinline__ bool pair_intervals(const d3 a0, const d3 a1, const d
   return (ta1 > tb0) && (ta0 < tb1);  // L153, strict
 }
 
-// D^T dE for one end-point E = x_k + tau (x_i - x_k) of triangle X cut by plane(Y), added with
-// weight s into g[own..own+8] (the three vertices of X) and g[oth..oth+8] (those of Y).
-//   own blocks: (1-tau) D at x_k, tau D at x_i, plus c dtau/dx with c = D.(x_i - x_k),
-//               dtau/dx_i = d_k nY / den^2, dtau/dx_k = -d_i nY / den^2, den = d_k - d_i
-//   other blocks: dtau/dy1 = (y2-y0) x (E-y0) / den, dtau/dy2 = (E-y0) x (y1-y0) / den,
-//               y0 from translation invariance (all six blocks of D^T dE sum to D).
-template <int OWN, int OTH>
-__device__ __forceinline__ void add_endpoint(double (&g)[18], double s, const d3 Dh, const d3 x0,
-                                             const d3 x1, const d3 x2, const double (&d)[3], const d3 y0,
-                                             const d3 y1, const d3 y2, const d3 nY, int k, int i,
-                                             double tau) {
-  const d3 xk = sel3(k, x0, x1, x2), xi = sel3(i, x0, x1, x2);
-  const double dk = sel3(k, d[0], d[1], d[2]), di = sel3(i, d[0], d[1], d[2]);
-  const double inv = (k == i) ? 0.0 : 1.0 / (dk - di);
-  const d3 e = xi - xk;
-  const double w = s * dot(Dh, e) * inv;  // s * c / den
-  const double wn = w * inv;              // s * c / den^2
-#pragma unroll
-  for (int m = 0; m < 3; ++m) {
-    const double cd = s * (((m == k) ? (1.0 - tau) : 0.0) + ((m == i) ? tau : 0.0));
-    const double cn = wn * (((m == i) ? dk : 0.0) - ((m == k) ? di : 0.0));
-    g[OWN + 3 * m + 0] += fma(cd, Dh.x, cn * nY.x);
-    g[OWN + 3 * m + 1] += fma(cd, Dh.y, cn * nY.y);
-    g[OWN + 3 * m + 2] += fma(cd, Dh.z, cn * nY.z);
+// ---- recorded branch decisions ("record the computation graph") ----------------
+// K1 classifies every candidate with the generic code above and RECORDS, per active pair and per
+// triangle X, the discrete decisions of App. A in 6 bits:
+//   k (bits 0-1): the vertex both end-points hang off (the lone vertex, L96-105)
+//   p (bits 2-3): the other vertex of the edge carrying the end-point with the SMALLER t (L149-152);
+//                 q = 3 - k - p carries the larger one
+//   z (bits 4-5): 1 / 2 = the smaller / larger end-point is a vertex lying exactly on the other
+//                 plane (L106-115): it is then represented as the edge (k, p or q) with tau = 1
+//                 and d tau := 0, which is App. A's S0 = V_z
+// K4 / K6 permute the vertex IDS by (k, p, q) before gathering, so the derivative code below is
+// straight-line: no sign tests, no min/max, no selects on doubles.
+__device__ __forceinline__ unsigned cut_config(const Cut& c) {
+  unsigned k, p, q, z;
+  if (c.k[0] == c.i[0]) {         // smaller end-point is the on-plane vertex
+    z = 1u; k = (unsigned)c.k[1]; p = (unsigned)c.k[0]; q = (unsigned)c.i[1];
+  } else if (c.k[1] == c.i[1]) {  // larger end-point is the on-plane vertex
+    z = 2u; k = (unsigned)c.k[0]; p = (unsigned)c.i[0]; q = (unsigned)c.k[1];
+  } else {
+    z = 0u; k = (unsigned)c.k[0]; p = (unsigned)c.i[0]; q = (unsigned)c.i[1];
   }
-  const d3 u = axpy(tau, e, xk) - y0;  // E - y0
-  const d3 h1 = w * cross(y2 - y0, u);
-  const d3 h2 = w * cross(u, y1 - y0);
-  g[OTH + 3] += h1.x;  g[OTH + 4] += h1.y;  g[OTH + 5] += h1.z;
-  g[OTH + 6] += h2.x;  g[OTH + 7] += h2.y;  g[OTH + 8] += h2.z;
-  g[OTH + 0] -= fma(w, nY.x, h1.x + h2.x);
-  g[OTH + 1] -= fma(w, nY.y, h1.y + h2.y);
-  g[OTH + 2] -= fma(w, nY.z, h1.z + h2.z);
+  (void)q;
+  return k | (p << 2) | (z << 4);
+}
+__device__ __forceinline__ unsigned pair_config(const PairGeom& g) {
+  return cut_config(g.ca) | (cut_config(g.cb) << 6);
 }
 
-// Step a3, first half: g0 = d tc0/dx = sigma (D^T dP_min - D^T dQ_max),
-//                      g1 = d tc1/dx = sigma (D^T dP_max - D^T dQ_min),  x = [a0,a1,a2,b0,b1,b2].
-__device__ __forceinline__ void pair_derivs(const d3 a0, const d3 a1, const d3 a2, const d3 b0,
-                                            const d3 b1, const d3 b2, double sigma, const PairGeom& q,
-                                            double (&g0)[18], double (&g1)[18]) {
-#pragma unroll
-  for (int i = 0; i < 18; ++i) { g0[i] = 0.0; g1[i] = 0.0; }
-  add_endpoint<0, 9>(g0, sigma, q.Dh, a0, a1, a2, q.alpha, b0, b1, b2, q.nb, q.ca.k[0], q.ca.i[0], q.ca.tau[0]);
-  add_endpoint<9, 0>(g0, -sigma, q.Dh, b0, b1, b2, q.beta, a0, a1, a2, q.na, q.cb.k[1], q.cb.i[1], q.cb.tau[1]);
-  add_endpoint<0, 9>(g1, sigma, q.Dh, a0, a1, a2, q.alpha, b0, b1, b2, q.nb, q.ca.k[1], q.ca.i[1], q.ca.tau[1]);
-  add_endpoint<9, 0>(g1, -sigma, q.Dh, b0, b1, b2, q.beta, a0, a1, a2, q.na, q.cb.k[0], q.cb.i[0], q.cb.tau[0]);
+// One end-point E = x_k + tau (x_e - x_k) of triangle X = (x_k, x_p, x_q) cut by plane(Y), and the
+// blocks of  s * D^T dE  (s = +-sigma):
+//   own blocks: (1-tau) D at x_k, tau D at x_e, plus c dtau/dx with c = D.(x_e - x_k),
+//               dtau/dx_e = d_k nY / den^2, dtau/dx_k = -d_e nY / den^2, den = d_k - d_e
+//   other blocks: dtau/dy_p = (y_q - y_k) x (E - y_k) / den, dtau/dy_q = (E - y_k) x (y_p - y_k) / den,
+//               y_k from translation invariance (all six blocks of D^T dE sum to D).
+// nY = (y_p - y_k) x (y_q - y_k) and the distances d are taken with THAT normal, so the formulas hold
+// for any labelling (k, p, q) of Y (an odd one flips nY and d together).
+struct EndPoint {
+  double t;                    // D . E
+  d3 ownk, owne, yk, yp, yq;   // blocks of s D^T dE
+};
+__device__ __forceinline__ EndPoint end_point(double s, const d3 Dh, const d3 xk, const d3 ex, double dk,
+                                              double de, double zmask, const d3 yk, const d3 eyp,
+                                              const d3 eyq, const d3 nY) {
+  EndPoint r;
+  const double inv = 1.0 / (dk - de);  // opposite signs: |dk - de| = |dk| + |de|, no cancellation
+  const double tau = dk * inv;
+  const d3 E = axpy(tau, ex, xk);
+  r.t = dot(Dh, E);
+  const double w = s * zmask * dot(Dh, ex) * inv;  // s c / den
+  const double wn = w * inv;                       // s c / den^2
+  r.ownk = axpy(s * (1.0 - tau), Dh, (-(wn * de)) * nY);
+  r.owne = axpy(s * tau, Dh, (wn * dk) * nY);
+  const d3 u = E - yk;
+  r.yp = w * cross(eyq, u);
+  r.yq = w * cross(u, eyp);
+  r.yk = mk(-fma(w, nY.x, r.yp.x + r.yq.x), -fma(w, nY.y, r.yp.y + r.yq.y), -fma(w, nY.z, r.yp.z + r.yq.z));
+  return r;
+}
+
+// Step a3, first half, straight-line: both triangles arrive permuted to (k, p, q) as recorded.
+//   g0 = d tc0/dx = sigma (D^T dE(a,p) - D^T dE(b,q)),  g1 = d tc1/dx = sigma (D^T dE(a,q) - D^T dE(b,p)),
+//   x = [a_k, a_p, a_q, b_k, b_p, b_q].  The line direction is taken from the PERMUTED normals, so
+//   (tc0, tc1, g0, g1) may come out as (-tc0, -tc1, -g0, -g1): Eq. 2-4 and L47's third quantity are
+//   even in that sign (every term pairs two of them), so energy, gradient and Hessian are unchanged.
+__device__ __forceinline__ void pair_derivs_recorded(const d3 ak, const d3 ap, const d3 aq, const d3 bk,
+                                                     const d3 bp, const d3 bq, double sigma, unsigned za,
+                                                     unsigned zb, double& tc0, double& tc1,
+                                                     double (&g0)[18], double (&g1)[18]) {
+  const d3 eap = ap - ak, eaq = aq - ak, ebp = bp - bk, ebq = bq - bk;
+  const d3 na = cross(eap, eaq), nb = cross(ebp, ebq);
+  const d3 ab = ak - bk;
+  const double dak = dot(nb, ab), dap = dot(nb, ap - bk), daq = dot(nb, aq - bk);
+  const double dbk = -dot(na, ab), dbp = dot(na, bp - ak), dbq = dot(na, bq - ak);
+  const d3 D = cross(na, nb);
+  const d3 Dh = rsqrt(dot(D, D)) * D;
+  const EndPoint Pa = end_point(sigma, Dh, ak, eap, dak, dap, za == 1u ? 0.0 : 1.0, bk, ebp, ebq, nb);
+  const EndPoint Qa = end_point(sigma, Dh, ak, eaq, dak, daq, za == 2u ? 0.0 : 1.0, bk, ebp, ebq, nb);
+  const EndPoint Pb = end_point(-sigma, Dh, bk, ebp, dbk, dbp, zb == 1u ? 0.0 : 1.0, ak, eap, eaq, na);
+  const EndPoint Qb = end_point(-sigma, Dh, bk, ebq, dbk, dbq, zb == 2u ? 0.0 : 1.0, ak, eap, eaq, na);
+  tc0 = sigma * (Pa.t - Qb.t);  // Eq. 1
+  tc1 = sigma * (Qa.t - Pb.t);
+  auto put = [](double (&g)[18], int o, const d3 v) { g[o] = v.x; g[o + 1] = v.y; g[o + 2] = v.z; };
+  put(g0, 0, Pa.ownk + Qb.yk);   put(g0, 3, Pa.owne + Qb.yp);   put(g0, 6, Qb.yq);
+  put(g0, 9, Pa.yk + Qb.ownk);   put(g0, 12, Pa.yp);            put(g0, 15, Pa.yq + Qb.owne);
+  put(g1, 0, Qa.ownk + Pb.yk);   put(g1, 3, Pb.yp);             put(g1, 6, Qa.owne + Pb.yq);
+  put(g1, 9, Qa.yk + Pb.ownk);   put(g1, 12, Qa.yp + Pb.owne);  put(g1, 15, Qa.yq);
 }
 
 // Step a3, second half: Eq. 3 and Eq. 4 coefficients.  keep = tt_hess_mode's treatment of the

@@ -81,12 +81,14 @@ template <typename T>
 __global__ void __launch_bounds__(CLS_THREADS)
 k_classify(const T* __restrict__ pos, const int* __restrict__ tris, const int2* __restrict__ pairs,
            int64_t P, double sigma, uint32_t* __restrict__ mask, int* __restrict__ blk_count,
-           double* __restrict__ blk_energy, T* __restrict__ e_pp, T* __restrict__ tc_out) {
+           double* __restrict__ blk_energy, T* __restrict__ e_pp, T* __restrict__ tc_out,
+           uint16_t* __restrict__ cfg_out) {
   __shared__ double s_e[CLS_THREADS / 32];
   __shared__ int s_c[CLS_THREADS / 32];
   const int64_t k = (int64_t)blockIdx.x * CLS_THREADS + threadIdx.x;
   bool active = false;
   double tc0 = 0.0, tc1 = 0.0, en = 0.0;
+  unsigned cfg = 0u;
   if (k < P) {
     const int2 pr = __ldg(pairs + k);
     int va[3], vb[3];
@@ -99,8 +101,10 @@ k_classify(const T* __restrict__ pos, const int* __restrict__ tris, const int2* 
         tc1 = g.tc1;
         const double pr2 = tc0 * tc1;
         en = pr2 * pr2;  // Eq. 2
+        cfg = ttg::pair_config(g);
       }
     }
+    if (cfg_out) cfg_out[k] = (uint16_t)cfg;
     if (e_pp) e_pp[k] = (T)en;
     if (tc_out) {
       tc_out[2 * k] = (T)tc0;
@@ -164,16 +168,19 @@ k_compact(const uint32_t* __restrict__ mask, const int* __restrict__ blk_off, in
 
 // ------------------------------------------------------------------------------------------ K3
 // Directed entries: active pair k = (s,t) -> (s -> t, side 0) and (t -> s, side 1).
-// key = (source << bitsT) | partner, payload = 2k + side (k = index into active_ids).
+// key = (source << bitsT) | partner, payload = side | recorded config of the canonical pair << 1.
 __global__ void k_emit_directed(const int2* __restrict__ pairs, const int* __restrict__ active_ids,
-                                int64_t A, int bitsT, uint64_t* __restrict__ keys, uint32_t* __restrict__ vals) {
+                                const uint16_t* __restrict__ cfg, int64_t A, int bitsT,
+                                uint64_t* __restrict__ keys, uint16_t* __restrict__ vals) {
   const int64_t k = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
   if (k >= A) return;
-  const int2 pr = __ldg(pairs + active_ids[k]);
+  const int id = active_ids[k];
+  const int2 pr = __ldg(pairs + id);
+  const unsigned c = (unsigned)__ldg(cfg + id) << 1;
   keys[2 * k] = ((uint64_t)(uint32_t)pr.x << bitsT) | (uint32_t)pr.y;
   keys[2 * k + 1] = ((uint64_t)(uint32_t)pr.y << bitsT) | (uint32_t)pr.x;
-  vals[2 * k] = (uint32_t)(2 * k);
-  vals[2 * k + 1] = (uint32_t)(2 * k + 1);
+  vals[2 * k] = (uint16_t)c;
+  vals[2 * k + 1] = (uint16_t)(c | 1u);
 }
 
 // Segment pointers from sorted keys: ptr[g] = first entry whose (key >> shift) >= g, g = 0..G.
@@ -441,11 +448,12 @@ __global__ void k_emit_vslots(const int* __restrict__ tris, const int* __restric
 // the <= 15 unaligned head / tail bytes by plain stores).  Address generation and full-line
 // writes are the copy engine's; the SM issues ~60 shared stores per entry and row.
 struct Entry {
-  double g0[18], g1[18];   // own triangle's 9 DOF first, partner's 9 after
+  double g0[18], g1[18];   // own triangle's 9 DOF first, partner's 9 after; vertices in RECORDED order (k, p, q)
   ttg::Coefs cf;
   double en;               // Eq. 2 energy if this is the canonical copy (side 0), else 0
   int s;                   // source triangle
-  int va[3], vb[3];        // vertex ids of (own, partner)
+  int va[3], vb[3];        // vertex ids of (own, partner) in recorded order
+  int po[3], pp[3];        // recorded order -> index 0..2 inside the own / partner triangle
 };
 
 template <typename T>
@@ -453,7 +461,7 @@ struct AsmParams {
   const T* pos;
   const int* tris;
   const uint64_t* keys;     // sorted directed keys (source << bitsT | partner)
-  const uint32_t* dvals;    // 2k + side
+  const uint16_t* dvals;    // side | recorded config << 1 (ttg::pair_config)
   const int* touched;       // [n_touched]
   const int* tfirst;        // [n_touched+1]
   const int* chunk_start;   // [n_chunks+1] first touched index of every round
@@ -473,28 +481,43 @@ struct AsmParams {
   double sigma;
 };
 
-// Evaluates directed entry e: canonical pair, J, coefficients; swaps halves so that "own" is first.
+// Evaluates directed entry e: canonical pair with both triangles permuted as K1 recorded, J by the
+// straight-line code, coefficients; swaps halves so that "own" is first.
 template <typename T>
 __device__ __forceinline__ void eval_entry(const AsmParams<T>& P, int e, Entry& E) {
   const uint64_t key = __ldg(P.keys + e);
+  const unsigned pay = (unsigned)__ldg(P.dvals + e);
   const uint64_t tmask = (1ull << P.bitsT) - 1ull;
   E.s = (int)(key >> P.bitsT);
   const int t = (int)(key & tmask);
-  const int side = (int)(__ldg(P.dvals + e) & 1u);
-  const int2 pr = side ? make_int2(t, E.s) : make_int2(E.s, t);  // canonical (pairs[k,0], pairs[k,1])
+  const bool side = (pay & 1u) != 0u;
+  const int ta = side ? t : E.s, tb = side ? E.s : t;  // canonical (pairs[k,0], pairs[k,1])
+  const unsigned ca = (pay >> 1) & 63u, cb = (pay >> 7) & 63u;
+  int pa[3], pb[3];
+  pa[0] = (int)(ca & 3u); pa[1] = (int)((ca >> 2) & 3u); pa[2] = 3 - pa[0] - pa[1];
+  pb[0] = (int)(cb & 3u); pb[1] = (int)((cb >> 2) & 3u); pb[2] = 3 - pb[0] - pb[1];
   int va[3], vb[3];
-  d3 a[3], b[3];
-  gather_pair(P.pos, P.tris, pr.x, pr.y, va, vb, a, b);
-  ttg::PairGeom q;
-  ttg::pair_intervals(a[0], a[1], a[2], b[0], b[1], b[2], P.sigma, q);  // active by construction
-  ttg::pair_derivs(a[0], a[1], a[2], b[0], b[1], b[2], P.sigma, q, E.g0, E.g1);
-  E.cf = ttg::pair_coefs(q.tc0, q.tc1, E.g0, E.g1, P.hess_mode);
-  const double tt = q.tc0 * q.tc1;
+#pragma unroll
+  for (int m = 0; m < 3; ++m) {
+    va[m] = __ldg(P.tris + 3 * (int64_t)ta + pa[m]);
+    vb[m] = __ldg(P.tris + 3 * (int64_t)tb + pb[m]);
+  }
+  // local frame: translate by -a_k (kills the cancellation in D.E, keeps fp32 inputs well scaled)
+  const d3 o = load_vertex(P.pos, va[0]);
+  const d3 ak = ttg::mk(0.0, 0.0, 0.0);
+  const d3 ap = load_vertex(P.pos, va[1]) - o, aq = load_vertex(P.pos, va[2]) - o;
+  const d3 bk = load_vertex(P.pos, vb[0]) - o, bp = load_vertex(P.pos, vb[1]) - o, bq = load_vertex(P.pos, vb[2]) - o;
+  double tc0, tc1;
+  ttg::pair_derivs_recorded(ak, ap, aq, bk, bp, bq, P.sigma, ca >> 4, cb >> 4, tc0, tc1, E.g0, E.g1);
+  E.cf = ttg::pair_coefs(tc0, tc1, E.g0, E.g1, P.hess_mode);
+  const double tt = tc0 * tc1;
   E.en = side ? 0.0 : tt * tt;  // Eq. 2, counted once per pair
 #pragma unroll
   for (int m = 0; m < 3; ++m) {
     E.va[m] = side ? vb[m] : va[m];
     E.vb[m] = side ? va[m] : vb[m];
+    E.po[m] = side ? pb[m] : pa[m];
+    E.pp[m] = side ? pa[m] : pb[m];
   }
   if (side) {
 #pragma unroll
@@ -503,6 +526,27 @@ __device__ __forceinline__ void eval_entry(const AsmParams<T>& P, int e, Entry& 
       const double t1 = E.g1[i]; E.g1[i] = E.g1[9 + i]; E.g1[9 + i] = t1;
     }
   }
+}
+
+// Brings the own half of J back to the triangle's own vertex order through the lane's private
+// slice of shared memory (18 stores at permuted addresses, 18 loads), and the partner's block
+// ranks into recorded order (integer selects).
+__device__ __forceinline__ void unpermute_own(Entry& E, double* lane_smem /*>= 18 doubles*/, int (&er)[3]) {
+#pragma unroll
+  for (int r = 0; r < 3; ++r)
+#pragma unroll
+    for (int cc = 0; cc < 3; ++cc) {
+      lane_smem[3 * E.po[r] + cc] = E.g0[3 * r + cc];
+      lane_smem[9 + 3 * E.po[r] + cc] = E.g1[3 * r + cc];
+    }
+#pragma unroll
+  for (int i = 0; i < 9; ++i) {
+    E.g0[i] = lane_smem[i];
+    E.g1[i] = lane_smem[9 + i];
+  }
+  const int e0 = er[0], e1 = er[1], e2 = er[2];
+#pragma unroll
+  for (int r = 0; r < 3; ++r) er[r] = (E.pp[r] == 0) ? e0 : ((E.pp[r] == 1) ? e1 : e2);
 }
 
 __device__ __forceinline__ void bulk_s2g(void* gdst, const void* ssrc, uint32_t bytes) {
@@ -596,9 +640,10 @@ k_assemble_tile(const AsmParams<T> P) {
   E.s = -1;
   int er[3] = {0, 0, 0};
   if (valid) {
-    eval_entry(P, e_lo + lane, E);
 #pragma unroll
     for (int n = 0; n < 3; ++n) er[n] = __ldg(P.erank + 3 * (int64_t)(e_lo + lane) + n);
+    eval_entry(P, e_lo + lane, E);
+    unpermute_own(E, S.stage + lane * STG_STRIDE, er);
   }
   int ti;
   {
@@ -711,10 +756,11 @@ k_assemble_long(const AsmParams<T> P) {
     Entry E;
     int er[3] = {0, 0, 0};
     if (valid) {
-      eval_entry(P, base + lane, E);
-      e_acc += E.en;
 #pragma unroll
       for (int n = 0; n < 3; ++n) er[n] = __ldg(P.erank + 3 * (int64_t)(base + lane) + n);
+      eval_entry(P, base + lane, E);
+      e_acc += E.en;
+      unpermute_own(E, S.stage + lane * STG_STRIDE, er);
     }
 #pragma unroll
     for (int m = 0; m < 3; ++m) {
@@ -803,7 +849,10 @@ k_entry_reduce(const AsmParams<T> P) {
         u1 = E.cf.c01 * j0 + E.cf.c11 * j1;
       }
 #pragma unroll
-      for (int i = 0; i < 9; ++i) stage[lane * 9 + i] = u0 * E.g0[i] + u1 * E.g1[i];
+      for (int r = 0; r < 3; ++r)
+#pragma unroll
+        for (int cc = 0; cc < 3; ++cc)
+          stage[lane * 9 + 3 * E.po[r] + cc] = u0 * E.g0[3 * r + cc] + u1 * E.g1[3 * r + cc];
     }
     src[lane] = s;
     __syncwarp();

@@ -61,7 +61,7 @@ struct tt_ctx {
   std::string err;
   int64_t launches = 0;
   // classification
-  DevBuf mask, blk_count, blk_off, blk_energy, counts, energy;
+  DevBuf mask, blk_count, blk_off, blk_energy, counts, energy, cfg;
   // active set + directed entries
   DevBuf active_ids, keys[2], dvals[2], tptr, vcnt, tflag, touched;
   // per-triangle symbolic
@@ -80,7 +80,7 @@ struct tt_ctx {
   int64_t A = 0, n_dir = 0, n_touched = 0, R = 0, U = 0, nnzb = 0, n_chunks = 0, n_long = 0, rows_excl = 0, rows_gen = 0;
   int bitsT = 1, bitsV = 1;
   uint64_t* keys_sorted = nullptr;
-  uint32_t* dvals_sorted = nullptr;
+  uint16_t* dvals_sorted = nullptr;
   uint64_t* rkeys_sorted = nullptr;
   uint32_t* rvals_sorted = nullptr;
   uint32_t* vvals_sorted = nullptr;
@@ -175,10 +175,11 @@ tt_status incl_scan_i32(tt_ctx* ctx, const int* in, int* out, int64_t n, cudaStr
   return TT_OK;
 }
 // stable LSD radix sort of (key, payload) on bits [0, end_bit); result pointers returned
+template <typename V>
 tt_status sort_pairs(tt_ctx* ctx, DevBuf (&kb)[2], DevBuf (&vb)[2], int64_t n, int end_bit,
-                     uint64_t** k_out, uint32_t** v_out, cudaStream_t st) {
+                     uint64_t** k_out, V** v_out, cudaStream_t st) {
   cub::DoubleBuffer<uint64_t> dk(kb[0].as<uint64_t>(), kb[1].as<uint64_t>());
-  cub::DoubleBuffer<uint32_t> dv(vb[0].as<uint32_t>(), vb[1].as<uint32_t>());
+  cub::DoubleBuffer<V> dv(vb[0].as<V>(), vb[1].as<V>());
   size_t tmp = 0;
   TT_CUDA(cub::DeviceRadixSort::SortPairs(nullptr, tmp, dk, dv, n, 0, end_bit, st));
   TT_CUDA(ctx->cub_tmp.ensure(tmp));
@@ -191,7 +192,7 @@ tt_status sort_pairs(tt_ctx* ctx, DevBuf (&kb)[2], DevBuf (&vb)[2], int64_t n, i
 
 // ---- K1 (+ sums): shared by tt_energy and tt_hess_symbolic -------------------------------------
 template <typename T>
-tt_status run_classify(tt_ctx* ctx, const tt_problem* q, T* e_pp, T* tc, cudaStream_t st, int64_t* nblk_out) {
+tt_status run_classify(tt_ctx* ctx, const tt_problem* q, T* e_pp, T* tc, bool record, cudaStream_t st, int64_t* nblk_out) {
   const int64_t P = q->n_pairs;
   const int64_t nblk = (P + ttk::CLS_THREADS - 1) / ttk::CLS_THREADS;
   *nblk_out = nblk;
@@ -201,12 +202,13 @@ tt_status run_classify(tt_ctx* ctx, const tt_problem* q, T* e_pp, T* tc, cudaStr
   TT_CUDA(ctx->blk_energy.ensure(sizeof(double) * (size_t)(nblk + 1)));
   TT_CUDA(ctx->counts.ensure(sizeof(int64_t) * 16));
   TT_CUDA(ctx->energy.ensure(sizeof(double) * 2));
+  if (record) TT_CUDA(ctx->cfg.ensure(sizeof(uint16_t) * (size_t)(P + 1)));
   TT_CUDA(cudaMemsetAsync(ctx->blk_count.as<int>() + nblk, 0, sizeof(int), st));
   if (nblk > 0) {
     TT_CUDA(cudaEventRecord(ctx->ev[0][0], st));
     ttk::k_classify<T><<<(unsigned)nblk, ttk::CLS_THREADS, 0, st>>>(
         (const T*)q->pos, q->tris, (const int2*)q->pairs, P, ctx->opt.tc_scale, ctx->mask.as<uint32_t>(),
-        ctx->blk_count.as<int>(), ctx->blk_energy.as<double>(), e_pp, tc);
+        ctx->blk_count.as<int>(), ctx->blk_energy.as<double>(), e_pp, tc, record ? ctx->cfg.as<uint16_t>() : nullptr);
     TT_LAUNCH_CHECK();
     TT_CUDA(cudaEventRecord(ctx->ev[0][1], st));
     ctx->ev_used[0] = true;
@@ -220,7 +222,7 @@ template <typename T>
 tt_status energy_impl(tt_ctx* ctx, const tt_problem* q, void* energy_sum, void* e_pp, uint32_t* active_mask,
                       void* tc, int64_t* n_active, cudaStream_t st) {
   int64_t nblk = 0;
-  tt_status s = run_classify<T>(ctx, q, (T*)e_pp, (T*)tc, st, &nblk);
+  tt_status s = run_classify<T>(ctx, q, (T*)e_pp, (T*)tc, false, st, &nblk);
   if (s != TT_OK) return s;
   ttk::k_sum_partials<T><<<1, 1024, 0, st>>>(ctx->blk_energy.as<double>(), nblk, 1.0, (T*)energy_sum);
   TT_LAUNCH_CHECK();
@@ -241,7 +243,7 @@ tt_status symbolic_impl(tt_ctx* ctx, const tt_problem* q, int64_t* nnzb_host, in
   ctx->sig.valid = false;
   const int64_t P = q->n_pairs, nT = q->n_tris, nV = q->n_verts;
   int64_t nblk = 0;
-  tt_status s = run_classify<T>(ctx, q, nullptr, nullptr, st, &nblk);
+  tt_status s = run_classify<T>(ctx, q, nullptr, nullptr, true, st, &nblk);
   if (s != TT_OK) return s;
   int64_t* d_counts = ctx->counts.as<int64_t>();
   k_set_count<<<1, 32, 0, st>>>(ctx->blk_off.as<int>(), ctx->blk_count.as<int>(), nblk, d_counts, nullptr);
@@ -265,13 +267,13 @@ tt_status symbolic_impl(tt_ctx* ctx, const tt_problem* q, int64_t* nnzb_host, in
   }
   for (int i = 0; i < 2; ++i) {
     TT_CUDA(ctx->keys[i].ensure(sizeof(uint64_t) * (size_t)(n + 1)));
-    TT_CUDA(ctx->dvals[i].ensure(sizeof(uint32_t) * (size_t)(n + 1)));
+    TT_CUDA(ctx->dvals[i].ensure(sizeof(uint16_t) * (size_t)(n + 1)));
   }
   ctx->keys_sorted = ctx->keys[0].as<uint64_t>();
-  ctx->dvals_sorted = ctx->dvals[0].as<uint32_t>();
+  ctx->dvals_sorted = ctx->dvals[0].as<uint16_t>();
   if (A > 0) {
-    k_emit_directed<<<grid_for(A, 256), 256, 0, st>>>((const int2*)q->pairs, ctx->active_ids.as<int>(), A, bitsT,
-                                                      ctx->keys[0].as<uint64_t>(), ctx->dvals[0].as<uint32_t>());
+    k_emit_directed<<<grid_for(A, 256), 256, 0, st>>>((const int2*)q->pairs, ctx->active_ids.as<int>(), ctx->cfg.as<uint16_t>(), A, bitsT,
+                                                      ctx->keys[0].as<uint64_t>(), ctx->dvals[0].as<uint16_t>());
     TT_LAUNCH_CHECK();
     s = sort_pairs(ctx, ctx->keys, ctx->dvals, n, 2 * bitsT, &ctx->keys_sorted, &ctx->dvals_sorted, st);
     if (s != TT_OK) return s;

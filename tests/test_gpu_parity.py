@@ -166,6 +166,27 @@ def test_long_rows_span_cta_rounds(oracle_mod):
 
 
 # ------------------------------------------------------------------------------------ edge cases
+@pytest.mark.parametrize("dtype", ["f64", "f32"])
+def test_vertex_exactly_on_plane(oracle_mod, dtype):
+    """App. A L106-115 (reading A4): a vertex lying exactly on the other plane (+,-,0).  The recorded
+    configuration marks that end-point as the vertex itself; all four placements (a or b carries the
+    vertex, it is the smaller or the larger end-point) must match the oracle's one-sided derivative."""
+    from paper_2606_06511_b200 import inputs
+    a = np.array([[-1, -1, 0], [3, -1, 0], [1, 1, 0.0]])
+    b = np.array([[0, 0, -1], [6, 0, 1], [1, 0, 0.0]])          # b2 on plane(a): tc = (-3, 1)
+    mirror = np.array([-1.0, 1.0, 1.0])                         # x -> -x: vertex end-point becomes the larger one
+    tris_pos, shift = [], np.array([10.0, 0, 0])
+    for k, (ta, tb) in enumerate([(a, b), (b, a), (a * mirror, b * mirror), (b[[1, 2, 0]] * mirror, a[[2, 0, 1]] * mirror)]):
+        tris_pos += [ta + k * shift, tb + k * shift]
+    pos = np.concatenate(tris_pos)
+    tris = np.arange(pos.shape[0], dtype=np.int32).reshape(-1, 3)
+    pairs = np.array([[0, 1], [2, 3], [4, 5], [6, 7]], dtype=np.int32)
+    pb = inputs.Problem(pos, tris, pairs, "on_plane", {})
+    ref, out, st = run_case(oracle_mod, pb, dtype, 0)
+    assert out["n_active"] == 4
+    np.testing.assert_allclose(ref["tc"][0], [-3, 1], atol=1e-14)
+
+
 def test_empty_and_inactive_inputs(oracle_mod):
     from paper_2606_06511_b200 import inputs, tt
     dev = _dev()
