@@ -211,16 +211,18 @@ __global__ void k_vertex_touch(const int* __restrict__ tris, const int* __restri
 // duplicates, decides which of the three rows are EXCLUSIVE (vertex used by no other touched
 // triangle, no duplicate column) and records:
 //   erank[e][n]   position of partner column (e, n) inside the row       (rank, or identity if dup)
-//   drank[s][n]   position of the diagonal column n
-//   rowlen[p]     = L for exclusive rows;  tlen[3s+m] = L for general rows (their blocks go to
+//   drank[ti][n]  position of the diagonal column n
+//   rowlen[p]     = L for exclusive rows;  tlen[3ti+m] = L for general rows (their blocks go to
 //                 the merge workspace, one merge record each)
+// Per-slot arrays (drank, tlen, toff, slot_excl, rowbase, tslot) are indexed by TOUCHED index ti:
+// the numeric kernels then need no triangle id to find them.
 // layout = rank (columns ascending) when there is no duplicate, else identity (3j+n, diag last).
 __global__ void __launch_bounds__(32 * SYM_WARPS)
 k_tri_symbolic(const int* __restrict__ tris, const int* __restrict__ touched, int64_t n_touched,
                const int* __restrict__ tptr, const uint64_t* __restrict__ keys, int bitsT,
                const int* __restrict__ vcnt, int force_general, int* __restrict__ erank /*[2A][3]*/,
-               int* __restrict__ drank /*[nT][3]*/, int* __restrict__ rowlen, int64_t* __restrict__ tlen /*[3nT]*/,
-               uint8_t* __restrict__ slot_excl /*[3nT]*/) {
+               int* __restrict__ drank /*[n_touched][3]*/, int* __restrict__ rowlen,
+               int64_t* __restrict__ tlen /*[3 n_touched]*/, uint8_t* __restrict__ slot_excl /*[3 n_touched]*/) {
   __shared__ int s_c[SYM_WARPS][SYM_LMAX];
   const int w = threadIdx.x >> 5, l = threadIdx.x & 31;
   const int64_t ti = (int64_t)blockIdx.x * SYM_WARPS + w;
@@ -256,13 +258,13 @@ k_tri_symbolic(const int* __restrict__ tris, const int* __restrict__ touched, in
     }
     const int j = idx / 3, n = idx - 3 * j;
     if (j < deg) erank[3 * (int64_t)(e0 + j) + n] = r;
-    else drank[3 * (int64_t)s + n] = r;
+    else drank[3 * ti + n] = r;
   }
   if (l < 3) {
     const int p = tris[3 * (int64_t)s + l];
     const bool excl = nodup && !force_general && (vcnt[p] == 1);
-    slot_excl[3 * (int64_t)s + l] = excl ? 1 : 0;
-    tlen[3 * (int64_t)s + l] = excl ? 0 : L;
+    slot_excl[3 * ti + l] = excl ? 1 : 0;
+    tlen[3 * ti + l] = excl ? 0 : L;
     if (excl) rowlen[p] = L;
   }
 }
@@ -282,14 +284,14 @@ k_emit_records(const int* __restrict__ tris, const int* __restrict__ touched, in
   const int L = 3 * (deg + 1);
   const uint64_t tmask = (1ull << bitsT) - 1ull;
   for (int m = 0; m < 3; ++m) {
-    if (slot_excl[3 * (int64_t)s + m]) continue;
+    if (slot_excl[3 * ti + m]) continue;
     const uint64_t p = (uint64_t)(uint32_t)tris[3 * (int64_t)s + m];
-    const int64_t base = toff[3 * (int64_t)s + m];
+    const int64_t base = toff[3 * ti + m];
     for (int idx = l; idx < L; idx += 32) {
       const int j = idx / 3, n = idx - 3 * j;
       const int t = (j < deg) ? (int)(keys[e0 + j] & tmask) : s;
       const int q = tris[3 * (int64_t)t + n];
-      const int r = (j < deg) ? erank[3 * (int64_t)(e0 + j) + n] : drank[3 * (int64_t)s + n];
+      const int r = (j < deg) ? erank[3 * (int64_t)(e0 + j) + n] : drank[3 * ti + n];
       rkeys[base + r] = (p << bitsV) | (uint32_t)q;
       rvals[base + r] = (uint32_t)(base + r);
     }
@@ -336,7 +338,7 @@ k_fill_rows(const int* __restrict__ tris, const int* __restrict__ touched, int64
             const int* __restrict__ tptr, const uint64_t* __restrict__ keys, int bitsT,
             const int* __restrict__ erank, const int* __restrict__ drank, const int64_t* __restrict__ toff,
             const uint8_t* __restrict__ slot_excl, const int* __restrict__ rowptr,
-            int64_t* __restrict__ rowbase /*[3nT]*/, int* __restrict__ colind) {
+            int64_t* __restrict__ rowbase /*[3 n_touched]*/, int* __restrict__ colind) {
   const int w = threadIdx.x >> 5, l = threadIdx.x & 31;
   const int64_t ti = (int64_t)blockIdx.x * SYM_WARPS + w;
   if (ti >= n_touched) return;
@@ -345,17 +347,17 @@ k_fill_rows(const int* __restrict__ tris, const int* __restrict__ touched, int64
   const int L = 3 * (deg + 1);
   const uint64_t tmask = (1ull << bitsT) - 1ull;
   for (int m = 0; m < 3; ++m) {
-    const int64_t slot = 3 * (int64_t)s + m;
+    const int64_t slot = 3 * ti + m;
     if (!slot_excl[slot]) {
       if (l == 0) rowbase[slot] = -(toff[slot] + 1);
       continue;
     }
-    const int rp = rowptr[tris[slot]];
+    const int rp = rowptr[tris[3 * (int64_t)s + m]];
     if (l == 0) rowbase[slot] = rp;
     for (int idx = l; idx < L; idx += 32) {
       const int j = idx / 3, n = idx - 3 * j;
       const int t = (j < deg) ? (int)(keys[e0 + j] & tmask) : s;
-      const int r = (j < deg) ? erank[3 * (int64_t)(e0 + j) + n] : drank[3 * (int64_t)s + n];
+      const int r = (j < deg) ? erank[3 * (int64_t)(e0 + j) + n] : drank[3 * ti + n];
       colind[rp + r] = tris[3 * (int64_t)t + n];
     }
   }
@@ -418,7 +420,7 @@ __global__ void k_chunk_pack(const int* __restrict__ tfirst, int64_t n_touched, 
   }
 }
 
-// vertex -> touched (triangle, slot) incidence keys: key = vertex, payload = 3s+m
+// vertex -> touched (triangle, slot) incidence keys: key = vertex, payload = slot 3 ti + m
 __global__ void k_emit_vslots(const int* __restrict__ tris, const int* __restrict__ touched,
                               int64_t n_touched, uint64_t* __restrict__ vkeys, uint32_t* __restrict__ vvals) {
   const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
@@ -427,7 +429,7 @@ __global__ void k_emit_vslots(const int* __restrict__ tris, const int* __restric
   const int m = (int)(i - 3 * ti);
   const int s = touched[ti];
   vkeys[i] = (uint64_t)(uint32_t)tris[3 * (int64_t)s + m];
-  vvals[i] = (uint32_t)(3 * s + m);
+  vvals[i] = (uint32_t)i;
 }
 
 // ------------------------------------------------------------------------------------------ K4
@@ -447,31 +449,34 @@ __global__ void k_emit_vslots(const int* __restrict__ tris, const int* __restric
 // and hands every run to the TMA engine (cp.async.bulk shared -> global, 16-byte aligned body;
 // the <= 15 unaligned head / tail bytes by plain stores).  Address generation and full-line
 // writes are the copy engine's; the SM issues ~60 shared stores per entry and row.
+//
+// The grid is PERSISTENT (a few CTAs per SM); a warp walks rounds c, c + G, c + 2G, ... and keeps
+// the operands of its NEXT round in flight while it works on the current one: descriptor two
+// rounds ahead, vertex ids / payload / ranks / row destinations one round ahead (issued at the
+// top of a round), positions one round ahead (issued after the current round's derivatives).
+// Every gather therefore has a full round (~2-3 k instructions) to land.
 struct Entry {
   double g0[18], g1[18];   // own triangle's 9 DOF first, partner's 9 after; vertices in RECORDED order (k, p, q)
   ttg::Coefs cf;
   double en;               // Eq. 2 energy if this is the canonical copy (side 0), else 0
-  int s;                   // source triangle
-  int va[3], vb[3];        // vertex ids of (own, partner) in recorded order
   int po[3], pp[3];        // recorded order -> index 0..2 inside the own / partner triangle
 };
 
 template <typename T>
 struct AsmParams {
   const T* pos;
-  const int* tris;
   const uint64_t* keys;     // sorted directed keys (source << bitsT | partner)
   const uint16_t* dvals;    // side | recorded config << 1 (ttg::pair_config)
-  const int* touched;       // [n_touched]
+  const int* everts;        // [2A][6] vertex ids of the canonical pair, both triangles in recorded order
+  const int4* rdesc;        // [n_chunks] round descriptor: first entry, entries, first touched index, triangles
   const int* tfirst;        // [n_touched+1]
-  const int* chunk_start;   // [n_chunks+1] first touched index of every round
   const int* long_list;     // [n_long] round ids of the long triangles
   const int* erank;         // [2A][3]
-  const int* drank;         // [nT][3]
-  const int64_t* rowbase;   // [3nT]
+  const int* drank;         // [n_touched][3]
+  const int64_t* rowbase;   // [3 n_touched]
   T* vals;                  // final BSR values
   T* tvals;                 // merge workspace values
-  T* tslot;                 // [3nT][3] per-slot gradient (K4) or H.p (K6) partials
+  T* tslot;                 // [3 n_touched][3] per-slot gradient (K4) or H.p (K6) partials
   double* chunk_energy;     // [n_chunks]
   const T* pvec;            // K6: p [nV,3]
   int64_t n_chunks;
@@ -481,41 +486,69 @@ struct AsmParams {
   double sigma;
 };
 
-// Evaluates directed entry e: canonical pair with both triangles permuted as K1 recorded, J by the
-// straight-line code, coefficients; swaps halves so that "own" is first.
-template <typename T>
-__device__ __forceinline__ void eval_entry(const AsmParams<T>& P, int e, Entry& E) {
-  const uint64_t key = __ldg(P.keys + e);
-  const unsigned pay = (unsigned)__ldg(P.dvals + e);
-  const uint64_t tmask = (1ull << P.bitsT) - 1ull;
-  E.s = (int)(key >> P.bitsT);
-  const int t = (int)(key & tmask);
+// Per-entry vertex ids of the canonical pair with both triangles permuted as K1 recorded
+// (symbolic phase, once per active set): everts[e] = [a_k, a_p, a_q, b_k, b_p, b_q].
+__global__ void k_ent_verts(const uint64_t* __restrict__ keys, const uint16_t* __restrict__ dvals,
+                            const int* __restrict__ tris, int64_t n_dir, int bitsT, int* __restrict__ everts) {
+  const int64_t e = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (e >= n_dir) return;
+  const uint64_t key = keys[e];
+  const unsigned pay = dvals[e];
+  const int s = (int)(key >> bitsT), t = (int)(key & ((1ull << bitsT) - 1ull));
   const bool side = (pay & 1u) != 0u;
-  const int ta = side ? t : E.s, tb = side ? E.s : t;  // canonical (pairs[k,0], pairs[k,1])
+  const int ta = side ? t : s, tb = side ? s : t;  // canonical (pairs[k,0], pairs[k,1])
+  const unsigned ca = (pay >> 1) & 63u, cb = (pay >> 7) & 63u;
+  const int ka = (int)(ca & 3u), pa = (int)((ca >> 2) & 3u), kb = (int)(cb & 3u), pb = (int)((cb >> 2) & 3u);
+  int* o = everts + 6 * e;
+  o[0] = __ldg(tris + 3 * (int64_t)ta + ka);
+  o[1] = __ldg(tris + 3 * (int64_t)ta + pa);
+  o[2] = __ldg(tris + 3 * (int64_t)ta + (3 - ka - pa));
+  o[3] = __ldg(tris + 3 * (int64_t)tb + kb);
+  o[4] = __ldg(tris + 3 * (int64_t)tb + pb);
+  o[5] = __ldg(tris + 3 * (int64_t)tb + (3 - kb - pb));
+}
+
+__global__ void k_round_desc(const int* __restrict__ chunk_start, const int* __restrict__ tfirst, int64_t n_chunks,
+                             int64_t n_touched, int4* __restrict__ rdesc) {
+  const int64_t c = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (c >= n_chunks) return;
+  const int t0 = chunk_start[c];
+  const int t1 = (c + 1 < n_chunks) ? chunk_start[c + 1] : (int)n_touched;
+  const int e0 = tfirst[t0];
+  rdesc[c] = make_int4(e0, tfirst[t1] - e0, t0, t1 - t0);
+}
+
+template <typename T>
+__device__ __forceinline__ void load_pos18(const T* __restrict__ pos, const int (&ids)[6], double (&x)[18]) {
+#pragma unroll
+  for (int v = 0; v < 6; ++v) {
+    const T* p = pos + 3 * (int64_t)ids[v];
+    x[3 * v] = (double)__ldg(p);
+    x[3 * v + 1] = (double)__ldg(p + 1);
+    x[3 * v + 2] = (double)__ldg(p + 2);
+  }
+}
+
+// J by the straight-line code on gathered positions x = [a_k, a_p, a_q, b_k, b_p, b_q] (raw),
+// coefficients, energy; swaps halves so that "own" is first.
+__device__ __forceinline__ void eval_core(const double (&x)[18], unsigned pay, double sigma, int hess_mode, Entry& E) {
+  const bool side = (pay & 1u) != 0u;
   const unsigned ca = (pay >> 1) & 63u, cb = (pay >> 7) & 63u;
   int pa[3], pb[3];
   pa[0] = (int)(ca & 3u); pa[1] = (int)((ca >> 2) & 3u); pa[2] = 3 - pa[0] - pa[1];
   pb[0] = (int)(cb & 3u); pb[1] = (int)((cb >> 2) & 3u); pb[2] = 3 - pb[0] - pb[1];
-  int va[3], vb[3];
-#pragma unroll
-  for (int m = 0; m < 3; ++m) {
-    va[m] = __ldg(P.tris + 3 * (int64_t)ta + pa[m]);
-    vb[m] = __ldg(P.tris + 3 * (int64_t)tb + pb[m]);
-  }
   // local frame: translate by -a_k (kills the cancellation in D.E, keeps fp32 inputs well scaled)
-  const d3 o = load_vertex(P.pos, va[0]);
+  const d3 o = ttg::mk(x[0], x[1], x[2]);
   const d3 ak = ttg::mk(0.0, 0.0, 0.0);
-  const d3 ap = load_vertex(P.pos, va[1]) - o, aq = load_vertex(P.pos, va[2]) - o;
-  const d3 bk = load_vertex(P.pos, vb[0]) - o, bp = load_vertex(P.pos, vb[1]) - o, bq = load_vertex(P.pos, vb[2]) - o;
+  const d3 ap = ttg::mk(x[3], x[4], x[5]) - o, aq = ttg::mk(x[6], x[7], x[8]) - o;
+  const d3 bk = ttg::mk(x[9], x[10], x[11]) - o, bp = ttg::mk(x[12], x[13], x[14]) - o, bq = ttg::mk(x[15], x[16], x[17]) - o;
   double tc0, tc1;
-  ttg::pair_derivs_recorded(ak, ap, aq, bk, bp, bq, P.sigma, ca >> 4, cb >> 4, tc0, tc1, E.g0, E.g1);
-  E.cf = ttg::pair_coefs(tc0, tc1, E.g0, E.g1, P.hess_mode);
+  ttg::pair_derivs_recorded(ak, ap, aq, bk, bp, bq, sigma, ca >> 4, cb >> 4, tc0, tc1, E.g0, E.g1);
+  E.cf = ttg::pair_coefs(tc0, tc1, E.g0, E.g1, hess_mode);
   const double tt = tc0 * tc1;
   E.en = side ? 0.0 : tt * tt;  // Eq. 2, counted once per pair
 #pragma unroll
   for (int m = 0; m < 3; ++m) {
-    E.va[m] = side ? vb[m] : va[m];
-    E.vb[m] = side ? va[m] : vb[m];
     E.po[m] = side ? pb[m] : pa[m];
     E.pp[m] = side ? pa[m] : pb[m];
   }
@@ -573,12 +606,49 @@ template <typename T>
 struct alignas(16) TileWarpSmem {
   unsigned char tile[TileCfg<T>::TILE_BYTES];
   double stage[32 * STG_STRIDE];
-  unsigned long long run_g[RND_MAX_TRI];  // global byte address of the triangle's run (current row)
-  int run_off[RND_MAX_TRI];               // its byte offset in the tile (same address mod 16)
-  int tri_first[RND_MAX_TRI + 1];         // first entry (lane) of every triangle of the round
-  int tri_id[RND_MAX_TRI];
-  int dr[RND_MAX_TRI][3];
+  int run_off[RND_MAX_TRI];               // byte offset of the triangle's run in the tile (current row)
+  int diag_off[RND_MAX_TRI][3];           // byte offset of its diagonal block n in the tile (current row)
 };
+
+// Operands of a round that depend only on its descriptor (loaded one round ahead).
+struct RoundOps {
+  int ids[6];        // lane = entry
+  unsigned pay;
+  int er[3];
+  int e0, e1;        // lane = triangle
+  int64_t rb[3];
+  int dr[3];
+};
+template <typename T>
+__device__ __forceinline__ void load_round_ops(const AsmParams<T>& P, const int4 d, int lane, RoundOps& R) {
+  const int nent = min(d.y, RND_MAX_ENT);
+#pragma unroll
+  for (int i = 0; i < 6; ++i) R.ids[i] = 0;
+  R.pay = 0u;
+  R.er[0] = R.er[1] = R.er[2] = 0;
+  R.e0 = R.e1 = 0;
+  R.rb[0] = R.rb[1] = R.rb[2] = 0;
+  R.dr[0] = R.dr[1] = R.dr[2] = 0;
+  if (lane < nent) {
+    const int64_t e = (int64_t)d.x + lane;
+    const int2* v = reinterpret_cast<const int2*>(P.everts + 6 * e);
+    const int2 v0 = __ldg(v), v1 = __ldg(v + 1), v2 = __ldg(v + 2);
+    R.ids[0] = v0.x; R.ids[1] = v0.y; R.ids[2] = v1.x; R.ids[3] = v1.y; R.ids[4] = v2.x; R.ids[5] = v2.y;
+    R.pay = (unsigned)__ldg(P.dvals + e);
+#pragma unroll
+    for (int n = 0; n < 3; ++n) R.er[n] = __ldg(P.erank + 3 * e + n);
+  }
+  if (lane < d.w) {
+    const int64_t ti = (int64_t)d.z + lane;
+    R.e0 = __ldg(P.tfirst + ti);
+    R.e1 = __ldg(P.tfirst + ti + 1);
+#pragma unroll
+    for (int m = 0; m < 3; ++m) {
+      R.rb[m] = __ldg(P.rowbase + 3 * ti + m);
+      R.dr[m] = __ldg(P.drank + 3 * ti + m);
+    }
+  }
+}
 
 template <typename T>
 __global__ void __launch_bounds__(32 * TILE_WARPS)
@@ -588,145 +658,167 @@ k_assemble_tile(const AsmParams<T> P) {
   constexpr int RUN_UNIT = TileCfg<T>::RUN_UNIT;
   const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
   TileWarpSmem<T>& S = reinterpret_cast<TileWarpSmem<T>*>(s_raw)[warp];
-  const int64_t c = (int64_t)blockIdx.x * TILE_WARPS + warp;
+  const int64_t G = (int64_t)gridDim.x * TILE_WARPS;
+  int64_t c = (int64_t)blockIdx.x * TILE_WARPS + warp;
   if (c >= P.n_chunks) return;
-  const int t_lo = __ldg(P.chunk_start + c), ntri = __ldg(P.chunk_start + c + 1) - t_lo;
-
-  // ---- lane = triangle: ids, entry ranges, row destinations, tile slots ----
-  int my_s = 0, my_e0 = 0, my_e1 = 0;
-  if (lane < ntri) {
-    my_s = __ldg(P.touched + t_lo + lane);
-    my_e0 = __ldg(P.tfirst + t_lo + lane);
-    my_e1 = __ldg(P.tfirst + t_lo + lane + 1);
-  }
-  const int e_lo = __shfl_sync(FULL, my_e0, 0);
-  const int nent = __shfl_sync(FULL, my_e1, ntri - 1) - e_lo;
-  if (nent > RND_MAX_ENT) {  // long triangle: k_assemble_long's
-    if (lane == 0) P.chunk_energy[c] = 0.0;
-    return;
-  }
-  const int run_bytes = RUN_UNIT * (my_e1 - my_e0 + 1);
-  int slot_off = 0;
-  unsigned long long my_g[3] = {0ull, 0ull, 0ull};
-  {
-    int incl = (lane < ntri) ? (((run_bytes + 15) & ~15) + 16) : 0;
-    const int mine = incl;
-#pragma unroll
-    for (int o = 1; o < 32; o <<= 1) {
-      const int v = __shfl_up_sync(FULL, incl, o);
-      if (lane >= o) incl += v;
-    }
-    slot_off = incl - mine;
-  }
-  if (lane < ntri) {
-#pragma unroll
-    for (int m = 0; m < 3; ++m) {
-      const int64_t rb = __ldg(P.rowbase + 3 * (int64_t)my_s + m);
-      my_g[m] = (unsigned long long)((rb >= 0) ? (P.vals + 9 * rb) : (P.tvals + 9 * (-rb - 1)));
-      S.dr[lane][m] = __ldg(P.drank + 3 * (int64_t)my_s + m);
-    }
-    S.tri_first[lane] = my_e0 - e_lo;
-    S.tri_id[lane] = my_s;
-  }
-  if (lane == 0) S.tri_first[ntri] = nent;
-
-  // ---- lane = entry: J, coefficients ----
-  const bool valid = lane < nent;
-  Entry E;
-#pragma unroll
-  for (int i = 0; i < 18; ++i) { E.g0[i] = 0.0; E.g1[i] = 0.0; }
-  E.cf = {0, 0, 0, 0, 0};
-  E.en = 0.0;
-  E.s = -1;
-  int er[3] = {0, 0, 0};
-  if (valid) {
-#pragma unroll
-    for (int n = 0; n < 3; ++n) er[n] = __ldg(P.erank + 3 * (int64_t)(e_lo + lane) + n);
-    eval_entry(P, e_lo + lane, E);
-    unpermute_own(E, S.stage + lane * STG_STRIDE, er);
-  }
-  int ti;
-  {
-    const int s_prev = __shfl_up_sync(FULL, E.s, 1);
-    const unsigned heads = __ballot_sync(FULL, valid && (lane == 0 || E.s != s_prev));
-    ti = __popc(heads & (0xffffffffu >> (31 - lane))) - 1;
-  }
   const int cn = (lane < 27) ? lane / 9 : 0, cq = (lane < 27) ? lane % 9 : 0;
+  const int4 dzero = make_int4(0, 0, 0, 0);
+
+  // ---- prologue: this warp's first round ----
+  int4 d_cur = __ldg(P.rdesc + c);
+  int4 d_nxt = (c + G < P.n_chunks) ? __ldg(P.rdesc + c + G) : dzero;
+  RoundOps cur;
+  load_round_ops(P, d_cur, lane, cur);
+  double x[18];
+#pragma unroll
+  for (int i = 0; i < 18; ++i) x[i] = 0.0;
+  if (lane < min(d_cur.y, RND_MAX_ENT)) load_pos18(P.pos, cur.ids, x);
+
+  while (true) {
+    const bool has_next = c + G < P.n_chunks;
+    // ---- operands of the next round (descriptor known since the previous round) ----
+    RoundOps nxt;
+    load_round_ops(P, d_nxt, lane, nxt);
+    const int4 d_nn = (c + 2 * G < P.n_chunks) ? __ldg(P.rdesc + c + 2 * G) : dzero;
+
+    const int e_lo = d_cur.x, nent = d_cur.y, t_lo = d_cur.z, ntri = d_cur.w;
+    const bool is_long = nent > RND_MAX_ENT;  // k_assemble_long's
+    const bool valid = !is_long && lane < nent;
+
+    // ---- lane = entry: J, coefficients ----
+    Entry E;
+#pragma unroll
+    for (int i = 0; i < 18; ++i) { E.g0[i] = 0.0; E.g1[i] = 0.0; }
+    E.cf = {0, 0, 0, 0, 0};
+    E.en = 0.0;
+    int er[3] = {cur.er[0], cur.er[1], cur.er[2]};
+    if (valid) {
+      eval_core(x, cur.pay, P.sigma, P.hess_mode, E);
+      unpermute_own(E, S.stage + lane * STG_STRIDE, er);
+    }
+    // ---- positions of the next round: its vertex ids were requested at the top of this round ----
+    if (lane < min(d_nxt.y, RND_MAX_ENT)) load_pos18(P.pos, nxt.ids, x);
+
+    if (!is_long) {
+      // lane = triangle: tile slots (16-byte slots, prefix sum over the round's triangles)
+      const int run_bytes = RUN_UNIT * (cur.e1 - cur.e0 + 1);
+      int slot_off;
+      {
+        int incl = (lane < ntri) ? (((run_bytes + 15) & ~15) + 16) : 0;
+        const int mine = incl;
+#pragma unroll
+        for (int o = 1; o < RND_MAX_TRI; o <<= 1) {
+          const int v = __shfl_up_sync(FULL, incl, o);
+          if (lane >= o) incl += v;
+        }
+        slot_off = incl - mine;
+      }
+      // bit i of heads: entry i is the first of its triangle; my_ti: triangle of entry `lane`
+      const unsigned heads = __reduce_or_sync(FULL, (lane < ntri) ? (1u << (cur.e0 - e_lo)) : 0u);
+      const int my_ti = __popc(heads & (0xffffffffu >> (31 - lane))) - 1;
 
 #pragma unroll
-  for (int m = 0; m < 3; ++m) {
-    // the tile is single-buffered: the copy engine must have read the previous row's runs
-    bulk_wait_read();
-    __syncwarp();
-    if (lane < ntri) {
-      S.run_g[lane] = my_g[m];
-      S.run_off[lane] = slot_off + (int)(my_g[m] & 15ull);
-    }
-    __syncwarp();
-    if (valid) {
-      const double g0m[3] = {E.g0[3 * m], E.g0[3 * m + 1], E.g0[3 * m + 2]};
-      const double g1m[3] = {E.g1[3 * m], E.g1[3 * m + 1], E.g1[3 * m + 2]};
-      double a[3], b[3];
+      for (int m = 0; m < 3; ++m) {
+        const unsigned long long g =
+            (unsigned long long)((cur.rb[m] >= 0) ? (P.vals + 9 * cur.rb[m]) : (P.tvals + 9 * (-cur.rb[m] - 1)));
+        const int my_off = slot_off + (int)(g & 15ull);
+        // the tile is single-buffered: the copy engine must have read the previous row's runs
+        bulk_wait_read();
+        __syncwarp();
+        if (lane < ntri) {
+          S.run_off[lane] = my_off;
 #pragma unroll
-      for (int i = 0; i < 3; ++i) {
-        a[i] = E.cf.c00 * g0m[i] + E.cf.c01 * g1m[i];
-        b[i] = E.cf.c01 * g0m[i] + E.cf.c11 * g1m[i];
+          for (int n = 0; n < 3; ++n) S.diag_off[lane][n] = my_off + 9 * (int)sizeof(T) * cur.dr[n];
+        }
+        __syncwarp();
+        if (valid) {
+          const double g0m[3] = {E.g0[3 * m], E.g0[3 * m + 1], E.g0[3 * m + 2]};
+          const double g1m[3] = {E.g1[3 * m], E.g1[3 * m + 1], E.g1[3 * m + 2]};
+          double a[3], b[3];
+#pragma unroll
+          for (int i = 0; i < 3; ++i) {
+            a[i] = E.cf.c00 * g0m[i] + E.cf.c01 * g1m[i];
+            b[i] = E.cf.c01 * g0m[i] + E.cf.c11 * g1m[i];
+          }
+          T* run = reinterpret_cast<T*>(S.tile + S.run_off[my_ti]);
+#pragma unroll
+          for (int n = 0; n < 3; ++n) {
+            T* blk = run + 9 * er[n];
+#pragma unroll
+            for (int i = 0; i < 3; ++i)
+#pragma unroll
+              for (int j = 0; j < 3; ++j) blk[3 * i + j] = (T)(a[i] * E.g0[9 + 3 * n + j] + b[i] * E.g1[9 + 3 * n + j]);
+          }
+          double* st = S.stage + lane * STG_STRIDE;
+#pragma unroll
+          for (int n = 0; n < 3; ++n)
+#pragma unroll
+            for (int i = 0; i < 3; ++i)
+#pragma unroll
+              for (int j = 0; j < 3; ++j) st[9 * n + 3 * i + j] = a[i] * E.g0[3 * n + j] + b[i] * E.g1[3 * n + j];
+#pragma unroll
+          for (int i = 0; i < 3; ++i) st[27 + i] = E.cf.cg0 * g0m[i] + E.cf.cg1 * g1m[i];
+        }
+        __syncwarp();
+        // ---- sum over each triangle's entries, lane = component, entry order; loads 4 deep ----
+        if (lane < NSTG) {
+          int tt = -1;
+          double acc = 0.0;
+          auto flush = [&](int t_, double v_) {
+            if (lane < 27) *reinterpret_cast<T*>(S.tile + S.diag_off[t_][cn] + cq * (int)sizeof(T)) = (T)v_;
+            else P.tslot[9 * ((int64_t)t_lo + t_) + 3 * m + (lane - 27)] = (T)v_;
+          };
+          for (int i0 = 0; i0 < nent; i0 += 4) {
+            double v[4];
+#pragma unroll
+            for (int u = 0; u < 4; ++u) v[u] = S.stage[min(i0 + u, 31) * STG_STRIDE + lane];
+#pragma unroll
+            for (int u = 0; u < 4; ++u) {
+              const int i = i0 + u;
+              if (i < nent) {
+                if ((heads >> i) & 1u) {
+                  if (tt >= 0) flush(tt, acc);
+                  acc = 0.0;
+                  ++tt;
+                }
+                acc += v[u];
+              }
+            }
+          }
+          flush(tt, acc);
+        }
+        fence_async_smem();
+        __syncwarp();
+        // ---- lane = triangle: hand the run to the copy engine ----
+        if (lane < ntri) {
+          const unsigned char* src = S.tile + my_off;
+          int head = (int)((16ull - (g & 15ull)) & 15ull);
+          head = min(head, run_bytes);
+          const int body = (run_bytes - head) & ~15;
+          for (int o = 0; o < head; o += (int)sizeof(T)) *reinterpret_cast<T*>(g + o) = *reinterpret_cast<const T*>(src + o);
+          if (body > 0) bulk_s2g(reinterpret_cast<void*>(g + head), src + head, (uint32_t)body);
+          for (int o = head + body; o < run_bytes; o += (int)sizeof(T))
+            *reinterpret_cast<T*>(g + o) = *reinterpret_cast<const T*>(src + o);
+          bulk_commit();
+        }
       }
-      T* run = reinterpret_cast<T*>(S.tile + S.run_off[ti]);
-#pragma unroll
-      for (int n = 0; n < 3; ++n) {
-        T* blk = run + 9 * er[n];
-#pragma unroll
-        for (int i = 0; i < 3; ++i)
-#pragma unroll
-          for (int j = 0; j < 3; ++j) blk[3 * i + j] = (T)(a[i] * E.g0[9 + 3 * n + j] + b[i] * E.g1[9 + 3 * n + j]);
-      }
-      double* st = S.stage + lane * STG_STRIDE;
-#pragma unroll
-      for (int n = 0; n < 3; ++n)
-#pragma unroll
-        for (int i = 0; i < 3; ++i)
-#pragma unroll
-          for (int j = 0; j < 3; ++j) st[9 * n + 3 * i + j] = a[i] * E.g0[3 * n + j] + b[i] * E.g1[3 * n + j];
-#pragma unroll
-      for (int i = 0; i < 3; ++i) st[27 + i] = E.cf.cg0 * g0m[i] + E.cf.cg1 * g1m[i];
     }
-    __syncwarp();
-    // ---- sum over each triangle's entries, lane = component, entry order ----
-    if (lane < NSTG) {
-      for (int tt = 0; tt < ntri; ++tt) {
-        const int i0 = S.tri_first[tt], i1 = S.tri_first[tt + 1];
-        double acc = 0.0;
-        for (int i = i0; i < i1; ++i) acc += S.stage[i * STG_STRIDE + lane];
-        if (lane < 27) reinterpret_cast<T*>(S.tile + S.run_off[tt])[9 * S.dr[tt][cn] + cq] = (T)acc;
-        else P.tslot[9 * (int64_t)S.tri_id[tt] + 3 * m + (lane - 27)] = (T)acc;
-      }
-    }
-    fence_async_smem();
-    __syncwarp();
-    // ---- lane = triangle: hand the run to the copy engine ----
-    if (lane < ntri) {
-      const unsigned long long g = my_g[m];
-      const unsigned char* src = S.tile + slot_off + (int)(g & 15ull);
-      int head = (int)((16ull - (g & 15ull)) & 15ull);
-      head = min(head, run_bytes);
-      const int body = (run_bytes - head) & ~15;
-      for (int o = 0; o < head; o += (int)sizeof(T)) *reinterpret_cast<T*>(g + o) = *reinterpret_cast<const T*>(src + o);
-      if (body > 0) bulk_s2g(reinterpret_cast<void*>(g + head), src + head, (uint32_t)body);
-      for (int o = head + body; o < run_bytes; o += (int)sizeof(T))
-        *reinterpret_cast<T*>(g + o) = *reinterpret_cast<const T*>(src + o);
-      bulk_commit();
-    }
+    double e_acc = E.en;
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) e_acc += __shfl_down_sync(FULL, e_acc, o);
+    if (lane == 0) P.chunk_energy[c] = e_acc;  // 0 for a long round: k_assemble_long overwrites it
+    if (!has_next) break;
+    c += G;
+    d_cur = d_nxt;
+    d_nxt = d_nn;
+    cur = nxt;
   }
-  double e_acc = E.en;
-#pragma unroll
-  for (int o = 16; o > 0; o >>= 1) e_acc += __shfl_down_sync(FULL, e_acc, o);
-  if (lane == 0) P.chunk_energy[c] = e_acc;
   bulk_wait_all();  // shared memory must outlive the engine's reads
 }
 
 // Long triangles (more than RND_MAX_ENT partners): one warp per triangle, entries in groups of 32,
 // off-diagonal blocks stored directly, diagonal rows and gradient carried across groups.
+// Launched after k_assemble_tile on the same stream (it overwrites that round's energy slot).
 template <typename T>
 __global__ void __launch_bounds__(32 * TILE_WARPS)
 k_assemble_long(const AsmParams<T> P) {
@@ -737,16 +829,16 @@ k_assemble_long(const AsmParams<T> P) {
   const int64_t li = (int64_t)blockIdx.x * TILE_WARPS + warp;
   if (li >= P.n_long) return;
   const int c = __ldg(P.long_list + li);
-  const int ti = __ldg(P.chunk_start + c);
-  const int s = __ldg(P.touched + ti);
-  const int e_lo = __ldg(P.tfirst + ti), e_hi = __ldg(P.tfirst + ti + 1);
+  const int4 d = __ldg(P.rdesc + c);
+  const int64_t ti = d.z;
+  const int e_lo = d.x, e_hi = d.x + d.y;
   T* rowp[3];
   int dr[3];
 #pragma unroll
   for (int m = 0; m < 3; ++m) {
-    const int64_t rb = __ldg(P.rowbase + 3 * (int64_t)s + m);
+    const int64_t rb = __ldg(P.rowbase + 3 * ti + m);
     rowp[m] = (rb >= 0) ? (P.vals + 9 * rb) : (P.tvals + 9 * (-rb - 1));
-    dr[m] = __ldg(P.drank + 3 * (int64_t)s + m);
+    dr[m] = __ldg(P.drank + 3 * ti + m);
   }
   const int cn = (lane < 27) ? lane / 9 : 0, cq = (lane < 27) ? lane % 9 : 0;
   double acc[3] = {0.0, 0.0, 0.0}, e_acc = 0.0;
@@ -756,9 +848,15 @@ k_assemble_long(const AsmParams<T> P) {
     Entry E;
     int er[3] = {0, 0, 0};
     if (valid) {
+      const int64_t e = (int64_t)base + lane;
+      int ids[6];
 #pragma unroll
-      for (int n = 0; n < 3; ++n) er[n] = __ldg(P.erank + 3 * (int64_t)(base + lane) + n);
-      eval_entry(P, base + lane, E);
+      for (int i = 0; i < 6; ++i) ids[i] = __ldg(P.everts + 6 * e + i);
+#pragma unroll
+      for (int n = 0; n < 3; ++n) er[n] = __ldg(P.erank + 3 * e + n);
+      double x[18];
+      load_pos18(P.pos, ids, x);
+      eval_core(x, (unsigned)__ldg(P.dvals + e), P.sigma, P.hess_mode, E);
       e_acc += E.en;
       unpermute_own(E, S.stage + lane * STG_STRIDE, er);
     }
@@ -798,7 +896,7 @@ k_assemble_long(const AsmParams<T> P) {
 #pragma unroll
   for (int m = 0; m < 3; ++m) {
     if (lane < 27) rowp[m][9 * (int64_t)dr[cn] + cq] = (T)acc[m];
-    else if (lane < NSTG) P.tslot[9 * (int64_t)s + 3 * m + (lane - 27)] = (T)acc[m];
+    else if (lane < NSTG) P.tslot[9 * ti + 3 * m + (lane - 27)] = (T)acc[m];
   }
 #pragma unroll
   for (int o = 16; o > 0; o >>= 1) e_acc += __shfl_down_sync(FULL, e_acc, o);
@@ -819,31 +917,45 @@ k_entry_reduce(const AsmParams<T> P) {
   const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
   const int64_t c = (int64_t)blockIdx.x * (RED_THREADS / 32) + warp;
   if (c >= P.n_chunks) return;
-  const int t_lo = __ldg(P.chunk_start + c), t_hi = __ldg(P.chunk_start + c + 1);
-  const int e_lo = __ldg(P.tfirst + t_lo), e_hi = __ldg(P.tfirst + t_hi);
+  const int4 d = __ldg(P.rdesc + c);
+  const int e_lo = d.x, e_hi = d.x + d.y;
   double* stage = s_stage[warp];
   int* src = s_src[warp];
   double acc = 0.0, e_acc = 0.0;
   int cur = -1;
+  int64_t cur_ti = (int64_t)d.z - 1;
   for (int base = e_lo; base < e_hi; base += 32) {
     const int nvalid = min(32, e_hi - base);
     int s = -1;
     if (lane < nvalid) {
+      const int64_t e = (int64_t)base + lane;
+      s = (int)(__ldg(P.keys + e) >> P.bitsT);
+      int ids[6];
+      {
+        const int2* v = reinterpret_cast<const int2*>(P.everts + 6 * e);
+        const int2 v0 = __ldg(v), v1 = __ldg(v + 1), v2 = __ldg(v + 2);
+        ids[0] = v0.x; ids[1] = v0.y; ids[2] = v1.x; ids[3] = v1.y; ids[4] = v2.x; ids[5] = v2.y;
+      }
+      double x[18];
+      load_pos18(P.pos, ids, x);
+      const unsigned pay = (unsigned)__ldg(P.dvals + e);
+      double pv[18];  // p of (own, partner) vertices, recorded order
+      if (MODE == 2) {
+        const bool side = (pay & 1u) != 0u;
+        const int pid[6] = {side ? ids[3] : ids[0], side ? ids[4] : ids[1], side ? ids[5] : ids[2],
+                            side ? ids[0] : ids[3], side ? ids[1] : ids[4], side ? ids[2] : ids[5]};
+        load_pos18(P.pvec, pid, pv);
+      }
       Entry E;
-      eval_entry(P, base + lane, E);
-      s = E.s;
+      eval_core(x, pay, P.sigma, P.hess_mode, E);
       e_acc += E.en;
       double u0 = E.cf.cg0, u1 = E.cf.cg1;  // MODE 1: Eq. 3
       if (MODE == 2) {
         double j0 = 0.0, j1 = 0.0;
 #pragma unroll
-        for (int v = 0; v < 3; ++v) {
-          const d3 pa = load_vertex(P.pvec, E.va[v]);
-          const d3 pb = load_vertex(P.pvec, E.vb[v]);
-          j0 += E.g0[3 * v] * pa.x + E.g0[3 * v + 1] * pa.y + E.g0[3 * v + 2] * pa.z;
-          j0 += E.g0[9 + 3 * v] * pb.x + E.g0[9 + 3 * v + 1] * pb.y + E.g0[9 + 3 * v + 2] * pb.z;
-          j1 += E.g1[3 * v] * pa.x + E.g1[3 * v + 1] * pa.y + E.g1[3 * v + 2] * pa.z;
-          j1 += E.g1[9 + 3 * v] * pb.x + E.g1[9 + 3 * v + 1] * pb.y + E.g1[9 + 3 * v + 2] * pb.z;
+        for (int i = 0; i < 18; ++i) {
+          j0 = fma(E.g0[i], pv[i], j0);
+          j1 = fma(E.g1[i], pv[i], j1);
         }
         u0 = E.cf.c00 * j0 + E.cf.c01 * j1;  // M (J p_loc)
         u1 = E.cf.c01 * j0 + E.cf.c11 * j1;
@@ -859,15 +971,16 @@ k_entry_reduce(const AsmParams<T> P) {
     for (int i = 0; i < nvalid; ++i) {
       const int si = src[i];
       if (si != cur) {  // warp-uniform
-        if (cur >= 0 && lane < 9) P.tslot[9 * (int64_t)cur + lane] = (T)acc;
+        if (cur >= 0 && lane < 9) P.tslot[9 * cur_ti + lane] = (T)acc;
         acc = 0.0;
         cur = si;
+        ++cur_ti;
       }
       if (lane < 9) acc += stage[i * 9 + lane];
     }
     __syncwarp();
   }
-  if (cur >= 0 && lane < 9) P.tslot[9 * (int64_t)cur + lane] = (T)acc;
+  if (cur >= 0 && lane < 9) P.tslot[9 * cur_ti + lane] = (T)acc;
   if (MODE == 1) {
 #pragma unroll
     for (int o = 16; o > 0; o >>= 1) e_acc += __shfl_down_sync(FULL, e_acc, o);

@@ -71,7 +71,7 @@ struct tt_ctx {
   // pattern
   DevBuf rowptr64, rowptr, colind;
   // numeric
-  DevBuf tfirst, bucket_cnt, bucket_off, long_cnt, long_off, chunk_start, long_list, asm_energy, tvals, tslot, vkeys[2], vvals[2], vptr;
+  DevBuf everts, rdesc, tfirst, bucket_cnt, bucket_off, long_cnt, long_off, chunk_start, long_list, asm_energy, tvals, tslot, vkeys[2], vvals[2], vptr;
   DevBuf cub_tmp;
   // host-API mirrors
   DevBuf h_pos, h_tris, h_pairs, h_p, o_vals, o_grad, o_energy, o_y;
@@ -79,6 +79,7 @@ struct tt_ctx {
   Signature sig;
   int64_t A = 0, n_dir = 0, n_touched = 0, R = 0, U = 0, nnzb = 0, n_chunks = 0, n_long = 0, rows_excl = 0, rows_gen = 0;
   int bitsT = 1, bitsV = 1;
+  int tile_grid[2] = {0, 0};  // persistent grid of k_assemble_tile<double / float>
   uint64_t* keys_sorted = nullptr;
   uint16_t* dvals_sorted = nullptr;
   uint64_t* rkeys_sorted = nullptr;
@@ -278,6 +279,11 @@ tt_status symbolic_impl(tt_ctx* ctx, const tt_problem* q, int64_t* nnzb_host, in
     s = sort_pairs(ctx, ctx->keys, ctx->dvals, n, 2 * bitsT, &ctx->keys_sorted, &ctx->dvals_sorted, st);
     if (s != TT_OK) return s;
   }
+  TT_CUDA(ctx->everts.ensure(sizeof(int) * 6 * (size_t)(n + 1)));
+  if (n > 0) {
+    k_ent_verts<<<grid_for(n, 256), 256, 0, st>>>(ctx->keys_sorted, ctx->dvals_sorted, q->tris, n, bitsT, ctx->everts.as<int>());
+    TT_LAUNCH_CHECK();
+  }
   TT_CUDA(ctx->tptr.ensure(sizeof(int) * (size_t)(nT + 2)));
   k_segment_ptr<<<grid_for(n + 1, 256), 256, 0, st>>>(ctx->keys_sorted, n, bitsT, nT, ctx->tptr.as<int>());
   TT_LAUNCH_CHECK();
@@ -308,15 +314,15 @@ tt_status symbolic_impl(tt_ctx* ctx, const tt_problem* q, int64_t* nnzb_host, in
 
   // ---- per-triangle ranks, exclusive rows, general-row workspace sizes ----
   TT_CUDA(ctx->erank.ensure(sizeof(int) * (size_t)(3 * n + 3)));
-  TT_CUDA(ctx->drank.ensure(sizeof(int) * (size_t)(3 * nT + 3)));
+  TT_CUDA(ctx->drank.ensure(sizeof(int) * (size_t)(3 * n_touched + 3)));
   TT_CUDA(ctx->rowlen.ensure(sizeof(int) * (size_t)(nV + 1)));
-  TT_CUDA(ctx->tlen.ensure(sizeof(int64_t) * (size_t)(3 * nT + 1)));
-  TT_CUDA(ctx->toff.ensure(sizeof(int64_t) * (size_t)(3 * nT + 1)));
-  TT_CUDA(ctx->slot_excl.ensure((size_t)(3 * nT + 1)));
-  TT_CUDA(ctx->rowbase.ensure(sizeof(int64_t) * (size_t)(3 * nT + 1)));
+  TT_CUDA(ctx->tlen.ensure(sizeof(int64_t) * (size_t)(3 * n_touched + 1)));
+  TT_CUDA(ctx->toff.ensure(sizeof(int64_t) * (size_t)(3 * n_touched + 1)));
+  TT_CUDA(ctx->slot_excl.ensure((size_t)(3 * n_touched + 1)));
+  TT_CUDA(ctx->rowbase.ensure(sizeof(int64_t) * (size_t)(3 * n_touched + 1)));
   TT_CUDA(cudaMemsetAsync(ctx->rowlen.p, 0, sizeof(int) * (size_t)(nV + 1), st));
-  TT_CUDA(cudaMemsetAsync(ctx->tlen.p, 0, sizeof(int64_t) * (size_t)(3 * nT + 1), st));
-  TT_CUDA(cudaMemsetAsync(ctx->slot_excl.p, 0, (size_t)(3 * nT + 1), st));
+  TT_CUDA(cudaMemsetAsync(ctx->tlen.p, 0, sizeof(int64_t) * (size_t)(3 * n_touched + 1), st));
+  TT_CUDA(cudaMemsetAsync(ctx->slot_excl.p, 0, (size_t)(3 * n_touched + 1), st));
   const unsigned tri_grid = grid_for(n_touched, SYM_WARPS);
   if (n_touched > 0) {
     k_tri_symbolic<<<tri_grid, 32 * SYM_WARPS, 0, st>>>(
@@ -325,10 +331,10 @@ tt_status symbolic_impl(tt_ctx* ctx, const tt_problem* q, int64_t* nnzb_host, in
         ctx->drank.as<int>(), ctx->rowlen.as<int>(), ctx->tlen.as<int64_t>(), ctx->slot_excl.as<uint8_t>());
     TT_LAUNCH_CHECK();
   }
-  s = scan_i64(ctx, ctx->tlen.as<int64_t>(), ctx->toff.as<int64_t>(), 3 * nT + 1, st);
+  s = scan_i64(ctx, ctx->tlen.as<int64_t>(), ctx->toff.as<int64_t>(), 3 * n_touched + 1, st);
   if (s != TT_OK) return s;
   int64_t R = 0;
-  TT_CUDA(cudaMemcpyAsync(&R, ctx->toff.as<int64_t>() + 3 * nT, sizeof(int64_t), cudaMemcpyDeviceToHost, st));
+  TT_CUDA(cudaMemcpyAsync(&R, ctx->toff.as<int64_t>() + 3 * n_touched, sizeof(int64_t), cudaMemcpyDeviceToHost, st));
   TT_CUDA(cudaStreamSynchronize(st));
   if (R >= (int64_t(1) << 31)) return fail(ctx, TT_ERR_INVALID_ARG, "general-row workspace exceeds 2^31 blocks");
   ctx->R = R;
@@ -431,15 +437,18 @@ tt_status symbolic_impl(tt_ctx* ctx, const tt_problem* q, int64_t* nnzb_host, in
     TT_CUDA(cudaStreamSynchronize(st));
     n_chunks = nc32[0];
     n_long = nc32[1];
-    const int nt32 = (int)n_touched;
-    TT_CUDA(cudaMemcpyAsync(ctx->chunk_start.as<int>() + n_chunks, &nt32, sizeof(int), cudaMemcpyHostToDevice, st));
-    TT_CUDA(cudaStreamSynchronize(st));  // nt32 lives on this stack frame
   }
   ctx->n_chunks = n_chunks;
   ctx->n_long = n_long;
+  TT_CUDA(ctx->rdesc.ensure(sizeof(int4) * (size_t)(n_chunks + 1)));
+  if (n_chunks > 0) {
+    k_round_desc<<<grid_for(n_chunks, 256), 256, 0, st>>>(ctx->chunk_start.as<int>(), ctx->tfirst.as<int>(), n_chunks, n_touched,
+                                                          ctx->rdesc.as<int4>());
+    TT_LAUNCH_CHECK();
+  }
   TT_CUDA(ctx->asm_energy.ensure(sizeof(double) * (size_t)(n_chunks + 1)));
   TT_CUDA(ctx->tvals.ensure(sizeof(T) * 9 * (size_t)(R + 1)));
-  TT_CUDA(ctx->tslot.ensure(sizeof(T) * 9 * (size_t)(nT + 1)));
+  TT_CUDA(ctx->tslot.ensure(sizeof(T) * 9 * (size_t)(n_touched + 1)));
   const int64_t nvs = 3 * n_touched;
   for (int i = 0; i < 2; ++i) {
     TT_CUDA(ctx->vkeys[i].ensure(sizeof(uint64_t) * (size_t)(nvs + 1)));
@@ -476,12 +485,11 @@ template <typename T>
 ttk::AsmParams<T> make_params(tt_ctx* ctx, const tt_problem* q) {
   ttk::AsmParams<T> p;
   p.pos = (const T*)q->pos;
-  p.tris = q->tris;
   p.keys = ctx->keys_sorted;
   p.dvals = ctx->dvals_sorted;
-  p.touched = ctx->touched.as<int>();
+  p.everts = ctx->everts.as<int>();
+  p.rdesc = ctx->rdesc.as<int4>();
   p.tfirst = ctx->tfirst.as<int>();
-  p.chunk_start = ctx->chunk_start.as<int>();
   p.long_list = ctx->long_list.as<int>();
   p.erank = ctx->erank.as<int>();
   p.drank = ctx->drank.as<int>();
@@ -520,7 +528,9 @@ tt_status numeric_impl(tt_ctx* ctx, const tt_problem* q, void* energy_sum, void*
     TT_CUDA(cudaEventRecord(ctx->ev[1][0], st));
     if (want_h) {
       const size_t smem = sizeof(TileWarpSmem<T>) * TILE_WARPS;
-      k_assemble_tile<T><<<grid_for(ctx->n_chunks, TILE_WARPS), 32 * TILE_WARPS, smem, st>>>(p);
+      const int64_t full = (ctx->n_chunks + TILE_WARPS - 1) / TILE_WARPS;
+      const int64_t pers = ctx->tile_grid[sizeof(T) == 8 ? 0 : 1];
+      k_assemble_tile<T><<<(unsigned)(full < pers ? full : pers), 32 * TILE_WARPS, smem, st>>>(p);
       if (ctx->n_long > 0) {
         TT_LAUNCH_CHECK();
         k_assemble_long<T><<<grid_for(ctx->n_long, TILE_WARPS), 32 * TILE_WARPS, smem, st>>>(p);
@@ -597,7 +607,13 @@ tt_status tt_create(const tt_options* opt, tt_ctx** out) {
     opt_in((const void*)ttk::k_assemble_long<double>, sizeof(ttk::TileWarpSmem<double>) * ttk::TILE_WARPS);
     opt_in((const void*)ttk::k_assemble_tile<float>, sizeof(ttk::TileWarpSmem<float>) * ttk::TILE_WARPS);
     opt_in((const void*)ttk::k_assemble_long<float>, sizeof(ttk::TileWarpSmem<float>) * ttk::TILE_WARPS);
+    int sms = 0, nb0 = 0, nb1 = 0;
+    if (e == cudaSuccess) e = cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, opt->device);
+    if (e == cudaSuccess) e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&nb0, ttk::k_assemble_tile<double>, 32 * ttk::TILE_WARPS, sizeof(ttk::TileWarpSmem<double>) * ttk::TILE_WARPS);
+    if (e == cudaSuccess) e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&nb1, ttk::k_assemble_tile<float>, 32 * ttk::TILE_WARPS, sizeof(ttk::TileWarpSmem<float>) * ttk::TILE_WARPS);
     if (e != cudaSuccess) { (void)cudaGetLastError(); delete c; return TT_ERR_CUDA; }
+    c->tile_grid[0] = sms * (nb0 > 0 ? nb0 : 1);  // one wave of resident CTAs: the kernel is persistent
+    c->tile_grid[1] = sms * (nb1 > 0 ? nb1 : 1);
   }
   *out = c;
   return TT_OK;
