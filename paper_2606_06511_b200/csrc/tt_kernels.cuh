@@ -593,8 +593,9 @@ __device__ __forceinline__ void bulk_wait_all() { asm volatile("cp.async.bulk.wa
 __device__ __forceinline__ void fence_async_smem() { asm volatile("fence.proxy.async.shared::cta;" ::: "memory"); }
 
 constexpr int TILE_WARPS = 2;             // warps per CTA (independent; sized by shared memory)
-constexpr int STG_STRIDE = 31;            // odd: lane = entry writes and lane = component reads conflict-free
-constexpr int NSTG = 30;                  // 27 diagonal-row values + 3 gradient values per entry and row
+constexpr int STG_STRIDE = 55;            // odd: lane = entry writes and lane = component reads conflict-free
+constexpr int NDIAG = 45;                 // upper triangle of the symmetric 9x9 diagonal block, row-major packed
+constexpr int NSTG = NDIAG + 9;           // + gradient of the three own vertices
 
 template <typename T>
 struct TileCfg {
@@ -606,6 +607,7 @@ template <typename T>
 struct alignas(16) TileWarpSmem {
   unsigned char tile[TileCfg<T>::TILE_BYTES];
   double stage[32 * STG_STRIDE];
+  int tri_first[RND_MAX_TRI + 1];         // first entry (lane) of every triangle of the round
   int run_off[RND_MAX_TRI];               // byte offset of the triangle's run in the tile (current row)
   int diag_off[RND_MAX_TRI][3];           // byte offset of its diagonal block n in the tile (current row)
 };
@@ -717,6 +719,50 @@ k_assemble_tile(const AsmParams<T> P) {
       const unsigned heads = __reduce_or_sync(FULL, (lane < ntri) ? (1u << (cur.e0 - e_lo)) : 0u);
       const int my_ti = __popc(heads & (0xffffffffu >> (31 - lane))) - 1;
 
+      // ---- diagonal 9x9 (symmetric: 45 unique) + gradient: stage per entry, sum per triangle ----
+      if (lane < ntri) S.tri_first[lane] = cur.e0 - e_lo;
+      if (lane == 0) S.tri_first[ntri] = nent;
+      if (valid) {
+        double d0[9], d1[9];
+#pragma unroll
+        for (int i = 0; i < 9; ++i) {
+          d0[i] = E.cf.c00 * E.g0[i] + E.cf.c01 * E.g1[i];
+          d1[i] = E.cf.c01 * E.g0[i] + E.cf.c11 * E.g1[i];
+        }
+        double* st = S.stage + lane * STG_STRIDE;
+        int k = 0;
+#pragma unroll
+        for (int r = 0; r < 9; ++r)
+#pragma unroll
+          for (int q = r; q < 9; ++q, ++k) st[k] = E.g0[r] * d0[q] + E.g1[r] * d1[q];
+#pragma unroll
+        for (int i = 0; i < 9; ++i) st[NDIAG + i] = E.cf.cg0 * E.g0[i] + E.cf.cg1 * E.g1[i];
+      }
+      __syncwarp();
+      // lane = component (two each), entries in order (deterministic); the sums replace the staged
+      // values of the triangle's first entry
+      if (lane < NSTG / 2) {
+        for (int tt = 0; tt < ntri; ++tt) {
+          const int i0 = S.tri_first[tt], i1 = S.tri_first[tt + 1];
+          double* p = S.stage + i0 * STG_STRIDE + lane;
+          double a0 = p[0], a1 = p[NSTG / 2];
+          for (int i = i0 + 1; i < i1; ++i) {
+            const double* pi = S.stage + i * STG_STRIDE + lane;
+            a0 += pi[0];
+            a1 += pi[NSTG / 2];
+          }
+          p[0] = a0;
+          p[NSTG / 2] = a1;
+        }
+      }
+      __syncwarp();
+      // gradient of the round's triangles (lane = component of the 9)
+      if (lane < 9)
+        for (int tt = 0; tt < ntri; ++tt) {
+          const int i0 = S.tri_first[tt];
+          P.tslot[9 * ((int64_t)t_lo + tt) + lane] = (T)S.stage[i0 * STG_STRIDE + NDIAG + lane];
+        }
+
 #pragma unroll
       for (int m = 0; m < 3; ++m) {
         const unsigned long long g =
@@ -732,13 +778,11 @@ k_assemble_tile(const AsmParams<T> P) {
         }
         __syncwarp();
         if (valid) {
-          const double g0m[3] = {E.g0[3 * m], E.g0[3 * m + 1], E.g0[3 * m + 2]};
-          const double g1m[3] = {E.g1[3 * m], E.g1[3 * m + 1], E.g1[3 * m + 2]};
           double a[3], b[3];
 #pragma unroll
           for (int i = 0; i < 3; ++i) {
-            a[i] = E.cf.c00 * g0m[i] + E.cf.c01 * g1m[i];
-            b[i] = E.cf.c01 * g0m[i] + E.cf.c11 * g1m[i];
+            a[i] = E.cf.c00 * E.g0[3 * m + i] + E.cf.c01 * E.g1[3 * m + i];
+            b[i] = E.cf.c01 * E.g0[3 * m + i] + E.cf.c11 * E.g1[3 * m + i];
           }
           T* run = reinterpret_cast<T*>(S.tile + S.run_off[my_ti]);
 #pragma unroll
@@ -749,43 +793,16 @@ k_assemble_tile(const AsmParams<T> P) {
 #pragma unroll
               for (int j = 0; j < 3; ++j) blk[3 * i + j] = (T)(a[i] * E.g0[9 + 3 * n + j] + b[i] * E.g1[9 + 3 * n + j]);
           }
-          double* st = S.stage + lane * STG_STRIDE;
-#pragma unroll
-          for (int n = 0; n < 3; ++n)
-#pragma unroll
-            for (int i = 0; i < 3; ++i)
-#pragma unroll
-              for (int j = 0; j < 3; ++j) st[9 * n + 3 * i + j] = a[i] * E.g0[3 * n + j] + b[i] * E.g1[3 * n + j];
-#pragma unroll
-          for (int i = 0; i < 3; ++i) st[27 + i] = E.cf.cg0 * g0m[i] + E.cf.cg1 * g1m[i];
         }
-        __syncwarp();
-        // ---- sum over each triangle's entries, lane = component, entry order; loads 4 deep ----
-        if (lane < NSTG) {
-          int tt = -1;
-          double acc = 0.0;
-          auto flush = [&](int t_, double v_) {
-            if (lane < 27) *reinterpret_cast<T*>(S.tile + S.diag_off[t_][cn] + cq * (int)sizeof(T)) = (T)v_;
-            else P.tslot[9 * ((int64_t)t_lo + t_) + 3 * m + (lane - 27)] = (T)v_;
-          };
-          for (int i0 = 0; i0 < nent; i0 += 4) {
-            double v[4];
-#pragma unroll
-            for (int u = 0; u < 4; ++u) v[u] = S.stage[min(i0 + u, 31) * STG_STRIDE + lane];
-#pragma unroll
-            for (int u = 0; u < 4; ++u) {
-              const int i = i0 + u;
-              if (i < nent) {
-                if ((heads >> i) & 1u) {
-                  if (tt >= 0) flush(tt, acc);
-                  acc = 0.0;
-                  ++tt;
-                }
-                acc += v[u];
-              }
-            }
+        // diagonal-row blocks (p_m, p_n): lane = element (n, i, j), from the packed upper triangle
+        if (lane < 27) {
+          const int r_ = 3 * m + cq / 3, c_ = 3 * cn + cq % 3;
+          const int lo = min(r_, c_), hi = max(r_, c_);
+          const int uidx = lo * 9 - (lo * (lo - 1)) / 2 + (hi - lo);
+          for (int tt = 0; tt < ntri; ++tt) {
+            const int i0 = S.tri_first[tt];
+            *reinterpret_cast<T*>(S.tile + S.diag_off[tt][cn] + cq * (int)sizeof(T)) = (T)S.stage[i0 * STG_STRIDE + uidx];
           }
-          flush(tt, acc);
         }
         fence_async_smem();
         __syncwarp();
@@ -802,6 +819,7 @@ k_assemble_tile(const AsmParams<T> P) {
           bulk_commit();
         }
       }
+      __syncwarp();  // the next round's spill / staging reuses S.stage
     }
     double e_acc = E.en;
 #pragma unroll
@@ -888,7 +906,7 @@ k_assemble_long(const AsmParams<T> P) {
         for (int i = 0; i < 3; ++i) st[27 + i] = E.cf.cg0 * E.g0[3 * m + i] + E.cf.cg1 * E.g1[3 * m + i];
       }
       __syncwarp();
-      if (lane < NSTG)
+      if (lane < 30)
         for (int i = 0; i < nvalid; ++i) acc[m] += S.stage[i * STG_STRIDE + lane];
       __syncwarp();
     }
@@ -896,7 +914,7 @@ k_assemble_long(const AsmParams<T> P) {
 #pragma unroll
   for (int m = 0; m < 3; ++m) {
     if (lane < 27) rowp[m][9 * (int64_t)dr[cn] + cq] = (T)acc[m];
-    else if (lane < NSTG) P.tslot[9 * ti + 3 * m + (lane - 27)] = (T)acc[m];
+    else if (lane < 30) P.tslot[9 * ti + 3 * m + (lane - 27)] = (T)acc[m];
   }
 #pragma unroll
   for (int o = 16; o > 0; o >>= 1) e_acc += __shfl_down_sync(FULL, e_acc, o);
