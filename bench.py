@@ -301,12 +301,13 @@ def main():
     asm_ms = float(np.mean(kms["assemble"]))
     achieved = alg_bytes / (asm_ms * 1e-3) / 1e9
     traffic = None
-    tpath = os.path.join(ROOT, "profiles", "k_assemble_traffic.json")
+    tpath = os.path.join(ROOT, "profiles", "k_assemble_traffic.csv")   # ncu dram bytes per launch, same workload
     if os.path.exists(tpath):
+        import csv
         with open(tpath) as f:
-            tj = json.load(f)
-        if tj.get("pairs") == args.pairs and tj.get("dtype") == args.dtype:
-            traffic = tj.get("dram_bytes_per_launch")
+            for row in csv.DictReader(f):
+                if int(row["pairs"]) == args.pairs and row["dtype"] == args.dtype:
+                    traffic = int(row["dram_bytes_per_launch"])
     roofline = {"bound": "hbm", "kernel": "k_assemble", "achieved": achieved, "peak": hbm, "unit": "GB/s",
                 "frac": achieved / hbm, "traffic": traffic, "peak_source": peak_src,
                 "algorithmic_bytes_per_launch": int(alg_bytes), "kernel_ms": asm_ms,
