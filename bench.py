@@ -107,10 +107,30 @@ class ClockSampler:
                 "reasons": sorted(reasons), "samples": len(sm)}
 
 
+def aggregate_ranks(ms_local, pairs_local, world, device="cpu"):
+    """Whole-job numbers of N independent replicas: time = MAX over ranks,
+    pairs = SUM over ranks.  One all-reduce each, outside the timed region; backend-agnostic
+    (nccl on the GPU box, gloo in tests/test_bench_ranks.py)."""
+    if world <= 1:
+        return float(ms_local), float(pairs_local)
+    import torch
+    import torch.distributed as dist
+    t = torch.tensor([float(ms_local)], dtype=torch.float64, device=device)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    n = torch.tensor([float(pairs_local)], dtype=torch.float64, device=device)
+    dist.all_reduce(n, op=dist.ReduceOp.SUM)
+    return float(t.item()), float(n.item())
+
+
+def rank_seed(base_seed, rank):
+    """Every replica works on its own seeded batch."""
+    return base_seed + 1000 * rank
+
+
 def make_problem(args, rank, device):
     from paper_2606_06511_b200 import inputs
     t = time.time()
-    pb = inputs.config4_sweep(n_tris=args.tris, n_pairs=args.pairs, seed=inputs.BASE_SEED + 4 + 1000 * rank,
+    pb = inputs.config4_sweep(n_tris=args.tris, n_pairs=args.pairs, seed=rank_seed(inputs.BASE_SEED + 4, rank),
                               device=device)
     log("[bench] rank %d generated %s: nV=%d nT=%d P=%d in %.1fs" % (rank, pb.name, pb.n_verts, pb.n_tris, pb.n_pairs,
                                                                     time.time() - t))
@@ -239,15 +259,7 @@ def main():
     t_wall1 = time.time()
     launches = ctx.tt_stats()["launches"] - l0
     ms_total = ev0.elapsed_time(ev1)
-    if world > 1:
-        tmax = torch.tensor([ms_total], dtype=torch.float64, device=dev)
-        dist.all_reduce(tmax, op=dist.ReduceOp.MAX)
-        ms_total = float(tmax.item())
-        ptot = torch.tensor([float(P)], dtype=torch.float64, device=dev)
-        dist.all_reduce(ptot, op=dist.ReduceOp.SUM)
-        P_all = float(ptot.item())
-    else:
-        P_all = float(P)
+    ms_total, P_all = aggregate_ranks(ms_total, P, world, dev)
     clocks = sampler.stop(t_wall0, t_wall1) if sampler else None
     ms_step = ms_total / args.steps
     value = P_all / (ms_step * 1e-3)
