@@ -222,11 +222,13 @@ k_tri_symbolic(const int* __restrict__ tris, const int* __restrict__ touched, in
                const int* __restrict__ tptr, const uint64_t* __restrict__ keys, int bitsT,
                const int* __restrict__ vcnt, int force_general, int* __restrict__ erank /*[2A][3]*/,
                int* __restrict__ drank /*[n_touched][3]*/, int* __restrict__ rowlen,
-               int64_t* __restrict__ tlen /*[3 n_touched]*/, uint8_t* __restrict__ slot_excl /*[3 n_touched]*/) {
+               int64_t* __restrict__ tlen /*[3 n_touched]*/, uint8_t* __restrict__ slot_excl /*[3 n_touched]*/,
+               const int* __restrict__ long_list, const int4* __restrict__ rdesc) {
   __shared__ int s_c[SYM_WARPS][SYM_LMAX];
   const int w = threadIdx.x >> 5, l = threadIdx.x & 31;
-  const int64_t ti = (int64_t)blockIdx.x * SYM_WARPS + w;
-  if (ti >= n_touched) return;
+  const int64_t li = (int64_t)blockIdx.x * SYM_WARPS + w;  // n_touched counts the LONG triangles here
+  if (li >= n_touched) return;
+  const int64_t ti = rdesc[long_list[li]].z;
   const int s = touched[ti];
   const int e0 = tptr[s], deg = tptr[s + 1] - e0;
   const int L = 3 * (deg + 1);
@@ -338,10 +340,12 @@ k_fill_rows(const int* __restrict__ tris, const int* __restrict__ touched, int64
             const int* __restrict__ tptr, const uint64_t* __restrict__ keys, int bitsT,
             const int* __restrict__ erank, const int* __restrict__ drank, const int64_t* __restrict__ toff,
             const uint8_t* __restrict__ slot_excl, const int* __restrict__ rowptr,
-            int64_t* __restrict__ rowbase /*[3 n_touched]*/, int* __restrict__ colind) {
+            int64_t* __restrict__ rowbase /*[3 n_touched]*/, int* __restrict__ colind,
+            const int* __restrict__ long_list, const int4* __restrict__ rdesc) {
   const int w = threadIdx.x >> 5, l = threadIdx.x & 31;
-  const int64_t ti = (int64_t)blockIdx.x * SYM_WARPS + w;
-  if (ti >= n_touched) return;
+  const int64_t li = (int64_t)blockIdx.x * SYM_WARPS + w;  // n_touched counts the LONG triangles here
+  if (li >= n_touched) return;
+  const int64_t ti = rdesc[long_list[li]].z;
   const int s = touched[ti];
   const int e0 = tptr[s], deg = tptr[s + 1] - e0;
   const int L = 3 * (deg + 1);
@@ -516,6 +520,216 @@ __global__ void k_round_desc(const int* __restrict__ chunk_start, const int* __r
   const int t1 = (c + 1 < n_chunks) ? chunk_start[c + 1] : (int)n_touched;
   const int e0 = tfirst[t0];
   rdesc[c] = make_int4(e0, tfirst[t1] - e0, t0, t1 - t0);
+}
+
+// ---- round-based symbolic kernels (one warp per round, lane = directed entry) -------------------
+// Same results as k_tri_symbolic / k_ent_verts / k_fill_rows, which remain for LONG triangles (more
+// than RND_MAX_ENT partners): a warp owns a round of whole triangles, so every gather is one lane
+// wide and 32 entries deep instead of one warp per (on average 5-entry) triangle.
+constexpr int RSYM_WARPS = 4;
+
+__device__ __forceinline__ int pick3(int i, int v0, int v1, int v2) { return i == 0 ? v0 : (i == 1 ? v1 : v2); }
+
+// Column ranks (erank / drank), duplicate detection, exclusive rows, row lengths and the per-entry
+// vertex ids (everts) of every non-long round.
+__global__ void __launch_bounds__(32 * RSYM_WARPS)
+k_round_symbolic(const int* __restrict__ tris, const int* __restrict__ touched, const int4* __restrict__ rdesc,
+                 int64_t n_chunks, const int* __restrict__ tfirst, const uint64_t* __restrict__ keys,
+                 const uint16_t* __restrict__ dvals, int bitsT, const int* __restrict__ vcnt, int force_general,
+                 int* __restrict__ erank, int* __restrict__ drank, int* __restrict__ rowlen,
+                 int64_t* __restrict__ tlen, uint8_t* __restrict__ slot_excl, int* __restrict__ everts) {
+  __shared__ int s_cand[RSYM_WARPS][3 * RND_MAX_ENT];  // partner vertex ids of entry i at [3 i + n]
+  __shared__ int s_own[RSYM_WARPS][3 * RND_MAX_TRI];   // own vertex ids of triangle tt at [3 tt + n]
+  __shared__ int s_first[RSYM_WARPS][RND_MAX_TRI + 1];
+  __shared__ int s_dup[RSYM_WARPS][RND_MAX_TRI];
+  constexpr unsigned FULL = 0xffffffffu;
+  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+  const int64_t c = (int64_t)blockIdx.x * RSYM_WARPS + warp;
+  if (c >= n_chunks) return;
+  const int4 d = __ldg(rdesc + c);
+  const int e_lo = d.x, nent = d.y, t_lo = d.z, ntri = d.w;
+  if (nent > RND_MAX_ENT) return;  // long triangle: k_tri_symbolic
+  int* cand = s_cand[warp];
+  int* own = s_own[warp];
+  int* first = s_first[warp];
+  int* dupf = s_dup[warp];
+  const uint64_t tmask = (1ull << bitsT) - 1ull;
+  // lane = triangle
+  int f = 0, l = 0, ov[3] = {0, 0, 0};
+  if (lane < ntri) {
+    const int s = __ldg(touched + t_lo + lane);
+    f = __ldg(tfirst + t_lo + lane) - e_lo;
+    l = __ldg(tfirst + t_lo + lane + 1) - e_lo;
+#pragma unroll
+    for (int n = 0; n < 3; ++n) {
+      ov[n] = __ldg(tris + 3 * (int64_t)s + n);
+      own[3 * lane + n] = ov[n];
+    }
+    first[lane] = f;
+    dupf[lane] = 0;
+  }
+  if (lane == 0) first[ntri] = nent;
+  // lane = entry
+  const bool valid = lane < nent;
+  int cv[3] = {0, 0, 0};
+  unsigned pay = 0u;
+  if (valid) {
+    const int64_t e = (int64_t)e_lo + lane;
+    const int t = (int)(__ldg(keys + e) & tmask);
+    pay = (unsigned)__ldg(dvals + e);
+#pragma unroll
+    for (int n = 0; n < 3; ++n) {
+      cv[n] = __ldg(tris + 3 * (int64_t)t + n);
+      cand[3 * lane + n] = cv[n];
+    }
+  }
+  const unsigned heads = __reduce_or_sync(FULL, (lane < ntri) ? (1u << f) : 0u);
+  const int my_ti = __popc(heads & (0xffffffffu >> (31 - lane))) - 1;
+  __syncwarp();
+  // ranks of the entry's three partner columns among the triangle's 3 (deg + 1) candidates
+  int r[3] = {0, 0, 0}, eq[3] = {0, 0, 0};
+  int myf = 0, deg = 0;
+  if (valid) {
+    myf = first[my_ti];
+    deg = first[my_ti + 1] - myf;
+  }
+  const int maxdeg = __reduce_max_sync(FULL, deg);
+  for (int k = 0; k < maxdeg; ++k) {
+    if (k < deg) {
+      const int* o = cand + 3 * (myf + k);
+      const int o0 = o[0], o1 = o[1], o2 = o[2];
+#pragma unroll
+      for (int n = 0; n < 3; ++n) {
+        r[n] += (o0 < cv[n]) + (o1 < cv[n]) + (o2 < cv[n]);
+        eq[n] += (o0 == cv[n]) + (o1 == cv[n]) + (o2 == cv[n]);
+      }
+    }
+  }
+  int mo[3] = {0, 0, 0};  // own vertex ids of the entry's triangle
+  if (valid) {
+#pragma unroll
+    for (int n = 0; n < 3; ++n) mo[n] = own[3 * my_ti + n];
+#pragma unroll
+    for (int n = 0; n < 3; ++n) {
+      r[n] += (mo[0] < cv[n]) + (mo[1] < cv[n]) + (mo[2] < cv[n]);
+      eq[n] += (mo[0] == cv[n]) + (mo[1] == cv[n]) + (mo[2] == cv[n]);
+    }
+    if (eq[0] > 1 || eq[1] > 1 || eq[2] > 1) dupf[my_ti] = 1;  // eq counts the column itself once
+  }
+  // ranks of the diagonal columns: lane = triangle
+  int dr[3] = {0, 0, 0};
+  if (lane < ntri) {
+    int dq[3] = {0, 0, 0};
+    for (int k = f; k < l; ++k) {
+      const int o0 = cand[3 * k], o1 = cand[3 * k + 1], o2 = cand[3 * k + 2];
+#pragma unroll
+      for (int n = 0; n < 3; ++n) {
+        dr[n] += (o0 < ov[n]) + (o1 < ov[n]) + (o2 < ov[n]);
+        dq[n] += (o0 == ov[n]) + (o1 == ov[n]) + (o2 == ov[n]);
+      }
+    }
+#pragma unroll
+    for (int n = 0; n < 3; ++n) {
+      dr[n] += (ov[0] < ov[n]) + (ov[1] < ov[n]) + (ov[2] < ov[n]);
+      dq[n] += (ov[0] == ov[n]) + (ov[1] == ov[n]) + (ov[2] == ov[n]);
+    }
+    if (dq[0] > 1 || dq[1] > 1 || dq[2] > 1) dupf[lane] = 1;
+  }
+  __syncwarp();
+  if (valid) {
+    const int64_t e = (int64_t)e_lo + lane;
+    const bool nodup = dupf[my_ti] == 0;
+    const int j = lane - myf;
+#pragma unroll
+    for (int n = 0; n < 3; ++n) erank[3 * e + n] = nodup ? r[n] : 3 * j + n;
+    // vertex ids of the canonical pair, both triangles in recorded (k, p, q) order
+    const bool side = (pay & 1u) != 0u;
+    const unsigned ca = (pay >> 1) & 63u, cb = (pay >> 7) & 63u;
+    const int ka = (int)(ca & 3u), pa = (int)((ca >> 2) & 3u), kb = (int)(cb & 3u), pb = (int)((cb >> 2) & 3u);
+    const int a0 = side ? cv[0] : mo[0], a1 = side ? cv[1] : mo[1], a2 = side ? cv[2] : mo[2];
+    const int b0 = side ? mo[0] : cv[0], b1 = side ? mo[1] : cv[1], b2 = side ? mo[2] : cv[2];
+    int2* o = reinterpret_cast<int2*>(everts + 6 * e);
+    o[0] = make_int2(pick3(ka, a0, a1, a2), pick3(pa, a0, a1, a2));
+    o[1] = make_int2(pick3(3 - ka - pa, a0, a1, a2), pick3(kb, b0, b1, b2));
+    o[2] = make_int2(pick3(pb, b0, b1, b2), pick3(3 - kb - pb, b0, b1, b2));
+  }
+  if (lane < ntri) {
+    const int64_t ti = (int64_t)t_lo + lane;
+    const bool nodup = dupf[lane] == 0;
+    const int dg = l - f, L = 3 * (dg + 1);
+#pragma unroll
+    for (int n = 0; n < 3; ++n) drank[3 * ti + n] = nodup ? dr[n] : 3 * dg + n;
+#pragma unroll
+    for (int m = 0; m < 3; ++m) {
+      const bool excl = nodup && !force_general && (__ldg(vcnt + ov[m]) == 1);
+      slot_excl[3 * ti + m] = excl ? 1 : 0;
+      tlen[3 * ti + m] = excl ? 0 : L;
+      if (excl) rowlen[ov[m]] = L;
+    }
+  }
+}
+
+// Column indices of the exclusive rows + row bases of every non-long round (after the rowptr scan).
+__global__ void __launch_bounds__(32 * RSYM_WARPS)
+k_round_fill(const int* __restrict__ tris, const int* __restrict__ touched, const int4* __restrict__ rdesc,
+             int64_t n_chunks, const int* __restrict__ tfirst, const uint64_t* __restrict__ keys, int bitsT,
+             const int* __restrict__ erank, const int* __restrict__ drank, const int64_t* __restrict__ toff,
+             const uint8_t* __restrict__ slot_excl, const int* __restrict__ rowptr,
+             int64_t* __restrict__ rowbase, int* __restrict__ colind) {
+  __shared__ int s_rp[RSYM_WARPS][3 * RND_MAX_TRI];  // first block of row m of triangle tt, or -1
+  constexpr unsigned FULL = 0xffffffffu;
+  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+  const int64_t c = (int64_t)blockIdx.x * RSYM_WARPS + warp;
+  if (c >= n_chunks) return;
+  const int4 d = __ldg(rdesc + c);
+  const int e_lo = d.x, nent = d.y, t_lo = d.z, ntri = d.w;
+  if (nent > RND_MAX_ENT) return;  // long triangle: k_fill_rows
+  int* rps = s_rp[warp];
+  const uint64_t tmask = (1ull << bitsT) - 1ull;
+  int f = 0;
+  if (lane < ntri) {
+    const int64_t ti = (int64_t)t_lo + lane;
+    const int s = __ldg(touched + ti);
+    f = __ldg(tfirst + ti) - e_lo;
+    int ov[3], dr[3];
+#pragma unroll
+    for (int n = 0; n < 3; ++n) {
+      ov[n] = __ldg(tris + 3 * (int64_t)s + n);
+      dr[n] = __ldg(drank + 3 * ti + n);
+    }
+#pragma unroll
+    for (int m = 0; m < 3; ++m) {
+      const bool excl = slot_excl[3 * ti + m] != 0;
+      const int rp = excl ? __ldg(rowptr + ov[m]) : -1;
+      rps[3 * lane + m] = rp;
+      rowbase[3 * ti + m] = excl ? (int64_t)rp : -(toff[3 * ti + m] + 1);
+      if (excl) {
+#pragma unroll
+        for (int n = 0; n < 3; ++n) colind[rp + dr[n]] = ov[n];
+      }
+    }
+  }
+  const unsigned heads = __reduce_or_sync(FULL, (lane < ntri) ? (1u << f) : 0u);
+  const int my_ti = __popc(heads & (0xffffffffu >> (31 - lane))) - 1;
+  __syncwarp();
+  if (lane < nent) {
+    const int64_t e = (int64_t)e_lo + lane;
+    const int t = (int)(__ldg(keys + e) & tmask);
+    int cv[3], er[3];
+#pragma unroll
+    for (int n = 0; n < 3; ++n) {
+      cv[n] = __ldg(tris + 3 * (int64_t)t + n);
+      er[n] = __ldg(erank + 3 * e + n);
+    }
+#pragma unroll
+    for (int m = 0; m < 3; ++m) {
+      const int rp = rps[3 * my_ti + m];
+      if (rp >= 0) {
+#pragma unroll
+        for (int n = 0; n < 3; ++n) colind[rp + er[n]] = cv[n];
+      }
+    }
+  }
 }
 
 template <typename T>

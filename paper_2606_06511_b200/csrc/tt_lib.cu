@@ -177,14 +177,14 @@ tt_status incl_scan_i32(tt_ctx* ctx, const int* in, int* out, int64_t n, cudaStr
 }
 // stable LSD radix sort of (key, payload) on bits [0, end_bit); result pointers returned
 template <typename V>
-tt_status sort_pairs(tt_ctx* ctx, DevBuf (&kb)[2], DevBuf (&vb)[2], int64_t n, int end_bit,
+tt_status sort_pairs(tt_ctx* ctx, DevBuf (&kb)[2], DevBuf (&vb)[2], int64_t n, int begin_bit, int end_bit,
                      uint64_t** k_out, V** v_out, cudaStream_t st) {
   cub::DoubleBuffer<uint64_t> dk(kb[0].as<uint64_t>(), kb[1].as<uint64_t>());
   cub::DoubleBuffer<V> dv(vb[0].as<V>(), vb[1].as<V>());
   size_t tmp = 0;
-  TT_CUDA(cub::DeviceRadixSort::SortPairs(nullptr, tmp, dk, dv, n, 0, end_bit, st));
+  TT_CUDA(cub::DeviceRadixSort::SortPairs(nullptr, tmp, dk, dv, n, begin_bit, end_bit, st));
   TT_CUDA(ctx->cub_tmp.ensure(tmp));
-  TT_CUDA(cub::DeviceRadixSort::SortPairs(ctx->cub_tmp.p, tmp, dk, dv, n, 0, end_bit, st));
+  TT_CUDA(cub::DeviceRadixSort::SortPairs(ctx->cub_tmp.p, tmp, dk, dv, n, begin_bit, end_bit, st));
   ctx->launches++;
   *k_out = dk.Current();
   *v_out = dv.Current();
@@ -276,14 +276,12 @@ tt_status symbolic_impl(tt_ctx* ctx, const tt_problem* q, int64_t* nnzb_host, in
     k_emit_directed<<<grid_for(A, 256), 256, 0, st>>>((const int2*)q->pairs, ctx->active_ids.as<int>(), ctx->cfg.as<uint16_t>(), A, bitsT,
                                                       ctx->keys[0].as<uint64_t>(), ctx->dvals[0].as<uint16_t>());
     TT_LAUNCH_CHECK();
-    s = sort_pairs(ctx, ctx->keys, ctx->dvals, n, 2 * bitsT, &ctx->keys_sorted, &ctx->dvals_sorted, st);
+    // stable sort on the SOURCE bits only: a triangle's entries become contiguous, in active-pair
+    // order (deterministic); nothing downstream needs the partners ascending (columns are ranked)
+    s = sort_pairs(ctx, ctx->keys, ctx->dvals, n, bitsT, 2 * bitsT, &ctx->keys_sorted, &ctx->dvals_sorted, st);
     if (s != TT_OK) return s;
   }
   TT_CUDA(ctx->everts.ensure(sizeof(int) * 6 * (size_t)(n + 1)));
-  if (n > 0) {
-    k_ent_verts<<<grid_for(n, 256), 256, 0, st>>>(ctx->keys_sorted, ctx->dvals_sorted, q->tris, n, bitsT, ctx->everts.as<int>());
-    TT_LAUNCH_CHECK();
-  }
   TT_CUDA(ctx->tptr.ensure(sizeof(int) * (size_t)(nT + 2)));
   k_segment_ptr<<<grid_for(n + 1, 256), 256, 0, st>>>(ctx->keys_sorted, n, bitsT, nT, ctx->tptr.as<int>());
   TT_LAUNCH_CHECK();
@@ -312,97 +310,7 @@ tt_status symbolic_impl(tt_ctx* ctx, const tt_problem* q, int64_t* nnzb_host, in
   }
   ctx->n_touched = n_touched;
 
-  // ---- per-triangle ranks, exclusive rows, general-row workspace sizes ----
-  TT_CUDA(ctx->erank.ensure(sizeof(int) * (size_t)(3 * n + 3)));
-  TT_CUDA(ctx->drank.ensure(sizeof(int) * (size_t)(3 * n_touched + 3)));
-  TT_CUDA(ctx->rowlen.ensure(sizeof(int) * (size_t)(nV + 1)));
-  TT_CUDA(ctx->tlen.ensure(sizeof(int64_t) * (size_t)(3 * n_touched + 1)));
-  TT_CUDA(ctx->toff.ensure(sizeof(int64_t) * (size_t)(3 * n_touched + 1)));
-  TT_CUDA(ctx->slot_excl.ensure((size_t)(3 * n_touched + 1)));
-  TT_CUDA(ctx->rowbase.ensure(sizeof(int64_t) * (size_t)(3 * n_touched + 1)));
-  TT_CUDA(cudaMemsetAsync(ctx->rowlen.p, 0, sizeof(int) * (size_t)(nV + 1), st));
-  TT_CUDA(cudaMemsetAsync(ctx->tlen.p, 0, sizeof(int64_t) * (size_t)(3 * n_touched + 1), st));
-  TT_CUDA(cudaMemsetAsync(ctx->slot_excl.p, 0, (size_t)(3 * n_touched + 1), st));
-  const unsigned tri_grid = grid_for(n_touched, SYM_WARPS);
-  if (n_touched > 0) {
-    k_tri_symbolic<<<tri_grid, 32 * SYM_WARPS, 0, st>>>(
-        q->tris, ctx->touched.as<int>(), n_touched, ctx->tptr.as<int>(), ctx->keys_sorted, bitsT,
-        ctx->vcnt.as<int>(), (ctx->opt.flags & TT_FLAG_FORCE_GENERAL_ROWS) ? 1 : 0, ctx->erank.as<int>(),
-        ctx->drank.as<int>(), ctx->rowlen.as<int>(), ctx->tlen.as<int64_t>(), ctx->slot_excl.as<uint8_t>());
-    TT_LAUNCH_CHECK();
-  }
-  s = scan_i64(ctx, ctx->tlen.as<int64_t>(), ctx->toff.as<int64_t>(), 3 * n_touched + 1, st);
-  if (s != TT_OK) return s;
-  int64_t R = 0;
-  TT_CUDA(cudaMemcpyAsync(&R, ctx->toff.as<int64_t>() + 3 * n_touched, sizeof(int64_t), cudaMemcpyDeviceToHost, st));
-  TT_CUDA(cudaStreamSynchronize(st));
-  if (R >= (int64_t(1) << 31)) return fail(ctx, TT_ERR_INVALID_ARG, "general-row workspace exceeds 2^31 blocks");
-  ctx->R = R;
-
-  // ---- general rows: merge records sorted by (row, col) ----
-  int64_t U = 0;
-  ctx->rkeys_sorted = nullptr;
-  ctx->rvals_sorted = nullptr;
-  if (R > 0) {
-    for (int i = 0; i < 2; ++i) {
-      TT_CUDA(ctx->rkeys[i].ensure(sizeof(uint64_t) * (size_t)R));
-      TT_CUDA(ctx->rvals[i].ensure(sizeof(uint32_t) * (size_t)R));
-    }
-    TT_CUDA(ctx->head.ensure(sizeof(int) * (size_t)R));
-    TT_CUDA(ctx->ord.ensure(sizeof(int) * (size_t)R));
-    TT_CUDA(ctx->rowfirst.ensure(sizeof(int) * (size_t)(nV + 1)));
-    TT_CUDA(ctx->run_start.ensure(sizeof(int) * (size_t)(R + 1)));
-    TT_CUDA(ctx->run_dest.ensure(sizeof(int) * (size_t)(R + 1)));
-    k_emit_records<<<tri_grid, 32 * SYM_WARPS, 0, st>>>(
-        q->tris, ctx->touched.as<int>(), n_touched, ctx->tptr.as<int>(), ctx->keys_sorted, bitsT, bitsV,
-        ctx->erank.as<int>(), ctx->drank.as<int>(), ctx->toff.as<int64_t>(), ctx->slot_excl.as<uint8_t>(),
-        ctx->rkeys[0].as<uint64_t>(), ctx->rvals[0].as<uint32_t>());
-    TT_LAUNCH_CHECK();
-    s = sort_pairs(ctx, ctx->rkeys, ctx->rvals, R, 2 * bitsV, &ctx->rkeys_sorted, &ctx->rvals_sorted, st);
-    if (s != TT_OK) return s;
-    k_record_heads<<<grid_for(R, 256), 256, 0, st>>>(ctx->rkeys_sorted, R, ctx->head.as<int>());
-    TT_LAUNCH_CHECK();
-    s = incl_scan_i32(ctx, ctx->head.as<int>(), ctx->ord.as<int>(), R, st);
-    if (s != TT_OK) return s;
-    k_record_rows<<<grid_for(R, 256), 256, 0, st>>>(ctx->rkeys_sorted, R, bitsV, ctx->head.as<int>(),
-                                                    ctx->ord.as<int>(), ctx->rowlen.as<int>(),
-                                                    ctx->rowfirst.as<int>(), ctx->run_start.as<int>());
-    TT_LAUNCH_CHECK();
-    int u32 = 0;
-    TT_CUDA(cudaMemcpyAsync(&u32, ctx->ord.as<int>() + (R - 1), sizeof(int), cudaMemcpyDeviceToHost, st));
-    TT_CUDA(cudaStreamSynchronize(st));
-    U = u32;
-  }
-  ctx->U = U;
-
-  // ---- row pointers ----
-  TT_CUDA(ctx->rowptr64.ensure(sizeof(int64_t) * (size_t)(nV + 1)));
-  TT_CUDA(ctx->rowptr.ensure(sizeof(int) * (size_t)(nV + 1)));
-  s = scan_i32_to_i64(ctx, ctx->rowlen.as<int>(), ctx->rowptr64.as<int64_t>(), nV + 1, st);
-  if (s != TT_OK) return s;
-  int64_t nnzb = 0;
-  TT_CUDA(cudaMemcpyAsync(&nnzb, ctx->rowptr64.as<int64_t>() + nV, sizeof(int64_t), cudaMemcpyDeviceToHost, st));
-  TT_CUDA(cudaStreamSynchronize(st));
-  if (nnzb >= (int64_t(1) << 31)) return fail(ctx, TT_ERR_INVALID_ARG, "nnzb %lld exceeds int32 BSR indexing", (long long)nnzb);
-  ctx->nnzb = nnzb;
-  k_i64_to_i32<<<grid_for(nV + 1, 256), 256, 0, st>>>(ctx->rowptr64.as<int64_t>(), nV + 1, ctx->rowptr.as<int>());
-  TT_LAUNCH_CHECK();
-  TT_CUDA(ctx->colind.ensure(sizeof(int) * (size_t)(nnzb + 1)));
-  if (U > 0) {
-    k_record_dest<<<grid_for(U + 1, 256), 256, 0, st>>>(ctx->rkeys_sorted, U, R, bitsV, ctx->run_start.as<int>(),
-                                                        ctx->rowptr.as<int>(), ctx->rowfirst.as<int>(),
-                                                        ctx->run_dest.as<int>(), ctx->colind.as<int>());
-    TT_LAUNCH_CHECK();
-  }
-  if (n_touched > 0) {
-    k_fill_rows<<<tri_grid, 32 * SYM_WARPS, 0, st>>>(
-        q->tris, ctx->touched.as<int>(), n_touched, ctx->tptr.as<int>(), ctx->keys_sorted, bitsT,
-        ctx->erank.as<int>(), ctx->drank.as<int>(), ctx->toff.as<int64_t>(), ctx->slot_excl.as<uint8_t>(),
-        ctx->rowptr.as<int>(), ctx->rowbase.as<int64_t>(), ctx->colind.as<int>());
-    TT_LAUNCH_CHECK();
-  }
-
-  // ---- numeric-phase work partition, per-slot buffers, vertex -> slot incidence ----
+  // ---- work partition shared by the symbolic round kernels, K4 and K6 ----
   // rounds: greedy packing of whole touched triangles (<= 32 entries, <= 16 triangles per round)
   int64_t n_chunks = 0, n_long = 0;
   TT_CUDA(ctx->tfirst.ensure(sizeof(int) * (size_t)(n_touched + 2)));
@@ -446,6 +354,117 @@ tt_status symbolic_impl(tt_ctx* ctx, const tt_problem* q, int64_t* nnzb_host, in
                                                           ctx->rdesc.as<int4>());
     TT_LAUNCH_CHECK();
   }
+  // ---- per-triangle ranks, exclusive rows, general-row workspace sizes ----
+  TT_CUDA(ctx->erank.ensure(sizeof(int) * (size_t)(3 * n + 3)));
+  TT_CUDA(ctx->drank.ensure(sizeof(int) * (size_t)(3 * n_touched + 3)));
+  TT_CUDA(ctx->rowlen.ensure(sizeof(int) * (size_t)(nV + 1)));
+  TT_CUDA(ctx->tlen.ensure(sizeof(int64_t) * (size_t)(3 * n_touched + 1)));
+  TT_CUDA(ctx->toff.ensure(sizeof(int64_t) * (size_t)(3 * n_touched + 1)));
+  TT_CUDA(ctx->slot_excl.ensure((size_t)(3 * n_touched + 1)));
+  TT_CUDA(ctx->rowbase.ensure(sizeof(int64_t) * (size_t)(3 * n_touched + 1)));
+  TT_CUDA(cudaMemsetAsync(ctx->rowlen.p, 0, sizeof(int) * (size_t)(nV + 1), st));
+  TT_CUDA(cudaMemsetAsync(ctx->tlen.p, 0, sizeof(int64_t) * (size_t)(3 * n_touched + 1), st));
+  TT_CUDA(cudaMemsetAsync(ctx->slot_excl.p, 0, (size_t)(3 * n_touched + 1), st));
+  const unsigned tri_grid = grid_for(n_touched, SYM_WARPS);
+  const unsigned rnd_grid = grid_for(n_chunks, RSYM_WARPS);
+  if (n_chunks > 0) {
+    k_round_symbolic<<<rnd_grid, 32 * RSYM_WARPS, 0, st>>>(
+        q->tris, ctx->touched.as<int>(), ctx->rdesc.as<int4>(), n_chunks, ctx->tfirst.as<int>(), ctx->keys_sorted,
+        ctx->dvals_sorted, bitsT, ctx->vcnt.as<int>(), (ctx->opt.flags & TT_FLAG_FORCE_GENERAL_ROWS) ? 1 : 0,
+        ctx->erank.as<int>(), ctx->drank.as<int>(), ctx->rowlen.as<int>(), ctx->tlen.as<int64_t>(),
+        ctx->slot_excl.as<uint8_t>(), ctx->everts.as<int>());
+    TT_LAUNCH_CHECK();
+  }
+  if (n_long > 0) {  // triangles with more than RND_MAX_ENT partners: one warp per triangle
+    k_ent_verts<<<grid_for(n, 256), 256, 0, st>>>(ctx->keys_sorted, ctx->dvals_sorted, q->tris, n, bitsT, ctx->everts.as<int>());
+    TT_LAUNCH_CHECK();
+    k_tri_symbolic<<<grid_for(n_long, SYM_WARPS), 32 * SYM_WARPS, 0, st>>>(
+        q->tris, ctx->touched.as<int>(), n_long, ctx->tptr.as<int>(), ctx->keys_sorted, bitsT,
+        ctx->vcnt.as<int>(), (ctx->opt.flags & TT_FLAG_FORCE_GENERAL_ROWS) ? 1 : 0, ctx->erank.as<int>(),
+        ctx->drank.as<int>(), ctx->rowlen.as<int>(), ctx->tlen.as<int64_t>(), ctx->slot_excl.as<uint8_t>(),
+        ctx->long_list.as<int>(), ctx->rdesc.as<int4>());
+    TT_LAUNCH_CHECK();
+  }
+  s = scan_i64(ctx, ctx->tlen.as<int64_t>(), ctx->toff.as<int64_t>(), 3 * n_touched + 1, st);
+  if (s != TT_OK) return s;
+  int64_t R = 0;
+  TT_CUDA(cudaMemcpyAsync(&R, ctx->toff.as<int64_t>() + 3 * n_touched, sizeof(int64_t), cudaMemcpyDeviceToHost, st));
+  TT_CUDA(cudaStreamSynchronize(st));
+  if (R >= (int64_t(1) << 31)) return fail(ctx, TT_ERR_INVALID_ARG, "general-row workspace exceeds 2^31 blocks");
+  ctx->R = R;
+
+  // ---- general rows: merge records sorted by (row, col) ----
+  int64_t U = 0;
+  ctx->rkeys_sorted = nullptr;
+  ctx->rvals_sorted = nullptr;
+  if (R > 0) {
+    for (int i = 0; i < 2; ++i) {
+      TT_CUDA(ctx->rkeys[i].ensure(sizeof(uint64_t) * (size_t)R));
+      TT_CUDA(ctx->rvals[i].ensure(sizeof(uint32_t) * (size_t)R));
+    }
+    TT_CUDA(ctx->head.ensure(sizeof(int) * (size_t)R));
+    TT_CUDA(ctx->ord.ensure(sizeof(int) * (size_t)R));
+    TT_CUDA(ctx->rowfirst.ensure(sizeof(int) * (size_t)(nV + 1)));
+    TT_CUDA(ctx->run_start.ensure(sizeof(int) * (size_t)(R + 1)));
+    TT_CUDA(ctx->run_dest.ensure(sizeof(int) * (size_t)(R + 1)));
+    k_emit_records<<<tri_grid, 32 * SYM_WARPS, 0, st>>>(
+        q->tris, ctx->touched.as<int>(), n_touched, ctx->tptr.as<int>(), ctx->keys_sorted, bitsT, bitsV,
+        ctx->erank.as<int>(), ctx->drank.as<int>(), ctx->toff.as<int64_t>(), ctx->slot_excl.as<uint8_t>(),
+        ctx->rkeys[0].as<uint64_t>(), ctx->rvals[0].as<uint32_t>());
+    TT_LAUNCH_CHECK();
+    s = sort_pairs(ctx, ctx->rkeys, ctx->rvals, R, 0, 2 * bitsV, &ctx->rkeys_sorted, &ctx->rvals_sorted, st);
+    if (s != TT_OK) return s;
+    k_record_heads<<<grid_for(R, 256), 256, 0, st>>>(ctx->rkeys_sorted, R, ctx->head.as<int>());
+    TT_LAUNCH_CHECK();
+    s = incl_scan_i32(ctx, ctx->head.as<int>(), ctx->ord.as<int>(), R, st);
+    if (s != TT_OK) return s;
+    k_record_rows<<<grid_for(R, 256), 256, 0, st>>>(ctx->rkeys_sorted, R, bitsV, ctx->head.as<int>(),
+                                                    ctx->ord.as<int>(), ctx->rowlen.as<int>(),
+                                                    ctx->rowfirst.as<int>(), ctx->run_start.as<int>());
+    TT_LAUNCH_CHECK();
+    int u32 = 0;
+    TT_CUDA(cudaMemcpyAsync(&u32, ctx->ord.as<int>() + (R - 1), sizeof(int), cudaMemcpyDeviceToHost, st));
+    TT_CUDA(cudaStreamSynchronize(st));
+    U = u32;
+  }
+  ctx->U = U;
+
+  // ---- row pointers ----
+  TT_CUDA(ctx->rowptr64.ensure(sizeof(int64_t) * (size_t)(nV + 1)));
+  TT_CUDA(ctx->rowptr.ensure(sizeof(int) * (size_t)(nV + 1)));
+  s = scan_i32_to_i64(ctx, ctx->rowlen.as<int>(), ctx->rowptr64.as<int64_t>(), nV + 1, st);
+  if (s != TT_OK) return s;
+  int64_t nnzb = 0;
+  TT_CUDA(cudaMemcpyAsync(&nnzb, ctx->rowptr64.as<int64_t>() + nV, sizeof(int64_t), cudaMemcpyDeviceToHost, st));
+  TT_CUDA(cudaStreamSynchronize(st));
+  if (nnzb >= (int64_t(1) << 31)) return fail(ctx, TT_ERR_INVALID_ARG, "nnzb %lld exceeds int32 BSR indexing", (long long)nnzb);
+  ctx->nnzb = nnzb;
+  k_i64_to_i32<<<grid_for(nV + 1, 256), 256, 0, st>>>(ctx->rowptr64.as<int64_t>(), nV + 1, ctx->rowptr.as<int>());
+  TT_LAUNCH_CHECK();
+  TT_CUDA(ctx->colind.ensure(sizeof(int) * (size_t)(nnzb + 1)));
+  if (U > 0) {
+    k_record_dest<<<grid_for(U + 1, 256), 256, 0, st>>>(ctx->rkeys_sorted, U, R, bitsV, ctx->run_start.as<int>(),
+                                                        ctx->rowptr.as<int>(), ctx->rowfirst.as<int>(),
+                                                        ctx->run_dest.as<int>(), ctx->colind.as<int>());
+    TT_LAUNCH_CHECK();
+  }
+  if (n_chunks > 0) {
+    k_round_fill<<<rnd_grid, 32 * RSYM_WARPS, 0, st>>>(
+        q->tris, ctx->touched.as<int>(), ctx->rdesc.as<int4>(), n_chunks, ctx->tfirst.as<int>(), ctx->keys_sorted, bitsT,
+        ctx->erank.as<int>(), ctx->drank.as<int>(), ctx->toff.as<int64_t>(), ctx->slot_excl.as<uint8_t>(),
+        ctx->rowptr.as<int>(), ctx->rowbase.as<int64_t>(), ctx->colind.as<int>());
+    TT_LAUNCH_CHECK();
+  }
+  if (n_long > 0) {
+    k_fill_rows<<<grid_for(n_long, SYM_WARPS), 32 * SYM_WARPS, 0, st>>>(
+        q->tris, ctx->touched.as<int>(), n_long, ctx->tptr.as<int>(), ctx->keys_sorted, bitsT,
+        ctx->erank.as<int>(), ctx->drank.as<int>(), ctx->toff.as<int64_t>(), ctx->slot_excl.as<uint8_t>(),
+        ctx->rowptr.as<int>(), ctx->rowbase.as<int64_t>(), ctx->colind.as<int>(), ctx->long_list.as<int>(),
+        ctx->rdesc.as<int4>());
+    TT_LAUNCH_CHECK();
+  }
+
+  // ---- per-slot buffers, vertex -> slot incidence ----
   TT_CUDA(ctx->asm_energy.ensure(sizeof(double) * (size_t)(n_chunks + 1)));
   TT_CUDA(ctx->tvals.ensure(sizeof(T) * 9 * (size_t)(R + 1)));
   TT_CUDA(ctx->tslot.ensure(sizeof(T) * 9 * (size_t)(n_touched + 1)));
@@ -461,7 +480,7 @@ tt_status symbolic_impl(tt_ctx* ctx, const tt_problem* q, int64_t* nnzb_host, in
     k_emit_vslots<<<grid_for(nvs, 256), 256, 0, st>>>(q->tris, ctx->touched.as<int>(), n_touched,
                                                       ctx->vkeys[0].as<uint64_t>(), ctx->vvals[0].as<uint32_t>());
     TT_LAUNCH_CHECK();
-    s = sort_pairs(ctx, ctx->vkeys, ctx->vvals, nvs, bitsV, &vkeys_sorted, &ctx->vvals_sorted, st);
+    s = sort_pairs(ctx, ctx->vkeys, ctx->vvals, nvs, 0, bitsV, &vkeys_sorted, &ctx->vvals_sorted, st);
     if (s != TT_OK) return s;
   }
   k_segment_ptr<<<grid_for(nvs + 1, 256), 256, 0, st>>>(vkeys_sorted, nvs, 0, nV, ctx->vptr.as<int>());
