@@ -1137,52 +1137,63 @@ k_assemble_long(const AsmParams<T> P) {
 
 // ------------------------------------------------------------------------------------------ K6
 // MODE 1: energy + gradient only.  MODE 2: matrix-free H.p:  y_s = sum_j (J^T M (J p_loc))_own.
-// Same rounds; a lane stages 9 values per entry, lane = component sums them per triangle in entry
-// order.  Long triangles simply take several groups of 32 entries.
+// Same rounds as K4, lane = directed entry.  A lane brings its 9 own-vertex values back to the
+// triangle's own vertex order (selects on the recorded permutation) and the per-triangle sums are
+// a SEGMENTED warp scan over the lanes (shuffles, fixed tree order: deterministic); the last lane
+// of each triangle writes its 9 sums.  No shared memory, no atomics.  A long triangle is a round of
+// its own and simply takes several groups of 32 entries, carried in registers.
 constexpr int RED_THREADS = 128;
+#ifndef TT_RED_MIN_CTAS
+#define TT_RED_MIN_CTAS 3
+#endif
 template <typename T, int MODE>
-__global__ void __launch_bounds__(RED_THREADS)
-k_entry_reduce(const AsmParams<T> P) {
-  __shared__ double s_stage[RED_THREADS / 32][32 * 9];
-  __shared__ int s_src[RED_THREADS / 32][32];
+__global__ void __launch_bounds__(RED_THREADS, TT_RED_MIN_CTAS)
+k_entry_reduce(const AsmParams<T> P, const int* __restrict__ round_list, int64_t n_rounds) {
   constexpr unsigned FULL = 0xffffffffu;
   const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-  const int64_t c = (int64_t)blockIdx.x * (RED_THREADS / 32) + warp;
-  if (c >= P.n_chunks) return;
+  const int64_t ci = (int64_t)blockIdx.x * (RED_THREADS / 32) + warp;
+  if (ci >= n_rounds) return;
+  const int64_t c = round_list ? (int64_t)__ldg(round_list + ci) : ci;
   const int4 d = __ldg(P.rdesc + c);
   const int e_lo = d.x, e_hi = d.x + d.y;
-  double* stage = s_stage[warp];
-  int* src = s_src[warp];
-  double acc = 0.0, e_acc = 0.0;
-  int cur = -1;
-  int64_t cur_ti = (int64_t)d.z - 1;
+  const bool is_long = d.y > RND_MAX_ENT;
+  unsigned heads = 1u;  // bit i: entry i opens a triangle
+  if (!is_long) {
+    const int f = (lane < d.w) ? __ldg(P.tfirst + d.z + lane) - e_lo : 0;
+    heads = __reduce_or_sync(FULL, (lane < d.w) ? (1u << f) : 0u);
+  }
+  const unsigned below = heads & (0xffffffffu >> (31 - lane));  // heads at or below this lane
+  const int segf = 31 - __clz((int)below);                      // first lane of this lane's triangle
+  double carry[9];
+#pragma unroll
+  for (int k = 0; k < 9; ++k) carry[k] = 0.0;
+  double e_acc = 0.0;
   for (int base = e_lo; base < e_hi; base += 32) {
     const int nvalid = min(32, e_hi - base);
-    int s = -1;
+    double v[9];
+#pragma unroll
+    for (int k = 0; k < 9; ++k) v[k] = 0.0;
     if (lane < nvalid) {
       const int64_t e = (int64_t)base + lane;
-      s = (int)(__ldg(P.keys + e) >> P.bitsT);
       int ids[6];
       {
-        const int2* v = reinterpret_cast<const int2*>(P.everts + 6 * e);
-        const int2 v0 = __ldg(v), v1 = __ldg(v + 1), v2 = __ldg(v + 2);
+        const int2* iv = reinterpret_cast<const int2*>(P.everts + 6 * e);
+        const int2 v0 = __ldg(iv), v1 = __ldg(iv + 1), v2 = __ldg(iv + 2);
         ids[0] = v0.x; ids[1] = v0.y; ids[2] = v1.x; ids[3] = v1.y; ids[4] = v2.x; ids[5] = v2.y;
       }
       double x[18];
       load_pos18(P.pos, ids, x);
       const unsigned pay = (unsigned)__ldg(P.dvals + e);
-      double pv[18];  // p of (own, partner) vertices, recorded order
-      if (MODE == 2) {
-        const bool side = (pay & 1u) != 0u;
-        const int pid[6] = {side ? ids[3] : ids[0], side ? ids[4] : ids[1], side ? ids[5] : ids[2],
-                            side ? ids[0] : ids[3], side ? ids[1] : ids[4], side ? ids[2] : ids[5]};
-        load_pos18(P.pvec, pid, pv);
-      }
       Entry E;
       eval_core(x, pay, P.sigma, P.hess_mode, E);
       e_acc += E.en;
       double u0 = E.cf.cg0, u1 = E.cf.cg1;  // MODE 1: Eq. 3
       if (MODE == 2) {
+        const bool side = (pay & 1u) != 0u;
+        const int pid[6] = {side ? ids[3] : ids[0], side ? ids[4] : ids[1], side ? ids[5] : ids[2],
+                            side ? ids[0] : ids[3], side ? ids[1] : ids[4], side ? ids[2] : ids[5]};
+        double pv[18];  // p of (own, partner) vertices, recorded order
+        load_pos18(P.pvec, pid, pv);
         double j0 = 0.0, j1 = 0.0;
 #pragma unroll
         for (int i = 0; i < 18; ++i) {
@@ -1192,32 +1203,234 @@ k_entry_reduce(const AsmParams<T> P) {
         u0 = E.cf.c00 * j0 + E.cf.c01 * j1;  // M (J p_loc)
         u1 = E.cf.c01 * j0 + E.cf.c11 * j1;
       }
+      double yr[9];  // own half, recorded order
 #pragma unroll
-      for (int r = 0; r < 3; ++r)
+      for (int i = 0; i < 9; ++i) yr[i] = u0 * E.g0[i] + u1 * E.g1[i];
+#pragma unroll
+      for (int i = 0; i < 3; ++i)  // own vertex i = recorded position r with po[r] == i
 #pragma unroll
         for (int cc = 0; cc < 3; ++cc)
-          stage[lane * 9 + 3 * E.po[r] + cc] = u0 * E.g0[3 * r + cc] + u1 * E.g1[3 * r + cc];
+          v[3 * i + cc] = (E.po[0] == i) ? yr[cc] : ((E.po[1] == i) ? yr[3 + cc] : yr[6 + cc]);
     }
-    src[lane] = s;
-    __syncwarp();
-    for (int i = 0; i < nvalid; ++i) {
-      const int si = src[i];
-      if (si != cur) {  // warp-uniform
-        if (cur >= 0 && lane < 9) P.tslot[9 * cur_ti + lane] = (T)acc;
-        acc = 0.0;
-        cur = si;
-        ++cur_ti;
+    // segmented inclusive scan over the lanes (segments = triangles)
+#pragma unroll
+    for (int o = 1; o < 32; o <<= 1) {
+      const bool take = (lane - o) >= segf;
+#pragma unroll
+      for (int k = 0; k < 9; ++k) {
+        const double up = __shfl_up_sync(FULL, v[k], o);
+        if (take) v[k] += up;
       }
-      if (lane < 9) acc += stage[i * 9 + lane];
     }
-    __syncwarp();
+    if (!is_long) {
+      const bool last = (lane < nvalid) && (lane == nvalid - 1 || (((heads >> 1) >> lane) & 1u));
+      if (last) {
+        const int64_t ti = (int64_t)d.z + __popc(below) - 1;
+#pragma unroll
+        for (int k = 0; k < 9; ++k) P.tslot[9 * ti + k] = (T)v[k];
+      }
+    } else {
+#pragma unroll
+      for (int k = 0; k < 9; ++k) carry[k] += __shfl_sync(FULL, v[k], nvalid - 1);
+    }
   }
-  if (cur >= 0 && lane < 9) P.tslot[9 * cur_ti + lane] = (T)acc;
+  if (is_long && lane == 0) {
+#pragma unroll
+    for (int k = 0; k < 9; ++k) P.tslot[9 * (int64_t)d.z + k] = (T)carry[k];
+  }
   if (MODE == 1) {
 #pragma unroll
     for (int o = 16; o > 0; o >>= 1) e_acc += __shfl_down_sync(FULL, e_acc, o);
     if (lane == 0) P.chunk_energy[c] = e_acc;
   }
+}
+
+// Pipelined form of the same kernel for the ordinary (non-long) rounds: persistent grid, a warp
+// walks rounds c, c + G, ...  Positions (and p) of the NEXT round travel global -> shared with
+// cp.async (LDGSTS: no registers held while in flight) into lane-private slots, vertex ids one
+// round further ahead and descriptors two, so that the three dependent gathers of a round
+// (descriptor -> vertex ids -> positions) are all off the critical path.
+template <typename T>
+__device__ __forceinline__ void cp_async_elem(T* sdst, const T* gsrc) {
+  const unsigned sa = (unsigned)__cvta_generic_to_shared(sdst);
+  if (sizeof(T) == 8) asm volatile("cp.async.ca.shared.global [%0], [%1], 8;" ::"r"(sa), "l"(gsrc) : "memory");
+  else asm volatile("cp.async.ca.shared.global [%0], [%1], 4;" ::"r"(sa), "l"(gsrc) : "memory");
+}
+__device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
+template <int N>
+__device__ __forceinline__ void cp_async_wait() { asm volatile("cp.async.wait_group %0;" ::"n"(N) : "memory"); }
+
+// 18 values of six vertices -> lane-private shared slots buf[k * 32 + lane]
+template <typename T>
+__device__ __forceinline__ void gather18_async(T* buf, int lane, const T* __restrict__ src, const int (&ids)[6]) {
+#pragma unroll
+  for (int v = 0; v < 6; ++v) {
+    const T* g = src + 3 * (int64_t)ids[v];
+#pragma unroll
+    for (int k = 0; k < 3; ++k) cp_async_elem(buf + (3 * v + k) * 32 + lane, g + k);
+  }
+}
+
+#ifndef TT_PIPE_WARPS
+#define TT_PIPE_WARPS 4
+#endif
+#ifndef TT_PIPE_MIN_CTAS
+#define TT_PIPE_MIN_CTAS 2
+#endif
+constexpr int PIPE_WARPS = TT_PIPE_WARPS;
+template <typename T, int MODE>
+struct PipeWarpSmem {
+  T x[2][18 * 32];
+  T p[MODE == 2 ? 18 * 32 : 1];
+};
+
+struct PipeOps {
+  int ids[6];
+  unsigned pay;
+};
+template <typename T>
+__device__ __forceinline__ void load_pipe_ops(const AsmParams<T>& P, const int4 d, int lane, PipeOps& R) {
+#pragma unroll
+  for (int i = 0; i < 6; ++i) R.ids[i] = 0;
+  R.pay = 0u;
+  if (d.y <= RND_MAX_ENT && lane < d.y) {
+    const int64_t e = (int64_t)d.x + lane;
+    const int2* v = reinterpret_cast<const int2*>(P.everts + 6 * e);
+    const int2 v0 = __ldg(v), v1 = __ldg(v + 1), v2 = __ldg(v + 2);
+    R.ids[0] = v0.x; R.ids[1] = v0.y; R.ids[2] = v1.x; R.ids[3] = v1.y; R.ids[4] = v2.x; R.ids[5] = v2.y;
+    R.pay = (unsigned)__ldg(P.dvals + e);
+  }
+}
+__device__ __forceinline__ void own_first_ids(const PipeOps& R, int (&pid)[6]) {
+  const bool side = (R.pay & 1u) != 0u;
+#pragma unroll
+  for (int i = 0; i < 3; ++i) {
+    pid[i] = side ? R.ids[3 + i] : R.ids[i];
+    pid[3 + i] = side ? R.ids[i] : R.ids[3 + i];
+  }
+}
+
+template <typename T, int MODE>
+__global__ void __launch_bounds__(32 * PIPE_WARPS, TT_PIPE_MIN_CTAS)
+k_entry_pipe(const AsmParams<T> P) {
+  extern __shared__ __align__(16) unsigned char s_raw[];
+  constexpr unsigned FULL = 0xffffffffu;
+  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+  PipeWarpSmem<T, MODE>& S = reinterpret_cast<PipeWarpSmem<T, MODE>*>(s_raw)[warp];
+  const int64_t G = (int64_t)gridDim.x * PIPE_WARPS;
+  int64_t c = (int64_t)blockIdx.x * PIPE_WARPS + warp;
+  if (c >= P.n_chunks) return;
+  const int4 dzero = make_int4(0, 0, 0, 0);
+  // ---- prologue ----
+  int4 d_cur = __ldg(P.rdesc + c);
+  int4 d_nxt = (c + G < P.n_chunks) ? __ldg(P.rdesc + c + G) : dzero;
+  int4 d_nn = (c + 2 * G < P.n_chunks) ? __ldg(P.rdesc + c + 2 * G) : dzero;
+  PipeOps cur, nxt;
+  load_pipe_ops(P, d_cur, lane, cur);
+  load_pipe_ops(P, d_nxt, lane, nxt);
+  if (d_cur.y <= RND_MAX_ENT && lane < d_cur.y) gather18_async(S.x[0], lane, P.pos, cur.ids);
+  cp_async_commit();
+  if (MODE == 2) {
+    if (d_cur.y <= RND_MAX_ENT && lane < d_cur.y) {
+      int pid[6];
+      own_first_ids(cur, pid);
+      gather18_async(S.p, lane, P.pvec, pid);
+    }
+    cp_async_commit();
+  }
+  int buf = 0;
+  while (true) {
+    const bool has_next = c + G < P.n_chunks;
+    // ---- top of round c: ids two rounds ahead, descriptor three, positions of the next round ----
+    PipeOps nn;
+    load_pipe_ops(P, d_nn, lane, nn);
+    const int4 d_nnn = (c + 3 * G < P.n_chunks) ? __ldg(P.rdesc + c + 3 * G) : dzero;
+    const bool nxt_ok = d_nxt.y <= RND_MAX_ENT && lane < d_nxt.y;
+    if (nxt_ok) gather18_async(S.x[buf ^ 1], lane, P.pos, nxt.ids);
+    cp_async_commit();
+    const int e_lo = d_cur.x, nent = d_cur.y;
+    const bool is_long = nent > RND_MAX_ENT;  // k_entry_reduce's (launched over long_list)
+    const bool valid = !is_long && lane < nent;
+    const bool tri_lane = !is_long && lane < d_cur.w;
+    const int f = tri_lane ? __ldg(P.tfirst + d_cur.z + lane) - e_lo : 0;  // consumed after the derivative code
+    if (MODE == 2) cp_async_wait<2>(); else cp_async_wait<1>();  // positions of THIS round have landed
+    double v[9];
+#pragma unroll
+    for (int k = 0; k < 9; ++k) v[k] = 0.0;
+    double e_acc = 0.0;
+    if (valid) {
+      double x[18];
+#pragma unroll
+      for (int k = 0; k < 18; ++k) x[k] = (double)S.x[buf][k * 32 + lane];
+      Entry E;
+      eval_core(x, cur.pay, P.sigma, P.hess_mode, E);
+      e_acc = E.en;
+      double u0 = E.cf.cg0, u1 = E.cf.cg1;  // MODE 1: Eq. 3
+      if (MODE == 2) {
+        cp_async_wait<1>();                 // p of THIS round
+        double j0 = 0.0, j1 = 0.0;
+#pragma unroll
+        for (int i = 0; i < 18; ++i) {
+          const double pv = (double)S.p[i * 32 + lane];
+          j0 = fma(E.g0[i], pv, j0);
+          j1 = fma(E.g1[i], pv, j1);
+        }
+        u0 = E.cf.c00 * j0 + E.cf.c01 * j1;  // M (J p_loc)
+        u1 = E.cf.c01 * j0 + E.cf.c11 * j1;
+      }
+      double yr[9];
+#pragma unroll
+      for (int i = 0; i < 9; ++i) yr[i] = u0 * E.g0[i] + u1 * E.g1[i];
+#pragma unroll
+      for (int i = 0; i < 3; ++i)
+#pragma unroll
+        for (int cc = 0; cc < 3; ++cc)
+          v[3 * i + cc] = (E.po[0] == i) ? yr[cc] : ((E.po[1] == i) ? yr[3 + cc] : yr[6 + cc]);
+    }
+    if (MODE == 2) {
+      cp_async_wait<1>();  // lanes that skipped the block above: same group accounting
+      if (nxt_ok) {        // this lane's p slots are free again: p of the next round
+        int pid[6];
+        own_first_ids(nxt, pid);
+        gather18_async(S.p, lane, P.pvec, pid);
+      }
+      cp_async_commit();
+    }
+    if (!is_long) {
+      const unsigned heads = __reduce_or_sync(FULL, tri_lane ? (1u << f) : 0u) | 1u;  // bit i: entry i opens a triangle
+      const unsigned below = heads & (0xffffffffu >> (31 - lane));
+      const int segf = 31 - __clz((int)below);
+#pragma unroll
+      for (int o = 1; o < 32; o <<= 1) {
+        const bool take = (lane - o) >= segf;
+#pragma unroll
+        for (int k = 0; k < 9; ++k) {
+          const double up = __shfl_up_sync(FULL, v[k], o);
+          if (take) v[k] += up;
+        }
+      }
+      const bool last = valid && (lane == nent - 1 || ((heads >> 1) >> lane) & 1u);
+      if (last) {
+        const int64_t ti = (int64_t)d_cur.z + __popc(below) - 1;
+#pragma unroll
+        for (int k = 0; k < 9; ++k) P.tslot[9 * ti + k] = (T)v[k];
+      }
+      if (MODE == 1) {
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) e_acc += __shfl_down_sync(FULL, e_acc, o);
+        if (lane == 0) P.chunk_energy[c] = e_acc;
+      }
+    }
+    if (!has_next) break;
+    c += G;
+    d_cur = d_nxt;
+    d_nxt = d_nn;
+    d_nn = d_nnn;
+    cur = nxt;
+    nxt = nn;
+    buf ^= 1;
+  }
+  cp_async_wait<0>();
 }
 
 // ------------------------------------------------------------------------------------------ K5

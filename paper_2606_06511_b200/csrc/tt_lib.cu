@@ -80,6 +80,7 @@ struct tt_ctx {
   int64_t A = 0, n_dir = 0, n_touched = 0, R = 0, U = 0, nnzb = 0, n_chunks = 0, n_long = 0, rows_excl = 0, rows_gen = 0;
   int bitsT = 1, bitsV = 1;
   int tile_grid[2] = {0, 0};  // persistent grid of k_assemble_tile<double / float>
+  int pipe_grid[2][2] = {{0, 0}, {0, 0}};  // persistent grid of k_entry_pipe<double / float, MODE 1 / 2>
   uint64_t* keys_sorted = nullptr;
   uint16_t* dvals_sorted = nullptr;
   uint64_t* rkeys_sorted = nullptr;
@@ -526,6 +527,22 @@ ttk::AsmParams<T> make_params(tt_ctx* ctx, const tt_problem* q) {
   return p;
 }
 
+// K6 launch: pipelined kernel over all rounds (skips long ones) + the plain kernel over the long rounds
+template <typename T, int MODE>
+tt_status launch_entry_reduce(tt_ctx* ctx, const ttk::AsmParams<T>& p, cudaStream_t st) {
+  using namespace ttk;
+  const size_t smem = sizeof(PipeWarpSmem<T, MODE>) * PIPE_WARPS;
+  const int64_t full = (ctx->n_chunks + PIPE_WARPS - 1) / PIPE_WARPS;
+  const int64_t pers = ctx->pipe_grid[sizeof(T) == 8 ? 0 : 1][MODE - 1];
+  k_entry_pipe<T, MODE><<<(unsigned)(full < pers ? full : pers), 32 * PIPE_WARPS, smem, st>>>(p);
+  TT_LAUNCH_CHECK();
+  if (ctx->n_long > 0) {
+    k_entry_reduce<T, MODE><<<grid_for(ctx->n_long, RED_THREADS / 32), RED_THREADS, 0, st>>>(p, ctx->long_list.as<int>(), ctx->n_long);
+    TT_LAUNCH_CHECK();
+  }
+  return TT_OK;
+}
+
 template <typename T>
 tt_status numeric_impl(tt_ctx* ctx, const tt_problem* q, void* energy_sum, void* grad, int32_t* rowptr,
                        int32_t* colind, void* vals, int64_t cap, cudaStream_t st) {
@@ -555,7 +572,8 @@ tt_status numeric_impl(tt_ctx* ctx, const tt_problem* q, void* energy_sum, void*
         k_assemble_long<T><<<grid_for(ctx->n_long, TILE_WARPS), 32 * TILE_WARPS, smem, st>>>(p);
       }
     } else {
-      k_entry_reduce<T, 1><<<grid_for(ctx->n_chunks, RED_THREADS / 32), RED_THREADS, 0, st>>>(p);
+      tt_status s1 = launch_entry_reduce<T, 1>(ctx, p, st);
+      if (s1 != TT_OK) return s1;
     }
     TT_LAUNCH_CHECK();
     TT_CUDA(cudaEventRecord(ctx->ev[1][1], st));
@@ -583,8 +601,8 @@ tt_status hessvec_impl(tt_ctx* ctx, const tt_problem* q, const void* pvec, void*
   p.chunk_energy = nullptr;
   if (ctx->n_chunks > 0) {
     TT_CUDA(cudaEventRecord(ctx->ev[2][0], st));
-    k_entry_reduce<T, 2><<<grid_for(ctx->n_chunks, RED_THREADS / 32), RED_THREADS, 0, st>>>(p);
-    TT_LAUNCH_CHECK();
+    tt_status s1 = launch_entry_reduce<T, 2>(ctx, p, st);
+    if (s1 != TT_OK) return s1;
     TT_CUDA(cudaEventRecord(ctx->ev[2][1], st));
     ctx->ev_used[2] = true;
   }
@@ -630,6 +648,17 @@ tt_status tt_create(const tt_options* opt, tt_ctx** out) {
     if (e == cudaSuccess) e = cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, opt->device);
     if (e == cudaSuccess) e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&nb0, ttk::k_assemble_tile<double>, 32 * ttk::TILE_WARPS, sizeof(ttk::TileWarpSmem<double>) * ttk::TILE_WARPS);
     if (e == cudaSuccess) e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&nb1, ttk::k_assemble_tile<float>, 32 * ttk::TILE_WARPS, sizeof(ttk::TileWarpSmem<float>) * ttk::TILE_WARPS);
+    if (e != cudaSuccess) { (void)cudaGetLastError(); delete c; return TT_ERR_CUDA; }
+    auto pipe_setup = [&](const void* f, size_t smem, int& grid) {
+      int nb = 0;
+      opt_in(f, smem);
+      if (e == cudaSuccess) e = cudaOccupancyMaxActiveBlocksPerMultiprocessorWithFlags(&nb, f, 32 * ttk::PIPE_WARPS, smem, cudaOccupancyDefault);
+      grid = sms * (nb > 0 ? nb : 1);
+    };
+    pipe_setup((const void*)ttk::k_entry_pipe<double, 1>, sizeof(ttk::PipeWarpSmem<double, 1>) * ttk::PIPE_WARPS, c->pipe_grid[0][0]);
+    pipe_setup((const void*)ttk::k_entry_pipe<double, 2>, sizeof(ttk::PipeWarpSmem<double, 2>) * ttk::PIPE_WARPS, c->pipe_grid[0][1]);
+    pipe_setup((const void*)ttk::k_entry_pipe<float, 1>, sizeof(ttk::PipeWarpSmem<float, 1>) * ttk::PIPE_WARPS, c->pipe_grid[1][0]);
+    pipe_setup((const void*)ttk::k_entry_pipe<float, 2>, sizeof(ttk::PipeWarpSmem<float, 2>) * ttk::PIPE_WARPS, c->pipe_grid[1][1]);
     if (e != cudaSuccess) { (void)cudaGetLastError(); delete c; return TT_ERR_CUDA; }
     c->tile_grid[0] = sms * (nb0 > 0 ? nb0 : 1);  // one wave of resident CTAs: the kernel is persistent
     c->tile_grid[1] = sms * (nb1 > 0 ? nb1 : 1);

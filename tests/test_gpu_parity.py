@@ -72,7 +72,9 @@ def run_case(oracle, pb, dtype="f64", hess_mode=1, sigma=1.0, flags=0, check_val
     g2 = torch.empty_like(out["grad"])
     ctx.tt_energy_grad_hess(out["prob"], e2, g2)
     torch.cuda.synchronize()
-    assert torch.equal(g2, out["grad"]) and torch.equal(e2, out["energy"])
+    # (K6 sums a triangle's entries in a fixed shuffle-tree order, K4 sequentially: equal up to rounding order)
+    assert rel(g2.cpu().numpy(), out["grad"].cpu().numpy()) <= (1e-13 if dtype == "f64" else 1e-6)
+    assert rel(e2.cpu().numpy(), out["energy"].cpu().numpy()) <= (1e-14 if dtype == "f64" else 1e-6)
     # matrix-free H.p (a5) == oracle's per-pair J^T M J p == BSR.p (P10)
     rng = np.random.default_rng(12345)
     p_np = rng.normal(size=pos_np.shape)
