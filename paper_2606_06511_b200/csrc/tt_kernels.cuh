@@ -374,7 +374,10 @@ k_fill_rows(const int* __restrict__ tris, const int* __restrict__ touched, int64
 // restarted at every bucket of CHK_BUCKET touched triangles so that buckets pack in parallel
 // (one thread per bucket; count pass, scan, fill pass).
 constexpr int RND_MAX_ENT = 32;
-constexpr int RND_MAX_TRI = 16;
+#ifndef TT_RND_MAX_TRI
+#define TT_RND_MAX_TRI 8
+#endif
+constexpr int RND_MAX_TRI = TT_RND_MAX_TRI;
 constexpr int CHK_BUCKET = 128;
 
 // tfirst[i] = first directed entry of touched triangle i; tfirst[n_touched] = n_dir
@@ -454,11 +457,18 @@ __global__ void k_emit_vslots(const int* __restrict__ tris, const int* __restric
 // the <= 15 unaligned head / tail bytes by plain stores).  Address generation and full-line
 // writes are the copy engine's; the SM issues ~60 shared stores per entry and row.
 //
-// The grid is PERSISTENT (a few CTAs per SM); a warp walks rounds c, c + G, c + 2G, ... and keeps
-// the operands of its NEXT round in flight while it works on the current one: descriptor two
-// rounds ahead, vertex ids / payload / ranks / row destinations one round ahead (issued at the
-// top of a round), positions one round ahead (issued after the current round's derivatives).
-// Every gather therefore has a full round (~2-3 k instructions) to land.
+// The grid is PERSISTENT (8 one-warp CTAs per SM: the kernel needs 255 registers); a warp walks
+// rounds c, c + G, c + 2G, ... with every gather of a round off its critical path:
+//   descriptor three rounds ahead, vertex ids two, payload / ranks / row destinations one (requested
+//   after the register peak of the derivative code); the positions of round c + G are pulled into
+//   L2 at the top of round c (prefetch.global.L2: no registers, no scoreboard) and loaded into
+//   registers at the end of round c, when J is dead.
+// cp.async (LDGSTS) is NOT used for the positions: cp.async.wait_group and
+// cp.async.bulk.wait_group.read both compile to DEPBAR on scoreboard SB0, so every wait for the
+// copy engine would also wait for the gathers in flight (measured: +40 % kernel time).
+// The staging area of the diagonal / gradient products aliases the row tile (12.5 KB of shared
+// memory per warp); the measured limiter is the L1 data pipe (shared-memory wavefronts of staging,
+// tile writes and the engine's reads: 62 % busy), not HBM (49 %) or instruction issue (31 %).
 struct Entry {
   double g0[18], g1[18];   // own triangle's 9 DOF first, partner's 9 after; vertices in RECORDED order (k, p, q)
   ttg::Coefs cf;
@@ -806,55 +816,112 @@ __device__ __forceinline__ void bulk_wait_read() { asm volatile("cp.async.bulk.w
 __device__ __forceinline__ void bulk_wait_all() { asm volatile("cp.async.bulk.wait_group 0;" ::: "memory"); }
 __device__ __forceinline__ void fence_async_smem() { asm volatile("fence.proxy.async.shared::cta;" ::: "memory"); }
 
-constexpr int TILE_WARPS = 2;             // warps per CTA (independent; sized by shared memory)
-constexpr int STG_STRIDE = 55;            // odd: lane = entry writes and lane = component reads conflict-free
+// ---- cp.async (LDGSTS): global -> shared gathers that hold no registers while in flight ---------
+template <typename T>
+__device__ __forceinline__ void cp_async_elem(T* sdst, const T* gsrc) {
+  const unsigned sa = (unsigned)__cvta_generic_to_shared(sdst);
+  if (sizeof(T) == 8) asm volatile("cp.async.ca.shared.global [%0], [%1], 8;" ::"r"(sa), "l"(gsrc) : "memory");
+  else asm volatile("cp.async.ca.shared.global [%0], [%1], 4;" ::"r"(sa), "l"(gsrc) : "memory");
+}
+__device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
+template <int N>
+__device__ __forceinline__ void cp_async_wait() { asm volatile("cp.async.wait_group %0;" ::"n"(N) : "memory"); }
+
+// 18 values of six vertices -> lane-private shared slots buf[k * 32 + lane]
+template <typename T>
+__device__ __forceinline__ void gather18_async(T* buf, int lane, const T* __restrict__ src, const int (&ids)[6]) {
+#pragma unroll
+  for (int v = 0; v < 6; ++v) {
+    const T* g = src + 3 * (int64_t)ids[v];
+#pragma unroll
+    for (int k = 0; k < 3; ++k) cp_async_elem(buf + (3 * v + k) * 32 + lane, g + k);
+  }
+}
+
+#ifndef TT_TILE_WARPS
+#define TT_TILE_WARPS 1
+#endif
+#ifndef TT_TILE_MAXNREG
+#define TT_TILE_MAXNREG 255               // 8 warps / SM.  Measured: 200 / 184 / 168 registers (10 / 11 / 12 warps) spill
+#endif                                    // 400-700 bytes per thread and run 20-60 % slower (profiles/r1_step_breakdown.md)
+#ifndef TT_RED_UNR
+#define TT_RED_UNR 8                      // entries per triangle whose staged values are loaded up front
+#endif
+constexpr int RED_UNR = TT_RED_UNR;
+constexpr int TILE_WARPS = TT_TILE_WARPS; // warps per CTA (independent; a CTA is only a packaging unit)
 constexpr int NDIAG = 45;                 // upper triangle of the symmetric 9x9 diagonal block, row-major packed
 constexpr int NSTG = NDIAG + 9;           // + gradient of the three own vertices
+constexpr int STG_PASS = NSTG / 2;        // the 54 per-entry values are staged in two passes of 27
+constexpr int STG_STRIDE = STG_PASS;      // 27 doubles: odd, so lane = entry writes are conflict-free
+constexpr int LONG_STRIDE = 31;           // k_assemble_long: 27 + 3 staged values per entry, odd stride
 
 template <typename T>
 struct TileCfg {
   static constexpr int RUN_UNIT = 27 * (int)sizeof(T);  // bytes one entry (or the diagonal) adds to a row run
   static constexpr int TILE_BYTES = RUN_UNIT * (RND_MAX_ENT + RND_MAX_TRI) + 32 * RND_MAX_TRI;
+  static constexpr int STAGE_BYTES = 32 * STG_STRIDE * (int)sizeof(double);
+  static constexpr int UNION_BYTES = TILE_BYTES > STAGE_BYTES ? TILE_BYTES : STAGE_BYTES;
 };
 
+// Shared memory of one warp.  `tile` holds, in turn, (1) the per-entry staging area of the
+// diagonal / gradient products and (2) the row tile the copy engine reads: the two never live at
+// the same time (the per-triangle sums move to `dsum` in between).
 template <typename T>
 struct alignas(16) TileWarpSmem {
-  unsigned char tile[TileCfg<T>::TILE_BYTES];
-  double stage[32 * STG_STRIDE];
-  int tri_first[RND_MAX_TRI + 1];         // first entry (lane) of every triangle of the round
+  unsigned char tile[TileCfg<T>::UNION_BYTES];
+  double dsum[RND_MAX_TRI][NSTG];         // per-triangle sums: 45 diagonal-block values + 9 gradient values
   int run_off[RND_MAX_TRI];               // byte offset of the triangle's run in the tile (current row)
   int diag_off[RND_MAX_TRI][3];           // byte offset of its diagonal block n in the tile (current row)
 };
+// Pulls the (at most two) 32-byte sectors of each of six vertices into L2.
+template <typename T>
+__device__ __forceinline__ void prefetch_pos_l2(const T* __restrict__ pos, const int (&ids)[6]) {
+#pragma unroll
+  for (int v = 0; v < 6; ++v) {
+    const T* p = pos + 3 * (int64_t)ids[v];
+    asm volatile("prefetch.global.L2 [%0];" ::"l"(p));
+    asm volatile("prefetch.global.L2 [%0];" ::"l"(p + 2));
+  }
+}
+struct alignas(16) LongWarpSmem {
+  double stage[32 * LONG_STRIDE];
+};
 
-// Operands of a round that depend only on its descriptor (loaded one round ahead).
+// Operands of a round that depend only on its descriptor.  Vertex ids travel two rounds ahead
+// (their positions are requested one round ahead), everything else one round ahead.
 struct RoundOps {
-  int ids[6];        // lane = entry
-  unsigned pay;
+  unsigned pay;      // lane = entry
   int er[3];
   int e0, e1;        // lane = triangle
   int64_t rb[3];
   int dr[3];
 };
+__device__ __forceinline__ int round_entries(const int4 d) { return d.y > RND_MAX_ENT ? 0 : d.y; }  // long rounds: none here
+
+template <typename T>
+__device__ __forceinline__ void load_round_ids(const AsmParams<T>& P, const int4 d, int lane, int (&ids)[6]) {
+#pragma unroll
+  for (int i = 0; i < 6; ++i) ids[i] = 0;
+  if (lane < round_entries(d)) {
+    const int2* v = reinterpret_cast<const int2*>(P.everts + 6 * ((int64_t)d.x + lane));
+    const int2 v0 = __ldg(v), v1 = __ldg(v + 1), v2 = __ldg(v + 2);
+    ids[0] = v0.x; ids[1] = v0.y; ids[2] = v1.x; ids[3] = v1.y; ids[4] = v2.x; ids[5] = v2.y;
+  }
+}
 template <typename T>
 __device__ __forceinline__ void load_round_ops(const AsmParams<T>& P, const int4 d, int lane, RoundOps& R) {
-  const int nent = min(d.y, RND_MAX_ENT);
-#pragma unroll
-  for (int i = 0; i < 6; ++i) R.ids[i] = 0;
   R.pay = 0u;
   R.er[0] = R.er[1] = R.er[2] = 0;
   R.e0 = R.e1 = 0;
   R.rb[0] = R.rb[1] = R.rb[2] = 0;
   R.dr[0] = R.dr[1] = R.dr[2] = 0;
-  if (lane < nent) {
+  if (lane < round_entries(d)) {
     const int64_t e = (int64_t)d.x + lane;
-    const int2* v = reinterpret_cast<const int2*>(P.everts + 6 * e);
-    const int2 v0 = __ldg(v), v1 = __ldg(v + 1), v2 = __ldg(v + 2);
-    R.ids[0] = v0.x; R.ids[1] = v0.y; R.ids[2] = v1.x; R.ids[3] = v1.y; R.ids[4] = v2.x; R.ids[5] = v2.y;
     R.pay = (unsigned)__ldg(P.dvals + e);
 #pragma unroll
     for (int n = 0; n < 3; ++n) R.er[n] = __ldg(P.erank + 3 * e + n);
   }
-  if (lane < d.w) {
+  if (d.y <= RND_MAX_ENT && lane < d.w) {
     const int64_t ti = (int64_t)d.z + lane;
     R.e0 = __ldg(P.tfirst + ti);
     R.e1 = __ldg(P.tfirst + ti + 1);
@@ -867,13 +934,14 @@ __device__ __forceinline__ void load_round_ops(const AsmParams<T>& P, const int4
 }
 
 template <typename T>
-__global__ void __launch_bounds__(32 * TILE_WARPS)
+__global__ void __maxnreg__(TT_TILE_MAXNREG)
 k_assemble_tile(const AsmParams<T> P) {
   extern __shared__ __align__(16) unsigned char s_raw[];
   constexpr unsigned FULL = 0xffffffffu;
   constexpr int RUN_UNIT = TileCfg<T>::RUN_UNIT;
   const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
   TileWarpSmem<T>& S = reinterpret_cast<TileWarpSmem<T>*>(s_raw)[warp];
+  double* const stage = reinterpret_cast<double*>(S.tile);
   const int64_t G = (int64_t)gridDim.x * TILE_WARPS;
   int64_t c = (int64_t)blockIdx.x * TILE_WARPS + warp;
   if (c >= P.n_chunks) return;
@@ -883,23 +951,29 @@ k_assemble_tile(const AsmParams<T> P) {
   // ---- prologue: this warp's first round ----
   int4 d_cur = __ldg(P.rdesc + c);
   int4 d_nxt = (c + G < P.n_chunks) ? __ldg(P.rdesc + c + G) : dzero;
+  int4 d_nn = (c + 2 * G < P.n_chunks) ? __ldg(P.rdesc + c + 2 * G) : dzero;
   RoundOps cur;
   load_round_ops(P, d_cur, lane, cur);
+  int ids_nxt[6];
   double x[18];
+  {
+    int ids_cur[6];
+    load_round_ids(P, d_cur, lane, ids_cur);
 #pragma unroll
-  for (int i = 0; i < 18; ++i) x[i] = 0.0;
-  if (lane < min(d_cur.y, RND_MAX_ENT)) load_pos18(P.pos, cur.ids, x);
+    for (int i = 0; i < 18; ++i) x[i] = 0.0;
+    if (lane < round_entries(d_cur)) load_pos18(P.pos, ids_cur, x);
+  }
+  load_round_ids(P, d_nxt, lane, ids_nxt);
 
   while (true) {
     const bool has_next = c + G < P.n_chunks;
-    // ---- operands of the next round (descriptor known since the previous round) ----
-    RoundOps nxt;
-    load_round_ops(P, d_nxt, lane, nxt);
-    const int4 d_nn = (c + 2 * G < P.n_chunks) ? __ldg(P.rdesc + c + 2 * G) : dzero;
-
     const int e_lo = d_cur.x, nent = d_cur.y, t_lo = d_cur.z, ntri = d_cur.w;
     const bool is_long = nent > RND_MAX_ENT;  // k_assemble_long's
     const bool valid = !is_long && lane < nent;
+
+    // positions of the NEXT round: pulled into L2 now (no registers, no scoreboard), loaded into
+    // registers at the end of this round, when the derivative registers are free again
+    if (lane < round_entries(d_nxt)) prefetch_pos_l2(P.pos, ids_nxt);
 
     // ---- lane = entry: J, coefficients ----
     Entry E;
@@ -908,12 +982,18 @@ k_assemble_tile(const AsmParams<T> P) {
     E.cf = {0, 0, 0, 0, 0};
     E.en = 0.0;
     int er[3] = {cur.er[0], cur.er[1], cur.er[2]};
-    if (valid) {
-      eval_core(x, cur.pay, P.sigma, P.hess_mode, E);
-      unpermute_own(E, S.stage + lane * STG_STRIDE, er);
-    }
-    // ---- positions of the next round: its vertex ids were requested at the top of this round ----
-    if (lane < min(d_nxt.y, RND_MAX_ENT)) load_pos18(P.pos, nxt.ids, x);
+    if (valid) eval_core(x, cur.pay, P.sigma, P.hess_mode, E);
+    // ---- operands of round c + G, vertex ids of c + 2G, descriptor of c + 3G: requested after the
+    //      register peak of the derivative code, consumed a round later ----
+    RoundOps nxt;
+    load_round_ops(P, d_nxt, lane, nxt);
+    int ids_nn[6];
+    load_round_ids(P, d_nn, lane, ids_nn);
+    const int4 d_nnn = (c + 3 * G < P.n_chunks) ? __ldg(P.rdesc + c + 3 * G) : dzero;
+    // the staging area aliases the row tile: the copy engine must have read the previous round's last row
+    bulk_wait_read();
+    __syncwarp();
+    if (valid) unpermute_own(E, stage + lane * STG_STRIDE, er);
 
     if (!is_long) {
       // lane = triangle: tile slots (16-byte slots, prefix sum over the round's triangles)
@@ -932,50 +1012,71 @@ k_assemble_tile(const AsmParams<T> P) {
       // bit i of heads: entry i is the first of its triangle; my_ti: triangle of entry `lane`
       const unsigned heads = __reduce_or_sync(FULL, (lane < ntri) ? (1u << (cur.e0 - e_lo)) : 0u);
       const int my_ti = __popc(heads & (0xffffffffu >> (31 - lane))) - 1;
+      const int my_first = (lane < ntri) ? cur.e0 - e_lo : nent;  // first entry of triangle `lane`; nent past the last
 
       // ---- diagonal 9x9 (symmetric: 45 unique) + gradient: stage per entry, sum per triangle ----
-      if (lane < ntri) S.tri_first[lane] = cur.e0 - e_lo;
-      if (lane == 0) S.tri_first[ntri] = nent;
-      if (valid) {
-        double d0[9], d1[9];
+      double d0[9], d1[9];
 #pragma unroll
-        for (int i = 0; i < 9; ++i) {
-          d0[i] = E.cf.c00 * E.g0[i] + E.cf.c01 * E.g1[i];
-          d1[i] = E.cf.c01 * E.g0[i] + E.cf.c11 * E.g1[i];
-        }
-        double* st = S.stage + lane * STG_STRIDE;
-        int k = 0;
-#pragma unroll
-        for (int r = 0; r < 9; ++r)
-#pragma unroll
-          for (int q = r; q < 9; ++q, ++k) st[k] = E.g0[r] * d0[q] + E.g1[r] * d1[q];
-#pragma unroll
-        for (int i = 0; i < 9; ++i) st[NDIAG + i] = E.cf.cg0 * E.g0[i] + E.cf.cg1 * E.g1[i];
+      for (int i = 0; i < 9; ++i) {
+        d0[i] = E.cf.c00 * E.g0[i] + E.cf.c01 * E.g1[i];
+        d1[i] = E.cf.c01 * E.g0[i] + E.cf.c11 * E.g1[i];
       }
-      __syncwarp();
-      // lane = component (two each), entries in order (deterministic); the sums replace the staged
-      // values of the triangle's first entry
-      if (lane < NSTG / 2) {
-        for (int tt = 0; tt < ntri; ++tt) {
-          const int i0 = S.tri_first[tt], i1 = S.tri_first[tt + 1];
-          double* p = S.stage + i0 * STG_STRIDE + lane;
-          double a0 = p[0], a1 = p[NSTG / 2];
-          for (int i = i0 + 1; i < i1; ++i) {
-            const double* pi = S.stage + i * STG_STRIDE + lane;
-            a0 += pi[0];
-            a1 += pi[NSTG / 2];
+#pragma unroll
+      for (int h = 0; h < 2; ++h) {
+        if (valid) {
+          double* st = stage + lane * STG_STRIDE - h * STG_PASS;
+          int k = 0;
+#pragma unroll
+          for (int r = 0; r < 9; ++r)
+#pragma unroll
+            for (int q = r; q < 9; ++q, ++k)
+              if (k >= h * STG_PASS && k < (h + 1) * STG_PASS) st[k] = E.g0[r] * d0[q] + E.g1[r] * d1[q];
+#pragma unroll
+          for (int i = 0; i < 9; ++i)
+            if (NDIAG + i >= h * STG_PASS && NDIAG + i < (h + 1) * STG_PASS)
+              st[NDIAG + i] = E.cf.cg0 * E.g0[i] + E.cf.cg1 * E.g1[i];
+        }
+        __syncwarp();
+        // per-triangle sums, lane = component, entries in ascending order (deterministic); two
+        // triangles at a time so that two independent load -> add chains are in flight.  The loops
+        // are warp-uniform: lanes >= STG_PASS only take part in the shuffles.
+        for (int tt = 0; tt < ntri; tt += 2) {
+          const int a0 = __shfl_sync(FULL, my_first, tt), a1 = __shfl_sync(FULL, my_first, tt + 1);
+          const int b1 = __shfl_sync(FULL, my_first, tt + 2);
+          const int dA = a1 - a0, dB = b1 - a1, dn = max(dA, dB);
+          if (lane < STG_PASS) {
+            const double* pA = stage + a0 * STG_STRIDE + lane;
+            const double* pB = stage + a1 * STG_STRIDE + lane;
+            // the first RED_UNR entries of both triangles are loaded before any add (one shared-memory
+            // latency per pair of triangles, not one per entry); longer triangles finish in a loop
+            double vA[RED_UNR], vB[RED_UNR];
+#pragma unroll
+            for (int j = 0; j < RED_UNR; ++j) {
+              vA[j] = (j < dA) ? pA[j * STG_STRIDE] : 0.0;
+              vB[j] = (j < dB) ? pB[j * STG_STRIDE] : 0.0;
+            }
+            double accA = vA[0], accB = vB[0];
+#pragma unroll
+            for (int j = 1; j < RED_UNR; ++j) {
+              accA += vA[j];
+              accB += vB[j];
+            }
+#pragma unroll 2
+            for (int j = RED_UNR; j < dn; ++j) {
+              if (j < dA) accA += pA[j * STG_STRIDE];
+              if (j < dB) accB += pB[j * STG_STRIDE];
+            }
+            S.dsum[tt][h * STG_PASS + lane] = accA;
+            if (dB > 0) S.dsum[tt + 1][h * STG_PASS + lane] = accB;
+            if (h == 1 && lane >= NDIAG - STG_PASS) {  // gradient of the triangle's three vertices
+              T* ts = P.tslot + 9 * ((int64_t)t_lo + tt) + (lane - (NDIAG - STG_PASS));
+              ts[0] = (T)accA;
+              if (dB > 0) ts[9] = (T)accB;
+            }
           }
-          p[0] = a0;
-          p[NSTG / 2] = a1;
         }
+        __syncwarp();
       }
-      __syncwarp();
-      // gradient of the round's triangles (lane = component of the 9)
-      if (lane < 9)
-        for (int tt = 0; tt < ntri; ++tt) {
-          const int i0 = S.tri_first[tt];
-          P.tslot[9 * ((int64_t)t_lo + tt) + lane] = (T)S.stage[i0 * STG_STRIDE + NDIAG + lane];
-        }
 
 #pragma unroll
       for (int m = 0; m < 3; ++m) {
@@ -983,8 +1084,10 @@ k_assemble_tile(const AsmParams<T> P) {
             (unsigned long long)((cur.rb[m] >= 0) ? (P.vals + 9 * cur.rb[m]) : (P.tvals + 9 * (-cur.rb[m] - 1)));
         const int my_off = slot_off + (int)(g & 15ull);
         // the tile is single-buffered: the copy engine must have read the previous row's runs
-        bulk_wait_read();
-        __syncwarp();
+        if (m > 0) {
+          bulk_wait_read();
+          __syncwarp();
+        }
         if (lane < ntri) {
           S.run_off[lane] = my_off;
 #pragma unroll
@@ -1013,11 +1116,19 @@ k_assemble_tile(const AsmParams<T> P) {
           const int r_ = 3 * m + cq / 3, c_ = 3 * cn + cq % 3;
           const int lo = min(r_, c_), hi = max(r_, c_);
           const int uidx = lo * 9 - (lo * (lo - 1)) / 2 + (hi - lo);
-          for (int tt = 0; tt < ntri; ++tt) {
-            const int i0 = S.tri_first[tt];
-            *reinterpret_cast<T*>(S.tile + S.diag_off[tt][cn] + cq * (int)sizeof(T)) = (T)S.stage[i0 * STG_STRIDE + uidx];
+          int off[RND_MAX_TRI];
+          T val[RND_MAX_TRI];
+#pragma unroll
+          for (int tt = 0; tt < RND_MAX_TRI; ++tt) {  // slots past ntri hold stale but readable data
+            off[tt] = S.diag_off[tt][cn];
+            val[tt] = (T)S.dsum[tt][uidx];
           }
+#pragma unroll
+          for (int tt = 0; tt < RND_MAX_TRI; ++tt)
+            if (tt < ntri) *reinterpret_cast<T*>(S.tile + off[tt] + cq * (int)sizeof(T)) = val[tt];
         }
+        // positions of the next round (L2 hits): requested as soon as this round's J is dead
+        if (m == 2 && lane < round_entries(d_nxt)) load_pos18(P.pos, ids_nxt, x);
         fence_async_smem();
         __syncwarp();
         // ---- lane = triangle: hand the run to the copy engine ----
@@ -1033,8 +1144,8 @@ k_assemble_tile(const AsmParams<T> P) {
           bulk_commit();
         }
       }
-      __syncwarp();  // the next round's spill / staging reuses S.stage
     }
+    if (is_long && lane < round_entries(d_nxt)) load_pos18(P.pos, ids_nxt, x);
     double e_acc = E.en;
 #pragma unroll
     for (int o = 16; o > 0; o >>= 1) e_acc += __shfl_down_sync(FULL, e_acc, o);
@@ -1043,7 +1154,10 @@ k_assemble_tile(const AsmParams<T> P) {
     c += G;
     d_cur = d_nxt;
     d_nxt = d_nn;
+    d_nn = d_nnn;
     cur = nxt;
+#pragma unroll
+    for (int i = 0; i < 6; ++i) ids_nxt[i] = ids_nn[i];
   }
   bulk_wait_all();  // shared memory must outlive the engine's reads
 }
@@ -1057,7 +1171,7 @@ k_assemble_long(const AsmParams<T> P) {
   extern __shared__ __align__(16) unsigned char s_raw[];
   constexpr unsigned FULL = 0xffffffffu;
   const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-  TileWarpSmem<T>& S = reinterpret_cast<TileWarpSmem<T>*>(s_raw)[warp];
+  LongWarpSmem& S = reinterpret_cast<LongWarpSmem*>(s_raw)[warp];
   const int64_t li = (int64_t)blockIdx.x * TILE_WARPS + warp;
   if (li >= P.n_long) return;
   const int c = __ldg(P.long_list + li);
@@ -1090,7 +1204,7 @@ k_assemble_long(const AsmParams<T> P) {
       load_pos18(P.pos, ids, x);
       eval_core(x, (unsigned)__ldg(P.dvals + e), P.sigma, P.hess_mode, E);
       e_acc += E.en;
-      unpermute_own(E, S.stage + lane * STG_STRIDE, er);
+      unpermute_own(E, S.stage + lane * LONG_STRIDE, er);
     }
 #pragma unroll
     for (int m = 0; m < 3; ++m) {
@@ -1109,7 +1223,7 @@ k_assemble_long(const AsmParams<T> P) {
 #pragma unroll
             for (int j = 0; j < 3; ++j) blk[3 * i + j] = (T)(a[i] * E.g0[9 + 3 * n + j] + b[i] * E.g1[9 + 3 * n + j]);
         }
-        double* st = S.stage + lane * STG_STRIDE;
+        double* st = S.stage + lane * LONG_STRIDE;
 #pragma unroll
         for (int n = 0; n < 3; ++n)
 #pragma unroll
@@ -1121,7 +1235,7 @@ k_assemble_long(const AsmParams<T> P) {
       }
       __syncwarp();
       if (lane < 30)
-        for (int i = 0; i < nvalid; ++i) acc[m] += S.stage[i * STG_STRIDE + lane];
+        for (int i = 0; i < nvalid; ++i) acc[m] += S.stage[i * LONG_STRIDE + lane];
       __syncwarp();
     }
   }
@@ -1250,27 +1364,6 @@ k_entry_reduce(const AsmParams<T> P, const int* __restrict__ round_list, int64_t
 // cp.async (LDGSTS: no registers held while in flight) into lane-private slots, vertex ids one
 // round further ahead and descriptors two, so that the three dependent gathers of a round
 // (descriptor -> vertex ids -> positions) are all off the critical path.
-template <typename T>
-__device__ __forceinline__ void cp_async_elem(T* sdst, const T* gsrc) {
-  const unsigned sa = (unsigned)__cvta_generic_to_shared(sdst);
-  if (sizeof(T) == 8) asm volatile("cp.async.ca.shared.global [%0], [%1], 8;" ::"r"(sa), "l"(gsrc) : "memory");
-  else asm volatile("cp.async.ca.shared.global [%0], [%1], 4;" ::"r"(sa), "l"(gsrc) : "memory");
-}
-__device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
-template <int N>
-__device__ __forceinline__ void cp_async_wait() { asm volatile("cp.async.wait_group %0;" ::"n"(N) : "memory"); }
-
-// 18 values of six vertices -> lane-private shared slots buf[k * 32 + lane]
-template <typename T>
-__device__ __forceinline__ void gather18_async(T* buf, int lane, const T* __restrict__ src, const int (&ids)[6]) {
-#pragma unroll
-  for (int v = 0; v < 6; ++v) {
-    const T* g = src + 3 * (int64_t)ids[v];
-#pragma unroll
-    for (int k = 0; k < 3; ++k) cp_async_elem(buf + (3 * v + k) * 32 + lane, g + k);
-  }
-}
-
 #ifndef TT_PIPE_WARPS
 #define TT_PIPE_WARPS 4
 #endif

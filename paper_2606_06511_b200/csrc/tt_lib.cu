@@ -569,7 +569,7 @@ tt_status numeric_impl(tt_ctx* ctx, const tt_problem* q, void* energy_sum, void*
       k_assemble_tile<T><<<(unsigned)(full < pers ? full : pers), 32 * TILE_WARPS, smem, st>>>(p);
       if (ctx->n_long > 0) {
         TT_LAUNCH_CHECK();
-        k_assemble_long<T><<<grid_for(ctx->n_long, TILE_WARPS), 32 * TILE_WARPS, smem, st>>>(p);
+        k_assemble_long<T><<<grid_for(ctx->n_long, TILE_WARPS), 32 * TILE_WARPS, sizeof(LongWarpSmem) * TILE_WARPS, st>>>(p);
       }
     } else {
       tt_status s1 = launch_entry_reduce<T, 1>(ctx, p, st);
@@ -641,10 +641,8 @@ tt_status tt_create(const tt_options* opt, tt_ctx** out) {
     cudaError_t e = cudaSuccess;
     auto opt_in = [&](const void* f, size_t smem) { if (e == cudaSuccess) e = cudaFuncSetAttribute(f, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem); };
     opt_in((const void*)ttk::k_assemble_tile<double>, sizeof(ttk::TileWarpSmem<double>) * ttk::TILE_WARPS);
-    opt_in((const void*)ttk::k_assemble_long<double>, sizeof(ttk::TileWarpSmem<double>) * ttk::TILE_WARPS);
-    opt_in((const void*)ttk::k_assemble_tile<float>, sizeof(ttk::TileWarpSmem<float>) * ttk::TILE_WARPS);
-    opt_in((const void*)ttk::k_assemble_long<float>, sizeof(ttk::TileWarpSmem<float>) * ttk::TILE_WARPS);
-    int sms = 0, nb0 = 0, nb1 = 0;
+        opt_in((const void*)ttk::k_assemble_tile<float>, sizeof(ttk::TileWarpSmem<float>) * ttk::TILE_WARPS);
+        int sms = 0, nb0 = 0, nb1 = 0;
     if (e == cudaSuccess) e = cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, opt->device);
     if (e == cudaSuccess) e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&nb0, ttk::k_assemble_tile<double>, 32 * ttk::TILE_WARPS, sizeof(ttk::TileWarpSmem<double>) * ttk::TILE_WARPS);
     if (e == cudaSuccess) e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&nb1, ttk::k_assemble_tile<float>, 32 * ttk::TILE_WARPS, sizeof(ttk::TileWarpSmem<float>) * ttk::TILE_WARPS);
