@@ -785,21 +785,24 @@ __device__ __forceinline__ void eval_core(const double (&x)[18], unsigned pay, d
   }
 }
 
-// Brings the own half of J back to the triangle's own vertex order through the lane's private
-// slice of shared memory (18 stores at permuted addresses, 18 loads), and the partner's block
-// ranks into recorded order (integer selects).
-__device__ __forceinline__ void unpermute_own(Entry& E, double* lane_smem /*>= 18 doubles*/, int (&er)[3]) {
-#pragma unroll
-  for (int r = 0; r < 3; ++r)
-#pragma unroll
-    for (int cc = 0; cc < 3; ++cc) {
-      lane_smem[3 * E.po[r] + cc] = E.g0[3 * r + cc];
-      lane_smem[9 + 3 * E.po[r] + cc] = E.g1[3 * r + cc];
-    }
+// Brings the own half of J back to the triangle's own vertex order (selects on the recorded
+// permutation: no shared-memory round trip, the L1 data pipe is the kernel's busiest unit), and the
+// partner's block ranks into recorded order.
+__device__ __forceinline__ void unpermute_own(Entry& E, int (&er)[3]) {
+  double t0[9], t1[9];
 #pragma unroll
   for (int i = 0; i < 9; ++i) {
-    E.g0[i] = lane_smem[i];
-    E.g1[i] = lane_smem[9 + i];
+    t0[i] = E.g0[i];
+    t1[i] = E.g1[i];
+  }
+#pragma unroll
+  for (int i = 0; i < 3; ++i) {  // own vertex i = recorded position r with po[r] == i
+    const bool p0 = E.po[0] == i, p1 = E.po[1] == i;
+#pragma unroll
+    for (int cc = 0; cc < 3; ++cc) {
+      E.g0[3 * i + cc] = p0 ? t0[cc] : (p1 ? t0[3 + cc] : t0[6 + cc]);
+      E.g1[3 * i + cc] = p0 ? t1[cc] : (p1 ? t1[3 + cc] : t1[6 + cc]);
+    }
   }
   const int e0 = er[0], e1 = er[1], e2 = er[2];
 #pragma unroll
@@ -993,7 +996,7 @@ k_assemble_tile(const AsmParams<T> P) {
     // the staging area aliases the row tile: the copy engine must have read the previous round's last row
     bulk_wait_read();
     __syncwarp();
-    if (valid) unpermute_own(E, stage + lane * STG_STRIDE, er);
+    if (valid) unpermute_own(E, er);
 
     if (!is_long) {
       // lane = triangle: tile slots (16-byte slots, prefix sum over the round's triangles)
@@ -1204,7 +1207,7 @@ k_assemble_long(const AsmParams<T> P) {
       load_pos18(P.pos, ids, x);
       eval_core(x, (unsigned)__ldg(P.dvals + e), P.sigma, P.hess_mode, E);
       e_acc += E.en;
-      unpermute_own(E, S.stage + lane * LONG_STRIDE, er);
+      unpermute_own(E, er);
     }
 #pragma unroll
     for (int m = 0; m < 3; ++m) {
