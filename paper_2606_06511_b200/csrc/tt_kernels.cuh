@@ -1165,12 +1165,168 @@ k_assemble_tile(const AsmParams<T> P) {
   bulk_wait_all();  // shared memory must outlive the engine's reads
 }
 
-// Long triangles (more than RND_MAX_ENT partners): one warp per triangle, entries in groups of 32,
+// Long triangles with at most LONG_TILE_MAX partners (a round of their own): one warp per triangle.
+// A row of the triangle is ONE run of 3 (deg + 1) blocks; it is built in a shared-memory tile and
+// handed to the copy engine like the runs of k_assemble_tile.  The tile holds one row, so the warp
+// makes three passes over the triangle's entries (m = 0, 1, 2).  CACHE = true (deg <= LONG_CACHE_MAX):
+// pass 0 leaves J and the coefficients of every entry in shared memory (lane-private columns) and
+// passes 1, 2 reload them; CACHE = false: J is re-evaluated in every pass (the derivative code is
+// ~20 % of an entry's cost; three tiles or a larger cache would not fit).  The diagonal blocks and
+// the gradient of row m are summed in registers: lane-private partial sums over the groups of 32
+// entries, then a reduce-scatter butterfly (fixed tree: deterministic) that leaves value L in lane L.
+// Launched after k_assemble_tile on the same stream (it overwrites that round's energy slot).
+constexpr int LONG_TILE_MAX = 127;
+constexpr int LONG_CACHE_MAX = 64;
+constexpr int JC_N = 41;  // g0[18], g1[18], c00, c11, c01, cg0, cg1
+template <typename T, bool CACHE>
+struct alignas(16) LongTileSmem {
+  unsigned char tile[27 * sizeof(T) * ((CACHE ? LONG_CACHE_MAX : LONG_TILE_MAX) + 1) + 16];
+  double jc[CACHE ? JC_N * LONG_CACHE_MAX : 1];  // value k of entry (group gi, lane) at [(gi * JC_N + k) * 32 + lane]
+};
+
+// v[0..32) per lane -> lane L returns the warp sum of v[L]
+__device__ __forceinline__ double warp_reduce_scatter32(double (&v)[32], int lane) {
+  constexpr unsigned FULL = 0xffffffffu;
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) {
+    const bool up = (lane & o) != 0;
+#pragma unroll
+    for (int i = 0; i < o; ++i) {
+      const double send = up ? v[i] : v[i + o];
+      const double keep = up ? v[i + o] : v[i];
+      v[i] = keep + __shfl_xor_sync(FULL, send, o);
+    }
+  }
+  return v[0];
+}
+
+template <typename T, bool CACHE>
+__global__ void __launch_bounds__(32)
+k_assemble_long_tile(const AsmParams<T> P) {
+  extern __shared__ __align__(16) unsigned char s_raw[];
+  constexpr unsigned FULL = 0xffffffffu;
+  LongTileSmem<T, CACHE>& S = *reinterpret_cast<LongTileSmem<T, CACHE>*>(s_raw);
+  const int lane = threadIdx.x;
+  const int64_t li = blockIdx.x;
+  if (li >= P.n_long) return;
+  const int c = __ldg(P.long_list + li);
+  const int4 d = __ldg(P.rdesc + c);
+  if (CACHE ? (d.y > LONG_CACHE_MAX) : (d.y <= LONG_CACHE_MAX || d.y > LONG_TILE_MAX)) return;  // another kernel's
+  const int64_t ti = d.z;
+  const int e_lo = d.x, e_hi = d.x + d.y;
+  const int run_bytes = 27 * (int)sizeof(T) * (d.y + 1);
+  double e_acc = 0.0;
+#pragma unroll 1
+  for (int m = 0; m < 3; ++m) {
+    const int64_t rb = __ldg(P.rowbase + 3 * ti + m);
+    const int my_dr = (lane < 27) ? __ldg(P.drank + 3 * ti + lane / 9) : 0;
+    const unsigned long long g = (unsigned long long)((rb >= 0) ? (P.vals + 9 * rb) : (P.tvals + 9 * (-rb - 1)));
+    unsigned char* const run = S.tile + (int)(g & 15ull);
+    double acc[32];  // diagonal-row blocks (p_m, p_n) at [9 n + 3 i + j], gradient of p_m at [27 + i]
+#pragma unroll
+    for (int k = 0; k < 32; ++k) acc[k] = 0.0;
+    if (m > 0) {  // the copy engine must have read the previous row
+      bulk_wait_read();
+      __syncwarp();
+    }
+    int gi = 0;
+    for (int base = e_lo; base < e_hi; base += 32, ++gi) {
+      if (base + lane < e_hi) {
+        const int64_t e = (int64_t)base + lane;
+        int er[3];
+#pragma unroll
+        for (int n = 0; n < 3; ++n) er[n] = __ldg(P.erank + 3 * e + n);
+        Entry E;
+        double* const jc = S.jc + gi * JC_N * 32 + lane;
+        if (!CACHE || m == 0) {
+          int ids[6];
+          {
+            const int2* iv = reinterpret_cast<const int2*>(P.everts + 6 * e);
+            const int2 v0 = __ldg(iv), v1 = __ldg(iv + 1), v2 = __ldg(iv + 2);
+            ids[0] = v0.x; ids[1] = v0.y; ids[2] = v1.x; ids[3] = v1.y; ids[4] = v2.x; ids[5] = v2.y;
+          }
+          double x[18];
+          load_pos18(P.pos, ids, x);
+          eval_core(x, (unsigned)__ldg(P.dvals + e), P.sigma, P.hess_mode, E);
+          if (m == 0) e_acc += E.en;
+          unpermute_own(E, er);
+          if (CACHE) {
+#pragma unroll
+            for (int k = 0; k < 18; ++k) {
+              jc[k * 32] = E.g0[k];
+              jc[(18 + k) * 32] = E.g1[k];
+            }
+            jc[36 * 32] = E.cf.c00; jc[37 * 32] = E.cf.c11; jc[38 * 32] = E.cf.c01;
+            jc[39 * 32] = E.cf.cg0; jc[40 * 32] = E.cf.cg1;
+          }
+        } else {
+#pragma unroll
+          for (int k = 0; k < 18; ++k) {
+            E.g0[k] = jc[k * 32];
+            E.g1[k] = jc[(18 + k) * 32];
+          }
+          E.cf.c00 = jc[36 * 32]; E.cf.c11 = jc[37 * 32]; E.cf.c01 = jc[38 * 32];
+          E.cf.cg0 = jc[39 * 32]; E.cf.cg1 = jc[40 * 32];
+          // er must follow the recorded -> partner order again (pp is not cached: redo the selects)
+          const unsigned pay = (unsigned)__ldg(P.dvals + e);
+          const bool side = (pay & 1u) != 0u;
+          const unsigned cp = side ? ((pay >> 1) & 63u) : ((pay >> 7) & 63u);  // partner triangle's config
+          int pp[3];
+          pp[0] = (int)(cp & 3u); pp[1] = (int)((cp >> 2) & 3u); pp[2] = 3 - pp[0] - pp[1];
+          const int e0 = er[0], e1 = er[1], e2 = er[2];
+#pragma unroll
+          for (int r = 0; r < 3; ++r) er[r] = (pp[r] == 0) ? e0 : ((pp[r] == 1) ? e1 : e2);
+        }
+        double a[3], b[3];
+#pragma unroll
+        for (int i = 0; i < 3; ++i) {  // own row m: dynamic m, selected from the three static rows
+          const double g0m = (m == 0) ? E.g0[i] : ((m == 1) ? E.g0[3 + i] : E.g0[6 + i]);
+          const double g1m = (m == 0) ? E.g1[i] : ((m == 1) ? E.g1[3 + i] : E.g1[6 + i]);
+          a[i] = E.cf.c00 * g0m + E.cf.c01 * g1m;
+          b[i] = E.cf.c01 * g0m + E.cf.c11 * g1m;
+          acc[27 + i] += E.cf.cg0 * g0m + E.cf.cg1 * g1m;
+        }
+#pragma unroll
+        for (int n = 0; n < 3; ++n) {
+          T* blk = reinterpret_cast<T*>(run) + 9 * er[n];
+#pragma unroll
+          for (int i = 0; i < 3; ++i)
+#pragma unroll
+            for (int j = 0; j < 3; ++j) {
+              blk[3 * i + j] = (T)(a[i] * E.g0[9 + 3 * n + j] + b[i] * E.g1[9 + 3 * n + j]);
+              acc[9 * n + 3 * i + j] += a[i] * E.g0[3 * n + j] + b[i] * E.g1[3 * n + j];
+            }
+        }
+      }
+    }
+    const double tot = warp_reduce_scatter32(acc, lane);  // lane L: sum of value L
+    if (lane < 27) reinterpret_cast<T*>(run)[9 * my_dr + lane % 9] = (T)tot;
+    else if (lane < 30) P.tslot[9 * ti + 3 * m + (lane - 27)] = (T)tot;
+    fence_async_smem();
+    __syncwarp();
+    if (lane == 0) {
+      int head = (int)((16ull - (g & 15ull)) & 15ull);
+      head = min(head, run_bytes);
+      const int body = (run_bytes - head) & ~15;
+      for (int o = 0; o < head; o += (int)sizeof(T)) *reinterpret_cast<T*>(g + o) = *reinterpret_cast<const T*>(run + o);
+      if (body > 0) bulk_s2g(reinterpret_cast<void*>(g + head), run + head, (uint32_t)body);
+      for (int o = head + body; o < run_bytes; o += (int)sizeof(T))
+        *reinterpret_cast<T*>(g + o) = *reinterpret_cast<const T*>(run + o);
+      bulk_commit();
+    }
+  }
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) e_acc += __shfl_down_sync(FULL, e_acc, o);
+  if (lane == 0) P.chunk_energy[c] = e_acc;
+  bulk_wait_all();  // shared memory must outlive the engine's reads
+}
+
+// Triangles with more than LONG_TILE_MAX partners: one warp per triangle, entries in groups of 32,
 // off-diagonal blocks stored directly, diagonal rows and gradient carried across groups.
 // Launched after k_assemble_tile on the same stream (it overwrites that round's energy slot).
 template <typename T>
 __global__ void __launch_bounds__(32 * TILE_WARPS)
-k_assemble_long(const AsmParams<T> P) {
+k_assemble_long_direct(const AsmParams<T> P) {
   extern __shared__ __align__(16) unsigned char s_raw[];
   constexpr unsigned FULL = 0xffffffffu;
   const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
@@ -1179,6 +1335,7 @@ k_assemble_long(const AsmParams<T> P) {
   if (li >= P.n_long) return;
   const int c = __ldg(P.long_list + li);
   const int4 d = __ldg(P.rdesc + c);
+  if (d.y <= LONG_TILE_MAX) return;  // k_assemble_long_tile's
   const int64_t ti = d.z;
   const int e_lo = d.x, e_hi = d.x + d.y;
   T* rowp[3];

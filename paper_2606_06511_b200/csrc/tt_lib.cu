@@ -90,6 +90,9 @@ struct tt_ctx {
   // device-side timing of the three big kernels (events recorded on the caller's stream)
   cudaEvent_t ev[3][2] = {{nullptr, nullptr}, {nullptr, nullptr}, {nullptr, nullptr}};
   bool ev_used[3] = {false, false, false};
+  // host-buffer entry point: copies that do not feed the next kernel travel on a second stream
+  cudaStream_t side = nullptr;
+  cudaEvent_t ev_in = nullptr, ev_p = nullptr, ev_num = nullptr, ev_side = nullptr;
 };
 
 namespace {
@@ -569,7 +572,11 @@ tt_status numeric_impl(tt_ctx* ctx, const tt_problem* q, void* energy_sum, void*
       k_assemble_tile<T><<<(unsigned)(full < pers ? full : pers), 32 * TILE_WARPS, smem, st>>>(p);
       if (ctx->n_long > 0) {
         TT_LAUNCH_CHECK();
-        k_assemble_long<T><<<grid_for(ctx->n_long, TILE_WARPS), 32 * TILE_WARPS, sizeof(LongWarpSmem) * TILE_WARPS, st>>>(p);
+        k_assemble_long_tile<T, true><<<(unsigned)ctx->n_long, 32, sizeof(LongTileSmem<T, true>), st>>>(p);
+        TT_LAUNCH_CHECK();
+        k_assemble_long_tile<T, false><<<(unsigned)ctx->n_long, 32, sizeof(LongTileSmem<T, false>), st>>>(p);
+        TT_LAUNCH_CHECK();
+        k_assemble_long_direct<T><<<grid_for(ctx->n_long, TILE_WARPS), 32 * TILE_WARPS, sizeof(LongWarpSmem) * TILE_WARPS, st>>>(p);
       }
     } else {
       tt_status s1 = launch_entry_reduce<T, 1>(ctx, p, st);
@@ -637,11 +644,24 @@ tt_status tt_create(const tt_options* opt, tt_ctx** out) {
   for (int i = 0; i < 3; ++i)
     for (int j = 0; j < 2; ++j)
       if (cudaEventCreate(&c->ev[i][j]) != cudaSuccess) { delete c; return TT_ERR_CUDA; }
+  if (cudaStreamCreateWithFlags(&c->side, cudaStreamNonBlocking) != cudaSuccess ||
+      cudaEventCreateWithFlags(&c->ev_in, cudaEventDisableTiming) != cudaSuccess ||
+      cudaEventCreateWithFlags(&c->ev_p, cudaEventDisableTiming) != cudaSuccess ||
+      cudaEventCreateWithFlags(&c->ev_num, cudaEventDisableTiming) != cudaSuccess ||
+      cudaEventCreateWithFlags(&c->ev_side, cudaEventDisableTiming) != cudaSuccess) {
+    (void)cudaGetLastError();
+    tt_destroy(c);
+    return TT_ERR_CUDA;
+  }
   {
     cudaError_t e = cudaSuccess;
     auto opt_in = [&](const void* f, size_t smem) { if (e == cudaSuccess) e = cudaFuncSetAttribute(f, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem); };
     opt_in((const void*)ttk::k_assemble_tile<double>, sizeof(ttk::TileWarpSmem<double>) * ttk::TILE_WARPS);
         opt_in((const void*)ttk::k_assemble_tile<float>, sizeof(ttk::TileWarpSmem<float>) * ttk::TILE_WARPS);
+    opt_in((const void*)ttk::k_assemble_long_tile<double, true>, sizeof(ttk::LongTileSmem<double, true>));
+    opt_in((const void*)ttk::k_assemble_long_tile<double, false>, sizeof(ttk::LongTileSmem<double, false>));
+    opt_in((const void*)ttk::k_assemble_long_tile<float, true>, sizeof(ttk::LongTileSmem<float, true>));
+    opt_in((const void*)ttk::k_assemble_long_tile<float, false>, sizeof(ttk::LongTileSmem<float, false>));
         int sms = 0, nb0 = 0, nb1 = 0;
     if (e == cudaSuccess) e = cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, opt->device);
     if (e == cudaSuccess) e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&nb0, ttk::k_assemble_tile<double>, 32 * ttk::TILE_WARPS, sizeof(ttk::TileWarpSmem<double>) * ttk::TILE_WARPS);
@@ -671,6 +691,9 @@ void tt_destroy(tt_ctx* ctx) {
   for (int i = 0; i < 3; ++i)
     for (int j = 0; j < 2; ++j)
       if (ctx->ev[i][j]) cudaEventDestroy(ctx->ev[i][j]);
+  for (cudaEvent_t e : {ctx->ev_in, ctx->ev_p, ctx->ev_num, ctx->ev_side})
+    if (e) cudaEventDestroy(e);
+  if (ctx->side) cudaStreamDestroy(ctx->side);
   delete ctx;
 }
 
@@ -737,44 +760,61 @@ tt_status tt_energy_grad_hess_host(tt_ctx* ctx, const tt_problem* prob, void* en
   TT_CUDA(ctx->h_pairs.ensure(sizeof(int) * 2 * (size_t)P + 16));
   TT_CUDA(ctx->o_grad.ensure(w * 3 * (size_t)nV + 16));
   TT_CUDA(ctx->o_energy.ensure(16));
+  // Copy schedule (PCIe is full duplex; the step is shorter than its copies):
+  //   stream : H2D pos, tris, pairs -> symbolic -> numeric -> [wait p] H.p -> D2H y
+  //   side   : [after the inputs] H2D p (under the symbolic / numeric phase)
+  //            [after numeric] D2H energy, grad, pattern, values (under H.p and the D2H of y)
+  const bool want_hv = p_host && nV;
+  if (want_hv) {
+    TT_CUDA(ctx->h_p.ensure(w * 3 * (size_t)nV + 16));
+    TT_CUDA(ctx->o_y.ensure(w * 3 * (size_t)nV + 16));
+  }
   if (nV) TT_CUDA(cudaMemcpyAsync(ctx->h_pos.p, prob->pos, w * 3 * (size_t)nV, cudaMemcpyHostToDevice, st));
   if (nT) TT_CUDA(cudaMemcpyAsync(ctx->h_tris.p, prob->tris, sizeof(int) * 3 * (size_t)nT, cudaMemcpyHostToDevice, st));
   if (P) TT_CUDA(cudaMemcpyAsync(ctx->h_pairs.p, prob->pairs, sizeof(int) * 2 * (size_t)P, cudaMemcpyHostToDevice, st));
+  TT_CUDA(cudaEventRecord(ctx->ev_in, st));
+  if (want_hv) {
+    TT_CUDA(cudaStreamWaitEvent(ctx->side, ctx->ev_in, 0));
+    TT_CUDA(cudaMemcpyAsync(ctx->h_p.p, p_host, w * 3 * (size_t)nV, cudaMemcpyHostToDevice, ctx->side));
+    TT_CUDA(cudaEventRecord(ctx->ev_p, ctx->side));
+  }
   tt_problem d = *prob;
   d.pos = ctx->h_pos.p;
   d.tris = ctx->h_tris.as<int32_t>();
   d.pairs = ctx->h_pairs.as<int32_t>();
   int64_t nnzb = 0, A = 0;
   s = ctx->opt.dtype == TT_F64 ? symbolic_impl<double>(ctx, &d, &nnzb, &A, st) : symbolic_impl<float>(ctx, &d, &nnzb, &A, st);
-  if (s != TT_OK) return s;
+  if (s != TT_OK) { cudaStreamSynchronize(ctx->side); return s; }
   *nnzb_host = nnzb;
   if (n_active_host) *n_active_host = A;
+  if ((colind_host || vals_host) && nnzb_capacity < nnzb) {
+    cudaStreamSynchronize(ctx->side);
+    cudaStreamSynchronize(st);
+    return fail(ctx, TT_ERR_CAPACITY, "nnzb_capacity %lld < nnzb %lld", (long long)nnzb_capacity, (long long)nnzb);
+  }
   TT_CUDA(ctx->o_vals.ensure(w * 9 * (size_t)nnzb + 16));
   s = ctx->opt.dtype == TT_F64
           ? numeric_impl<double>(ctx, &d, ctx->o_energy.p, ctx->o_grad.p, ctx->rowptr.as<int>(), ctx->colind.as<int>(), ctx->o_vals.p, nnzb, st)
           : numeric_impl<float>(ctx, &d, ctx->o_energy.p, ctx->o_grad.p, ctx->rowptr.as<int>(), ctx->colind.as<int>(), ctx->o_vals.p, nnzb, st);
-  if (s != TT_OK) return s;
+  if (s != TT_OK) { cudaStreamSynchronize(ctx->side); return s; }
   ctx->host_nnzb = nnzb;
-  if (p_host && nV) {
-    TT_CUDA(ctx->h_p.ensure(w * 3 * (size_t)nV + 16));
-    TT_CUDA(ctx->o_y.ensure(w * 3 * (size_t)nV + 16));
-    TT_CUDA(cudaMemcpyAsync(ctx->h_p.p, p_host, w * 3 * (size_t)nV, cudaMemcpyHostToDevice, st));
+  TT_CUDA(cudaEventRecord(ctx->ev_num, st));
+  // results of the numeric phase leave on the side stream while H.p runs
+  TT_CUDA(cudaStreamWaitEvent(ctx->side, ctx->ev_num, 0));
+  TT_CUDA(cudaMemcpyAsync(energy_host, ctx->o_energy.p, w, cudaMemcpyDeviceToHost, ctx->side));
+  if (grad_host && nV) TT_CUDA(cudaMemcpyAsync(grad_host, ctx->o_grad.p, w * 3 * (size_t)nV, cudaMemcpyDeviceToHost, ctx->side));
+  if (rowptr_host) TT_CUDA(cudaMemcpyAsync(rowptr_host, ctx->rowptr.p, sizeof(int) * (size_t)(nV + 1), cudaMemcpyDeviceToHost, ctx->side));
+  if (colind_host && nnzb) TT_CUDA(cudaMemcpyAsync(colind_host, ctx->colind.p, sizeof(int) * (size_t)nnzb, cudaMemcpyDeviceToHost, ctx->side));
+  if (vals_host && nnzb) TT_CUDA(cudaMemcpyAsync(vals_host, ctx->o_vals.p, w * 9 * (size_t)nnzb, cudaMemcpyDeviceToHost, ctx->side));
+  TT_CUDA(cudaEventRecord(ctx->ev_side, ctx->side));
+  if (want_hv) {
+    TT_CUDA(cudaStreamWaitEvent(st, ctx->ev_p, 0));
     s = ctx->opt.dtype == TT_F64 ? hessvec_impl<double>(ctx, &d, ctx->h_p.p, ctx->o_y.p, st)
                                  : hessvec_impl<float>(ctx, &d, ctx->h_p.p, ctx->o_y.p, st);
-    if (s != TT_OK) return s;
+    if (s != TT_OK) { cudaStreamSynchronize(ctx->side); return s; }
     TT_CUDA(cudaMemcpyAsync(y_host, ctx->o_y.p, w * 3 * (size_t)nV, cudaMemcpyDeviceToHost, st));
   }
-  TT_CUDA(cudaMemcpyAsync(energy_host, ctx->o_energy.p, w, cudaMemcpyDeviceToHost, st));
-  if (grad_host && nV) TT_CUDA(cudaMemcpyAsync(grad_host, ctx->o_grad.p, w * 3 * (size_t)nV, cudaMemcpyDeviceToHost, st));
-  if (rowptr_host) TT_CUDA(cudaMemcpyAsync(rowptr_host, ctx->rowptr.p, sizeof(int) * (size_t)(nV + 1), cudaMemcpyDeviceToHost, st));
-  if (colind_host || vals_host) {
-    if (nnzb_capacity < nnzb) {
-      cudaStreamSynchronize(st);
-      return fail(ctx, TT_ERR_CAPACITY, "nnzb_capacity %lld < nnzb %lld", (long long)nnzb_capacity, (long long)nnzb);
-    }
-    if (colind_host && nnzb) TT_CUDA(cudaMemcpyAsync(colind_host, ctx->colind.p, sizeof(int) * (size_t)nnzb, cudaMemcpyDeviceToHost, st));
-    if (vals_host && nnzb) TT_CUDA(cudaMemcpyAsync(vals_host, ctx->o_vals.p, w * 9 * (size_t)nnzb, cudaMemcpyDeviceToHost, st));
-  }
+  TT_CUDA(cudaStreamWaitEvent(st, ctx->ev_side, 0));  // `stream` completes only after the side copies
   TT_CUDA(cudaStreamSynchronize(st));
   return TT_OK;
 }

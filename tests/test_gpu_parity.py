@@ -100,7 +100,7 @@ def run_case(oracle, pb, dtype="f64", hess_mode=1, sigma=1.0, flags=0, check_val
 def test_config0_soup(oracle_mod, mode, dtype):
     from paper_2606_06511_b200 import inputs
     ref, out, st = run_case(oracle_mod, inputs.config0_soup(), dtype, mode)
-    assert st["blocks_merged"] == 0          # own-vertex soup: every row is exclusive
+    assert st["blocks_merged"] == 0          # own-vertex soup: every row is exclusive (long triangles included)
     assert 500 < out["n_active"] < 800
 
 
@@ -159,12 +159,19 @@ def test_config4_sweep_reduced(oracle_mod, dtype):
     assert abs(out["n_active"] / pb.n_pairs - 0.5) < 0.01
 
 
-def test_long_rows_span_cta_rounds(oracle_mod):
-    """Few triangles, many pairs each: a triangle's entries span several 128-entry rounds and
-    exceed the shared-memory ranking limit for some rows (general path by size)."""
+@pytest.mark.parametrize("n_pairs,dtype", [(16_000, "f64"), (16_000, "f32"), (60_000, "f64")])
+def test_long_triangles(oracle_mod, n_pairs, dtype):
+    """Few triangles, many pairs each.  16k pairs: ~40 partners per triangle, a mix of ordinary rounds
+    and long triangles that fit the one-row tile (k_assemble_long_tile); 60k pairs: ~150 partners,
+    beyond the tile (k_assemble_long_direct)."""
     from paper_2606_06511_b200 import inputs
-    pb = inputs.config4_sweep(n_tris=400, n_pairs=60_000, seed=4242)
-    ref, out, st = run_case(oracle_mod, pb, "f64", 1)
+    pb = inputs.config4_sweep(n_tris=400, n_pairs=n_pairs, seed=4242)
+    ref, out, st = run_case(oracle_mod, pb, dtype, 1)
+    deg = np.bincount(pb.pairs[ref["active"].astype(bool)].ravel(), minlength=400)
+    if n_pairs == 16_000:
+        assert ((deg > 32) & (deg <= 127)).sum() > 50 and (deg <= 32).sum() > 20
+    else:
+        assert (deg > 127).sum() > 50
 
 
 # ------------------------------------------------------------------------------------ edge cases
