@@ -77,8 +77,11 @@ __device__ __forceinline__ double block_sum(double v, double* smem /*[THREADS/32
 }
 
 // ------------------------------------------------------------------------------------------ K1
+#ifndef TT_CLS_MIN_CTAS
+#define TT_CLS_MIN_CTAS 3   // 85 registers, 24 warps / SM: 0.755 -> 0.69 ms at 10M candidates (4: 0.73)
+#endif
 template <typename T>
-__global__ void __launch_bounds__(CLS_THREADS)
+__global__ void __launch_bounds__(CLS_THREADS, TT_CLS_MIN_CTAS)
 k_classify(const T* __restrict__ pos, const int* __restrict__ tris, const int2* __restrict__ pairs,
            int64_t P, double sigma, uint32_t* __restrict__ mask, int* __restrict__ blk_count,
            double* __restrict__ blk_energy, T* __restrict__ e_pp, T* __restrict__ tc_out,
@@ -552,6 +555,8 @@ k_round_symbolic(const int* __restrict__ tris, const int* __restrict__ touched, 
   __shared__ int s_own[RSYM_WARPS][3 * RND_MAX_TRI];   // own vertex ids of triangle tt at [3 tt + n]
   __shared__ int s_first[RSYM_WARPS][RND_MAX_TRI + 1];
   __shared__ int s_dup[RSYM_WARPS][RND_MAX_TRI];
+  __shared__ int s_dacc[RSYM_WARPS][3 * RND_MAX_TRI];  // per own column: partner columns below it
+  __shared__ int s_rsum[RSYM_WARPS][RND_MAX_TRI];      // per triangle: sum of the partner columns' ranks
   constexpr unsigned FULL = 0xffffffffu;
   const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
   const int64_t c = (int64_t)blockIdx.x * RSYM_WARPS + warp;
@@ -563,6 +568,8 @@ k_round_symbolic(const int* __restrict__ tris, const int* __restrict__ touched, 
   int* own = s_own[warp];
   int* first = s_first[warp];
   int* dupf = s_dup[warp];
+  int* dacc = s_dacc[warp];
+  int* rsum = s_rsum[warp];
   const uint64_t tmask = (1ull << bitsT) - 1ull;
   // lane = triangle
   int f = 0, l = 0, ov[3] = {0, 0, 0};
@@ -577,6 +584,8 @@ k_round_symbolic(const int* __restrict__ tris, const int* __restrict__ touched, 
     }
     first[lane] = f;
     dupf[lane] = 0;
+    rsum[lane] = 0;
+    dacc[3 * lane] = dacc[3 * lane + 1] = dacc[3 * lane + 2] = 0;
   }
   if (lane == 0) first[ntri] = nent;
   // lane = entry
@@ -596,12 +605,19 @@ k_round_symbolic(const int* __restrict__ tris, const int* __restrict__ touched, 
   const unsigned heads = __reduce_or_sync(FULL, (lane < ntri) ? (1u << f) : 0u);
   const int my_ti = __popc(heads & (0xffffffffu >> (31 - lane))) - 1;
   __syncwarp();
-  // ranks of the entry's three partner columns among the triangle's 3 (deg + 1) candidates
-  int r[3] = {0, 0, 0}, eq[3] = {0, 0, 0};
+  // Rank of a column = number of smaller columns among the triangle's L = 3 (deg + 1) candidates.
+  // Duplicates: the ranks of L distinct values sum to L (L - 1) / 2 and every tied pair lowers the sum
+  // by one, so one integer per triangle (shared-memory atomics: the RESULT is order independent)
+  // replaces all equality counting.  The diagonal columns are ranked by the entries' lanes too:
+  // each adds how many of its three columns lie below each own column.
+  int r[3] = {0, 0, 0};
   int myf = 0, deg = 0;
+  int mo[3] = {0, 0, 0};  // own vertex ids of the entry's triangle
   if (valid) {
     myf = first[my_ti];
     deg = first[my_ti + 1] - myf;
+#pragma unroll
+    for (int n = 0; n < 3; ++n) mo[n] = own[3 * my_ti + n];
   }
   const int maxdeg = __reduce_max_sync(FULL, deg);
   for (int k = 0; k < maxdeg; ++k) {
@@ -609,41 +625,28 @@ k_round_symbolic(const int* __restrict__ tris, const int* __restrict__ touched, 
       const int* o = cand + 3 * (myf + k);
       const int o0 = o[0], o1 = o[1], o2 = o[2];
 #pragma unroll
-      for (int n = 0; n < 3; ++n) {
-        r[n] += (o0 < cv[n]) + (o1 < cv[n]) + (o2 < cv[n]);
-        eq[n] += (o0 == cv[n]) + (o1 == cv[n]) + (o2 == cv[n]);
-      }
+      for (int n = 0; n < 3; ++n) r[n] += (o0 < cv[n]) + (o1 < cv[n]) + (o2 < cv[n]);
     }
   }
-  int mo[3] = {0, 0, 0};  // own vertex ids of the entry's triangle
   if (valid) {
-#pragma unroll
-    for (int n = 0; n < 3; ++n) mo[n] = own[3 * my_ti + n];
 #pragma unroll
     for (int n = 0; n < 3; ++n) {
       r[n] += (mo[0] < cv[n]) + (mo[1] < cv[n]) + (mo[2] < cv[n]);
-      eq[n] += (mo[0] == cv[n]) + (mo[1] == cv[n]) + (mo[2] == cv[n]);
+      atomicAdd(&dacc[3 * my_ti + n], (cv[0] < mo[n]) + (cv[1] < mo[n]) + (cv[2] < mo[n]));
     }
-    if (eq[0] > 1 || eq[1] > 1 || eq[2] > 1) dupf[my_ti] = 1;  // eq counts the column itself once
+    atomicAdd(&rsum[my_ti], r[0] + r[1] + r[2]);
   }
-  // ranks of the diagonal columns: lane = triangle
+  __syncwarp();
   int dr[3] = {0, 0, 0};
   if (lane < ntri) {
-    int dq[3] = {0, 0, 0};
-    for (int k = f; k < l; ++k) {
-      const int o0 = cand[3 * k], o1 = cand[3 * k + 1], o2 = cand[3 * k + 2];
-#pragma unroll
-      for (int n = 0; n < 3; ++n) {
-        dr[n] += (o0 < ov[n]) + (o1 < ov[n]) + (o2 < ov[n]);
-        dq[n] += (o0 == ov[n]) + (o1 == ov[n]) + (o2 == ov[n]);
-      }
-    }
+    int tot = rsum[lane];
 #pragma unroll
     for (int n = 0; n < 3; ++n) {
-      dr[n] += (ov[0] < ov[n]) + (ov[1] < ov[n]) + (ov[2] < ov[n]);
-      dq[n] += (ov[0] == ov[n]) + (ov[1] == ov[n]) + (ov[2] == ov[n]);
+      dr[n] = dacc[3 * lane + n] + (ov[0] < ov[n]) + (ov[1] < ov[n]) + (ov[2] < ov[n]);
+      tot += dr[n];
     }
-    if (dq[0] > 1 || dq[1] > 1 || dq[2] > 1) dupf[lane] = 1;
+    const int L = 3 * (l - f + 1);
+    dupf[lane] = (2 * tot != L * (L - 1)) ? 1 : 0;
   }
   __syncwarp();
   if (valid) {
