@@ -226,7 +226,7 @@ k_tri_symbolic(const int* __restrict__ tris, const int* __restrict__ touched, in
                const int* __restrict__ vcnt, int force_general, int* __restrict__ erank /*[2A][3]*/,
                int* __restrict__ drank /*[n_touched][3]*/, int* __restrict__ rowlen,
                int64_t* __restrict__ tlen /*[3 n_touched]*/, uint8_t* __restrict__ slot_excl /*[3 n_touched]*/,
-               const int* __restrict__ long_list, const int4* __restrict__ rdesc) {
+               const int* __restrict__ long_list, const int4* __restrict__ rdesc, int* __restrict__ vslot1) {
   __shared__ int s_c[SYM_WARPS][SYM_LMAX];
   const int w = threadIdx.x >> 5, l = threadIdx.x & 31;
   const int64_t li = (int64_t)blockIdx.x * SYM_WARPS + w;  // n_touched counts the LONG triangles here
@@ -268,6 +268,7 @@ k_tri_symbolic(const int* __restrict__ tris, const int* __restrict__ touched, in
   if (l < 3) {
     const int p = tris[3 * (int64_t)s + l];
     const bool excl = nodup && !force_general && (vcnt[p] == 1);
+    if (vcnt[p] == 1) vslot1[p] = (int)(3 * ti + l);  // the vertex's only slot (k_gather3)
     slot_excl[3 * ti + l] = excl ? 1 : 0;
     tlen[3 * ti + l] = excl ? 0 : L;
     if (excl) rowlen[p] = L;
@@ -550,7 +551,8 @@ k_round_symbolic(const int* __restrict__ tris, const int* __restrict__ touched, 
                  int64_t n_chunks, const int* __restrict__ tfirst, const uint64_t* __restrict__ keys,
                  const uint16_t* __restrict__ dvals, int bitsT, const int* __restrict__ vcnt, int force_general,
                  int* __restrict__ erank, int* __restrict__ drank, int* __restrict__ rowlen,
-                 int64_t* __restrict__ tlen, uint8_t* __restrict__ slot_excl, int* __restrict__ everts) {
+                 int64_t* __restrict__ tlen, uint8_t* __restrict__ slot_excl, int* __restrict__ everts,
+                 int* __restrict__ vslot1) {
   __shared__ int s_cand[RSYM_WARPS][3 * RND_MAX_ENT];  // partner vertex ids of entry i at [3 i + n]
   __shared__ int s_own[RSYM_WARPS][3 * RND_MAX_TRI];   // own vertex ids of triangle tt at [3 tt + n]
   __shared__ int s_first[RSYM_WARPS][RND_MAX_TRI + 1];
@@ -674,7 +676,9 @@ k_round_symbolic(const int* __restrict__ tris, const int* __restrict__ touched, 
     for (int n = 0; n < 3; ++n) drank[3 * ti + n] = nodup ? dr[n] : 3 * dg + n;
 #pragma unroll
     for (int m = 0; m < 3; ++m) {
-      const bool excl = nodup && !force_general && (__ldg(vcnt + ov[m]) == 1);
+      const bool single = __ldg(vcnt + ov[m]) == 1;
+      const bool excl = nodup && !force_general && single;
+      if (single) vslot1[ov[m]] = (int)(3 * ti + m);  // the vertex's only slot (k_gather3)
       slot_excl[3 * ti + m] = excl ? 1 : 0;
       tlen[3 * ti + m] = excl ? 0 : L;
       if (excl) rowlen[ov[m]] = L;
@@ -1704,18 +1708,27 @@ __global__ void k_merge(const int* __restrict__ run_start, const int* __restrict
   vals[9 * (int64_t)run_dest[u] + comp] = (T)acc;
 }
 
-// out[v] = sum over touched slots of vertex v of tslot[slot] (sorted incidence, fixed order);
-// zero for vertices no active pair touches.
+// out[v] = sum over the touched slots of vertex v of tslot[slot]; zero for vertices no active pair
+// touches.  A vertex with a single slot (always, in a soup) reads it through vslot1; the sorted
+// vertex -> slot incidence (vptr / vslots, fixed order) is built only when some vertex has several.
 template <typename T>
-__global__ void k_gather3(const int* __restrict__ vptr, const uint32_t* __restrict__ vslots, int64_t nV,
-                          const T* __restrict__ tslot, T* __restrict__ out) {
+__global__ void k_gather3(const int* __restrict__ vcnt, const int* __restrict__ vslot1, const int* __restrict__ vptr,
+                          const uint32_t* __restrict__ vslots, int64_t nV, const T* __restrict__ tslot,
+                          T* __restrict__ out) {
   const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
   if (i >= 3 * nV) return;
   const int64_t v = i / 3;
   const int comp = (int)(i - 3 * v);
-  double acc = 0.0;
-  for (int j = vptr[v]; j < vptr[v + 1]; ++j) acc += (double)tslot[3 * (int64_t)vslots[j] + comp];
-  out[i] = (T)acc;
+  const int n = __ldg(vcnt + v);
+  T r = (T)0;
+  if (n == 1) {
+    r = tslot[3 * (int64_t)__ldg(vslot1 + v) + comp];
+  } else if (n > 1) {
+    double acc = 0.0;
+    for (int j = vptr[v]; j < vptr[v + 1]; ++j) acc += (double)tslot[3 * (int64_t)vslots[j] + comp];
+    r = (T)acc;
+  }
+  out[i] = r;
 }
 
 __global__ void k_iota(uint32_t* __restrict__ v, int64_t n) {

@@ -71,7 +71,7 @@ struct tt_ctx {
   // pattern
   DevBuf rowptr64, rowptr, colind;
   // numeric
-  DevBuf everts, rdesc, tfirst, bucket_cnt, bucket_off, long_cnt, long_off, chunk_start, long_list, asm_energy, tvals, tslot, vkeys[2], vvals[2], vptr;
+  DevBuf everts, rdesc, tfirst, bucket_cnt, bucket_off, long_cnt, long_off, chunk_start, long_list, asm_energy, tvals, tslot, vkeys[2], vvals[2], vptr, vslot1;
   DevBuf cub_tmp;
   // host-API mirrors
   DevBuf h_pos, h_tris, h_pairs, h_p, o_vals, o_grad, o_energy, o_y;
@@ -366,6 +366,7 @@ tt_status symbolic_impl(tt_ctx* ctx, const tt_problem* q, int64_t* nnzb_host, in
   TT_CUDA(ctx->toff.ensure(sizeof(int64_t) * (size_t)(3 * n_touched + 1)));
   TT_CUDA(ctx->slot_excl.ensure((size_t)(3 * n_touched + 1)));
   TT_CUDA(ctx->rowbase.ensure(sizeof(int64_t) * (size_t)(3 * n_touched + 1)));
+  TT_CUDA(ctx->vslot1.ensure(sizeof(int) * (size_t)(nV + 1)));
   TT_CUDA(cudaMemsetAsync(ctx->rowlen.p, 0, sizeof(int) * (size_t)(nV + 1), st));
   TT_CUDA(cudaMemsetAsync(ctx->tlen.p, 0, sizeof(int64_t) * (size_t)(3 * n_touched + 1), st));
   TT_CUDA(cudaMemsetAsync(ctx->slot_excl.p, 0, (size_t)(3 * n_touched + 1), st));
@@ -376,7 +377,7 @@ tt_status symbolic_impl(tt_ctx* ctx, const tt_problem* q, int64_t* nnzb_host, in
         q->tris, ctx->touched.as<int>(), ctx->rdesc.as<int4>(), n_chunks, ctx->tfirst.as<int>(), ctx->keys_sorted,
         ctx->dvals_sorted, bitsT, ctx->vcnt.as<int>(), (ctx->opt.flags & TT_FLAG_FORCE_GENERAL_ROWS) ? 1 : 0,
         ctx->erank.as<int>(), ctx->drank.as<int>(), ctx->rowlen.as<int>(), ctx->tlen.as<int64_t>(),
-        ctx->slot_excl.as<uint8_t>(), ctx->everts.as<int>());
+        ctx->slot_excl.as<uint8_t>(), ctx->everts.as<int>(), ctx->vslot1.as<int>());
     TT_LAUNCH_CHECK();
   }
   if (n_long > 0) {  // triangles with more than RND_MAX_ENT partners: one warp per triangle
@@ -386,7 +387,7 @@ tt_status symbolic_impl(tt_ctx* ctx, const tt_problem* q, int64_t* nnzb_host, in
         q->tris, ctx->touched.as<int>(), n_long, ctx->tptr.as<int>(), ctx->keys_sorted, bitsT,
         ctx->vcnt.as<int>(), (ctx->opt.flags & TT_FLAG_FORCE_GENERAL_ROWS) ? 1 : 0, ctx->erank.as<int>(),
         ctx->drank.as<int>(), ctx->rowlen.as<int>(), ctx->tlen.as<int64_t>(), ctx->slot_excl.as<uint8_t>(),
-        ctx->long_list.as<int>(), ctx->rdesc.as<int4>());
+        ctx->long_list.as<int>(), ctx->rdesc.as<int4>(), ctx->vslot1.as<int>());
     TT_LAUNCH_CHECK();
   }
   s = scan_i64(ctx, ctx->tlen.as<int64_t>(), ctx->toff.as<int64_t>(), 3 * n_touched + 1, st);
@@ -472,23 +473,26 @@ tt_status symbolic_impl(tt_ctx* ctx, const tt_problem* q, int64_t* nnzb_host, in
   TT_CUDA(ctx->asm_energy.ensure(sizeof(double) * (size_t)(n_chunks + 1)));
   TT_CUDA(ctx->tvals.ensure(sizeof(T) * 9 * (size_t)(R + 1)));
   TT_CUDA(ctx->tslot.ensure(sizeof(T) * 9 * (size_t)(n_touched + 1)));
-  const int64_t nvs = 3 * n_touched;
-  for (int i = 0; i < 2; ++i) {
-    TT_CUDA(ctx->vkeys[i].ensure(sizeof(uint64_t) * (size_t)(nvs + 1)));
-    TT_CUDA(ctx->vvals[i].ensure(sizeof(uint32_t) * (size_t)(nvs + 1)));
-  }
-  TT_CUDA(ctx->vptr.ensure(sizeof(int) * (size_t)(nV + 2)));
-  uint64_t* vkeys_sorted = ctx->vkeys[0].as<uint64_t>();
-  ctx->vvals_sorted = ctx->vvals[0].as<uint32_t>();
-  if (nvs > 0) {
+  // vertex -> slot incidence: only when some vertex has more than one slot.  R == 0 means every slot
+  // is exclusive, hence every touched vertex has exactly one (k_gather3 then reads vslot1 only).
+  ctx->vvals_sorted = nullptr;
+  if (R > 0) {
+    const int64_t nvs = 3 * n_touched;
+    for (int i = 0; i < 2; ++i) {
+      TT_CUDA(ctx->vkeys[i].ensure(sizeof(uint64_t) * (size_t)(nvs + 1)));
+      TT_CUDA(ctx->vvals[i].ensure(sizeof(uint32_t) * (size_t)(nvs + 1)));
+    }
+    TT_CUDA(ctx->vptr.ensure(sizeof(int) * (size_t)(nV + 2)));
+    uint64_t* vkeys_sorted = ctx->vkeys[0].as<uint64_t>();
+    ctx->vvals_sorted = ctx->vvals[0].as<uint32_t>();
     k_emit_vslots<<<grid_for(nvs, 256), 256, 0, st>>>(q->tris, ctx->touched.as<int>(), n_touched,
                                                       ctx->vkeys[0].as<uint64_t>(), ctx->vvals[0].as<uint32_t>());
     TT_LAUNCH_CHECK();
     s = sort_pairs(ctx, ctx->vkeys, ctx->vvals, nvs, 0, bitsV, &vkeys_sorted, &ctx->vvals_sorted, st);
     if (s != TT_OK) return s;
+    k_segment_ptr<<<grid_for(nvs + 1, 256), 256, 0, st>>>(vkeys_sorted, nvs, 0, nV, ctx->vptr.as<int>());
+    TT_LAUNCH_CHECK();
   }
-  k_segment_ptr<<<grid_for(nvs + 1, 256), 256, 0, st>>>(vkeys_sorted, nvs, 0, nV, ctx->vptr.as<int>());
-  TT_LAUNCH_CHECK();
   TT_CUDA(cudaStreamSynchronize(st));
 
   ctx->sig.pos = q->pos;
@@ -592,7 +596,7 @@ tt_status numeric_impl(tt_ctx* ctx, const tt_problem* q, void* energy_sum, void*
     }
   }
   if (grad && nV > 0) {
-    k_gather3<T><<<grid_for(3 * nV, 256), 256, 0, st>>>(ctx->vptr.as<int>(), ctx->vvals_sorted, nV, ctx->tslot.as<T>(), (T*)grad);
+    k_gather3<T><<<grid_for(3 * nV, 256), 256, 0, st>>>(ctx->vcnt.as<int>(), ctx->vslot1.as<int>(), ctx->vptr.as<int>(), ctx->vvals_sorted, nV, ctx->tslot.as<T>(), (T*)grad);
     TT_LAUNCH_CHECK();
   }
   k_sum_partials<T><<<1, 1024, 0, st>>>(ctx->asm_energy.as<double>(), ctx->n_chunks, 1.0, (T*)energy_sum);
@@ -614,7 +618,7 @@ tt_status hessvec_impl(tt_ctx* ctx, const tt_problem* q, const void* pvec, void*
     ctx->ev_used[2] = true;
   }
   if (q->n_verts > 0) {
-    k_gather3<T><<<grid_for(3 * q->n_verts, 256), 256, 0, st>>>(ctx->vptr.as<int>(), ctx->vvals_sorted, q->n_verts,
+    k_gather3<T><<<grid_for(3 * q->n_verts, 256), 256, 0, st>>>(ctx->vcnt.as<int>(), ctx->vslot1.as<int>(), ctx->vptr.as<int>(), ctx->vvals_sorted, q->n_verts,
                                                                 ctx->tslot.as<T>(), (T*)y);
     TT_LAUNCH_CHECK();
   }
