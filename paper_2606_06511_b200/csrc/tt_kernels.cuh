@@ -687,13 +687,20 @@ k_round_symbolic(const int* __restrict__ tris, const int* __restrict__ touched, 
 }
 
 // Column indices of the exclusive rows + row bases of every non-long round (after the rowptr scan).
+// The three rows of a triangle have the SAME column run: it is built once in shared memory (ranks
+// are positions in the run) and written out three times with consecutive lanes on consecutive
+// addresses, instead of nine scattered 4-byte stores per entry.
 __global__ void __launch_bounds__(32 * RSYM_WARPS)
 k_round_fill(const int* __restrict__ tris, const int* __restrict__ touched, const int4* __restrict__ rdesc,
              int64_t n_chunks, const int* __restrict__ tfirst, const uint64_t* __restrict__ keys, int bitsT,
              const int* __restrict__ erank, const int* __restrict__ drank, const int64_t* __restrict__ toff,
              const uint8_t* __restrict__ slot_excl, const int* __restrict__ rowptr,
              int64_t* __restrict__ rowbase, int* __restrict__ colind) {
-  __shared__ int s_rp[RSYM_WARPS][3 * RND_MAX_TRI];  // first block of row m of triangle tt, or -1
+  constexpr int UNITS = RND_MAX_ENT + RND_MAX_TRI;       // a triangle's run has deg + 1 units of 3 columns
+  __shared__ int s_rp[RSYM_WARPS][3 * RND_MAX_TRI];       // first block of row m of triangle tt, or -1
+  __shared__ int s_ci[RSYM_WARPS][3 * UNITS];             // column runs of the round's triangles, back to back
+  __shared__ int s_first[RSYM_WARPS][RND_MAX_TRI];        // first entry of triangle tt
+  __shared__ unsigned char s_utt[RSYM_WARPS][UNITS];      // unit -> triangle
   constexpr unsigned FULL = 0xffffffffu;
   const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
   const int64_t c = (int64_t)blockIdx.x * RSYM_WARPS + warp;
@@ -702,49 +709,58 @@ k_round_fill(const int* __restrict__ tris, const int* __restrict__ touched, cons
   const int e_lo = d.x, nent = d.y, t_lo = d.z, ntri = d.w;
   if (nent > RND_MAX_ENT) return;  // long triangle: k_fill_rows
   int* rps = s_rp[warp];
+  int* ci = s_ci[warp];
+  int* first = s_first[warp];
+  unsigned char* utt = s_utt[warp];
   const uint64_t tmask = (1ull << bitsT) - 1ull;
+  // entry lanes: partner columns and ranks (independent of the triangle lanes' loads)
+  int cv[3] = {0, 0, 0}, er[3] = {0, 0, 0};
+  if (lane < nent) {
+    const int64_t e = (int64_t)e_lo + lane;
+    const int t = (int)(__ldg(keys + e) & tmask);
+#pragma unroll
+    for (int n = 0; n < 3; ++n) {
+      cv[n] = __ldg(tris + 3 * (int64_t)t + n);
+      er[n] = __ldg(erank + 3 * e + n);
+    }
+  }
   int f = 0;
   if (lane < ntri) {
     const int64_t ti = (int64_t)t_lo + lane;
     const int s = __ldg(touched + ti);
     f = __ldg(tfirst + ti) - e_lo;
-    int ov[3], dr[3];
+    const int l = __ldg(tfirst + ti + 1) - e_lo;
+    first[lane] = f;
+    utt[l + lane] = (unsigned char)lane;  // the diagonal's unit closes the run
 #pragma unroll
-    for (int n = 0; n < 3; ++n) {
-      ov[n] = __ldg(tris + 3 * (int64_t)s + n);
-      dr[n] = __ldg(drank + 3 * ti + n);
-    }
+    for (int n = 0; n < 3; ++n) ci[3 * (f + lane) + __ldg(drank + 3 * ti + n)] = __ldg(tris + 3 * (int64_t)s + n);
 #pragma unroll
     for (int m = 0; m < 3; ++m) {
       const bool excl = slot_excl[3 * ti + m] != 0;
-      const int rp = excl ? __ldg(rowptr + ov[m]) : -1;
+      const int rp = excl ? __ldg(rowptr + __ldg(tris + 3 * (int64_t)s + m)) : -1;
       rps[3 * lane + m] = rp;
       rowbase[3 * ti + m] = excl ? (int64_t)rp : -(toff[3 * ti + m] + 1);
-      if (excl) {
-#pragma unroll
-        for (int n = 0; n < 3; ++n) colind[rp + dr[n]] = ov[n];
-      }
     }
   }
   const unsigned heads = __reduce_or_sync(FULL, (lane < ntri) ? (1u << f) : 0u);
   const int my_ti = __popc(heads & (0xffffffffu >> (31 - lane))) - 1;
   __syncwarp();
   if (lane < nent) {
-    const int64_t e = (int64_t)e_lo + lane;
-    const int t = (int)(__ldg(keys + e) & tmask);
-    int cv[3], er[3];
+    utt[lane + my_ti] = (unsigned char)my_ti;
+    const int base = 3 * (first[my_ti] + my_ti);
 #pragma unroll
-    for (int n = 0; n < 3; ++n) {
-      cv[n] = __ldg(tris + 3 * (int64_t)t + n);
-      er[n] = __ldg(erank + 3 * e + n);
-    }
+    for (int n = 0; n < 3; ++n) ci[base + er[n]] = cv[n];
+  }
+  __syncwarp();
+  const int total = 3 * (nent + ntri);
+  for (int idx = lane; idx < total; idx += 32) {
+    const int tt = utt[idx / 3];
+    const int off = idx - 3 * (first[tt] + tt);
+    const int v = ci[idx];
 #pragma unroll
     for (int m = 0; m < 3; ++m) {
-      const int rp = rps[3 * my_ti + m];
-      if (rp >= 0) {
-#pragma unroll
-        for (int n = 0; n < 3; ++n) colind[rp + er[n]] = cv[n];
-      }
+      const int rp = rps[3 * tt + m];
+      if (rp >= 0) colind[rp + off] = v;
     }
   }
 }
