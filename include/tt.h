@@ -31,8 +31,10 @@
  *     pattern is the union over active pairs of their 6x6 vertex pairs (both triangles, full --
  *     not only the upper triangle).
  *   - All work is enqueued on `stream` (a cudaStream_t passed as void*, NULL = default stream).
- *     tt_energy, tt_energy_grad_hess and tt_hess_vec are asynchronous; tt_hess_symbolic and the
- *     *_host call synchronise the stream before returning (they hand sizes/results to the host).
+ *     tt_energy, tt_energy_grad_hess and tt_hess_vec are asynchronous; tt_hess_symbolic blocks
+ *     until the sizes it hands to the host are known (three host round trips on `stream`; its last
+ *     kernels may still be running on return, later calls on the same stream are ordered after
+ *     them); the *_host call synchronises the stream before returning.
  *   - Outputs are OVERWRITTEN, never accumulated into: grad / y / vals are fully defined on
  *     return (zeros where nothing contributes).
  *   - Errors: every call returns a tt_status (negative = failure) and leaves a message readable
@@ -103,7 +105,7 @@ tt_status tt_energy(tt_ctx* ctx, const tt_problem* prob, void* energy_sum, void*
  * the active pairs (order preserving) and builds the BSR pattern.  Caches all of it in ctx.
  *   nnzb_host     HOST [1]: number of 3x3 blocks the numeric phase will write
  *   n_active_host HOST [1] or NULL
- * Synchronises `stream`.                                                                          */
+ * Blocks until nnzb is known; the tail of the phase completes asynchronously on `stream`.         */
 tt_status tt_hess_symbolic(tt_ctx* ctx, const tt_problem* prob, int64_t* nnzb_host,
                            int64_t* n_active_host, void* stream);
 

@@ -385,9 +385,10 @@ constexpr int RND_MAX_TRI = TT_RND_MAX_TRI;
 constexpr int CHK_BUCKET = 128;
 
 // tfirst[i] = first directed entry of touched triangle i; tfirst[n_touched] = n_dir
-__global__ void k_touched_first(const int* __restrict__ touched, int64_t n_touched, const int* __restrict__ tptr,
-                                int64_t n_dir, int* __restrict__ tfirst) {
+__global__ void k_touched_first(const int* __restrict__ touched, const int* __restrict__ n_touched_dev,
+                                const int* __restrict__ tptr, int64_t n_dir, int* __restrict__ tfirst) {
   const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  const int64_t n_touched = *n_touched_dev;  // still on the device: the grid covers its bound
   if (i < n_touched) tfirst[i] = tptr[touched[i]];
   if (i == n_touched) tfirst[i] = (int)n_dir;
 }
@@ -396,12 +397,14 @@ __global__ void k_touched_first(const int* __restrict__ touched, int64_t n_touch
 // FILL = true : chunk_start[bucket_off[b] + k] = first touched index of the k-th round of bucket b,
 //               long_list[long_off[b] + k] = round id of the k-th long triangle.
 template <bool FILL>
-__global__ void k_chunk_pack(const int* __restrict__ tfirst, int64_t n_touched, int64_t n_buckets,
+__global__ void k_chunk_pack(const int* __restrict__ tfirst, const int* __restrict__ n_touched_dev,
                              int* __restrict__ bucket_cnt, int* __restrict__ long_cnt,
                              const int* __restrict__ bucket_off, const int* __restrict__ long_off,
                              int* __restrict__ chunk_start, int* __restrict__ long_list) {
   const int64_t b = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
-  if (b >= n_buckets) return;
+  const int64_t n_touched = *n_touched_dev;  // still on the device: the grid covers its bound
+  const int64_t n_buckets = (n_touched + CHK_BUCKET - 1) / CHK_BUCKET;
+  if (b >= n_buckets) return;             // the counts of the buckets beyond stay zero
   const int64_t i0 = b * CHK_BUCKET, i1 = min(i0 + (int64_t)CHK_BUCKET, n_touched);
   int nch = 0, nlong = 0, ent = 0, tri = 0;
   const int cbase = FILL ? bucket_off[b] : 0, lbase = FILL ? long_off[b] : 0;
@@ -1731,20 +1734,24 @@ template <typename T>
 __global__ void k_gather3(const int* __restrict__ vcnt, const int* __restrict__ vslot1, const int* __restrict__ vptr,
                           const uint32_t* __restrict__ vslots, int64_t nV, const T* __restrict__ tslot,
                           T* __restrict__ out) {
-  const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
-  if (i >= 3 * nV) return;
-  const int64_t v = i / 3;
-  const int comp = (int)(i - 3 * v);
+  const int64_t v = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;  // one thread per vertex: 3 consecutive values
+  if (v >= nV) return;
   const int n = __ldg(vcnt + v);
-  T r = (T)0;
+  T r0 = (T)0, r1 = (T)0, r2 = (T)0;
   if (n == 1) {
-    r = tslot[3 * (int64_t)__ldg(vslot1 + v) + comp];
+    const T* t = tslot + 3 * (int64_t)__ldg(vslot1 + v);
+    r0 = t[0]; r1 = t[1]; r2 = t[2];
   } else if (n > 1) {
-    double acc = 0.0;
-    for (int j = vptr[v]; j < vptr[v + 1]; ++j) acc += (double)tslot[3 * (int64_t)vslots[j] + comp];
-    r = (T)acc;
+    double a0 = 0.0, a1 = 0.0, a2 = 0.0;
+    for (int j = vptr[v]; j < vptr[v + 1]; ++j) {
+      const T* t = tslot + 3 * (int64_t)vslots[j];
+      a0 += (double)t[0]; a1 += (double)t[1]; a2 += (double)t[2];
+    }
+    r0 = (T)a0; r1 = (T)a1; r2 = (T)a2;
   }
-  out[i] = r;
+  out[3 * v] = r0;
+  out[3 * v + 1] = r1;
+  out[3 * v + 2] = r2;
 }
 
 __global__ void k_iota(uint32_t* __restrict__ v, int64_t n) {

@@ -290,13 +290,20 @@ tt_status symbolic_impl(tt_ctx* ctx, const tt_problem* q, int64_t* nnzb_host, in
   k_segment_ptr<<<grid_for(n + 1, 256), 256, 0, st>>>(ctx->keys_sorted, n, bitsT, nT, ctx->tptr.as<int>());
   TT_LAUNCH_CHECK();
 
-  // ---- touched triangles and vertex use counts ----
+  // ---- touched triangles, vertex use counts and the work partition (rounds) shared by the symbolic
+  //      round kernels, K4 and K6.  The number of touched triangles stays on the device until the
+  //      rounds are packed (grids and buffers use the bound min(nT, 2A)): one host round trip for
+  //      n_touched, n_chunks and n_long instead of two. ----
   TT_CUDA(ctx->vcnt.ensure(sizeof(int) * (size_t)(nV + 1)));
   TT_CUDA(ctx->tflag.ensure(sizeof(int) * (size_t)(nT + 1)));
   TT_CUDA(ctx->touched.ensure(sizeof(int) * (size_t)(nT + 1)));
   TT_CUDA(cudaMemsetAsync(ctx->vcnt.p, 0, sizeof(int) * (size_t)(nV + 1), st));
-  int64_t n_touched = 0;
-  if (nT > 0) {
+  int64_t n_touched = 0, n_chunks = 0, n_long = 0;
+  const int64_t touched_ub = nT < n ? nT : n;
+  TT_CUDA(ctx->tfirst.ensure(sizeof(int) * (size_t)(touched_ub + 2)));
+  TT_CUDA(ctx->chunk_start.ensure(sizeof(int) * (size_t)(touched_ub + 2)));
+  TT_CUDA(ctx->long_list.ensure(sizeof(int) * (size_t)(n / (RND_MAX_ENT + 1) + 2)));
+  if (touched_ub > 0) {
     k_vertex_touch<<<grid_for(nT, 256), 256, 0, st>>>(q->tris, ctx->tptr.as<int>(), nT, ctx->vcnt.as<int>(),
                                                       ctx->tflag.as<int>());
     TT_LAUNCH_CHECK();
@@ -307,49 +314,37 @@ tt_status symbolic_impl(tt_ctx* ctx, const tt_problem* q, int64_t* nnzb_host, in
     TT_CUDA(ctx->cub_tmp.ensure(tmp));
     TT_CUDA(cub::DeviceSelect::Flagged(ctx->cub_tmp.p, tmp, iota, ctx->tflag.as<int>(), ctx->touched.as<int>(), d_num, (int)nT, st));
     ctx->launches++;
-    int nt32 = 0;
-    TT_CUDA(cudaMemcpyAsync(&nt32, d_num, sizeof(int), cudaMemcpyDeviceToHost, st));
+    const int64_t buckets_ub = (touched_ub + CHK_BUCKET - 1) / CHK_BUCKET;
+    TT_CUDA(ctx->bucket_cnt.ensure(sizeof(int) * (size_t)(buckets_ub + 1)));
+    TT_CUDA(ctx->bucket_off.ensure(sizeof(int) * (size_t)(buckets_ub + 1)));
+    TT_CUDA(ctx->long_cnt.ensure(sizeof(int) * (size_t)(buckets_ub + 1)));
+    TT_CUDA(ctx->long_off.ensure(sizeof(int) * (size_t)(buckets_ub + 1)));
+    k_touched_first<<<grid_for(touched_ub + 1, 256), 256, 0, st>>>(ctx->touched.as<int>(), d_num, ctx->tptr.as<int>(), n,
+                                                                   ctx->tfirst.as<int>());
+    TT_LAUNCH_CHECK();
+    TT_CUDA(cudaMemsetAsync(ctx->bucket_cnt.p, 0, sizeof(int) * (size_t)(buckets_ub + 1), st));
+    TT_CUDA(cudaMemsetAsync(ctx->long_cnt.p, 0, sizeof(int) * (size_t)(buckets_ub + 1), st));
+    k_chunk_pack<false><<<grid_for(buckets_ub, 128), 128, 0, st>>>(ctx->tfirst.as<int>(), d_num, ctx->bucket_cnt.as<int>(),
+                                                                  ctx->long_cnt.as<int>(), nullptr, nullptr, nullptr, nullptr);
+    TT_LAUNCH_CHECK();
+    s = scan_i32(ctx, ctx->bucket_cnt.as<int>(), ctx->bucket_off.as<int>(), buckets_ub + 1, st);
+    if (s != TT_OK) return s;
+    s = scan_i32(ctx, ctx->long_cnt.as<int>(), ctx->long_off.as<int>(), buckets_ub + 1, st);
+    if (s != TT_OK) return s;
+    k_chunk_pack<true><<<grid_for(buckets_ub, 128), 128, 0, st>>>(ctx->tfirst.as<int>(), d_num, nullptr, nullptr,
+                                                                 ctx->bucket_off.as<int>(), ctx->long_off.as<int>(),
+                                                                 ctx->chunk_start.as<int>(), ctx->long_list.as<int>());
+    TT_LAUNCH_CHECK();
+    int cnt32[3] = {0, 0, 0};
+    TT_CUDA(cudaMemcpyAsync(&cnt32[0], d_num, sizeof(int), cudaMemcpyDeviceToHost, st));
+    TT_CUDA(cudaMemcpyAsync(&cnt32[1], ctx->bucket_off.as<int>() + buckets_ub, sizeof(int), cudaMemcpyDeviceToHost, st));
+    TT_CUDA(cudaMemcpyAsync(&cnt32[2], ctx->long_off.as<int>() + buckets_ub, sizeof(int), cudaMemcpyDeviceToHost, st));
     TT_CUDA(cudaStreamSynchronize(st));
-    n_touched = nt32;
+    n_touched = cnt32[0];
+    n_chunks = cnt32[1];
+    n_long = cnt32[2];
   }
   ctx->n_touched = n_touched;
-
-  // ---- work partition shared by the symbolic round kernels, K4 and K6 ----
-  // rounds: greedy packing of whole touched triangles (<= 32 entries, <= 16 triangles per round)
-  int64_t n_chunks = 0, n_long = 0;
-  TT_CUDA(ctx->tfirst.ensure(sizeof(int) * (size_t)(n_touched + 2)));
-  TT_CUDA(ctx->chunk_start.ensure(sizeof(int) * (size_t)(n_touched + 2)));
-  TT_CUDA(ctx->long_list.ensure(sizeof(int) * (size_t)(n / (RND_MAX_ENT + 1) + 2)));
-  if (n_touched > 0) {
-    const int64_t n_buckets = (n_touched + CHK_BUCKET - 1) / CHK_BUCKET;
-    TT_CUDA(ctx->bucket_cnt.ensure(sizeof(int) * (size_t)(n_buckets + 1)));
-    TT_CUDA(ctx->bucket_off.ensure(sizeof(int) * (size_t)(n_buckets + 1)));
-    TT_CUDA(ctx->long_cnt.ensure(sizeof(int) * (size_t)(n_buckets + 1)));
-    TT_CUDA(ctx->long_off.ensure(sizeof(int) * (size_t)(n_buckets + 1)));
-    k_touched_first<<<grid_for(n_touched + 1, 256), 256, 0, st>>>(ctx->touched.as<int>(), n_touched, ctx->tptr.as<int>(), n,
-                                                                  ctx->tfirst.as<int>());
-    TT_LAUNCH_CHECK();
-    TT_CUDA(cudaMemsetAsync(ctx->bucket_cnt.as<int>() + n_buckets, 0, sizeof(int), st));
-    TT_CUDA(cudaMemsetAsync(ctx->long_cnt.as<int>() + n_buckets, 0, sizeof(int), st));
-    k_chunk_pack<false><<<grid_for(n_buckets, 128), 128, 0, st>>>(ctx->tfirst.as<int>(), n_touched, n_buckets,
-                                                                 ctx->bucket_cnt.as<int>(), ctx->long_cnt.as<int>(), nullptr,
-                                                                 nullptr, nullptr, nullptr);
-    TT_LAUNCH_CHECK();
-    s = scan_i32(ctx, ctx->bucket_cnt.as<int>(), ctx->bucket_off.as<int>(), n_buckets + 1, st);
-    if (s != TT_OK) return s;
-    s = scan_i32(ctx, ctx->long_cnt.as<int>(), ctx->long_off.as<int>(), n_buckets + 1, st);
-    if (s != TT_OK) return s;
-    k_chunk_pack<true><<<grid_for(n_buckets, 128), 128, 0, st>>>(ctx->tfirst.as<int>(), n_touched, n_buckets, nullptr, nullptr,
-                                                                ctx->bucket_off.as<int>(), ctx->long_off.as<int>(),
-                                                                ctx->chunk_start.as<int>(), ctx->long_list.as<int>());
-    TT_LAUNCH_CHECK();
-    int nc32[2] = {0, 0};
-    TT_CUDA(cudaMemcpyAsync(&nc32[0], ctx->bucket_off.as<int>() + n_buckets, sizeof(int), cudaMemcpyDeviceToHost, st));
-    TT_CUDA(cudaMemcpyAsync(&nc32[1], ctx->long_off.as<int>() + n_buckets, sizeof(int), cudaMemcpyDeviceToHost, st));
-    TT_CUDA(cudaStreamSynchronize(st));
-    n_chunks = nc32[0];
-    n_long = nc32[1];
-  }
   ctx->n_chunks = n_chunks;
   ctx->n_long = n_long;
   TT_CUDA(ctx->rdesc.ensure(sizeof(int4) * (size_t)(n_chunks + 1)));
@@ -392,8 +387,15 @@ tt_status symbolic_impl(tt_ctx* ctx, const tt_problem* q, int64_t* nnzb_host, in
   }
   s = scan_i64(ctx, ctx->tlen.as<int64_t>(), ctx->toff.as<int64_t>(), 3 * n_touched + 1, st);
   if (s != TT_OK) return s;
-  int64_t R = 0;
+  // The row-pointer scan is issued speculatively: if there are no general rows (R == 0: always, in a
+  // soup) the exclusive row lengths are already final and nnzb arrives in the same host round trip.
+  TT_CUDA(ctx->rowptr64.ensure(sizeof(int64_t) * (size_t)(nV + 1)));
+  TT_CUDA(ctx->rowptr.ensure(sizeof(int) * (size_t)(nV + 1)));
+  s = scan_i32_to_i64(ctx, ctx->rowlen.as<int>(), ctx->rowptr64.as<int64_t>(), nV + 1, st);
+  if (s != TT_OK) return s;
+  int64_t R = 0, nnzb = 0;
   TT_CUDA(cudaMemcpyAsync(&R, ctx->toff.as<int64_t>() + 3 * n_touched, sizeof(int64_t), cudaMemcpyDeviceToHost, st));
+  TT_CUDA(cudaMemcpyAsync(&nnzb, ctx->rowptr64.as<int64_t>() + nV, sizeof(int64_t), cudaMemcpyDeviceToHost, st));
   TT_CUDA(cudaStreamSynchronize(st));
   if (R >= (int64_t(1) << 31)) return fail(ctx, TT_ERR_INVALID_ARG, "general-row workspace exceeds 2^31 blocks");
   ctx->R = R;
@@ -434,14 +436,13 @@ tt_status symbolic_impl(tt_ctx* ctx, const tt_problem* q, int64_t* nnzb_host, in
   }
   ctx->U = U;
 
-  // ---- row pointers ----
-  TT_CUDA(ctx->rowptr64.ensure(sizeof(int64_t) * (size_t)(nV + 1)));
-  TT_CUDA(ctx->rowptr.ensure(sizeof(int) * (size_t)(nV + 1)));
-  s = scan_i32_to_i64(ctx, ctx->rowlen.as<int>(), ctx->rowptr64.as<int64_t>(), nV + 1, st);
-  if (s != TT_OK) return s;
-  int64_t nnzb = 0;
-  TT_CUDA(cudaMemcpyAsync(&nnzb, ctx->rowptr64.as<int64_t>() + nV, sizeof(int64_t), cudaMemcpyDeviceToHost, st));
-  TT_CUDA(cudaStreamSynchronize(st));
+  // ---- row pointers (again, if general rows added to the row lengths) ----
+  if (R > 0) {
+    s = scan_i32_to_i64(ctx, ctx->rowlen.as<int>(), ctx->rowptr64.as<int64_t>(), nV + 1, st);
+    if (s != TT_OK) return s;
+    TT_CUDA(cudaMemcpyAsync(&nnzb, ctx->rowptr64.as<int64_t>() + nV, sizeof(int64_t), cudaMemcpyDeviceToHost, st));
+    TT_CUDA(cudaStreamSynchronize(st));
+  }
   if (nnzb >= (int64_t(1) << 31)) return fail(ctx, TT_ERR_INVALID_ARG, "nnzb %lld exceeds int32 BSR indexing", (long long)nnzb);
   ctx->nnzb = nnzb;
   k_i64_to_i32<<<grid_for(nV + 1, 256), 256, 0, st>>>(ctx->rowptr64.as<int64_t>(), nV + 1, ctx->rowptr.as<int>());
@@ -493,7 +494,6 @@ tt_status symbolic_impl(tt_ctx* ctx, const tt_problem* q, int64_t* nnzb_host, in
     k_segment_ptr<<<grid_for(nvs + 1, 256), 256, 0, st>>>(vkeys_sorted, nvs, 0, nV, ctx->vptr.as<int>());
     TT_LAUNCH_CHECK();
   }
-  TT_CUDA(cudaStreamSynchronize(st));
 
   ctx->sig.pos = q->pos;
   ctx->sig.tris = q->tris;
@@ -596,7 +596,7 @@ tt_status numeric_impl(tt_ctx* ctx, const tt_problem* q, void* energy_sum, void*
     }
   }
   if (grad && nV > 0) {
-    k_gather3<T><<<grid_for(3 * nV, 256), 256, 0, st>>>(ctx->vcnt.as<int>(), ctx->vslot1.as<int>(), ctx->vptr.as<int>(), ctx->vvals_sorted, nV, ctx->tslot.as<T>(), (T*)grad);
+    k_gather3<T><<<grid_for(nV, 256), 256, 0, st>>>(ctx->vcnt.as<int>(), ctx->vslot1.as<int>(), ctx->vptr.as<int>(), ctx->vvals_sorted, nV, ctx->tslot.as<T>(), (T*)grad);
     TT_LAUNCH_CHECK();
   }
   k_sum_partials<T><<<1, 1024, 0, st>>>(ctx->asm_energy.as<double>(), ctx->n_chunks, 1.0, (T*)energy_sum);
@@ -618,7 +618,7 @@ tt_status hessvec_impl(tt_ctx* ctx, const tt_problem* q, const void* pvec, void*
     ctx->ev_used[2] = true;
   }
   if (q->n_verts > 0) {
-    k_gather3<T><<<grid_for(3 * q->n_verts, 256), 256, 0, st>>>(ctx->vcnt.as<int>(), ctx->vslot1.as<int>(), ctx->vptr.as<int>(), ctx->vvals_sorted, q->n_verts,
+    k_gather3<T><<<grid_for(q->n_verts, 256), 256, 0, st>>>(ctx->vcnt.as<int>(), ctx->vslot1.as<int>(), ctx->vptr.as<int>(), ctx->vvals_sorted, q->n_verts,
                                                                 ctx->tslot.as<T>(), (T*)y);
     TT_LAUNCH_CHECK();
   }
