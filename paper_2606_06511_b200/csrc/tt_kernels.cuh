@@ -1131,13 +1131,28 @@ k_assemble_tile(const AsmParams<T> P) {
             b[i] = E.cf.c01 * E.g0[3 * m + i] + E.cf.c11 * E.g1[3 * m + i];
           }
           T* run = reinterpret_cast<T*>(S.tile + S.run_off[my_ti]);
+          // The two outer products of a block run in the OUTPUT precision (fp32 variant: FFMA on the
+          // rounded J, 1e-7 relative per block against a 1e-3 tolerance; J, the coefficients and every
+          // sum over pairs stay fp64 -- reading A12).
+          T at[3], bt[3];
+#pragma unroll
+          for (int i = 0; i < 3; ++i) {
+            at[i] = (T)a[i];
+            bt[i] = (T)b[i];
+          }
 #pragma unroll
           for (int n = 0; n < 3; ++n) {
             T* blk = run + 9 * er[n];
+            T p0[3], p1[3];
+#pragma unroll
+            for (int j = 0; j < 3; ++j) {
+              p0[j] = (T)E.g0[9 + 3 * n + j];
+              p1[j] = (T)E.g1[9 + 3 * n + j];
+            }
 #pragma unroll
             for (int i = 0; i < 3; ++i)
 #pragma unroll
-              for (int j = 0; j < 3; ++j) blk[3 * i + j] = (T)(a[i] * E.g0[9 + 3 * n + j] + b[i] * E.g1[9 + 3 * n + j]);
+              for (int j = 0; j < 3; ++j) blk[3 * i + j] = at[i] * p0[j] + bt[i] * p1[j];
           }
         }
         // diagonal-row blocks (p_m, p_n): lane = element (n, i, j), from the packed upper triangle
