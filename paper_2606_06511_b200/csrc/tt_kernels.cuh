@@ -1181,10 +1181,17 @@ k_assemble_tile(const AsmParams<T> P) {
           int head = (int)((16ull - (g & 15ull)) & 15ull);
           head = min(head, run_bytes);
           const int body = (run_bytes - head) & ~15;
-          for (int o = 0; o < head; o += (int)sizeof(T)) *reinterpret_cast<T*>(g + o) = *reinterpret_cast<const T*>(src + o);
-          if (body > 0) bulk_s2g(reinterpret_cast<void*>(g + head), src + head, (uint32_t)body);
-          for (int o = head + body; o < run_bytes; o += (int)sizeof(T))
-            *reinterpret_cast<T*>(g + o) = *reinterpret_cast<const T*>(src + o);
+          if (sizeof(T) == 8) {  // blocks are 8-byte aligned: at most one value before and one after the body
+            if (head > 0) *reinterpret_cast<T*>(g) = *reinterpret_cast<const T*>(src);
+            if (body > 0) bulk_s2g(reinterpret_cast<void*>(g + head), src + head, (uint32_t)body);
+            if (head + body < run_bytes)
+              *reinterpret_cast<T*>(g + head + body) = *reinterpret_cast<const T*>(src + head + body);
+          } else {
+            for (int o = 0; o < head; o += (int)sizeof(T)) *reinterpret_cast<T*>(g + o) = *reinterpret_cast<const T*>(src + o);
+            if (body > 0) bulk_s2g(reinterpret_cast<void*>(g + head), src + head, (uint32_t)body);
+            for (int o = head + body; o < run_bytes; o += (int)sizeof(T))
+              *reinterpret_cast<T*>(g + o) = *reinterpret_cast<const T*>(src + o);
+          }
           bulk_commit();
         }
       }
