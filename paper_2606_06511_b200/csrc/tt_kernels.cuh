@@ -1581,26 +1581,32 @@ k_entry_reduce(const AsmParams<T> P, const int* __restrict__ round_list, int64_t
 constexpr int PIPE_WARPS = TT_PIPE_WARPS;
 template <typename T, int MODE>
 struct PipeWarpSmem {
-  T x[2][18 * 32];
-  T p[MODE == 2 ? 18 * 32 : 1];
+  T xp[2][9 * 32];                          // partner triangle's positions, lane-private slots [k * 32 + lane]
+  T xo[2][9 * RND_MAX_TRI];                 // own triangle's positions, ONE copy per triangle (head lane's order)
+  T pp[MODE == 2 ? 9 * 32 : 1];             // p of the partner's vertices
+  T po[MODE == 2 ? 9 * RND_MAX_TRI : 1];    // p of the own vertices, one copy per triangle
 };
 
 struct PipeOps {
-  int ids[6];
+  int ids[6];      // lane = entry: canonical pair, recorded order
   unsigned pay;
+  int f;           // lane = triangle: first entry of the triangle, relative to the round
 };
 template <typename T>
 __device__ __forceinline__ void load_pipe_ops(const AsmParams<T>& P, const int4 d, int lane, PipeOps& R) {
 #pragma unroll
   for (int i = 0; i < 6; ++i) R.ids[i] = 0;
   R.pay = 0u;
-  if (d.y <= RND_MAX_ENT && lane < d.y) {
+  R.f = 0;
+  if (d.y > RND_MAX_ENT) return;  // long round: k_entry_reduce's
+  if (lane < d.y) {
     const int64_t e = (int64_t)d.x + lane;
     const int2* v = reinterpret_cast<const int2*>(P.everts + 6 * e);
     const int2 v0 = __ldg(v), v1 = __ldg(v + 1), v2 = __ldg(v + 2);
     R.ids[0] = v0.x; R.ids[1] = v0.y; R.ids[2] = v1.x; R.ids[3] = v1.y; R.ids[4] = v2.x; R.ids[5] = v2.y;
     R.pay = (unsigned)__ldg(P.dvals + e);
   }
+  if (lane < d.w) R.f = __ldg(P.tfirst + d.z + lane) - d.x;
 }
 __device__ __forceinline__ void own_first_ids(const PipeOps& R, int (&pid)[6]) {
   const bool side = (R.pay & 1u) != 0u;
@@ -1609,6 +1615,64 @@ __device__ __forceinline__ void own_first_ids(const PipeOps& R, int (&pid)[6]) {
     pid[i] = side ? R.ids[3 + i] : R.ids[i];
     pid[3 + i] = side ? R.ids[i] : R.ids[3 + i];
   }
+}
+
+// Where a lane finds its triangle's shared (own-vertex) slots: triangle index inside the round and,
+// for each of its three own vertices in ITS recorded order, the position in the head lane's order.
+struct OwnMap {
+  int ti;
+  int rp[3];
+};
+
+// The gathers of one round.  Every entry needs its partner's three vertices (lane-private slots),
+// but the entries of one triangle all need the SAME three own vertices: only the triangle's first
+// lane (head) requests them, once, and the others read the head's copy.  K6 is bound by the number
+// of gather requests the L1 accepts (measured: dropping the own-vertex requests of the non-head
+// lanes is worth 20 % of the kernel), not by bytes.
+template <typename T>
+__device__ __forceinline__ OwnMap issue_round_gather(const T* __restrict__ src, const PipeOps& o, const int4 d,
+                                                     int lane, T* part, T* own) {
+  constexpr unsigned FULL = 0xffffffffu;
+  const bool ok = d.y <= RND_MAX_ENT;
+  const bool valid = ok && lane < d.y;
+  const unsigned heads = __reduce_or_sync(FULL, (ok && lane < d.w) ? (1u << o.f) : 0u) | 1u;
+  const unsigned below = heads & (0xffffffffu >> (31 - lane));
+  const int head_lane = 31 - __clz((int)below);
+  int pid[6];
+  own_first_ids(o, pid);
+  OwnMap m;
+  m.ti = __popc(below) - 1;
+  const int h0 = __shfl_sync(FULL, pid[0], head_lane), h1 = __shfl_sync(FULL, pid[1], head_lane);
+#pragma unroll
+  for (int r = 0; r < 3; ++r) m.rp[r] = (pid[r] == h0) ? 0 : ((pid[r] == h1) ? 1 : 2);
+  if (valid) {
+#pragma unroll
+    for (int v = 0; v < 3; ++v) {
+      const T* g = src + 3 * (int64_t)pid[3 + v];
+#pragma unroll
+      for (int k = 0; k < 3; ++k) cp_async_elem(part + (3 * v + k) * 32 + lane, g + k);
+    }
+    if (lane == head_lane && m.ti < RND_MAX_TRI) {
+#pragma unroll
+      for (int v = 0; v < 3; ++v) {
+        const T* g = src + 3 * (int64_t)pid[v];
+#pragma unroll
+        for (int k = 0; k < 3; ++k) cp_async_elem(own + 9 * m.ti + 3 * v + k, g + k);
+      }
+    }
+  }
+  return m;
+}
+// own-first values [own r = 0..2 | partner] of a lane, from the round's two areas
+template <typename T>
+__device__ __forceinline__ void read_round_gather(const T* part, const T* own, const OwnMap& m, int lane,
+                                                  double (&v)[18]) {
+#pragma unroll
+  for (int r = 0; r < 3; ++r)
+#pragma unroll
+    for (int k = 0; k < 3; ++k) v[3 * r + k] = (double)own[9 * m.ti + 3 * m.rp[r] + k];
+#pragma unroll
+  for (int i = 0; i < 9; ++i) v[9 + i] = (double)part[i * 32 + lane];
 }
 
 template <typename T, int MODE>
@@ -1629,14 +1693,10 @@ k_entry_pipe(const AsmParams<T> P) {
   PipeOps cur, nxt;
   load_pipe_ops(P, d_cur, lane, cur);
   load_pipe_ops(P, d_nxt, lane, nxt);
-  if (d_cur.y <= RND_MAX_ENT && lane < d_cur.y) gather18_async(S.x[0], lane, P.pos, cur.ids);
+  OwnMap m_cur = issue_round_gather(P.pos, cur, d_cur, lane, S.xp[0], S.xo[0]);
   cp_async_commit();
   if (MODE == 2) {
-    if (d_cur.y <= RND_MAX_ENT && lane < d_cur.y) {
-      int pid[6];
-      own_first_ids(cur, pid);
-      gather18_async(S.p, lane, P.pvec, pid);
-    }
+    issue_round_gather(P.pvec, cur, d_cur, lane, S.pp, S.po);
     cp_async_commit();
   }
   int buf = 0;
@@ -1646,35 +1706,47 @@ k_entry_pipe(const AsmParams<T> P) {
     PipeOps nn;
     load_pipe_ops(P, d_nn, lane, nn);
     const int4 d_nnn = (c + 3 * G < P.n_chunks) ? __ldg(P.rdesc + c + 3 * G) : dzero;
-    const bool nxt_ok = d_nxt.y <= RND_MAX_ENT && lane < d_nxt.y;
-    if (nxt_ok) gather18_async(S.x[buf ^ 1], lane, P.pos, nxt.ids);
+    const OwnMap m_nxt = issue_round_gather(P.pos, nxt, d_nxt, lane, S.xp[buf ^ 1], S.xo[buf ^ 1]);
     cp_async_commit();
-    const int e_lo = d_cur.x, nent = d_cur.y;
+    const int nent = d_cur.y;
     const bool is_long = nent > RND_MAX_ENT;  // k_entry_reduce's (launched over long_list)
     const bool valid = !is_long && lane < nent;
     const bool tri_lane = !is_long && lane < d_cur.w;
-    const int f = tri_lane ? __ldg(P.tfirst + d_cur.z + lane) - e_lo : 0;  // consumed after the derivative code
     if (MODE == 2) cp_async_wait<2>(); else cp_async_wait<1>();  // positions of THIS round have landed
+    __syncwarp();                                                 // ... including the head lanes' copies
     double v[9];
 #pragma unroll
     for (int k = 0; k < 9; ++k) v[k] = 0.0;
     double e_acc = 0.0;
+    Entry E;
     if (valid) {
-      double x[18];
+      double xf[18], x[18];
+      read_round_gather(S.xp[buf], S.xo[buf], m_cur, lane, xf);
+      const bool side = (cur.pay & 1u) != 0u;  // eval_core wants the canonical order (T_a first)
 #pragma unroll
-      for (int k = 0; k < 18; ++k) x[k] = (double)S.x[buf][k * 32 + lane];
-      Entry E;
+      for (int k = 0; k < 9; ++k) {
+        x[k] = side ? xf[9 + k] : xf[k];
+        x[9 + k] = side ? xf[k] : xf[9 + k];
+      }
       eval_core(x, cur.pay, P.sigma, P.hess_mode, E);
       e_acc = E.en;
-      double u0 = E.cf.cg0, u1 = E.cf.cg1;  // MODE 1: Eq. 3
+    }
+    double u0 = 0.0, u1 = 0.0;
+    if (MODE == 2) {
+      cp_async_wait<1>();  // p of THIS round
+      __syncwarp();
+    }
+    if (valid) {
+      u0 = E.cf.cg0;  // MODE 1: Eq. 3
+      u1 = E.cf.cg1;
       if (MODE == 2) {
-        cp_async_wait<1>();                 // p of THIS round
+        double pv[18];
+        read_round_gather(S.pp, S.po, m_cur, lane, pv);
         double j0 = 0.0, j1 = 0.0;
 #pragma unroll
         for (int i = 0; i < 18; ++i) {
-          const double pv = (double)S.p[i * 32 + lane];
-          j0 = fma(E.g0[i], pv, j0);
-          j1 = fma(E.g1[i], pv, j1);
+          j0 = fma(E.g0[i], pv[i], j0);
+          j1 = fma(E.g1[i], pv[i], j1);
         }
         u0 = E.cf.c00 * j0 + E.cf.c01 * j1;  // M (J p_loc)
         u1 = E.cf.c01 * j0 + E.cf.c11 * j1;
@@ -1689,16 +1761,12 @@ k_entry_pipe(const AsmParams<T> P) {
           v[3 * i + cc] = (E.po[0] == i) ? yr[cc] : ((E.po[1] == i) ? yr[3 + cc] : yr[6 + cc]);
     }
     if (MODE == 2) {
-      cp_async_wait<1>();  // lanes that skipped the block above: same group accounting
-      if (nxt_ok) {        // this lane's p slots are free again: p of the next round
-        int pid[6];
-        own_first_ids(nxt, pid);
-        gather18_async(S.p, lane, P.pvec, pid);
-      }
+      __syncwarp();  // every lane has read the shared p slots of this round: p of the next round
+      issue_round_gather(P.pvec, nxt, d_nxt, lane, S.pp, S.po);
       cp_async_commit();
     }
     if (!is_long) {
-      const unsigned heads = __reduce_or_sync(FULL, tri_lane ? (1u << f) : 0u) | 1u;  // bit i: entry i opens a triangle
+      const unsigned heads = __reduce_or_sync(FULL, tri_lane ? (1u << cur.f) : 0u) | 1u;  // bit i: entry i opens a triangle
       const unsigned below = heads & (0xffffffffu >> (31 - lane));
       const int segf = 31 - __clz((int)below);
 #pragma unroll
@@ -1729,6 +1797,7 @@ k_entry_pipe(const AsmParams<T> P) {
     d_nn = d_nnn;
     cur = nxt;
     nxt = nn;
+    m_cur = m_nxt;
     buf ^= 1;
   }
   cp_async_wait<0>();
