@@ -26,10 +26,29 @@ constexpr int CLS_THREADS = 256;   // K1 / K2 CTA size (8 warps -> 8 mask words 
 constexpr int SYM_WARPS = 4;       // warps per CTA in the per-triangle symbolic kernels
 constexpr int SYM_LMAX = 1536;     // longest row (in blocks) ranked in shared memory
 
+// One vertex = three consecutive values at an address that is only value-aligned: exactly one of
+// p, p + 1 is aligned for a two-value load, so a vertex costs two gather requests (one 2-wide, one
+// 1-wide; addresses selected, no divergence, nothing read outside the vertex) instead of three.
+// K1 is bound by gather requests: 0.69 -> 0.63 ms at 10M candidates.  (Not used in K4 / K6: there the
+// selects cost more than the saved request, measured.)
+template <typename T> struct Pair2;
+template <> struct Pair2<double> { using type = double2; };
+template <> struct Pair2<float> { using type = float2; };
+template <typename T>
+__device__ __forceinline__ void load3(const T* __restrict__ p, double& x, double& y, double& z) {
+  using V2 = typename Pair2<T>::type;
+  const bool lo = (reinterpret_cast<uintptr_t>(p) & (2 * sizeof(T) - 1)) == 0;
+  const V2 q = __ldg(reinterpret_cast<const V2*>(lo ? p : p + 1));
+  const T s = __ldg(lo ? p + 2 : p);
+  x = (double)(lo ? q.x : s);
+  y = (double)(lo ? q.y : q.x);
+  z = (double)(lo ? s : q.y);
+}
 template <typename T>
 __device__ __forceinline__ d3 load_vertex(const T* __restrict__ pos, int v) {
-  const T* p = pos + 3 * (int64_t)v;
-  return ttg::mk((double)__ldg(p), (double)__ldg(p + 1), (double)__ldg(p + 2));
+  d3 r;
+  load3(pos + 3 * (int64_t)v, r.x, r.y, r.z);
+  return r;
 }
 
 // Gathers the six vertices of candidate (ta, tb) translated by -a0 (local frame: kills the
