@@ -44,6 +44,14 @@ __device__ __forceinline__ void load3(const T* __restrict__ p, double& x, double
   y = (double)(lo ? q.y : q.x);
   z = (double)(lo ? s : q.y);
 }
+__device__ __forceinline__ void load3i(const int* __restrict__ p, int (&v)[3]) {  // same, for a triangle's vertex ids
+  const bool lo = (reinterpret_cast<uintptr_t>(p) & 7) == 0;
+  const int2 q = __ldg(reinterpret_cast<const int2*>(lo ? p : p + 1));
+  const int s = __ldg(lo ? p + 2 : p);
+  v[0] = lo ? q.x : s;
+  v[1] = lo ? q.y : q.x;
+  v[2] = lo ? s : q.y;
+}
 template <typename T>
 __device__ __forceinline__ d3 load_vertex(const T* __restrict__ pos, int v) {
   d3 r;
@@ -58,11 +66,8 @@ template <typename T>
 __device__ __forceinline__ bool gather_pair(const T* __restrict__ pos, const int* __restrict__ tris,
                                             int ta, int tb, int (&va)[3], int (&vb)[3], d3 (&a)[3],
                                             d3 (&b)[3]) {
-#pragma unroll
-  for (int m = 0; m < 3; ++m) {
-    va[m] = __ldg(tris + 3 * (int64_t)ta + m);
-    vb[m] = __ldg(tris + 3 * (int64_t)tb + m);
-  }
+  load3i(tris + 3 * (int64_t)ta, va);
+  load3i(tris + 3 * (int64_t)tb, vb);
   bool adj = false;
 #pragma unroll
   for (int m = 0; m < 3; ++m)
