@@ -933,7 +933,8 @@ __device__ __forceinline__ void prefetch_pos_l2(const T* __restrict__ pos, const
   for (int v = 0; v < 6; ++v) {
     const T* p = pos + 3 * (int64_t)ids[v];
     asm volatile("prefetch.global.L2 [%0];" ::"l"(p));
-    asm volatile("prefetch.global.L2 [%0];" ::"l"(p + 2));
+    if ((reinterpret_cast<uintptr_t>(p) & 31) + 3 * sizeof(T) > 32)  // the vertex straddles two sectors
+      asm volatile("prefetch.global.L2 [%0];" ::"l"(p + 2));
   }
 }
 struct alignas(16) LongWarpSmem {
