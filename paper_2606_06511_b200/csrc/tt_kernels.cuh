@@ -625,11 +625,9 @@ k_round_symbolic(const int* __restrict__ tris, const int* __restrict__ touched, 
     const int64_t e = (int64_t)e_lo + lane;
     const int t = (int)(__ldg(keys + e) & tmask);
     pay = (unsigned)__ldg(dvals + e);
+    load3i(tris + 3 * (int64_t)t, cv);
 #pragma unroll
-    for (int n = 0; n < 3; ++n) {
-      cv[n] = __ldg(tris + 3 * (int64_t)t + n);
-      cand[3 * lane + n] = cv[n];
-    }
+    for (int n = 0; n < 3; ++n) cand[3 * lane + n] = cv[n];
   }
   const unsigned heads = __reduce_or_sync(FULL, (lane < ntri) ? (1u << f) : 0u);
   const int my_ti = __popc(heads & (0xffffffffu >> (31 - lane))) - 1;
@@ -745,11 +743,8 @@ k_round_fill(const int* __restrict__ tris, const int* __restrict__ touched, cons
   if (lane < nent) {
     const int64_t e = (int64_t)e_lo + lane;
     const int t = (int)(__ldg(keys + e) & tmask);
-#pragma unroll
-    for (int n = 0; n < 3; ++n) {
-      cv[n] = __ldg(tris + 3 * (int64_t)t + n);
-      er[n] = __ldg(erank + 3 * e + n);
-    }
+    load3i(tris + 3 * (int64_t)t, cv);
+    load3i(erank + 3 * e, er);
   }
   int f = 0;
   if (lane < ntri) {
