@@ -9,10 +9,11 @@
 //                                warp per round of whole triangles: recompute J analytically,
 //                                build each row's run of 3x3 blocks in a shared-memory tile,
 //                                sum diagonal rows + gradient in fixed order (no atomics), write
-//                                the runs out with TMA bulk copies (k_assemble_long: triangles
-//                                with more than 32 partners)
+//                                the runs out with TMA bulk copies (k_assemble_long_tile /
+//                                k_assemble_long_direct: triangles with more than 32 partners)
 //   K5  k_merge / k_gather3    : general rows (vertices shared by several touched triangles)
-//   K6  k_entry_reduce  a5     : matrix-free H.p (and the gradient-only call), same rounds
+//   K6  k_entry_pipe    a5     : matrix-free H.p (and the gradient-only call), same rounds
+//                                (k_entry_reduce: triangles with more than 32 partners)
 #pragma once
 #include <cstdint>
 #include <cuda_runtime.h>
@@ -874,17 +875,6 @@ __device__ __forceinline__ void cp_async_elem(T* sdst, const T* gsrc) {
 __device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
 template <int N>
 __device__ __forceinline__ void cp_async_wait() { asm volatile("cp.async.wait_group %0;" ::"n"(N) : "memory"); }
-
-// 18 values of six vertices -> lane-private shared slots buf[k * 32 + lane]
-template <typename T>
-__device__ __forceinline__ void gather18_async(T* buf, int lane, const T* __restrict__ src, const int (&ids)[6]) {
-#pragma unroll
-  for (int v = 0; v < 6; ++v) {
-    const T* g = src + 3 * (int64_t)ids[v];
-#pragma unroll
-    for (int k = 0; k < 3; ++k) cp_async_elem(buf + (3 * v + k) * 32 + lane, g + k);
-  }
-}
 
 #ifndef TT_TILE_WARPS
 #define TT_TILE_WARPS 1
@@ -1863,11 +1853,6 @@ __global__ void k_gather3(const int* __restrict__ vcnt, const int* __restrict__ 
   out[3 * v] = r0;
   out[3 * v + 1] = r1;
   out[3 * v + 2] = r2;
-}
-
-__global__ void k_iota(uint32_t* __restrict__ v, int64_t n) {
-  const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
-  if (i < n) v[i] = (uint32_t)i;
 }
 
 __global__ void k_i64_to_i32(const int64_t* __restrict__ in, int64_t n, int* __restrict__ out) {
