@@ -145,7 +145,7 @@ tt_status tt_bsr_device(tt_ctx* ctx, const int32_t** rowptr, const int32_t** col
 
 /* Counters of the last tt_hess_symbolic: what[0]=n_active, [1]=directed entries (2*n_active),
  * [2]=touched triangles, [3]=blocks written directly (exclusive rows), [4]=blocks produced by the
- * general-row merge, [5]=merge records, [6]=nnzb, [7]=kernel launches issued by this ctx so far.                     */
+ * general-row merge, [5]=merge records, [6]=nnzb, [7]=kernels launched by this ctx so far (CUB calls counted by the kernels they launch).                     */
 tt_status tt_stats(const tt_ctx* ctx, int64_t* what, int32_t n);
 
 /* Device durations (CUDA events on the caller's stream) of the most recent launch of the three

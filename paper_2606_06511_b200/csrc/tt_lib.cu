@@ -151,7 +151,7 @@ tt_status scan_i32(tt_ctx* ctx, const int* in, int* out, int64_t n_plus_1, cudaS
   TT_CUDA(cub::DeviceScan::ExclusiveSum(nullptr, tmp, in, out, n_plus_1, st));
   TT_CUDA(ctx->cub_tmp.ensure(tmp));
   TT_CUDA(cub::DeviceScan::ExclusiveSum(ctx->cub_tmp.p, tmp, in, out, n_plus_1, st));
-  ctx->launches++;
+  ctx->launches += 2;  // CUB scan: init + scan kernel
   return TT_OK;
 }
 tt_status scan_i64(tt_ctx* ctx, const int64_t* in, int64_t* out, int64_t n_plus_1, cudaStream_t st) {
@@ -159,7 +159,7 @@ tt_status scan_i64(tt_ctx* ctx, const int64_t* in, int64_t* out, int64_t n_plus_
   TT_CUDA(cub::DeviceScan::ExclusiveSum(nullptr, tmp, in, out, n_plus_1, st));
   TT_CUDA(ctx->cub_tmp.ensure(tmp));
   TT_CUDA(cub::DeviceScan::ExclusiveSum(ctx->cub_tmp.p, tmp, in, out, n_plus_1, st));
-  ctx->launches++;
+  ctx->launches += 2;  // CUB scan: init + scan kernel
   return TT_OK;
 }
 tt_status scan_i32_to_i64(tt_ctx* ctx, const int* in, int64_t* out, int64_t n_plus_1, cudaStream_t st) {
@@ -168,7 +168,7 @@ tt_status scan_i32_to_i64(tt_ctx* ctx, const int* in, int64_t* out, int64_t n_pl
   TT_CUDA(cub::DeviceScan::ExclusiveSum(nullptr, tmp, it, out, n_plus_1, st));
   TT_CUDA(ctx->cub_tmp.ensure(tmp));
   TT_CUDA(cub::DeviceScan::ExclusiveSum(ctx->cub_tmp.p, tmp, it, out, n_plus_1, st));
-  ctx->launches++;
+  ctx->launches += 2;  // CUB scan: init + scan kernel
   return TT_OK;
 }
 tt_status incl_scan_i32(tt_ctx* ctx, const int* in, int* out, int64_t n, cudaStream_t st) {
@@ -176,7 +176,7 @@ tt_status incl_scan_i32(tt_ctx* ctx, const int* in, int* out, int64_t n, cudaStr
   TT_CUDA(cub::DeviceScan::InclusiveSum(nullptr, tmp, in, out, n, st));
   TT_CUDA(ctx->cub_tmp.ensure(tmp));
   TT_CUDA(cub::DeviceScan::InclusiveSum(ctx->cub_tmp.p, tmp, in, out, n, st));
-  ctx->launches++;
+  ctx->launches += 2;  // CUB scan: init + scan kernel
   return TT_OK;
 }
 // stable LSD radix sort of (key, payload) on bits [0, end_bit); result pointers returned
@@ -189,7 +189,7 @@ tt_status sort_pairs(tt_ctx* ctx, DevBuf (&kb)[2], DevBuf (&vb)[2], int64_t n, i
   TT_CUDA(cub::DeviceRadixSort::SortPairs(nullptr, tmp, dk, dv, n, begin_bit, end_bit, st));
   TT_CUDA(ctx->cub_tmp.ensure(tmp));
   TT_CUDA(cub::DeviceRadixSort::SortPairs(ctx->cub_tmp.p, tmp, dk, dv, n, begin_bit, end_bit, st));
-  ctx->launches++;
+  ctx->launches += 2 + (end_bit - begin_bit + 7) / 8;  // CUB onesweep sort: histogram + exclusive sum + one kernel per 8-bit pass
   *k_out = dk.Current();
   *v_out = dv.Current();
   return TT_OK;
@@ -313,7 +313,7 @@ tt_status symbolic_impl(tt_ctx* ctx, const tt_problem* q, int64_t* nnzb_host, in
     TT_CUDA(cub::DeviceSelect::Flagged(nullptr, tmp, iota, ctx->tflag.as<int>(), ctx->touched.as<int>(), d_num, (int)nT, st));
     TT_CUDA(ctx->cub_tmp.ensure(tmp));
     TT_CUDA(cub::DeviceSelect::Flagged(ctx->cub_tmp.p, tmp, iota, ctx->tflag.as<int>(), ctx->touched.as<int>(), d_num, (int)nT, st));
-    ctx->launches++;
+    ctx->launches += 2;  // CUB select: init + sweep kernel
     const int64_t buckets_ub = (touched_ub + CHK_BUCKET - 1) / CHK_BUCKET;
     TT_CUDA(ctx->bucket_cnt.ensure(sizeof(int) * (size_t)(buckets_ub + 1)));
     TT_CUDA(ctx->bucket_off.ensure(sizeof(int) * (size_t)(buckets_ub + 1)));
