@@ -231,10 +231,22 @@ def main():
     yvec = torch.empty_like(pvec)
     log("[bench] rank %d: A=%d nnzb=%d (vals %.2f GB)" % (rank, n_active, nnzb, nnzb * 9 * w / 1e9))
 
-    def step():
+    phase_ev = []                                     # per timed step: 4 events around the three calls
+
+    def step(record=False):
+        ev = [torch.cuda.Event(enable_timing=True) for _ in range(4)] if record else None
+        if record:
+            ev[0].record(stream)
         ctx.tt_hess_symbolic(prob)
+        if record:
+            ev[1].record(stream)
         ctx.tt_energy_grad_hess(prob, energy, grad, rowptr, colind, vals, max(nnzb, 1))
+        if record:
+            ev[2].record(stream)
         ctx.tt_hess_vec(prob, pvec, yvec)
+        if record:
+            ev[3].record(stream)
+            phase_ev.append(ev)
 
     for _ in range(args.warmup):
         step()
@@ -249,7 +261,7 @@ def main():
     t_wall0 = time.time()
     ev0.record(stream)
     for _ in range(args.steps):
-        step()
+        step(record=True)
         for k, v in ctx.tt_kernel_ms().items():      # waits for the step's last kernel; no extra work
             kms[k].append(v)
     ev1.record(stream)
@@ -342,6 +354,8 @@ def main():
            "roofline": roofline, "cpu_baseline": cpu, "e2e": e2e, "gpu_launches": int(launches),
            "clocks": clocks,
            "kernel_ms": {k: float(np.mean(v)) for k, v in kms.items()},
+           "phase_ms": {name: float(np.mean([e[i].elapsed_time(e[i + 1]) for e in phase_ev]))
+                        for i, name in enumerate(("tt_hess_symbolic", "tt_energy_grad_hess", "tt_hess_vec"))},
            "active_pairs_per_s": n_active * world / (ms_step * 1e-3)}
     print(json.dumps(out), flush=True)
     if world > 1:
