@@ -45,6 +45,7 @@ __device__ __forceinline__ void load3(const T* __restrict__ p, double& x, double
   y = (double)(lo ? q.y : q.x);
   z = (double)(lo ? s : q.y);
 }
+__device__ __forceinline__ int pick3(int i, int v0, int v1, int v2) { return i == 0 ? v0 : (i == 1 ? v1 : v2); }
 __device__ __forceinline__ void load3i(const int* __restrict__ p, int (&v)[3]) {  // same, for a triangle's vertex ids
   const bool lo = (reinterpret_cast<uintptr_t>(p) & 7) == 0;
   const int2 q = __ldg(reinterpret_cast<const int2*>(lo ? p : p + 1));
@@ -245,14 +246,18 @@ __global__ void k_vertex_touch(const int* __restrict__ tris, const int* __restri
 // Per-slot arrays (drank, tlen, toff, slot_excl, rowbase, tslot) are indexed by TOUCHED index ti:
 // the numeric kernels then need no triangle id to find them.
 // layout = rank (columns ascending) when there is no duplicate, else identity (3j+n, diag last).
+// Duplicates are detected as in k_round_symbolic: the ranks of L distinct values sum to L (L - 1) / 2.
+// Also writes the per-entry vertex ids (everts) of the triangle's entries.
 __global__ void __launch_bounds__(32 * SYM_WARPS)
 k_tri_symbolic(const int* __restrict__ tris, const int* __restrict__ touched, int64_t n_touched,
-               const int* __restrict__ tptr, const uint64_t* __restrict__ keys, int bitsT,
-               const int* __restrict__ vcnt, int force_general, int* __restrict__ erank /*[2A][3]*/,
+               const int* __restrict__ tptr, const uint64_t* __restrict__ keys, const uint16_t* __restrict__ dvals,
+               int bitsT, const int* __restrict__ vcnt, int force_general, int* __restrict__ erank /*[2A][3]*/,
                int* __restrict__ drank /*[n_touched][3]*/, int* __restrict__ rowlen,
                int64_t* __restrict__ tlen /*[3 n_touched]*/, uint8_t* __restrict__ slot_excl /*[3 n_touched]*/,
-               const int* __restrict__ long_list, const int4* __restrict__ rdesc, int* __restrict__ vslot1) {
+               const int* __restrict__ long_list, const int4* __restrict__ rdesc, int* __restrict__ vslot1,
+               int* __restrict__ everts) {
   __shared__ int s_c[SYM_WARPS][SYM_LMAX];
+  constexpr unsigned FULL = 0xffffffffu;
   const int w = threadIdx.x >> 5, l = threadIdx.x & 31;
   const int64_t li = (int64_t)blockIdx.x * SYM_WARPS + w;  // n_touched counts the LONG triangles here
   if (li >= n_touched) return;
@@ -261,7 +266,25 @@ k_tri_symbolic(const int* __restrict__ tris, const int* __restrict__ touched, in
   const int e0 = tptr[s], deg = tptr[s + 1] - e0;
   const int L = 3 * (deg + 1);
   const uint64_t tmask = (1ull << bitsT) - 1ull;
-  bool nodup = (L <= SYM_LMAX);
+  int own[3];
+  load3i(tris + 3 * (int64_t)s, own);
+  // vertex ids of the canonical pair of every entry, both triangles in recorded (k, p, q) order
+  for (int j = l; j < deg; j += 32) {
+    const int64_t e = (int64_t)e0 + j;
+    int cv[3];
+    load3i(tris + 3 * (int64_t)(keys[e] & tmask), cv);
+    const unsigned pay = dvals[e];
+    const bool side = (pay & 1u) != 0u;
+    const unsigned ca = (pay >> 1) & 63u, cb = (pay >> 7) & 63u;
+    const int ka = (int)(ca & 3u), pa = (int)((ca >> 2) & 3u), kb = (int)(cb & 3u), pb = (int)((cb >> 2) & 3u);
+    const int a0 = side ? cv[0] : own[0], a1 = side ? cv[1] : own[1], a2 = side ? cv[2] : own[2];
+    const int b0 = side ? own[0] : cv[0], b1 = side ? own[1] : cv[1], b2 = side ? own[2] : cv[2];
+    int2* o = reinterpret_cast<int2*>(everts + 6 * e);
+    o[0] = make_int2(pick3(ka, a0, a1, a2), pick3(pa, a0, a1, a2));
+    o[1] = make_int2(pick3(3 - ka - pa, a0, a1, a2), pick3(kb, b0, b1, b2));
+    o[2] = make_int2(pick3(pb, b0, b1, b2), pick3(3 - kb - pb, b0, b1, b2));
+  }
+  bool nodup = (L <= SYM_LMAX);  // longer rows: identity layout, general rows
   int* c = s_c[w];
   if (nodup) {
     for (int idx = l; idx < L; idx += 32) {
@@ -270,28 +293,29 @@ k_tri_symbolic(const int* __restrict__ tris, const int* __restrict__ touched, in
       c[idx] = tris[3 * (int64_t)t + n];
     }
     __syncwarp();
-    bool dup = false;
+    long long sum = 0;
     for (int idx = l; idx < L; idx += 32) {
       const int me = c[idx];
-      int eq = 0;
-      for (int x = 0; x < L; ++x) eq += (c[x] == me);
-      dup |= (eq > 1);
-    }
-    nodup = !__any_sync(0xffffffffu, dup);
-  }
-  for (int idx = l; idx < L; idx += 32) {
-    int r = idx;
-    if (nodup) {
-      const int me = c[idx];
-      r = 0;
+      int r = 0;
       for (int x = 0; x < L; ++x) r += (c[x] < me);
+      sum += r;
+      const int j = idx / 3, n = idx - 3 * j;
+      if (j < deg) erank[3 * (int64_t)(e0 + j) + n] = r;
+      else drank[3 * ti + n] = r;
     }
-    const int j = idx / 3, n = idx - 3 * j;
-    if (j < deg) erank[3 * (int64_t)(e0 + j) + n] = r;
-    else drank[3 * ti + n] = r;
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) sum += __shfl_xor_sync(FULL, sum, o);
+    nodup = (2 * sum == (long long)L * (L - 1));
+  }
+  if (!nodup) {
+    for (int idx = l; idx < L; idx += 32) {
+      const int j = idx / 3, n = idx - 3 * j;
+      if (j < deg) erank[3 * (int64_t)(e0 + j) + n] = idx;
+      else drank[3 * ti + n] = idx;
+    }
   }
   if (l < 3) {
-    const int p = tris[3 * (int64_t)s + l];
+    const int p = own[l == 0 ? 0 : (l == 1 ? 1 : 2)];
     const bool excl = nodup && !force_general && (vcnt[p] == 1);
     if (vcnt[p] == 1) vslot1[p] = (int)(3 * ti + l);  // the vertex's only slot (k_gather3)
     slot_excl[3 * ti + l] = excl ? 1 : 0;
@@ -532,28 +556,6 @@ struct AsmParams {
   double sigma;
 };
 
-// Per-entry vertex ids of the canonical pair with both triangles permuted as K1 recorded
-// (symbolic phase, once per active set): everts[e] = [a_k, a_p, a_q, b_k, b_p, b_q].
-__global__ void k_ent_verts(const uint64_t* __restrict__ keys, const uint16_t* __restrict__ dvals,
-                            const int* __restrict__ tris, int64_t n_dir, int bitsT, int* __restrict__ everts) {
-  const int64_t e = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
-  if (e >= n_dir) return;
-  const uint64_t key = keys[e];
-  const unsigned pay = dvals[e];
-  const int s = (int)(key >> bitsT), t = (int)(key & ((1ull << bitsT) - 1ull));
-  const bool side = (pay & 1u) != 0u;
-  const int ta = side ? t : s, tb = side ? s : t;  // canonical (pairs[k,0], pairs[k,1])
-  const unsigned ca = (pay >> 1) & 63u, cb = (pay >> 7) & 63u;
-  const int ka = (int)(ca & 3u), pa = (int)((ca >> 2) & 3u), kb = (int)(cb & 3u), pb = (int)((cb >> 2) & 3u);
-  int* o = everts + 6 * e;
-  o[0] = __ldg(tris + 3 * (int64_t)ta + ka);
-  o[1] = __ldg(tris + 3 * (int64_t)ta + pa);
-  o[2] = __ldg(tris + 3 * (int64_t)ta + (3 - ka - pa));
-  o[3] = __ldg(tris + 3 * (int64_t)tb + kb);
-  o[4] = __ldg(tris + 3 * (int64_t)tb + pb);
-  o[5] = __ldg(tris + 3 * (int64_t)tb + (3 - kb - pb));
-}
-
 __global__ void k_round_desc(const int* __restrict__ chunk_start, const int* __restrict__ tfirst, int64_t n_chunks,
                              int64_t n_touched, int4* __restrict__ rdesc) {
   const int64_t c = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
@@ -570,7 +572,6 @@ __global__ void k_round_desc(const int* __restrict__ chunk_start, const int* __r
 // wide and 32 entries deep instead of one warp per (on average 5-entry) triangle.
 constexpr int RSYM_WARPS = 4;
 
-__device__ __forceinline__ int pick3(int i, int v0, int v1, int v2) { return i == 0 ? v0 : (i == 1 ? v1 : v2); }
 
 // Column ranks (erank / drank), duplicate detection, exclusive rows, row lengths and the per-entry
 // vertex ids (everts) of every non-long round.

@@ -376,13 +376,11 @@ tt_status symbolic_impl(tt_ctx* ctx, const tt_problem* q, int64_t* nnzb_host, in
     TT_LAUNCH_CHECK();
   }
   if (n_long > 0) {  // triangles with more than RND_MAX_ENT partners: one warp per triangle
-    k_ent_verts<<<grid_for(n, 256), 256, 0, st>>>(ctx->keys_sorted, ctx->dvals_sorted, q->tris, n, bitsT, ctx->everts.as<int>());
-    TT_LAUNCH_CHECK();
     k_tri_symbolic<<<grid_for(n_long, SYM_WARPS), 32 * SYM_WARPS, 0, st>>>(
-        q->tris, ctx->touched.as<int>(), n_long, ctx->tptr.as<int>(), ctx->keys_sorted, bitsT,
+        q->tris, ctx->touched.as<int>(), n_long, ctx->tptr.as<int>(), ctx->keys_sorted, ctx->dvals_sorted, bitsT,
         ctx->vcnt.as<int>(), (ctx->opt.flags & TT_FLAG_FORCE_GENERAL_ROWS) ? 1 : 0, ctx->erank.as<int>(),
         ctx->drank.as<int>(), ctx->rowlen.as<int>(), ctx->tlen.as<int64_t>(), ctx->slot_excl.as<uint8_t>(),
-        ctx->long_list.as<int>(), ctx->rdesc.as<int4>(), ctx->vslot1.as<int>());
+        ctx->long_list.as<int>(), ctx->rdesc.as<int4>(), ctx->vslot1.as<int>(), ctx->everts.as<int>());
     TT_LAUNCH_CHECK();
   }
   s = scan_i64(ctx, ctx->tlen.as<int64_t>(), ctx->toff.as<int64_t>(), 3 * n_touched + 1, st);
