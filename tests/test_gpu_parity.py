@@ -159,17 +159,18 @@ def test_config4_sweep_reduced(oracle_mod, dtype):
     assert abs(out["n_active"] / pb.n_pairs - 0.5) < 0.01
 
 
-@pytest.mark.parametrize("n_pairs,dtype", [(16_000, "f64"), (16_000, "f32"), (60_000, "f64")])
+@pytest.mark.parametrize("n_pairs,dtype", [(24_000, "f64"), (24_000, "f32"), (60_000, "f64")])
 def test_long_triangles(oracle_mod, n_pairs, dtype):
-    """Few triangles, many pairs each.  16k pairs: ~40 partners per triangle, a mix of ordinary rounds
-    and long triangles that fit the one-row tile (k_assemble_long_tile); 60k pairs: ~150 partners,
-    beyond the tile (k_assemble_long_direct)."""
+    """Few triangles, many pairs each.  24k pairs: ~60 partners per triangle, a mix of ordinary rounds,
+    long triangles with J cached (33..64 partners) and re-evaluated (65..127) in the one-row tile
+    (k_assemble_long_tile<true / false>); 60k pairs: ~150 partners, beyond the tile
+    (k_assemble_long_direct)."""
     from paper_2606_06511_b200 import inputs
     pb = inputs.config4_sweep(n_tris=400, n_pairs=n_pairs, seed=4242)
     ref, out, st = run_case(oracle_mod, pb, dtype, 1)
     deg = np.bincount(pb.pairs[ref["active"].astype(bool)].ravel(), minlength=400)
-    if n_pairs == 16_000:
-        assert ((deg > 32) & (deg <= 127)).sum() > 50 and (deg <= 32).sum() > 20
+    if n_pairs == 24_000:
+        assert ((deg > 32) & (deg <= 64)).sum() > 50 and ((deg > 64) & (deg <= 127)).sum() > 30 and (deg <= 32).sum() > 20
     else:
         assert (deg > 127).sum() > 50
 
