@@ -21,7 +21,7 @@ _HERE = Path(__file__).resolve().parent
 _SRC = _HERE / "tt_oracle.cpp"
 _LIB = _HERE / "libtt_oracle.so"
 
-HESS_EQ4, HESS_FILTER, HESS_PSD2 = 0, 1, 2
+HESS_EQ4, HESS_FILTER, HESS_PSD2, HESS_PSDPROJ = 0, 1, 2, 3
 
 _lib = None
 

@@ -238,6 +238,67 @@ inline void hess_coeffs(const double tc[2], const double g0[NDOF], const double 
   c[2] = 4.0 * tc[0] * tc[1] * keep;
 }
 
+// mode 3 PSDPROJ (the literal "eigenanalysis" of L47 carried through): the
+// per-pair Hessian is the projection of Eq. 4's 18x18 matrix onto the positive semi-definite cone,
+//   H+ = sum_i max(lambda_i, 0) v_i v_i^T,   H_EQ4 = sum_i lambda_i v_i v_i^T,
+// written out as that definition: cyclic Jacobi eigen-decomposition of the dense symmetric matrix
+// (no use of its rank-2 structure; the GPU path uses a closed 2x2 form instead).
+inline void jacobi_eigh(double* A /*[n*n], destroyed: diagonal = eigenvalues*/, double* V /*[n*n] columns*/, int n) {
+  for (int i = 0; i < n; ++i)
+    for (int j = 0; j < n; ++j) V[i * n + j] = (i == j) ? 1.0 : 0.0;
+  for (int sweep = 0; sweep < 64; ++sweep) {
+    double off = 0.0, diag = 0.0;
+    for (int i = 0; i < n; ++i)
+      for (int j = 0; j < n; ++j) (i == j ? diag : off) += A[i * n + j] * A[i * n + j];
+    if (off <= 1e-60 + 1e-32 * diag) break;
+    for (int p = 0; p < n - 1; ++p)
+      for (int q = p + 1; q < n; ++q) {
+        const double apq = A[p * n + q];
+        if (apq == 0.0) continue;
+        const double theta = (A[q * n + q] - A[p * n + p]) / (2.0 * apq);
+        const double t = (theta >= 0.0 ? 1.0 : -1.0) / (std::fabs(theta) + std::sqrt(theta * theta + 1.0));
+        const double c = 1.0 / std::sqrt(t * t + 1.0), sn = t * c;
+        for (int k = 0; k < n; ++k) {  // A <- A R (columns p, q)
+          const double akp = A[k * n + p], akq = A[k * n + q];
+          A[k * n + p] = c * akp - sn * akq;
+          A[k * n + q] = sn * akp + c * akq;
+        }
+        for (int k = 0; k < n; ++k) {  // A <- R^T A (rows p, q)
+          const double apk = A[p * n + k], aqk = A[q * n + k];
+          A[p * n + k] = c * apk - sn * aqk;
+          A[q * n + k] = sn * apk + c * aqk;
+        }
+        for (int k = 0; k < n; ++k) {  // V <- V R
+          const double vkp = V[k * n + p], vkq = V[k * n + q];
+          V[k * n + p] = c * vkp - sn * vkq;
+          V[k * n + q] = sn * vkp + c * vkq;
+        }
+      }
+  }
+}
+// Dense per-pair Hessian in the given mode.  Modes 0-2: Eq. 4 with hess_coeffs; mode 3: PSD projection.
+inline void pair_hessian(const double tc[2], const double g0[NDOF], const double g1[NDOF], int mode,
+                         double H[NDOF * NDOF]) {
+  double c[3], lam[3];
+  hess_coeffs(tc, g0, g1, mode == 3 ? 0 : mode, c, lam);
+  for (int i = 0; i < NDOF; ++i)
+    for (int j = 0; j < NDOF; ++j)
+      H[i * NDOF + j] = c[0] * g0[i] * g0[j] + c[1] * g1[i] * g1[j] + c[2] * (g1[i] * g0[j] + g0[i] * g1[j]);
+  if (mode != 3) return;
+  double A[NDOF * NDOF], V[NDOF * NDOF];
+  std::memcpy(A, H, sizeof(A));
+  jacobi_eigh(A, V, NDOF);
+  for (int i = 0; i < NDOF; ++i)
+    for (int j = 0; j < NDOF; ++j) {
+      double s = 0.0;
+      for (int k = 0; k < NDOF; ++k) {
+        const double lk = A[k * NDOF + k];
+        if (lk > 0.0) s += lk * V[i * NDOF + k] * V[j * NDOF + k];
+      }
+      H[i * NDOF + j] = s;
+    }
+}
+
 inline bool share_vertex(const int32_t* ta, const int32_t* tb) {
   for (int i = 0; i < 3; ++i)
     for (int j = 0; j < 3; ++j)
@@ -291,11 +352,10 @@ void tt_oracle_pair(const double* x, double sigma, int hess_mode, int* active, d
   }
   if (grad)
     for (int i = 0; i < NDOF; ++i) grad[i] = cg[0] * r.g[0][i] + cg[1] * r.g[1][i];
-  if (H)
-    for (int i = 0; i < NDOF; ++i)
-      for (int j = 0; j < NDOF; ++j)
-        H[i * NDOF + j] = c[0] * r.g[0][i] * r.g[0][j] + c[1] * r.g[1][i] * r.g[1][j] +
-                          c[2] * (r.g[1][i] * r.g[0][j] + r.g[0][i] * r.g[1][j]);
+  if (H) {
+    if (r.active) pair_hessian(r.tc, r.g[0], r.g[1], hess_mode, H);
+    else std::memset(H, 0, sizeof(double) * NDOF * NDOF);
+  }
   if (lam) { lam[0] = l[0]; lam[1] = l[1]; lam[2] = l[2]; }
 }
 
@@ -382,9 +442,9 @@ void tt_oracle_assemble(int64_t n_verts, const int32_t* tris, const int32_t* pai
     }
     const double* g0 = J + 36 * k;
     const double* g1 = g0 + 18;
-    double cg[2], c[3], lam[3];
+    double cg[2], Hk[NDOF * NDOF];
     grad_coeffs(tc + 2 * k, cg);
-    hess_coeffs(tc + 2 * k, g0, g1, hess_mode, c, lam);
+    if (vals) pair_hessian(tc + 2 * k, g0, g1, hess_mode, Hk);
     if (grad)
       for (int v = 0; v < 6; ++v)
         for (int a = 0; a < 3; ++a)
@@ -397,11 +457,7 @@ void tt_oracle_assemble(int64_t n_verts, const int32_t* tris, const int32_t* pai
           const int32_t* it = std::lower_bound(lo, hi, vid[q]);
           double* blk = vals + 9 * (int64_t)(it - colind);
           for (int a = 0; a < 3; ++a)
-            for (int b = 0; b < 3; ++b) {
-              int i = 3 * p + a, j = 3 * q + b;
-              blk[3 * a + b] += c[0] * g0[i] * g0[j] + c[1] * g1[i] * g1[j] +
-                                c[2] * (g1[i] * g0[j] + g0[i] * g1[j]);
-            }
+            for (int b = 0; b < 3; ++b) blk[3 * a + b] += Hk[(3 * p + a) * NDOF + 3 * q + b];
         }
   }
 }
@@ -420,6 +476,16 @@ void tt_oracle_hess_vec_pairs(int64_t n_verts, const int32_t* tris, const int32_
     }
     const double* g0 = J + 36 * k;
     const double* g1 = g0 + 18;
+    if (hess_mode == 3) {   // y_loc = H+ p_loc with the dense projected matrix
+      double Hk[NDOF * NDOF];
+      pair_hessian(tc + 2 * k, g0, g1, 3, Hk);
+      for (int i = 0; i < NDOF; ++i) {
+        double acc = 0.0;
+        for (int j = 0; j < NDOF; ++j) acc += Hk[i * NDOF + j] * p[3 * (int64_t)vid[j / 3] + j % 3];
+        y[3 * (int64_t)vid[i / 3] + i % 3] += acc;
+      }
+      continue;
+    }
     double c[3], lam[3];
     hess_coeffs(tc + 2 * k, g0, g1, hess_mode, c, lam);
     double s0 = 0.0, s1 = 0.0;   // J p_loc

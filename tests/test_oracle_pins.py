@@ -327,7 +327,7 @@ def test_monte_carlo_intersection_probability(oracle_mod):
 
 
 # ---------------------------------------------------------------- P9 / P10: assembly
-@pytest.mark.parametrize("mode", [0, 1, 2])
+@pytest.mark.parametrize("mode", [0, 1, 2, 3])
 def test_assembly_against_dense(oracle_mod, mode):
     """BSR of config 0 (192 block rows) == dense 576x576 accumulation of the per-pair 18x18;
     H.p three ways; with p = x and EQ4, H x = 3 grad (I6)."""
@@ -374,6 +374,49 @@ def test_assembly_against_dense(oracle_mod, mode):
         if mode == 0:
             yx = oracle_mod.hess_vec_pairs(nV, pb.tris, pb.pairs, out["active"], out["tc"], out["J"], pb.pos, mode)
             np.testing.assert_allclose(yx, 3 * out["grad"], atol=1e-10 * np.abs(out["grad"]).max())
+
+
+def test_psd_projection_mode(oracle_mod):
+    """hess_mode 3: the per-pair Hessian is the PSD projection of Eq. 4's matrix.
+    Pins: (a) worked example A by hand -- the non-zero eigenvalues of J^T M J are those of M G with
+    G = J J^T = [[15/4, -3/4], [-3/4, 11/4]], M = [[2, -12], [-12, 18]]: trace 75, determinant
+    det M det G = (-108)(39/4) = -1053, so lambda = (75 +- sqrt(9837)) / 2 and H+ is rank one with
+    Frobenius norm = trace = lambda_+; (b) LAPACK's eigh (numpy) of the oracle's own Eq. 4 matrix on
+    random active pairs (the oracle uses its own Jacobi sweeps); (c) H+ is symmetric, PSD, keeps the
+    translation null space, H+ - H_EQ4 is PSD, and H+ = H for a matrix that is PSD already (PSD2)."""
+    x = x_of(load_fixture("example_A.txt"))
+    lam_p = (75.0 + np.sqrt(9837.0)) / 2.0
+    lam_m = (75.0 - np.sqrt(9837.0)) / 2.0
+    H3 = oracle_mod.pair(x, 1.0, 3)["H"]
+    H0 = oracle_mod.pair(x, 1.0, 0)["H"]
+    np.testing.assert_allclose(np.linalg.norm(H3), lam_p, rtol=1e-12)
+    np.testing.assert_allclose(np.trace(H3), lam_p, rtol=1e-12)
+    np.testing.assert_allclose(np.trace(H3 - H0), -lam_m, rtol=1e-11)
+    w = np.linalg.eigvalsh(H3)
+    assert w[0] > -1e-12 * lam_p and abs(w[-2]) < 1e-12 * lam_p                 # PSD, rank one
+    rng = np.random.default_rng(33)
+    seen = 0
+    while seen < 40:
+        xr = rng.uniform(0, 1, 18)
+        r0 = oracle_mod.pair(xr, 1.0, 0)
+        if not r0["active"]:
+            continue
+        seen += 1
+        H3 = oracle_mod.pair(xr, 1.0, 3)["H"]
+        lam, U = np.linalg.eigh(r0["H"])
+        ref = (U * np.maximum(lam, 0.0)) @ U.T
+        sc = np.abs(r0["H"]).max()
+        np.testing.assert_allclose(H3, ref, atol=1e-11 * sc)
+        np.testing.assert_allclose(H3, H3.T, atol=1e-13 * sc)
+        assert np.linalg.eigvalsh(H3)[0] > -1e-11 * sc
+        assert np.linalg.eigvalsh(H3 - r0["H"])[0] > -1e-11 * sc
+        shift = np.tile(rng.normal(size=3), 6)
+        assert np.abs(H3 @ shift).max() < 1e-10 * sc * np.abs(shift).max()
+    # a matrix that is PSD already is its own projection: parts one and two only
+    xa = x_of(load_fixture("example_A.txt"))
+    r2 = oracle_mod.pair(xa, 1.0, 2)
+    lam, U = np.linalg.eigh(r2["H"])
+    assert lam[0] > -1e-12 * lam[-1]
 
 
 def test_generator_classifier_matches_oracle(oracle_mod):
