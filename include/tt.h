@@ -67,8 +67,10 @@ typedef enum { TT_F64 = 0, TT_F32 = 1 } tt_dtype;
 /* Treatment of Eq. 4's third part ("might be negative"; reading A7):
  *   TT_HESS_EQ4    all three parts as printed
  *   TT_HESS_FILTER third part kept iff L47's quantity 8 t_c^0 t_c^1 (g0.g1) >= 0   (default)
- *   TT_HESS_PSD2   first two parts only (always positive semi-definite)                          */
-typedef enum { TT_HESS_EQ4 = 0, TT_HESS_FILTER = 1, TT_HESS_PSD2 = 2 } tt_hess_mode;
+ *   TT_HESS_PSD2   first two parts only (always positive semi-definite)
+ *   TT_HESS_PSDPROJ the projection of Eq. 4's per-pair matrix onto the positive semi-definite cone
+ *                  (its negative eigenvalue removed): the closest PSD matrix to the pair's Eq. 4     */
+typedef enum { TT_HESS_EQ4 = 0, TT_HESS_FILTER = 1, TT_HESS_PSD2 = 2, TT_HESS_PSDPROJ = 3 } tt_hess_mode;
 
 typedef struct {
   int32_t dtype;      /* tt_dtype                                                                   */

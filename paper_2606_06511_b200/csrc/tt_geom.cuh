@@ -215,10 +215,47 @@ __device__ __forceinline__ void pair_derivs_recorded(const d3 ak, const d3 ap, c
 
 // Step a3, second half: Eq. 3 and Eq. 4 coefficients.  keep = tt_hess_mode's treatment of the
 // third part (L47): EQ4 -> 1, PSD2 -> 0, FILTER -> [8 tc0 tc1 (g0.g1) >= 0].
+// PSDPROJ (mode 3): H = J^T M J has rank 2, so its projection onto the PSD cone is J^T M+ J with a
+// 2x2 M+ in closed form.  With G = J J^T = L L^T (Cholesky), Q = L^-1 J has orthonormal rows and
+// H = Q^T S Q, S = L^T M L; det M = -12 tc0^2 tc1^2 < 0 makes S indefinite for every active pair, so
+// S+ = lambda_+ (S - lambda_- I) / (lambda_+ - lambda_-) (spectral projector of the positive
+// eigenvalue) and M+ = L^-T S+ L^-1.  The coefficients (c00, c11, c01) become the entries of M+ and
+// everything downstream is unchanged.  (The oracle projects the dense 18x18 matrix instead.)
 struct Coefs {
   double cg0, cg1;       // Eq. 3: grad = cg0 g0 + cg1 g1
   double c00, c11, c01;  // Eq. 4: H = c00 g0g0^T + c11 g1g1^T + c01 (g1g0^T + g0g1^T)
 };
+// PSDPROJ's 2x2 algebra, kept out of line (scalars in, scalars out): the three default modes then
+// compile as without it -- K4 runs at ~254 of 255 registers and is sensitive to every live value.
+// G = J J^T = [[p, q], [q, r]], M = [[a, b], [b, d]]; returns M+ as (m00, m11, m01).
+struct Sym2 {
+  double m00, m11, m01;
+};
+__device__ __noinline__ Sym2 psd_project_2x2(double p, double q, double r, double a, double b, double d) {
+  Sym2 o{a, d, 0.0};  // fallback (g0 parallel to g1: cannot happen away from degenerate pairs): PSD2
+  const double l11 = sqrt(p), l21 = q / l11;
+  const double l22sq = r - l21 * l21;
+  if (l22sq > 1e-24 * r) {
+    const double l22 = sqrt(l22sq);
+    // S = L^T M L
+    const double t1 = a * l11 + b * l21, t2 = b * l11 + d * l21;
+    const double s11 = l11 * t1 + l21 * t2, s12 = l22 * t2, s22 = l22 * l22 * d;
+    const double mid = 0.5 * (s11 + s22), half = 0.5 * (s11 - s22);
+    const double rad = sqrt(fma(half, half, s12 * s12));
+    const double lp = mid + rad, lm = mid - rad;
+    const double f = (lp > 0.0) ? lp / (lp - lm) : 0.0;  // S+ = f (S - lm I)
+    const double p11 = f * (s11 - lm), p12 = f * s12, p22 = f * (s22 - lm);
+    // M+ = L^-T S+ L^-1,  L^-1 = [[1/l11, 0], [-l21/(l11 l22), 1/l22]]
+    const double i11 = 1.0 / l11, i22 = 1.0 / l22, i21 = -l21 * i11 * i22;
+    const double u1 = p11 * i11 + p12 * i21, u2 = p12 * i11 + p22 * i21;  // (S+ L^-1)[:, 0]
+    o.m00 = i11 * u1 + i21 * u2;
+    o.m01 = i22 * u2;
+    o.m11 = i22 * i22 * p22;
+  }
+  return o;
+}
+
+template <bool PROJ = true>  // PROJ = false: TT_HESS_PSDPROJ compiled out (K4's default instantiation)
 __device__ __forceinline__ Coefs pair_coefs(double tc0, double tc1, const double (&g0)[18],
                                             const double (&g1)[18], int hess_mode) {
   Coefs c;
@@ -236,6 +273,19 @@ __device__ __forceinline__ Coefs pair_coefs(double tc0, double tc1, const double
     keep = 0.0;
   }
   c.c01 = 4.0 * tc0 * tc1 * keep;
+  if (PROJ && hess_mode == 3) {
+    double p = 0.0, q = 0.0, r = 0.0;
+#pragma unroll
+    for (int i = 0; i < 18; ++i) {
+      p = fma(g0[i], g0[i], p);
+      q = fma(g0[i], g1[i], q);
+      r = fma(g1[i], g1[i], r);
+    }
+    const Sym2 m = psd_project_2x2(p, q, r, c.c00, c.c01, c.c11);
+    c.c00 = m.m00;
+    c.c11 = m.m11;
+    c.c01 = m.m01;
+  }
   return c;
 }
 

@@ -802,6 +802,7 @@ __device__ __forceinline__ void load_pos18(const T* __restrict__ pos, const int 
 
 // J by the straight-line code on gathered positions x = [a_k, a_p, a_q, b_k, b_p, b_q] (raw),
 // coefficients, energy; swaps halves so that "own" is first.
+template <bool PROJ = true>
 __device__ __forceinline__ void eval_core(const double (&x)[18], unsigned pay, double sigma, int hess_mode, Entry& E) {
   const bool side = (pay & 1u) != 0u;
   const unsigned ca = (pay >> 1) & 63u, cb = (pay >> 7) & 63u;
@@ -815,7 +816,7 @@ __device__ __forceinline__ void eval_core(const double (&x)[18], unsigned pay, d
   const d3 bk = ttg::mk(x[9], x[10], x[11]) - o, bp = ttg::mk(x[12], x[13], x[14]) - o, bq = ttg::mk(x[15], x[16], x[17]) - o;
   double tc0, tc1;
   ttg::pair_derivs_recorded(ak, ap, aq, bk, bp, bq, sigma, ca >> 4, cb >> 4, tc0, tc1, E.g0, E.g1);
-  E.cf = ttg::pair_coefs(tc0, tc1, E.g0, E.g1, hess_mode);
+  E.cf = ttg::pair_coefs<PROJ>(tc0, tc1, E.g0, E.g1, hess_mode);
   const double tt = tc0 * tc1;
   E.en = side ? 0.0 : tt * tt;  // Eq. 2, counted once per pair
 #pragma unroll
@@ -973,7 +974,7 @@ __device__ __forceinline__ void load_round_ops(const AsmParams<T>& P, const int4
   }
 }
 
-template <typename T>
+template <typename T, bool PROJ>  // PROJ: TT_HESS_PSDPROJ compiled in (the other modes run the leaner instantiation)
 __global__ void __maxnreg__(TT_TILE_MAXNREG)
 k_assemble_tile(const AsmParams<T> P) {
   extern __shared__ __align__(16) unsigned char s_raw[];
@@ -1022,7 +1023,7 @@ k_assemble_tile(const AsmParams<T> P) {
     E.cf = {0, 0, 0, 0, 0};
     E.en = 0.0;
     int er[3] = {cur.er[0], cur.er[1], cur.er[2]};
-    if (valid) eval_core(x, cur.pay, P.sigma, P.hess_mode, E);
+    if (valid) eval_core<PROJ>(x, cur.pay, P.sigma, P.hess_mode, E);
     // ---- operands of round c + G, vertex ids of c + 2G, descriptor of c + 3G: requested after the
     //      register peak of the derivative code, consumed a round later ----
     RoundOps nxt;

@@ -17,7 +17,7 @@ LIB_PATH = _HERE / "libtt.so"
 
 TT_OK = 0
 TT_F64, TT_F32 = 0, 1
-TT_HESS_EQ4, TT_HESS_FILTER, TT_HESS_PSD2 = 0, 1, 2
+TT_HESS_EQ4, TT_HESS_FILTER, TT_HESS_PSD2, TT_HESS_PSDPROJ = 0, 1, 2, 3
 TT_FLAG_FORCE_GENERAL_ROWS = 1
 
 EXPORTS = ["tt_create", "tt_destroy", "tt_energy", "tt_hess_symbolic", "tt_energy_grad_hess", "tt_hess_vec",

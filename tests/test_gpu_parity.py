@@ -95,7 +95,7 @@ def run_case(oracle, pb, dtype="f64", hess_mode=1, sigma=1.0, flags=0, check_val
 
 
 # ------------------------------------------------------------------------------------ configs
-@pytest.mark.parametrize("mode", [0, 1, 2])
+@pytest.mark.parametrize("mode", [0, 1, 2, 3])
 @pytest.mark.parametrize("dtype", ["f64", "f32"])
 def test_config0_soup(oracle_mod, mode, dtype):
     from paper_2606_06511_b200 import inputs
@@ -122,6 +122,26 @@ def test_config0_forced_general_rows_equal_exclusive(oracle_mod):
     assert sa["blocks_merged"] == 0 and sb["blocks_direct"] == 0
     assert torch.equal(a["colind"], b["colind"]) and torch.equal(a["rowptr"], b["rowptr"])
     assert rel(a["vals"].cpu().numpy(), b["vals"].cpu().numpy()) < 1e-14
+
+
+def test_psd_projection_mode_meshes(oracle_mod):
+    """hess_mode 3 (PSD projection, closed 2x2 form on the GPU vs dense Jacobi in the oracle) on shared
+    vertices (general rows) and on the icospheres; the assembled matrix is PSD on a small case."""
+    from paper_2606_06511_b200 import inputs
+    ref, out, st = run_case(oracle_mod, inputs.config0_soup(n_tris=48, pool=40, seed=5), "f64", 3)
+    assert st["blocks_merged"] > 0
+    run_case(oracle_mod, inputs.config1_icospheres(), "f64", 3)
+    pb = inputs.config0_soup(n_tris=24, seed=9)
+    ref, out, st = run_case(oracle_mod, pb, "f64", 3)
+    nV = pb.n_verts
+    H = np.zeros((3 * nV, 3 * nV))
+    rp, ci, va = out["rowptr"].cpu().numpy(), out["colind"].cpu().numpy(), out["vals"].cpu().numpy()
+    for r in range(nV):
+        for e in range(rp[r], rp[r + 1]):
+            H[3 * r:3 * r + 3, 3 * ci[e]:3 * ci[e] + 3] = va[e]
+    w = np.linalg.eigvalsh(0.5 * (H + H.T))
+    assert w[0] > -1e-9 * w[-1]
+    assert np.abs(H - H.T).max() <= 1e-9 * np.abs(H).max()
 
 
 def test_sigma_half(oracle_mod):
