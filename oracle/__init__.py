@@ -60,6 +60,8 @@ def _load():
         lib.tt_oracle_hess_vec_pairs.restype = None
         lib.tt_oracle_bsr_matvec.argtypes = [i64, c_ip, c_ip, c_dp, c_dp, c_dp]
         lib.tt_oracle_bsr_matvec.restype = None
+        lib.tt_oracle_broad_phase.argtypes = [c_dp, c_ip, i64, ctypes.c_double, c_ip, i64]
+        lib.tt_oracle_broad_phase.restype = i64
         lib.tt_oracle_max_threads.argtypes = []
         lib.tt_oracle_max_threads.restype = ctypes.c_int
         _lib = lib
@@ -164,6 +166,18 @@ def hess_vec_pairs(nV, tris, pair_ids, active, tc, J, p, hess_mode: int = HESS_F
                                  _bp(np.ascontiguousarray(active, dtype=np.uint8)), _dp(_f64(tc)),
                                  _dp(_f64(J)), int(hess_mode), _dp(p), _dp(y))
     return y
+
+
+def broad_phase(pos, tris, inflate: float = 0.0):
+    """All non-adjacent triangle pairs i < j whose inflated AABBs overlap, lexicographic, by testing
+    every pair.  Returns int32 [n,2]."""
+    lib = _load()
+    pos = _f64(pos)
+    tris = _i32(tris)
+    n = lib.tt_oracle_broad_phase(_dp(pos), _ip(tris), tris.shape[0], float(inflate), None, 0)
+    out = np.zeros((max(int(n), 1), 2), dtype=np.int32)
+    lib.tt_oracle_broad_phase(_dp(pos), _ip(tris), tris.shape[0], float(inflate), _ip(out), int(n))
+    return out[:int(n)]
 
 
 def bsr_matvec(rowptr, colind, vals, p):

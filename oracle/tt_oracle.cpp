@@ -516,6 +516,48 @@ void tt_oracle_bsr_matvec(int64_t n_verts, const int32_t* rowptr, const int32_t*
   }
 }
 
+// Broad phase (PAPER.md L51 names spatial hashing [Pabst et al. 2010] and gives
+// no detail, so the operation is defined by its RESULT): all pairs i < j of triangles that share no
+// vertex index and whose axis-aligned bounding boxes, each grown by `inflate` on every side, overlap
+// (closed intervals), in lexicographic order.  Written out as that definition: every pair is tested.
+// Pass pairs = NULL to count; returns the number of pairs (written only up to `capacity`).
+int64_t tt_oracle_broad_phase(const double* pos, const int32_t* tris, int64_t n_tris, double inflate,
+                              int32_t* pairs, int64_t capacity) {
+  std::vector<double> lo(3 * (size_t)n_tris), hi(3 * (size_t)n_tris);
+  for (int64_t t = 0; t < n_tris; ++t)
+    for (int c = 0; c < 3; ++c) {
+      double a = pos[3 * (int64_t)tris[3 * t] + c], b = pos[3 * (int64_t)tris[3 * t + 1] + c],
+             d = pos[3 * (int64_t)tris[3 * t + 2] + c];
+      lo[3 * t + c] = std::min(a, std::min(b, d)) - inflate;
+      hi[3 * t + c] = std::max(a, std::max(b, d)) + inflate;
+    }
+  std::vector<int64_t> cnt((size_t)n_tris + 1, 0);
+  for (int pass = 0; pass < 2; ++pass) {
+#pragma omp parallel for schedule(dynamic, 64)
+    for (int64_t i = 0; i < n_tris; ++i) {
+      int64_t k = pass ? cnt[i] : 0;
+      for (int64_t j = i + 1; j < n_tris; ++j) {
+        bool ov = true;
+        for (int c = 0; c < 3; ++c) ov = ov && lo[3 * i + c] <= hi[3 * j + c] && lo[3 * j + c] <= hi[3 * i + c];
+        if (!ov || share_vertex(tris + 3 * i, tris + 3 * j)) continue;
+        if (pass) {
+          if (k < capacity) {
+            pairs[2 * k] = (int32_t)i;
+            pairs[2 * k + 1] = (int32_t)j;
+          }
+        }
+        ++k;
+      }
+      if (!pass) cnt[i + 1] = k;
+    }
+    if (!pass) {
+      for (int64_t i = 0; i < n_tris; ++i) cnt[i + 1] += cnt[i];  // cnt[i] = first output slot of row i
+      if (!pairs) break;
+    }
+  }
+  return cnt[n_tris];
+}
+
 int tt_oracle_max_threads(void) {
 #ifdef _OPENMP
   return omp_get_max_threads();

@@ -419,6 +419,41 @@ def test_psd_projection_mode(oracle_mod):
     assert lam[0] > -1e-12 * lam[-1]
 
 
+def test_broad_phase_oracle(oracle_mod):
+    """NEXT-1: candidate pairs = non-adjacent triangle pairs whose inflated AABBs overlap.
+    Pins: hand cases (overlap, touching boxes are closed intervals, a gap closes exactly when
+    2 * inflate reaches it, shared-vertex pairs dropped), lexicographic uniqueness, and agreement
+    with the generators' uniform-grid routine (a different algorithm) on a mesh and a soup."""
+    from paper_2606_06511_b200 import inputs
+    tri = np.array([[0, 0, 0], [1, 0, 0], [0, 1, 0]], dtype=np.float64)
+    def two(shift, inflate, share=False):
+        pos = np.concatenate([tri, tri + np.asarray(shift, dtype=np.float64)])
+        tris = np.array([[0, 1, 2], [3, 4, 5]], dtype=np.int32)
+        if share:
+            tris[1, 0] = 0
+        return oracle_mod.broad_phase(pos, tris, inflate)
+    assert two((0.5, 0.5, 0.0), 0.0).tolist() == [[0, 1]]
+    assert two((1.0, 0.0, 0.0), 0.0).tolist() == [[0, 1]]            # boxes touch: closed intervals
+    assert two((1.5, 0.0, 0.0), 0.0).shape[0] == 0                   # gap 0.5
+    assert two((1.5, 0.0, 0.0), 0.2).shape[0] == 0                   # 2 * 0.2 < 0.5
+    assert two((1.5, 0.0, 0.0), 0.25).tolist() == [[0, 1]]           # 2 * 0.25 = 0.5 (exact in binary)
+    assert two((0.0, 0.0, 3.0), 0.0).shape[0] == 0                   # separated along z only
+    assert two((0.5, 0.5, 0.0), 0.0, share=True).shape[0] == 0       # shares vertex 0: adjacent
+    rng = np.random.default_rng(8)
+    soup_pos = rng.uniform(0, 1, (1500, 3)) * np.array([1.0, 1.0, 0.2])
+    soup_pos[1::3] = soup_pos[0::3] + rng.normal(0, 0.03, (500, 3))
+    soup_pos[2::3] = soup_pos[0::3] + rng.normal(0, 0.03, (500, 3))
+    soup_tris = np.arange(1500, dtype=np.int32).reshape(500, 3)
+    ico = inputs.config1_icospheres(subdiv=3)
+    for pos, tris, inflate in ((soup_pos, soup_tris, 0.0), (soup_pos, soup_tris, 0.01), (ico.pos, ico.tris, 0.02)):
+        pr = oracle_mod.broad_phase(pos, tris, inflate)
+        key = pr[:, 0].astype(np.int64) * tris.shape[0] + pr[:, 1]
+        assert (pr[:, 0] < pr[:, 1]).all() and (np.diff(key) > 0).all()
+        ref = inputs.aabb_candidates(pos, tris, inflate)
+        assert pr.shape == ref.shape and (pr == ref).all()
+        assert pr.shape[0] > 100
+
+
 def test_generator_classifier_matches_oracle(oracle_mod):
     """The generators' orientation classifier (workload shaping only) agrees with the oracle's
     Moeller predicate, and the degeneracy filter keeps |tc| >= 1e-6 * edge (north_star)."""
