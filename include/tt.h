@@ -140,6 +140,23 @@ tt_status tt_energy_grad_hess_host(tt_ctx* ctx, const tt_problem* prob, void* en
                                    int64_t nnzb_capacity, const void* p_host, void* y_host,
                                    void* stream);
 
+/* Broad phase ("we use spatial hashing structure [Pabst et al. 2010] to eliminate
+ * redundant computations").  The paper gives no detail, so the operation is
+ * defined by its result: ALL pairs i < j of triangles that share no vertex index and whose
+ * axis-aligned bounding boxes, each grown by `inflate` (>= 0) on every side, overlap (closed
+ * intervals; bounds in fp64 from the stored positions), in lexicographic order -- i.e. a `pairs`
+ * array for tt_problem.  Built on a uniform grid (cell = largest box extent), sort based, no atomics;
+ * the result is deterministic and independent of the grid.
+ *   pos [nV,3] dtype, tris [nT,3] int32: DEVICE, read only.   n_pairs_host HOST [1].
+ * The pairs stay in ctx (device memory owned by ctx, valid until the next tt_broad_phase or
+ * tt_destroy): tt_broad_phase_pairs returns the view, tt_broad_phase_copy copies them to a caller
+ * array [capacity,2] (TT_ERR_CAPACITY if too small).  tt_broad_phase blocks until the count is known
+ * (two host round trips on `stream`); TT_ERR_INVALID_ARG if the count reaches 2^30.               */
+tt_status tt_broad_phase(tt_ctx* ctx, const void* pos, int64_t n_verts, const int32_t* tris,
+                         int64_t n_tris, double inflate, int64_t* n_pairs_host, void* stream);
+tt_status tt_broad_phase_pairs(tt_ctx* ctx, const int32_t** pairs, int64_t* n_pairs);
+tt_status tt_broad_phase_copy(tt_ctx* ctx, int32_t* pairs_out, int64_t capacity, void* stream);
+
 /* Device views of the BSR produced by the last tt_energy_grad_hess_host (owned by ctx, valid
  * until the next *_host call or tt_destroy).                                                      */
 tt_status tt_bsr_device(tt_ctx* ctx, const int32_t** rowptr, const int32_t** colind,

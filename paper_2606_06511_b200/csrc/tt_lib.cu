@@ -10,6 +10,7 @@
 #include <cub/cub.cuh>
 
 #include "../../include/tt.h"
+#include "tt_broad.cuh"
 #include "tt_kernels.cuh"
 #include "tt_probe.cuh"
 
@@ -73,6 +74,9 @@ struct tt_ctx {
   // numeric
   DevBuf everts, rdesc, tfirst, bucket_cnt, bucket_off, long_cnt, long_off, chunk_start, long_list, asm_energy, tvals, tslot, vkeys[2], vvals[2], vptr, vslot1;
   DevBuf cub_tmp;
+  // broad phase (tt_broad_phase): boxes, grid, (cell, triangle) records, pair keys, result
+  DevBuf bp_box, bp_part, bp_grid, bp_cnt, bp_off, bp_keys[2], bp_vals[2], bp_pcnt, bp_poff, bp_pkeys[2], bp_pairs;
+  int64_t bp_n_pairs = -1;
   // host-API mirrors
   DevBuf h_pos, h_tris, h_pairs, h_p, o_vals, o_grad, o_energy, o_y;
   // cached symbolic state
@@ -626,6 +630,89 @@ tt_status hessvec_impl(tt_ctx* ctx, const tt_problem* q, const void* pvec, void*
   return TT_OK;
 }
 
+// ---- broad phase (tt_broad.cuh) ------------------------------------------------------------------
+template <typename T>
+tt_status broad_impl(tt_ctx* ctx, const void* pos, int64_t nV, const int32_t* tris, int64_t nT, double inflate,
+                     int64_t* n_pairs_host, cudaStream_t st) {
+  using namespace ttb;
+  (void)nV;
+  ctx->bp_n_pairs = -1;
+  *n_pairs_host = 0;
+  if (nT < 2) {
+    ctx->bp_n_pairs = 0;
+    return TT_OK;
+  }
+  const unsigned gridT = grid_for(nT, BP_THREADS);
+  TT_CUDA(ctx->bp_box.ensure(sizeof(double) * 6 * (size_t)nT));
+  TT_CUDA(ctx->bp_part.ensure(sizeof(double) * 7 * (size_t)gridT));
+  TT_CUDA(ctx->bp_grid.ensure(sizeof(Grid)));
+  TT_CUDA(ctx->bp_cnt.ensure(sizeof(int) * (size_t)(nT + 1)));
+  TT_CUDA(ctx->bp_off.ensure(sizeof(int) * (size_t)(nT + 1)));
+  k_bp_aabb<T><<<gridT, BP_THREADS, 0, st>>>((const T*)pos, tris, nT, inflate, ctx->bp_box.as<double>(), ctx->bp_part.as<double>());
+  TT_LAUNCH_CHECK();
+  k_bp_grid<<<1, BP_THREADS, 0, st>>>(ctx->bp_part.as<double>(), (int64_t)gridT, ctx->bp_grid.as<Grid>());
+  TT_LAUNCH_CHECK();
+  k_bp_cells<false><<<gridT, BP_THREADS, 0, st>>>(ctx->bp_box.as<double>(), nT, ctx->bp_grid.as<Grid>(), ctx->bp_cnt.as<int>(),
+                                                  nullptr, nullptr, nullptr);
+  TT_LAUNCH_CHECK();
+  TT_CUDA(cudaMemsetAsync(ctx->bp_cnt.as<int>() + nT, 0, sizeof(int), st));
+  tt_status s = scan_i32(ctx, ctx->bp_cnt.as<int>(), ctx->bp_off.as<int>(), nT + 1, st);
+  if (s != TT_OK) return s;
+  int n_rec32 = 0;
+  Grid g;
+  TT_CUDA(cudaMemcpyAsync(&n_rec32, ctx->bp_off.as<int>() + nT, sizeof(int), cudaMemcpyDeviceToHost, st));
+  TT_CUDA(cudaMemcpyAsync(&g, ctx->bp_grid.p, sizeof(Grid), cudaMemcpyDeviceToHost, st));
+  TT_CUDA(cudaStreamSynchronize(st));
+  const int64_t n_rec = n_rec32;
+  const double n_cells = (double)g.dims[0] * (double)g.dims[1] * (double)g.dims[2];
+  if (n_cells >= 9.0e18) return fail(ctx, TT_ERR_INVALID_ARG, "broad phase: grid of %d x %d x %d cells exceeds 63-bit keys", g.dims[0], g.dims[1], g.dims[2]);
+  int cell_bits = 1;
+  while (cell_bits < 63 && (double)(1ull << cell_bits) < n_cells) ++cell_bits;
+  for (int i = 0; i < 2; ++i) {
+    TT_CUDA(ctx->bp_keys[i].ensure(sizeof(uint64_t) * (size_t)(n_rec + 1)));
+    TT_CUDA(ctx->bp_vals[i].ensure(sizeof(uint32_t) * (size_t)(n_rec + 1)));
+  }
+  k_bp_cells<true><<<gridT, BP_THREADS, 0, st>>>(ctx->bp_box.as<double>(), nT, ctx->bp_grid.as<Grid>(), nullptr,
+                                                 ctx->bp_off.as<int>(), ctx->bp_keys[0].as<uint64_t>(), ctx->bp_vals[0].as<uint32_t>());
+  TT_LAUNCH_CHECK();
+  uint64_t* keys = nullptr;
+  uint32_t* vals = nullptr;
+  s = sort_pairs(ctx, ctx->bp_keys, ctx->bp_vals, n_rec, 0, cell_bits, &keys, &vals, st);
+  if (s != TT_OK) return s;
+  TT_CUDA(ctx->bp_pcnt.ensure(sizeof(int) * (size_t)(n_rec + 1)));
+  TT_CUDA(ctx->bp_poff.ensure(sizeof(int64_t) * (size_t)(n_rec + 1)));
+  const unsigned gridR = grid_for(n_rec, BP_THREADS);
+  k_bp_pairs<false><<<gridR, BP_THREADS, 0, st>>>(keys, vals, n_rec, ctx->bp_box.as<double>(), tris, nT, ctx->bp_grid.as<Grid>(),
+                                                  ctx->bp_pcnt.as<int>(), nullptr, nullptr);
+  TT_LAUNCH_CHECK();
+  TT_CUDA(cudaMemsetAsync(ctx->bp_pcnt.as<int>() + n_rec, 0, sizeof(int), st));
+  s = scan_i32_to_i64(ctx, ctx->bp_pcnt.as<int>(), ctx->bp_poff.as<int64_t>(), n_rec + 1, st);
+  if (s != TT_OK) return s;
+  int64_t P = 0;
+  TT_CUDA(cudaMemcpyAsync(&P, ctx->bp_poff.as<int64_t>() + n_rec, sizeof(int64_t), cudaMemcpyDeviceToHost, st));
+  TT_CUDA(cudaStreamSynchronize(st));
+  if (P >= (int64_t(1) << 30)) return fail(ctx, TT_ERR_INVALID_ARG, "broad phase: %lld candidate pairs exceed the 2^30 limit of tt_problem", (long long)P);
+  for (int i = 0; i < 2; ++i) TT_CUDA(ctx->bp_pkeys[i].ensure(sizeof(uint64_t) * (size_t)(P + 1)));
+  TT_CUDA(ctx->bp_pairs.ensure(sizeof(int2) * (size_t)(P + 1)));
+  if (P > 0) {
+    k_bp_pairs<true><<<gridR, BP_THREADS, 0, st>>>(keys, vals, n_rec, ctx->bp_box.as<double>(), tris, nT, ctx->bp_grid.as<Grid>(),
+                                                   nullptr, ctx->bp_poff.as<int64_t>(), ctx->bp_pkeys[0].as<uint64_t>());
+    TT_LAUNCH_CHECK();
+    cub::DoubleBuffer<uint64_t> dk(ctx->bp_pkeys[0].as<uint64_t>(), ctx->bp_pkeys[1].as<uint64_t>());
+    const int bits = 2 * ceil_log2(nT > 1 ? nT : 2);
+    size_t tmp = 0;
+    TT_CUDA(cub::DeviceRadixSort::SortKeys(nullptr, tmp, dk, P, 0, bits, st));
+    TT_CUDA(ctx->cub_tmp.ensure(tmp));
+    TT_CUDA(cub::DeviceRadixSort::SortKeys(ctx->cub_tmp.p, tmp, dk, P, 0, bits, st));
+    ctx->launches += 2 + (bits + 7) / 8;
+    k_bp_unpack<<<grid_for(P, 256), 256, 0, st>>>(dk.Current(), P, nT, ctx->bp_pairs.as<int2>());
+    TT_LAUNCH_CHECK();
+  }
+  ctx->bp_n_pairs = P;
+  *n_pairs_host = P;
+  return TT_OK;
+}
+
 }  // namespace
 
 // =================================================================================== C ABI
@@ -823,6 +910,41 @@ tt_status tt_energy_grad_hess_host(tt_ctx* ctx, const tt_problem* prob, void* en
   }
   TT_CUDA(cudaStreamWaitEvent(st, ctx->ev_side, 0));  // `stream` completes only after the side copies
   TT_CUDA(cudaStreamSynchronize(st));
+  return TT_OK;
+}
+
+tt_status tt_broad_phase(tt_ctx* ctx, const void* pos, int64_t n_verts, const int32_t* tris, int64_t n_tris,
+                         double inflate, int64_t* n_pairs_host, void* stream) {
+  if (!ctx) return TT_ERR_INVALID_ARG;
+  if (!n_pairs_host) return fail(ctx, TT_ERR_INVALID_ARG, "n_pairs_host is NULL");
+  if (n_verts < 0 || n_tris < 0 || !(inflate >= 0.0)) return fail(ctx, TT_ERR_INVALID_ARG, "negative size or inflate");
+  if (n_verts >= (int64_t(1) << 31) / 3 || n_tris >= (int64_t(1) << 31) / 8)
+    return fail(ctx, TT_ERR_INVALID_ARG, "sizes exceed int32 indexing (nV < 2^31/3, nT < 2^31/8)");
+  if ((n_verts > 0 && !pos) || (n_tris > 0 && !tris)) return fail(ctx, TT_ERR_INVALID_ARG, "NULL array with non-zero size");
+  TT_CUDA(cudaSetDevice(ctx->opt.device));
+  cudaStream_t st = (cudaStream_t)stream;
+  return ctx->opt.dtype == TT_F64 ? broad_impl<double>(ctx, pos, n_verts, tris, n_tris, inflate, n_pairs_host, st)
+                                  : broad_impl<float>(ctx, pos, n_verts, tris, n_tris, inflate, n_pairs_host, st);
+}
+
+tt_status tt_broad_phase_pairs(tt_ctx* ctx, const int32_t** pairs, int64_t* n_pairs) {
+  if (!ctx) return TT_ERR_INVALID_ARG;
+  if (ctx->bp_n_pairs < 0) return fail(ctx, TT_ERR_STATE, "tt_broad_phase_pairs: no tt_broad_phase result");
+  if (pairs) *pairs = ctx->bp_pairs.as<int32_t>();
+  if (n_pairs) *n_pairs = ctx->bp_n_pairs;
+  return TT_OK;
+}
+
+tt_status tt_broad_phase_copy(tt_ctx* ctx, int32_t* pairs_out, int64_t capacity, void* stream) {
+  if (!ctx) return TT_ERR_INVALID_ARG;
+  if (ctx->bp_n_pairs < 0) return fail(ctx, TT_ERR_STATE, "tt_broad_phase_copy: no tt_broad_phase result");
+  if (capacity < ctx->bp_n_pairs) return fail(ctx, TT_ERR_CAPACITY, "capacity %lld < %lld pairs", (long long)capacity, (long long)ctx->bp_n_pairs);
+  if (ctx->bp_n_pairs > 0) {
+    if (!pairs_out) return fail(ctx, TT_ERR_INVALID_ARG, "pairs_out is NULL");
+    TT_CUDA(cudaSetDevice(ctx->opt.device));
+    TT_CUDA(cudaMemcpyAsync(pairs_out, ctx->bp_pairs.p, sizeof(int32_t) * 2 * (size_t)ctx->bp_n_pairs, cudaMemcpyDeviceToDevice,
+                            (cudaStream_t)stream));
+  }
   return TT_OK;
 }
 

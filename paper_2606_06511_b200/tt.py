@@ -21,7 +21,7 @@ TT_HESS_EQ4, TT_HESS_FILTER, TT_HESS_PSD2, TT_HESS_PSDPROJ = 0, 1, 2, 3
 TT_FLAG_FORCE_GENERAL_ROWS = 1
 
 EXPORTS = ["tt_create", "tt_destroy", "tt_energy", "tt_hess_symbolic", "tt_energy_grad_hess", "tt_hess_vec",
-           "tt_energy_grad_hess_host", "tt_bsr_device", "tt_stats", "tt_kernel_ms", "tt_probe_peaks", "tt_status_string", "tt_last_error"]
+           "tt_energy_grad_hess_host", "tt_broad_phase", "tt_broad_phase_pairs", "tt_broad_phase_copy", "tt_bsr_device", "tt_stats", "tt_kernel_ms", "tt_probe_peaks", "tt_status_string", "tt_last_error"]
 
 
 class TTOptions(ctypes.Structure):
@@ -68,6 +68,12 @@ def load_library():
     lib.tt_energy_grad_hess_host.argtypes = [vp, ctypes.POINTER(TTProblem), vp, vp, ctypes.POINTER(i64),
                                              ctypes.POINTER(i64), vp, vp, vp, i64, vp, vp, vp]
     lib.tt_energy_grad_hess_host.restype = ctypes.c_int
+    lib.tt_broad_phase.argtypes = [vp, vp, i64, vp, i64, ctypes.c_double, ctypes.POINTER(i64), vp]
+    lib.tt_broad_phase.restype = ctypes.c_int
+    lib.tt_broad_phase_pairs.argtypes = [vp, ctypes.POINTER(vp), ctypes.POINTER(i64)]
+    lib.tt_broad_phase_pairs.restype = ctypes.c_int
+    lib.tt_broad_phase_copy.argtypes = [vp, vp, i64, vp]
+    lib.tt_broad_phase_copy.restype = ctypes.c_int
     lib.tt_bsr_device.argtypes = [vp, ctypes.POINTER(vp), ctypes.POINTER(vp), ctypes.POINTER(vp), ctypes.POINTER(i64)]
     lib.tt_bsr_device.restype = ctypes.c_int
     lib.tt_stats.argtypes = [vp, ctypes.POINTER(i64), ctypes.c_int32]
@@ -170,6 +176,18 @@ class Context:
                                                       _ptr(colind_h), _ptr(vals_h), int(nnzb_capacity),
                                                       _ptr(p_h), _ptr(y_h), _stream_ptr(stream)))
         return nnzb.value, na.value
+
+    def tt_broad_phase(self, pos, tris, inflate=0.0, stream=None):
+        """Candidate pairs of (pos, tris): returns a new int32 [P,2] device tensor (tt_broad_phase +
+        tt_broad_phase_copy)."""
+        n = ctypes.c_int64(0)
+        sp = _stream_ptr(stream)
+        assert pos.dtype == self.dtype and tris.dtype == torch.int32 and pos.is_contiguous() and tris.is_contiguous()
+        self._check(self.lib.tt_broad_phase(self.h, _ptr(pos), pos.shape[0], _ptr(tris), tris.shape[0], float(inflate),
+                                            ctypes.byref(n), sp))
+        out = torch.empty((int(n.value), 2), dtype=torch.int32, device=pos.device)
+        self._check(self.lib.tt_broad_phase_copy(self.h, _ptr(out) if n.value else None, int(n.value), sp))
+        return out
 
     def tt_kernel_ms(self):
         arr = (ctypes.c_float * 3)()
