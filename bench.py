@@ -47,6 +47,8 @@ def parse():
     ap.add_argument("--tris", type=int, default=2_000_000)
     ap.add_argument("--dtype", default="f64", choices=["f64", "f32"])
     ap.add_argument("--hess-mode", type=int, default=1)
+    ap.add_argument("--broad-phase", default=None, choices=["config2", "config3"],
+                    help="time tt_broad_phase (SURVEY 8(f) NEXT-1) on that mesh instead of the hot path; prints its own JSON line")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     return ap.parse_args()
@@ -189,10 +191,52 @@ def run_reference(args):
     print(json.dumps(out), flush=True)
 
 
+def run_broad_phase(args):
+    """Side measurement, not the headline: tt_broad_phase on a mesh config (inputs resident, CUDA events)."""
+    import torch
+    from paper_2606_06511_b200 import inputs, tt
+    dev = torch.device("cuda", 0)
+    if args.broad_phase == "config2":
+        pb, inflate = inputs.config2_cloth(), 0.002
+        pos_np, tris_np = pb.pos, pb.tris
+    else:   # the torus mesh without the generator's own (CPU) candidate search
+        saved = inputs.aabb_candidates
+        inputs.aabb_candidates = lambda pos, tris, inflate=0.0, max_pairs=None: np.zeros((0, 2), dtype=np.int32)
+        try:
+            pb = inputs.config3_torus()
+        finally:
+            inputs.aabb_candidates = saved
+        pos_np, tris_np, inflate = pb.pos, pb.tris, 0.0
+    ctx = tt.Context(torch.float64, 1, 1.0, 0)
+    pos = torch.from_numpy(pos_np).to(dev)
+    tris = torch.from_numpy(tris_np).to(dev)
+    stream = torch.cuda.current_stream()
+    for _ in range(args.warmup):
+        out = ctx.tt_broad_phase(pos, tris, inflate)
+    torch.cuda.synchronize()
+    ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    ev0.record(stream)
+    for _ in range(args.steps):
+        out = ctx.tt_broad_phase(pos, tris, inflate)
+    ev1.record(stream)
+    torch.cuda.synchronize()
+    ms = ev0.elapsed_time(ev1) / args.steps
+    n = int(out.shape[0])
+    print(json.dumps({"metric": "broad phase: candidate pairs/s (tt_broad_phase, fp64 boxes)", "value": n / (ms * 1e-3),
+                      "unit": UNIT, "n_gpus": 1, "steps": args.steps, "warmup": args.warmup, "ms_per_step": ms,
+                      "higher_is_better": True, "dtype": "f64", "data": "synthetic",
+                      "config": {"workload": "%s mesh, %d triangles, inflate %g -> %d candidate pairs" % (
+                          args.broad_phase, tris_np.shape[0], inflate, n)}}), flush=True)
+    ctx.close()
+
+
 def main():
     args = parse()
     if args.impl == "reference":
         run_reference(args)
+        return
+    if args.broad_phase:
+        run_broad_phase(args)
         return
     import torch
     import torch.distributed as dist
