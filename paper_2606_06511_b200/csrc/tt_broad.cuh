@@ -4,10 +4,10 @@
 // axis-aligned bounding boxes, each grown by `inflate` on every side, overlap (closed intervals),
 // in lexicographic order -- the `pairs` array the hot path consumes.
 //
-// Uniform grid with cell = largest box extent (so a box touches at most 2 cells per axis):
+// Uniform grid (cell size: k_bp_grid; a box touches at most 5 cells per axis):
 //   k_bp_aabb      boxes in fp64 + per-CTA partial bounds          (HBM: 3 vertices in, 48 B out)
 //   k_bp_grid      origin, cell size, grid dimensions (one CTA, fixed order)
-//   k_bp_cells     <COUNT / EMIT> (cell key, triangle) records, <= 8 per triangle
+//   k_bp_cells     <COUNT / EMIT> (cell key, triangle) records, <= 125 per triangle (typically 2-4)
 //   CUB radix sort of the records by cell key (stable: triangles ascending inside a cell)
 //   k_bp_pairs     <COUNT / EMIT> one thread per record walks the later records of its cell; a pair is
 //                  reported only in the cell that owns the point max(lo_i, lo_j), which lies in both
@@ -33,10 +33,10 @@ constexpr int BP_THREADS = 256;
 template <typename T>
 __global__ void __launch_bounds__(BP_THREADS)
 k_bp_aabb(const T* __restrict__ pos, const int* __restrict__ tris, int64_t nT, double inflate,
-          double* __restrict__ box /*[nT][6] lo, hi*/, double* __restrict__ part /*[grid][7] min lo, max hi, max extent*/) {
-  __shared__ double s[BP_THREADS / 32][7];
+          double* __restrict__ box /*[nT][6] lo, hi*/, double* __restrict__ part /*[grid][8] min lo, max hi, max extent, sum of extents*/) {
+  __shared__ double s[BP_THREADS / 32][8];
   const int64_t t = (int64_t)blockIdx.x * BP_THREADS + threadIdx.x;
-  double v[7] = {1e300, 1e300, 1e300, -1e300, -1e300, -1e300, 0.0};
+  double v[8] = {1e300, 1e300, 1e300, -1e300, -1e300, -1e300, 0.0, 0.0};
   if (t < nT) {
     double lo[3], hi[3];
 #pragma unroll
@@ -51,42 +51,49 @@ k_bp_aabb(const T* __restrict__ pos, const int* __restrict__ tris, int64_t nT, d
       v[3 + c] = hi[c];
       v[6] = fmax(v[6], hi[c] - lo[c]);
     }
+    v[7] = v[6];  // this triangle's largest extent
   }
 #pragma unroll
-  for (int k = 0; k < 7; ++k)
+  for (int k = 0; k < 8; ++k)
 #pragma unroll
     for (int o = 16; o > 0; o >>= 1) {
       const double u = __shfl_xor_sync(0xffffffffu, v[k], o);
-      v[k] = (k < 3) ? fmin(v[k], u) : fmax(v[k], u);
+      v[k] = (k < 3) ? fmin(v[k], u) : ((k < 7) ? fmax(v[k], u) : v[k] + u);
     }
   const int w = threadIdx.x >> 5, l = threadIdx.x & 31;
   if (l == 0)
 #pragma unroll
-    for (int k = 0; k < 7; ++k) s[w][k] = v[k];
+    for (int k = 0; k < 8; ++k) s[w][k] = v[k];
   __syncthreads();
-  if (threadIdx.x < 7) {
+  if (threadIdx.x < 8) {
     const int k = threadIdx.x;
     double r = s[0][k];
-    for (int i = 1; i < BP_THREADS / 32; ++i) r = (k < 3) ? fmin(r, s[i][k]) : fmax(r, s[i][k]);
-    part[7 * (int64_t)blockIdx.x + k] = r;
+    for (int i = 1; i < BP_THREADS / 32; ++i) r = (k < 3) ? fmin(r, s[i][k]) : ((k < 7) ? fmax(r, s[i][k]) : r + s[i][k]);
+    part[8 * (int64_t)blockIdx.x + k] = r;
   }
 }
 
+// Cell size: never larger than the largest box (then a box touches <= 2 cells per axis), but when a
+// few boxes are much larger than the rest, 2 x the mean extent, floored at a quarter of the largest
+// (a box then touches <= 5 cells per axis, <= 125 in all): the candidate list does not depend on it.
 __global__ void __launch_bounds__(BP_THREADS)
-k_bp_grid(const double* __restrict__ part, int64_t n_part, Grid* __restrict__ g) {
-  __shared__ double s[BP_THREADS][7];
-  double v[7] = {1e300, 1e300, 1e300, -1e300, -1e300, -1e300, 0.0};
+k_bp_grid(const double* __restrict__ part, int64_t n_part, int64_t nT, Grid* __restrict__ g) {
+  __shared__ double s[BP_THREADS][8];
+  double v[8] = {1e300, 1e300, 1e300, -1e300, -1e300, -1e300, 0.0, 0.0};
   for (int64_t i = threadIdx.x; i < n_part; i += BP_THREADS)
 #pragma unroll
-    for (int k = 0; k < 7; ++k) v[k] = (k < 3) ? fmin(v[k], part[7 * i + k]) : fmax(v[k], part[7 * i + k]);
+    for (int k = 0; k < 8; ++k)
+      v[k] = (k < 3) ? fmin(v[k], part[8 * i + k]) : ((k < 7) ? fmax(v[k], part[8 * i + k]) : v[k] + part[8 * i + k]);
 #pragma unroll
-  for (int k = 0; k < 7; ++k) s[threadIdx.x][k] = v[k];
+  for (int k = 0; k < 8; ++k) s[threadIdx.x][k] = v[k];
   __syncthreads();
   if (threadIdx.x == 0) {
     for (int i = 1; i < BP_THREADS; ++i)
 #pragma unroll
-      for (int k = 0; k < 7; ++k) v[k] = (k < 3) ? fmin(v[k], s[i][k]) : fmax(v[k], s[i][k]);
-    const double cell = (v[6] > 0.0) ? v[6] * 1.0001 : 1.0;  // strictly larger than every box extent
+      for (int k = 0; k < 8; ++k) v[k] = (k < 3) ? fmin(v[k], s[i][k]) : ((k < 7) ? fmax(v[k], s[i][k]) : v[k] + s[i][k]);
+    const double big = v[6] * 1.0001, mean = v[7] / (double)(nT > 0 ? nT : 1);
+    double cell = fmin(big, fmax(2.0 * mean, 0.25 * big));
+    if (!(cell > 0.0)) cell = 1.0;
     g->inv_cell = 1.0 / cell;
     for (int c = 0; c < 3; ++c) {
       g->org[c] = v[c];
@@ -104,7 +111,7 @@ __device__ __forceinline__ uint64_t cell_key(const Grid& g, int cx, int cy, int 
   return ((uint64_t)cx * (uint64_t)g.dims[1] + (uint64_t)cy) * (uint64_t)g.dims[2] + (uint64_t)cz;
 }
 
-// COUNT: cnt[t] = cells box t touches (1..8).  EMIT: records at off[t].
+// COUNT: cnt[t] = cells box t touches (1..125).  EMIT: records at off[t].
 template <bool EMIT>
 __global__ void __launch_bounds__(BP_THREADS)
 k_bp_cells(const double* __restrict__ box, int64_t nT, const Grid* __restrict__ gp, int* __restrict__ cnt,
@@ -117,7 +124,6 @@ k_bp_cells(const double* __restrict__ box, int64_t nT, const Grid* __restrict__ 
   for (int c = 0; c < 3; ++c) {
     lo[c] = cell_coord(box[6 * t + c], g.org[c], g.inv_cell, g.dims[c]);
     hi[c] = cell_coord(box[6 * t + 3 + c], g.org[c], g.inv_cell, g.dims[c]);
-    hi[c] = min(hi[c], lo[c] + 1);  // cell > extent: cannot be more; guards rounding at the far face
   }
   if (!EMIT) {
     cnt[t] = (hi[0] - lo[0] + 1) * (hi[1] - lo[1] + 1) * (hi[2] - lo[2] + 1);

@@ -644,13 +644,13 @@ tt_status broad_impl(tt_ctx* ctx, const void* pos, int64_t nV, const int32_t* tr
   }
   const unsigned gridT = grid_for(nT, BP_THREADS);
   TT_CUDA(ctx->bp_box.ensure(sizeof(double) * 6 * (size_t)nT));
-  TT_CUDA(ctx->bp_part.ensure(sizeof(double) * 7 * (size_t)gridT));
+  TT_CUDA(ctx->bp_part.ensure(sizeof(double) * 8 * (size_t)gridT));
   TT_CUDA(ctx->bp_grid.ensure(sizeof(Grid)));
   TT_CUDA(ctx->bp_cnt.ensure(sizeof(int) * (size_t)(nT + 1)));
   TT_CUDA(ctx->bp_off.ensure(sizeof(int) * (size_t)(nT + 1)));
   k_bp_aabb<T><<<gridT, BP_THREADS, 0, st>>>((const T*)pos, tris, nT, inflate, ctx->bp_box.as<double>(), ctx->bp_part.as<double>());
   TT_LAUNCH_CHECK();
-  k_bp_grid<<<1, BP_THREADS, 0, st>>>(ctx->bp_part.as<double>(), (int64_t)gridT, ctx->bp_grid.as<Grid>());
+  k_bp_grid<<<1, BP_THREADS, 0, st>>>(ctx->bp_part.as<double>(), (int64_t)gridT, nT, ctx->bp_grid.as<Grid>());
   TT_LAUNCH_CHECK();
   k_bp_cells<false><<<gridT, BP_THREADS, 0, st>>>(ctx->bp_box.as<double>(), nT, ctx->bp_grid.as<Grid>(), ctx->bp_cnt.as<int>(),
                                                   nullptr, nullptr, nullptr);
@@ -918,8 +918,8 @@ tt_status tt_broad_phase(tt_ctx* ctx, const void* pos, int64_t n_verts, const in
   if (!ctx) return TT_ERR_INVALID_ARG;
   if (!n_pairs_host) return fail(ctx, TT_ERR_INVALID_ARG, "n_pairs_host is NULL");
   if (n_verts < 0 || n_tris < 0 || !(inflate >= 0.0)) return fail(ctx, TT_ERR_INVALID_ARG, "negative size or inflate");
-  if (n_verts >= (int64_t(1) << 31) / 3 || n_tris >= (int64_t(1) << 31) / 8)
-    return fail(ctx, TT_ERR_INVALID_ARG, "sizes exceed int32 indexing (nV < 2^31/3, nT < 2^31/8)");
+  if (n_verts >= (int64_t(1) << 31) / 3 || n_tris >= (int64_t(1) << 31) / 128)
+    return fail(ctx, TT_ERR_INVALID_ARG, "sizes exceed int32 indexing (nV < 2^31/3, nT < 2^31/128)");
   if ((n_verts > 0 && !pos) || (n_tris > 0 && !tris)) return fail(ctx, TT_ERR_INVALID_ARG, "NULL array with non-zero size");
   TT_CUDA(cudaSetDevice(ctx->opt.device));
   cudaStream_t st = (cudaStream_t)stream;
