@@ -83,6 +83,11 @@ typedef struct {
 /* Force every BSR row through the general (shared-vertex) merge path; used by tests to cover it
  * on inputs whose rows would otherwise all take the exclusive-row fast path.                      */
 #define TT_FLAG_FORCE_GENERAL_ROWS 1
+/* Check every index on the device before it is used: tris < n_verts (tt_energy, tt_hess_symbolic,
+ * the *_host call, tt_broad_phase) and pairs < n_tris; an out-of-range index returns
+ * TT_ERR_INVALID_ARG with the count in tt_last_error.  Costs one small kernel and one host round
+ * trip per call; without the flag out-of-range indices are undefined behaviour (not checked).      */
+#define TT_FLAG_VALIDATE_INDICES 2
 
 typedef struct {
   const void* pos;      int64_t n_verts;   /* [nV,3] dtype                                          */

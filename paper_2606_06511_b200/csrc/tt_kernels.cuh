@@ -1857,6 +1857,12 @@ __global__ void k_gather3(const int* __restrict__ vcnt, const int* __restrict__ 
   out[3 * v + 2] = r2;
 }
 
+// TT_FLAG_VALIDATE_INDICES: counts the entries of an index array outside [0, bound)
+__global__ void k_count_out_of_range(const int* __restrict__ idx, int64_t n, int64_t bound, int* __restrict__ bad) {
+  const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (i < n && (idx[i] < 0 || (int64_t)idx[i] >= bound)) atomicAdd(bad, 1);
+}
+
 __global__ void k_i64_to_i32(const int64_t* __restrict__ in, int64_t n, int* __restrict__ out) {
   const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
   if (i < n) out[i] = (int)in[i];

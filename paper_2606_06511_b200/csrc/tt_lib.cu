@@ -149,6 +149,30 @@ tt_status check_problem(tt_ctx* ctx, const tt_problem* q) {
   return TT_OK;
 }
 
+// TT_FLAG_VALIDATE_INDICES: tris < nV and (if given) pairs < nT, checked on the device
+tt_status validate_indices(tt_ctx* ctx, const int32_t* tris, int64_t nT, int64_t nV, const int32_t* pairs, int64_t P,
+                           cudaStream_t st) {
+  if (!(ctx->opt.flags & TT_FLAG_VALIDATE_INDICES)) return TT_OK;
+  TT_CUDA(ctx->counts.ensure(sizeof(int64_t) * 16));
+  int* d_bad = reinterpret_cast<int*>(ctx->counts.as<int64_t>() + 8);
+  TT_CUDA(cudaMemsetAsync(d_bad, 0, 2 * sizeof(int), st));
+  if (nT > 0) {
+    ttk::k_count_out_of_range<<<grid_for(3 * nT, 256), 256, 0, st>>>(tris, 3 * nT, nV, d_bad);
+    TT_LAUNCH_CHECK();
+  }
+  if (pairs && P > 0) {
+    ttk::k_count_out_of_range<<<grid_for(2 * P, 256), 256, 0, st>>>(pairs, 2 * P, nT, d_bad + 1);
+    TT_LAUNCH_CHECK();
+  }
+  int bad[2] = {0, 0};
+  TT_CUDA(cudaMemcpyAsync(bad, d_bad, 2 * sizeof(int), cudaMemcpyDeviceToHost, st));
+  TT_CUDA(cudaStreamSynchronize(st));
+  if (bad[0] || bad[1])
+    return fail(ctx, TT_ERR_INVALID_ARG, "%d vertex indices of tris outside [0, %lld), %d triangle indices of pairs outside [0, %lld)",
+                bad[0], (long long)nV, bad[1], (long long)nT);
+  return TT_OK;
+}
+
 // exclusive sum of n ints (+ grand total in out[n]); `in` must have n+1 entries with in[n] == 0
 tt_status scan_i32(tt_ctx* ctx, const int* in, int* out, int64_t n_plus_1, cudaStream_t st) {
   size_t tmp = 0;
@@ -231,7 +255,9 @@ template <typename T>
 tt_status energy_impl(tt_ctx* ctx, const tt_problem* q, void* energy_sum, void* e_pp, uint32_t* active_mask,
                       void* tc, int64_t* n_active, cudaStream_t st) {
   int64_t nblk = 0;
-  tt_status s = run_classify<T>(ctx, q, (T*)e_pp, (T*)tc, false, st, &nblk);
+  tt_status s = validate_indices(ctx, q->tris, q->n_tris, q->n_verts, q->pairs, q->n_pairs, st);
+  if (s != TT_OK) return s;
+  s = run_classify<T>(ctx, q, (T*)e_pp, (T*)tc, false, st, &nblk);
   if (s != TT_OK) return s;
   ttk::k_sum_partials<T><<<1, 1024, 0, st>>>(ctx->blk_energy.as<double>(), nblk, 1.0, (T*)energy_sum);
   TT_LAUNCH_CHECK();
@@ -252,7 +278,9 @@ tt_status symbolic_impl(tt_ctx* ctx, const tt_problem* q, int64_t* nnzb_host, in
   ctx->sig.valid = false;
   const int64_t P = q->n_pairs, nT = q->n_tris, nV = q->n_verts;
   int64_t nblk = 0;
-  tt_status s = run_classify<T>(ctx, q, nullptr, nullptr, true, st, &nblk);
+  tt_status s = validate_indices(ctx, q->tris, nT, nV, q->pairs, P, st);
+  if (s != TT_OK) return s;
+  s = run_classify<T>(ctx, q, nullptr, nullptr, true, st, &nblk);
   if (s != TT_OK) return s;
   int64_t* d_counts = ctx->counts.as<int64_t>();
   k_set_count<<<1, 32, 0, st>>>(ctx->blk_off.as<int>(), ctx->blk_count.as<int>(), nblk, d_counts, nullptr);
@@ -635,12 +663,15 @@ template <typename T>
 tt_status broad_impl(tt_ctx* ctx, const void* pos, int64_t nV, const int32_t* tris, int64_t nT, double inflate,
                      int64_t* n_pairs_host, cudaStream_t st) {
   using namespace ttb;
-  (void)nV;
   ctx->bp_n_pairs = -1;
   *n_pairs_host = 0;
   if (nT < 2) {
     ctx->bp_n_pairs = 0;
     return TT_OK;
+  }
+  {
+    tt_status sv = validate_indices(ctx, tris, nT, nV, nullptr, 0, st);
+    if (sv != TT_OK) return sv;
   }
   const unsigned gridT = grid_for(nT, BP_THREADS);
   TT_CUDA(ctx->bp_box.ensure(sizeof(double) * 6 * (size_t)nT));

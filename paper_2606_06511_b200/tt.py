@@ -19,6 +19,7 @@ TT_OK = 0
 TT_F64, TT_F32 = 0, 1
 TT_HESS_EQ4, TT_HESS_FILTER, TT_HESS_PSD2, TT_HESS_PSDPROJ = 0, 1, 2, 3
 TT_FLAG_FORCE_GENERAL_ROWS = 1
+TT_FLAG_VALIDATE_INDICES = 2
 
 EXPORTS = ["tt_create", "tt_destroy", "tt_energy", "tt_hess_symbolic", "tt_energy_grad_hess", "tt_hess_vec",
            "tt_energy_grad_hess_host", "tt_broad_phase", "tt_broad_phase_pairs", "tt_broad_phase_copy", "tt_bsr_device", "tt_stats", "tt_kernel_ms", "tt_probe_peaks", "tt_status_string", "tt_last_error"]

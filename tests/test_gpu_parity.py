@@ -283,6 +283,37 @@ def test_error_paths(oracle_mod):
     ctx.close()
 
 
+def test_validate_indices_flag(oracle_mod):
+    """TT_FLAG_VALIDATE_INDICES: an out-of-range vertex or triangle index is reported, not dereferenced;
+    valid input gives the same result as without the flag."""
+    from paper_2606_06511_b200 import inputs, tt
+    dev = _dev()
+    pb = inputs.config0_soup()
+    ctx = tt.Context(torch.float64, 1, 1.0, 0, tt.TT_FLAG_VALIDATE_INDICES)
+    pos = torch.from_numpy(pb.pos).to(dev)
+    tris = torch.from_numpy(pb.tris).to(dev)
+    prs = torch.from_numpy(pb.pairs).to(dev)
+    e = torch.zeros(1, dtype=torch.float64, device=dev)
+    bad_tris = tris.clone()
+    bad_tris[5, 1] = pos.shape[0]                       # one past the last vertex
+    with pytest.raises(tt.TTError) as ei:
+        ctx.tt_hess_symbolic(ctx.problem(pos, bad_tris, prs))
+    assert ei.value.status == -1 and "1 vertex indices" in str(ei.value)
+    bad_prs = prs.clone()
+    bad_prs[7, 0] = -1
+    bad_prs[9, 1] = tris.shape[0]
+    with pytest.raises(tt.TTError) as ei:
+        ctx.tt_energy(ctx.problem(pos, tris, bad_prs), e)
+    assert ei.value.status == -1 and "2 triangle indices" in str(ei.value)
+    with pytest.raises(tt.TTError):
+        ctx.tt_broad_phase(pos, bad_tris, 0.0)
+    out = tt.assemble(ctx, pos, tris, prs)             # valid input: unchanged behaviour
+    ref = oracle_mod.assemble(pb.pos, pb.tris, pb.pairs, 1.0, 1)
+    torch.cuda.synchronize()
+    assert out["nnzb"] == ref["nnzb"] and out["n_active"] == int(ref["active"].sum())
+    ctx.close()
+
+
 def test_host_buffer_entry_point(oracle_mod):
     """tt_energy_grad_hess_host (the e2e call bench.py times) == device-buffer path == oracle."""
     from paper_2606_06511_b200 import inputs, tt
