@@ -8,7 +8,7 @@
 //   k_bp_aabb      boxes in fp64 + per-CTA partial bounds          (HBM: 3 vertices in, 48 B out)
 //   k_bp_grid      origin, cell size, grid dimensions (one CTA, fixed order)
 //   k_bp_cells     <COUNT / EMIT> (cell key, triangle) records, <= 125 per triangle (typically 2-4)
-//   CUB radix sort of the records by cell key (stable: triangles ascending inside a cell)
+//   CUB radix sort of the records by (cell, quantised lo.x): sweep-and-prune inside a cell
 //   k_bp_pairs     <COUNT / EMIT> one thread per record walks the later records of its cell; a pair is
 //                  reported only in the cell that owns the point max(lo_i, lo_j), which lies in both
 //                  boxes when they overlap, so every pair is reported exactly once
@@ -111,7 +111,18 @@ __device__ __forceinline__ uint64_t cell_key(const Grid& g, int cx, int cy, int 
   return ((uint64_t)cx * (uint64_t)g.dims[1] + (uint64_t)cy) * (uint64_t)g.dims[2] + (uint64_t)cz;
 }
 
-// COUNT: cnt[t] = cells box t touches (1..125).  EMIT: records at off[t].
+// Sweep-and-prune inside a cell: the records of a cell are sorted by the x of their box's lower bound,
+// quantised to BP_QBITS bits of the cell width (monotone, so the pruning below is conservative):
+// a walk stops at the first record whose quantised lo.x exceeds the walker's quantised hi.x.
+constexpr int BP_QBITS = 16;
+__device__ __forceinline__ unsigned quant_x(double x, const Grid& g, int cx) {
+  const double f = (x - g.org[0]) * g.inv_cell - (double)cx;  // position inside cell cx, in cell widths
+  const double q = floor(f * (double)(1u << BP_QBITS));
+  return (unsigned)fmin(fmax(q, 0.0), (double)((1u << BP_QBITS) - 1u));
+}
+
+// COUNT: cnt[t] = cells box t touches (1..125).  EMIT: records at off[t],
+// key = cell << BP_QBITS | quantised lo.x inside that cell.
 template <bool EMIT>
 __global__ void __launch_bounds__(BP_THREADS)
 k_bp_cells(const double* __restrict__ box, int64_t nT, const Grid* __restrict__ gp, int* __restrict__ cnt,
@@ -133,7 +144,7 @@ k_bp_cells(const double* __restrict__ box, int64_t nT, const Grid* __restrict__ 
   for (int cx = lo[0]; cx <= hi[0]; ++cx)
     for (int cy = lo[1]; cy <= hi[1]; ++cy)
       for (int cz = lo[2]; cz <= hi[2]; ++cz) {
-        keys[o] = cell_key(g, cx, cy, cz);
+        keys[o] = (cell_key(g, cx, cy, cz) << BP_QBITS) | quant_x(box[6 * t], g, cx);
         vals[o] = (uint32_t)t;
         ++o;
       }
@@ -154,7 +165,7 @@ k_bp_pairs(const uint64_t* __restrict__ keys, const uint32_t* __restrict__ vals,
   const int64_t r = (int64_t)blockIdx.x * BP_THREADS + threadIdx.x;
   if (r >= n_rec) return;
   const Grid g = *gp;
-  const uint64_t key = keys[r];
+  const uint64_t key = keys[r] >> BP_QBITS;  // the cell
   const int64_t i = vals[r];
   double lo[3], hi[3];
 #pragma unroll
@@ -162,9 +173,12 @@ k_bp_pairs(const uint64_t* __restrict__ keys, const uint32_t* __restrict__ vals,
     lo[c] = box[6 * i + c];
     hi[c] = box[6 * i + 3 + c];
   }
+  // last quantised lo.x a partner can have: hi.x of this box inside this cell
+  const int cx = (int)(key / ((uint64_t)g.dims[1] * (uint64_t)g.dims[2]));
+  const uint64_t stop = (key << BP_QBITS) | quant_x(hi[0], g, cx);
   int n = 0;
   int64_t o = EMIT ? off[r] : 0;
-  for (int64_t q = r + 1; q < n_rec && keys[q] == key; ++q) {
+  for (int64_t q = r + 1; q < n_rec && keys[q] <= stop; ++q) {
     const int64_t j = vals[q];
     double m[3];
     bool ov = true;

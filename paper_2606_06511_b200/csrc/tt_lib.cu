@@ -696,9 +696,9 @@ tt_status broad_impl(tt_ctx* ctx, const void* pos, int64_t nV, const int32_t* tr
   TT_CUDA(cudaStreamSynchronize(st));
   const int64_t n_rec = n_rec32;
   const double n_cells = (double)g.dims[0] * (double)g.dims[1] * (double)g.dims[2];
-  if (n_cells >= 9.0e18) return fail(ctx, TT_ERR_INVALID_ARG, "broad phase: grid of %d x %d x %d cells exceeds 63-bit keys", g.dims[0], g.dims[1], g.dims[2]);
+  if (n_cells >= 1.0e14) return fail(ctx, TT_ERR_INVALID_ARG, "broad phase: grid of %d x %d x %d cells exceeds 47-bit cell keys", g.dims[0], g.dims[1], g.dims[2]);
   int cell_bits = 1;
-  while (cell_bits < 63 && (double)(1ull << cell_bits) < n_cells) ++cell_bits;
+  while (cell_bits < 63 - ttb::BP_QBITS && (double)(1ull << cell_bits) < n_cells) ++cell_bits;
   for (int i = 0; i < 2; ++i) {
     TT_CUDA(ctx->bp_keys[i].ensure(sizeof(uint64_t) * (size_t)(n_rec + 1)));
     TT_CUDA(ctx->bp_vals[i].ensure(sizeof(uint32_t) * (size_t)(n_rec + 1)));
@@ -708,7 +708,7 @@ tt_status broad_impl(tt_ctx* ctx, const void* pos, int64_t nV, const int32_t* tr
   TT_LAUNCH_CHECK();
   uint64_t* keys = nullptr;
   uint32_t* vals = nullptr;
-  s = sort_pairs(ctx, ctx->bp_keys, ctx->bp_vals, n_rec, 0, cell_bits, &keys, &vals, st);
+  s = sort_pairs(ctx, ctx->bp_keys, ctx->bp_vals, n_rec, 0, cell_bits + ttb::BP_QBITS, &keys, &vals, st);
   if (s != TT_OK) return s;
   TT_CUDA(ctx->bp_pcnt.ensure(sizeof(int) * (size_t)(n_rec + 1)));
   TT_CUDA(ctx->bp_poff.ensure(sizeof(int64_t) * (size_t)(n_rec + 1)));
