@@ -886,9 +886,9 @@ tt_status tt_energy_grad_hess_host(tt_ctx* ctx, const tt_problem* prob, void* en
   TT_CUDA(ctx->o_grad.ensure(w * 3 * (size_t)nV + 16));
   TT_CUDA(ctx->o_energy.ensure(16));
   // Copy schedule (PCIe is full duplex; the step is shorter than its copies):
-  //   stream : H2D pos, tris, pairs -> symbolic -> numeric -> [wait p] H.p -> D2H y
-  //   side   : [after the inputs] H2D p (under the symbolic / numeric phase)
-  //            [after numeric] D2H energy, grad, pattern, values (under H.p and the D2H of y)
+  //   stream : H2D pos, tris, pairs -> symbolic -> [wait p] H.p -> numeric -> D2H energy, grad, pattern, values
+  //   side   : [after the inputs] H2D p (under the symbolic phase)
+  //            [after H.p] D2H y (under the numeric phase)
   const bool want_hv = p_host && nV;
   if (want_hv) {
     TT_CUDA(ctx->h_p.ensure(w * 3 * (size_t)nV + 16));
@@ -918,27 +918,28 @@ tt_status tt_energy_grad_hess_host(tt_ctx* ctx, const tt_problem* prob, void* en
     return fail(ctx, TT_ERR_CAPACITY, "nnzb_capacity %lld < nnzb %lld", (long long)nnzb_capacity, (long long)nnzb);
   }
   TT_CUDA(ctx->o_vals.ensure(w * 9 * (size_t)nnzb + 16));
-  s = ctx->opt.dtype == TT_F64
-          ? numeric_impl<double>(ctx, &d, ctx->o_energy.p, ctx->o_grad.p, ctx->rowptr.as<int>(), ctx->colind.as<int>(), ctx->o_vals.p, nnzb, st)
-          : numeric_impl<float>(ctx, &d, ctx->o_energy.p, ctx->o_grad.p, ctx->rowptr.as<int>(), ctx->colind.as<int>(), ctx->o_vals.p, nnzb, st);
-  if (s != TT_OK) { cudaStreamSynchronize(ctx->side); return s; }
-  ctx->host_nnzb = nnzb;
-  TT_CUDA(cudaEventRecord(ctx->ev_num, st));
-  // results of the numeric phase leave on the side stream while H.p runs
-  TT_CUDA(cudaStreamWaitEvent(ctx->side, ctx->ev_num, 0));
-  TT_CUDA(cudaMemcpyAsync(energy_host, ctx->o_energy.p, w, cudaMemcpyDeviceToHost, ctx->side));
-  if (grad_host && nV) TT_CUDA(cudaMemcpyAsync(grad_host, ctx->o_grad.p, w * 3 * (size_t)nV, cudaMemcpyDeviceToHost, ctx->side));
-  if (rowptr_host) TT_CUDA(cudaMemcpyAsync(rowptr_host, ctx->rowptr.p, sizeof(int) * (size_t)(nV + 1), cudaMemcpyDeviceToHost, ctx->side));
-  if (colind_host && nnzb) TT_CUDA(cudaMemcpyAsync(colind_host, ctx->colind.p, sizeof(int) * (size_t)nnzb, cudaMemcpyDeviceToHost, ctx->side));
-  if (vals_host && nnzb) TT_CUDA(cudaMemcpyAsync(vals_host, ctx->o_vals.p, w * 9 * (size_t)nnzb, cudaMemcpyDeviceToHost, ctx->side));
-  TT_CUDA(cudaEventRecord(ctx->ev_side, ctx->side));
+  // H.p first: it needs only the symbolic phase and p, and its result then leaves (side stream)
+  // under the numeric phase; the numeric results leave last.
   if (want_hv) {
     TT_CUDA(cudaStreamWaitEvent(st, ctx->ev_p, 0));
     s = ctx->opt.dtype == TT_F64 ? hessvec_impl<double>(ctx, &d, ctx->h_p.p, ctx->o_y.p, st)
                                  : hessvec_impl<float>(ctx, &d, ctx->h_p.p, ctx->o_y.p, st);
     if (s != TT_OK) { cudaStreamSynchronize(ctx->side); return s; }
-    TT_CUDA(cudaMemcpyAsync(y_host, ctx->o_y.p, w * 3 * (size_t)nV, cudaMemcpyDeviceToHost, st));
+    TT_CUDA(cudaEventRecord(ctx->ev_num, st));
+    TT_CUDA(cudaStreamWaitEvent(ctx->side, ctx->ev_num, 0));
+    TT_CUDA(cudaMemcpyAsync(y_host, ctx->o_y.p, w * 3 * (size_t)nV, cudaMemcpyDeviceToHost, ctx->side));
   }
+  s = ctx->opt.dtype == TT_F64
+          ? numeric_impl<double>(ctx, &d, ctx->o_energy.p, ctx->o_grad.p, ctx->rowptr.as<int>(), ctx->colind.as<int>(), ctx->o_vals.p, nnzb, st)
+          : numeric_impl<float>(ctx, &d, ctx->o_energy.p, ctx->o_grad.p, ctx->rowptr.as<int>(), ctx->colind.as<int>(), ctx->o_vals.p, nnzb, st);
+  if (s != TT_OK) { cudaStreamSynchronize(ctx->side); return s; }
+  ctx->host_nnzb = nnzb;
+  TT_CUDA(cudaMemcpyAsync(energy_host, ctx->o_energy.p, w, cudaMemcpyDeviceToHost, st));
+  if (grad_host && nV) TT_CUDA(cudaMemcpyAsync(grad_host, ctx->o_grad.p, w * 3 * (size_t)nV, cudaMemcpyDeviceToHost, st));
+  if (rowptr_host) TT_CUDA(cudaMemcpyAsync(rowptr_host, ctx->rowptr.p, sizeof(int) * (size_t)(nV + 1), cudaMemcpyDeviceToHost, st));
+  if (colind_host && nnzb) TT_CUDA(cudaMemcpyAsync(colind_host, ctx->colind.p, sizeof(int) * (size_t)nnzb, cudaMemcpyDeviceToHost, st));
+  if (vals_host && nnzb) TT_CUDA(cudaMemcpyAsync(vals_host, ctx->o_vals.p, w * 9 * (size_t)nnzb, cudaMemcpyDeviceToHost, st));
+  TT_CUDA(cudaEventRecord(ctx->ev_side, ctx->side));
   TT_CUDA(cudaStreamWaitEvent(st, ctx->ev_side, 0));  // `stream` completes only after the side copies
   TT_CUDA(cudaStreamSynchronize(st));
   return TT_OK;
