@@ -157,7 +157,17 @@ k_classify(const T* __restrict__ pos, const int* __restrict__ tris, const int2* 
   }
 }
 
-// Fixed-order sum of n doubles by ONE CTA (deterministic), scaled, written as T.
+// Fixed-order sum of n doubles (deterministic), scaled, written as T.  Large n: k_sum_stage first
+// reduces fixed slices of SUM_SLICE values per CTA, then ONE CTA sums the slice sums.
+constexpr int SUM_SLICE = 8192;
+__global__ void __launch_bounds__(256) k_sum_stage(const double* __restrict__ part, int64_t n, double* __restrict__ out) {
+  __shared__ double s[8];
+  const int64_t lo = (int64_t)blockIdx.x * SUM_SLICE, hi = min(lo + (int64_t)SUM_SLICE, n);
+  double v = 0.0;
+  for (int64_t i = lo + threadIdx.x; i < hi; i += 256) v += part[i];
+  const double r = block_sum<256>(v, s);
+  if (threadIdx.x == 0) out[blockIdx.x] = r;
+}
 template <typename T>
 __global__ void __launch_bounds__(1024) k_sum_partials(const double* __restrict__ part, int64_t n,
                                                        double scale, T* __restrict__ out) {
@@ -178,9 +188,13 @@ __global__ void k_set_count(const int* __restrict__ blk_off, const int* __restri
 }
 
 // ------------------------------------------------------------------------------------------ K2
+// With pairs / cfg / keys given it also emits the directed entries: active pair k = (s,t) -> (s -> t,
+// side 0) and (t -> s, side 1), key = (source << bitsT) | partner, payload = side | recorded config of
+// the canonical pair << 1.
 __global__ void __launch_bounds__(CLS_THREADS)
 k_compact(const uint32_t* __restrict__ mask, const int* __restrict__ blk_off, int64_t P,
-          int* __restrict__ active_ids) {
+          int* __restrict__ active_ids, const int2* __restrict__ pairs, const uint16_t* __restrict__ cfg, int bitsT,
+          uint64_t* __restrict__ keys, uint16_t* __restrict__ vals) {
   const int64_t k = (int64_t)blockIdx.x * CLS_THREADS + threadIdx.x;
   const int w = threadIdx.x >> 5, l = threadIdx.x & 31;
   const int64_t word0 = (int64_t)blockIdx.x * (CLS_THREADS / 32);
@@ -192,26 +206,21 @@ k_compact(const uint32_t* __restrict__ mask, const int* __restrict__ blk_off, in
     if (i < w) before += __popc(m);
     if (i == w) mine = m;
   }
-  if ((mine >> l) & 1u) active_ids[blk_off[blockIdx.x] + before + __popc(mine & ((1u << l) - 1u))] = (int)k;
+  if ((mine >> l) & 1u) {
+    const int64_t a = (int64_t)blk_off[blockIdx.x] + before + __popc(mine & ((1u << l) - 1u));
+    active_ids[a] = (int)k;
+    if (keys) {
+      const int2 pr = __ldg(pairs + k);
+      const unsigned c = (unsigned)__ldg(cfg + k) << 1;
+      keys[2 * a] = ((uint64_t)(uint32_t)pr.x << bitsT) | (uint32_t)pr.y;
+      keys[2 * a + 1] = ((uint64_t)(uint32_t)pr.y << bitsT) | (uint32_t)pr.x;
+      vals[2 * a] = (uint16_t)c;
+      vals[2 * a + 1] = (uint16_t)(c | 1u);
+    }
+  }
 }
 
 // ------------------------------------------------------------------------------------------ K3
-// Directed entries: active pair k = (s,t) -> (s -> t, side 0) and (t -> s, side 1).
-// key = (source << bitsT) | partner, payload = side | recorded config of the canonical pair << 1.
-__global__ void k_emit_directed(const int2* __restrict__ pairs, const int* __restrict__ active_ids,
-                                const uint16_t* __restrict__ cfg, int64_t A, int bitsT,
-                                uint64_t* __restrict__ keys, uint16_t* __restrict__ vals) {
-  const int64_t k = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
-  if (k >= A) return;
-  const int id = active_ids[k];
-  const int2 pr = __ldg(pairs + id);
-  const unsigned c = (unsigned)__ldg(cfg + id) << 1;
-  keys[2 * k] = ((uint64_t)(uint32_t)pr.x << bitsT) | (uint32_t)pr.y;
-  keys[2 * k + 1] = ((uint64_t)(uint32_t)pr.y << bitsT) | (uint32_t)pr.x;
-  vals[2 * k] = (uint16_t)c;
-  vals[2 * k + 1] = (uint16_t)(c | 1u);
-}
-
 // Segment pointers from sorted keys: ptr[g] = first entry whose (key >> shift) >= g, g = 0..G.
 __global__ void k_segment_ptr(const uint64_t* __restrict__ keys, int64_t n, int shift, int64_t G,
                               int* __restrict__ ptr) {

@@ -62,7 +62,7 @@ struct tt_ctx {
   std::string err;
   int64_t launches = 0;
   // classification
-  DevBuf mask, blk_count, blk_off, blk_energy, counts, energy, cfg;
+  DevBuf mask, blk_count, blk_off, blk_energy, counts, energy, cfg, sum_stage;
   // active set + directed entries
   DevBuf active_ids, keys[2], dvals[2], tptr, vcnt, tflag, touched;
   // per-triangle symbolic
@@ -251,6 +251,23 @@ tt_status run_classify(tt_ctx* ctx, const tt_problem* q, T* e_pp, T* tc, bool re
   return TT_OK;
 }
 
+// deterministic sum of n partials -> out[0] (two levels above SUM_SLICE values)
+template <typename T>
+tt_status sum_partials(tt_ctx* ctx, const double* part, int64_t n, T* out, cudaStream_t st) {
+  using namespace ttk;
+  if (n > 4 * SUM_SLICE) {
+    const int64_t ns = (n + SUM_SLICE - 1) / SUM_SLICE;
+    TT_CUDA(ctx->sum_stage.ensure(sizeof(double) * (size_t)ns));
+    k_sum_stage<<<(unsigned)ns, 256, 0, st>>>(part, n, ctx->sum_stage.as<double>());
+    TT_LAUNCH_CHECK();
+    part = ctx->sum_stage.as<double>();
+    n = ns;
+  }
+  k_sum_partials<T><<<1, 1024, 0, st>>>(part, n, 1.0, out);
+  TT_LAUNCH_CHECK();
+  return TT_OK;
+}
+
 template <typename T>
 tt_status energy_impl(tt_ctx* ctx, const tt_problem* q, void* energy_sum, void* e_pp, uint32_t* active_mask,
                       void* tc, int64_t* n_active, cudaStream_t st) {
@@ -259,8 +276,8 @@ tt_status energy_impl(tt_ctx* ctx, const tt_problem* q, void* energy_sum, void* 
   if (s != TT_OK) return s;
   s = run_classify<T>(ctx, q, (T*)e_pp, (T*)tc, false, st, &nblk);
   if (s != TT_OK) return s;
-  ttk::k_sum_partials<T><<<1, 1024, 0, st>>>(ctx->blk_energy.as<double>(), nblk, 1.0, (T*)energy_sum);
-  TT_LAUNCH_CHECK();
+  s = sum_partials<T>(ctx, ctx->blk_energy.as<double>(), nblk, (T*)energy_sum, st);
+  if (s != TT_OK) return s;
   if (n_active) {
     ttk::k_set_count<<<1, 32, 0, st>>>(ctx->blk_off.as<int>(), ctx->blk_count.as<int>(), nblk, n_active, nullptr);
     TT_LAUNCH_CHECK();
@@ -297,21 +314,19 @@ tt_status symbolic_impl(tt_ctx* ctx, const tt_problem* q, int64_t* nnzb_host, in
 
   // ---- compaction + directed entries sorted by (source, partner) ----
   TT_CUDA(ctx->active_ids.ensure(sizeof(int) * (size_t)(A + 1)));
-  if (nblk > 0) {
-    k_compact<<<(unsigned)nblk, CLS_THREADS, 0, st>>>(ctx->mask.as<uint32_t>(), ctx->blk_off.as<int>(), P,
-                                                      ctx->active_ids.as<int>());
-    TT_LAUNCH_CHECK();
-  }
   for (int i = 0; i < 2; ++i) {
     TT_CUDA(ctx->keys[i].ensure(sizeof(uint64_t) * (size_t)(n + 1)));
     TT_CUDA(ctx->dvals[i].ensure(sizeof(uint16_t) * (size_t)(n + 1)));
   }
   ctx->keys_sorted = ctx->keys[0].as<uint64_t>();
   ctx->dvals_sorted = ctx->dvals[0].as<uint16_t>();
-  if (A > 0) {
-    k_emit_directed<<<grid_for(A, 256), 256, 0, st>>>((const int2*)q->pairs, ctx->active_ids.as<int>(), ctx->cfg.as<uint16_t>(), A, bitsT,
+  if (nblk > 0) {  // active ids + the two directed entries of every active pair, in one pass
+    k_compact<<<(unsigned)nblk, CLS_THREADS, 0, st>>>(ctx->mask.as<uint32_t>(), ctx->blk_off.as<int>(), P, ctx->active_ids.as<int>(),
+                                                      (const int2*)q->pairs, ctx->cfg.as<uint16_t>(), bitsT,
                                                       ctx->keys[0].as<uint64_t>(), ctx->dvals[0].as<uint16_t>());
     TT_LAUNCH_CHECK();
+  }
+  if (A > 0) {
     // stable sort on the SOURCE bits only: a triangle's entries become contiguous, in active-pair
     // order (deterministic); nothing downstream needs the partners ascending (columns are ranked)
     s = sort_pairs(ctx, ctx->keys, ctx->dvals, n, bitsT, 2 * bitsT, &ctx->keys_sorted, &ctx->dvals_sorted, st);
@@ -632,9 +647,7 @@ tt_status numeric_impl(tt_ctx* ctx, const tt_problem* q, void* energy_sum, void*
     k_gather3<T><<<grid_for(nV, 256), 256, 0, st>>>(ctx->vcnt.as<int>(), ctx->vslot1.as<int>(), ctx->vptr.as<int>(), ctx->vvals_sorted, nV, ctx->tslot.as<T>(), (T*)grad);
     TT_LAUNCH_CHECK();
   }
-  k_sum_partials<T><<<1, 1024, 0, st>>>(ctx->asm_energy.as<double>(), ctx->n_chunks, 1.0, (T*)energy_sum);
-  TT_LAUNCH_CHECK();
-  return TT_OK;
+  return sum_partials<T>(ctx, ctx->asm_energy.as<double>(), ctx->n_chunks, (T*)energy_sum, st);
 }
 
 template <typename T>
