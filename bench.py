@@ -1,7 +1,8 @@
 #!/usr/bin/env python
 """bench.py -- throughput of the whole hot path.
 
-    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--pairs P] [--dtype f64|f32]
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--config 0..4] [--pairs P]
+                    [--dtype f64|f32] [--sweep P1,P2,...]
 
 One "step" = one pass over all hot-path rows on one batch of synthetic input (BASELINE.json
 configs[4], the throughput sweep: 2M-triangle random soup, P seeded candidate pairs, ~50 % active):
@@ -11,6 +12,8 @@ tt_hess_symbolic (classification a1/a2, compaction a2', BSR pattern a4) + tt_ene
   value        candidate pairs / s, inputs already resident in HBM (CUDA events on the launching stream)
   e2e          the same through tt_energy_grad_hess_host: pinned HOST buffers, H2D + D2H inside the timed region
   roofline     dominant kernel (k_assemble): algorithmic bytes / its CUDA-event duration vs measured HBM peak
+  roofline_all the same for each of the three calls of the step, and step_frac for the step as a whole
+  sweep        config 4 only: the same step at other points of BASELINE's 1M-50M sweep (fewer steps each)
   cpu_baseline the CPU oracle, as it stands, on a bounded sample (rank 0, N=1)
 
 --impl reference times the oracle (the tier's reference arm).  N>1 (torchrun): independent
@@ -43,7 +46,12 @@ def parse():
     ap.add_argument("--steps", type=int, default=10)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
-    ap.add_argument("--pairs", type=int, default=10_000_000)
+    ap.add_argument("--config", type=int, default=4, choices=[0, 1, 2, 3, 4],
+                    help="BASELINE.json configs[i]; 4 (the throughput sweep the metric is quoted on) is the default")
+    ap.add_argument("--pairs", type=int, default=10_000_000, help="config 4: candidate pairs of the headline workload")
+    ap.add_argument("--sweep", default="1000000,50000000",
+                    help="config 4: further sweep points reported under 'sweep' (comma separated pair counts, '' = none)")
+    ap.add_argument("--sweep-steps", type=int, default=5)
     ap.add_argument("--tris", type=int, default=2_000_000)
     ap.add_argument("--dtype", default="f64", choices=["f64", "f32"])
     ap.add_argument("--hess-mode", type=int, default=1)
@@ -129,11 +137,14 @@ def rank_seed(base_seed, rank):
     return base_seed + 1000 * rank
 
 
-def make_problem(args, rank, device):
+def make_problem(args, rank, device, n_pairs=None):
     from paper_2606_06511_b200 import inputs
     t = time.time()
-    pb = inputs.config4_sweep(n_tris=args.tris, n_pairs=args.pairs, seed=rank_seed(inputs.BASE_SEED + 4, rank),
-                              device=device)
+    if args.config == 4:
+        pb = inputs.config4_sweep(n_tris=args.tris, n_pairs=n_pairs or args.pairs,
+                                  seed=rank_seed(inputs.BASE_SEED + 4, rank), device=device)
+    else:
+        pb = inputs.by_name("config%d" % args.config, seed=rank_seed(inputs.BASE_SEED + args.config, rank))
     log("[bench] rank %d generated %s: nV=%d nT=%d P=%d in %.1fs" % (rank, pb.name, pb.n_verts, pb.n_tris, pb.n_pairs,
                                                                     time.time() - t))
     return pb
@@ -158,7 +169,9 @@ def cpu_baseline(pb, hess_mode, budget_s=15.0):
     n = int(min(pb.n_pairs, max(n0, n0 * budget_s / max(t0, 1e-3))))
     t = oracle_step(oracle, pb, n, hess_mode, p)
     return {"value": n / t, "unit": UNIT, "cores": oracle.max_threads(), "kind": "oracle",
-            "sample": "first %d of %d candidate pairs of the same workload, energy+grad+BSR+H.p, %.1f s wall" % (n, pb.n_pairs, t)}
+            "sample": "first %d of %d candidate pairs of the same workload, energy+grad+BSR+H.p, %.1f s wall" % (n, pb.n_pairs, t),
+            "note": "the oracle as it stands: per-pair loop (18-partial dual numbers) and H.p run under OpenMP on `cores` "
+                    "threads, its pattern sort and BSR accumulation are serial; a baseline, not a tuned CPU figure"}
 
 
 def run_reference(args):
@@ -230,6 +243,140 @@ def run_broad_phase(args):
     ctx.close()
 
 
+WORKLOADS = {0: "configs[0] 64-triangle soup, all pairs", 1: "configs[1] two icospheres, inflated-AABB candidates",
+             2: "configs[2] folded cloth 256x256, inflated-AABB candidates", 3: "configs[3] twisted torus 1M triangles, AABB candidates",
+             4: "configs[4] throughput sweep: random soup, seeded random candidate pairs"}
+
+
+def measure(ctx, pb, args, dev, steps, warmup, world=1, rank=0, sampler_rank0=False):
+    """W warm-up + K timed steps of symbolic + numeric + H.p on one resident workload.  No synchronisation
+    inside the timed loop: phase events are recorded on the launching stream, the library records the
+    events of its three large kernels itself (tt_kernel_ms_mean), all read after the loop."""
+    import torch
+    import torch.distributed as dist
+    tdt = ctx.dtype
+    w = 8 if tdt == torch.float64 else 4
+    pos_np = pb.pos if w == 8 else pb.pos.astype(np.float32)
+    pos = torch.from_numpy(pos_np).to(dev)
+    tris = torch.from_numpy(pb.tris).to(dev)
+    pairs = torch.from_numpy(pb.pairs).to(dev)
+    P, nV, nT = pb.n_pairs, pb.n_verts, pb.n_tris
+    prob = ctx.problem(pos, tris, pairs)
+    stream = torch.cuda.current_stream()
+    # sizes are a property of the input: allocate outputs once (a Newton loop would do the same)
+    nnzb, n_active = ctx.tt_hess_symbolic(prob)
+    energy = torch.zeros(1, dtype=tdt, device=dev)
+    grad = torch.empty((nV, 3), dtype=tdt, device=dev)
+    rowptr = torch.empty(nV + 1, dtype=torch.int32, device=dev)
+    colind = torch.empty(max(nnzb, 1), dtype=torch.int32, device=dev)
+    vals = torch.empty((max(nnzb, 1), 3, 3), dtype=tdt, device=dev)
+    pvec = torch.randn((nV, 3), dtype=tdt, device=dev)
+    yvec = torch.empty_like(pvec)
+    log("[bench] rank %d: P=%d A=%d nnzb=%d (vals %.2f GB)" % (rank, P, n_active, nnzb, nnzb * 9 * w / 1e9))
+    phase_ev = []
+
+    def step(record=False):
+        ev = [torch.cuda.Event(enable_timing=True) for _ in range(4)] if record else None
+        if record:
+            ev[0].record(stream)
+        ctx.tt_hess_symbolic(prob)
+        if record:
+            ev[1].record(stream)
+        ctx.tt_energy_grad_hess(prob, energy, grad, rowptr, colind, vals, max(nnzb, 1))
+        if record:
+            ev[2].record(stream)
+        ctx.tt_hess_vec(prob, pvec, yvec)
+        if record:
+            ev[3].record(stream)
+            phase_ev.append(ev)
+
+    for _ in range(warmup):
+        step()
+    torch.cuda.synchronize()
+    if world > 1:
+        dist.barrier()
+    torch.cuda.synchronize()
+    ctx.tt_kernel_ms_mean(reset=True)
+    sampler = ClockSampler(dev.index) if sampler_rank0 else None
+    l0 = ctx.tt_stats()["launches"]
+    ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    t_wall0 = time.time()
+    ev0.record(stream)
+    for _ in range(steps):
+        step(record=True)
+    ev1.record(stream)
+    torch.cuda.synchronize()
+    if world > 1:
+        dist.barrier()
+    t_wall1 = time.time()
+    launches = ctx.tt_stats()["launches"] - l0
+    kms, kcount = ctx.tt_kernel_ms_mean(reset=True)          # events of the timed steps only (ring of 64 launches)
+    ms_local = ev0.elapsed_time(ev1)
+    ms_total, P_all = aggregate_ranks(ms_local, P, world, dev)
+    clocks = sampler.stop(t_wall0, t_wall1) if sampler else None
+    ms_step = ms_total / steps
+    phase_ms = {name: float(np.mean([e[i].elapsed_time(e[i + 1]) for e in phase_ev]))
+                for i, name in enumerate(("tt_hess_symbolic", "tt_energy_grad_hess", "tt_hess_vec"))}
+
+    # ---- algorithmic bytes (SURVEY 8(d): every unique item once; staging is not counted) ----
+    hbm, peak_src = peaks()
+    st = ctx.tt_stats()
+    n_touch = st["n_touched_tris"]                                    # triangles of ACTIVE pairs
+    rows_touched = int((rowptr[1:] != rowptr[:-1]).sum().item())      # their vertices (= non-empty rows)
+    cand_tris = int(torch.unique(pairs).numel())                      # triangles any CANDIDATE refers to
+    cand_verts = int(torch.unique(tris[torch.unique(pairs).long()]).numel()) if P else 0
+    b_sym = 8 * P + 12 * cand_tris + 3 * w * cand_verts + P // 8 + 4 * (nV + 1) + 4 * nnzb
+    b_k4 = 9 * w * nnzb + 3 * w * rows_touched + 12 * n_touch + 8 * n_active + 3 * w * rows_touched
+    b_num = b_k4 + 3 * w * nV                                         # + the dense gradient [nV,3]
+    b_hv = 4 * n_active + 12 * n_touch + 3 * w * rows_touched + 6 * w * nV
+    b_k1 = 8 * P + 12 * cand_tris + 3 * w * cand_verts + P // 8
+
+    def roof(name, nbytes, ms):
+        a = nbytes / (ms * 1e-3) / 1e9 if ms and ms > 0 else 0.0
+        return {"call": name, "bound": "hbm", "algorithmic_bytes": int(nbytes), "ms": ms, "achieved": a, "peak": hbm,
+                "unit": "GB/s", "frac": a / hbm}
+
+    roofline_all = [roof("tt_hess_symbolic", b_sym, phase_ms["tt_hess_symbolic"]),
+                    roof("tt_energy_grad_hess", b_num, phase_ms["tt_energy_grad_hess"]),
+                    roof("tt_hess_vec", b_hv, phase_ms["tt_hess_vec"])]
+    step_bytes = b_sym + b_num + b_hv
+    res = dict(ms_step=ms_step, P_all=P_all, P=P, nV=nV, nT=nT, nnzb=nnzb, n_active=n_active, launches=int(launches),
+               kernel_ms=kms, kernel_launches=kcount, phase_ms=phase_ms, clocks=clocks, roofline_all=roofline_all,
+               step_frac=step_bytes / (ms_step * 1e-3) / 1e9 / hbm, step_bytes=int(step_bytes),
+               k4=roof("k_assemble", b_k4, kms["assemble"]), k1=roof("k_classify", b_k1, kms["classify"]),
+               k6=roof("k_entry_pipe", b_hv - 6 * w * nV + 3 * w * nV, kms["hess_vec"]),
+               hbm=hbm, peak_src=peak_src, w=w, in_bytes=pos.numel() * w + tris.numel() * 4 + pairs.numel() * 4,
+               tensors=(pos_np, pvec))
+    del vals, colind, grad, rowptr, yvec
+    torch.cuda.empty_cache()
+    return res
+
+
+def stored_traffic(kernel, pairs, dtype, config):
+    """ncu dram__bytes_read.sum + dram__bytes_write.sum per launch, from the committed captures."""
+    tpath = os.path.join(ROOT, "profiles", "k_assemble_traffic.csv")
+    if not os.path.exists(tpath):
+        return None, None
+    import csv
+    with open(tpath) as f:
+        for row in csv.DictReader(f):
+            if (row.get("kernel", "k_assemble") == kernel and int(row["pairs"]) == pairs and row["dtype"] == dtype
+                    and int(row.get("config", 4)) == config):
+                return int(row["dram_bytes_per_launch"]), row.get("capture", "profiles/")
+    return None, None
+
+
+def self_spawn(args):
+    """`python bench.py --gpus N` without torchrun: start the N ranks ourselves (replicas only)."""
+    import socket
+    with socket.socket() as so:
+        so.bind(("127.0.0.1", 0))
+        port = so.getsockname()[1]
+    cmd = [sys.executable, "-m", "torch.distributed.run", "--nnodes=1", "--nproc-per-node", str(args.gpus),
+           "--master-addr", "127.0.0.1", "--master-port", str(port), os.path.abspath(__file__)] + sys.argv[1:]
+    raise SystemExit(subprocess.call(cmd))
+
+
 def main():
     args = parse()
     if args.impl == "reference":
@@ -238,6 +385,8 @@ def main():
     if args.broad_phase:
         run_broad_phase(args)
         return
+    if args.gpus > 1 and "WORLD_SIZE" not in os.environ:
+        self_spawn(args)
     import torch
     import torch.distributed as dist
     from paper_2606_06511_b200 import tt
@@ -255,69 +404,11 @@ def main():
     tdt = torch.float64 if args.dtype == "f64" else torch.float32
     w = 8 if args.dtype == "f64" else 4
     pb = make_problem(args, rank, "cuda:%d" % local_rank)
-    pos_np = pb.pos if args.dtype == "f64" else pb.pos.astype(np.float32)
-    pos = torch.from_numpy(pos_np).to(dev)
-    tris = torch.from_numpy(pb.tris).to(dev)
-    pairs = torch.from_numpy(pb.pairs).to(dev)
-    P, nV, nT = pb.n_pairs, pb.n_verts, pb.n_tris
     ctx = tt.Context(tdt, args.hess_mode, 1.0, local_rank)
-    prob = ctx.problem(pos, tris, pairs)
-    stream = torch.cuda.current_stream()
-
-    # sizes are a property of the input: allocate outputs once (a Newton loop would do the same)
-    nnzb, n_active = ctx.tt_hess_symbolic(prob)
-    energy = torch.zeros(1, dtype=tdt, device=dev)
-    grad = torch.empty((nV, 3), dtype=tdt, device=dev)
-    rowptr = torch.empty(nV + 1, dtype=torch.int32, device=dev)
-    colind = torch.empty(max(nnzb, 1), dtype=torch.int32, device=dev)
-    vals = torch.empty((max(nnzb, 1), 3, 3), dtype=tdt, device=dev)
-    pvec = torch.randn((nV, 3), dtype=tdt, device=dev)
-    yvec = torch.empty_like(pvec)
-    log("[bench] rank %d: A=%d nnzb=%d (vals %.2f GB)" % (rank, n_active, nnzb, nnzb * 9 * w / 1e9))
-
-    phase_ev = []                                     # per timed step: 4 events around the three calls
-
-    def step(record=False):
-        ev = [torch.cuda.Event(enable_timing=True) for _ in range(4)] if record else None
-        if record:
-            ev[0].record(stream)
-        ctx.tt_hess_symbolic(prob)
-        if record:
-            ev[1].record(stream)
-        ctx.tt_energy_grad_hess(prob, energy, grad, rowptr, colind, vals, max(nnzb, 1))
-        if record:
-            ev[2].record(stream)
-        ctx.tt_hess_vec(prob, pvec, yvec)
-        if record:
-            ev[3].record(stream)
-            phase_ev.append(ev)
-
-    for _ in range(args.warmup):
-        step()
-    torch.cuda.synchronize()
-    if world > 1:
-        dist.barrier()
-    torch.cuda.synchronize()
-    sampler = ClockSampler(local_rank) if rank == 0 else None
-    l0 = ctx.tt_stats()["launches"]
-    kms = {"classify": [], "assemble": [], "hess_vec": []}
-    ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-    t_wall0 = time.time()
-    ev0.record(stream)
-    for _ in range(args.steps):
-        step(record=True)
-        for k, v in ctx.tt_kernel_ms().items():      # waits for the step's last kernel; no extra work
-            kms[k].append(v)
-    ev1.record(stream)
-    torch.cuda.synchronize()
-    if world > 1:
-        dist.barrier()
-    t_wall1 = time.time()
-    launches = ctx.tt_stats()["launches"] - l0
-    ms_total = ev0.elapsed_time(ev1)
-    ms_total, P_all = aggregate_ranks(ms_total, P, world, dev)
-    clocks = sampler.stop(t_wall0, t_wall1) if sampler else None
-    ms_step = ms_total / args.steps
+    m = measure(ctx, pb, args, dev, args.steps, args.warmup, world, rank, sampler_rank0=(rank == 0))
+    pos_np, pvec = m.pop("tensors")
+    P, nV, nT, nnzb, n_active = m["P"], m["nV"], m["nT"], m["nnzb"], m["n_active"]
+    ms_step, P_all = m["ms_step"], m["P_all"]
     value = P_all / (ms_step * 1e-3)
 
     # ---- e2e through the host-buffer C-ABI call (pinned host memory, copies inside the timed region) ----
@@ -330,8 +421,6 @@ def main():
         g_h = torch.zeros((nV, 3), dtype=tdt).pin_memory()
         p_h = pvec.cpu().pin_memory()
         y_h = torch.zeros((nV, 3), dtype=tdt).pin_memory()
-        del vals, colind                              # the host call keeps its own device BSR
-        torch.cuda.empty_cache()
 
         def host_step():
             return ctx.tt_energy_grad_hess_host(pos_h, tris_h, pairs_h, e_h, g_h, None, None, None, 0, p_h, y_h)
@@ -354,32 +443,49 @@ def main():
         d2h = w + g_h.numel() * w + y_h.numel() * w
         e2e = {"value": P_all / t_e2e, "unit": UNIT, "h2d_bytes_per_step": int(h2d), "d2h_bytes_per_step": int(d2h),
                "ms_per_step": 1e3 * t_e2e, "steps": k2,
-               "note": "tt_energy_grad_hess_host: pinned host pos/tris/pairs/p in; energy, grad, y out; BSR left on device"}
+               "note": "tt_energy_grad_hess_host: pinned host pos/tris/pairs/p in; energy, grad, y out; the BSR "
+                       "(%.2f GB) stays on the device for the PCG that consumes it there (tt_bsr_device / tt_pcg_solve); "
+                       "copying it out too would add %.0f ms at ~55 GB/s PCIe Gen5" % (
+                           nnzb * (9 * w + 4) / 1e9, nnzb * (9 * w + 4) / 55e9 * 1e3)}
+        del pos_h, tris_h, pairs_h, g_h, p_h, y_h
+    del pvec
+
+    # ---- further points of the 1M-50M sweep (config 4, rank 0's replica only; fewer steps) ----
+    sweep = None
+    if args.config == 4 and args.sweep and world == 1:
+        sweep = []
+        ctx.close()
+        torch.cuda.empty_cache()
+        for n_pairs in [int(x) for x in args.sweep.split(",") if x]:
+            if n_pairs == args.pairs:
+                continue
+            pbs = make_problem(args, rank, "cuda:%d" % local_rank, n_pairs)
+            cs = tt.Context(tdt, args.hess_mode, 1.0, local_rank)
+            ms = measure(cs, pbs, args, dev, args.sweep_steps, 3)
+            ms.pop("tensors")
+            sweep.append({"pairs": ms["P"], "n_active": ms["n_active"], "nnzb": ms["nnzb"], "steps": args.sweep_steps,
+                          "ms_per_step": ms["ms_step"], "pairs_per_s": ms["P"] / (ms["ms_step"] * 1e-3),
+                          "k4_ms": ms["k4"]["ms"], "k4_frac": ms["k4"]["frac"], "step_frac": ms["step_frac"],
+                          "phase_ms": ms["phase_ms"], "kernel_ms": ms["kernel_ms"]})
+            cs.close()
+            del pbs
+            torch.cuda.empty_cache()
 
     if rank != 0:
         if world > 1:
             dist.destroy_process_group()
         return
 
-    # ---- roofline of the dominant kernel (k_assemble), DESIGN.md "Roofline" ----
-    hbm, peak_src = peaks()
-    n_touch = ctx.tt_stats()["n_touched_tris"]
-    rows_touched = int((rowptr[1:] != rowptr[:-1]).sum().item())
-    alg_bytes = 9 * w * nnzb + 3 * w * rows_touched + 12 * n_touch + 8 * n_active + 3 * w * 3 * n_touch
-    asm_ms = float(np.mean(kms["assemble"]))
-    achieved = alg_bytes / (asm_ms * 1e-3) / 1e9
-    traffic = None
-    tpath = os.path.join(ROOT, "profiles", "k_assemble_traffic.csv")   # ncu dram bytes per launch, same workload
-    if os.path.exists(tpath):
-        import csv
-        with open(tpath) as f:
-            for row in csv.DictReader(f):
-                if int(row["pairs"]) == args.pairs and row["dtype"] == args.dtype:
-                    traffic = int(row["dram_bytes_per_launch"])
-    roofline = {"bound": "hbm", "kernel": "k_assemble", "achieved": achieved, "peak": hbm, "unit": "GB/s",
-                "frac": achieved / hbm, "traffic": traffic, "peak_source": peak_src,
-                "algorithmic_bytes_per_launch": int(alg_bytes), "kernel_ms": asm_ms,
-                "share_of_step": asm_ms / ms_step}
+    # ---- roofline of the dominant kernel: K4 (assembly) on the sweep; on the mesh configs
+    #      (< 1 % of the candidates active) the step is the classification kernel K1 ----
+    dom = m["k4"] if args.config == 4 else m["k1"]
+    traffic, capture = stored_traffic(dom["call"], args.pairs if args.config == 4 else P, args.dtype, args.config)
+    roofline = {"bound": "hbm", "kernel": dom["call"], "achieved": dom["achieved"], "peak": m["hbm"], "unit": "GB/s",
+                "frac": dom["frac"], "traffic": traffic,
+                "traffic_source": ("stored ncu capture (%s), not measured in this run" % capture) if traffic else None,
+                "peak_source": m["peak_src"], "algorithmic_bytes_per_launch": dom["algorithmic_bytes"],
+                "kernel_ms": dom["ms"], "share_of_step": dom["ms"] / ms_step,
+                "kernel_launches_averaged": m["kernel_launches"]}
 
     cpu = None
     if world == 1 and not args.no_cpu_baseline:
@@ -388,18 +494,20 @@ def main():
     out = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
            "ms_per_step": ms_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
            "dtype": args.dtype, "data": "synthetic",
-           "config": {"workload": "BASELINE configs[4] throughput sweep: %d-triangle random soup, %d candidate pairs, "
-                                  "%.1f%% active, energy+grad+BSR Hessian (+pattern) + one matrix-free H.p per step"
-                                  % (nT, P, 100.0 * n_active / max(P, 1)),
-                      "n_tris": nT, "n_verts": nV, "n_pairs": P, "n_active": n_active, "nnzb": nnzb,
-                      "hess_mode": args.hess_mode, "replicas": world,
-                      "l2": "inputs (%.0f MB) and outputs (%.1f GB) exceed the 126 MB L2; no flush needed" % (
-                          (pos.numel() * w + tris.numel() * 4 + pairs.numel() * 4) / 1e6, nnzb * 9 * w / 1e9)},
-           "roofline": roofline, "cpu_baseline": cpu, "e2e": e2e, "gpu_launches": int(launches),
-           "clocks": clocks,
-           "kernel_ms": {k: float(np.mean(v)) for k, v in kms.items()},
-           "phase_ms": {name: float(np.mean([e[i].elapsed_time(e[i + 1]) for e in phase_ev]))
-                        for i, name in enumerate(("tt_hess_symbolic", "tt_energy_grad_hess", "tt_hess_vec"))},
+           "config": {"workload": "BASELINE %s: %d triangles, %d candidate pairs, %.1f%% active; step = pattern "
+                                  "(tt_hess_symbolic) + energy+grad+BSR Hessian (tt_energy_grad_hess) + one matrix-free H.p "
+                                  "(tt_hess_vec)" % (WORKLOADS[args.config], nT, P, 100.0 * n_active / max(P, 1)),
+                      "config_index": args.config, "n_tris": nT, "n_verts": nV, "n_pairs": P, "n_active": n_active,
+                      "nnzb": nnzb, "hess_mode": args.hess_mode, "replicas": world,
+                      "l2": ("inputs (%.0f MB) and outputs (%.1f GB) exceed the 126 MB L2; no flush needed" % (
+                          m["in_bytes"] / 1e6, nnzb * 9 * w / 1e9)) if m["in_bytes"] + nnzb * 9 * w > 2.0e8 else
+                            "working set fits the L2: every step rewrites the same buffers (L2-resident numbers, stated)"},
+           "roofline": roofline, "roofline_all": m["roofline_all"], "step_frac": m["step_frac"],
+           "step_algorithmic_bytes": m["step_bytes"],
+           "cpu_baseline": cpu, "e2e": e2e, "gpu_launches": m["launches"],
+           "clocks": m["clocks"], "kernel_ms": m["kernel_ms"],
+           "kernel_roofline": {k: {"frac": m[k]["frac"], "algorithmic_bytes": m[k]["algorithmic_bytes"]} for k in ("k1", "k4", "k6")},
+           "phase_ms": m["phase_ms"], "sweep": sweep,
            "active_pairs_per_s": n_active * world / (ms_step * 1e-3)}
     print(json.dumps(out), flush=True)
     if world > 1:

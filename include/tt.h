@@ -2,8 +2,9 @@
  * "Differentiable 3D Triangle-Triangle Intersection Energy".
  *
  * The problem is stated as the paper states it: vertex positions,
- * triangles, and a list of candidate triangle pairs (the broad phase that produces them, L51,
- * is a separate structure and not part of this library).  For every candidate pair (T_a, T_b)
+ * triangles, and a list of candidate triangle pairs.  The candidate list is an INPUT of the hot
+ * path; the broad phase that produces it (L51) is a separate call of this library, tt_broad_phase
+ * below, whose output can be passed straight in.  For every candidate pair (T_a, T_b)
  * that is not topologically adjacent (shares no vertex index, L11):
  *   1. Moeller's intervals I_a, I_b on the planes' intersection line and
  *      I_c = [t_c^0, t_c^1] = [t_a^0 - t_b^1, t_a^1 - t_b^0]            (L9-15, Eq. 1);
@@ -59,7 +60,7 @@ typedef enum {
   TT_ERR_CUDA = -2,        /* a CUDA runtime call failed (message holds cudaGetErrorString)        */
   TT_ERR_NOMEM = -3,       /* workspace allocation failed                                           */
   TT_ERR_CAPACITY = -4,    /* nnzb_capacity smaller than the pattern computed by tt_hess_symbolic   */
-  TT_ERR_STATE = -5        /* numeric / H.p call without a matching tt_hess_symbolic                */
+  TT_ERR_STATE = -5        /* numeric / H.p call without a matching tt_hess_symbolic, or `pos` changed since */
 } tt_status;
 
 typedef enum { TT_F64 = 0, TT_F32 = 1 } tt_dtype;
@@ -88,6 +89,13 @@ typedef struct {
  * TT_ERR_INVALID_ARG with the count in tt_last_error.  Costs one small kernel and one host round
  * trip per call; without the flag out-of-range indices are undefined behaviour (not checked).      */
 #define TT_FLAG_VALIDATE_INDICES 2
+/* tt_energy_grad_hess and tt_hess_vec replay the branch decisions (lone vertex, min/max order,
+ * on-plane flag, active mask) that tt_hess_symbolic recorded at the positions it saw.  By default
+ * both calls re-take a 64-bit checksum of `pos` (one read of the array, ~0.03 ms per 6 M vertices,
+ * plus one short host round trip) and return TT_ERR_STATE if the positions have changed since
+ * tt_hess_symbolic.  This flag skips the check: the caller then guarantees unchanged positions
+ * (tt_pcg_solve checks once per solve, not per product).                                          */
+#define TT_FLAG_NO_STATE_CHECK 4
 
 typedef struct {
   const void* pos;      int64_t n_verts;   /* [nV,3] dtype                                          */
@@ -117,8 +125,9 @@ tt_status tt_hess_symbolic(tt_ctx* ctx, const tt_problem* prob, int64_t* nnzb_ho
                            int64_t* n_active_host, void* stream);
 
 /* Steps 2-4 (Eq. 2-4), numeric phase, on the active set cached by tt_hess_symbolic for
- * the same problem (same pointers and sizes; positions must be unchanged since, else TT_ERR_STATE
- * cannot be detected and the cached active set is evaluated at the new positions).
+ * the same problem (same pointers and sizes, and unchanged positions: TT_ERR_STATE otherwise --
+ * the positions are verified by checksum unless TT_FLAG_NO_STATE_CHECK, which makes this call block
+ * for one short host round trip before its kernels are enqueued).
  *   energy_sum [1] dtype; grad [nV,3] dtype or NULL;
  *   bsr_rowptr [nV+1], bsr_colind [nnzb_capacity], bsr_vals [nnzb_capacity,3,3] dtype -- all
  *   three NULL to skip the Hessian.  TT_ERR_CAPACITY if nnzb_capacity < nnzb.                     */
@@ -127,7 +136,8 @@ tt_status tt_energy_grad_hess(tt_ctx* ctx, const tt_problem* prob, void* energy_
                               int64_t nnzb_capacity, void* stream);
 
 /* Matrix-free y = H p with the same Hessian (Eq. 4, same tt_hess_mode) on the cached active set;
- * never forms a block.  p, y: [nV,3] dtype, p != y.  Needs tt_hess_symbolic first.               */
+ * never forms a block.  p, y: [nV,3] dtype, p != y.  Needs tt_hess_symbolic first, at the same
+ * positions (checked like tt_energy_grad_hess).                                                   */
 tt_status tt_hess_vec(tt_ctx* ctx, const tt_problem* prob, const void* p, void* y, void* stream);
 
 /* End-to-end convenience with HOST buffers: copies pos/tris/pairs host->device (pinned host
@@ -150,8 +160,11 @@ tt_status tt_energy_grad_hess_host(tt_ctx* ctx, const tt_problem* prob, void* en
  * defined by its result: ALL pairs i < j of triangles that share no vertex index and whose
  * axis-aligned bounding boxes, each grown by `inflate` (>= 0) on every side, overlap (closed
  * intervals; bounds in fp64 from the stored positions), in lexicographic order -- i.e. a `pairs`
- * array for tt_problem.  Built on a uniform grid (cell = largest box extent), sort based, no atomics;
- * the result is deterministic and independent of the grid.
+ * array for tt_problem.  Built on a uniform grid, sort based, no atomics.  Cell size =
+ * min(largest box extent, max(2 x mean extent, largest / 4)), raised if needed so that no axis has
+ * more than 32768 cells; a box is registered in every cell it touches (at most 5 per axis) and a pair
+ * is reported only by the cell that owns max(lo_i, lo_j).  The result is deterministic and
+ * independent of the grid.
  *   pos [nV,3] dtype, tris [nT,3] int32: DEVICE, read only.   n_pairs_host HOST [1].
  * The pairs stay in ctx (device memory owned by ctx, valid until the next tt_broad_phase or
  * tt_destroy): tt_broad_phase_pairs returns the view, tt_broad_phase_copy copies them to a caller
@@ -176,6 +189,11 @@ tt_status tt_stats(const tt_ctx* ctx, int64_t* what, int32_t n);
  * large kernels: ms[0] = classification (K1), ms[1] = assembly (K4), ms[2] = H.p (K6); -1 if the
  * kernel has not run.  Blocks until those launches have finished.                                 */
 tt_status tt_kernel_ms(tt_ctx* ctx, float* ms, int32_t n);
+/* The same, averaged over the launches recorded since the last reset (the library keeps the events of
+ * the last 64 launches of each kernel, so a timed loop needs no synchronisation inside it):
+ *   ms HOST [n]: mean duration, -1 if none; launches HOST [n] or NULL: how many were averaged;
+ *   reset != 0 forgets the recorded launches afterwards.  Blocks until those launches have finished. */
+tt_status tt_kernel_ms_mean(tt_ctx* ctx, float* ms, int32_t* launches, int32_t n, int32_t reset);
 
 /* Diagnostic (not on the hot path): measured vector-FMA issue rate of `device`, FMA = 2 flop.
  *   tflops HOST [2]: [0] = fp64 (DFMA), [1] = fp32 (FFMA).  Runs ~10 ms of register-only FMA

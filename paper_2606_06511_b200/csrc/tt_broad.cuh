@@ -76,6 +76,7 @@ k_bp_aabb(const T* __restrict__ pos, const int* __restrict__ tris, int64_t nT, d
 // Cell size: never larger than the largest box (then a box touches <= 2 cells per axis), but when a
 // few boxes are much larger than the rest, 2 x the mean extent, floored at a quarter of the largest
 // (a box then touches <= 5 cells per axis, <= 125 in all): the candidate list does not depend on it.
+constexpr int BP_MAX_DIM = 32768;  // cells per axis: the cell key stays below 2^45
 __global__ void __launch_bounds__(BP_THREADS)
 k_bp_grid(const double* __restrict__ part, int64_t n_part, int64_t nT, Grid* __restrict__ g) {
   __shared__ double s[BP_THREADS][8];
@@ -93,11 +94,17 @@ k_bp_grid(const double* __restrict__ part, int64_t n_part, int64_t nT, Grid* __r
       for (int k = 0; k < 8; ++k) v[k] = (k < 3) ? fmin(v[k], s[i][k]) : ((k < 7) ? fmax(v[k], s[i][k]) : v[k] + s[i][k]);
     const double big = v[6] * 1.0001, mean = v[7] / (double)(nT > 0 ? nT : 1);
     double cell = fmin(big, fmax(2.0 * mean, 0.25 * big));
-    if (!(cell > 0.0)) cell = 1.0;
+    // a sparse scene (domain >> boxes) must not overflow the cell coordinates: at most BP_MAX_DIM cells per
+    // axis (a larger cell only registers a box in fewer cells; the candidate list does not depend on it)
+    for (int c = 0; c < 3; ++c)
+      if (n_part > 0 && v[3 + c] >= v[c]) cell = fmax(cell, (v[3 + c] - v[c]) / (double)(BP_MAX_DIM - 1));
+    if (!(cell > 0.0) || !(cell < 1e300)) cell = 1.0;
     g->inv_cell = 1.0 / cell;
     for (int c = 0; c < 3; ++c) {
       g->org[c] = v[c];
-      g->dims[c] = (n_part > 0 && v[3 + c] >= v[c]) ? (int)floor((v[3 + c] - v[c]) * g->inv_cell) + 1 : 1;
+      double d = (n_part > 0 && v[3 + c] >= v[c]) ? floor((v[3 + c] - v[c]) * g->inv_cell) + 1.0 : 1.0;
+      d = fmin(fmax(d, 1.0), (double)BP_MAX_DIM);   // computed in double: never wraps an int
+      g->dims[c] = (int)d;
     }
     g->pad = 0;
   }

@@ -1866,6 +1866,32 @@ __global__ void k_gather3(const int* __restrict__ vcnt, const int* __restrict__ 
   out[3 * v + 2] = r2;
 }
 
+// Order-independent 64-bit checksum of n 32-bit words (each word mixed with its index, integer adds:
+// associative and commutative, so the result does not depend on the schedule).  tt_hess_symbolic
+// takes it of `pos`; the numeric phase and H.p re-take it and refuse to replay the recorded branch
+// decisions at positions that have moved (TT_ERR_STATE).
+__device__ __forceinline__ unsigned long long mix64(unsigned long long z) {
+  z = (z ^ (z >> 30)) * 0xbf58476d1ce4e5b9ull;
+  z = (z ^ (z >> 27)) * 0x94d049bb133111ebull;
+  return z ^ (z >> 31);
+}
+__global__ void __launch_bounds__(256) k_checksum(const uint32_t* __restrict__ w, int64_t n, unsigned long long* __restrict__ out) {
+  unsigned long long acc = 0ull;
+  const int64_t stride = (int64_t)gridDim.x * 256;
+  const int64_t n4 = ((reinterpret_cast<uintptr_t>(w) & 15) == 0) ? n / 4 : 0;  // 16-byte body when aligned
+  const uint4* w4 = reinterpret_cast<const uint4*>(w);
+  for (int64_t i = (int64_t)blockIdx.x * 256 + threadIdx.x; i < n4; i += stride) {
+    const uint4 v = __ldg(w4 + i);
+    const unsigned long long k = (unsigned long long)i * 0x9e3779b97f4a7c15ull;
+    acc += mix64((((unsigned long long)v.y << 32) | v.x) ^ k) + mix64((((unsigned long long)v.w << 32) | v.z) ^ ~k);
+  }
+  for (int64_t i = 4 * n4 + (int64_t)blockIdx.x * 256 + threadIdx.x; i < n; i += stride)
+    acc += mix64((unsigned long long)__ldg(w + i) ^ ((unsigned long long)i * 0xd1b54a32d192ed03ull));
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) acc += __shfl_down_sync(0xffffffffu, acc, o);
+  if ((threadIdx.x & 31) == 0 && acc) atomicAdd(out, acc);
+}
+
 // TT_FLAG_VALIDATE_INDICES: counts the entries of an index array outside [0, bound)
 __global__ void k_count_out_of_range(const int* __restrict__ idx, int64_t n, int64_t bound, int* __restrict__ bad) {
   const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;

@@ -74,6 +74,7 @@ struct tt_ctx {
   // numeric
   DevBuf everts, rdesc, tfirst, bucket_cnt, bucket_off, long_cnt, long_off, chunk_start, long_list, asm_energy, tvals, tslot, vkeys[2], vvals[2], vptr, vslot1;
   DevBuf cub_tmp;
+  DevBuf possig;  // [2] u64: checksum of pos at tt_hess_symbolic, and at the last numeric / H.p call
   // broad phase (tt_broad_phase): boxes, grid, (cell, triangle) records, pair keys, result
   DevBuf bp_box, bp_part, bp_grid, bp_cnt, bp_off, bp_keys[2], bp_vals[2], bp_pcnt, bp_poff, bp_pkeys[2], bp_pairs;
   int64_t bp_n_pairs = -1;
@@ -92,8 +93,10 @@ struct tt_ctx {
   uint32_t* vvals_sorted = nullptr;
   int64_t host_nnzb = 0;
   // device-side timing of the three big kernels (events recorded on the caller's stream)
-  cudaEvent_t ev[3][2] = {{nullptr, nullptr}, {nullptr, nullptr}, {nullptr, nullptr}};
-  bool ev_used[3] = {false, false, false};
+  // (a ring of EV_RING launches per kernel: tt_kernel_ms reads the latest, tt_kernel_ms_mean all of them)
+  static constexpr int EV_RING = 64;
+  cudaEvent_t evr[3][EV_RING][2] = {};
+  int64_t ev_n[3] = {0, 0, 0};   // launches recorded since the last reset
   // host-buffer entry point: copies that do not feed the next kernel travel on a second stream
   cudaStream_t side = nullptr;
   cudaEvent_t ev_in = nullptr, ev_p = nullptr, ev_num = nullptr, ev_side = nullptr;
@@ -173,6 +176,32 @@ tt_status validate_indices(tt_ctx* ctx, const int32_t* tris, int64_t nT, int64_t
   return TT_OK;
 }
 
+// checksum of pos -> possig[slot] (enqueued on st)
+tt_status pos_checksum(tt_ctx* ctx, const tt_problem* q, int slot, cudaStream_t st) {
+  TT_CUDA(ctx->possig.ensure(sizeof(unsigned long long) * 2));
+  unsigned long long* d = ctx->possig.as<unsigned long long>() + slot;
+  TT_CUDA(cudaMemsetAsync(d, 0, sizeof(unsigned long long), st));
+  const int64_t words = 3 * q->n_verts * (ctx->opt.dtype == TT_F64 ? 2 : 1);
+  if (words > 0) {
+    const int64_t want = (words / 4 + 255) / 256;
+    ttk::k_checksum<<<(unsigned)(want < 148 * 8 ? (want > 0 ? want : 1) : 148 * 8), 256, 0, st>>>((const uint32_t*)q->pos, words, d);
+    TT_LAUNCH_CHECK();
+  }
+  return TT_OK;
+}
+// TT_ERR_STATE unless pos still has the checksum tt_hess_symbolic took (one short host round trip)
+tt_status check_positions(tt_ctx* ctx, const tt_problem* q, const char* who, cudaStream_t st) {
+  if (ctx->opt.flags & TT_FLAG_NO_STATE_CHECK) return TT_OK;
+  tt_status s = pos_checksum(ctx, q, 1, st);
+  if (s != TT_OK) return s;
+  unsigned long long sig[2] = {0ull, 0ull};
+  TT_CUDA(cudaMemcpyAsync(sig, ctx->possig.p, sizeof(sig), cudaMemcpyDeviceToHost, st));
+  TT_CUDA(cudaStreamSynchronize(st));
+  if (sig[0] != sig[1])
+    return fail(ctx, TT_ERR_STATE, "%s: positions changed since tt_hess_symbolic (the cached active set and branch decisions are stale): call tt_hess_symbolic again", who);
+  return TT_OK;
+}
+
 // exclusive sum of n ints (+ grand total in out[n]); `in` must have n+1 entries with in[n] == 0
 tt_status scan_i32(tt_ctx* ctx, const int* in, int* out, int64_t n_plus_1, cudaStream_t st) {
   size_t tmp = 0;
@@ -238,13 +267,14 @@ tt_status run_classify(tt_ctx* ctx, const tt_problem* q, T* e_pp, T* tc, bool re
   if (record) TT_CUDA(ctx->cfg.ensure(sizeof(uint16_t) * (size_t)(P + 1)));
   TT_CUDA(cudaMemsetAsync(ctx->blk_count.as<int>() + nblk, 0, sizeof(int), st));
   if (nblk > 0) {
-    TT_CUDA(cudaEventRecord(ctx->ev[0][0], st));
+    cudaEvent_t* ev_k1 = ctx->evr[0][ctx->ev_n[0] % tt_ctx::EV_RING];
+    TT_CUDA(cudaEventRecord(ev_k1[0], st));
     ttk::k_classify<T><<<(unsigned)nblk, ttk::CLS_THREADS, 0, st>>>(
         (const T*)q->pos, q->tris, (const int2*)q->pairs, P, ctx->opt.tc_scale, ctx->mask.as<uint32_t>(),
         ctx->blk_count.as<int>(), ctx->blk_energy.as<double>(), e_pp, tc, record ? ctx->cfg.as<uint16_t>() : nullptr);
     TT_LAUNCH_CHECK();
-    TT_CUDA(cudaEventRecord(ctx->ev[0][1], st));
-    ctx->ev_used[0] = true;
+    TT_CUDA(cudaEventRecord(ev_k1[1], st));
+    ctx->ev_n[0]++;
   }
   tt_status s = scan_i32(ctx, ctx->blk_count.as<int>(), ctx->blk_off.as<int>(), nblk + 1, st);
   if (s != TT_OK) return s;
@@ -296,6 +326,8 @@ tt_status symbolic_impl(tt_ctx* ctx, const tt_problem* q, int64_t* nnzb_host, in
   const int64_t P = q->n_pairs, nT = q->n_tris, nV = q->n_verts;
   int64_t nblk = 0;
   tt_status s = validate_indices(ctx, q->tris, nT, nV, q->pairs, P, st);
+  if (s != TT_OK) return s;
+  s = pos_checksum(ctx, q, 0, st);
   if (s != TT_OK) return s;
   s = run_classify<T>(ctx, q, nullptr, nullptr, true, st, &nblk);
   if (s != TT_OK) return s;
@@ -613,7 +645,8 @@ tt_status numeric_impl(tt_ctx* ctx, const tt_problem* q, void* energy_sum, void*
   AsmParams<T> p = make_params<T>(ctx, q);
   p.vals = (T*)vals;
   if (ctx->n_chunks > 0) {
-    TT_CUDA(cudaEventRecord(ctx->ev[1][0], st));
+    cudaEvent_t* ev_k4 = ctx->evr[1][ctx->ev_n[1] % tt_ctx::EV_RING];
+    TT_CUDA(cudaEventRecord(ev_k4[0], st));
     if (want_h) {
       const size_t smem = sizeof(TileWarpSmem<T>) * TILE_WARPS;
       const int64_t full = (ctx->n_chunks + TILE_WARPS - 1) / TILE_WARPS;
@@ -635,8 +668,8 @@ tt_status numeric_impl(tt_ctx* ctx, const tt_problem* q, void* energy_sum, void*
       if (s1 != TT_OK) return s1;
     }
     TT_LAUNCH_CHECK();
-    TT_CUDA(cudaEventRecord(ctx->ev[1][1], st));
-    ctx->ev_used[1] = true;
+    TT_CUDA(cudaEventRecord(ev_k4[1], st));
+    ctx->ev_n[1]++;
     if (want_h && ctx->U > 0) {
       k_merge<T><<<grid_for(9 * ctx->U, 256), 256, 0, st>>>(ctx->run_start.as<int>(), ctx->run_dest.as<int>(),
                                                             ctx->rvals_sorted, ctx->U, ctx->tvals.as<T>(), (T*)vals);
@@ -657,11 +690,12 @@ tt_status hessvec_impl(tt_ctx* ctx, const tt_problem* q, const void* pvec, void*
   p.pvec = (const T*)pvec;
   p.chunk_energy = nullptr;
   if (ctx->n_chunks > 0) {
-    TT_CUDA(cudaEventRecord(ctx->ev[2][0], st));
+    cudaEvent_t* ev_k6 = ctx->evr[2][ctx->ev_n[2] % tt_ctx::EV_RING];
+    TT_CUDA(cudaEventRecord(ev_k6[0], st));
     tt_status s1 = launch_entry_reduce<T, 2>(ctx, p, st);
     if (s1 != TT_OK) return s1;
-    TT_CUDA(cudaEventRecord(ctx->ev[2][1], st));
-    ctx->ev_used[2] = true;
+    TT_CUDA(cudaEventRecord(ev_k6[1], st));
+    ctx->ev_n[2]++;
   }
   if (q->n_verts > 0) {
     k_gather3<T><<<grid_for(q->n_verts, 256), 256, 0, st>>>(ctx->vcnt.as<int>(), ctx->vslot1.as<int>(), ctx->vptr.as<int>(), ctx->vvals_sorted, q->n_verts,
@@ -708,6 +742,9 @@ tt_status broad_impl(tt_ctx* ctx, const void* pos, int64_t nV, const int32_t* tr
   TT_CUDA(cudaMemcpyAsync(&g, ctx->bp_grid.p, sizeof(Grid), cudaMemcpyDeviceToHost, st));
   TT_CUDA(cudaStreamSynchronize(st));
   const int64_t n_rec = n_rec32;
+  for (int c = 0; c < 3; ++c)
+    if (g.dims[c] <= 0 || g.dims[c] > ttb::BP_MAX_DIM)
+      return fail(ctx, TT_ERR_INVALID_ARG, "broad phase: invalid grid dimension %d (non-finite positions?)", g.dims[c]);
   const double n_cells = (double)g.dims[0] * (double)g.dims[1] * (double)g.dims[2];
   if (n_cells >= 1.0e14) return fail(ctx, TT_ERR_INVALID_ARG, "broad phase: grid of %d x %d x %d cells exceeds 47-bit cell keys", g.dims[0], g.dims[1], g.dims[2]);
   int cell_bits = 1;
@@ -778,8 +815,9 @@ tt_status tt_create(const tt_options* opt, tt_ctx** out) {
   if (!c) return TT_ERR_NOMEM;
   c->opt = *opt;
   for (int i = 0; i < 3; ++i)
-    for (int j = 0; j < 2; ++j)
-      if (cudaEventCreate(&c->ev[i][j]) != cudaSuccess) { delete c; return TT_ERR_CUDA; }
+    for (int r = 0; r < tt_ctx::EV_RING; ++r)
+      for (int j = 0; j < 2; ++j)
+        if (cudaEventCreate(&c->evr[i][r][j]) != cudaSuccess) { (void)cudaGetLastError(); tt_destroy(c); return TT_ERR_CUDA; }
   if (cudaStreamCreateWithFlags(&c->side, cudaStreamNonBlocking) != cudaSuccess ||
       cudaEventCreateWithFlags(&c->ev_in, cudaEventDisableTiming) != cudaSuccess ||
       cudaEventCreateWithFlags(&c->ev_p, cudaEventDisableTiming) != cudaSuccess ||
@@ -827,8 +865,9 @@ void tt_destroy(tt_ctx* ctx) {
   if (!ctx) return;
   cudaSetDevice(ctx->opt.device);
   for (int i = 0; i < 3; ++i)
-    for (int j = 0; j < 2; ++j)
-      if (ctx->ev[i][j]) cudaEventDestroy(ctx->ev[i][j]);
+    for (int r = 0; r < tt_ctx::EV_RING; ++r)
+      for (int j = 0; j < 2; ++j)
+        if (ctx->evr[i][r][j]) cudaEventDestroy(ctx->evr[i][r][j]);
   for (cudaEvent_t e : {ctx->ev_in, ctx->ev_p, ctx->ev_num, ctx->ev_side})
     if (e) cudaEventDestroy(e);
   if (ctx->side) cudaStreamDestroy(ctx->side);
@@ -866,6 +905,8 @@ tt_status tt_energy_grad_hess(tt_ctx* ctx, const tt_problem* prob, void* energy_
   if (!ctx->sig.matches(prob)) return fail(ctx, TT_ERR_STATE, "tt_energy_grad_hess: no matching tt_hess_symbolic for this problem");
   TT_CUDA(cudaSetDevice(ctx->opt.device));
   cudaStream_t st = (cudaStream_t)stream;
+  s = check_positions(ctx, prob, "tt_energy_grad_hess", st);
+  if (s != TT_OK) return s;
   return ctx->opt.dtype == TT_F64
              ? numeric_impl<double>(ctx, prob, energy_sum, grad, bsr_rowptr, bsr_colind, bsr_vals, nnzb_capacity, st)
              : numeric_impl<float>(ctx, prob, energy_sum, grad, bsr_rowptr, bsr_colind, bsr_vals, nnzb_capacity, st);
@@ -878,19 +919,18 @@ tt_status tt_hess_vec(tt_ctx* ctx, const tt_problem* prob, const void* p, void* 
   if (!ctx->sig.matches(prob)) return fail(ctx, TT_ERR_STATE, "tt_hess_vec: no matching tt_hess_symbolic for this problem");
   TT_CUDA(cudaSetDevice(ctx->opt.device));
   cudaStream_t st = (cudaStream_t)stream;
+  s = check_positions(ctx, prob, "tt_hess_vec", st);
+  if (s != TT_OK) return s;
   return ctx->opt.dtype == TT_F64 ? hessvec_impl<double>(ctx, prob, p, y, st) : hessvec_impl<float>(ctx, prob, p, y, st);
 }
 
-tt_status tt_energy_grad_hess_host(tt_ctx* ctx, const tt_problem* prob, void* energy_host, void* grad_host,
-                                   int64_t* nnzb_host, int64_t* n_active_host, int32_t* rowptr_host,
-                                   int32_t* colind_host, void* vals_host, int64_t nnzb_capacity,
-                                   const void* p_host, void* y_host, void* stream) {
-  tt_status s = check_problem(ctx, prob);
-  if ((p_host == nullptr) != (y_host == nullptr)) return fail(ctx, TT_ERR_INVALID_ARG, "p_host and y_host must both be set or both NULL");
-  if (s != TT_OK) return s;
-  if (!energy_host || !nnzb_host) return fail(ctx, TT_ERR_INVALID_ARG, "energy_host / nnzb_host is NULL");
-  TT_CUDA(cudaSetDevice(ctx->opt.device));
-  cudaStream_t st = (cudaStream_t)stream;
+namespace {
+// body of tt_energy_grad_hess_host; the wrapper below drains both streams on ANY failure, so that no
+// copy from / into the caller's host buffers is still in flight when an error is returned
+tt_status host_impl(tt_ctx* ctx, const tt_problem* prob, void* energy_host, void* grad_host, int64_t* nnzb_host,
+                    int64_t* n_active_host, int32_t* rowptr_host, int32_t* colind_host, void* vals_host,
+                    int64_t nnzb_capacity, const void* p_host, void* y_host, cudaStream_t st) {
+  tt_status s = TT_OK;
   const size_t w = ctx->opt.dtype == TT_F64 ? 8 : 4;
   const int64_t nV = prob->n_verts, nT = prob->n_tris, P = prob->n_pairs;
   TT_CUDA(ctx->h_pos.ensure(w * 3 * (size_t)nV + 16));
@@ -922,22 +962,20 @@ tt_status tt_energy_grad_hess_host(tt_ctx* ctx, const tt_problem* prob, void* en
   d.pairs = ctx->h_pairs.as<int32_t>();
   int64_t nnzb = 0, A = 0;
   s = ctx->opt.dtype == TT_F64 ? symbolic_impl<double>(ctx, &d, &nnzb, &A, st) : symbolic_impl<float>(ctx, &d, &nnzb, &A, st);
-  if (s != TT_OK) { cudaStreamSynchronize(ctx->side); return s; }
+  if (s != TT_OK) return s;
   *nnzb_host = nnzb;
   if (n_active_host) *n_active_host = A;
-  if ((colind_host || vals_host) && nnzb_capacity < nnzb) {
-    cudaStreamSynchronize(ctx->side);
-    cudaStreamSynchronize(st);
+  if ((colind_host || vals_host) && nnzb_capacity < nnzb)
     return fail(ctx, TT_ERR_CAPACITY, "nnzb_capacity %lld < nnzb %lld", (long long)nnzb_capacity, (long long)nnzb);
-  }
   TT_CUDA(ctx->o_vals.ensure(w * 9 * (size_t)nnzb + 16));
   // H.p first: it needs only the symbolic phase and p, and its result then leaves (side stream)
-  // under the numeric phase; the numeric results leave last.
+  // under the numeric phase; the numeric results leave last.  (The positions are the ctx-owned copy
+  // made above: no state check needed.)
   if (want_hv) {
     TT_CUDA(cudaStreamWaitEvent(st, ctx->ev_p, 0));
     s = ctx->opt.dtype == TT_F64 ? hessvec_impl<double>(ctx, &d, ctx->h_p.p, ctx->o_y.p, st)
                                  : hessvec_impl<float>(ctx, &d, ctx->h_p.p, ctx->o_y.p, st);
-    if (s != TT_OK) { cudaStreamSynchronize(ctx->side); return s; }
+    if (s != TT_OK) return s;
     TT_CUDA(cudaEventRecord(ctx->ev_num, st));
     TT_CUDA(cudaStreamWaitEvent(ctx->side, ctx->ev_num, 0));
     TT_CUDA(cudaMemcpyAsync(y_host, ctx->o_y.p, w * 3 * (size_t)nV, cudaMemcpyDeviceToHost, ctx->side));
@@ -945,7 +983,7 @@ tt_status tt_energy_grad_hess_host(tt_ctx* ctx, const tt_problem* prob, void* en
   s = ctx->opt.dtype == TT_F64
           ? numeric_impl<double>(ctx, &d, ctx->o_energy.p, ctx->o_grad.p, ctx->rowptr.as<int>(), ctx->colind.as<int>(), ctx->o_vals.p, nnzb, st)
           : numeric_impl<float>(ctx, &d, ctx->o_energy.p, ctx->o_grad.p, ctx->rowptr.as<int>(), ctx->colind.as<int>(), ctx->o_vals.p, nnzb, st);
-  if (s != TT_OK) { cudaStreamSynchronize(ctx->side); return s; }
+  if (s != TT_OK) return s;
   ctx->host_nnzb = nnzb;
   TT_CUDA(cudaMemcpyAsync(energy_host, ctx->o_energy.p, w, cudaMemcpyDeviceToHost, st));
   if (grad_host && nV) TT_CUDA(cudaMemcpyAsync(grad_host, ctx->o_grad.p, w * 3 * (size_t)nV, cudaMemcpyDeviceToHost, st));
@@ -956,6 +994,27 @@ tt_status tt_energy_grad_hess_host(tt_ctx* ctx, const tt_problem* prob, void* en
   TT_CUDA(cudaStreamWaitEvent(st, ctx->ev_side, 0));  // `stream` completes only after the side copies
   TT_CUDA(cudaStreamSynchronize(st));
   return TT_OK;
+}
+}  // namespace
+
+tt_status tt_energy_grad_hess_host(tt_ctx* ctx, const tt_problem* prob, void* energy_host, void* grad_host,
+                                   int64_t* nnzb_host, int64_t* n_active_host, int32_t* rowptr_host,
+                                   int32_t* colind_host, void* vals_host, int64_t nnzb_capacity,
+                                   const void* p_host, void* y_host, void* stream) {
+  tt_status s = check_problem(ctx, prob);
+  if (s != TT_OK) return s;
+  if ((p_host == nullptr) != (y_host == nullptr)) return fail(ctx, TT_ERR_INVALID_ARG, "p_host and y_host must both be set or both NULL");
+  if (!energy_host || !nnzb_host) return fail(ctx, TT_ERR_INVALID_ARG, "energy_host / nnzb_host is NULL");
+  TT_CUDA(cudaSetDevice(ctx->opt.device));
+  cudaStream_t st = (cudaStream_t)stream;
+  s = host_impl(ctx, prob, energy_host, grad_host, nnzb_host, n_active_host, rowptr_host, colind_host, vals_host,
+                nnzb_capacity, p_host, y_host, st);
+  if (s != TT_OK) {  // no DMA from / into the caller's buffers may outlive a failed call
+    (void)cudaStreamSynchronize(ctx->side);
+    (void)cudaStreamSynchronize(st);
+    (void)cudaGetLastError();
+  }
+  return s;
 }
 
 tt_status tt_broad_phase(tt_ctx* ctx, const void* pos, int64_t n_verts, const int32_t* tris, int64_t n_tris,
@@ -1014,10 +1073,32 @@ tt_status tt_kernel_ms(tt_ctx* ctx, float* ms, int32_t n) {
   if (!ctx || !ms || n < 0) return TT_ERR_INVALID_ARG;
   for (int i = 0; i < n && i < 3; ++i) {
     ms[i] = -1.0f;
-    if (!ctx->ev_used[i]) continue;
-    TT_CUDA(cudaEventSynchronize(ctx->ev[i][1]));
-    TT_CUDA(cudaEventElapsedTime(&ms[i], ctx->ev[i][0], ctx->ev[i][1]));
+    if (ctx->ev_n[i] == 0) continue;
+    cudaEvent_t* e = ctx->evr[i][(ctx->ev_n[i] - 1) % tt_ctx::EV_RING];
+    TT_CUDA(cudaEventSynchronize(e[1]));
+    TT_CUDA(cudaEventElapsedTime(&ms[i], e[0], e[1]));
   }
+  return TT_OK;
+}
+
+tt_status tt_kernel_ms_mean(tt_ctx* ctx, float* ms, int32_t* launches, int32_t n, int32_t reset) {
+  if (!ctx || !ms || n < 0) return TT_ERR_INVALID_ARG;
+  for (int i = 0; i < n && i < 3; ++i) {
+    ms[i] = -1.0f;
+    const int64_t cnt = ctx->ev_n[i] < tt_ctx::EV_RING ? ctx->ev_n[i] : tt_ctx::EV_RING;
+    if (launches) launches[i] = (int32_t)cnt;
+    if (cnt == 0) continue;
+    double tot = 0.0;
+    for (int64_t k = 0; k < cnt; ++k) {
+      cudaEvent_t* e = ctx->evr[i][(ctx->ev_n[i] - 1 - k) % tt_ctx::EV_RING];
+      float t = 0.0f;
+      TT_CUDA(cudaEventSynchronize(e[1]));
+      TT_CUDA(cudaEventElapsedTime(&t, e[0], e[1]));
+      tot += t;
+    }
+    ms[i] = (float)(tot / (double)cnt);
+  }
+  if (reset) ctx->ev_n[0] = ctx->ev_n[1] = ctx->ev_n[2] = 0;
   return TT_OK;
 }
 

@@ -20,9 +20,10 @@ TT_F64, TT_F32 = 0, 1
 TT_HESS_EQ4, TT_HESS_FILTER, TT_HESS_PSD2, TT_HESS_PSDPROJ = 0, 1, 2, 3
 TT_FLAG_FORCE_GENERAL_ROWS = 1
 TT_FLAG_VALIDATE_INDICES = 2
+TT_FLAG_NO_STATE_CHECK = 4
 
 EXPORTS = ["tt_create", "tt_destroy", "tt_energy", "tt_hess_symbolic", "tt_energy_grad_hess", "tt_hess_vec",
-           "tt_energy_grad_hess_host", "tt_broad_phase", "tt_broad_phase_pairs", "tt_broad_phase_copy", "tt_bsr_device", "tt_stats", "tt_kernel_ms", "tt_probe_peaks", "tt_status_string", "tt_last_error"]
+           "tt_energy_grad_hess_host", "tt_broad_phase", "tt_broad_phase_pairs", "tt_broad_phase_copy", "tt_bsr_device", "tt_stats", "tt_kernel_ms", "tt_kernel_ms_mean", "tt_probe_peaks", "tt_status_string", "tt_last_error"]
 
 
 class TTOptions(ctypes.Structure):
@@ -81,6 +82,9 @@ def load_library():
     lib.tt_stats.restype = ctypes.c_int
     lib.tt_kernel_ms.argtypes = [vp, ctypes.POINTER(ctypes.c_float), ctypes.c_int32]
     lib.tt_kernel_ms.restype = ctypes.c_int
+    lib.tt_kernel_ms_mean.argtypes = [vp, ctypes.POINTER(ctypes.c_float), ctypes.POINTER(ctypes.c_int32), ctypes.c_int32,
+                                      ctypes.c_int32]
+    lib.tt_kernel_ms_mean.restype = ctypes.c_int
     lib.tt_probe_peaks.argtypes = [ctypes.c_int32, ctypes.POINTER(ctypes.c_double)]
     lib.tt_probe_peaks.restype = ctypes.c_int
     lib.tt_status_string.argtypes = [ctypes.c_int]
@@ -194,6 +198,14 @@ class Context:
         arr = (ctypes.c_float * 3)()
         self._check(self.lib.tt_kernel_ms(self.h, arr, 3))
         return dict(classify=float(arr[0]), assemble=float(arr[1]), hess_vec=float(arr[2]))
+
+    def tt_kernel_ms_mean(self, reset=False):
+        """Mean duration of the launches recorded since the last reset: (dict of ms, dict of launch counts)."""
+        arr = (ctypes.c_float * 3)()
+        cnt = (ctypes.c_int32 * 3)()
+        self._check(self.lib.tt_kernel_ms_mean(self.h, arr, cnt, 3, 1 if reset else 0))
+        names = ("classify", "assemble", "hess_vec")
+        return {k: float(arr[i]) for i, k in enumerate(names)}, {k: int(cnt[i]) for i, k in enumerate(names)}
 
     def tt_stats(self):
         arr = (ctypes.c_int64 * 8)()

@@ -94,7 +94,11 @@ def test_full_size_sampled(oracle_mod):
 
 
 def test_pairs_feed_the_hot_path(oracle_mod):
-    """The device list goes straight into tt_problem: energy of the broad phase's candidates == oracle."""
+    """The device list goes into tt_problem: energy of the broad phase's candidates == oracle.  The
+    broad phase (unlike the generators) applies no margins, so the pairs within the G-margins of a
+    discrete decision are dropped from BOTH sides first: the exact active count
+    is only demanded of pairs the bit-exactness contract covers."""
+    from helpers import filter_margins
     from paper_2606_06511_b200 import inputs, tt
     dev = torch.device("cuda:0")
     pb = inputs.config1_icospheres()
@@ -102,12 +106,20 @@ def test_pairs_feed_the_hot_path(oracle_mod):
     pos = torch.from_numpy(pb.pos).to(dev)
     tris = torch.from_numpy(pb.tris).to(dev)
     pairs = ctx.tt_broad_phase(pos, tris, 0.02)
+    cand = oracle_mod.broad_phase(pb.pos, pb.tris, 0.02)
+    assert (pairs.cpu().numpy() == cand).all()
+    _, degenerate = inputs.classify_pairs(pb.pos, pb.tris, cand, 1e-6)
+    kept = filter_margins(oracle_mod, inputs.Problem(pb.pos, pb.tris, np.ascontiguousarray(cand[~degenerate])), 1)
+    key = cand[:, 0].astype(np.int64) * pb.n_tris + cand[:, 1]
+    keep = np.isin(key, kept[:, 0].astype(np.int64) * pb.n_tris + kept[:, 1])
+    assert keep.sum() == kept.shape[0] and keep.sum() > 0.9 * cand.shape[0]
+    pairs = pairs[torch.from_numpy(keep).to(dev)].contiguous()      # still the broad phase's device array
     prob = ctx.problem(pos, tris, pairs)
     e = torch.zeros(1, dtype=torch.float64, device=dev)
     na = torch.zeros(1, dtype=torch.int64, device=dev)
     ctx.tt_energy(prob, e, None, None, None, na)
     torch.cuda.synchronize()
-    ref = oracle_mod.pairs(pb.pos, pb.tris, oracle_mod.broad_phase(pb.pos, pb.tris, 0.02), 1.0, want_J=False)
+    ref = oracle_mod.pairs(pb.pos, pb.tris, kept, 1.0, want_J=False)
     assert int(na.cpu()[0]) == int(ref["active"].sum())
     assert abs(float(e.cpu()[0]) - ref["T"].sum()) <= 1e-9 * ref["T"].sum()
     ctx.close()

@@ -5,7 +5,8 @@ fp32 variant 1e-4 / 1e-3."""
 import numpy as np
 import pytest
 
-from helpers import filter_margins, rel, unpack_mask
+from helpers import (ROW_TOL, filter_margins, grad_row_scale, hp_row_scale, max_block_err, max_row_err, rel,
+                     unpack_mask)
 
 torch = pytest.importorskip("torch")
 pytestmark = pytest.mark.gpu
@@ -62,11 +63,17 @@ def run_case(oracle, pb, dtype="f64", hess_mode=1, sigma=1.0, flags=0, check_val
     assert out["n_active"] == int(act_ref.sum())
     assert rel(out["energy"].cpu().numpy()[0], ref["energy"]) <= tol["e"]
     assert rel(out["grad"].cpu().numpy(), ref["grad"]) <= tol["g"]
+    rt = ROW_TOL[dtype]
+    nV = pos_np.shape[0]
+    # every gradient row against ITS OWN contribution scale (a wrong small row cannot hide in the global norm)
+    assert max_row_err(out["grad"].cpu().numpy(), ref["grad"], grad_row_scale(nV, pb.tris, pairs, ref)) <= rt["g"]
     assert out["nnzb"] == ref["nnzb"]
     assert (out["rowptr"].cpu().numpy() == ref["rowptr"]).all()
     assert (out["colind"].cpu().numpy() == ref["colind"]).all()
     if check_vals:
         assert rel(out["vals"].cpu().numpy(), ref["vals"]) <= tol["h"]
+        # every block against its own norm (+ 1e-3 of its row's): one mis-scattered block fails here
+        assert max_block_err(out["vals"].cpu().numpy(), ref["vals"], ref["rowptr"]) <= rt["h"]
     # gradient-only call must agree with the full call
     e2 = torch.zeros(1, dtype=tdt, device=dev)
     g2 = torch.empty_like(out["grad"])
@@ -86,6 +93,7 @@ def run_case(oracle, pb, dtype="f64", hess_mode=1, sigma=1.0, flags=0, check_val
     torch.cuda.synchronize()
     y_ref = oracle.hess_vec_pairs(pos_np.shape[0], pb.tris, pairs, ref["active"], ref["tc"], ref["J"], p_np, hess_mode)
     assert rel(y.cpu().numpy(), y_ref) <= tol["y"]
+    assert max_row_err(y.cpu().numpy(), y_ref, hp_row_scale(ref["rowptr"], ref["colind"], ref["vals"], p_np)) <= rt["y"]
     y_bsr = oracle.bsr_matvec(out["rowptr"].cpu().numpy(), out["colind"].cpu().numpy(),
                               out["vals"].cpu().numpy().astype(np.float64), p_np)
     assert rel(y_bsr, y_ref) <= tol["y"]
@@ -156,9 +164,10 @@ def test_config1_icospheres(oracle_mod, dtype):
     assert out["n_active"] > 100 and st["blocks_merged"] > 0
 
 
-def test_config2_cloth(oracle_mod):
+@pytest.mark.parametrize("dtype", ["f64", "f32"])
+def test_config2_cloth(oracle_mod, dtype):
     from paper_2606_06511_b200 import inputs
-    ref, out, st = run_case(oracle_mod, inputs.config2_cloth(), "f64", 1)
+    ref, out, st = run_case(oracle_mod, inputs.config2_cloth(), dtype, 1)
     assert out["n_active"] > 1000
 
 
@@ -281,6 +290,57 @@ def test_error_paths(oracle_mod):
     ctx.tt_energy_grad_hess(prob, e, g, rp, ci, va, nnzb)   # still usable after errors
     torch.cuda.synchronize()
     ctx.close()
+
+
+def test_positions_moved_after_symbolic(oracle_mod):
+    """K4 / K6 replay the branch decisions recorded by tt_hess_symbolic.  A Newton or
+    line-search update of `pos` IN PLACE (same pointer) must not be evaluated with the stale decisions:
+    tt_energy_grad_hess and tt_hess_vec return TT_ERR_STATE until tt_hess_symbolic is called again, and the
+    result then equals the oracle at the NEW positions."""
+    from paper_2606_06511_b200 import inputs, tt
+    dev = _dev()
+    pb = inputs.config0_soup()
+    ctx = tt.Context(torch.float64, 1, 1.0, 0)
+    pos = torch.from_numpy(pb.pos).to(dev)
+    tris = torch.from_numpy(pb.tris).to(dev)
+    prs = torch.from_numpy(pb.pairs).to(dev)
+    prob = ctx.problem(pos, tris, prs)
+    nnzb, _ = ctx.tt_hess_symbolic(prob)
+    e = torch.zeros(1, dtype=torch.float64, device=dev)
+    g = torch.zeros_like(pos)
+    ctx.tt_energy_grad_hess(prob, e, g)                       # unchanged positions: fine
+    saved = pos.clone()
+    pos += 0.05 * torch.from_numpy(np.random.default_rng(3).normal(size=pb.pos.shape)).to(dev)   # in place
+    with pytest.raises(tt.TTError) as ei:
+        ctx.tt_energy_grad_hess(prob, e, g)
+    assert ei.value.status == -5 and "positions changed" in str(ei.value)
+    with pytest.raises(tt.TTError) as ei:
+        ctx.tt_hess_vec(prob, g, torch.empty_like(g))
+    assert ei.value.status == -5
+    pos.copy_(saved)                                           # bit-identical positions again: accepted
+    ctx.tt_energy_grad_hess(prob, e, g)
+    pos[7, 2] += 1e-13                                         # one changed value (a few ulps) is enough
+    with pytest.raises(tt.TTError):
+        ctx.tt_energy_grad_hess(prob, e, g)
+    # re-running the symbolic phase at the new positions gives the oracle's result there
+    pos += 0.05 * torch.from_numpy(np.random.default_rng(4).normal(size=pb.pos.shape)).to(dev)
+    pb2 = inputs.Problem(pos.cpu().numpy(), pb.tris, pb.pairs, "moved", {})
+    pairs2 = filter_margins(oracle_mod, pb2, 1)
+    ref = oracle_mod.assemble(pb2.pos, pb2.tris, pairs2, 1.0, 1)
+    out = tt.assemble(ctx, pos, tris, torch.from_numpy(pairs2).to(dev))
+    torch.cuda.synchronize()
+    assert out["n_active"] == int(ref["active"].sum()) and out["nnzb"] == ref["nnzb"]
+    assert rel(out["grad"].cpu().numpy(), ref["grad"]) <= 1e-10
+    assert rel(out["vals"].cpu().numpy(), ref["vals"]) <= 1e-9
+    # TT_FLAG_NO_STATE_CHECK: the caller vouches for the positions, no check is made
+    ctx2 = tt.Context(torch.float64, 1, 1.0, 0, tt.TT_FLAG_NO_STATE_CHECK)
+    prob2 = ctx2.problem(pos, tris, prs)
+    ctx2.tt_hess_symbolic(prob2)
+    pos[0, 0] += 1e-9
+    ctx2.tt_energy_grad_hess(prob2, e, g)
+    torch.cuda.synchronize()
+    ctx.close()
+    ctx2.close()
 
 
 def test_validate_indices_flag(oracle_mod):
