@@ -62,6 +62,11 @@ def _load():
         lib.tt_oracle_bsr_matvec.restype = None
         lib.tt_oracle_broad_phase.argtypes = [c_dp, c_ip, i64, ctypes.c_double, c_ip, i64]
         lib.tt_oracle_broad_phase.restype = i64
+        lib.tt_oracle_block_jacobi.argtypes = [i64, c_ip, c_ip, c_dp, ctypes.c_double, c_dp]
+        lib.tt_oracle_block_jacobi.restype = None
+        lib.tt_oracle_pcg.argtypes = [i64, c_ip, c_ip, c_dp, ctypes.c_double, c_dp, c_dp, i64, ctypes.c_double,
+                                      c_dp, c_dp, c_dp]
+        lib.tt_oracle_pcg.restype = i64
         lib.tt_oracle_max_threads.argtypes = []
         lib.tt_oracle_max_threads.restype = ctypes.c_int
         _lib = lib
@@ -191,3 +196,35 @@ def bsr_matvec(rowptr, colind, vals, p):
     vals = _f64(vals) if len(vals) else np.zeros((1, 3, 3))
     lib.tt_oracle_bsr_matvec(nV, _ip(rowptr), _ip(colind), _dp(vals), _dp(p), _dp(y))
     return y
+
+
+def block_jacobi(rowptr, colind, vals, shift: float = 0.0):
+    """Inverses of the 3x3 diagonal blocks of (H + shift I): [nV,3,3]."""
+    lib = _load()
+    rowptr = _i32(rowptr)
+    nV = rowptr.shape[0] - 1
+    colind = _i32(colind) if len(colind) else np.zeros(1, dtype=np.int32)
+    vals = _f64(vals) if len(vals) else np.zeros((1, 3, 3))
+    minv = np.zeros((nV, 3, 3))
+    lib.tt_oracle_block_jacobi(nV, _ip(rowptr), _ip(colind), _dp(vals), float(shift), _dp(minv))
+    return minv
+
+
+def pcg(rowptr, colind, vals, b, shift: float = 0.0, max_iter: int = 50, rtol: float = 0.0, precond: bool = True,
+        history: bool = False) -> dict:
+    """Textbook preconditioned CG for (H + shift I) x = b from x_0 = 0, block-Jacobi preconditioner
+    (precond=False: plain CG).  Returns x, iters, res (|r_k| per step) and, with history, every iterate."""
+    lib = _load()
+    rowptr = _i32(rowptr)
+    nV = rowptr.shape[0] - 1
+    colind = _i32(colind) if len(colind) else np.zeros(1, dtype=np.int32)
+    vals = _f64(vals) if len(vals) else np.zeros((1, 3, 3))
+    b = _f64(b).reshape(nV, 3)
+    minv = block_jacobi(rowptr, colind, vals, shift) if precond else None
+    x = np.zeros((nV, 3))
+    xh = np.zeros((max_iter + 1, nV, 3)) if history else None
+    res = np.zeros(max_iter + 1)
+    k = lib.tt_oracle_pcg(nV, _ip(rowptr), _ip(colind), _dp(vals), float(shift), _dp(minv), _dp(b), int(max_iter),
+                          float(rtol), _dp(x), _dp(xh), _dp(res))
+    k = int(k)
+    return dict(x=x, iters=k, res=res[:k + 1], x_hist=None if xh is None else xh[:k + 1], minv=minv)

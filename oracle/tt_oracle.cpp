@@ -558,6 +558,97 @@ int64_t tt_oracle_broad_phase(const double* pos, const int32_t* tris, int64_t n_
   return cnt[n_tris];
 }
 
+// ---- inexact-Newton linear solve ("inexact Newton optimization route") ------
+// The paper names the route and gives no detail, so the operations are their textbook definitions:
+//   * block-Jacobi preconditioner: the inverse of every 3x3 diagonal block of (H + shift I)
+//     (a row without a stored diagonal block has the block shift I);
+//   * preconditioned conjugate gradients (Hestenes-Stiefel; e.g. Saad, "Iterative Methods for Sparse
+//     Linear Systems", Alg. 9.1) for (H + shift I) x = b from x_0 = 0:
+//         r_0 = b, z_0 = M r_0, p_0 = z_0;
+//         alpha_k = (r_k.z_k)/(p_k.A p_k); x_{k+1} = x_k + alpha_k p_k; r_{k+1} = r_k - alpha_k A p_k;
+//         z_{k+1} = M r_{k+1}; beta_k = (r_{k+1}.z_{k+1})/(r_k.z_k); p_{k+1} = z_{k+1} + beta_k p_k,
+//     stopped before step k when |r_k|_2 <= rtol |b|_2, or after max_iter steps.
+// Written out as those definitions: Gauss-Jordan with partial pivoting for the 3x3 inverses, the plain BSR
+// product above for A p, Neumaier-compensated dot products.  (The GPU inverts by cofactors and sums in trees.)
+void tt_oracle_block_jacobi(int64_t n_verts, const int32_t* rowptr, const int32_t* colind, const double* vals,
+                            double shift, double* minv /*[n_verts,3,3]*/) {
+  for (int64_t r = 0; r < n_verts; ++r) {
+    double a[3][6];
+    for (int i = 0; i < 3; ++i)
+      for (int j = 0; j < 6; ++j) a[i][j] = (j == i + 3) ? 1.0 : 0.0;
+    for (int32_t e = rowptr[r]; e < rowptr[r + 1]; ++e)
+      if (colind[e] == r)
+        for (int i = 0; i < 3; ++i)
+          for (int j = 0; j < 3; ++j) a[i][j] += vals[9 * (int64_t)e + 3 * i + j];
+    for (int i = 0; i < 3; ++i) a[i][i] += shift;
+    for (int c = 0; c < 3; ++c) {  // Gauss-Jordan, partial pivoting
+      int piv = c;
+      for (int i = c + 1; i < 3; ++i)
+        if (std::fabs(a[i][c]) > std::fabs(a[piv][c])) piv = i;
+      for (int j = 0; j < 6; ++j) std::swap(a[c][j], a[piv][j]);
+      const double d = a[c][c];
+      for (int j = 0; j < 6; ++j) a[c][j] /= d;
+      for (int i = 0; i < 3; ++i)
+        if (i != c) {
+          const double f = a[i][c];
+          for (int j = 0; j < 6; ++j) a[i][j] -= f * a[c][j];
+        }
+    }
+    for (int i = 0; i < 3; ++i)
+      for (int j = 0; j < 3; ++j) minv[9 * r + 3 * i + j] = a[i][3 + j];
+  }
+}
+
+namespace {
+double ndot(const double* a, const double* b, int64_t n) {
+  Neumaier s;
+  for (int64_t i = 0; i < n; ++i) s.add(a[i] * b[i]);
+  return s.value();
+}
+void apply_blocks(int64_t nv, const double* minv, const double* r, double* z) {  // z = M r; minv == NULL: identity
+  for (int64_t v = 0; v < nv; ++v)
+    for (int i = 0; i < 3; ++i)
+      z[3 * v + i] = minv ? minv[9 * v + 3 * i] * r[3 * v] + minv[9 * v + 3 * i + 1] * r[3 * v + 1] +
+                                minv[9 * v + 3 * i + 2] * r[3 * v + 2]
+                          : r[3 * v + i];
+}
+}  // namespace
+
+// Returns the number of steps taken.  x [n] = last iterate; x_hist (or NULL) [(max_iter+1) n]: every iterate
+// x_0..x_k; res_hist (or NULL) [max_iter+1]: |r_k|_2 of the RECURRED residual.  minv: tt_oracle_block_jacobi's
+// output, or NULL for plain CG.
+int64_t tt_oracle_pcg(int64_t n_verts, const int32_t* rowptr, const int32_t* colind, const double* vals,
+                      double shift, const double* minv, const double* b, int64_t max_iter, double rtol,
+                      double* x, double* x_hist, double* res_hist) {
+  const int64_t n = 3 * n_verts;
+  std::vector<double> r(b, b + n), z((size_t)n), p((size_t)n), q((size_t)n);
+  for (int64_t i = 0; i < n; ++i) x[i] = 0.0;
+  apply_blocks(n_verts, minv, r.data(), z.data());
+  p = z;
+  double rz = ndot(r.data(), z.data(), n);
+  const double bnorm = std::sqrt(ndot(b, b, n));
+  int64_t k = 0;
+  for (;; ++k) {
+    const double rnorm = std::sqrt(ndot(r.data(), r.data(), n));
+    if (res_hist) res_hist[k] = rnorm;
+    if (x_hist) std::memcpy(x_hist + k * n, x, sizeof(double) * (size_t)n);
+    if (k == max_iter || rnorm <= rtol * bnorm) break;
+    tt_oracle_bsr_matvec(n_verts, rowptr, colind, vals, p.data(), q.data());
+    for (int64_t i = 0; i < n; ++i) q[i] += shift * p[i];
+    const double alpha = rz / ndot(p.data(), q.data(), n);
+    for (int64_t i = 0; i < n; ++i) {
+      x[i] += alpha * p[i];
+      r[i] -= alpha * q[i];
+    }
+    apply_blocks(n_verts, minv, r.data(), z.data());
+    const double rz_new = ndot(r.data(), z.data(), n);
+    const double beta = rz_new / rz;
+    rz = rz_new;
+    for (int64_t i = 0; i < n; ++i) p[i] = z[i] + beta * p[i];
+  }
+  return k;
+}
+
 int tt_oracle_max_threads(void) {
 #ifdef _OPENMP
   return omp_get_max_threads();
