@@ -180,6 +180,41 @@ tt_status tt_broad_phase_copy(tt_ctx* ctx, int32_t* pairs_out, int64_t capacity,
 tt_status tt_bsr_device(tt_ctx* ctx, const int32_t** rowptr, const int32_t** colind,
                         const void** vals, int64_t* nnzb);
 
+/* ---- The consumer of the assembly ("a GPU-based inexact Newton optimization route";
+ * SURVEY.md 8(f) NEXT-2).  The paper gives no detail, so each operation is its textbook definition.
+ * All arrays DEVICE; vectors [n_rows,3] dtype; the BSR layout is this library's (3x3 row-major blocks,
+ * int32 rowptr / colind, columns ascending within a row).
+ *
+ * tt_bsr_spmv:     y = (H + shift I) x.   x != y.
+ * tt_block_jacobi: minv [n_rows,3,3] dtype = inverse of every 3x3 diagonal block of (H + shift I); a row
+ *                  without a stored diagonal block gets I / shift.  The blocks must be non-singular (with a
+ *                  PSD hess_mode -- TT_HESS_PSD2 or TT_HESS_PSDPROJ -- any shift > 0 guarantees it).
+ * tt_pcg_solve:    preconditioned conjugate gradients (Hestenes-Stiefel recurrences) for (H + shift I) x = b
+ *                  from x_0 = 0, stopped before step k when |r_k|_2 <= rtol |b|_2 or after max_iter steps.
+ *                    vals != NULL : H is the BSR matrix (rowptr, colind, vals)            [assembled back end]
+ *                    vals == NULL : H p is tt_hess_vec on `prob` (needs tt_hess_symbolic at the current
+ *                                   positions; checked once per solve, TT_ERR_STATE)       [matrix-free back end]
+ *                    minv         : tt_block_jacobi's output, or NULL for plain CG
+ *                  prob->n_verts is the number of rows.  All scalars of the recurrence live on the device and
+ *                  every dot product is a fixed-order tree (deterministic; no floating-point atomics); with
+ *                  rtol > 0 the host looks at the residual every `check_every` steps (0 = 8), the iterate is
+ *                  frozen ON THE DEVICE at the first step that meets the bound, so x does not depend on
+ *                  check_every.  iters_host / relres_host (HOST [1], may be NULL): steps taken and
+ *                  |r|_2 / |b|_2 of the recurred residual; if either is given the call synchronises `stream`. */
+typedef struct {
+  int32_t max_iter;     /* >= 0                                                                       */
+  int32_t check_every;  /* host convergence checks (only if rtol > 0); 0 = every 8 steps              */
+  double rtol;          /* >= 0; 0 = run exactly max_iter steps, fully asynchronous                   */
+  double shift;         /* mu >= 0 added to the diagonal (Levenberg-Marquardt / "stay close" term)    */
+} tt_pcg_options;
+tt_status tt_bsr_spmv(tt_ctx* ctx, int64_t n_rows, const int32_t* rowptr, const int32_t* colind,
+                      const void* vals, double shift, const void* x, void* y, void* stream);
+tt_status tt_block_jacobi(tt_ctx* ctx, int64_t n_rows, const int32_t* rowptr, const int32_t* colind,
+                          const void* vals, double shift, void* minv, void* stream);
+tt_status tt_pcg_solve(tt_ctx* ctx, const tt_problem* prob, const int32_t* rowptr, const int32_t* colind,
+                       const void* vals, const void* minv, const void* b, void* x,
+                       const tt_pcg_options* opt, int32_t* iters_host, double* relres_host, void* stream);
+
 /* Counters of the last tt_hess_symbolic: what[0]=n_active, [1]=directed entries (2*n_active),
  * [2]=touched triangles, [3]=blocks written directly (exclusive rows), [4]=blocks produced by the
  * general-row merge, [5]=merge records, [6]=nnzb, [7]=kernels launched by this ctx so far (CUB calls counted by the kernels they launch).                     */

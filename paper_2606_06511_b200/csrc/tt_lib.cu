@@ -13,6 +13,7 @@
 #include "tt_broad.cuh"
 #include "tt_kernels.cuh"
 #include "tt_probe.cuh"
+#include "tt_solve.cuh"
 
 namespace {
 
@@ -74,6 +75,7 @@ struct tt_ctx {
   // numeric
   DevBuf everts, rdesc, tfirst, bucket_cnt, bucket_off, long_cnt, long_off, chunk_start, long_list, asm_energy, tvals, tslot, vkeys[2], vvals[2], vptr, vslot1;
   DevBuf cub_tmp;
+  DevBuf pcg_r, pcg_p, pcg_q, pcg_part[2], pcg_sc, pcg_hist;  // tt_pcg_solve workspace
   DevBuf possig;  // [2] u64: checksum of pos at tt_hess_symbolic, and at the last numeric / H.p call
   // broad phase (tt_broad_phase): boxes, grid, (cell, triangle) records, pair keys, result
   DevBuf bp_box, bp_part, bp_grid, bp_cnt, bp_off, bp_keys[2], bp_vals[2], bp_pcnt, bp_poff, bp_pkeys[2], bp_pairs;
@@ -705,6 +707,75 @@ tt_status hessvec_impl(tt_ctx* ctx, const tt_problem* q, const void* pvec, void*
   return TT_OK;
 }
 
+// ---- the consumer: BSR product, block-Jacobi, PCG (tt_solve.cuh) ----------------------
+template <typename T>
+tt_status spmv_impl(tt_ctx* ctx, int64_t nV, const int32_t* rowptr, const int32_t* colind, const void* vals, double shift,
+                    const void* x, void* y, cudaStream_t st) {
+  if (nV == 0) return TT_OK;
+  tts::k_bsr_spmv<T><<<grid_for(32 * nV, tts::VEC_THREADS), tts::VEC_THREADS, 0, st>>>(rowptr, colind, (const T*)vals, (const T*)x,
+                                                                                       (T*)y, nV, shift);
+  TT_LAUNCH_CHECK();
+  return TT_OK;
+}
+
+template <typename T>
+tt_status pcg_impl(tt_ctx* ctx, const tt_problem* q, const int32_t* rowptr, const int32_t* colind, const void* vals,
+                   const void* minv, const void* b, void* x, const tt_pcg_options* opt, int32_t* iters_host,
+                   double* relres_host, cudaStream_t st) {
+  using namespace tts;
+  const int64_t nV = q->n_verts, n = 3 * nV;
+  const bool matrix_free = (vals == nullptr);
+  if (iters_host) *iters_host = 0;
+  if (relres_host) *relres_host = 0.0;
+  if (nV == 0) return TT_OK;
+  const unsigned gv = grid_for(nV, VEC_THREADS), gn = grid_for(n, VEC_THREADS);
+  TT_CUDA(ctx->pcg_r.ensure(sizeof(T) * (size_t)n));
+  TT_CUDA(ctx->pcg_p.ensure(sizeof(T) * (size_t)n));
+  TT_CUDA(ctx->pcg_q.ensure(sizeof(T) * (size_t)n));
+  for (int i = 0; i < 2; ++i) TT_CUDA(ctx->pcg_part[i].ensure(sizeof(double) * (size_t)(gn + 1)));
+  TT_CUDA(ctx->pcg_sc.ensure(sizeof(PcgScalars)));
+  TT_CUDA(ctx->pcg_hist.ensure(sizeof(double) * (size_t)(opt->max_iter + 2)));
+  T* r = ctx->pcg_r.as<T>();
+  T* p = ctx->pcg_p.as<T>();
+  T* Ap = ctx->pcg_q.as<T>();
+  double* part0 = ctx->pcg_part[0].as<double>();
+  double* part1 = ctx->pcg_part[1].as<double>();
+  PcgScalars* sc = ctx->pcg_sc.as<PcgScalars>();
+  double* hist = ctx->pcg_hist.as<double>();
+  k_pcg_init<T><<<gv, VEC_THREADS, 0, st>>>((const T*)b, (const T*)minv, nV, (T*)x, r, p, part0, part1);
+  TT_LAUNCH_CHECK();
+  k_pcg_init_final<<<1, 1024, 0, st>>>(part0, part1, (int64_t)gv, opt->rtol, sc, hist);
+  TT_LAUNCH_CHECK();
+  const int check_every = opt->rtol > 0.0 ? (opt->check_every > 0 ? opt->check_every : 8) : 0;
+  PcgScalars h;
+  for (int it = 0; it < opt->max_iter; ++it) {
+    tt_status s = matrix_free ? hessvec_impl<T>(ctx, q, p, Ap, st) : spmv_impl<T>(ctx, nV, rowptr, colind, vals, opt->shift, p, Ap, st);
+    if (s != TT_OK) return s;
+    k_pcg_pq<T><<<gn, VEC_THREADS, 0, st>>>(p, Ap, n, opt->shift, matrix_free ? 1 : 0, part0);
+    TT_LAUNCH_CHECK();
+    k_pcg_alpha<<<1, 1024, 0, st>>>(part0, (int64_t)gn, sc);
+    TT_LAUNCH_CHECK();
+    k_pcg_update<T><<<gv, VEC_THREADS, 0, st>>>(p, Ap, (const T*)minv, nV, (T*)x, r, sc, part0, part1);
+    TT_LAUNCH_CHECK();
+    k_pcg_beta<<<1, 1024, 0, st>>>(part0, part1, (int64_t)gv, sc, hist);
+    TT_LAUNCH_CHECK();
+    k_pcg_dir<T><<<gn, VEC_THREADS, 0, st>>>(Ap, p, n, sc);
+    TT_LAUNCH_CHECK();
+    if (check_every && (it + 1) % check_every == 0 && it + 1 < opt->max_iter) {  // the device has already frozen x if converged
+      TT_CUDA(cudaMemcpyAsync(&h, sc, sizeof(h), cudaMemcpyDeviceToHost, st));
+      TT_CUDA(cudaStreamSynchronize(st));
+      if (h.done) break;
+    }
+  }
+  if (iters_host || relres_host) {
+    TT_CUDA(cudaMemcpyAsync(&h, sc, sizeof(h), cudaMemcpyDeviceToHost, st));
+    TT_CUDA(cudaStreamSynchronize(st));
+    if (iters_host) *iters_host = h.iters;
+    if (relres_host) *relres_host = h.bb > 0.0 ? sqrt(h.rr / h.bb) : 0.0;
+  }
+  return TT_OK;
+}
+
 // ---- broad phase (tt_broad.cuh) ------------------------------------------------------------------
 template <typename T>
 tt_status broad_impl(tt_ctx* ctx, const void* pos, int64_t nV, const int32_t* tris, int64_t nT, double inflate,
@@ -1050,6 +1121,54 @@ tt_status tt_broad_phase_copy(tt_ctx* ctx, int32_t* pairs_out, int64_t capacity,
                             (cudaStream_t)stream));
   }
   return TT_OK;
+}
+
+tt_status tt_bsr_spmv(tt_ctx* ctx, int64_t n_rows, const int32_t* rowptr, const int32_t* colind, const void* vals,
+                      double shift, const void* x, void* y, void* stream) {
+  if (!ctx) return TT_ERR_INVALID_ARG;
+  if (n_rows < 0 || n_rows >= (int64_t(1) << 31) / 3) return fail(ctx, TT_ERR_INVALID_ARG, "tt_bsr_spmv: n_rows out of range");
+  if (n_rows > 0 && (!rowptr || !x || !y || x == y)) return fail(ctx, TT_ERR_INVALID_ARG, "tt_bsr_spmv: NULL or aliased argument");
+  TT_CUDA(cudaSetDevice(ctx->opt.device));
+  cudaStream_t st = (cudaStream_t)stream;
+  return ctx->opt.dtype == TT_F64 ? spmv_impl<double>(ctx, n_rows, rowptr, colind, vals, shift, x, y, st)
+                                  : spmv_impl<float>(ctx, n_rows, rowptr, colind, vals, shift, x, y, st);
+}
+
+tt_status tt_block_jacobi(tt_ctx* ctx, int64_t n_rows, const int32_t* rowptr, const int32_t* colind, const void* vals,
+                          double shift, void* minv, void* stream) {
+  if (!ctx) return TT_ERR_INVALID_ARG;
+  if (n_rows < 0 || n_rows >= (int64_t(1) << 31) / 3) return fail(ctx, TT_ERR_INVALID_ARG, "tt_block_jacobi: n_rows out of range");
+  if (n_rows > 0 && (!rowptr || !minv)) return fail(ctx, TT_ERR_INVALID_ARG, "tt_block_jacobi: NULL argument");
+  if (n_rows == 0) return TT_OK;
+  TT_CUDA(cudaSetDevice(ctx->opt.device));
+  cudaStream_t st = (cudaStream_t)stream;
+  if (ctx->opt.dtype == TT_F64)
+    tts::k_block_jacobi<double><<<grid_for(n_rows, tts::VEC_THREADS), tts::VEC_THREADS, 0, st>>>(rowptr, colind, (const double*)vals, n_rows, shift, (double*)minv);
+  else
+    tts::k_block_jacobi<float><<<grid_for(n_rows, tts::VEC_THREADS), tts::VEC_THREADS, 0, st>>>(rowptr, colind, (const float*)vals, n_rows, shift, (float*)minv);
+  TT_LAUNCH_CHECK();
+  return TT_OK;
+}
+
+tt_status tt_pcg_solve(tt_ctx* ctx, const tt_problem* prob, const int32_t* rowptr, const int32_t* colind, const void* vals,
+                       const void* minv, const void* b, void* x, const tt_pcg_options* opt, int32_t* iters_host,
+                       double* relres_host, void* stream) {
+  tt_status s = check_problem(ctx, prob);
+  if (s != TT_OK) return s;
+  if (!opt || opt->max_iter < 0 || !(opt->rtol >= 0.0) || !(opt->shift >= 0.0))
+    return fail(ctx, TT_ERR_INVALID_ARG, "tt_pcg_solve: options NULL or max_iter / rtol / shift negative");
+  if (prob->n_verts > 0 && (!b || !x || b == x)) return fail(ctx, TT_ERR_INVALID_ARG, "tt_pcg_solve: b / x NULL or aliased");
+  const bool matrix_free = (vals == nullptr);
+  if (!matrix_free && (!rowptr || !colind)) return fail(ctx, TT_ERR_INVALID_ARG, "tt_pcg_solve: rowptr / colind / vals must be all set (BSR) or all NULL (matrix-free)");
+  TT_CUDA(cudaSetDevice(ctx->opt.device));
+  cudaStream_t st = (cudaStream_t)stream;
+  if (matrix_free) {
+    if (!ctx->sig.matches(prob)) return fail(ctx, TT_ERR_STATE, "tt_pcg_solve (matrix-free): no matching tt_hess_symbolic for this problem");
+    s = check_positions(ctx, prob, "tt_pcg_solve", st);  // once per solve, not per product
+    if (s != TT_OK) return s;
+  }
+  return ctx->opt.dtype == TT_F64 ? pcg_impl<double>(ctx, prob, rowptr, colind, vals, minv, b, x, opt, iters_host, relres_host, st)
+                                  : pcg_impl<float>(ctx, prob, rowptr, colind, vals, minv, b, x, opt, iters_host, relres_host, st);
 }
 
 tt_status tt_bsr_device(tt_ctx* ctx, const int32_t** rowptr, const int32_t** colind, const void** vals, int64_t* nnzb) {

@@ -23,7 +23,7 @@ TT_FLAG_VALIDATE_INDICES = 2
 TT_FLAG_NO_STATE_CHECK = 4
 
 EXPORTS = ["tt_create", "tt_destroy", "tt_energy", "tt_hess_symbolic", "tt_energy_grad_hess", "tt_hess_vec",
-           "tt_energy_grad_hess_host", "tt_broad_phase", "tt_broad_phase_pairs", "tt_broad_phase_copy", "tt_bsr_device", "tt_stats", "tt_kernel_ms", "tt_kernel_ms_mean", "tt_probe_peaks", "tt_status_string", "tt_last_error"]
+           "tt_energy_grad_hess_host", "tt_broad_phase", "tt_broad_phase_pairs", "tt_broad_phase_copy", "tt_bsr_device", "tt_bsr_spmv", "tt_block_jacobi", "tt_pcg_solve", "tt_stats", "tt_kernel_ms", "tt_kernel_ms_mean", "tt_probe_peaks", "tt_status_string", "tt_last_error"]
 
 
 class TTOptions(ctypes.Structure):
@@ -34,6 +34,11 @@ class TTOptions(ctypes.Structure):
 class TTProblem(ctypes.Structure):
     _fields_ = [("pos", ctypes.c_void_p), ("n_verts", ctypes.c_int64), ("tris", ctypes.c_void_p),
                 ("n_tris", ctypes.c_int64), ("pairs", ctypes.c_void_p), ("n_pairs", ctypes.c_int64)]
+
+
+class TTPcgOptions(ctypes.Structure):
+    _fields_ = [("max_iter", ctypes.c_int32), ("check_every", ctypes.c_int32), ("rtol", ctypes.c_double),
+                ("shift", ctypes.c_double)]
 
 
 class TTError(RuntimeError):
@@ -78,6 +83,13 @@ def load_library():
     lib.tt_broad_phase_copy.restype = ctypes.c_int
     lib.tt_bsr_device.argtypes = [vp, ctypes.POINTER(vp), ctypes.POINTER(vp), ctypes.POINTER(vp), ctypes.POINTER(i64)]
     lib.tt_bsr_device.restype = ctypes.c_int
+    lib.tt_bsr_spmv.argtypes = [vp, i64, vp, vp, vp, ctypes.c_double, vp, vp, vp]
+    lib.tt_bsr_spmv.restype = ctypes.c_int
+    lib.tt_block_jacobi.argtypes = [vp, i64, vp, vp, vp, ctypes.c_double, vp, vp]
+    lib.tt_block_jacobi.restype = ctypes.c_int
+    lib.tt_pcg_solve.argtypes = [vp, ctypes.POINTER(TTProblem), vp, vp, vp, vp, vp, vp, ctypes.POINTER(TTPcgOptions),
+                                 ctypes.POINTER(ctypes.c_int32), ctypes.POINTER(ctypes.c_double), vp]
+    lib.tt_pcg_solve.restype = ctypes.c_int
     lib.tt_stats.argtypes = [vp, ctypes.POINTER(i64), ctypes.c_int32]
     lib.tt_stats.restype = ctypes.c_int
     lib.tt_kernel_ms.argtypes = [vp, ctypes.POINTER(ctypes.c_float), ctypes.c_int32]
@@ -193,6 +205,26 @@ class Context:
         out = torch.empty((int(n.value), 2), dtype=torch.int32, device=pos.device)
         self._check(self.lib.tt_broad_phase_copy(self.h, _ptr(out) if n.value else None, int(n.value), sp))
         return out
+
+    # ---- the consumer: BSR product, block-Jacobi, PCG ----
+    def tt_bsr_spmv(self, rowptr, colind, vals, x, y, shift=0.0, stream=None):
+        self._check(self.lib.tt_bsr_spmv(self.h, x.shape[0], _ptr(rowptr), _ptr(colind), _ptr(vals), float(shift), _ptr(x),
+                                         _ptr(y), _stream_ptr(stream)))
+
+    def tt_block_jacobi(self, rowptr, colind, vals, minv, shift=0.0, stream=None):
+        self._check(self.lib.tt_block_jacobi(self.h, minv.shape[0], _ptr(rowptr), _ptr(colind), _ptr(vals), float(shift),
+                                             _ptr(minv), _stream_ptr(stream)))
+
+    def tt_pcg_solve(self, prob, b, x, rowptr=None, colind=None, vals=None, minv=None, max_iter=50, rtol=0.0, shift=0.0,
+                     check_every=0, want_stats=True, stream=None):
+        """vals given: assembled (BSR) back end; vals None: matrix-free (tt_hess_vec).  Returns (iters, relres)
+        (synchronises) or None with want_stats=False (fully asynchronous when rtol == 0)."""
+        opt = TTPcgOptions(int(max_iter), int(check_every), float(rtol), float(shift))
+        it, rr = ctypes.c_int32(0), ctypes.c_double(0.0)
+        self._check(self.lib.tt_pcg_solve(self.h, ctypes.byref(prob[0]), _ptr(rowptr), _ptr(colind), _ptr(vals), _ptr(minv),
+                                          _ptr(b), _ptr(x), ctypes.byref(opt), ctypes.byref(it) if want_stats else None,
+                                          ctypes.byref(rr) if want_stats else None, _stream_ptr(stream)))
+        return (it.value, rr.value) if want_stats else None
 
     def tt_kernel_ms(self):
         arr = (ctypes.c_float * 3)()

@@ -3,7 +3,7 @@ same seed, same three C-ABI calls per step):
 
   config 4 (throughput sweep)  2 M-triangle soup, 10 M candidate pairs, fp64 and fp32   (bench.py's default line)
   config 4 at the top of the sweep: 50 M pairs, fp64  (29 % of the triangles have more than 32 partners;
-                                 value offsets pass 2^32)
+                                 value offsets pass 2^31)
   config 3 (twisted torus)     1000 x 500 quads = 1 M triangles, ~8.1 M candidates, fp64 and fp32
                                  (shared vertices: the general-row merge path at scale)
 
@@ -177,12 +177,12 @@ def test_config4_full_size(oracle_mod, dtype):
 
 
 def test_config4_top_of_sweep_50M(oracle_mod):
-    """BASELINE.json configs[4] "1M-50M": the 50 M point, fp64.  nnzb * 9 exceeds 2^32 and about 29 % of
+    """BASELINE.json configs[4] "1M-50M": the 50 M point, fp64.  The value count nnzb * 9 exceeds 2^31 (33.7 GB of blocks) and about 29 % of
     the touched triangles have more than 32 partners (the long-triangle paths of K4 and K6)."""
     from paper_2606_06511_b200 import inputs
     pb = inputs.config4_sweep(n_tris=N_TRIS, n_pairs=50_000_000, seed=inputs.BASE_SEED + 4, device="cuda:0")
     st, sz = full_size_case(oracle_mod, pb, "f64")
-    assert sz["nnzb"] * 9 > 2 ** 32
+    assert sz["nnzb"] * 9 > 2 ** 31          # value offsets do not fit an int32
     deg = np.bincount(pb.pairs.ravel(), minlength=N_TRIS)           # candidates per triangle (~2x the active degree)
     assert (deg > 64).mean() > 0.1
 
