@@ -111,7 +111,7 @@ __global__ void __launch_bounds__(CLS_THREADS, TT_CLS_MIN_CTAS)
 k_classify(const T* __restrict__ pos, const int* __restrict__ tris, const int2* __restrict__ pairs,
            int64_t P, double sigma, uint32_t* __restrict__ mask, int* __restrict__ blk_count,
            double* __restrict__ blk_energy, T* __restrict__ e_pp, T* __restrict__ tc_out,
-           uint16_t* __restrict__ cfg_out) {
+           uint16_t* __restrict__ cfg_out, int* __restrict__ deg) {
   __shared__ double s_e[CLS_THREADS / 32];
   __shared__ int s_c[CLS_THREADS / 32];
   const int64_t k = (int64_t)blockIdx.x * CLS_THREADS + threadIdx.x;
@@ -131,6 +131,10 @@ k_classify(const T* __restrict__ pos, const int* __restrict__ tris, const int2* 
         const double pr2 = tc0 * tc1;
         en = pr2 * pr2;  // Eq. 2
         cfg = ttg::pair_config(g);
+        if (deg) {  // histogram of the directed entries by source triangle (integer RED: the result is order independent)
+          atomicAdd(deg + pr.x, 1);
+          atomicAdd(deg + pr.y, 1);
+        }
       }
     }
     if (cfg_out) cfg_out[k] = (uint16_t)cfg;
@@ -188,13 +192,18 @@ __global__ void k_set_count(const int* __restrict__ blk_off, const int* __restri
 }
 
 // ------------------------------------------------------------------------------------------ K2
-// With pairs / cfg / keys given it also emits the directed entries: active pair k = (s,t) -> (s -> t,
-// side 0) and (t -> s, side 1), key = (source << bitsT) | partner, payload = side | recorded config of
-// the canonical pair << 1.
+// Order-preserving compaction of the active pair ids (ballot / popc positions + per-CTA offsets) and, in
+// the same pass, the COUNTING SORT of the directed entries by source triangle: active pair (s, t) becomes
+// the entries s -> t (side 0) and t -> s (side 1); K1 has counted the entries of every triangle (deg), the
+// scan of deg is tptr, and an entry takes the next free place of its triangle's segment (integer atomics).
+// The order INSIDE a segment is whatever the atomics give; the symbolic kernels sort every segment by
+// (partner, side) before anything depends on it, so all results are deterministic (two entries with the
+// same key are the same pair listed twice: bit-identical contributions).
+//   ent[slot] = (partner triangle, side | recorded config of the canonical pair << 1)
 __global__ void __launch_bounds__(CLS_THREADS)
 k_compact(const uint32_t* __restrict__ mask, const int* __restrict__ blk_off, int64_t P,
-          int* __restrict__ active_ids, const int2* __restrict__ pairs, const uint16_t* __restrict__ cfg, int bitsT,
-          uint64_t* __restrict__ keys, uint16_t* __restrict__ vals) {
+          int* __restrict__ active_ids, const int2* __restrict__ pairs, const uint16_t* __restrict__ cfg,
+          const int* __restrict__ tptr, int* __restrict__ fill, uint2* __restrict__ ent) {
   const int64_t k = (int64_t)blockIdx.x * CLS_THREADS + threadIdx.x;
   const int w = threadIdx.x >> 5, l = threadIdx.x & 31;
   const int64_t word0 = (int64_t)blockIdx.x * (CLS_THREADS / 32);
@@ -209,15 +218,20 @@ k_compact(const uint32_t* __restrict__ mask, const int* __restrict__ blk_off, in
   if ((mine >> l) & 1u) {
     const int64_t a = (int64_t)blk_off[blockIdx.x] + before + __popc(mine & ((1u << l) - 1u));
     active_ids[a] = (int)k;
-    if (keys) {
+    if (ent) {
       const int2 pr = __ldg(pairs + k);
       const unsigned c = (unsigned)__ldg(cfg + k) << 1;
-      keys[2 * a] = ((uint64_t)(uint32_t)pr.x << bitsT) | (uint32_t)pr.y;
-      keys[2 * a + 1] = ((uint64_t)(uint32_t)pr.y << bitsT) | (uint32_t)pr.x;
-      vals[2 * a] = (uint16_t)c;
-      vals[2 * a + 1] = (uint16_t)(c | 1u);
+      const int sa = __ldg(tptr + pr.x) + atomicAdd(fill + pr.x, 1);
+      const int sb = __ldg(tptr + pr.y) + atomicAdd(fill + pr.y, 1);
+      ent[sa] = make_uint2((unsigned)pr.y, c);
+      ent[sb] = make_uint2((unsigned)pr.x, c | 1u);
     }
   }
+}
+
+// Sort key of a directed entry inside its triangle's segment.
+__device__ __forceinline__ unsigned long long entry_key(const uint2 e) {
+  return ((unsigned long long)e.x << 1) | (unsigned long long)(e.y & 1u);
 }
 
 // ------------------------------------------------------------------------------------------ K3
@@ -232,22 +246,51 @@ __global__ void k_segment_ptr(const uint64_t* __restrict__ keys, int64_t n, int 
 }
 
 // Touched triangles count their vertices (integer atomics: the RESULT is order independent).
-__global__ void k_vertex_touch(const int* __restrict__ tris, const int* __restrict__ tptr, int64_t nT,
-                               int* __restrict__ vcnt, int* __restrict__ tflag) {
+__global__ void k_vertex_touch(const int* __restrict__ tris, const int* __restrict__ deg, int64_t nT,
+                               int* __restrict__ vcnt) {
   const int64_t s = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
   if (s >= nT) return;
-  const int touched = tptr[s + 1] > tptr[s];
-  tflag[s] = touched;
-  if (touched) {
+  if (deg[s] > 0) {
 #pragma unroll
     for (int m = 0; m < 3; ++m) atomicAdd(vcnt + tris[3 * s + m], 1);
   }
 }
 
-// Per touched triangle s (one warp): candidate columns C = verts(partners in tadj order) ++ verts(s),
-// L = 3 (deg + 1).  Ranks each candidate among C by counting (shared memory, all pairs), detects
-// duplicates, decides which of the three rows are EXCLUSIVE (vertex used by no other touched
-// triangle, no duplicate column) and records:
+// Sorts the n entries of one segment by (partner, side) into (partner_out, dvals_out), one warp: every
+// entry counts the keys below it (ties by position: tied entries are identical pairs).  Keys are staged
+// in shared memory when they fit (skey, cap entries), else read through L1.
+__device__ __forceinline__ void warp_sort_segment(const uint2* __restrict__ ent, int n, unsigned long long* skey, int cap,
+                                                  int* __restrict__ partner_out, uint16_t* __restrict__ dvals_out, int lane) {
+  const bool staged = n <= cap;
+  if (staged) {
+    for (int j = lane; j < n; j += 32) skey[j] = entry_key(__ldg(ent + j));
+    __syncwarp();
+  }
+  for (int j = lane; j < n; j += 32) {
+    const uint2 me = __ldg(ent + j);
+    const unsigned long long key = entry_key(me);
+    int r = 0;
+    if (staged) {
+      for (int x = 0; x < n; ++x) {
+        const unsigned long long kx = skey[x];
+        r += (kx < key) || (kx == key && x < j);
+      }
+    } else {
+      for (int x = 0; x < n; ++x) {
+        const unsigned long long kx = entry_key(__ldg(ent + x));
+        r += (kx < key) || (kx == key && x < j);
+      }
+    }
+    partner_out[r] = (int)me.x;
+    dvals_out[r] = (uint16_t)me.y;
+  }
+  __syncwarp();
+}
+
+// Per LONG touched triangle s (more than RND_MAX_ENT partners; one warp): sorts its entries, then
+// candidate columns C = verts(partners in sorted order) ++ verts(s), L = 3 (deg + 1).  Ranks each
+// candidate among C by counting (shared memory, all pairs), detects duplicates, decides which of the
+// three rows are EXCLUSIVE (vertex used by no other touched triangle, no duplicate column) and records:
 //   erank[e][n]   position of partner column (e, n) inside the row       (rank, or identity if dup)
 //   drank[ti][n]  position of the diagonal column n
 //   rowlen[p]     = L for exclusive rows;  tlen[3ti+m] = L for general rows (their blocks go to
@@ -258,78 +301,80 @@ __global__ void k_vertex_touch(const int* __restrict__ tris, const int* __restri
 // Duplicates are detected as in k_round_symbolic: the ranks of L distinct values sum to L (L - 1) / 2.
 // Also writes the per-entry vertex ids (everts) of the triangle's entries.
 __global__ void __launch_bounds__(32 * SYM_WARPS)
-k_tri_symbolic(const int* __restrict__ tris, const int* __restrict__ touched, int64_t n_touched,
-               const int* __restrict__ tptr, const uint64_t* __restrict__ keys, const uint16_t* __restrict__ dvals,
-               int bitsT, const int* __restrict__ vcnt, int force_general, int* __restrict__ erank /*[2A][3]*/,
-               int* __restrict__ drank /*[n_touched][3]*/, int* __restrict__ rowlen,
+k_tri_symbolic(const int* __restrict__ tris, const int* __restrict__ touched, const int* __restrict__ n_long_dev,
+               const int* __restrict__ tfirst, const uint2* __restrict__ ent, int* partner /*sorted, out*/,
+               uint16_t* dvals /*sorted, out*/, const int* __restrict__ vcnt, int force_general,
+               int* __restrict__ erank /*[2A][3]*/, int* __restrict__ drank /*[n_touched][3]*/, int* __restrict__ rowlen,
                int64_t* __restrict__ tlen /*[3 n_touched]*/, uint8_t* __restrict__ slot_excl /*[3 n_touched]*/,
                const int* __restrict__ long_list, const int4* __restrict__ rdesc, int* __restrict__ vslot1,
                int* __restrict__ everts) {
-  __shared__ int s_c[SYM_WARPS][SYM_LMAX];
+  __shared__ __align__(8) int s_c[SYM_WARPS][SYM_LMAX];
   constexpr unsigned FULL = 0xffffffffu;
   const int w = threadIdx.x >> 5, l = threadIdx.x & 31;
-  const int64_t li = (int64_t)blockIdx.x * SYM_WARPS + w;  // n_touched counts the LONG triangles here
-  if (li >= n_touched) return;
-  const int64_t ti = rdesc[long_list[li]].z;
-  const int s = touched[ti];
-  const int e0 = tptr[s], deg = tptr[s + 1] - e0;
-  const int L = 3 * (deg + 1);
-  const uint64_t tmask = (1ull << bitsT) - 1ull;
-  int own[3];
-  load3i(tris + 3 * (int64_t)s, own);
-  // vertex ids of the canonical pair of every entry, both triangles in recorded (k, p, q) order
-  for (int j = l; j < deg; j += 32) {
-    const int64_t e = (int64_t)e0 + j;
-    int cv[3];
-    load3i(tris + 3 * (int64_t)(keys[e] & tmask), cv);
-    const unsigned pay = dvals[e];
-    const bool side = (pay & 1u) != 0u;
-    const unsigned ca = (pay >> 1) & 63u, cb = (pay >> 7) & 63u;
-    const int ka = (int)(ca & 3u), pa = (int)((ca >> 2) & 3u), kb = (int)(cb & 3u), pb = (int)((cb >> 2) & 3u);
-    const int a0 = side ? cv[0] : own[0], a1 = side ? cv[1] : own[1], a2 = side ? cv[2] : own[2];
-    const int b0 = side ? own[0] : cv[0], b1 = side ? own[1] : cv[1], b2 = side ? own[2] : cv[2];
-    int2* o = reinterpret_cast<int2*>(everts + 6 * e);
-    o[0] = make_int2(pick3(ka, a0, a1, a2), pick3(pa, a0, a1, a2));
-    o[1] = make_int2(pick3(3 - ka - pa, a0, a1, a2), pick3(kb, b0, b1, b2));
-    o[2] = make_int2(pick3(pb, b0, b1, b2), pick3(3 - kb - pb, b0, b1, b2));
-  }
-  bool nodup = (L <= SYM_LMAX);  // longer rows: identity layout, general rows
-  int* c = s_c[w];
-  if (nodup) {
-    for (int idx = l; idx < L; idx += 32) {
-      const int j = idx / 3, n = idx - 3 * j;
-      const int t = (j < deg) ? (int)(keys[e0 + j] & tmask) : s;
-      c[idx] = tris[3 * (int64_t)t + n];
+  const int64_t n_long = *n_long_dev;
+  for (int64_t li = (int64_t)blockIdx.x * SYM_WARPS + w; li < n_long; li += (int64_t)gridDim.x * SYM_WARPS) {
+    const int64_t ti = rdesc[long_list[li]].z;
+    const int s = touched[ti];
+    const int e0 = tfirst[ti], deg = tfirst[ti + 1] - e0;
+    const int L = 3 * (deg + 1);
+    int own[3];
+    load3i(tris + 3 * (int64_t)s, own);
+    warp_sort_segment(ent + e0, deg, reinterpret_cast<unsigned long long*>(s_c[w]), SYM_LMAX / 2, partner + e0, dvals + e0, l);
+    // vertex ids of the canonical pair of every entry, both triangles in recorded (k, p, q) order
+    for (int j = l; j < deg; j += 32) {
+      const int64_t e = (int64_t)e0 + j;
+      int cv[3];
+      load3i(tris + 3 * (int64_t)partner[e], cv);
+      const unsigned pay = dvals[e];
+      const bool side = (pay & 1u) != 0u;
+      const unsigned ca = (pay >> 1) & 63u, cb = (pay >> 7) & 63u;
+      const int ka = (int)(ca & 3u), pa = (int)((ca >> 2) & 3u), kb = (int)(cb & 3u), pb = (int)((cb >> 2) & 3u);
+      const int a0 = side ? cv[0] : own[0], a1 = side ? cv[1] : own[1], a2 = side ? cv[2] : own[2];
+      const int b0 = side ? own[0] : cv[0], b1 = side ? own[1] : cv[1], b2 = side ? own[2] : cv[2];
+      int2* o = reinterpret_cast<int2*>(everts + 6 * e);
+      o[0] = make_int2(pick3(ka, a0, a1, a2), pick3(pa, a0, a1, a2));
+      o[1] = make_int2(pick3(3 - ka - pa, a0, a1, a2), pick3(kb, b0, b1, b2));
+      o[2] = make_int2(pick3(pb, b0, b1, b2), pick3(3 - kb - pb, b0, b1, b2));
     }
-    __syncwarp();
-    long long sum = 0;
-    for (int idx = l; idx < L; idx += 32) {
-      const int me = c[idx];
-      int r = 0;
-      for (int x = 0; x < L; ++x) r += (c[x] < me);
-      sum += r;
-      const int j = idx / 3, n = idx - 3 * j;
-      if (j < deg) erank[3 * (int64_t)(e0 + j) + n] = r;
-      else drank[3 * ti + n] = r;
-    }
+    bool nodup = (L <= SYM_LMAX);  // longer rows: identity layout, general rows
+    int* c = s_c[w];
+    if (nodup) {
+      for (int idx = l; idx < L; idx += 32) {
+        const int j = idx / 3, n = idx - 3 * j;
+        const int t = (j < deg) ? partner[e0 + j] : s;
+        c[idx] = tris[3 * (int64_t)t + n];
+      }
+      __syncwarp();
+      long long sum = 0;
+      for (int idx = l; idx < L; idx += 32) {
+        const int me = c[idx];
+        int r = 0;
+        for (int x = 0; x < L; ++x) r += (c[x] < me);
+        sum += r;
+        const int j = idx / 3, n = idx - 3 * j;
+        if (j < deg) erank[3 * (int64_t)(e0 + j) + n] = r;
+        else drank[3 * ti + n] = r;
+      }
 #pragma unroll
-    for (int o = 16; o > 0; o >>= 1) sum += __shfl_xor_sync(FULL, sum, o);
-    nodup = (2 * sum == (long long)L * (L - 1));
-  }
-  if (!nodup) {
-    for (int idx = l; idx < L; idx += 32) {
-      const int j = idx / 3, n = idx - 3 * j;
-      if (j < deg) erank[3 * (int64_t)(e0 + j) + n] = idx;
-      else drank[3 * ti + n] = idx;
+      for (int o = 16; o > 0; o >>= 1) sum += __shfl_xor_sync(FULL, sum, o);
+      nodup = (2 * sum == (long long)L * (L - 1));
     }
-  }
-  if (l < 3) {
-    const int p = own[l == 0 ? 0 : (l == 1 ? 1 : 2)];
-    const bool excl = nodup && !force_general && (vcnt[p] == 1);
-    if (vcnt[p] == 1) vslot1[p] = (int)(3 * ti + l);  // the vertex's only slot (k_gather3)
-    slot_excl[3 * ti + l] = excl ? 1 : 0;
-    tlen[3 * ti + l] = excl ? 0 : L;
-    if (excl) rowlen[p] = L;
+    if (!nodup) {
+      for (int idx = l; idx < L; idx += 32) {
+        const int j = idx / 3, n = idx - 3 * j;
+        if (j < deg) erank[3 * (int64_t)(e0 + j) + n] = idx;
+        else drank[3 * ti + n] = idx;
+      }
+    }
+    if (l < 3) {
+      const int p = own[l == 0 ? 0 : (l == 1 ? 1 : 2)];
+      const bool excl = nodup && !force_general && (vcnt[p] == 1);
+      if (vcnt[p] == 1) vslot1[p] = (int)(3 * ti + l);  // the vertex's only slot (k_gather3)
+      slot_excl[3 * ti + l] = excl ? 1 : 0;
+      tlen[3 * ti + l] = excl ? 0 : L;
+      if (excl) rowlen[p] = L;
+    }
+    __syncwarp();  // s_c is reused by the next triangle
   }
 }
 
@@ -337,23 +382,22 @@ k_tri_symbolic(const int* __restrict__ tris, const int* __restrict__ touched, in
 // payload = workspace block index (assigned by the caller's iota; record index == block index).
 __global__ void __launch_bounds__(32 * SYM_WARPS)
 k_emit_records(const int* __restrict__ tris, const int* __restrict__ touched, int64_t n_touched,
-               const int* __restrict__ tptr, const uint64_t* __restrict__ keys, int bitsT, int bitsV,
+               const int* __restrict__ tfirst, const int* __restrict__ partner, int bitsV,
                const int* __restrict__ erank, const int* __restrict__ drank, const int64_t* __restrict__ toff,
                const uint8_t* __restrict__ slot_excl, uint64_t* __restrict__ rkeys, uint32_t* __restrict__ rvals) {
   const int w = threadIdx.x >> 5, l = threadIdx.x & 31;
   const int64_t ti = (int64_t)blockIdx.x * SYM_WARPS + w;
   if (ti >= n_touched) return;
   const int s = touched[ti];
-  const int e0 = tptr[s], deg = tptr[s + 1] - e0;
+  const int e0 = tfirst[ti], deg = tfirst[ti + 1] - e0;
   const int L = 3 * (deg + 1);
-  const uint64_t tmask = (1ull << bitsT) - 1ull;
   for (int m = 0; m < 3; ++m) {
     if (slot_excl[3 * ti + m]) continue;
     const uint64_t p = (uint64_t)(uint32_t)tris[3 * (int64_t)s + m];
     const int64_t base = toff[3 * ti + m];
     for (int idx = l; idx < L; idx += 32) {
       const int j = idx / 3, n = idx - 3 * j;
-      const int t = (j < deg) ? (int)(keys[e0 + j] & tmask) : s;
+      const int t = (j < deg) ? partner[e0 + j] : s;
       const int q = tris[3 * (int64_t)t + n];
       const int r = (j < deg) ? erank[3 * (int64_t)(e0 + j) + n] : drank[3 * ti + n];
       rkeys[base + r] = (p << bitsV) | (uint32_t)q;
@@ -399,7 +443,7 @@ __global__ void k_record_dest(const uint64_t* __restrict__ rkeys, int64_t U, int
 // Exclusive rows: column indices + row bases (>= 0: block index into vals; < 0: -(workspace+1)).
 __global__ void __launch_bounds__(32 * SYM_WARPS)
 k_fill_rows(const int* __restrict__ tris, const int* __restrict__ touched, int64_t n_touched,
-            const int* __restrict__ tptr, const uint64_t* __restrict__ keys, int bitsT,
+            const int* __restrict__ tfirst, const int* __restrict__ partner,
             const int* __restrict__ erank, const int* __restrict__ drank, const int64_t* __restrict__ toff,
             const uint8_t* __restrict__ slot_excl, const int* __restrict__ rowptr,
             int64_t* __restrict__ rowbase /*[3 n_touched]*/, int* __restrict__ colind,
@@ -409,9 +453,8 @@ k_fill_rows(const int* __restrict__ tris, const int* __restrict__ touched, int64
   if (li >= n_touched) return;
   const int64_t ti = rdesc[long_list[li]].z;
   const int s = touched[ti];
-  const int e0 = tptr[s], deg = tptr[s + 1] - e0;
+  const int e0 = tfirst[ti], deg = tfirst[ti + 1] - e0;
   const int L = 3 * (deg + 1);
-  const uint64_t tmask = (1ull << bitsT) - 1ull;
   for (int m = 0; m < 3; ++m) {
     const int64_t slot = 3 * ti + m;
     if (!slot_excl[slot]) {
@@ -422,7 +465,7 @@ k_fill_rows(const int* __restrict__ tris, const int* __restrict__ touched, int64
     if (l == 0) rowbase[slot] = rp;
     for (int idx = l; idx < L; idx += 32) {
       const int j = idx / 3, n = idx - 3 * j;
-      const int t = (j < deg) ? (int)(keys[e0 + j] & tmask) : s;
+      const int t = (j < deg) ? partner[e0 + j] : s;
       const int r = (j < deg) ? erank[3 * (int64_t)(e0 + j) + n] : drank[3 * ti + n];
       colind[rp + r] = tris[3 * (int64_t)t + n];
     }
@@ -444,21 +487,21 @@ constexpr int CHK_BUCKET = 128;
 
 // tfirst[i] = first directed entry of touched triangle i; tfirst[n_touched] = n_dir
 __global__ void k_touched_first(const int* __restrict__ touched, const int* __restrict__ n_touched_dev,
-                                const int* __restrict__ tptr, int64_t n_dir, int* __restrict__ tfirst) {
+                                const int* __restrict__ tptr, int64_t nT, int* __restrict__ tfirst) {
   const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
   const int64_t n_touched = *n_touched_dev;  // still on the device: the grid covers its bound
   if (i < n_touched) tfirst[i] = tptr[touched[i]];
-  if (i == n_touched) tfirst[i] = (int)n_dir;
+  if (i == n_touched) tfirst[i] = tptr[nT];  // = number of directed entries
 }
 
 // FILL = false: bucket_cnt[b] = rounds of bucket b (+ long_cnt[b] = long triangles).
-// FILL = true : chunk_start[bucket_off[b] + k] = first touched index of the k-th round of bucket b,
-//               long_list[long_off[b] + k] = round id of the k-th long triangle.
+// FILL = true : rdesc[bucket_off[b] + k] = descriptor of the k-th round of bucket b (first entry, entries,
+//               first touched index, triangles), long_list[long_off[b] + k] = round id of the k-th long triangle.
 template <bool FILL>
 __global__ void k_chunk_pack(const int* __restrict__ tfirst, const int* __restrict__ n_touched_dev,
                              int* __restrict__ bucket_cnt, int* __restrict__ long_cnt,
                              const int* __restrict__ bucket_off, const int* __restrict__ long_off,
-                             int* __restrict__ chunk_start, int* __restrict__ long_list) {
+                             int4* __restrict__ rdesc, int* __restrict__ long_list) {
   const int64_t b = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
   const int64_t n_touched = *n_touched_dev;  // still on the device: the grid covers its bound
   const int64_t n_buckets = (n_touched + CHK_BUCKET - 1) / CHK_BUCKET;
@@ -466,14 +509,16 @@ __global__ void k_chunk_pack(const int* __restrict__ tfirst, const int* __restri
   const int64_t i0 = b * CHK_BUCKET, i1 = min(i0 + (int64_t)CHK_BUCKET, n_touched);
   int nch = 0, nlong = 0, ent = 0, tri = 0;
   const int cbase = FILL ? bucket_off[b] : 0, lbase = FILL ? long_off[b] : 0;
-  int e_prev = tfirst[i0];
+  int e_i = tfirst[i0];
+  int t0 = (int)i0, e0 = e_i;             // the open round
   for (int64_t i = i0; i < i1; ++i) {
     const int e_next = tfirst[i + 1];
-    const int d = e_next - e_prev;
-    e_prev = e_next;
+    const int d = e_next - e_i;
     const bool is_long = d > RND_MAX_ENT;
     if (tri == 0 || is_long || ent + d > RND_MAX_ENT || tri + 1 > RND_MAX_TRI) {  // open a new round at i
-      if (FILL) chunk_start[cbase + nch] = (int)i;
+      if (FILL && nch > 0) rdesc[cbase + nch - 1] = make_int4(e0, e_i - e0, t0, (int)i - t0);
+      t0 = (int)i;
+      e0 = e_i;
       if (is_long) {
         if (FILL) long_list[lbase + nlong] = cbase + nch;
         ++nlong;
@@ -485,7 +530,9 @@ __global__ void k_chunk_pack(const int* __restrict__ tfirst, const int* __restri
     ent += d;
     tri += 1;
     if (is_long) tri = RND_MAX_TRI;  // closes the round: the next triangle opens a new one
+    e_i = e_next;
   }
+  if (FILL && nch > 0) rdesc[cbase + nch - 1] = make_int4(e0, e_i - e0, t0, (int)i1 - t0);
   if (!FILL) {
     bucket_cnt[b] = nch;
     long_cnt[b] = nlong;
@@ -544,7 +591,6 @@ struct Entry {
 template <typename T>
 struct AsmParams {
   const T* pos;
-  const uint64_t* keys;     // sorted directed keys (source << bitsT | partner)
   const uint16_t* dvals;    // side | recorded config << 1 (ttg::pair_config)
   const int* everts;        // [2A][6] vertex ids of the canonical pair, both triangles in recorded order
   const int4* rdesc;        // [n_chunks] round descriptor: first entry, entries, first touched index, triangles
@@ -560,20 +606,9 @@ struct AsmParams {
   const T* pvec;            // K6: p [nV,3]
   int64_t n_chunks;
   int64_t n_long;
-  int bitsT;
   int hess_mode;
   double sigma;
 };
-
-__global__ void k_round_desc(const int* __restrict__ chunk_start, const int* __restrict__ tfirst, int64_t n_chunks,
-                             int64_t n_touched, int4* __restrict__ rdesc) {
-  const int64_t c = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
-  if (c >= n_chunks) return;
-  const int t0 = chunk_start[c];
-  const int t1 = (c + 1 < n_chunks) ? chunk_start[c + 1] : (int)n_touched;
-  const int e0 = tfirst[t0];
-  rdesc[c] = make_int4(e0, tfirst[t1] - e0, t0, t1 - t0);
-}
 
 // ---- round-based symbolic kernels (one warp per round, lane = directed entry) -------------------
 // Same results as k_tri_symbolic / k_ent_verts / k_fill_rows, which remain for LONG triangles (more
@@ -582,143 +617,167 @@ __global__ void k_round_desc(const int* __restrict__ chunk_start, const int* __r
 constexpr int RSYM_WARPS = 4;
 
 
-// Column ranks (erank / drank), duplicate detection, exclusive rows, row lengths and the per-entry
-// vertex ids (everts) of every non-long round.
+// Segment sort by (partner, side), column ranks (erank / drank), duplicate detection, exclusive rows,
+// row lengths and the per-entry vertex ids (everts) of every non-long round.  Persistent grid: a warp
+// walks rounds c, c + G, ... (the number of rounds is still on the device when this kernel is enqueued).
 __global__ void __launch_bounds__(32 * RSYM_WARPS)
 k_round_symbolic(const int* __restrict__ tris, const int* __restrict__ touched, const int4* __restrict__ rdesc,
-                 int64_t n_chunks, const int* __restrict__ tfirst, const uint64_t* __restrict__ keys,
-                 const uint16_t* __restrict__ dvals, int bitsT, const int* __restrict__ vcnt, int force_general,
-                 int* __restrict__ erank, int* __restrict__ drank, int* __restrict__ rowlen,
-                 int64_t* __restrict__ tlen, uint8_t* __restrict__ slot_excl, int* __restrict__ everts,
-                 int* __restrict__ vslot1) {
+                 const int* __restrict__ n_chunks_dev, const int* __restrict__ tfirst, const uint2* __restrict__ ent,
+                 const int* __restrict__ vcnt, int force_general, int* __restrict__ partner_out,
+                 uint16_t* __restrict__ dvals_out, int* __restrict__ erank, int* __restrict__ drank,
+                 int* __restrict__ rowlen, int64_t* __restrict__ tlen, uint8_t* __restrict__ slot_excl,
+                 int* __restrict__ everts, int* __restrict__ vslot1) {
   __shared__ int s_cand[RSYM_WARPS][3 * RND_MAX_ENT];  // partner vertex ids of entry i at [3 i + n]
   __shared__ int s_own[RSYM_WARPS][3 * RND_MAX_TRI];   // own vertex ids of triangle tt at [3 tt + n]
   __shared__ int s_first[RSYM_WARPS][RND_MAX_TRI + 1];
   __shared__ int s_dup[RSYM_WARPS][RND_MAX_TRI];
   __shared__ int s_dacc[RSYM_WARPS][3 * RND_MAX_TRI];  // per own column: partner columns below it
   __shared__ int s_rsum[RSYM_WARPS][RND_MAX_TRI];      // per triangle: sum of the partner columns' ranks
+  __shared__ unsigned long long s_key[RSYM_WARPS][RND_MAX_ENT];
+  __shared__ uint2 s_ent[RSYM_WARPS][RND_MAX_ENT];
   constexpr unsigned FULL = 0xffffffffu;
   const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-  const int64_t c = (int64_t)blockIdx.x * RSYM_WARPS + warp;
-  if (c >= n_chunks) return;
-  const int4 d = __ldg(rdesc + c);
-  const int e_lo = d.x, nent = d.y, t_lo = d.z, ntri = d.w;
-  if (nent > RND_MAX_ENT) return;  // long triangle: k_tri_symbolic
   int* cand = s_cand[warp];
   int* own = s_own[warp];
   int* first = s_first[warp];
   int* dupf = s_dup[warp];
   int* dacc = s_dacc[warp];
   int* rsum = s_rsum[warp];
-  const uint64_t tmask = (1ull << bitsT) - 1ull;
-  // lane = triangle
-  int f = 0, l = 0, ov[3] = {0, 0, 0};
-  if (lane < ntri) {
-    const int s = __ldg(touched + t_lo + lane);
-    f = __ldg(tfirst + t_lo + lane) - e_lo;
-    l = __ldg(tfirst + t_lo + lane + 1) - e_lo;
+  unsigned long long* skey = s_key[warp];
+  uint2* sent = s_ent[warp];
+  const int64_t n_chunks = *n_chunks_dev;
+  for (int64_t c = (int64_t)blockIdx.x * RSYM_WARPS + warp; c < n_chunks; c += (int64_t)gridDim.x * RSYM_WARPS) {
+    const int4 d = __ldg(rdesc + c);
+    const int e_lo = d.x, nent = d.y, t_lo = d.z, ntri = d.w;
+    if (nent > RND_MAX_ENT) continue;  // long triangle: k_tri_symbolic
+    // lane = triangle
+    int f = 0, l = 0, ov[3] = {0, 0, 0};
+    if (lane < ntri) {
+      const int s = __ldg(touched + t_lo + lane);
+      f = __ldg(tfirst + t_lo + lane) - e_lo;
+      l = __ldg(tfirst + t_lo + lane + 1) - e_lo;
 #pragma unroll
-    for (int n = 0; n < 3; ++n) {
-      ov[n] = __ldg(tris + 3 * (int64_t)s + n);
-      own[3 * lane + n] = ov[n];
+      for (int n = 0; n < 3; ++n) {
+        ov[n] = __ldg(tris + 3 * (int64_t)s + n);
+        own[3 * lane + n] = ov[n];
+      }
+      first[lane] = f;
+      dupf[lane] = 0;
+      rsum[lane] = 0;
+      dacc[3 * lane] = dacc[3 * lane + 1] = dacc[3 * lane + 2] = 0;
     }
-    first[lane] = f;
-    dupf[lane] = 0;
-    rsum[lane] = 0;
-    dacc[3 * lane] = dacc[3 * lane + 1] = dacc[3 * lane + 2] = 0;
-  }
-  if (lane == 0) first[ntri] = nent;
-  // lane = entry
-  const bool valid = lane < nent;
-  int cv[3] = {0, 0, 0};
-  unsigned pay = 0u;
-  if (valid) {
-    const int64_t e = (int64_t)e_lo + lane;
-    const int t = (int)(__ldg(keys + e) & tmask);
-    pay = (unsigned)__ldg(dvals + e);
-    load3i(tris + 3 * (int64_t)t, cv);
+    if (lane == 0) first[ntri] = nent;
+    // lane = entry, in the order the counting sort left them
+    const bool valid = lane < nent;
+    uint2 me = make_uint2(0u, 0u);
+    if (valid) me = __ldg(ent + e_lo + lane);
+    const unsigned long long key = entry_key(me);
+    skey[lane] = key;
+    const unsigned heads = __reduce_or_sync(FULL, (lane < ntri) ? (1u << f) : 0u);
+    const int my_ti = __popc(heads & (0xffffffffu >> (31 - lane))) - 1;
+    __syncwarp();
+    int myf = 0, deg = 0;
+    int mo[3] = {0, 0, 0};  // own vertex ids of the entry's triangle
+    if (valid) {
+      myf = first[my_ti];
+      deg = first[my_ti + 1] - myf;
 #pragma unroll
-    for (int n = 0; n < 3; ++n) cand[3 * lane + n] = cv[n];
-  }
-  const unsigned heads = __reduce_or_sync(FULL, (lane < ntri) ? (1u << f) : 0u);
-  const int my_ti = __popc(heads & (0xffffffffu >> (31 - lane))) - 1;
-  __syncwarp();
-  // Rank of a column = number of smaller columns among the triangle's L = 3 (deg + 1) candidates.
-  // Duplicates: the ranks of L distinct values sum to L (L - 1) / 2 and every tied pair lowers the sum
-  // by one, so one integer per triangle (shared-memory atomics: the RESULT is order independent)
-  // replaces all equality counting.  The diagonal columns are ranked by the entries' lanes too:
-  // each adds how many of its three columns lie below each own column.
-  int r[3] = {0, 0, 0};
-  int myf = 0, deg = 0;
-  int mo[3] = {0, 0, 0};  // own vertex ids of the entry's triangle
-  if (valid) {
-    myf = first[my_ti];
-    deg = first[my_ti + 1] - myf;
-#pragma unroll
-    for (int n = 0; n < 3; ++n) mo[n] = own[3 * my_ti + n];
-  }
-  const int maxdeg = __reduce_max_sync(FULL, deg);
-  for (int k = 0; k < maxdeg; ++k) {
-    if (k < deg) {
-      const int* o = cand + 3 * (myf + k);
-      const int o0 = o[0], o1 = o[1], o2 = o[2];
-#pragma unroll
-      for (int n = 0; n < 3; ++n) r[n] += (o0 < cv[n]) + (o1 < cv[n]) + (o2 < cv[n]);
+      for (int n = 0; n < 3; ++n) mo[n] = own[3 * my_ti + n];
     }
-  }
-  if (valid) {
-#pragma unroll
-    for (int n = 0; n < 3; ++n) {
-      r[n] += (mo[0] < cv[n]) + (mo[1] < cv[n]) + (mo[2] < cv[n]);
-      atomicAdd(&dacc[3 * my_ti + n], (cv[0] < mo[n]) + (cv[1] < mo[n]) + (cv[2] < mo[n]));
+    const int maxdeg = __reduce_max_sync(FULL, deg);
+    // ---- sort the triangle's segment by (partner, side): position = number of keys below (ties by lane) ----
+    {
+      int pos = 0;
+      for (int k = 0; k < maxdeg; ++k) {
+        if (k < deg) {
+          const unsigned long long kx = skey[myf + k];
+          pos += (kx < key) || (kx == key && myf + k < lane);
+        }
+      }
+      if (valid) sent[myf + pos] = me;
+      __syncwarp();
+      if (valid) me = sent[lane];
     }
-    atomicAdd(&rsum[my_ti], r[0] + r[1] + r[2]);
-  }
-  __syncwarp();
-  int dr[3] = {0, 0, 0};
-  if (lane < ntri) {
-    int tot = rsum[lane];
+    int cv[3] = {0, 0, 0};
+    const unsigned pay = me.y;
+    if (valid) {
+      const int64_t e = (int64_t)e_lo + lane;
+      partner_out[e] = (int)me.x;
+      dvals_out[e] = (uint16_t)me.y;
+      load3i(tris + 3 * (int64_t)me.x, cv);
 #pragma unroll
-    for (int n = 0; n < 3; ++n) {
-      dr[n] = dacc[3 * lane + n] + (ov[0] < ov[n]) + (ov[1] < ov[n]) + (ov[2] < ov[n]);
-      tot += dr[n];
+      for (int n = 0; n < 3; ++n) cand[3 * lane + n] = cv[n];
     }
-    const int L = 3 * (l - f + 1);
-    dupf[lane] = (2 * tot != L * (L - 1)) ? 1 : 0;
-  }
-  __syncwarp();
-  if (valid) {
-    const int64_t e = (int64_t)e_lo + lane;
-    const bool nodup = dupf[my_ti] == 0;
-    const int j = lane - myf;
+    __syncwarp();
+    // Rank of a column = number of smaller columns among the triangle's L = 3 (deg + 1) candidates.
+    // Duplicates: the ranks of L distinct values sum to L (L - 1) / 2 and every tied pair lowers the sum
+    // by one, so one integer per triangle (shared-memory atomics: the RESULT is order independent)
+    // replaces all equality counting.  The diagonal columns are ranked by the entries' lanes too:
+    // each adds how many of its three columns lie below each own column.
+    int r[3] = {0, 0, 0};
+    for (int k = 0; k < maxdeg; ++k) {
+      if (k < deg) {
+        const int* o = cand + 3 * (myf + k);
+        const int o0 = o[0], o1 = o[1], o2 = o[2];
 #pragma unroll
-    for (int n = 0; n < 3; ++n) erank[3 * e + n] = nodup ? r[n] : 3 * j + n;
-    // vertex ids of the canonical pair, both triangles in recorded (k, p, q) order
-    const bool side = (pay & 1u) != 0u;
-    const unsigned ca = (pay >> 1) & 63u, cb = (pay >> 7) & 63u;
-    const int ka = (int)(ca & 3u), pa = (int)((ca >> 2) & 3u), kb = (int)(cb & 3u), pb = (int)((cb >> 2) & 3u);
-    const int a0 = side ? cv[0] : mo[0], a1 = side ? cv[1] : mo[1], a2 = side ? cv[2] : mo[2];
-    const int b0 = side ? mo[0] : cv[0], b1 = side ? mo[1] : cv[1], b2 = side ? mo[2] : cv[2];
-    int2* o = reinterpret_cast<int2*>(everts + 6 * e);
-    o[0] = make_int2(pick3(ka, a0, a1, a2), pick3(pa, a0, a1, a2));
-    o[1] = make_int2(pick3(3 - ka - pa, a0, a1, a2), pick3(kb, b0, b1, b2));
-    o[2] = make_int2(pick3(pb, b0, b1, b2), pick3(3 - kb - pb, b0, b1, b2));
-  }
-  if (lane < ntri) {
-    const int64_t ti = (int64_t)t_lo + lane;
-    const bool nodup = dupf[lane] == 0;
-    const int dg = l - f, L = 3 * (dg + 1);
-#pragma unroll
-    for (int n = 0; n < 3; ++n) drank[3 * ti + n] = nodup ? dr[n] : 3 * dg + n;
-#pragma unroll
-    for (int m = 0; m < 3; ++m) {
-      const bool single = __ldg(vcnt + ov[m]) == 1;
-      const bool excl = nodup && !force_general && single;
-      if (single) vslot1[ov[m]] = (int)(3 * ti + m);  // the vertex's only slot (k_gather3)
-      slot_excl[3 * ti + m] = excl ? 1 : 0;
-      tlen[3 * ti + m] = excl ? 0 : L;
-      if (excl) rowlen[ov[m]] = L;
+        for (int n = 0; n < 3; ++n) r[n] += (o0 < cv[n]) + (o1 < cv[n]) + (o2 < cv[n]);
+      }
     }
+    if (valid) {
+#pragma unroll
+      for (int n = 0; n < 3; ++n) {
+        r[n] += (mo[0] < cv[n]) + (mo[1] < cv[n]) + (mo[2] < cv[n]);
+        atomicAdd(&dacc[3 * my_ti + n], (cv[0] < mo[n]) + (cv[1] < mo[n]) + (cv[2] < mo[n]));
+      }
+      atomicAdd(&rsum[my_ti], r[0] + r[1] + r[2]);
+    }
+    __syncwarp();
+    int dr[3] = {0, 0, 0};
+    if (lane < ntri) {
+      int tot = rsum[lane];
+#pragma unroll
+      for (int n = 0; n < 3; ++n) {
+        dr[n] = dacc[3 * lane + n] + (ov[0] < ov[n]) + (ov[1] < ov[n]) + (ov[2] < ov[n]);
+        tot += dr[n];
+      }
+      const int L = 3 * (l - f + 1);
+      dupf[lane] = (2 * tot != L * (L - 1)) ? 1 : 0;
+    }
+    __syncwarp();
+    if (valid) {
+      const int64_t e = (int64_t)e_lo + lane;
+      const bool nodup = dupf[my_ti] == 0;
+      const int j = lane - myf;
+#pragma unroll
+      for (int n = 0; n < 3; ++n) erank[3 * e + n] = nodup ? r[n] : 3 * j + n;
+      // vertex ids of the canonical pair, both triangles in recorded (k, p, q) order
+      const bool side = (pay & 1u) != 0u;
+      const unsigned ca = (pay >> 1) & 63u, cb = (pay >> 7) & 63u;
+      const int ka = (int)(ca & 3u), pa = (int)((ca >> 2) & 3u), kb = (int)(cb & 3u), pb = (int)((cb >> 2) & 3u);
+      const int a0 = side ? cv[0] : mo[0], a1 = side ? cv[1] : mo[1], a2 = side ? cv[2] : mo[2];
+      const int b0 = side ? mo[0] : cv[0], b1 = side ? mo[1] : cv[1], b2 = side ? mo[2] : cv[2];
+      int2* o = reinterpret_cast<int2*>(everts + 6 * e);
+      o[0] = make_int2(pick3(ka, a0, a1, a2), pick3(pa, a0, a1, a2));
+      o[1] = make_int2(pick3(3 - ka - pa, a0, a1, a2), pick3(kb, b0, b1, b2));
+      o[2] = make_int2(pick3(pb, b0, b1, b2), pick3(3 - kb - pb, b0, b1, b2));
+    }
+    if (lane < ntri) {
+      const int64_t ti = (int64_t)t_lo + lane;
+      const bool nodup = dupf[lane] == 0;
+      const int dg = l - f, L = 3 * (dg + 1);
+#pragma unroll
+      for (int n = 0; n < 3; ++n) drank[3 * ti + n] = nodup ? dr[n] : 3 * dg + n;
+#pragma unroll
+      for (int m = 0; m < 3; ++m) {
+        const bool single = __ldg(vcnt + ov[m]) == 1;
+        const bool excl = nodup && !force_general && single;
+        if (single) vslot1[ov[m]] = (int)(3 * ti + m);  // the vertex's only slot (k_gather3)
+        slot_excl[3 * ti + m] = excl ? 1 : 0;
+        tlen[3 * ti + m] = excl ? 0 : L;
+        if (excl) rowlen[ov[m]] = L;
+      }
+    }
+    __syncwarp();  // shared memory is reused by the next round
   }
 }
 
@@ -728,7 +787,7 @@ k_round_symbolic(const int* __restrict__ tris, const int* __restrict__ touched, 
 // addresses, instead of nine scattered 4-byte stores per entry.
 __global__ void __launch_bounds__(32 * RSYM_WARPS)
 k_round_fill(const int* __restrict__ tris, const int* __restrict__ touched, const int4* __restrict__ rdesc,
-             int64_t n_chunks, const int* __restrict__ tfirst, const uint64_t* __restrict__ keys, int bitsT,
+             int64_t n_chunks, const int* __restrict__ tfirst, const int* __restrict__ partner,
              const int* __restrict__ erank, const int* __restrict__ drank, const int64_t* __restrict__ toff,
              const uint8_t* __restrict__ slot_excl, const int* __restrict__ rowptr,
              int64_t* __restrict__ rowbase, int* __restrict__ colind) {
@@ -748,12 +807,11 @@ k_round_fill(const int* __restrict__ tris, const int* __restrict__ touched, cons
   int* ci = s_ci[warp];
   int* first = s_first[warp];
   unsigned char* utt = s_utt[warp];
-  const uint64_t tmask = (1ull << bitsT) - 1ull;
   // entry lanes: partner columns and ranks (independent of the triangle lanes' loads)
   int cv[3] = {0, 0, 0}, er[3] = {0, 0, 0};
   if (lane < nent) {
     const int64_t e = (int64_t)e_lo + lane;
-    const int t = (int)(__ldg(keys + e) & tmask);
+    const int t = __ldg(partner + e);
     load3i(tris + 3 * (int64_t)t, cv);
     load3i(erank + 3 * e, er);
   }

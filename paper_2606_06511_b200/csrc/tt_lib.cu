@@ -4,6 +4,7 @@
 // hand-written kernels.
 #include <cstdarg>
 #include <cstdio>
+#include <cstdlib>
 #include <cstring>
 #include <string>
 
@@ -65,15 +66,17 @@ struct tt_ctx {
   // classification
   DevBuf mask, blk_count, blk_off, blk_energy, counts, energy, cfg, sum_stage;
   // active set + directed entries
-  DevBuf active_ids, keys[2], dvals[2], tptr, vcnt, tflag, touched;
+  DevBuf active_ids, ent_in, partner, dvals, tptr, zero_blk, touched;
   // per-triangle symbolic
-  DevBuf erank, drank, rowlen, tlen, toff, slot_excl, rowbase;
+  DevBuf erank, drank, tlen, toff, slot_excl, rowbase;
+  int* vcnt_p = nullptr;    // views into zero_blk (one memset per symbolic call)
+  int* rowlen_p = nullptr;
   // merge path
   DevBuf rkeys[2], rvals[2], head, ord, rowfirst, run_start, run_dest;
   // pattern
   DevBuf rowptr64, rowptr, colind;
   // numeric
-  DevBuf everts, rdesc, tfirst, bucket_cnt, bucket_off, long_cnt, long_off, chunk_start, long_list, asm_energy, tvals, tslot, vkeys[2], vvals[2], vptr, vslot1;
+  DevBuf everts, rdesc, tfirst, bucket_cnt, bucket_off, long_cnt, long_off, long_list, asm_energy, tvals, tslot, vkeys[2], vvals[2], vptr, vslot1;
   DevBuf cub_tmp;
   DevBuf pcg_r, pcg_p, pcg_q, pcg_part[2], pcg_sc, pcg_hist;  // tt_pcg_solve workspace
   DevBuf possig;  // [2] u64: checksum of pos at tt_hess_symbolic, and at the last numeric / H.p call
@@ -85,11 +88,11 @@ struct tt_ctx {
   // cached symbolic state
   Signature sig;
   int64_t A = 0, n_dir = 0, n_touched = 0, R = 0, U = 0, nnzb = 0, n_chunks = 0, n_long = 0, rows_excl = 0, rows_gen = 0;
-  int bitsT = 1, bitsV = 1;
+  int bitsT = 1, bitsV = 1, sms = 148;
+  // L2 persisting window over `pos` for the gather-bound kernels (K1, K4, K6); 0 = off
+  size_t l2_persist_bytes = 0, l2_max_window = 0;
   int tile_grid[2] = {0, 0};  // persistent grid of k_assemble_tile<double / float>
   int pipe_grid[2][2] = {{0, 0}, {0, 0}};  // persistent grid of k_entry_pipe<double / float, MODE 1 / 2>
-  uint64_t* keys_sorted = nullptr;
-  uint16_t* dvals_sorted = nullptr;
   uint64_t* rkeys_sorted = nullptr;
   uint32_t* rvals_sorted = nullptr;
   uint32_t* vvals_sorted = nullptr;
@@ -131,6 +134,24 @@ tt_status fail(tt_ctx* c, tt_status s, const char* fmt, ...) {
     ctx->launches++;                                                                             \
     TT_CUDA(cudaGetLastError());                                                                 \
   } while (0)
+
+// Marks `pos` as L2-persisting for the kernels enqueued on `st` until l2_window_off: the random
+// vertex gathers of K1 / K4 / K6 are the kernels' DRAM traffic, and a soup's positions (144 MB in fp64)
+// just miss the 126 MB L2, so plain LRU keeps ~40 % of them resident; a persisting window with
+// hitRatio = set-aside / window pins a fixed fraction instead of letting the streams evict it.
+inline void l2_window(tt_ctx* ctx, cudaStream_t st, const void* base, size_t bytes) {
+  if (!ctx->l2_persist_bytes) return;
+  cudaStreamAttrValue a;
+  memset(&a, 0, sizeof(a));
+  const size_t win = bytes < ctx->l2_max_window ? bytes : ctx->l2_max_window;
+  a.accessPolicyWindow.base_ptr = const_cast<void*>(base);
+  a.accessPolicyWindow.num_bytes = base ? win : 0;
+  a.accessPolicyWindow.hitRatio = (base && win) ? (float)((double)ctx->l2_persist_bytes / (double)win < 1.0 ? (double)ctx->l2_persist_bytes / (double)win : 1.0) : 0.0f;
+  a.accessPolicyWindow.hitProp = cudaAccessPropertyPersisting;
+  a.accessPolicyWindow.missProp = cudaAccessPropertyStreaming;
+  if (cudaStreamSetAttribute(st, cudaStreamAttributeAccessPolicyWindow, &a) != cudaSuccess) (void)cudaGetLastError();
+}
+inline void l2_window_off(tt_ctx* ctx, cudaStream_t st) { l2_window(ctx, st, nullptr, 0); }
 
 inline int ceil_log2(int64_t n) {
   int b = 1;
@@ -256,7 +277,7 @@ tt_status sort_pairs(tt_ctx* ctx, DevBuf (&kb)[2], DevBuf (&vb)[2], int64_t n, i
 
 // ---- K1 (+ sums): shared by tt_energy and tt_hess_symbolic -------------------------------------
 template <typename T>
-tt_status run_classify(tt_ctx* ctx, const tt_problem* q, T* e_pp, T* tc, bool record, cudaStream_t st, int64_t* nblk_out) {
+tt_status run_classify(tt_ctx* ctx, const tt_problem* q, T* e_pp, T* tc, bool record, int* deg, cudaStream_t st, int64_t* nblk_out) {
   const int64_t P = q->n_pairs;
   const int64_t nblk = (P + ttk::CLS_THREADS - 1) / ttk::CLS_THREADS;
   *nblk_out = nblk;
@@ -270,12 +291,14 @@ tt_status run_classify(tt_ctx* ctx, const tt_problem* q, T* e_pp, T* tc, bool re
   TT_CUDA(cudaMemsetAsync(ctx->blk_count.as<int>() + nblk, 0, sizeof(int), st));
   if (nblk > 0) {
     cudaEvent_t* ev_k1 = ctx->evr[0][ctx->ev_n[0] % tt_ctx::EV_RING];
+    l2_window(ctx, st, q->pos, sizeof(T) * 3 * (size_t)q->n_verts);
     TT_CUDA(cudaEventRecord(ev_k1[0], st));
     ttk::k_classify<T><<<(unsigned)nblk, ttk::CLS_THREADS, 0, st>>>(
         (const T*)q->pos, q->tris, (const int2*)q->pairs, P, ctx->opt.tc_scale, ctx->mask.as<uint32_t>(),
-        ctx->blk_count.as<int>(), ctx->blk_energy.as<double>(), e_pp, tc, record ? ctx->cfg.as<uint16_t>() : nullptr);
+        ctx->blk_count.as<int>(), ctx->blk_energy.as<double>(), e_pp, tc, record ? ctx->cfg.as<uint16_t>() : nullptr, deg);
     TT_LAUNCH_CHECK();
     TT_CUDA(cudaEventRecord(ev_k1[1], st));
+    l2_window_off(ctx, st);
     ctx->ev_n[0]++;
   }
   tt_status s = scan_i32(ctx, ctx->blk_count.as<int>(), ctx->blk_off.as<int>(), nblk + 1, st);
@@ -306,7 +329,7 @@ tt_status energy_impl(tt_ctx* ctx, const tt_problem* q, void* energy_sum, void* 
   int64_t nblk = 0;
   tt_status s = validate_indices(ctx, q->tris, q->n_tris, q->n_verts, q->pairs, q->n_pairs, st);
   if (s != TT_OK) return s;
-  s = run_classify<T>(ctx, q, (T*)e_pp, (T*)tc, false, st, &nblk);
+  s = run_classify<T>(ctx, q, (T*)e_pp, (T*)tc, false, nullptr, st, &nblk);
   if (s != TT_OK) return s;
   s = sum_partials<T>(ctx, ctx->blk_energy.as<double>(), nblk, (T*)energy_sum, st);
   if (s != TT_OK) return s;
@@ -320,6 +343,17 @@ tt_status energy_impl(tt_ctx* ctx, const tt_problem* q, void* energy_sum, void* 
   return TT_OK;
 }
 
+// 0 beyond 3 * n_touched (still on the device): the scan of the general-row lengths runs over the host-known bound
+struct MaskedLen {
+  const int64_t* tlen;
+  const int* n_touched;
+  __host__ __device__ int64_t operator()(int64_t i) const { return i < 3 * (int64_t)(*n_touched) ? tlen[i] : 0; }
+};
+struct DegFlag {
+  const int* deg;
+  __host__ __device__ int operator()(int t) const { return deg[t] > 0 ? 1 : 0; }
+};
+
 template <typename T>
 tt_status symbolic_impl(tt_ctx* ctx, const tt_problem* q, int64_t* nnzb_host, int64_t* n_active_host,
                         cudaStream_t st) {
@@ -331,80 +365,84 @@ tt_status symbolic_impl(tt_ctx* ctx, const tt_problem* q, int64_t* nnzb_host, in
   if (s != TT_OK) return s;
   s = pos_checksum(ctx, q, 0, st);
   if (s != TT_OK) return s;
-  s = run_classify<T>(ctx, q, nullptr, nullptr, true, st, &nblk);
+  ctx->bitsV = ceil_log2(nV > 1 ? nV : 2);
+  const int bitsV = ctx->bitsV;
+  // Everything up to the pattern sizes is enqueued WITHOUT a host round trip: buffers and grids use the
+  // bounds  directed entries <= 2 P,  touched triangles <= min(nT, 2 P),  and the kernels read the true
+  // counts from device memory.  One synchronisation (below) then brings all counts to the host.
+  const int64_t n_ub = 2 * P;
+  const int64_t touched_ub = nT < n_ub ? nT : n_ub;
+  // ---- one zeroed block: deg [nT+1], fill [nT+1], vcnt [nV+1], rowlen [nV+1] ----
+  const size_t zints = 2 * (size_t)(nT + 1) + 2 * (size_t)(nV + 1);
+  TT_CUDA(ctx->zero_blk.ensure(sizeof(int) * zints));
+  TT_CUDA(cudaMemsetAsync(ctx->zero_blk.p, 0, sizeof(int) * zints, st));
+  int* deg = ctx->zero_blk.as<int>();
+  int* fill = deg + (nT + 1);
+  int* vcnt = fill + (nT + 1);
+  int* rowlen = vcnt + (nV + 1);
+  ctx->vcnt_p = vcnt;
+  ctx->rowlen_p = rowlen;
+  // ---- K1: classification, recorded decisions, degree histogram ----
+  s = run_classify<T>(ctx, q, nullptr, nullptr, true, deg, st, &nblk);
   if (s != TT_OK) return s;
   int64_t* d_counts = ctx->counts.as<int64_t>();
   k_set_count<<<1, 32, 0, st>>>(ctx->blk_off.as<int>(), ctx->blk_count.as<int>(), nblk, d_counts, nullptr);
   TT_LAUNCH_CHECK();
-  int64_t A = 0;
-  TT_CUDA(cudaMemcpyAsync(&A, d_counts, sizeof(int64_t), cudaMemcpyDeviceToHost, st));
-  TT_CUDA(cudaStreamSynchronize(st));
-  ctx->A = A;
-  const int64_t n = 2 * A;
-  ctx->n_dir = n;
-  ctx->bitsT = ceil_log2(nT > 1 ? nT : 2);
-  ctx->bitsV = ceil_log2(nV > 1 ? nV : 2);
-  const int bitsT = ctx->bitsT, bitsV = ctx->bitsV;
-
-  // ---- compaction + directed entries sorted by (source, partner) ----
-  TT_CUDA(ctx->active_ids.ensure(sizeof(int) * (size_t)(A + 1)));
-  for (int i = 0; i < 2; ++i) {
-    TT_CUDA(ctx->keys[i].ensure(sizeof(uint64_t) * (size_t)(n + 1)));
-    TT_CUDA(ctx->dvals[i].ensure(sizeof(uint16_t) * (size_t)(n + 1)));
-  }
-  ctx->keys_sorted = ctx->keys[0].as<uint64_t>();
-  ctx->dvals_sorted = ctx->dvals[0].as<uint16_t>();
-  if (nblk > 0) {  // active ids + the two directed entries of every active pair, in one pass
+  TT_CUDA(ctx->tptr.ensure(sizeof(int) * (size_t)(nT + 2)));
+  s = scan_i32(ctx, deg, ctx->tptr.as<int>(), nT + 1, st);  // tptr[nT] = directed entries = 2 A
+  if (s != TT_OK) return s;
+  // ---- K2: compaction + counting sort of the directed entries by source triangle ----
+  TT_CUDA(ctx->active_ids.ensure(sizeof(int) * (size_t)(P + 1)));
+  TT_CUDA(ctx->ent_in.ensure(sizeof(uint2) * (size_t)(n_ub + 1)));
+  TT_CUDA(ctx->partner.ensure(sizeof(int) * (size_t)(n_ub + 1)));
+  TT_CUDA(ctx->dvals.ensure(sizeof(uint16_t) * (size_t)(n_ub + 2)));
+  if (nblk > 0) {
     k_compact<<<(unsigned)nblk, CLS_THREADS, 0, st>>>(ctx->mask.as<uint32_t>(), ctx->blk_off.as<int>(), P, ctx->active_ids.as<int>(),
-                                                      (const int2*)q->pairs, ctx->cfg.as<uint16_t>(), bitsT,
-                                                      ctx->keys[0].as<uint64_t>(), ctx->dvals[0].as<uint16_t>());
+                                                      (const int2*)q->pairs, ctx->cfg.as<uint16_t>(), ctx->tptr.as<int>(), fill,
+                                                      ctx->ent_in.as<uint2>());
     TT_LAUNCH_CHECK();
   }
-  if (A > 0) {
-    // stable sort on the SOURCE bits only: a triangle's entries become contiguous, in active-pair
-    // order (deterministic); nothing downstream needs the partners ascending (columns are ranked)
-    s = sort_pairs(ctx, ctx->keys, ctx->dvals, n, bitsT, 2 * bitsT, &ctx->keys_sorted, &ctx->dvals_sorted, st);
-    if (s != TT_OK) return s;
-  }
-  TT_CUDA(ctx->everts.ensure(sizeof(int) * 6 * (size_t)(n + 1)));
-  TT_CUDA(ctx->tptr.ensure(sizeof(int) * (size_t)(nT + 2)));
-  k_segment_ptr<<<grid_for(n + 1, 256), 256, 0, st>>>(ctx->keys_sorted, n, bitsT, nT, ctx->tptr.as<int>());
-  TT_LAUNCH_CHECK();
-
-  // ---- touched triangles, vertex use counts and the work partition (rounds) shared by the symbolic
-  //      round kernels, K4 and K6.  The number of touched triangles stays on the device until the
-  //      rounds are packed (grids and buffers use the bound min(nT, 2A)): one host round trip for
-  //      n_touched, n_chunks and n_long instead of two. ----
-  TT_CUDA(ctx->vcnt.ensure(sizeof(int) * (size_t)(nV + 1)));
-  TT_CUDA(ctx->tflag.ensure(sizeof(int) * (size_t)(nT + 1)));
+  // ---- touched triangles, vertex use counts, the work partition (rounds) shared by the symbolic round
+  //      kernels, K4 and K6 ----
   TT_CUDA(ctx->touched.ensure(sizeof(int) * (size_t)(nT + 1)));
-  TT_CUDA(cudaMemsetAsync(ctx->vcnt.p, 0, sizeof(int) * (size_t)(nV + 1), st));
-  int64_t n_touched = 0, n_chunks = 0, n_long = 0;
-  const int64_t touched_ub = nT < n ? nT : n;
   TT_CUDA(ctx->tfirst.ensure(sizeof(int) * (size_t)(touched_ub + 2)));
-  TT_CUDA(ctx->chunk_start.ensure(sizeof(int) * (size_t)(touched_ub + 2)));
-  TT_CUDA(ctx->long_list.ensure(sizeof(int) * (size_t)(n / (RND_MAX_ENT + 1) + 2)));
+  TT_CUDA(ctx->rdesc.ensure(sizeof(int4) * (size_t)(touched_ub + 1)));
+  TT_CUDA(ctx->long_list.ensure(sizeof(int) * (size_t)(n_ub / (RND_MAX_ENT + 1) + 2)));
+  const int64_t buckets_ub = (touched_ub + CHK_BUCKET - 1) / CHK_BUCKET;
+  TT_CUDA(ctx->bucket_cnt.ensure(sizeof(int) * (size_t)(buckets_ub + 1)));
+  TT_CUDA(ctx->bucket_off.ensure(sizeof(int) * (size_t)(buckets_ub + 1)));
+  TT_CUDA(ctx->long_cnt.ensure(sizeof(int) * (size_t)(buckets_ub + 1)));
+  TT_CUDA(ctx->long_off.ensure(sizeof(int) * (size_t)(buckets_ub + 1)));
+  TT_CUDA(ctx->erank.ensure(sizeof(int) * (size_t)(3 * n_ub + 3)));
+  TT_CUDA(ctx->everts.ensure(sizeof(int) * 6 * (size_t)(n_ub + 1)));
+  TT_CUDA(ctx->drank.ensure(sizeof(int) * (size_t)(3 * touched_ub + 3)));
+  TT_CUDA(ctx->tlen.ensure(sizeof(int64_t) * (size_t)(3 * touched_ub + 1)));
+  TT_CUDA(ctx->toff.ensure(sizeof(int64_t) * (size_t)(3 * touched_ub + 2)));
+  TT_CUDA(ctx->slot_excl.ensure((size_t)(3 * touched_ub + 1)));
+  TT_CUDA(ctx->rowbase.ensure(sizeof(int64_t) * (size_t)(3 * touched_ub + 1)));
+  TT_CUDA(ctx->vslot1.ensure(sizeof(int) * (size_t)(nV + 1)));
+  TT_CUDA(ctx->rowptr64.ensure(sizeof(int64_t) * (size_t)(nV + 1)));
+  TT_CUDA(ctx->rowptr.ensure(sizeof(int) * (size_t)(nV + 1)));
+  int* d_num = reinterpret_cast<int*>(d_counts + 1);                   // n_touched
+  int* d_nchunks = ctx->bucket_off.as<int>() + buckets_ub;             // totals of the two scans
+  int* d_nlong = ctx->long_off.as<int>() + buckets_ub;
+  TT_CUDA(cudaMemsetAsync(d_num, 0, sizeof(int), st));
+  TT_CUDA(cudaMemsetAsync(ctx->bucket_cnt.p, 0, sizeof(int) * (size_t)(buckets_ub + 1), st));
+  TT_CUDA(cudaMemsetAsync(ctx->long_cnt.p, 0, sizeof(int) * (size_t)(buckets_ub + 1), st));
+  const int force_general = (ctx->opt.flags & TT_FLAG_FORCE_GENERAL_ROWS) ? 1 : 0;
   if (touched_ub > 0) {
-    k_vertex_touch<<<grid_for(nT, 256), 256, 0, st>>>(q->tris, ctx->tptr.as<int>(), nT, ctx->vcnt.as<int>(),
-                                                      ctx->tflag.as<int>());
+    k_vertex_touch<<<grid_for(nT, 256), 256, 0, st>>>(q->tris, deg, nT, vcnt);
     TT_LAUNCH_CHECK();
     cub::CountingInputIterator<int> iota(0);
+    cub::TransformInputIterator<int, DegFlag, cub::CountingInputIterator<int>> flags(iota, DegFlag{deg});
     size_t tmp = 0;
-    int* d_num = reinterpret_cast<int*>(d_counts + 1);
-    TT_CUDA(cub::DeviceSelect::Flagged(nullptr, tmp, iota, ctx->tflag.as<int>(), ctx->touched.as<int>(), d_num, (int)nT, st));
+    TT_CUDA(cub::DeviceSelect::Flagged(nullptr, tmp, iota, flags, ctx->touched.as<int>(), d_num, (int)nT, st));
     TT_CUDA(ctx->cub_tmp.ensure(tmp));
-    TT_CUDA(cub::DeviceSelect::Flagged(ctx->cub_tmp.p, tmp, iota, ctx->tflag.as<int>(), ctx->touched.as<int>(), d_num, (int)nT, st));
+    TT_CUDA(cub::DeviceSelect::Flagged(ctx->cub_tmp.p, tmp, iota, flags, ctx->touched.as<int>(), d_num, (int)nT, st));
     ctx->launches += 2;  // CUB select: init + sweep kernel
-    const int64_t buckets_ub = (touched_ub + CHK_BUCKET - 1) / CHK_BUCKET;
-    TT_CUDA(ctx->bucket_cnt.ensure(sizeof(int) * (size_t)(buckets_ub + 1)));
-    TT_CUDA(ctx->bucket_off.ensure(sizeof(int) * (size_t)(buckets_ub + 1)));
-    TT_CUDA(ctx->long_cnt.ensure(sizeof(int) * (size_t)(buckets_ub + 1)));
-    TT_CUDA(ctx->long_off.ensure(sizeof(int) * (size_t)(buckets_ub + 1)));
-    k_touched_first<<<grid_for(touched_ub + 1, 256), 256, 0, st>>>(ctx->touched.as<int>(), d_num, ctx->tptr.as<int>(), n,
+    k_touched_first<<<grid_for(touched_ub + 1, 256), 256, 0, st>>>(ctx->touched.as<int>(), d_num, ctx->tptr.as<int>(), nT,
                                                                    ctx->tfirst.as<int>());
     TT_LAUNCH_CHECK();
-    TT_CUDA(cudaMemsetAsync(ctx->bucket_cnt.p, 0, sizeof(int) * (size_t)(buckets_ub + 1), st));
-    TT_CUDA(cudaMemsetAsync(ctx->long_cnt.p, 0, sizeof(int) * (size_t)(buckets_ub + 1), st));
     k_chunk_pack<false><<<grid_for(buckets_ub, 128), 128, 0, st>>>(ctx->tfirst.as<int>(), d_num, ctx->bucket_cnt.as<int>(),
                                                                   ctx->long_cnt.as<int>(), nullptr, nullptr, nullptr, nullptr);
     TT_LAUNCH_CHECK();
@@ -414,70 +452,63 @@ tt_status symbolic_impl(tt_ctx* ctx, const tt_problem* q, int64_t* nnzb_host, in
     if (s != TT_OK) return s;
     k_chunk_pack<true><<<grid_for(buckets_ub, 128), 128, 0, st>>>(ctx->tfirst.as<int>(), d_num, nullptr, nullptr,
                                                                  ctx->bucket_off.as<int>(), ctx->long_off.as<int>(),
-                                                                 ctx->chunk_start.as<int>(), ctx->long_list.as<int>());
+                                                                 ctx->rdesc.as<int4>(), ctx->long_list.as<int>());
     TT_LAUNCH_CHECK();
-    int cnt32[3] = {0, 0, 0};
-    TT_CUDA(cudaMemcpyAsync(&cnt32[0], d_num, sizeof(int), cudaMemcpyDeviceToHost, st));
-    TT_CUDA(cudaMemcpyAsync(&cnt32[1], ctx->bucket_off.as<int>() + buckets_ub, sizeof(int), cudaMemcpyDeviceToHost, st));
-    TT_CUDA(cudaMemcpyAsync(&cnt32[2], ctx->long_off.as<int>() + buckets_ub, sizeof(int), cudaMemcpyDeviceToHost, st));
-    TT_CUDA(cudaStreamSynchronize(st));
-    n_touched = cnt32[0];
-    n_chunks = cnt32[1];
-    n_long = cnt32[2];
+    // ---- per-triangle segment sort, column ranks, exclusive rows, general-row workspace sizes
+    //      (persistent grids: the round / long-triangle counts are read on the device) ----
+    const int64_t rounds_ub = (touched_ub + RSYM_WARPS - 1) / RSYM_WARPS;
+    const int64_t sym_pers = (int64_t)ctx->sms * 16;
+    k_round_symbolic<<<(unsigned)(rounds_ub < sym_pers ? rounds_ub : sym_pers), 32 * RSYM_WARPS, 0, st>>>(
+        q->tris, ctx->touched.as<int>(), ctx->rdesc.as<int4>(), d_nchunks, ctx->tfirst.as<int>(), ctx->ent_in.as<uint2>(),
+        vcnt, force_general, ctx->partner.as<int>(), ctx->dvals.as<uint16_t>(), ctx->erank.as<int>(), ctx->drank.as<int>(),
+        rowlen, ctx->tlen.as<int64_t>(), ctx->slot_excl.as<uint8_t>(), ctx->everts.as<int>(), ctx->vslot1.as<int>());
+    TT_LAUNCH_CHECK();
+    const int64_t long_ub = n_ub / (RND_MAX_ENT + 1);
+    if (long_ub > 0) {  // triangles with more than RND_MAX_ENT partners: one warp per triangle
+      const int64_t lg = (long_ub + SYM_WARPS - 1) / SYM_WARPS;
+      const int64_t lpers = (int64_t)ctx->sms * 8;
+      k_tri_symbolic<<<(unsigned)(lg < lpers ? lg : lpers), 32 * SYM_WARPS, 0, st>>>(
+          q->tris, ctx->touched.as<int>(), d_nlong, ctx->tfirst.as<int>(), ctx->ent_in.as<uint2>(), ctx->partner.as<int>(),
+          ctx->dvals.as<uint16_t>(), vcnt, force_general, ctx->erank.as<int>(), ctx->drank.as<int>(), rowlen,
+          ctx->tlen.as<int64_t>(), ctx->slot_excl.as<uint8_t>(), ctx->long_list.as<int>(), ctx->rdesc.as<int4>(),
+          ctx->vslot1.as<int>(), ctx->everts.as<int>());
+      TT_LAUNCH_CHECK();
+    }
   }
+  {  // general-row workspace offsets: scan over the bound, lengths beyond 3 n_touched read as 0
+    cub::CountingInputIterator<int64_t> idx(0);
+    cub::TransformInputIterator<int64_t, MaskedLen, cub::CountingInputIterator<int64_t>> it(idx, MaskedLen{ctx->tlen.as<int64_t>(), d_num});
+    size_t tmp = 0;
+    TT_CUDA(cub::DeviceScan::ExclusiveSum(nullptr, tmp, it, ctx->toff.as<int64_t>(), 3 * touched_ub + 1, st));
+    TT_CUDA(ctx->cub_tmp.ensure(tmp));
+    TT_CUDA(cub::DeviceScan::ExclusiveSum(ctx->cub_tmp.p, tmp, it, ctx->toff.as<int64_t>(), 3 * touched_ub + 1, st));
+    ctx->launches += 2;
+  }
+  // The row-pointer scan is issued speculatively: if there are no general rows (R == 0: always, in a
+  // soup) the exclusive row lengths are already final and nnzb arrives in the same host round trip.
+  s = scan_i32_to_i64(ctx, rowlen, ctx->rowptr64.as<int64_t>(), nV + 1, st);
+  if (s != TT_OK) return s;
+  // ---- the ONE host round trip of the phase (soup; general rows add the merge pass below) ----
+  int64_t A = 0, R = 0, nnzb = 0;
+  int cnt32[3] = {0, 0, 0};
+  TT_CUDA(cudaMemcpyAsync(&A, d_counts, sizeof(int64_t), cudaMemcpyDeviceToHost, st));
+  TT_CUDA(cudaMemcpyAsync(&cnt32[0], d_num, sizeof(int), cudaMemcpyDeviceToHost, st));
+  TT_CUDA(cudaMemcpyAsync(&cnt32[1], d_nchunks, sizeof(int), cudaMemcpyDeviceToHost, st));
+  TT_CUDA(cudaMemcpyAsync(&cnt32[2], d_nlong, sizeof(int), cudaMemcpyDeviceToHost, st));
+  TT_CUDA(cudaMemcpyAsync(&R, ctx->toff.as<int64_t>() + 3 * touched_ub, sizeof(int64_t), cudaMemcpyDeviceToHost, st));
+  TT_CUDA(cudaMemcpyAsync(&nnzb, ctx->rowptr64.as<int64_t>() + nV, sizeof(int64_t), cudaMemcpyDeviceToHost, st));
+  TT_CUDA(cudaStreamSynchronize(st));
+  const int64_t n = 2 * A;
+  const int64_t n_touched = touched_ub > 0 ? cnt32[0] : 0, n_chunks = touched_ub > 0 ? cnt32[1] : 0, n_long = touched_ub > 0 ? cnt32[2] : 0;
+  ctx->A = A;
+  ctx->n_dir = n;
   ctx->n_touched = n_touched;
   ctx->n_chunks = n_chunks;
   ctx->n_long = n_long;
-  TT_CUDA(ctx->rdesc.ensure(sizeof(int4) * (size_t)(n_chunks + 1)));
-  if (n_chunks > 0) {
-    k_round_desc<<<grid_for(n_chunks, 256), 256, 0, st>>>(ctx->chunk_start.as<int>(), ctx->tfirst.as<int>(), n_chunks, n_touched,
-                                                          ctx->rdesc.as<int4>());
-    TT_LAUNCH_CHECK();
-  }
-  // ---- per-triangle ranks, exclusive rows, general-row workspace sizes ----
-  TT_CUDA(ctx->erank.ensure(sizeof(int) * (size_t)(3 * n + 3)));
-  TT_CUDA(ctx->drank.ensure(sizeof(int) * (size_t)(3 * n_touched + 3)));
-  TT_CUDA(ctx->rowlen.ensure(sizeof(int) * (size_t)(nV + 1)));
-  TT_CUDA(ctx->tlen.ensure(sizeof(int64_t) * (size_t)(3 * n_touched + 1)));
-  TT_CUDA(ctx->toff.ensure(sizeof(int64_t) * (size_t)(3 * n_touched + 1)));
-  TT_CUDA(ctx->slot_excl.ensure((size_t)(3 * n_touched + 1)));
-  TT_CUDA(ctx->rowbase.ensure(sizeof(int64_t) * (size_t)(3 * n_touched + 1)));
-  TT_CUDA(ctx->vslot1.ensure(sizeof(int) * (size_t)(nV + 1)));
-  TT_CUDA(cudaMemsetAsync(ctx->rowlen.p, 0, sizeof(int) * (size_t)(nV + 1), st));
-  TT_CUDA(cudaMemsetAsync(ctx->tlen.p, 0, sizeof(int64_t) * (size_t)(3 * n_touched + 1), st));
-  TT_CUDA(cudaMemsetAsync(ctx->slot_excl.p, 0, (size_t)(3 * n_touched + 1), st));
-  const unsigned tri_grid = grid_for(n_touched, SYM_WARPS);
-  const unsigned rnd_grid = grid_for(n_chunks, RSYM_WARPS);
-  if (n_chunks > 0) {
-    k_round_symbolic<<<rnd_grid, 32 * RSYM_WARPS, 0, st>>>(
-        q->tris, ctx->touched.as<int>(), ctx->rdesc.as<int4>(), n_chunks, ctx->tfirst.as<int>(), ctx->keys_sorted,
-        ctx->dvals_sorted, bitsT, ctx->vcnt.as<int>(), (ctx->opt.flags & TT_FLAG_FORCE_GENERAL_ROWS) ? 1 : 0,
-        ctx->erank.as<int>(), ctx->drank.as<int>(), ctx->rowlen.as<int>(), ctx->tlen.as<int64_t>(),
-        ctx->slot_excl.as<uint8_t>(), ctx->everts.as<int>(), ctx->vslot1.as<int>());
-    TT_LAUNCH_CHECK();
-  }
-  if (n_long > 0) {  // triangles with more than RND_MAX_ENT partners: one warp per triangle
-    k_tri_symbolic<<<grid_for(n_long, SYM_WARPS), 32 * SYM_WARPS, 0, st>>>(
-        q->tris, ctx->touched.as<int>(), n_long, ctx->tptr.as<int>(), ctx->keys_sorted, ctx->dvals_sorted, bitsT,
-        ctx->vcnt.as<int>(), (ctx->opt.flags & TT_FLAG_FORCE_GENERAL_ROWS) ? 1 : 0, ctx->erank.as<int>(),
-        ctx->drank.as<int>(), ctx->rowlen.as<int>(), ctx->tlen.as<int64_t>(), ctx->slot_excl.as<uint8_t>(),
-        ctx->long_list.as<int>(), ctx->rdesc.as<int4>(), ctx->vslot1.as<int>(), ctx->everts.as<int>());
-    TT_LAUNCH_CHECK();
-  }
-  s = scan_i64(ctx, ctx->tlen.as<int64_t>(), ctx->toff.as<int64_t>(), 3 * n_touched + 1, st);
-  if (s != TT_OK) return s;
-  // The row-pointer scan is issued speculatively: if there are no general rows (R == 0: always, in a
-  // soup) the exclusive row lengths are already final and nnzb arrives in the same host round trip.
-  TT_CUDA(ctx->rowptr64.ensure(sizeof(int64_t) * (size_t)(nV + 1)));
-  TT_CUDA(ctx->rowptr.ensure(sizeof(int) * (size_t)(nV + 1)));
-  s = scan_i32_to_i64(ctx, ctx->rowlen.as<int>(), ctx->rowptr64.as<int64_t>(), nV + 1, st);
-  if (s != TT_OK) return s;
-  int64_t R = 0, nnzb = 0;
-  TT_CUDA(cudaMemcpyAsync(&R, ctx->toff.as<int64_t>() + 3 * n_touched, sizeof(int64_t), cudaMemcpyDeviceToHost, st));
-  TT_CUDA(cudaMemcpyAsync(&nnzb, ctx->rowptr64.as<int64_t>() + nV, sizeof(int64_t), cudaMemcpyDeviceToHost, st));
-  TT_CUDA(cudaStreamSynchronize(st));
   if (R >= (int64_t(1) << 31)) return fail(ctx, TT_ERR_INVALID_ARG, "general-row workspace exceeds 2^31 blocks");
   ctx->R = R;
+  const unsigned tri_grid = grid_for(n_touched, SYM_WARPS);
+  const unsigned rnd_grid = grid_for(n_chunks, RSYM_WARPS);
 
   // ---- general rows: merge records sorted by (row, col) ----
   int64_t U = 0;
@@ -494,7 +525,7 @@ tt_status symbolic_impl(tt_ctx* ctx, const tt_problem* q, int64_t* nnzb_host, in
     TT_CUDA(ctx->run_start.ensure(sizeof(int) * (size_t)(R + 1)));
     TT_CUDA(ctx->run_dest.ensure(sizeof(int) * (size_t)(R + 1)));
     k_emit_records<<<tri_grid, 32 * SYM_WARPS, 0, st>>>(
-        q->tris, ctx->touched.as<int>(), n_touched, ctx->tptr.as<int>(), ctx->keys_sorted, bitsT, bitsV,
+        q->tris, ctx->touched.as<int>(), n_touched, ctx->tfirst.as<int>(), ctx->partner.as<int>(), bitsV,
         ctx->erank.as<int>(), ctx->drank.as<int>(), ctx->toff.as<int64_t>(), ctx->slot_excl.as<uint8_t>(),
         ctx->rkeys[0].as<uint64_t>(), ctx->rvals[0].as<uint32_t>());
     TT_LAUNCH_CHECK();
@@ -505,23 +536,19 @@ tt_status symbolic_impl(tt_ctx* ctx, const tt_problem* q, int64_t* nnzb_host, in
     s = incl_scan_i32(ctx, ctx->head.as<int>(), ctx->ord.as<int>(), R, st);
     if (s != TT_OK) return s;
     k_record_rows<<<grid_for(R, 256), 256, 0, st>>>(ctx->rkeys_sorted, R, bitsV, ctx->head.as<int>(),
-                                                    ctx->ord.as<int>(), ctx->rowlen.as<int>(),
+                                                    ctx->ord.as<int>(), rowlen,
                                                     ctx->rowfirst.as<int>(), ctx->run_start.as<int>());
     TT_LAUNCH_CHECK();
+    // row pointers again: the general rows have added their (deduplicated) lengths
+    s = scan_i32_to_i64(ctx, rowlen, ctx->rowptr64.as<int64_t>(), nV + 1, st);
+    if (s != TT_OK) return s;
     int u32 = 0;
     TT_CUDA(cudaMemcpyAsync(&u32, ctx->ord.as<int>() + (R - 1), sizeof(int), cudaMemcpyDeviceToHost, st));
+    TT_CUDA(cudaMemcpyAsync(&nnzb, ctx->rowptr64.as<int64_t>() + nV, sizeof(int64_t), cudaMemcpyDeviceToHost, st));
     TT_CUDA(cudaStreamSynchronize(st));
     U = u32;
   }
   ctx->U = U;
-
-  // ---- row pointers (again, if general rows added to the row lengths) ----
-  if (R > 0) {
-    s = scan_i32_to_i64(ctx, ctx->rowlen.as<int>(), ctx->rowptr64.as<int64_t>(), nV + 1, st);
-    if (s != TT_OK) return s;
-    TT_CUDA(cudaMemcpyAsync(&nnzb, ctx->rowptr64.as<int64_t>() + nV, sizeof(int64_t), cudaMemcpyDeviceToHost, st));
-    TT_CUDA(cudaStreamSynchronize(st));
-  }
   if (nnzb >= (int64_t(1) << 31)) return fail(ctx, TT_ERR_INVALID_ARG, "nnzb %lld exceeds int32 BSR indexing", (long long)nnzb);
   ctx->nnzb = nnzb;
   k_i64_to_i32<<<grid_for(nV + 1, 256), 256, 0, st>>>(ctx->rowptr64.as<int64_t>(), nV + 1, ctx->rowptr.as<int>());
@@ -535,14 +562,14 @@ tt_status symbolic_impl(tt_ctx* ctx, const tt_problem* q, int64_t* nnzb_host, in
   }
   if (n_chunks > 0) {
     k_round_fill<<<rnd_grid, 32 * RSYM_WARPS, 0, st>>>(
-        q->tris, ctx->touched.as<int>(), ctx->rdesc.as<int4>(), n_chunks, ctx->tfirst.as<int>(), ctx->keys_sorted, bitsT,
+        q->tris, ctx->touched.as<int>(), ctx->rdesc.as<int4>(), n_chunks, ctx->tfirst.as<int>(), ctx->partner.as<int>(),
         ctx->erank.as<int>(), ctx->drank.as<int>(), ctx->toff.as<int64_t>(), ctx->slot_excl.as<uint8_t>(),
         ctx->rowptr.as<int>(), ctx->rowbase.as<int64_t>(), ctx->colind.as<int>());
     TT_LAUNCH_CHECK();
   }
   if (n_long > 0) {
     k_fill_rows<<<grid_for(n_long, SYM_WARPS), 32 * SYM_WARPS, 0, st>>>(
-        q->tris, ctx->touched.as<int>(), n_long, ctx->tptr.as<int>(), ctx->keys_sorted, bitsT,
+        q->tris, ctx->touched.as<int>(), n_long, ctx->tfirst.as<int>(), ctx->partner.as<int>(),
         ctx->erank.as<int>(), ctx->drank.as<int>(), ctx->toff.as<int64_t>(), ctx->slot_excl.as<uint8_t>(),
         ctx->rowptr.as<int>(), ctx->rowbase.as<int64_t>(), ctx->colind.as<int>(), ctx->long_list.as<int>(),
         ctx->rdesc.as<int4>());
@@ -591,8 +618,7 @@ template <typename T>
 ttk::AsmParams<T> make_params(tt_ctx* ctx, const tt_problem* q) {
   ttk::AsmParams<T> p;
   p.pos = (const T*)q->pos;
-  p.keys = ctx->keys_sorted;
-  p.dvals = ctx->dvals_sorted;
+  p.dvals = ctx->dvals.as<uint16_t>();
   p.everts = ctx->everts.as<int>();
   p.rdesc = ctx->rdesc.as<int4>();
   p.tfirst = ctx->tfirst.as<int>();
@@ -607,7 +633,6 @@ ttk::AsmParams<T> make_params(tt_ctx* ctx, const tt_problem* q) {
   p.n_chunks = ctx->n_chunks;
   p.n_long = ctx->n_long;
   p.pvec = nullptr;
-  p.bitsT = ctx->bitsT;
   p.hess_mode = ctx->opt.hess_mode;
   p.sigma = ctx->opt.tc_scale;
   return p;
@@ -648,6 +673,7 @@ tt_status numeric_impl(tt_ctx* ctx, const tt_problem* q, void* energy_sum, void*
   p.vals = (T*)vals;
   if (ctx->n_chunks > 0) {
     cudaEvent_t* ev_k4 = ctx->evr[1][ctx->ev_n[1] % tt_ctx::EV_RING];
+    l2_window(ctx, st, q->pos, sizeof(T) * 3 * (size_t)q->n_verts);
     TT_CUDA(cudaEventRecord(ev_k4[0], st));
     if (want_h) {
       const size_t smem = sizeof(TileWarpSmem<T>) * TILE_WARPS;
@@ -671,6 +697,7 @@ tt_status numeric_impl(tt_ctx* ctx, const tt_problem* q, void* energy_sum, void*
     }
     TT_LAUNCH_CHECK();
     TT_CUDA(cudaEventRecord(ev_k4[1], st));
+    l2_window_off(ctx, st);
     ctx->ev_n[1]++;
     if (want_h && ctx->U > 0) {
       k_merge<T><<<grid_for(9 * ctx->U, 256), 256, 0, st>>>(ctx->run_start.as<int>(), ctx->run_dest.as<int>(),
@@ -679,7 +706,7 @@ tt_status numeric_impl(tt_ctx* ctx, const tt_problem* q, void* energy_sum, void*
     }
   }
   if (grad && nV > 0) {
-    k_gather3<T><<<grid_for(nV, 256), 256, 0, st>>>(ctx->vcnt.as<int>(), ctx->vslot1.as<int>(), ctx->vptr.as<int>(), ctx->vvals_sorted, nV, ctx->tslot.as<T>(), (T*)grad);
+    k_gather3<T><<<grid_for(nV, 256), 256, 0, st>>>(ctx->vcnt_p, ctx->vslot1.as<int>(), ctx->vptr.as<int>(), ctx->vvals_sorted, nV, ctx->tslot.as<T>(), (T*)grad);
     TT_LAUNCH_CHECK();
   }
   return sum_partials<T>(ctx, ctx->asm_energy.as<double>(), ctx->n_chunks, (T*)energy_sum, st);
@@ -693,14 +720,16 @@ tt_status hessvec_impl(tt_ctx* ctx, const tt_problem* q, const void* pvec, void*
   p.chunk_energy = nullptr;
   if (ctx->n_chunks > 0) {
     cudaEvent_t* ev_k6 = ctx->evr[2][ctx->ev_n[2] % tt_ctx::EV_RING];
+    l2_window(ctx, st, q->pos, sizeof(T) * 3 * (size_t)q->n_verts);
     TT_CUDA(cudaEventRecord(ev_k6[0], st));
     tt_status s1 = launch_entry_reduce<T, 2>(ctx, p, st);
     if (s1 != TT_OK) return s1;
     TT_CUDA(cudaEventRecord(ev_k6[1], st));
+    l2_window_off(ctx, st);
     ctx->ev_n[2]++;
   }
   if (q->n_verts > 0) {
-    k_gather3<T><<<grid_for(q->n_verts, 256), 256, 0, st>>>(ctx->vcnt.as<int>(), ctx->vslot1.as<int>(), ctx->vptr.as<int>(), ctx->vvals_sorted, q->n_verts,
+    k_gather3<T><<<grid_for(q->n_verts, 256), 256, 0, st>>>(ctx->vcnt_p, ctx->vslot1.as<int>(), ctx->vptr.as<int>(), ctx->vvals_sorted, q->n_verts,
                                                                 ctx->tslot.as<T>(), (T*)y);
     TT_LAUNCH_CHECK();
   }
@@ -925,6 +954,23 @@ tt_status tt_create(const tt_options* opt, tt_ctx** out) {
     pipe_setup((const void*)ttk::k_entry_pipe<float, 1>, sizeof(ttk::PipeWarpSmem<float, 1>) * ttk::PIPE_WARPS, c->pipe_grid[1][0]);
     pipe_setup((const void*)ttk::k_entry_pipe<float, 2>, sizeof(ttk::PipeWarpSmem<float, 2>) * ttk::PIPE_WARPS, c->pipe_grid[1][1]);
     if (e != cudaSuccess) { (void)cudaGetLastError(); delete c; return TT_ERR_CUDA; }
+    c->sms = sms;
+    if (const char* env = getenv("TT_L2_PERSIST")) {  // experiment switch: fraction of the maximum set-aside
+      const double frac = atof(env);
+      int max_persist = 0, max_win = 0;
+      cudaDeviceGetAttribute(&max_persist, cudaDevAttrMaxPersistingL2CacheSize, opt->device);
+      cudaDeviceGetAttribute(&max_win, cudaDevAttrMaxAccessPolicyWindowSize, opt->device);
+      if (frac > 0.0 && max_persist > 0 && max_win > 0) {
+        const size_t want = (size_t)(frac * (double)max_persist);
+        if (cudaDeviceSetLimit(cudaLimitPersistingL2CacheSize, want) == cudaSuccess) {
+          c->l2_persist_bytes = want;
+          c->l2_max_window = (size_t)max_win;
+        } else {
+          (void)cudaGetLastError();
+        }
+      }
+      if (getenv("TT_VERBOSE")) fprintf(stderr, "[tt] L2 persisting: max %d B, window max %d B, set-aside %zu B\n", max_persist, max_win, c->l2_persist_bytes);
+    }
     c->tile_grid[0] = sms * (nb0 > 0 ? nb0 : 1);  // one wave of resident CTAs: the kernel is persistent
     c->tile_grid[1] = sms * (nb1 > 0 ? nb1 : 1);
   }

@@ -80,19 +80,27 @@ k_block_jacobi(const int* __restrict__ rowptr, const int* __restrict__ colind, c
 #pragma unroll
     for (int k = 0; k < 9; ++k) a[k] += (double)__ldg(vals + 9 * (int64_t)lo + k);
   }
-  const double c00 = a[4] * a[8] - a[5] * a[7], c01 = a[5] * a[6] - a[3] * a[8], c02 = a[3] * a[7] - a[4] * a[6];
-  const double det = a[0] * c00 + a[1] * c01 + a[2] * c02;
+  // 2x2 minors as Kahan's difference of products (error <= 1.5 ulp each: with a large low-rank block plus a
+  // small shift the plain a*d - b*c loses every digit the shift contributes), determinant along the first row
+  auto dop = [](double p, double q, double r, double t) {  // p*q - r*t
+    const double w = r * t;
+    const double e = fma(-r, t, w);
+    const double f = fma(p, q, -w);
+    return f + e;
+  };
+  const double c00 = dop(a[4], a[8], a[5], a[7]), c01 = dop(a[5], a[6], a[3], a[8]), c02 = dop(a[3], a[7], a[4], a[6]);
+  const double det = fma(a[0], c00, fma(a[1], c01, a[2] * c02));
   const double id = 1.0 / det;
   T* o = minv + 9 * v;
   o[0] = (T)(c00 * id);
-  o[1] = (T)((a[2] * a[7] - a[1] * a[8]) * id);
-  o[2] = (T)((a[1] * a[5] - a[2] * a[4]) * id);
+  o[1] = (T)(dop(a[2], a[7], a[1], a[8]) * id);
+  o[2] = (T)(dop(a[1], a[5], a[2], a[4]) * id);
   o[3] = (T)(c01 * id);
-  o[4] = (T)((a[0] * a[8] - a[2] * a[6]) * id);
-  o[5] = (T)((a[2] * a[3] - a[0] * a[5]) * id);
+  o[4] = (T)(dop(a[0], a[8], a[2], a[6]) * id);
+  o[5] = (T)(dop(a[2], a[3], a[0], a[5]) * id);
   o[6] = (T)(c02 * id);
-  o[7] = (T)((a[1] * a[6] - a[0] * a[7]) * id);
-  o[8] = (T)((a[0] * a[4] - a[1] * a[3]) * id);
+  o[7] = (T)(dop(a[1], a[6], a[0], a[7]) * id);
+  o[8] = (T)(dop(a[0], a[4], a[1], a[3]) * id);
 }
 
 // ---- fixed-order reductions -------------------------------------------------------------------------
