@@ -217,7 +217,10 @@ tt_status tt_pcg_solve(tt_ctx* ctx, const tt_problem* prob, const int32_t* rowpt
 
 /* Counters of the last tt_hess_symbolic: what[0]=n_active, [1]=directed entries (2*n_active),
  * [2]=touched triangles, [3]=blocks written directly (exclusive rows), [4]=blocks produced by the
- * general-row merge, [5]=merge records, [6]=nnzb, [7]=kernels launched by this ctx so far (CUB calls counted by the kernels they launch).                     */
+ * general-row merge, [5]=merge records, [6]=nnzb, [7]=kernels launched by this ctx so far (CUB calls
+ * counted by the kernels they launch), [8]=slots of the work partition, [9]=triangles with more than 32
+ * partners that were split into parts, [10]=parts, [11]=such triangles that could not be split (rounds of
+ * their own, long-triangle kernels).                                                                 */
 tt_status tt_stats(const tt_ctx* ctx, int64_t* what, int32_t n);
 
 /* Device durations (CUDA events on the caller's stream) of the most recent launch of the three

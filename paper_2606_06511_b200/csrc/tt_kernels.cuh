@@ -26,6 +26,7 @@ using ttg::d3;
 constexpr int CLS_THREADS = 256;   // K1 / K2 CTA size (8 warps -> 8 mask words per CTA)
 constexpr int SYM_WARPS = 4;       // warps per CTA in the per-triangle symbolic kernels
 constexpr int SYM_LMAX = 1536;     // longest row (in blocks) ranked in shared memory
+constexpr int SLOT_PART = (int)0x80000000;  // flag in sinfo.x: the slot is a part of a split triangle
 
 // One vertex = three consecutive values at an address that is only value-aligned: exactly one of
 // p, p + 1 is aligned for a two-value load, so a vertex costs two gather requests (one 2-wide, one
@@ -106,18 +107,22 @@ __device__ __forceinline__ double block_sum(double v, double* smem /*[THREADS/32
 #ifndef TT_CLS_MIN_CTAS
 #define TT_CLS_MIN_CTAS 3   // 85 registers, 24 warps / SM: 0.755 -> 0.69 ms at 10M candidates (4: 0.73)
 #endif
+// Per-candidate record written by K1 for the symbolic phase: recorded branch decisions (ttg::pair_config,
+// 12 bits) | place of the entry a -> b in a's segment (26 bits) | place of b -> a in b's segment (26 bits).
+constexpr int REC_P0_SHIFT = 12, REC_P1_SHIFT = 38;
+constexpr unsigned long long REC_CFG_MASK = 0xfffull, REC_P_MASK = 0x3ffffffull;
 template <typename T>
 __global__ void __launch_bounds__(CLS_THREADS, TT_CLS_MIN_CTAS)
 k_classify(const T* __restrict__ pos, const int* __restrict__ tris, const int2* __restrict__ pairs,
            int64_t P, double sigma, uint32_t* __restrict__ mask, int* __restrict__ blk_count,
            double* __restrict__ blk_energy, T* __restrict__ e_pp, T* __restrict__ tc_out,
-           uint16_t* __restrict__ cfg_out, int* __restrict__ deg) {
+           uint64_t* __restrict__ rec_out, int* __restrict__ deg) {
   __shared__ double s_e[CLS_THREADS / 32];
   __shared__ int s_c[CLS_THREADS / 32];
   const int64_t k = (int64_t)blockIdx.x * CLS_THREADS + threadIdx.x;
   bool active = false;
   double tc0 = 0.0, tc1 = 0.0, en = 0.0;
-  unsigned cfg = 0u;
+  unsigned long long cfg = 0ull;
   if (k < P) {
     const int2 pr = __ldg(pairs + k);
     int va[3], vb[3];
@@ -131,13 +136,18 @@ k_classify(const T* __restrict__ pos, const int* __restrict__ tris, const int2* 
         const double pr2 = tc0 * tc1;
         en = pr2 * pr2;  // Eq. 2
         cfg = ttg::pair_config(g);
-        if (deg) {  // histogram of the directed entries by source triangle (integer RED: the result is order independent)
-          atomicAdd(deg + pr.x, 1);
-          atomicAdd(deg + pr.y, 1);
+        if (deg) {
+          // Counting sort of the directed entries by source triangle, first half: the histogram, and -- the
+          // value the atomic returns -- this entry's place inside its triangle's segment.  (Integer atomics:
+          // WHICH place an entry gets depends on the schedule, the segment's CONTENT does not, and every
+          // segment is sorted before anything depends on its order.)
+          const unsigned long long p0 = (unsigned)atomicAdd(deg + pr.x, 1);
+          const unsigned long long p1 = (unsigned)atomicAdd(deg + pr.y, 1);
+          cfg |= (p0 << REC_P0_SHIFT) | (p1 << REC_P1_SHIFT);
         }
       }
     }
-    if (cfg_out) cfg_out[k] = (uint16_t)cfg;
+    if (rec_out) rec_out[k] = cfg;
     if (e_pp) e_pp[k] = (T)en;
     if (tc_out) {
       tc_out[2 * k] = (T)tc0;
@@ -195,15 +205,15 @@ __global__ void k_set_count(const int* __restrict__ blk_off, const int* __restri
 // Order-preserving compaction of the active pair ids (ballot / popc positions + per-CTA offsets) and, in
 // the same pass, the COUNTING SORT of the directed entries by source triangle: active pair (s, t) becomes
 // the entries s -> t (side 0) and t -> s (side 1); K1 has counted the entries of every triangle (deg), the
-// scan of deg is tptr, and an entry takes the next free place of its triangle's segment (integer atomics).
-// The order INSIDE a segment is whatever the atomics give; the symbolic kernels sort every segment by
+// scan of deg is tptr, and an entry goes to the place inside its triangle's segment that K1's atomic returned.
+// The order INSIDE a segment is whatever the atomics gave; the symbolic kernels sort every segment by
 // (partner, side) before anything depends on it, so all results are deterministic (two entries with the
 // same key are the same pair listed twice: bit-identical contributions).
 //   ent[slot] = (partner triangle, side | recorded config of the canonical pair << 1)
 __global__ void __launch_bounds__(CLS_THREADS)
 k_compact(const uint32_t* __restrict__ mask, const int* __restrict__ blk_off, int64_t P,
-          int* __restrict__ active_ids, const int2* __restrict__ pairs, const uint16_t* __restrict__ cfg,
-          const int* __restrict__ tptr, int* __restrict__ fill, uint2* __restrict__ ent) {
+          int* __restrict__ active_ids, const int2* __restrict__ pairs, const uint64_t* __restrict__ rec,
+          const int* __restrict__ tptr, uint2* __restrict__ ent) {
   const int64_t k = (int64_t)blockIdx.x * CLS_THREADS + threadIdx.x;
   const int w = threadIdx.x >> 5, l = threadIdx.x & 31;
   const int64_t word0 = (int64_t)blockIdx.x * (CLS_THREADS / 32);
@@ -217,12 +227,15 @@ k_compact(const uint32_t* __restrict__ mask, const int* __restrict__ blk_off, in
   }
   if ((mine >> l) & 1u) {
     const int64_t a = (int64_t)blk_off[blockIdx.x] + before + __popc(mine & ((1u << l) - 1u));
-    active_ids[a] = (int)k;
+    __stcs(active_ids + a, (int)k);
     if (ent) {
-      const int2 pr = __ldg(pairs + k);
-      const unsigned c = (unsigned)__ldg(cfg + k) << 1;
-      const int sa = __ldg(tptr + pr.x) + atomicAdd(fill + pr.x, 1);
-      const int sb = __ldg(tptr + pr.y) + atomicAdd(fill + pr.y, 1);
+      // streaming loads / stores for everything that is touched once, so that the 8-byte scattered
+      // stores of the entries find their lines still in L2 when the line's other entries arrive
+      const int2 pr = __ldcs(pairs + k);
+      const unsigned long long r = __ldcs(rec + k);
+      const unsigned c = (unsigned)(r & REC_CFG_MASK) << 1;
+      const int sa = __ldg(tptr + pr.x) + (int)((r >> REC_P0_SHIFT) & REC_P_MASK);
+      const int sb = __ldg(tptr + pr.y) + (int)((r >> REC_P1_SHIFT) & REC_P_MASK);
       ent[sa] = make_uint2((unsigned)pr.y, c);
       ent[sb] = make_uint2((unsigned)pr.x, c | 1u);
     }
@@ -287,7 +300,7 @@ __device__ __forceinline__ void warp_sort_segment(const uint2* __restrict__ ent,
   __syncwarp();
 }
 
-// Per LONG touched triangle s (more than RND_MAX_ENT partners; one warp): sorts its entries, then
+// Per LONG touched triangle s that k_long_prep could not split (one warp; the segment is already sorted):
 // candidate columns C = verts(partners in sorted order) ++ verts(s), L = 3 (deg + 1).  Ranks each
 // candidate among C by counting (shared memory, all pairs), detects duplicates, decides which of the
 // three rows are EXCLUSIVE (vertex used by no other touched triangle, no duplicate column) and records:
@@ -295,15 +308,15 @@ __device__ __forceinline__ void warp_sort_segment(const uint2* __restrict__ ent,
 //   drank[ti][n]  position of the diagonal column n
 //   rowlen[p]     = L for exclusive rows;  tlen[3ti+m] = L for general rows (their blocks go to
 //                 the merge workspace, one merge record each)
-// Per-slot arrays (drank, tlen, toff, slot_excl, rowbase, tslot) are indexed by TOUCHED index ti:
-// the numeric kernels then need no triangle id to find them.
+// Per-slot arrays (drank, tlen, toff, slot_excl, rowbase, tslot) are indexed by SLOT (here: the triangle's
+// only slot): the numeric kernels then need no triangle id to find them.
 // layout = rank (columns ascending) when there is no duplicate, else identity (3j+n, diag last).
 // Duplicates are detected as in k_round_symbolic: the ranks of L distinct values sum to L (L - 1) / 2.
 // Also writes the per-entry vertex ids (everts) of the triangle's entries.
 __global__ void __launch_bounds__(32 * SYM_WARPS)
 k_tri_symbolic(const int* __restrict__ tris, const int* __restrict__ touched, const int* __restrict__ n_long_dev,
-               const int* __restrict__ tfirst, const uint2* __restrict__ ent, int* partner /*sorted, out*/,
-               uint16_t* dvals /*sorted, out*/, const int* __restrict__ vcnt, int force_general,
+               const int* __restrict__ tfirst, const int4* __restrict__ sinfo, const int* __restrict__ partner,
+               const uint16_t* __restrict__ dvals, const int* __restrict__ vcnt, int force_general,
                int* __restrict__ erank /*[2A][3]*/, int* __restrict__ drank /*[n_touched][3]*/, int* __restrict__ rowlen,
                int64_t* __restrict__ tlen /*[3 n_touched]*/, uint8_t* __restrict__ slot_excl /*[3 n_touched]*/,
                const int* __restrict__ long_list, const int4* __restrict__ rdesc, int* __restrict__ vslot1,
@@ -313,13 +326,13 @@ k_tri_symbolic(const int* __restrict__ tris, const int* __restrict__ touched, co
   const int w = threadIdx.x >> 5, l = threadIdx.x & 31;
   const int64_t n_long = *n_long_dev;
   for (int64_t li = (int64_t)blockIdx.x * SYM_WARPS + w; li < n_long; li += (int64_t)gridDim.x * SYM_WARPS) {
-    const int64_t ti = rdesc[long_list[li]].z;
+    const int64_t sl = rdesc[long_list[li]].z;
+    const int64_t ti = sinfo[sl].x;
     const int s = touched[ti];
     const int e0 = tfirst[ti], deg = tfirst[ti + 1] - e0;
     const int L = 3 * (deg + 1);
     int own[3];
     load3i(tris + 3 * (int64_t)s, own);
-    warp_sort_segment(ent + e0, deg, reinterpret_cast<unsigned long long*>(s_c[w]), SYM_LMAX / 2, partner + e0, dvals + e0, l);
     // vertex ids of the canonical pair of every entry, both triangles in recorded (k, p, q) order
     for (int j = l; j < deg; j += 32) {
       const int64_t e = (int64_t)e0 + j;
@@ -353,7 +366,7 @@ k_tri_symbolic(const int* __restrict__ tris, const int* __restrict__ touched, co
         sum += r;
         const int j = idx / 3, n = idx - 3 * j;
         if (j < deg) erank[3 * (int64_t)(e0 + j) + n] = r;
-        else drank[3 * ti + n] = r;
+        else drank[3 * sl + n] = r;
       }
 #pragma unroll
       for (int o = 16; o > 0; o >>= 1) sum += __shfl_xor_sync(FULL, sum, o);
@@ -363,15 +376,15 @@ k_tri_symbolic(const int* __restrict__ tris, const int* __restrict__ touched, co
       for (int idx = l; idx < L; idx += 32) {
         const int j = idx / 3, n = idx - 3 * j;
         if (j < deg) erank[3 * (int64_t)(e0 + j) + n] = idx;
-        else drank[3 * ti + n] = idx;
+        else drank[3 * sl + n] = idx;
       }
     }
     if (l < 3) {
       const int p = own[l == 0 ? 0 : (l == 1 ? 1 : 2)];
       const bool excl = nodup && !force_general && (vcnt[p] == 1);
-      if (vcnt[p] == 1) vslot1[p] = (int)(3 * ti + l);  // the vertex's only slot (k_gather3)
-      slot_excl[3 * ti + l] = excl ? 1 : 0;
-      tlen[3 * ti + l] = excl ? 0 : L;
+      if (vcnt[p] == 1) vslot1[p] = (int)(3 * sl + l);  // the vertex's only slot (k_gather3)
+      slot_excl[3 * sl + l] = excl ? 1 : 0;
+      tlen[3 * sl + l] = excl ? 0 : L;
       if (excl) rowlen[p] = L;
     }
     __syncwarp();  // s_c is reused by the next triangle
@@ -380,26 +393,29 @@ k_tri_symbolic(const int* __restrict__ tris, const int* __restrict__ touched, co
 
 // General rows: one merge record per workspace block: key = (row vertex << bitsV) | column vertex,
 // payload = workspace block index (assigned by the caller's iota; record index == block index).
+// One warp per slot (parts have exclusive rows: nothing to emit).
 __global__ void __launch_bounds__(32 * SYM_WARPS)
-k_emit_records(const int* __restrict__ tris, const int* __restrict__ touched, int64_t n_touched,
-               const int* __restrict__ tfirst, const int* __restrict__ partner, int bitsV,
+k_emit_records(const int* __restrict__ tris, const int* __restrict__ touched, int64_t n_slots,
+               const int* __restrict__ sfirst, const int4* __restrict__ sinfo, const int* __restrict__ partner, int bitsV,
                const int* __restrict__ erank, const int* __restrict__ drank, const int64_t* __restrict__ toff,
                const uint8_t* __restrict__ slot_excl, uint64_t* __restrict__ rkeys, uint32_t* __restrict__ rvals) {
   const int w = threadIdx.x >> 5, l = threadIdx.x & 31;
-  const int64_t ti = (int64_t)blockIdx.x * SYM_WARPS + w;
-  if (ti >= n_touched) return;
-  const int s = touched[ti];
-  const int e0 = tfirst[ti], deg = tfirst[ti + 1] - e0;
+  const int64_t sl = (int64_t)blockIdx.x * SYM_WARPS + w;
+  if (sl >= n_slots) return;
+  const int4 si = sinfo[sl];
+  if (si.x & SLOT_PART) return;
+  const int s = touched[si.x];
+  const int e0 = sfirst[sl], deg = sfirst[sl + 1] - e0;
   const int L = 3 * (deg + 1);
   for (int m = 0; m < 3; ++m) {
-    if (slot_excl[3 * ti + m]) continue;
+    if (slot_excl[3 * sl + m]) continue;
     const uint64_t p = (uint64_t)(uint32_t)tris[3 * (int64_t)s + m];
-    const int64_t base = toff[3 * ti + m];
+    const int64_t base = toff[3 * sl + m];
     for (int idx = l; idx < L; idx += 32) {
       const int j = idx / 3, n = idx - 3 * j;
       const int t = (j < deg) ? partner[e0 + j] : s;
       const int q = tris[3 * (int64_t)t + n];
-      const int r = (j < deg) ? erank[3 * (int64_t)(e0 + j) + n] : drank[3 * ti + n];
+      const int r = (j < deg) ? erank[3 * (int64_t)(e0 + j) + n] : drank[3 * sl + n];
       rkeys[base + r] = (p << bitsV) | (uint32_t)q;
       rvals[base + r] = (uint32_t)(base + r);
     }
@@ -440,23 +456,24 @@ __global__ void k_record_dest(const uint64_t* __restrict__ rkeys, int64_t U, int
   colind[dest] = q;
 }
 
-// Exclusive rows: column indices + row bases (>= 0: block index into vals; < 0: -(workspace+1)).
+// Long unsplittable triangles: column indices of their exclusive rows + row bases (>= 0: block index into
+// vals; < 0: -(workspace + 1)).
 __global__ void __launch_bounds__(32 * SYM_WARPS)
-k_fill_rows(const int* __restrict__ tris, const int* __restrict__ touched, int64_t n_touched,
-            const int* __restrict__ tfirst, const int* __restrict__ partner,
+k_fill_rows(const int* __restrict__ tris, const int* __restrict__ touched, int64_t n_long,
+            const int* __restrict__ sfirst, const int4* __restrict__ sinfo, const int* __restrict__ partner,
             const int* __restrict__ erank, const int* __restrict__ drank, const int64_t* __restrict__ toff,
             const uint8_t* __restrict__ slot_excl, const int* __restrict__ rowptr,
-            int64_t* __restrict__ rowbase /*[3 n_touched]*/, int* __restrict__ colind,
+            int64_t* __restrict__ rowbase /*[3 n_slots]*/, int* __restrict__ colind,
             const int* __restrict__ long_list, const int4* __restrict__ rdesc) {
   const int w = threadIdx.x >> 5, l = threadIdx.x & 31;
-  const int64_t li = (int64_t)blockIdx.x * SYM_WARPS + w;  // n_touched counts the LONG triangles here
-  if (li >= n_touched) return;
-  const int64_t ti = rdesc[long_list[li]].z;
-  const int s = touched[ti];
-  const int e0 = tfirst[ti], deg = tfirst[ti + 1] - e0;
+  const int64_t li = (int64_t)blockIdx.x * SYM_WARPS + w;
+  if (li >= n_long) return;
+  const int64_t sl = rdesc[long_list[li]].z;
+  const int s = touched[sinfo[sl].x];
+  const int e0 = sfirst[sl], deg = sfirst[sl + 1] - e0;
   const int L = 3 * (deg + 1);
   for (int m = 0; m < 3; ++m) {
-    const int64_t slot = 3 * ti + m;
+    const int64_t slot = 3 * sl + m;
     if (!slot_excl[slot]) {
       if (l == 0) rowbase[slot] = -(toff[slot] + 1);
       continue;
@@ -466,24 +483,39 @@ k_fill_rows(const int* __restrict__ tris, const int* __restrict__ touched, int64
     for (int idx = l; idx < L; idx += 32) {
       const int j = idx / 3, n = idx - 3 * j;
       const int t = (j < deg) ? partner[e0 + j] : s;
-      const int r = (j < deg) ? erank[3 * (int64_t)(e0 + j) + n] : drank[3 * ti + n];
+      const int r = (j < deg) ? erank[3 * (int64_t)(e0 + j) + n] : drank[3 * sl + n];
       colind[rp + r] = tris[3 * (int64_t)t + n];
     }
   }
 }
 
-// Work partition of K4/K6.  A ROUND is a run of consecutive touched triangles, kept whole, with at
-// most RND_MAX_ENT directed entries (one lane each) and RND_MAX_TRI triangles; one warp owns one
-// round.  A triangle with more than RND_MAX_ENT partners is a round of its own ("long": no smem
-// tile can hold its rows; K4 hands it to k_assemble_long).  Packing is greedy in touched order,
-// restarted at every bucket of CHK_BUCKET touched triangles so that buckets pack in parallel
-// (one thread per bucket; count pass, scan, fill pass).
+// Work partition of K4/K6.  A SLOT is what a warp treats as "one triangle's entries": a whole touched
+// triangle, or -- for a triangle with more than RND_MAX_ENT partners whose row layout allows it
+// (k_long_prep) -- a PART: a run of consecutive entries of its (partner-sorted) segment that does not
+// straddle the position of the diagonal columns.  A ROUND is a run of consecutive slots with at most
+// RND_MAX_ENT directed entries (one lane each) and RND_MAX_TRI slots; one warp owns one round.  Parts are
+// cut wherever a round fills up, so rounds that meet a splittable long triangle are full.  A long
+// triangle that cannot be split is a slot and a round of its own ("long": k_assemble_long*).
+// Packing is greedy in touched order, restarted at every bucket of CHK_BUCKET touched triangles so that
+// buckets pack in parallel (one thread per bucket; count pass, scan, fill pass).
 constexpr int RND_MAX_ENT = 32;
 #ifndef TT_RND_MAX_TRI
 #define TT_RND_MAX_TRI 8
 #endif
 constexpr int RND_MAX_TRI = TT_RND_MAX_TRI;
 constexpr int CHK_BUCKET = 128;
+
+struct PackCount {  // per-bucket counts, scanned together
+  int rounds, longs, slots, splits, parts;
+};
+struct PackAdd {
+  __host__ __device__ PackCount operator()(const PackCount& a, const PackCount& b) const {
+    return PackCount{a.rounds + b.rounds, a.longs + b.longs, a.slots + b.slots, a.splits + b.splits, a.parts + b.parts};
+  }
+};
+// sinfo[slot] = (touched index | SLOT_PART, unit offset of the part inside its triangle's row run, part ordinal
+// or -1, unused).  A unit is a group of 3 columns: entry j of a split triangle is unit j + (j >= pos_d), the
+// diagonal columns are unit pos_d.
 
 // tfirst[i] = first directed entry of touched triangle i; tfirst[n_touched] = n_dir
 __global__ void k_touched_first(const int* __restrict__ touched, const int* __restrict__ n_touched_dev,
@@ -494,60 +526,157 @@ __global__ void k_touched_first(const int* __restrict__ touched, const int* __re
   if (i == n_touched) tfirst[i] = tptr[nT];  // = number of directed entries
 }
 
-// FILL = false: bucket_cnt[b] = rounds of bucket b (+ long_cnt[b] = long triangles).
-// FILL = true : rdesc[bucket_off[b] + k] = descriptor of the k-th round of bucket b (first entry, entries,
-//               first touched index, triangles), long_list[long_off[b] + k] = round id of the k-th long triangle.
+// Long triangles (more than RND_MAX_ENT partners), one warp each: sorts the segment by (partner, side)
+// and decides whether the triangle can be SPLIT into parts.  It can when its three rows are exclusive and
+// the vertex-id intervals [min, max] of its partners (in sorted order) and of the triangle itself are
+// pairwise disjoint and ascending: the sorted columns of the row are then the partners' (sorted) triples
+// one after the other, with the triangle's own triple in between at unit pos_d = number of partners
+// below it -- so any run of consecutive entries owns a CONTIGUOUS piece of every row run, and the column
+// ranks need no counting.  (Always true in a soup, where a triangle's vertex ids are 3t, 3t+1, 3t+2.)
+//   tsplit[ti] = pos_d, or -1 (not splittable: k_tri_symbolic + the long assembly kernels)
+__device__ __forceinline__ int min3i(int a, int b, int c) { return min(a, min(b, c)); }
+__device__ __forceinline__ int max3i(int a, int b, int c) { return max(a, max(b, c)); }
+
+__global__ void __launch_bounds__(32 * SYM_WARPS)
+k_long_prep(const int* __restrict__ tris, const int* __restrict__ touched, const int* __restrict__ n_touched_dev,
+            const int* __restrict__ tfirst, const uint2* __restrict__ ent, const int* __restrict__ vcnt,
+            int force_general, int* partner, uint16_t* dvals, int* __restrict__ tsplit) {
+  __shared__ unsigned long long s_key[SYM_WARPS][SYM_LMAX / 2];
+  constexpr unsigned FULL = 0xffffffffu;
+  const int w = threadIdx.x >> 5, l = threadIdx.x & 31;
+  const int64_t n_touched = *n_touched_dev;
+  const int64_t stride = (int64_t)gridDim.x * SYM_WARPS * 32;
+  for (int64_t base = ((int64_t)blockIdx.x * SYM_WARPS + w) * 32; base < n_touched; base += stride) {
+    const int64_t mine = base + l;
+    const int dmine = (mine < n_touched) ? __ldg(tfirst + mine + 1) - __ldg(tfirst + mine) : 0;
+    unsigned todo = __ballot_sync(FULL, dmine > RND_MAX_ENT);
+    while (todo) {
+      const int b = __ffs(todo) - 1;
+      todo &= todo - 1;
+      const int64_t ti = base + b;
+      const int s = __ldg(touched + ti);
+      const int e0 = __ldg(tfirst + ti), deg = __ldg(tfirst + ti + 1) - e0;
+      warp_sort_segment(ent + e0, deg, s_key[w], SYM_LMAX / 2, partner + e0, dvals + e0, l);
+      int own[3];
+      load3i(tris + 3 * (int64_t)s, own);
+      const int mn_s = min3i(own[0], own[1], own[2]), mx_s = max3i(own[0], own[1], own[2]);
+      bool ok = !force_general && __ldg(vcnt + own[0]) == 1 && __ldg(vcnt + own[1]) == 1 && __ldg(vcnt + own[2]) == 1;
+      int pos = 0;
+      for (int j = l; j < deg; j += 32) {
+        int cv[3];
+        load3i(tris + 3 * (int64_t)partner[e0 + j], cv);
+        const int mn = min3i(cv[0], cv[1], cv[2]), mx = max3i(cv[0], cv[1], cv[2]);
+        if (j + 1 < deg) {
+          int nv[3];
+          load3i(tris + 3 * (int64_t)partner[e0 + j + 1], nv);
+          ok = ok && (mx < min3i(nv[0], nv[1], nv[2]));
+        }
+        ok = ok && ((mx < mn_s) || (mx_s < mn));
+        pos += (mx < mn_s) ? 1 : 0;
+      }
+      ok = __all_sync(FULL, ok);
+#pragma unroll
+      for (int o = 16; o > 0; o >>= 1) pos += __shfl_xor_sync(FULL, pos, o);
+      if (l == 0) tsplit[ti] = ok ? pos : -1;
+      __syncwarp();  // s_key is reused by the next triangle
+    }
+  }
+}
+
+// FILL = false: bucket_cnt[b] = counts of bucket b.
+// FILL = true : round descriptors (first entry, entries, first slot, slots), slot tables, the list of
+//               long (unsplittable) rounds and the list of split triangles, at the offsets bucket_off[b].
 template <bool FILL>
 __global__ void k_chunk_pack(const int* __restrict__ tfirst, const int* __restrict__ n_touched_dev,
-                             int* __restrict__ bucket_cnt, int* __restrict__ long_cnt,
-                             const int* __restrict__ bucket_off, const int* __restrict__ long_off,
-                             int4* __restrict__ rdesc, int* __restrict__ long_list) {
+                             const int* __restrict__ tsplit, PackCount* __restrict__ bucket_cnt,
+                             const PackCount* __restrict__ bucket_off, int4* __restrict__ rdesc,
+                             int* __restrict__ long_list, int* __restrict__ sfirst, int4* __restrict__ sinfo,
+                             int4* __restrict__ split_list) {
   const int64_t b = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
   const int64_t n_touched = *n_touched_dev;  // still on the device: the grid covers its bound
   const int64_t n_buckets = (n_touched + CHK_BUCKET - 1) / CHK_BUCKET;
   if (b >= n_buckets) return;             // the counts of the buckets beyond stay zero
   const int64_t i0 = b * CHK_BUCKET, i1 = min(i0 + (int64_t)CHK_BUCKET, n_touched);
-  int nch = 0, nlong = 0, ent = 0, tri = 0;
-  const int cbase = FILL ? bucket_off[b] : 0, lbase = FILL ? long_off[b] : 0;
+  PackCount base = PackCount{0, 0, 0, 0, 0};
+  if (FILL) base = bucket_off[b];
+  int nch = 0, nlong = 0, nslot = 0, nsplit = 0, npart = 0, ent = 0, tri = 0;
   int e_i = tfirst[i0];
-  int t0 = (int)i0, e0 = e_i;             // the open round
+  int r_e0 = e_i, r_s0 = 0;               // the open round: first entry, first slot (relative to the bucket)
+  auto close_round = [&](int e_end) {
+    if (FILL && nch > 0) rdesc[base.rounds + nch - 1] = make_int4(r_e0, e_end - r_e0, base.slots + r_s0, nslot - r_s0);
+  };
+  auto open_round = [&](int e_begin) {
+    close_round(e_begin);
+    r_e0 = e_begin;
+    r_s0 = nslot;
+    ++nch;
+    ent = 0;
+    tri = 0;
+  };
+  auto add_slot = [&](int e_begin, int cnt, int ti_flag, int u0, int pidx) {
+    if (FILL) {
+      sfirst[base.slots + nslot] = e_begin;
+      sinfo[base.slots + nslot] = make_int4(ti_flag, u0, pidx, 0);
+    }
+    ++nslot;
+    ent += cnt;
+    tri += 1;
+  };
   for (int64_t i = i0; i < i1; ++i) {
     const int e_next = tfirst[i + 1];
     const int d = e_next - e_i;
-    const bool is_long = d > RND_MAX_ENT;
-    if (tri == 0 || is_long || ent + d > RND_MAX_ENT || tri + 1 > RND_MAX_TRI) {  // open a new round at i
-      if (FILL && nch > 0) rdesc[cbase + nch - 1] = make_int4(e0, e_i - e0, t0, (int)i - t0);
-      t0 = (int)i;
-      e0 = e_i;
-      if (is_long) {
-        if (FILL) long_list[lbase + nlong] = cbase + nch;
+    if (d <= RND_MAX_ENT) {
+      if (tri == 0 || ent + d > RND_MAX_ENT || tri + 1 > RND_MAX_TRI) open_round(e_i);
+      add_slot(e_i, d, (int)i, 0, -1);
+    } else {
+      const int sp = tsplit[i];
+      if (sp < 0) {  // a round of its own
+        open_round(e_i);
+        if (FILL) long_list[base.longs + nlong] = base.rounds + nch - 1;
         ++nlong;
+        add_slot(e_i, d, (int)i, 0, -1);
+        tri = RND_MAX_TRI;  // closes the round: the next slot opens a new one
+      } else {
+        const int first_slot = nslot;
+        if (FILL) split_list[base.splits + nsplit] = make_int4(base.slots + nslot, 0, (int)i, base.parts + npart);
+#pragma unroll 1
+        for (int seg = 0; seg < 2; ++seg) {  // entries below / above the diagonal columns
+          int j = seg ? sp : 0;
+          const int j1 = seg ? d : sp;
+          while (j < j1) {
+            if (tri == 0 || ent >= RND_MAX_ENT || tri + 1 > RND_MAX_TRI) open_round(e_i + j);
+            const int take = min(j1 - j, RND_MAX_ENT - ent);
+            add_slot(e_i + j, take, (int)i | SLOT_PART, j + seg, base.parts + npart);
+            ++npart;
+            j += take;
+          }
+        }
+        if (FILL) split_list[base.splits + nsplit].y = nslot - first_slot;
+        ++nsplit;
       }
-      ++nch;
-      ent = 0;
-      tri = 0;
     }
-    ent += d;
-    tri += 1;
-    if (is_long) tri = RND_MAX_TRI;  // closes the round: the next triangle opens a new one
     e_i = e_next;
   }
-  if (FILL && nch > 0) rdesc[cbase + nch - 1] = make_int4(e0, e_i - e0, t0, (int)i1 - t0);
-  if (!FILL) {
-    bucket_cnt[b] = nch;
-    long_cnt[b] = nlong;
-  }
+  close_round(e_i);
+  if (FILL && b == n_buckets - 1) sfirst[base.slots + nslot] = e_i;  // sentinel: number of directed entries
+  if (!FILL) bucket_cnt[b] = PackCount{nch, nlong, nslot, nsplit, npart};
 }
 
-// vertex -> touched (triangle, slot) incidence keys: key = vertex, payload = slot 3 ti + m
-__global__ void k_emit_vslots(const int* __restrict__ tris, const int* __restrict__ touched,
-                              int64_t n_touched, uint64_t* __restrict__ vkeys, uint32_t* __restrict__ vvals) {
+// vertex -> slot incidence keys: key = vertex, payload = 3 slot + m.  Only the slot that holds a triangle's
+// summed gradient / H.p partial takes part: whole slots and the FIRST part of a split triangle
+// (k_split_finish adds the other parts into it); the others get the key nV, which sorts past every vertex.
+__global__ void k_emit_vslots(const int* __restrict__ tris, const int* __restrict__ touched, int64_t n_slots,
+                              const int4* __restrict__ sinfo, const int* __restrict__ tsplit, int64_t nV,
+                              uint64_t* __restrict__ vkeys, uint32_t* __restrict__ vvals) {
   const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
-  if (i >= 3 * n_touched) return;
-  const int64_t ti = i / 3;
-  const int m = (int)(i - 3 * ti);
-  const int s = touched[ti];
-  vkeys[i] = (uint64_t)(uint32_t)tris[3 * (int64_t)s + m];
+  if (i >= 3 * n_slots) return;
+  const int64_t sl = i / 3;
+  const int m = (int)(i - 3 * sl);
+  const int4 si = sinfo[sl];
+  const int ti = si.x & ~SLOT_PART;
+  bool holder = true;
+  if (si.x & SLOT_PART) holder = (si.y == 0) || (si.y == 1 && tsplit[ti] == 0);
+  vkeys[i] = holder ? (uint64_t)(uint32_t)tris[3 * (int64_t)touched[ti] + m] : (uint64_t)nV;
   vvals[i] = (uint32_t)i;
 }
 
@@ -594,15 +723,16 @@ struct AsmParams {
   const uint16_t* dvals;    // side | recorded config << 1 (ttg::pair_config)
   const int* everts;        // [2A][6] vertex ids of the canonical pair, both triangles in recorded order
   const int4* rdesc;        // [n_chunks] round descriptor: first entry, entries, first touched index, triangles
-  const int* tfirst;        // [n_touched+1]
+  const int* tfirst;        // [n_slots+1] first entry of every slot
   const int* long_list;     // [n_long] round ids of the long triangles
   const int* erank;         // [2A][3]
-  const int* drank;         // [n_touched][3]
-  const int64_t* rowbase;   // [3 n_touched]
+  const int* drank;         // [n_slots][3]; a part: [0] = -1 - part ordinal
+  const int64_t* rowbase;   // [3 n_slots]
   T* vals;                  // final BSR values
   T* tvals;                 // merge workspace values
-  T* tslot;                 // [3 n_touched][3] per-slot gradient (K4) or H.p (K6) partials
+  T* tslot;                 // [3 n_slots][3] per-slot gradient (K4) or H.p (K6) partials
   double* chunk_energy;     // [n_chunks]
+  double* dpart;            // [n_parts][NDIAG] diagonal partial sums of the parts of split triangles
   const T* pvec;            // K6: p [nV,3]
   int64_t n_chunks;
   int64_t n_long;
@@ -620,19 +750,28 @@ constexpr int RSYM_WARPS = 4;
 // Segment sort by (partner, side), column ranks (erank / drank), duplicate detection, exclusive rows,
 // row lengths and the per-entry vertex ids (everts) of every non-long round.  Persistent grid: a warp
 // walks rounds c, c + G, ... (the number of rounds is still on the device when this kernel is enqueued).
+// Lane = slot for the per-slot work, lane = directed entry for the per-entry work.
+//   whole slot: its segment is sorted here.  Ranks: if the vertex-id intervals of the (sorted) partners and
+//               of the triangle are pairwise disjoint and ascending, the rank of column n of entry j is
+//               3 (j + [j >= pos_d]) + (rank of the vertex inside its own triple) -- no counting; if any
+//               slot of the round fails that test the round falls back to counting (all pairs).
+//   part slot : sorted and tested by k_long_prep; ranks are relative to the part's own run:
+//               3 i + local rank, i = position inside the part.
 __global__ void __launch_bounds__(32 * RSYM_WARPS)
 k_round_symbolic(const int* __restrict__ tris, const int* __restrict__ touched, const int4* __restrict__ rdesc,
-                 const int* __restrict__ n_chunks_dev, const int* __restrict__ tfirst, const uint2* __restrict__ ent,
-                 const int* __restrict__ vcnt, int force_general, int* __restrict__ partner_out,
-                 uint16_t* __restrict__ dvals_out, int* __restrict__ erank, int* __restrict__ drank,
+                 const int* __restrict__ n_chunks_dev, const int* __restrict__ tfirst, const int* __restrict__ sfirst,
+                 const int4* __restrict__ sinfo, const int* __restrict__ tsplit, const uint2* __restrict__ ent,
+                 const int* __restrict__ vcnt, int force_general, int* partner /*in (parts) / out*/,
+                 uint16_t* dvals /*in (parts) / out*/, int* __restrict__ erank, int* __restrict__ drank,
                  int* __restrict__ rowlen, int64_t* __restrict__ tlen, uint8_t* __restrict__ slot_excl,
                  int* __restrict__ everts, int* __restrict__ vslot1) {
   __shared__ int s_cand[RSYM_WARPS][3 * RND_MAX_ENT];  // partner vertex ids of entry i at [3 i + n]
-  __shared__ int s_own[RSYM_WARPS][3 * RND_MAX_TRI];   // own vertex ids of triangle tt at [3 tt + n]
+  __shared__ int s_own[RSYM_WARPS][3 * RND_MAX_TRI];   // own vertex ids of slot tt at [3 tt + n]
   __shared__ int s_first[RSYM_WARPS][RND_MAX_TRI + 1];
   __shared__ int s_dup[RSYM_WARPS][RND_MAX_TRI];
   __shared__ int s_dacc[RSYM_WARPS][3 * RND_MAX_TRI];  // per own column: partner columns below it
-  __shared__ int s_rsum[RSYM_WARPS][RND_MAX_TRI];      // per triangle: sum of the partner columns' ranks
+  __shared__ int s_rsum[RSYM_WARPS][RND_MAX_TRI];      // per slot: sum of the partner columns' ranks
+  __shared__ int s_posd[RSYM_WARPS][RND_MAX_TRI];      // per slot: entries below the diagonal columns (fast path)
   __shared__ unsigned long long s_key[RSYM_WARPS][RND_MAX_ENT];
   __shared__ uint2 s_ent[RSYM_WARPS][RND_MAX_ENT];
   constexpr unsigned FULL = 0xffffffffu;
@@ -643,38 +782,47 @@ k_round_symbolic(const int* __restrict__ tris, const int* __restrict__ touched, 
   int* dupf = s_dup[warp];
   int* dacc = s_dacc[warp];
   int* rsum = s_rsum[warp];
+  int* posd = s_posd[warp];
   unsigned long long* skey = s_key[warp];
   uint2* sent = s_ent[warp];
   const int64_t n_chunks = *n_chunks_dev;
   for (int64_t c = (int64_t)blockIdx.x * RSYM_WARPS + warp; c < n_chunks; c += (int64_t)gridDim.x * RSYM_WARPS) {
     const int4 d = __ldg(rdesc + c);
-    const int e_lo = d.x, nent = d.y, t_lo = d.z, ntri = d.w;
+    const int e_lo = d.x, nent = d.y, s_lo = d.z, nsl = d.w;
     if (nent > RND_MAX_ENT) continue;  // long triangle: k_tri_symbolic
-    // lane = triangle
+    // ---- lane = slot ----
     int f = 0, l = 0, ov[3] = {0, 0, 0};
-    if (lane < ntri) {
-      const int s = __ldg(touched + t_lo + lane);
-      f = __ldg(tfirst + t_lo + lane) - e_lo;
-      l = __ldg(tfirst + t_lo + lane + 1) - e_lo;
+    int4 si = make_int4(0, 0, -1, 0);
+    if (lane < nsl) {
+      si = __ldg(sinfo + s_lo + lane);
+      const int s = __ldg(touched + (si.x & ~SLOT_PART));
+      f = __ldg(sfirst + s_lo + lane) - e_lo;
+      l = __ldg(sfirst + s_lo + lane + 1) - e_lo;
+      load3i(tris + 3 * (int64_t)s, ov);
 #pragma unroll
-      for (int n = 0; n < 3; ++n) {
-        ov[n] = __ldg(tris + 3 * (int64_t)s + n);
-        own[3 * lane + n] = ov[n];
-      }
+      for (int n = 0; n < 3; ++n) own[3 * lane + n] = ov[n];
       first[lane] = f;
       dupf[lane] = 0;
       rsum[lane] = 0;
+      posd[lane] = 0;
       dacc[3 * lane] = dacc[3 * lane + 1] = dacc[3 * lane + 2] = 0;
     }
-    if (lane == 0) first[ntri] = nent;
-    // lane = entry, in the order the counting sort left them
+    const bool slot_is_part = (si.x & SLOT_PART) != 0;
+    if (lane == 0) first[nsl] = nent;
+    const unsigned heads = __reduce_or_sync(FULL, (lane < nsl) ? (1u << f) : 0u);
+    const unsigned partmask = __ballot_sync(FULL, lane < nsl && slot_is_part);  // bit tt: slot tt is a part
+    // ---- lane = entry ----
     const bool valid = lane < nent;
+    const int my_ti = __popc(heads & (0xffffffffu >> (31 - lane))) - 1;
+    const bool in_part = valid && ((partmask >> my_ti) & 1u);
     uint2 me = make_uint2(0u, 0u);
-    if (valid) me = __ldg(ent + e_lo + lane);
+    if (valid) {
+      const int64_t e = (int64_t)e_lo + lane;
+      if (in_part) me = make_uint2((unsigned)partner[e], (unsigned)dvals[e]);  // sorted by k_long_prep
+      else me = __ldg(ent + e);                                                  // as the counting sort left them
+    }
     const unsigned long long key = entry_key(me);
     skey[lane] = key;
-    const unsigned heads = __reduce_or_sync(FULL, (lane < ntri) ? (1u << f) : 0u);
-    const int my_ti = __popc(heads & (0xffffffffu >> (31 - lane))) - 1;
     __syncwarp();
     int myf = 0, deg = 0;
     int mo[3] = {0, 0, 0};  // own vertex ids of the entry's triangle
@@ -684,12 +832,13 @@ k_round_symbolic(const int* __restrict__ tris, const int* __restrict__ touched, 
 #pragma unroll
       for (int n = 0; n < 3; ++n) mo[n] = own[3 * my_ti + n];
     }
-    const int maxdeg = __reduce_max_sync(FULL, deg);
-    // ---- sort the triangle's segment by (partner, side): position = number of keys below (ties by lane) ----
+    const int sortdeg = in_part ? 0 : deg;
+    const int maxdeg = __reduce_max_sync(FULL, sortdeg);
+    // ---- sort every whole slot's segment by (partner, side): position = number of keys below (ties by lane) ----
     {
-      int pos = 0;
+      int pos = in_part ? lane - myf : 0;
       for (int k = 0; k < maxdeg; ++k) {
-        if (k < deg) {
+        if (k < sortdeg) {
           const unsigned long long kx = skey[myf + k];
           pos += (kx < key) || (kx == key && myf + k < lane);
         }
@@ -702,48 +851,88 @@ k_round_symbolic(const int* __restrict__ tris, const int* __restrict__ touched, 
     const unsigned pay = me.y;
     if (valid) {
       const int64_t e = (int64_t)e_lo + lane;
-      partner_out[e] = (int)me.x;
-      dvals_out[e] = (uint16_t)me.y;
+      if (!in_part) {
+        partner[e] = (int)me.x;
+        dvals[e] = (uint16_t)me.y;
+      }
       load3i(tris + 3 * (int64_t)me.x, cv);
 #pragma unroll
       for (int n = 0; n < 3; ++n) cand[3 * lane + n] = cv[n];
     }
+    // ---- fast path test: disjoint ascending vertex-id intervals ----
+    const int mn = min3i(cv[0], cv[1], cv[2]), mx = max3i(cv[0], cv[1], cv[2]);
+    const int mn_s = min3i(mo[0], mo[1], mo[2]), mx_s = max3i(mo[0], mo[1], mo[2]);
+    const int mn_next = __shfl_down_sync(FULL, mn, 1);
+    const bool last_of_slot = valid && (lane == myf + deg - 1);
+    bool ordered = true;
+    if (valid && !in_part) ordered = (last_of_slot || mx < mn_next) && ((mx < mn_s) || (mx_s < mn));
+    const bool fast = __all_sync(FULL, ordered);
+    const bool below = valid && (mx < mn_s);
+    const unsigned below_mask = __ballot_sync(FULL, below);
     __syncwarp();
-    // Rank of a column = number of smaller columns among the triangle's L = 3 (deg + 1) candidates.
-    // Duplicates: the ranks of L distinct values sum to L (L - 1) / 2 and every tied pair lowers the sum
-    // by one, so one integer per triangle (shared-memory atomics: the RESULT is order independent)
-    // replaces all equality counting.  The diagonal columns are ranked by the entries' lanes too:
-    // each adds how many of its three columns lie below each own column.
+    const int lr0 = (cv[1] < cv[0]) + (cv[2] < cv[0]), lr1 = (cv[0] < cv[1]) + (cv[2] < cv[1]), lr2 = (cv[0] < cv[2]) + (cv[1] < cv[2]);
     int r[3] = {0, 0, 0};
-    for (int k = 0; k < maxdeg; ++k) {
-      if (k < deg) {
-        const int* o = cand + 3 * (myf + k);
-        const int o0 = o[0], o1 = o[1], o2 = o[2];
-#pragma unroll
-        for (int n = 0; n < 3; ++n) r[n] += (o0 < cv[n]) + (o1 < cv[n]) + (o2 < cv[n]);
-      }
-    }
-    if (valid) {
-#pragma unroll
-      for (int n = 0; n < 3; ++n) {
-        r[n] += (mo[0] < cv[n]) + (mo[1] < cv[n]) + (mo[2] < cv[n]);
-        atomicAdd(&dacc[3 * my_ti + n], (cv[0] < mo[n]) + (cv[1] < mo[n]) + (cv[2] < mo[n]));
-      }
-      atomicAdd(&rsum[my_ti], r[0] + r[1] + r[2]);
-    }
-    __syncwarp();
     int dr[3] = {0, 0, 0};
-    if (lane < ntri) {
-      int tot = rsum[lane];
-#pragma unroll
-      for (int n = 0; n < 3; ++n) {
-        dr[n] = dacc[3 * lane + n] + (ov[0] < ov[n]) + (ov[1] < ov[n]) + (ov[2] < ov[n]);
-        tot += dr[n];
+    if (fast) {
+      if (valid) {
+        const unsigned seg = (deg >= 32) ? 0xffffffffu : (((1u << deg) - 1u) << myf);
+        const int pd = __popc(below_mask & seg);       // entries of my slot below the diagonal columns
+        const int j = lane - myf;
+        const int unit = in_part ? j : j + (j >= pd ? 1 : 0);
+        r[0] = 3 * unit + lr0;
+        r[1] = 3 * unit + lr1;
+        r[2] = 3 * unit + lr2;
+        if (j == 0) posd[my_ti] = pd;
       }
-      const int L = 3 * (l - f + 1);
-      dupf[lane] = (2 * tot != L * (L - 1)) ? 1 : 0;
+      __syncwarp();
+      if (lane < nsl) {
+        const int pd = (l > f) ? posd[lane] : 0;
+#pragma unroll
+        for (int n = 0; n < 3; ++n) dr[n] = 3 * pd + (ov[0] < ov[n]) + (ov[1] < ov[n]) + (ov[2] < ov[n]);
+      }
+    } else {
+      // Rank of a column = number of smaller columns among the triangle's L = 3 (deg + 1) candidates.
+      // Duplicates: the ranks of L distinct values sum to L (L - 1) / 2 and every tied pair lowers the sum
+      // by one, so one integer per triangle (shared-memory atomics: the RESULT is order independent)
+      // replaces all equality counting.  The diagonal columns are ranked by the entries' lanes too:
+      // each adds how many of its three columns lie below each own column.  (Part slots keep their own.)
+      const int cdeg = in_part ? 0 : deg;
+      const int cmax = __reduce_max_sync(FULL, cdeg);
+      for (int k = 0; k < cmax; ++k) {
+        if (k < cdeg) {
+          const int* o = cand + 3 * (myf + k);
+          const int o0 = o[0], o1 = o[1], o2 = o[2];
+#pragma unroll
+          for (int n = 0; n < 3; ++n) r[n] += (o0 < cv[n]) + (o1 < cv[n]) + (o2 < cv[n]);
+        }
+      }
+      if (valid && !in_part) {
+#pragma unroll
+        for (int n = 0; n < 3; ++n) {
+          r[n] += (mo[0] < cv[n]) + (mo[1] < cv[n]) + (mo[2] < cv[n]);
+          atomicAdd(&dacc[3 * my_ti + n], (cv[0] < mo[n]) + (cv[1] < mo[n]) + (cv[2] < mo[n]));
+        }
+        atomicAdd(&rsum[my_ti], r[0] + r[1] + r[2]);
+      }
+      if (in_part) {
+        const int j = lane - myf;
+        r[0] = 3 * j + lr0;
+        r[1] = 3 * j + lr1;
+        r[2] = 3 * j + lr2;
+      }
+      __syncwarp();
+      if (lane < nsl && !slot_is_part) {
+        int tot = rsum[lane];
+#pragma unroll
+        for (int n = 0; n < 3; ++n) {
+          dr[n] = dacc[3 * lane + n] + (ov[0] < ov[n]) + (ov[1] < ov[n]) + (ov[2] < ov[n]);
+          tot += dr[n];
+        }
+        const int L = 3 * (l - f + 1);
+        dupf[lane] = (2 * tot != L * (L - 1)) ? 1 : 0;
+      }
+      __syncwarp();
     }
-    __syncwarp();
     if (valid) {
       const int64_t e = (int64_t)e_lo + lane;
       const bool nodup = dupf[my_ti] == 0;
@@ -761,20 +950,39 @@ k_round_symbolic(const int* __restrict__ tris, const int* __restrict__ touched, 
       o[1] = make_int2(pick3(3 - ka - pa, a0, a1, a2), pick3(kb, b0, b1, b2));
       o[2] = make_int2(pick3(pb, b0, b1, b2), pick3(3 - kb - pb, b0, b1, b2));
     }
-    if (lane < ntri) {
-      const int64_t ti = (int64_t)t_lo + lane;
-      const bool nodup = dupf[lane] == 0;
-      const int dg = l - f, L = 3 * (dg + 1);
+    if (lane < nsl) {
+      const int64_t sl = (int64_t)s_lo + lane;
+      if (!slot_is_part) {
+        const bool nodup = dupf[lane] == 0;
+        const int dg = l - f, L = 3 * (dg + 1);
 #pragma unroll
-      for (int n = 0; n < 3; ++n) drank[3 * ti + n] = nodup ? dr[n] : 3 * dg + n;
+        for (int n = 0; n < 3; ++n) drank[3 * sl + n] = nodup ? dr[n] : 3 * dg + n;
 #pragma unroll
-      for (int m = 0; m < 3; ++m) {
-        const bool single = __ldg(vcnt + ov[m]) == 1;
-        const bool excl = nodup && !force_general && single;
-        if (single) vslot1[ov[m]] = (int)(3 * ti + m);  // the vertex's only slot (k_gather3)
-        slot_excl[3 * ti + m] = excl ? 1 : 0;
-        tlen[3 * ti + m] = excl ? 0 : L;
-        if (excl) rowlen[ov[m]] = L;
+        for (int m = 0; m < 3; ++m) {
+          const bool single = __ldg(vcnt + ov[m]) == 1;
+          const bool excl = nodup && !force_general && single;
+          if (single) vslot1[ov[m]] = (int)(3 * sl + m);  // the vertex's only slot (k_gather3)
+          slot_excl[3 * sl + m] = excl ? 1 : 0;
+          tlen[3 * sl + m] = excl ? 0 : L;
+          if (excl) rowlen[ov[m]] = L;
+        }
+      } else {  // part of a split triangle: exclusive rows by construction; the triangle's first part owns its rows
+        const int ti = si.x & ~SLOT_PART;
+        const int pd = __ldg(tsplit + ti);
+        const bool first_part = (si.y == 0) || (si.y == 1 && pd == 0);
+        drank[3 * sl] = -1 - si.z;   // part ordinal (diagonal partial sums: k_split_finish)
+        drank[3 * sl + 1] = 0;
+        drank[3 * sl + 2] = 0;
+        const int L = 3 * (__ldg(tfirst + ti + 1) - __ldg(tfirst + ti) + 1);
+#pragma unroll
+        for (int m = 0; m < 3; ++m) {
+          slot_excl[3 * sl + m] = 1;
+          tlen[3 * sl + m] = 0;
+          if (first_part) {
+            vslot1[ov[m]] = (int)(3 * sl + m);
+            rowlen[ov[m]] = L;
+          }
+        }
       }
     }
     __syncwarp();  // shared memory is reused by the next round
@@ -782,32 +990,35 @@ k_round_symbolic(const int* __restrict__ tris, const int* __restrict__ touched, 
 }
 
 // Column indices of the exclusive rows + row bases of every non-long round (after the rowptr scan).
-// The three rows of a triangle have the SAME column run: it is built once in shared memory (ranks
-// are positions in the run) and written out three times with consecutive lanes on consecutive
-// addresses, instead of nine scattered 4-byte stores per entry.
+// The three rows of a slot have the SAME column run: it is built once in shared memory (ranks are
+// positions in the run) and written out three times with consecutive lanes on consecutive addresses,
+// instead of nine scattered 4-byte stores per entry.  A whole slot's run has deg + 1 units of 3 columns
+// (the last unit in the staging area is the diagonal's); a part's run has one unit per entry and starts
+// 3 u0 blocks into the triangle's rows; the first part of a split triangle also writes the diagonal columns.
 __global__ void __launch_bounds__(32 * RSYM_WARPS)
 k_round_fill(const int* __restrict__ tris, const int* __restrict__ touched, const int4* __restrict__ rdesc,
-             int64_t n_chunks, const int* __restrict__ tfirst, const int* __restrict__ partner,
+             int64_t n_chunks, const int* __restrict__ sfirst, const int4* __restrict__ sinfo,
+             const int* __restrict__ tsplit, const int* __restrict__ partner,
              const int* __restrict__ erank, const int* __restrict__ drank, const int64_t* __restrict__ toff,
              const uint8_t* __restrict__ slot_excl, const int* __restrict__ rowptr,
              int64_t* __restrict__ rowbase, int* __restrict__ colind) {
-  constexpr int UNITS = RND_MAX_ENT + RND_MAX_TRI;       // a triangle's run has deg + 1 units of 3 columns
-  __shared__ int s_rp[RSYM_WARPS][3 * RND_MAX_TRI];       // first block of row m of triangle tt, or -1
-  __shared__ int s_ci[RSYM_WARPS][3 * UNITS];             // column runs of the round's triangles, back to back
-  __shared__ int s_first[RSYM_WARPS][RND_MAX_TRI];        // first entry of triangle tt
-  __shared__ unsigned char s_utt[RSYM_WARPS][UNITS];      // unit -> triangle
+  constexpr int UNITS = RND_MAX_ENT + RND_MAX_TRI;
+  __shared__ int s_rp[RSYM_WARPS][3 * RND_MAX_TRI];       // first block of the run of row m of slot tt, or -1
+  __shared__ int s_ci[RSYM_WARPS][3 * UNITS];             // column runs of the round's slots, back to back
+  __shared__ int s_ub[RSYM_WARPS][RND_MAX_TRI];           // first unit of slot tt in s_ci
+  __shared__ unsigned char s_utt[RSYM_WARPS][UNITS];      // unit -> slot
   constexpr unsigned FULL = 0xffffffffu;
   const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
   const int64_t c = (int64_t)blockIdx.x * RSYM_WARPS + warp;
   if (c >= n_chunks) return;
   const int4 d = __ldg(rdesc + c);
-  const int e_lo = d.x, nent = d.y, t_lo = d.z, ntri = d.w;
+  const int e_lo = d.x, nent = d.y, s_lo = d.z, nsl = d.w;
   if (nent > RND_MAX_ENT) return;  // long triangle: k_fill_rows
   int* rps = s_rp[warp];
   int* ci = s_ci[warp];
-  int* first = s_first[warp];
+  int* ubase = s_ub[warp];
   unsigned char* utt = s_utt[warp];
-  // entry lanes: partner columns and ranks (independent of the triangle lanes' loads)
+  // entry lanes: partner columns and ranks (independent of the slot lanes' loads)
   int cv[3] = {0, 0, 0}, er[3] = {0, 0, 0};
   if (lane < nent) {
     const int64_t e = (int64_t)e_lo + lane;
@@ -815,38 +1026,68 @@ k_round_fill(const int* __restrict__ tris, const int* __restrict__ touched, cons
     load3i(tris + 3 * (int64_t)t, cv);
     load3i(erank + 3 * e, er);
   }
-  int f = 0;
-  if (lane < ntri) {
-    const int64_t ti = (int64_t)t_lo + lane;
+  // slot lanes
+  int f = 0, l = 0;
+  int4 si = make_int4(0, 0, -1, 0);
+  if (lane < nsl) {
+    si = __ldg(sinfo + s_lo + lane);
+    f = __ldg(sfirst + s_lo + lane) - e_lo;
+    l = __ldg(sfirst + s_lo + lane + 1) - e_lo;
+  }
+  const bool is_part = (si.x & SLOT_PART) != 0;
+  const unsigned wholemask = __ballot_sync(FULL, lane < nsl && !is_part);
+  const int ub = f + __popc(wholemask & ((1u << lane) - 1u));   // every whole slot before adds one (diagonal) unit
+  const unsigned heads = __reduce_or_sync(FULL, (lane < nsl) ? (1u << f) : 0u);
+  const int my_ti = __popc(heads & (0xffffffffu >> (31 - lane))) - 1;
+  if (lane < nsl) {
+    const int64_t sl = (int64_t)s_lo + lane;
+    const int ti = si.x & ~SLOT_PART;
     const int s = __ldg(touched + ti);
-    f = __ldg(tfirst + ti) - e_lo;
-    const int l = __ldg(tfirst + ti + 1) - e_lo;
-    first[lane] = f;
-    utt[l + lane] = (unsigned char)lane;  // the diagonal's unit closes the run
+    int ov[3];
+    load3i(tris + 3 * (int64_t)s, ov);
+    ubase[lane] = ub;
+    if (!is_part) {
+      utt[ub + (l - f)] = (unsigned char)lane;  // the diagonal's unit closes the run
 #pragma unroll
-    for (int n = 0; n < 3; ++n) ci[3 * (f + lane) + __ldg(drank + 3 * ti + n)] = __ldg(tris + 3 * (int64_t)s + n);
+      for (int n = 0; n < 3; ++n) ci[3 * ub + __ldg(drank + 3 * sl + n)] = ov[n];
 #pragma unroll
-    for (int m = 0; m < 3; ++m) {
-      const bool excl = slot_excl[3 * ti + m] != 0;
-      const int rp = excl ? __ldg(rowptr + __ldg(tris + 3 * (int64_t)s + m)) : -1;
-      rps[3 * lane + m] = rp;
-      rowbase[3 * ti + m] = excl ? (int64_t)rp : -(toff[3 * ti + m] + 1);
+      for (int m = 0; m < 3; ++m) {
+        const bool excl = slot_excl[3 * sl + m] != 0;
+        const int rp = excl ? __ldg(rowptr + ov[m]) : -1;
+        rps[3 * lane + m] = rp;
+        rowbase[3 * sl + m] = excl ? (int64_t)rp : -(toff[3 * sl + m] + 1);
+      }
+    } else {
+      const int pd = __ldg(tsplit + ti);
+      const bool first_part = (si.y == 0) || (si.y == 1 && pd == 0);
+#pragma unroll
+      for (int m = 0; m < 3; ++m) {
+        const int row0 = __ldg(rowptr + ov[m]);
+        const int rp = row0 + 3 * si.y;
+        rps[3 * lane + m] = rp;
+        rowbase[3 * sl + m] = (int64_t)rp;
+        if (first_part) {
+#pragma unroll
+          for (int n = 0; n < 3; ++n) colind[row0 + 3 * pd + (ov[0] < ov[n]) + (ov[1] < ov[n]) + (ov[2] < ov[n])] = ov[n];
+        }
+      }
     }
   }
-  const unsigned heads = __reduce_or_sync(FULL, (lane < ntri) ? (1u << f) : 0u);
-  const int my_ti = __popc(heads & (0xffffffffu >> (31 - lane))) - 1;
   __syncwarp();
+  // first entry of my slot, by shuffle from the slot lane
+  const int myf = __shfl_sync(FULL, f, my_ti < 0 ? 0 : my_ti);
   if (lane < nent) {
-    utt[lane + my_ti] = (unsigned char)my_ti;
-    const int base = 3 * (first[my_ti] + my_ti);
+    const int u = ubase[my_ti];
+    utt[u + (lane - myf)] = (unsigned char)my_ti;
+    const int base = 3 * u;
 #pragma unroll
     for (int n = 0; n < 3; ++n) ci[base + er[n]] = cv[n];
   }
   __syncwarp();
-  const int total = 3 * (nent + ntri);
+  const int total = 3 * (nent + __popc(wholemask));
   for (int idx = lane; idx < total; idx += 32) {
     const int tt = utt[idx / 3];
-    const int off = idx - 3 * (first[tt] + tt);
+    const int off = idx - 3 * ubase[tt];
     const int v = ci[idx];
 #pragma unroll
     for (int m = 0; m < 3; ++m) {
@@ -1105,7 +1346,8 @@ k_assemble_tile(const AsmParams<T> P) {
 
     if (!is_long) {
       // lane = triangle: tile slots (16-byte slots, prefix sum over the round's triangles)
-      const int run_bytes = RUN_UNIT * (cur.e1 - cur.e0 + 1);
+      const bool part_slot = cur.dr[0] < 0;  // a part of a split triangle: no diagonal blocks in its runs
+      const int run_bytes = RUN_UNIT * (cur.e1 - cur.e0 + (part_slot ? 0 : 1));
       int slot_off;
       {
         int incl = (lane < ntri) ? (((run_bytes + 15) & ~15) + 16) : 0;
@@ -1186,6 +1428,16 @@ k_assemble_tile(const AsmParams<T> P) {
         __syncwarp();
       }
 
+      {  // parts hand their diagonal partial sums to k_split_finish
+        const int pidx = (lane < ntri && part_slot) ? (-1 - cur.dr[0]) : -1;
+        if (__ballot_sync(FULL, pidx >= 0)) {
+          for (int tt = 0; tt < ntri; ++tt) {
+            const int px = __shfl_sync(FULL, pidx, tt);
+            if (px >= 0)
+              for (int k = lane; k < NDIAG; k += 32) P.dpart[(int64_t)NDIAG * px + k] = S.dsum[tt][k];
+          }
+        }
+      }
 #pragma unroll
       for (int m = 0; m < 3; ++m) {
         const unsigned long long g =
@@ -1199,7 +1451,7 @@ k_assemble_tile(const AsmParams<T> P) {
         if (lane < ntri) {
           S.run_off[lane] = my_off;
 #pragma unroll
-          for (int n = 0; n < 3; ++n) S.diag_off[lane][n] = my_off + 9 * (int)sizeof(T) * cur.dr[n];
+          for (int n = 0; n < 3; ++n) S.diag_off[lane][n] = part_slot ? -1 : my_off + 9 * (int)sizeof(T) * cur.dr[n];
         }
         __syncwarp();
         if (valid) {
@@ -1248,7 +1500,7 @@ k_assemble_tile(const AsmParams<T> P) {
           }
 #pragma unroll
           for (int tt = 0; tt < RND_MAX_TRI; ++tt)
-            if (tt < ntri) *reinterpret_cast<T*>(S.tile + off[tt] + cq * (int)sizeof(T)) = val[tt];
+            if (tt < ntri && off[tt] >= 0) *reinterpret_cast<T*>(S.tile + off[tt] + cq * (int)sizeof(T)) = val[tt];
         }
         // positions of the next round (L2 hits): requested as soon as this round's J is dead
         if (m == 2 && lane < round_entries(d_nxt)) load_pos18(P.pos, ids_nxt, x);
@@ -1880,6 +2132,49 @@ k_entry_pipe(const AsmParams<T> P) {
     buf ^= 1;
   }
   cp_async_wait<0>();
+}
+
+// Split triangles (one warp each), after K4 / K6: adds the parts' gradient (or H.p) partials into the
+// triangle's first slot -- the one k_gather3 reads -- and, with HESS, sums the parts' diagonal partial sums
+// (fixed order) and writes the triangle's nine diagonal blocks (rows exclusive by construction).
+template <typename T, bool HESS>
+__global__ void __launch_bounds__(128)
+k_split_finish(const int4* __restrict__ split_list, int64_t n_split, const int* __restrict__ tris,
+               const int* __restrict__ touched, const int* __restrict__ tsplit, const int* __restrict__ rowptr,
+               const double* __restrict__ dpart, T* tslot, T* __restrict__ vals) {
+  __shared__ double s_d[4][NDIAG];
+  const int w = threadIdx.x >> 5, lane = threadIdx.x & 31;
+  const int64_t i = (int64_t)blockIdx.x * 4 + w;
+  if (i >= n_split) return;
+  const int4 sp = __ldg(split_list + i);  // first slot, parts, touched index, first part ordinal
+  if (lane < 9) {
+    double a = 0.0;
+    for (int k = 0; k < sp.y; ++k) a += (double)tslot[9 * ((int64_t)sp.x + k) + lane];
+    tslot[9 * (int64_t)sp.x + lane] = (T)a;
+  }
+  if (HESS) {
+    for (int k = lane; k < NDIAG; k += 32) {
+      double a = 0.0;
+      for (int q = 0; q < sp.y; ++q) a += __ldg(dpart + (int64_t)NDIAG * (sp.w + q) + k);
+      s_d[w][k] = a;
+    }
+    __syncwarp();
+    int ov[3];
+    load3i(tris + 3 * (int64_t)__ldg(touched + sp.z), ov);
+    const int pd = __ldg(tsplit + sp.z);
+    if (lane < 27) {
+      const int n = lane / 9, q = lane % 9;
+      const int on = pick3(n, ov[0], ov[1], ov[2]);
+      const int lr = (ov[0] < on) + (ov[1] < on) + (ov[2] < on);
+#pragma unroll
+      for (int m = 0; m < 3; ++m) {
+        const int r_ = 3 * m + q / 3, c_ = 3 * n + q % 3;
+        const int lo = min(r_, c_), hi = max(r_, c_);
+        const int uidx = lo * 9 - (lo * (lo - 1)) / 2 + (hi - lo);
+        vals[9 * ((int64_t)__ldg(rowptr + ov[m]) + 3 * pd + lr) + q] = (T)s_d[w][uidx];
+      }
+    }
+  }
 }
 
 // ------------------------------------------------------------------------------------------ K5

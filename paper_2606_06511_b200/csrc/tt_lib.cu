@@ -64,7 +64,7 @@ struct tt_ctx {
   std::string err;
   int64_t launches = 0;
   // classification
-  DevBuf mask, blk_count, blk_off, blk_energy, counts, energy, cfg, sum_stage;
+  DevBuf mask, blk_count, blk_off, blk_energy, counts, energy, rec, sum_stage;
   // active set + directed entries
   DevBuf active_ids, ent_in, partner, dvals, tptr, zero_blk, touched;
   // per-triangle symbolic
@@ -76,7 +76,7 @@ struct tt_ctx {
   // pattern
   DevBuf rowptr64, rowptr, colind;
   // numeric
-  DevBuf everts, rdesc, tfirst, bucket_cnt, bucket_off, long_cnt, long_off, long_list, asm_energy, tvals, tslot, vkeys[2], vvals[2], vptr, vslot1;
+  DevBuf everts, rdesc, tfirst, sfirst, sinfo, tsplit, split_list, dpart, bucket_cnt, bucket_off, long_list, asm_energy, tvals, tslot, vkeys[2], vvals[2], vptr, vslot1;
   DevBuf cub_tmp;
   DevBuf pcg_r, pcg_p, pcg_q, pcg_part[2], pcg_sc, pcg_hist;  // tt_pcg_solve workspace
   DevBuf possig;  // [2] u64: checksum of pos at tt_hess_symbolic, and at the last numeric / H.p call
@@ -88,9 +88,8 @@ struct tt_ctx {
   // cached symbolic state
   Signature sig;
   int64_t A = 0, n_dir = 0, n_touched = 0, R = 0, U = 0, nnzb = 0, n_chunks = 0, n_long = 0, rows_excl = 0, rows_gen = 0;
+  int64_t n_slots = 0, n_split = 0, n_parts = 0;
   int bitsT = 1, bitsV = 1, sms = 148;
-  // L2 persisting window over `pos` for the gather-bound kernels (K1, K4, K6); 0 = off
-  size_t l2_persist_bytes = 0, l2_max_window = 0;
   int tile_grid[2] = {0, 0};  // persistent grid of k_assemble_tile<double / float>
   int pipe_grid[2][2] = {{0, 0}, {0, 0}};  // persistent grid of k_entry_pipe<double / float, MODE 1 / 2>
   uint64_t* rkeys_sorted = nullptr;
@@ -134,24 +133,6 @@ tt_status fail(tt_ctx* c, tt_status s, const char* fmt, ...) {
     ctx->launches++;                                                                             \
     TT_CUDA(cudaGetLastError());                                                                 \
   } while (0)
-
-// Marks `pos` as L2-persisting for the kernels enqueued on `st` until l2_window_off: the random
-// vertex gathers of K1 / K4 / K6 are the kernels' DRAM traffic, and a soup's positions (144 MB in fp64)
-// just miss the 126 MB L2, so plain LRU keeps ~40 % of them resident; a persisting window with
-// hitRatio = set-aside / window pins a fixed fraction instead of letting the streams evict it.
-inline void l2_window(tt_ctx* ctx, cudaStream_t st, const void* base, size_t bytes) {
-  if (!ctx->l2_persist_bytes) return;
-  cudaStreamAttrValue a;
-  memset(&a, 0, sizeof(a));
-  const size_t win = bytes < ctx->l2_max_window ? bytes : ctx->l2_max_window;
-  a.accessPolicyWindow.base_ptr = const_cast<void*>(base);
-  a.accessPolicyWindow.num_bytes = base ? win : 0;
-  a.accessPolicyWindow.hitRatio = (base && win) ? (float)((double)ctx->l2_persist_bytes / (double)win < 1.0 ? (double)ctx->l2_persist_bytes / (double)win : 1.0) : 0.0f;
-  a.accessPolicyWindow.hitProp = cudaAccessPropertyPersisting;
-  a.accessPolicyWindow.missProp = cudaAccessPropertyStreaming;
-  if (cudaStreamSetAttribute(st, cudaStreamAttributeAccessPolicyWindow, &a) != cudaSuccess) (void)cudaGetLastError();
-}
-inline void l2_window_off(tt_ctx* ctx, cudaStream_t st) { l2_window(ctx, st, nullptr, 0); }
 
 inline int ceil_log2(int64_t n) {
   int b = 1;
@@ -287,18 +268,16 @@ tt_status run_classify(tt_ctx* ctx, const tt_problem* q, T* e_pp, T* tc, bool re
   TT_CUDA(ctx->blk_energy.ensure(sizeof(double) * (size_t)(nblk + 1)));
   TT_CUDA(ctx->counts.ensure(sizeof(int64_t) * 16));
   TT_CUDA(ctx->energy.ensure(sizeof(double) * 2));
-  if (record) TT_CUDA(ctx->cfg.ensure(sizeof(uint16_t) * (size_t)(P + 1)));
+  if (record) TT_CUDA(ctx->rec.ensure(sizeof(uint64_t) * (size_t)(P + 1)));
   TT_CUDA(cudaMemsetAsync(ctx->blk_count.as<int>() + nblk, 0, sizeof(int), st));
   if (nblk > 0) {
     cudaEvent_t* ev_k1 = ctx->evr[0][ctx->ev_n[0] % tt_ctx::EV_RING];
-    l2_window(ctx, st, q->pos, sizeof(T) * 3 * (size_t)q->n_verts);
     TT_CUDA(cudaEventRecord(ev_k1[0], st));
     ttk::k_classify<T><<<(unsigned)nblk, ttk::CLS_THREADS, 0, st>>>(
         (const T*)q->pos, q->tris, (const int2*)q->pairs, P, ctx->opt.tc_scale, ctx->mask.as<uint32_t>(),
-        ctx->blk_count.as<int>(), ctx->blk_energy.as<double>(), e_pp, tc, record ? ctx->cfg.as<uint16_t>() : nullptr, deg);
+        ctx->blk_count.as<int>(), ctx->blk_energy.as<double>(), e_pp, tc, record ? ctx->rec.as<uint64_t>() : nullptr, deg);
     TT_LAUNCH_CHECK();
     TT_CUDA(cudaEventRecord(ev_k1[1], st));
-    l2_window_off(ctx, st);
     ctx->ev_n[0]++;
   }
   tt_status s = scan_i32(ctx, ctx->blk_count.as<int>(), ctx->blk_off.as<int>(), nblk + 1, st);
@@ -346,8 +325,8 @@ tt_status energy_impl(tt_ctx* ctx, const tt_problem* q, void* energy_sum, void* 
 // 0 beyond 3 * n_touched (still on the device): the scan of the general-row lengths runs over the host-known bound
 struct MaskedLen {
   const int64_t* tlen;
-  const int* n_touched;
-  __host__ __device__ int64_t operator()(int64_t i) const { return i < 3 * (int64_t)(*n_touched) ? tlen[i] : 0; }
+  const int* n_slots;
+  __host__ __device__ int64_t operator()(int64_t i) const { return i < 3 * (int64_t)(*n_slots) ? tlen[i] : 0; }
 };
 struct DegFlag {
   const int* deg;
@@ -368,21 +347,23 @@ tt_status symbolic_impl(tt_ctx* ctx, const tt_problem* q, int64_t* nnzb_host, in
   ctx->bitsV = ceil_log2(nV > 1 ? nV : 2);
   const int bitsV = ctx->bitsV;
   // Everything up to the pattern sizes is enqueued WITHOUT a host round trip: buffers and grids use the
-  // bounds  directed entries <= 2 P,  touched triangles <= min(nT, 2 P),  and the kernels read the true
-  // counts from device memory.  One synchronisation (below) then brings all counts to the host.
+  // bounds  directed entries <= 2 P,  touched triangles <= min(nT, 2 P),  slots <= touched + entries / 8
+  // (a part ends where its segment ends -- twice per split triangle, which has > 32 entries -- or where a
+  // round is full -- once per 32 entries),  and the kernels read the true counts from device memory.
+  // One synchronisation (below) then brings all counts to the host.
   const int64_t n_ub = 2 * P;
   const int64_t touched_ub = nT < n_ub ? nT : n_ub;
-  // ---- one zeroed block: deg [nT+1], fill [nT+1], vcnt [nV+1], rowlen [nV+1] ----
-  const size_t zints = 2 * (size_t)(nT + 1) + 2 * (size_t)(nV + 1);
+  const int64_t slots_ub = touched_ub + n_ub / 8 + 8;
+  // ---- one zeroed block: deg [nT+1], vcnt [nV+1], rowlen [nV+1] ----
+  const size_t zints = (size_t)(nT + 1) + 2 * (size_t)(nV + 1);
   TT_CUDA(ctx->zero_blk.ensure(sizeof(int) * zints));
   TT_CUDA(cudaMemsetAsync(ctx->zero_blk.p, 0, sizeof(int) * zints, st));
   int* deg = ctx->zero_blk.as<int>();
-  int* fill = deg + (nT + 1);
-  int* vcnt = fill + (nT + 1);
+  int* vcnt = deg + (nT + 1);
   int* rowlen = vcnt + (nV + 1);
   ctx->vcnt_p = vcnt;
   ctx->rowlen_p = rowlen;
-  // ---- K1: classification, recorded decisions, degree histogram ----
+  // ---- K1: classification, recorded decisions, degree histogram + place of every entry in its segment ----
   s = run_classify<T>(ctx, q, nullptr, nullptr, true, deg, st, &nblk);
   if (s != TT_OK) return s;
   int64_t* d_counts = ctx->counts.as<int64_t>();
@@ -391,44 +372,44 @@ tt_status symbolic_impl(tt_ctx* ctx, const tt_problem* q, int64_t* nnzb_host, in
   TT_CUDA(ctx->tptr.ensure(sizeof(int) * (size_t)(nT + 2)));
   s = scan_i32(ctx, deg, ctx->tptr.as<int>(), nT + 1, st);  // tptr[nT] = directed entries = 2 A
   if (s != TT_OK) return s;
-  // ---- K2: compaction + counting sort of the directed entries by source triangle ----
+  // ---- K2: compaction + counting-sort scatter of the directed entries by source triangle ----
   TT_CUDA(ctx->active_ids.ensure(sizeof(int) * (size_t)(P + 1)));
   TT_CUDA(ctx->ent_in.ensure(sizeof(uint2) * (size_t)(n_ub + 1)));
   TT_CUDA(ctx->partner.ensure(sizeof(int) * (size_t)(n_ub + 1)));
   TT_CUDA(ctx->dvals.ensure(sizeof(uint16_t) * (size_t)(n_ub + 2)));
   if (nblk > 0) {
     k_compact<<<(unsigned)nblk, CLS_THREADS, 0, st>>>(ctx->mask.as<uint32_t>(), ctx->blk_off.as<int>(), P, ctx->active_ids.as<int>(),
-                                                      (const int2*)q->pairs, ctx->cfg.as<uint16_t>(), ctx->tptr.as<int>(), fill,
+                                                      (const int2*)q->pairs, ctx->rec.as<uint64_t>(), ctx->tptr.as<int>(),
                                                       ctx->ent_in.as<uint2>());
     TT_LAUNCH_CHECK();
   }
-  // ---- touched triangles, vertex use counts, the work partition (rounds) shared by the symbolic round
-  //      kernels, K4 and K6 ----
+  // ---- touched triangles, vertex use counts, the work partition (slots, rounds) shared by the symbolic
+  //      round kernels, K4 and K6 ----
   TT_CUDA(ctx->touched.ensure(sizeof(int) * (size_t)(nT + 1)));
   TT_CUDA(ctx->tfirst.ensure(sizeof(int) * (size_t)(touched_ub + 2)));
-  TT_CUDA(ctx->rdesc.ensure(sizeof(int4) * (size_t)(touched_ub + 1)));
+  TT_CUDA(ctx->tsplit.ensure(sizeof(int) * (size_t)(touched_ub + 1)));
+  TT_CUDA(ctx->sfirst.ensure(sizeof(int) * (size_t)(slots_ub + 2)));
+  TT_CUDA(ctx->sinfo.ensure(sizeof(int4) * (size_t)(slots_ub + 1)));
+  TT_CUDA(ctx->rdesc.ensure(sizeof(int4) * (size_t)(slots_ub + 1)));
   TT_CUDA(ctx->long_list.ensure(sizeof(int) * (size_t)(n_ub / (RND_MAX_ENT + 1) + 2)));
+  TT_CUDA(ctx->split_list.ensure(sizeof(int4) * (size_t)(n_ub / (RND_MAX_ENT + 1) + 2)));
   const int64_t buckets_ub = (touched_ub + CHK_BUCKET - 1) / CHK_BUCKET;
-  TT_CUDA(ctx->bucket_cnt.ensure(sizeof(int) * (size_t)(buckets_ub + 1)));
-  TT_CUDA(ctx->bucket_off.ensure(sizeof(int) * (size_t)(buckets_ub + 1)));
-  TT_CUDA(ctx->long_cnt.ensure(sizeof(int) * (size_t)(buckets_ub + 1)));
-  TT_CUDA(ctx->long_off.ensure(sizeof(int) * (size_t)(buckets_ub + 1)));
+  TT_CUDA(ctx->bucket_cnt.ensure(sizeof(PackCount) * (size_t)(buckets_ub + 1)));
+  TT_CUDA(ctx->bucket_off.ensure(sizeof(PackCount) * (size_t)(buckets_ub + 1)));
   TT_CUDA(ctx->erank.ensure(sizeof(int) * (size_t)(3 * n_ub + 3)));
   TT_CUDA(ctx->everts.ensure(sizeof(int) * 6 * (size_t)(n_ub + 1)));
-  TT_CUDA(ctx->drank.ensure(sizeof(int) * (size_t)(3 * touched_ub + 3)));
-  TT_CUDA(ctx->tlen.ensure(sizeof(int64_t) * (size_t)(3 * touched_ub + 1)));
-  TT_CUDA(ctx->toff.ensure(sizeof(int64_t) * (size_t)(3 * touched_ub + 2)));
-  TT_CUDA(ctx->slot_excl.ensure((size_t)(3 * touched_ub + 1)));
-  TT_CUDA(ctx->rowbase.ensure(sizeof(int64_t) * (size_t)(3 * touched_ub + 1)));
+  TT_CUDA(ctx->drank.ensure(sizeof(int) * (size_t)(3 * slots_ub + 3)));
+  TT_CUDA(ctx->tlen.ensure(sizeof(int64_t) * (size_t)(3 * slots_ub + 1)));
+  TT_CUDA(ctx->toff.ensure(sizeof(int64_t) * (size_t)(3 * slots_ub + 2)));
+  TT_CUDA(ctx->slot_excl.ensure((size_t)(3 * slots_ub + 1)));
+  TT_CUDA(ctx->rowbase.ensure(sizeof(int64_t) * (size_t)(3 * slots_ub + 1)));
   TT_CUDA(ctx->vslot1.ensure(sizeof(int) * (size_t)(nV + 1)));
   TT_CUDA(ctx->rowptr64.ensure(sizeof(int64_t) * (size_t)(nV + 1)));
   TT_CUDA(ctx->rowptr.ensure(sizeof(int) * (size_t)(nV + 1)));
-  int* d_num = reinterpret_cast<int*>(d_counts + 1);                   // n_touched
-  int* d_nchunks = ctx->bucket_off.as<int>() + buckets_ub;             // totals of the two scans
-  int* d_nlong = ctx->long_off.as<int>() + buckets_ub;
+  int* d_num = reinterpret_cast<int*>(d_counts + 1);                              // n_touched
+  PackCount* d_tot = ctx->bucket_off.as<PackCount>() + buckets_ub;                // totals of the scan
   TT_CUDA(cudaMemsetAsync(d_num, 0, sizeof(int), st));
-  TT_CUDA(cudaMemsetAsync(ctx->bucket_cnt.p, 0, sizeof(int) * (size_t)(buckets_ub + 1), st));
-  TT_CUDA(cudaMemsetAsync(ctx->long_cnt.p, 0, sizeof(int) * (size_t)(buckets_ub + 1), st));
+  TT_CUDA(cudaMemsetAsync(ctx->bucket_cnt.p, 0, sizeof(PackCount) * (size_t)(buckets_ub + 1), st));
   const int force_general = (ctx->opt.flags & TT_FLAG_FORCE_GENERAL_ROWS) ? 1 : 0;
   if (touched_ub > 0) {
     k_vertex_touch<<<grid_for(nT, 256), 256, 0, st>>>(q->tris, deg, nT, vcnt);
@@ -443,45 +424,62 @@ tt_status symbolic_impl(tt_ctx* ctx, const tt_problem* q, int64_t* nnzb_host, in
     k_touched_first<<<grid_for(touched_ub + 1, 256), 256, 0, st>>>(ctx->touched.as<int>(), d_num, ctx->tptr.as<int>(), nT,
                                                                    ctx->tfirst.as<int>());
     TT_LAUNCH_CHECK();
-    k_chunk_pack<false><<<grid_for(buckets_ub, 128), 128, 0, st>>>(ctx->tfirst.as<int>(), d_num, ctx->bucket_cnt.as<int>(),
-                                                                  ctx->long_cnt.as<int>(), nullptr, nullptr, nullptr, nullptr);
+    const int64_t prep_pers = (int64_t)ctx->sms * 8;
+    const int64_t prep_full = (touched_ub + 32 * SYM_WARPS - 1) / (32 * SYM_WARPS);
+    if (n_ub > RND_MAX_ENT) {  // long triangles: segment sort + can it be split into parts?
+      k_long_prep<<<(unsigned)(prep_full < prep_pers ? prep_full : prep_pers), 32 * SYM_WARPS, 0, st>>>(
+          q->tris, ctx->touched.as<int>(), d_num, ctx->tfirst.as<int>(), ctx->ent_in.as<uint2>(), vcnt, force_general,
+          ctx->partner.as<int>(), ctx->dvals.as<uint16_t>(), ctx->tsplit.as<int>());
+      TT_LAUNCH_CHECK();
+    }
+    k_chunk_pack<false><<<grid_for(buckets_ub, 128), 128, 0, st>>>(ctx->tfirst.as<int>(), d_num, ctx->tsplit.as<int>(),
+                                                                  ctx->bucket_cnt.as<PackCount>(), nullptr, nullptr, nullptr,
+                                                                  nullptr, nullptr, nullptr);
     TT_LAUNCH_CHECK();
-    s = scan_i32(ctx, ctx->bucket_cnt.as<int>(), ctx->bucket_off.as<int>(), buckets_ub + 1, st);
-    if (s != TT_OK) return s;
-    s = scan_i32(ctx, ctx->long_cnt.as<int>(), ctx->long_off.as<int>(), buckets_ub + 1, st);
-    if (s != TT_OK) return s;
-    k_chunk_pack<true><<<grid_for(buckets_ub, 128), 128, 0, st>>>(ctx->tfirst.as<int>(), d_num, nullptr, nullptr,
-                                                                 ctx->bucket_off.as<int>(), ctx->long_off.as<int>(),
-                                                                 ctx->rdesc.as<int4>(), ctx->long_list.as<int>());
+    {
+      size_t tmp2 = 0;
+      const PackCount zero{0, 0, 0, 0, 0};
+      TT_CUDA(cub::DeviceScan::ExclusiveScan(nullptr, tmp2, ctx->bucket_cnt.as<PackCount>(), ctx->bucket_off.as<PackCount>(),
+                                             PackAdd(), zero, buckets_ub + 1, st));
+      TT_CUDA(ctx->cub_tmp.ensure(tmp2));
+      TT_CUDA(cub::DeviceScan::ExclusiveScan(ctx->cub_tmp.p, tmp2, ctx->bucket_cnt.as<PackCount>(), ctx->bucket_off.as<PackCount>(),
+                                             PackAdd(), zero, buckets_ub + 1, st));
+      ctx->launches += 2;
+    }
+    k_chunk_pack<true><<<grid_for(buckets_ub, 128), 128, 0, st>>>(ctx->tfirst.as<int>(), d_num, ctx->tsplit.as<int>(), nullptr,
+                                                                 ctx->bucket_off.as<PackCount>(), ctx->rdesc.as<int4>(),
+                                                                 ctx->long_list.as<int>(), ctx->sfirst.as<int>(),
+                                                                 ctx->sinfo.as<int4>(), ctx->split_list.as<int4>());
     TT_LAUNCH_CHECK();
-    // ---- per-triangle segment sort, column ranks, exclusive rows, general-row workspace sizes
+    // ---- per-slot segment sort, column ranks, exclusive rows, general-row workspace sizes
     //      (persistent grids: the round / long-triangle counts are read on the device) ----
-    const int64_t rounds_ub = (touched_ub + RSYM_WARPS - 1) / RSYM_WARPS;
+    const int64_t rounds_ub = (slots_ub + RSYM_WARPS - 1) / RSYM_WARPS;
     const int64_t sym_pers = (int64_t)ctx->sms * 16;
     k_round_symbolic<<<(unsigned)(rounds_ub < sym_pers ? rounds_ub : sym_pers), 32 * RSYM_WARPS, 0, st>>>(
-        q->tris, ctx->touched.as<int>(), ctx->rdesc.as<int4>(), d_nchunks, ctx->tfirst.as<int>(), ctx->ent_in.as<uint2>(),
-        vcnt, force_general, ctx->partner.as<int>(), ctx->dvals.as<uint16_t>(), ctx->erank.as<int>(), ctx->drank.as<int>(),
-        rowlen, ctx->tlen.as<int64_t>(), ctx->slot_excl.as<uint8_t>(), ctx->everts.as<int>(), ctx->vslot1.as<int>());
+        q->tris, ctx->touched.as<int>(), ctx->rdesc.as<int4>(), &d_tot->rounds, ctx->tfirst.as<int>(), ctx->sfirst.as<int>(),
+        ctx->sinfo.as<int4>(), ctx->tsplit.as<int>(), ctx->ent_in.as<uint2>(), vcnt, force_general, ctx->partner.as<int>(),
+        ctx->dvals.as<uint16_t>(), ctx->erank.as<int>(), ctx->drank.as<int>(), rowlen, ctx->tlen.as<int64_t>(),
+        ctx->slot_excl.as<uint8_t>(), ctx->everts.as<int>(), ctx->vslot1.as<int>());
     TT_LAUNCH_CHECK();
     const int64_t long_ub = n_ub / (RND_MAX_ENT + 1);
-    if (long_ub > 0) {  // triangles with more than RND_MAX_ENT partners: one warp per triangle
+    if (long_ub > 0) {  // long triangles that could not be split: one warp per triangle
       const int64_t lg = (long_ub + SYM_WARPS - 1) / SYM_WARPS;
       const int64_t lpers = (int64_t)ctx->sms * 8;
       k_tri_symbolic<<<(unsigned)(lg < lpers ? lg : lpers), 32 * SYM_WARPS, 0, st>>>(
-          q->tris, ctx->touched.as<int>(), d_nlong, ctx->tfirst.as<int>(), ctx->ent_in.as<uint2>(), ctx->partner.as<int>(),
+          q->tris, ctx->touched.as<int>(), &d_tot->longs, ctx->tfirst.as<int>(), ctx->sinfo.as<int4>(), ctx->partner.as<int>(),
           ctx->dvals.as<uint16_t>(), vcnt, force_general, ctx->erank.as<int>(), ctx->drank.as<int>(), rowlen,
           ctx->tlen.as<int64_t>(), ctx->slot_excl.as<uint8_t>(), ctx->long_list.as<int>(), ctx->rdesc.as<int4>(),
           ctx->vslot1.as<int>(), ctx->everts.as<int>());
       TT_LAUNCH_CHECK();
     }
   }
-  {  // general-row workspace offsets: scan over the bound, lengths beyond 3 n_touched read as 0
+  {  // general-row workspace offsets: scan over the bound, lengths beyond 3 n_slots read as 0
     cub::CountingInputIterator<int64_t> idx(0);
-    cub::TransformInputIterator<int64_t, MaskedLen, cub::CountingInputIterator<int64_t>> it(idx, MaskedLen{ctx->tlen.as<int64_t>(), d_num});
+    cub::TransformInputIterator<int64_t, MaskedLen, cub::CountingInputIterator<int64_t>> it(idx, MaskedLen{ctx->tlen.as<int64_t>(), &d_tot->slots});
     size_t tmp = 0;
-    TT_CUDA(cub::DeviceScan::ExclusiveSum(nullptr, tmp, it, ctx->toff.as<int64_t>(), 3 * touched_ub + 1, st));
+    TT_CUDA(cub::DeviceScan::ExclusiveSum(nullptr, tmp, it, ctx->toff.as<int64_t>(), 3 * slots_ub + 1, st));
     TT_CUDA(ctx->cub_tmp.ensure(tmp));
-    TT_CUDA(cub::DeviceScan::ExclusiveSum(ctx->cub_tmp.p, tmp, it, ctx->toff.as<int64_t>(), 3 * touched_ub + 1, st));
+    TT_CUDA(cub::DeviceScan::ExclusiveSum(ctx->cub_tmp.p, tmp, it, ctx->toff.as<int64_t>(), 3 * slots_ub + 1, st));
     ctx->launches += 2;
   }
   // The row-pointer scan is issued speculatively: if there are no general rows (R == 0: always, in a
@@ -490,16 +488,19 @@ tt_status symbolic_impl(tt_ctx* ctx, const tt_problem* q, int64_t* nnzb_host, in
   if (s != TT_OK) return s;
   // ---- the ONE host round trip of the phase (soup; general rows add the merge pass below) ----
   int64_t A = 0, R = 0, nnzb = 0;
-  int cnt32[3] = {0, 0, 0};
+  int ntch = 0;
+  PackCount tot{0, 0, 0, 0, 0};
   TT_CUDA(cudaMemcpyAsync(&A, d_counts, sizeof(int64_t), cudaMemcpyDeviceToHost, st));
-  TT_CUDA(cudaMemcpyAsync(&cnt32[0], d_num, sizeof(int), cudaMemcpyDeviceToHost, st));
-  TT_CUDA(cudaMemcpyAsync(&cnt32[1], d_nchunks, sizeof(int), cudaMemcpyDeviceToHost, st));
-  TT_CUDA(cudaMemcpyAsync(&cnt32[2], d_nlong, sizeof(int), cudaMemcpyDeviceToHost, st));
-  TT_CUDA(cudaMemcpyAsync(&R, ctx->toff.as<int64_t>() + 3 * touched_ub, sizeof(int64_t), cudaMemcpyDeviceToHost, st));
+  TT_CUDA(cudaMemcpyAsync(&ntch, d_num, sizeof(int), cudaMemcpyDeviceToHost, st));
+  if (touched_ub > 0) TT_CUDA(cudaMemcpyAsync(&tot, d_tot, sizeof(PackCount), cudaMemcpyDeviceToHost, st));
+  TT_CUDA(cudaMemcpyAsync(&R, ctx->toff.as<int64_t>() + 3 * slots_ub, sizeof(int64_t), cudaMemcpyDeviceToHost, st));
   TT_CUDA(cudaMemcpyAsync(&nnzb, ctx->rowptr64.as<int64_t>() + nV, sizeof(int64_t), cudaMemcpyDeviceToHost, st));
   TT_CUDA(cudaStreamSynchronize(st));
   const int64_t n = 2 * A;
-  const int64_t n_touched = touched_ub > 0 ? cnt32[0] : 0, n_chunks = touched_ub > 0 ? cnt32[1] : 0, n_long = touched_ub > 0 ? cnt32[2] : 0;
+  const int64_t n_touched = touched_ub > 0 ? ntch : 0, n_chunks = tot.rounds, n_long = tot.longs, n_slots = tot.slots;
+  ctx->n_slots = n_slots;
+  ctx->n_split = tot.splits;
+  ctx->n_parts = tot.parts;
   ctx->A = A;
   ctx->n_dir = n;
   ctx->n_touched = n_touched;
@@ -507,7 +508,7 @@ tt_status symbolic_impl(tt_ctx* ctx, const tt_problem* q, int64_t* nnzb_host, in
   ctx->n_long = n_long;
   if (R >= (int64_t(1) << 31)) return fail(ctx, TT_ERR_INVALID_ARG, "general-row workspace exceeds 2^31 blocks");
   ctx->R = R;
-  const unsigned tri_grid = grid_for(n_touched, SYM_WARPS);
+  const unsigned tri_grid = grid_for(n_slots, SYM_WARPS);
   const unsigned rnd_grid = grid_for(n_chunks, RSYM_WARPS);
 
   // ---- general rows: merge records sorted by (row, col) ----
@@ -525,7 +526,7 @@ tt_status symbolic_impl(tt_ctx* ctx, const tt_problem* q, int64_t* nnzb_host, in
     TT_CUDA(ctx->run_start.ensure(sizeof(int) * (size_t)(R + 1)));
     TT_CUDA(ctx->run_dest.ensure(sizeof(int) * (size_t)(R + 1)));
     k_emit_records<<<tri_grid, 32 * SYM_WARPS, 0, st>>>(
-        q->tris, ctx->touched.as<int>(), n_touched, ctx->tfirst.as<int>(), ctx->partner.as<int>(), bitsV,
+        q->tris, ctx->touched.as<int>(), n_slots, ctx->sfirst.as<int>(), ctx->sinfo.as<int4>(), ctx->partner.as<int>(), bitsV,
         ctx->erank.as<int>(), ctx->drank.as<int>(), ctx->toff.as<int64_t>(), ctx->slot_excl.as<uint8_t>(),
         ctx->rkeys[0].as<uint64_t>(), ctx->rvals[0].as<uint32_t>());
     TT_LAUNCH_CHECK();
@@ -562,14 +563,15 @@ tt_status symbolic_impl(tt_ctx* ctx, const tt_problem* q, int64_t* nnzb_host, in
   }
   if (n_chunks > 0) {
     k_round_fill<<<rnd_grid, 32 * RSYM_WARPS, 0, st>>>(
-        q->tris, ctx->touched.as<int>(), ctx->rdesc.as<int4>(), n_chunks, ctx->tfirst.as<int>(), ctx->partner.as<int>(),
+        q->tris, ctx->touched.as<int>(), ctx->rdesc.as<int4>(), n_chunks, ctx->sfirst.as<int>(), ctx->sinfo.as<int4>(),
+        ctx->tsplit.as<int>(), ctx->partner.as<int>(),
         ctx->erank.as<int>(), ctx->drank.as<int>(), ctx->toff.as<int64_t>(), ctx->slot_excl.as<uint8_t>(),
         ctx->rowptr.as<int>(), ctx->rowbase.as<int64_t>(), ctx->colind.as<int>());
     TT_LAUNCH_CHECK();
   }
   if (n_long > 0) {
     k_fill_rows<<<grid_for(n_long, SYM_WARPS), 32 * SYM_WARPS, 0, st>>>(
-        q->tris, ctx->touched.as<int>(), n_long, ctx->tfirst.as<int>(), ctx->partner.as<int>(),
+        q->tris, ctx->touched.as<int>(), n_long, ctx->sfirst.as<int>(), ctx->sinfo.as<int4>(), ctx->partner.as<int>(),
         ctx->erank.as<int>(), ctx->drank.as<int>(), ctx->toff.as<int64_t>(), ctx->slot_excl.as<uint8_t>(),
         ctx->rowptr.as<int>(), ctx->rowbase.as<int64_t>(), ctx->colind.as<int>(), ctx->long_list.as<int>(),
         ctx->rdesc.as<int4>());
@@ -579,12 +581,13 @@ tt_status symbolic_impl(tt_ctx* ctx, const tt_problem* q, int64_t* nnzb_host, in
   // ---- per-slot buffers, vertex -> slot incidence ----
   TT_CUDA(ctx->asm_energy.ensure(sizeof(double) * (size_t)(n_chunks + 1)));
   TT_CUDA(ctx->tvals.ensure(sizeof(T) * 9 * (size_t)(R + 1)));
-  TT_CUDA(ctx->tslot.ensure(sizeof(T) * 9 * (size_t)(n_touched + 1)));
+  TT_CUDA(ctx->tslot.ensure(sizeof(T) * 9 * (size_t)(n_slots + 1)));
+  TT_CUDA(ctx->dpart.ensure(sizeof(double) * NDIAG * (size_t)(ctx->n_parts + 1)));
   // vertex -> slot incidence: only when some vertex has more than one slot.  R == 0 means every slot
   // is exclusive, hence every touched vertex has exactly one (k_gather3 then reads vslot1 only).
   ctx->vvals_sorted = nullptr;
   if (R > 0) {
-    const int64_t nvs = 3 * n_touched;
+    const int64_t nvs = 3 * n_slots;
     for (int i = 0; i < 2; ++i) {
       TT_CUDA(ctx->vkeys[i].ensure(sizeof(uint64_t) * (size_t)(nvs + 1)));
       TT_CUDA(ctx->vvals[i].ensure(sizeof(uint32_t) * (size_t)(nvs + 1)));
@@ -592,10 +595,11 @@ tt_status symbolic_impl(tt_ctx* ctx, const tt_problem* q, int64_t* nnzb_host, in
     TT_CUDA(ctx->vptr.ensure(sizeof(int) * (size_t)(nV + 2)));
     uint64_t* vkeys_sorted = ctx->vkeys[0].as<uint64_t>();
     ctx->vvals_sorted = ctx->vvals[0].as<uint32_t>();
-    k_emit_vslots<<<grid_for(nvs, 256), 256, 0, st>>>(q->tris, ctx->touched.as<int>(), n_touched,
-                                                      ctx->vkeys[0].as<uint64_t>(), ctx->vvals[0].as<uint32_t>());
+    k_emit_vslots<<<grid_for(nvs, 256), 256, 0, st>>>(q->tris, ctx->touched.as<int>(), n_slots, ctx->sinfo.as<int4>(),
+                                                      ctx->tsplit.as<int>(), nV, ctx->vkeys[0].as<uint64_t>(),
+                                                      ctx->vvals[0].as<uint32_t>());
     TT_LAUNCH_CHECK();
-    s = sort_pairs(ctx, ctx->vkeys, ctx->vvals, nvs, 0, bitsV, &vkeys_sorted, &ctx->vvals_sorted, st);
+    s = sort_pairs(ctx, ctx->vkeys, ctx->vvals, nvs, 0, ceil_log2(nV + 1), &vkeys_sorted, &ctx->vvals_sorted, st);
     if (s != TT_OK) return s;
     k_segment_ptr<<<grid_for(nvs + 1, 256), 256, 0, st>>>(vkeys_sorted, nvs, 0, nV, ctx->vptr.as<int>());
     TT_LAUNCH_CHECK();
@@ -621,7 +625,8 @@ ttk::AsmParams<T> make_params(tt_ctx* ctx, const tt_problem* q) {
   p.dvals = ctx->dvals.as<uint16_t>();
   p.everts = ctx->everts.as<int>();
   p.rdesc = ctx->rdesc.as<int4>();
-  p.tfirst = ctx->tfirst.as<int>();
+  p.tfirst = ctx->sfirst.as<int>();
+  p.dpart = ctx->dpart.as<double>();
   p.long_list = ctx->long_list.as<int>();
   p.erank = ctx->erank.as<int>();
   p.drank = ctx->drank.as<int>();
@@ -636,6 +641,17 @@ ttk::AsmParams<T> make_params(tt_ctx* ctx, const tt_problem* q) {
   p.hess_mode = ctx->opt.hess_mode;
   p.sigma = ctx->opt.tc_scale;
   return p;
+}
+
+// split triangles: parts' partial sums -> the triangle's first slot (+ the diagonal blocks after K4)
+template <typename T, bool HESS>
+tt_status launch_split_finish(tt_ctx* ctx, const tt_problem* q, T* vals, cudaStream_t st) {
+  if (ctx->n_split <= 0) return TT_OK;
+  ttk::k_split_finish<T, HESS><<<grid_for(ctx->n_split, 4), 128, 0, st>>>(
+      ctx->split_list.as<int4>(), ctx->n_split, q->tris, ctx->touched.as<int>(), ctx->tsplit.as<int>(), ctx->rowptr.as<int>(),
+      ctx->dpart.as<double>(), ctx->tslot.as<T>(), vals);
+  TT_LAUNCH_CHECK();
+  return TT_OK;
 }
 
 // K6 launch: pipelined kernel over all rounds (skips long ones) + the plain kernel over the long rounds
@@ -673,7 +689,6 @@ tt_status numeric_impl(tt_ctx* ctx, const tt_problem* q, void* energy_sum, void*
   p.vals = (T*)vals;
   if (ctx->n_chunks > 0) {
     cudaEvent_t* ev_k4 = ctx->evr[1][ctx->ev_n[1] % tt_ctx::EV_RING];
-    l2_window(ctx, st, q->pos, sizeof(T) * 3 * (size_t)q->n_verts);
     TT_CUDA(cudaEventRecord(ev_k4[0], st));
     if (want_h) {
       const size_t smem = sizeof(TileWarpSmem<T>) * TILE_WARPS;
@@ -691,13 +706,16 @@ tt_status numeric_impl(tt_ctx* ctx, const tt_problem* q, void* energy_sum, void*
         TT_LAUNCH_CHECK();
         k_assemble_long_direct<T><<<grid_for(ctx->n_long, TILE_WARPS), 32 * TILE_WARPS, sizeof(LongWarpSmem) * TILE_WARPS, st>>>(p);
       }
+      TT_LAUNCH_CHECK();
+      tt_status s2 = launch_split_finish<T, true>(ctx, q, (T*)vals, st);
+      if (s2 != TT_OK) return s2;
     } else {
       tt_status s1 = launch_entry_reduce<T, 1>(ctx, p, st);
       if (s1 != TT_OK) return s1;
+      s1 = launch_split_finish<T, false>(ctx, q, (T*)nullptr, st);
+      if (s1 != TT_OK) return s1;
     }
-    TT_LAUNCH_CHECK();
     TT_CUDA(cudaEventRecord(ev_k4[1], st));
-    l2_window_off(ctx, st);
     ctx->ev_n[1]++;
     if (want_h && ctx->U > 0) {
       k_merge<T><<<grid_for(9 * ctx->U, 256), 256, 0, st>>>(ctx->run_start.as<int>(), ctx->run_dest.as<int>(),
@@ -720,12 +738,12 @@ tt_status hessvec_impl(tt_ctx* ctx, const tt_problem* q, const void* pvec, void*
   p.chunk_energy = nullptr;
   if (ctx->n_chunks > 0) {
     cudaEvent_t* ev_k6 = ctx->evr[2][ctx->ev_n[2] % tt_ctx::EV_RING];
-    l2_window(ctx, st, q->pos, sizeof(T) * 3 * (size_t)q->n_verts);
     TT_CUDA(cudaEventRecord(ev_k6[0], st));
     tt_status s1 = launch_entry_reduce<T, 2>(ctx, p, st);
     if (s1 != TT_OK) return s1;
+    s1 = launch_split_finish<T, false>(ctx, q, (T*)nullptr, st);
+    if (s1 != TT_OK) return s1;
     TT_CUDA(cudaEventRecord(ev_k6[1], st));
-    l2_window_off(ctx, st);
     ctx->ev_n[2]++;
   }
   if (q->n_verts > 0) {
@@ -955,22 +973,6 @@ tt_status tt_create(const tt_options* opt, tt_ctx** out) {
     pipe_setup((const void*)ttk::k_entry_pipe<float, 2>, sizeof(ttk::PipeWarpSmem<float, 2>) * ttk::PIPE_WARPS, c->pipe_grid[1][1]);
     if (e != cudaSuccess) { (void)cudaGetLastError(); delete c; return TT_ERR_CUDA; }
     c->sms = sms;
-    if (const char* env = getenv("TT_L2_PERSIST")) {  // experiment switch: fraction of the maximum set-aside
-      const double frac = atof(env);
-      int max_persist = 0, max_win = 0;
-      cudaDeviceGetAttribute(&max_persist, cudaDevAttrMaxPersistingL2CacheSize, opt->device);
-      cudaDeviceGetAttribute(&max_win, cudaDevAttrMaxAccessPolicyWindowSize, opt->device);
-      if (frac > 0.0 && max_persist > 0 && max_win > 0) {
-        const size_t want = (size_t)(frac * (double)max_persist);
-        if (cudaDeviceSetLimit(cudaLimitPersistingL2CacheSize, want) == cudaSuccess) {
-          c->l2_persist_bytes = want;
-          c->l2_max_window = (size_t)max_win;
-        } else {
-          (void)cudaGetLastError();
-        }
-      }
-      if (getenv("TT_VERBOSE")) fprintf(stderr, "[tt] L2 persisting: max %d B, window max %d B, set-aside %zu B\n", max_persist, max_win, c->l2_persist_bytes);
-    }
     c->tile_grid[0] = sms * (nb0 > 0 ? nb0 : 1);  // one wave of resident CTAs: the kernel is persistent
     c->tile_grid[1] = sms * (nb1 > 0 ? nb1 : 1);
   }
@@ -1229,8 +1231,9 @@ tt_status tt_bsr_device(tt_ctx* ctx, const int32_t** rowptr, const int32_t** col
 
 tt_status tt_stats(const tt_ctx* ctx, int64_t* what, int32_t n) {
   if (!ctx || !what || n < 0) return TT_ERR_INVALID_ARG;
-  const int64_t v[8] = {ctx->A, ctx->n_dir, ctx->n_touched, ctx->nnzb - ctx->U, ctx->U, ctx->R, ctx->nnzb, ctx->launches};
-  for (int i = 0; i < n && i < 8; ++i) what[i] = v[i];
+  const int64_t v[12] = {ctx->A, ctx->n_dir, ctx->n_touched, ctx->nnzb - ctx->U, ctx->U, ctx->R, ctx->nnzb, ctx->launches,
+                         ctx->n_slots, ctx->n_split, ctx->n_parts, ctx->n_long};
+  for (int i = 0; i < n && i < 12; ++i) what[i] = v[i];
   return TT_OK;
 }
 

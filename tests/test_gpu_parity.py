@@ -189,19 +189,39 @@ def test_config4_sweep_reduced(oracle_mod, dtype):
 
 
 @pytest.mark.parametrize("n_pairs,dtype", [(24_000, "f64"), (24_000, "f32"), (60_000, "f64")])
-def test_long_triangles(oracle_mod, n_pairs, dtype):
-    """Few triangles, many pairs each.  24k pairs: ~60 partners per triangle, a mix of ordinary rounds,
-    long triangles with J cached (33..64 partners) and re-evaluated (65..127) in the one-row tile
-    (k_assemble_long_tile<true / false>); 60k pairs: ~150 partners, beyond the tile
-    (k_assemble_long_direct)."""
+@pytest.mark.parametrize("layout", ["soup", "shuffled"])
+def test_long_triangles(oracle_mod, n_pairs, dtype, layout):
+    """Few triangles, many pairs each.  24k pairs: ~60 partners per triangle; 60k pairs: ~150.
+    layout "soup" (vertex ids 3t, 3t+1, 3t+2): every triangle with more than 32 partners is SPLIT into parts
+    that ride in ordinary rounds (k_long_prep, part slots in K4 / K6, k_split_finish).
+    layout "shuffled" (the same soup with its vertex ids randomly permuted): the partners' columns interleave,
+    so no long triangle can be split and all three long-triangle kernels run (k_assemble_long_tile<true> for
+    33..64 partners, <false> for 65..127, k_assemble_long_direct beyond), rows still exclusive."""
     from paper_2606_06511_b200 import inputs
     pb = inputs.config4_sweep(n_tris=400, n_pairs=n_pairs, seed=4242)
+    if layout == "shuffled":
+        perm = np.random.default_rng(1).permutation(pb.n_verts)          # new id of old vertex v = perm[v]
+        pos = np.empty_like(pb.pos)
+        pos[perm] = pb.pos
+        pb = inputs.Problem(pos, perm[pb.tris].astype(np.int32), pb.pairs, pb.name + "_shuffled", pb.meta)
     ref, out, st = run_case(oracle_mod, pb, dtype, 1)
     deg = np.bincount(pb.pairs[ref["active"].astype(bool)].ravel(), minlength=400)
     if n_pairs == 24_000:
         assert ((deg > 32) & (deg <= 64)).sum() > 50 and ((deg > 64) & (deg <= 127)).sum() > 30 and (deg <= 32).sum() > 20
     else:
         assert (deg > 127).sum() > 50
+    assert st["blocks_merged"] == 0
+    assert (st["split_triangles"] > 50) if layout == "soup" else (st["split_triangles"] == 0 and st["long_rounds"] > 50)
+
+
+def test_long_triangles_shared_vertices(oracle_mod):
+    """Long triangles on a shared-vertex pool: not splittable, general (merge) rows, all four hess modes' worth of
+    structure in one: k_tri_symbolic ranking with duplicates, the long kernels writing to the merge workspace."""
+    from paper_2606_06511_b200 import inputs
+    pb = inputs.config0_soup(n_tris=260, pool=400, seed=31)
+    ref, out, st = run_case(oracle_mod, pb, "f64", 1)
+    deg = np.bincount(pb.pairs[ref["active"].astype(bool)].ravel(), minlength=260)
+    assert (deg > 32).sum() > 20 and st["blocks_merged"] > 0 and st["long_rounds"] > 20
 
 
 # ------------------------------------------------------------------------------------ edge cases

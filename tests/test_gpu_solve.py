@@ -102,7 +102,7 @@ def test_pcg_iterates_match_oracle(oracle_mod, backend, precond):
             torch.cuda.synchronize()
             assert iters == k
             assert rel(x.cpu().numpy(), orc["x_hist"][k]) <= tol, (pb.name, k)
-            assert abs(relres - orc["res"][k] / orc["res"][0]) <= 1e-6 * (orc["res"][k] / orc["res"][0]) + 1e-14
+            assert abs(relres - orc["res"][k] / orc["res"][0]) <= max(1e-6, 20 * tol) * (orc["res"][k] / orc["res"][0]) + 1e-14
         ctx.close()
 
 
