@@ -12,20 +12,26 @@
 
 namespace ttg {
 
-struct d3 {
-  double x, y, z;
+// 3-vector over the scalar S: double everywhere a discrete decision is taken (K1) and in the fp64
+// variant; float in the derivative / outer-product arithmetic of the fp32 variant (reading A12).
+template <typename S>
+struct v3 {
+  S x, y, z;
 };
-__device__ __forceinline__ d3 mk(double x, double y, double z) { return d3{x, y, z}; }
-__device__ __forceinline__ d3 operator+(d3 a, d3 b) { return mk(a.x + b.x, a.y + b.y, a.z + b.z); }
-__device__ __forceinline__ d3 operator-(d3 a, d3 b) { return mk(a.x - b.x, a.y - b.y, a.z - b.z); }
-__device__ __forceinline__ d3 operator*(double s, d3 a) { return mk(s * a.x, s * a.y, s * a.z); }
-__device__ __forceinline__ double dot(d3 a, d3 b) { return fma(a.x, b.x, fma(a.y, b.y, a.z * b.z)); }
-__device__ __forceinline__ d3 cross(d3 a, d3 b) {
-  return mk(fma(a.y, b.z, -(a.z * b.y)), fma(a.z, b.x, -(a.x * b.z)), fma(a.x, b.y, -(a.y * b.x)));
+using d3 = v3<double>;
+template <typename S> __device__ __forceinline__ v3<S> mk(S x, S y, S z) { return v3<S>{x, y, z}; }
+template <typename S> __device__ __forceinline__ v3<S> operator+(v3<S> a, v3<S> b) { return mk<S>(a.x + b.x, a.y + b.y, a.z + b.z); }
+template <typename S> __device__ __forceinline__ v3<S> operator-(v3<S> a, v3<S> b) { return mk<S>(a.x - b.x, a.y - b.y, a.z - b.z); }
+template <typename S> __device__ __forceinline__ v3<S> operator*(S s, v3<S> a) { return mk<S>(s * a.x, s * a.y, s * a.z); }
+template <typename S> __device__ __forceinline__ S dot(v3<S> a, v3<S> b) { return fma(a.x, b.x, fma(a.y, b.y, a.z * b.z)); }
+template <typename S> __device__ __forceinline__ v3<S> cross(v3<S> a, v3<S> b) {
+  return mk<S>(fma(a.y, b.z, -(a.z * b.y)), fma(a.z, b.x, -(a.x * b.z)), fma(a.x, b.y, -(a.y * b.x)));
 }
-__device__ __forceinline__ d3 axpy(double s, d3 a, d3 b) {  // s*a + b
-  return mk(fma(s, a.x, b.x), fma(s, a.y, b.y), fma(s, a.z, b.z));
+template <typename S> __device__ __forceinline__ v3<S> axpy(S s, v3<S> a, v3<S> b) {  // s*a + b
+  return mk<S>(fma(s, a.x, b.x), fma(s, a.y, b.y), fma(s, a.z, b.z));
 }
+__device__ __forceinline__ double inv_sqrt(double x) { return rsqrt(x); }
+__device__ __forceinline__ float inv_sqrt(float x) { return rsqrtf(x); }
 __device__ __forceinline__ d3 sel3(int i, d3 v0, d3 v1, d3 v2) {
   d3 r = v2;
   if (i == 1) r = v1;
@@ -161,26 +167,28 @@ __device__ __forceinline__ unsigned pair_config(const PairGeom& g) {
 //               y_k from translation invariance (all six blocks of D^T dE sum to D).
 // nY = (y_p - y_k) x (y_q - y_k) and the distances d are taken with THAT normal, so the formulas hold
 // for any labelling (k, p, q) of Y (an odd one flips nY and d together).
+template <typename S>
 struct EndPoint {
-  double t;                    // D . E
-  d3 ownk, owne, yk, yp, yq;   // blocks of s D^T dE
+  S t;                            // D . E
+  v3<S> ownk, owne, yk, yp, yq;   // blocks of s D^T dE
 };
-__device__ __forceinline__ EndPoint end_point(double s, const d3 Dh, const d3 xk, const d3 ex, double dk,
-                                              double de, double zmask, const d3 yk, const d3 eyp,
-                                              const d3 eyq, const d3 nY) {
-  EndPoint r;
-  const double inv = 1.0 / (dk - de);  // opposite signs: |dk - de| = |dk| + |de|, no cancellation
-  const double tau = dk * inv;
-  const d3 E = axpy(tau, ex, xk);
+template <typename S>
+__device__ __forceinline__ EndPoint<S> end_point(S s, const v3<S> Dh, const v3<S> xk, const v3<S> ex, S dk,
+                                                 S de, S zmask, const v3<S> yk, const v3<S> eyp,
+                                                 const v3<S> eyq, const v3<S> nY) {
+  EndPoint<S> r;
+  const S inv = S(1) / (dk - de);  // opposite signs: |dk - de| = |dk| + |de|, no cancellation
+  const S tau = dk * inv;
+  const v3<S> E = axpy(tau, ex, xk);
   r.t = dot(Dh, E);
-  const double w = s * zmask * dot(Dh, ex) * inv;  // s c / den
-  const double wn = w * inv;                       // s c / den^2
-  r.ownk = axpy(s * (1.0 - tau), Dh, (-(wn * de)) * nY);
+  const S w = s * zmask * dot(Dh, ex) * inv;  // s c / den
+  const S wn = w * inv;                       // s c / den^2
+  r.ownk = axpy(s * (S(1) - tau), Dh, (-(wn * de)) * nY);
   r.owne = axpy(s * tau, Dh, (wn * dk) * nY);
-  const d3 u = E - yk;
+  const v3<S> u = E - yk;
   r.yp = w * cross(eyq, u);
   r.yq = w * cross(u, eyp);
-  r.yk = mk(-fma(w, nY.x, r.yp.x + r.yq.x), -fma(w, nY.y, r.yp.y + r.yq.y), -fma(w, nY.z, r.yp.z + r.yq.z));
+  r.yk = mk<S>(-fma(w, nY.x, r.yp.x + r.yq.x), -fma(w, nY.y, r.yp.y + r.yq.y), -fma(w, nY.z, r.yp.z + r.yq.z));
   return r;
 }
 
@@ -189,24 +197,25 @@ __device__ __forceinline__ EndPoint end_point(double s, const d3 Dh, const d3 xk
 //   x = [a_k, a_p, a_q, b_k, b_p, b_q].  The line direction is taken from the PERMUTED normals, so
 //   (tc0, tc1, g0, g1) may come out as (-tc0, -tc1, -g0, -g1): Eq. 2-4 and L47's third quantity are
 //   even in that sign (every term pairs two of them), so energy, gradient and Hessian are unchanged.
-__device__ __forceinline__ void pair_derivs_recorded(const d3 ak, const d3 ap, const d3 aq, const d3 bk,
-                                                     const d3 bp, const d3 bq, double sigma, unsigned za,
-                                                     unsigned zb, double& tc0, double& tc1,
-                                                     double (&g0)[18], double (&g1)[18]) {
-  const d3 eap = ap - ak, eaq = aq - ak, ebp = bp - bk, ebq = bq - bk;
-  const d3 na = cross(eap, eaq), nb = cross(ebp, ebq);
-  const d3 ab = ak - bk;
-  const double dak = dot(nb, ab), dap = dot(nb, ap - bk), daq = dot(nb, aq - bk);
-  const double dbk = -dot(na, ab), dbp = dot(na, bp - ak), dbq = dot(na, bq - ak);
-  const d3 D = cross(na, nb);
-  const d3 Dh = rsqrt(dot(D, D)) * D;
-  const EndPoint Pa = end_point(sigma, Dh, ak, eap, dak, dap, za == 1u ? 0.0 : 1.0, bk, ebp, ebq, nb);
-  const EndPoint Qa = end_point(sigma, Dh, ak, eaq, dak, daq, za == 2u ? 0.0 : 1.0, bk, ebp, ebq, nb);
-  const EndPoint Pb = end_point(-sigma, Dh, bk, ebp, dbk, dbp, zb == 1u ? 0.0 : 1.0, ak, eap, eaq, na);
-  const EndPoint Qb = end_point(-sigma, Dh, bk, ebq, dbk, dbq, zb == 2u ? 0.0 : 1.0, ak, eap, eaq, na);
+template <typename S>
+__device__ __forceinline__ void pair_derivs_recorded(const v3<S> ak, const v3<S> ap, const v3<S> aq, const v3<S> bk,
+                                                     const v3<S> bp, const v3<S> bq, S sigma, unsigned za,
+                                                     unsigned zb, S& tc0, S& tc1,
+                                                     S (&g0)[18], S (&g1)[18]) {
+  const v3<S> eap = ap - ak, eaq = aq - ak, ebp = bp - bk, ebq = bq - bk;
+  const v3<S> na = cross(eap, eaq), nb = cross(ebp, ebq);
+  const v3<S> ab = ak - bk;
+  const S dak = dot(nb, ab), dap = dot(nb, ap - bk), daq = dot(nb, aq - bk);
+  const S dbk = -dot(na, ab), dbp = dot(na, bp - ak), dbq = dot(na, bq - ak);
+  const v3<S> D = cross(na, nb);
+  const v3<S> Dh = inv_sqrt(dot(D, D)) * D;
+  const EndPoint<S> Pa = end_point<S>(sigma, Dh, ak, eap, dak, dap, za == 1u ? S(0) : S(1), bk, ebp, ebq, nb);
+  const EndPoint<S> Qa = end_point<S>(sigma, Dh, ak, eaq, dak, daq, za == 2u ? S(0) : S(1), bk, ebp, ebq, nb);
+  const EndPoint<S> Pb = end_point<S>(-sigma, Dh, bk, ebp, dbk, dbp, zb == 1u ? S(0) : S(1), ak, eap, eaq, na);
+  const EndPoint<S> Qb = end_point<S>(-sigma, Dh, bk, ebq, dbk, dbq, zb == 2u ? S(0) : S(1), ak, eap, eaq, na);
   tc0 = sigma * (Pa.t - Qb.t);  // Eq. 1
   tc1 = sigma * (Qa.t - Pb.t);
-  auto put = [](double (&g)[18], int o, const d3 v) { g[o] = v.x; g[o + 1] = v.y; g[o + 2] = v.z; };
+  auto put = [](S (&g)[18], int o, const v3<S> v) { g[o] = v.x; g[o + 1] = v.y; g[o + 2] = v.z; };
   put(g0, 0, Pa.ownk + Qb.yk);   put(g0, 3, Pa.owne + Qb.yp);   put(g0, 6, Qb.yq);
   put(g0, 9, Pa.yk + Qb.ownk);   put(g0, 12, Pa.yp);            put(g0, 15, Pa.yq + Qb.owne);
   put(g1, 0, Qa.ownk + Pb.yk);   put(g1, 3, Pb.yp);             put(g1, 6, Qa.owne + Pb.yq);
@@ -221,9 +230,10 @@ __device__ __forceinline__ void pair_derivs_recorded(const d3 ak, const d3 ap, c
 // S+ = lambda_+ (S - lambda_- I) / (lambda_+ - lambda_-) (spectral projector of the positive
 // eigenvalue) and M+ = L^-T S+ L^-1.  The coefficients (c00, c11, c01) become the entries of M+ and
 // everything downstream is unchanged.  (The oracle projects the dense 18x18 matrix instead.)
+template <typename S>
 struct Coefs {
-  double cg0, cg1;       // Eq. 3: grad = cg0 g0 + cg1 g1
-  double c00, c11, c01;  // Eq. 4: H = c00 g0g0^T + c11 g1g1^T + c01 (g1g0^T + g0g1^T)
+  S cg0, cg1;       // Eq. 3: grad = cg0 g0 + cg1 g1
+  S c00, c11, c01;  // Eq. 4: H = c00 g0g0^T + c11 g1g1^T + c01 (g1g0^T + g0g1^T)
 };
 // PSDPROJ's 2x2 algebra, kept out of line (scalars in, scalars out): the three default modes then
 // compile as without it -- K4 runs at ~254 of 255 registers and is sensitive to every live value.
@@ -255,36 +265,36 @@ __device__ __noinline__ Sym2 psd_project_2x2(double p, double q, double r, doubl
   return o;
 }
 
-template <bool PROJ = true>  // PROJ = false: TT_HESS_PSDPROJ compiled out (K4's default instantiation)
-__device__ __forceinline__ Coefs pair_coefs(double tc0, double tc1, const double (&g0)[18],
-                                            const double (&g1)[18], int hess_mode) {
-  Coefs c;
-  c.cg0 = 2.0 * tc0 * (tc1 * tc1);
-  c.cg1 = 2.0 * tc1 * (tc0 * tc0);
-  c.c00 = 2.0 * (tc1 * tc1);
-  c.c11 = 2.0 * (tc0 * tc0);
-  double keep = 1.0;
+template <typename S, bool PROJ = true>  // PROJ = false: TT_HESS_PSDPROJ compiled out (K4's default instantiation)
+__device__ __forceinline__ Coefs<S> pair_coefs(S tc0, S tc1, const S (&g0)[18], const S (&g1)[18], int hess_mode) {
+  Coefs<S> c;
+  c.cg0 = S(2) * tc0 * (tc1 * tc1);
+  c.cg1 = S(2) * tc1 * (tc0 * tc0);
+  c.c00 = S(2) * (tc1 * tc1);
+  c.c11 = S(2) * (tc0 * tc0);
+  S keep = S(1);
   if (hess_mode == 1) {
-    double g01 = 0.0;
+    S g01 = S(0);
 #pragma unroll
     for (int i = 0; i < 18; ++i) g01 = fma(g0[i], g1[i], g01);
-    keep = (8.0 * tc0 * tc1 * g01 >= 0.0) ? 1.0 : 0.0;
+    keep = (tc0 * tc1 * g01 >= S(0)) ? S(1) : S(0);  // sign of L47's 8 tc0 tc1 (g0.g1)
   } else if (hess_mode == 2) {
-    keep = 0.0;
+    keep = S(0);
   }
-  c.c01 = 4.0 * tc0 * tc1 * keep;
+  c.c01 = S(4) * tc0 * tc1 * keep;
   if (PROJ && hess_mode == 3) {
-    double p = 0.0, q = 0.0, r = 0.0;
+    S p = S(0), q = S(0), r = S(0);
 #pragma unroll
     for (int i = 0; i < 18; ++i) {
       p = fma(g0[i], g0[i], p);
       q = fma(g0[i], g1[i], q);
       r = fma(g1[i], g1[i], r);
     }
-    const Sym2 m = psd_project_2x2(p, q, r, c.c00, c.c01, c.c11);
-    c.c00 = m.m00;
-    c.c11 = m.m11;
-    c.c01 = m.m01;
+    // the 2x2 algebra (a Cholesky factor with a cancelling pivot) always in fp64: six scalars
+    const Sym2 m = psd_project_2x2((double)p, (double)q, (double)r, (double)c.c00, (double)c.c01, (double)c.c11);
+    c.c00 = (S)m.m00;
+    c.c11 = (S)m.m11;
+    c.c01 = (S)m.m01;
   }
   return c;
 }

@@ -710,10 +710,14 @@ __global__ void k_emit_vslots(const int* __restrict__ tris, const int* __restric
 // The staging area of the diagonal / gradient products aliases the row tile (12.5 KB of shared
 // memory per warp); the measured limiter is the L1 data pipe (shared-memory wavefronts of staging,
 // tile writes and the engine's reads: 62 % busy), not HBM (49 %) or instruction issue (31 %).
+// C = the arithmetic type of the derivative code: double in every kernel of the hot path (reading A12; the
+// fp32 instantiation was measured -- it misses the 1e-4 gradient bar on config 3 and buys 14 % on K4 -- and
+// is not used); TT_HESS_EXACT instantiates it with second-order information (tt_exact.cuh).
+template <typename C>
 struct Entry {
-  double g0[18], g1[18];   // own triangle's 9 DOF first, partner's 9 after; vertices in RECORDED order (k, p, q)
-  ttg::Coefs cf;
-  double en;               // Eq. 2 energy if this is the canonical copy (side 0), else 0
+  C g0[18], g1[18];        // own triangle's 9 DOF first, partner's 9 after; vertices in RECORDED order (k, p, q)
+  ttg::Coefs<C> cf;
+  C en;                    // Eq. 2 energy if this is the canonical copy (side 0), else 0
   int po[3], pp[3];        // recorded order -> index 0..2 inside the own / partner triangle
 };
 
@@ -1097,36 +1101,37 @@ k_round_fill(const int* __restrict__ tris, const int* __restrict__ touched, cons
   }
 }
 
-template <typename T>
-__device__ __forceinline__ void load_pos18(const T* __restrict__ pos, const int (&ids)[6], double (&x)[18]) {
+template <typename T, typename C>
+__device__ __forceinline__ void load_pos18(const T* __restrict__ pos, const int (&ids)[6], C (&x)[18]) {
 #pragma unroll
   for (int v = 0; v < 6; ++v) {
     const T* p = pos + 3 * (int64_t)ids[v];
-    x[3 * v] = (double)__ldg(p);
-    x[3 * v + 1] = (double)__ldg(p + 1);
-    x[3 * v + 2] = (double)__ldg(p + 2);
+    x[3 * v] = (C)__ldg(p);
+    x[3 * v + 1] = (C)__ldg(p + 1);
+    x[3 * v + 2] = (C)__ldg(p + 2);
   }
 }
 
 // J by the straight-line code on gathered positions x = [a_k, a_p, a_q, b_k, b_p, b_q] (raw),
 // coefficients, energy; swaps halves so that "own" is first.
-template <bool PROJ = true>
-__device__ __forceinline__ void eval_core(const double (&x)[18], unsigned pay, double sigma, int hess_mode, Entry& E) {
+template <typename C, bool PROJ = true>
+__device__ __forceinline__ void eval_core(const C (&x)[18], unsigned pay, C sigma, int hess_mode, Entry<C>& E) {
+  using V = ttg::v3<C>;
   const bool side = (pay & 1u) != 0u;
   const unsigned ca = (pay >> 1) & 63u, cb = (pay >> 7) & 63u;
   int pa[3], pb[3];
   pa[0] = (int)(ca & 3u); pa[1] = (int)((ca >> 2) & 3u); pa[2] = 3 - pa[0] - pa[1];
   pb[0] = (int)(cb & 3u); pb[1] = (int)((cb >> 2) & 3u); pb[2] = 3 - pb[0] - pb[1];
   // local frame: translate by -a_k (kills the cancellation in D.E, keeps fp32 inputs well scaled)
-  const d3 o = ttg::mk(x[0], x[1], x[2]);
-  const d3 ak = ttg::mk(0.0, 0.0, 0.0);
-  const d3 ap = ttg::mk(x[3], x[4], x[5]) - o, aq = ttg::mk(x[6], x[7], x[8]) - o;
-  const d3 bk = ttg::mk(x[9], x[10], x[11]) - o, bp = ttg::mk(x[12], x[13], x[14]) - o, bq = ttg::mk(x[15], x[16], x[17]) - o;
-  double tc0, tc1;
-  ttg::pair_derivs_recorded(ak, ap, aq, bk, bp, bq, sigma, ca >> 4, cb >> 4, tc0, tc1, E.g0, E.g1);
-  E.cf = ttg::pair_coefs<PROJ>(tc0, tc1, E.g0, E.g1, hess_mode);
-  const double tt = tc0 * tc1;
-  E.en = side ? 0.0 : tt * tt;  // Eq. 2, counted once per pair
+  const V o = ttg::mk<C>(x[0], x[1], x[2]);
+  const V ak = ttg::mk<C>(C(0), C(0), C(0));
+  const V ap = ttg::mk<C>(x[3], x[4], x[5]) - o, aq = ttg::mk<C>(x[6], x[7], x[8]) - o;
+  const V bk = ttg::mk<C>(x[9], x[10], x[11]) - o, bp = ttg::mk<C>(x[12], x[13], x[14]) - o, bq = ttg::mk<C>(x[15], x[16], x[17]) - o;
+  C tc0, tc1;
+  ttg::pair_derivs_recorded<C>(ak, ap, aq, bk, bp, bq, sigma, ca >> 4, cb >> 4, tc0, tc1, E.g0, E.g1);
+  E.cf = ttg::pair_coefs<C, PROJ>(tc0, tc1, E.g0, E.g1, hess_mode);
+  const C tt = tc0 * tc1;
+  E.en = side ? C(0) : tt * tt;  // Eq. 2, counted once per pair
 #pragma unroll
   for (int m = 0; m < 3; ++m) {
     E.po[m] = side ? pb[m] : pa[m];
@@ -1135,8 +1140,8 @@ __device__ __forceinline__ void eval_core(const double (&x)[18], unsigned pay, d
   if (side) {
 #pragma unroll
     for (int i = 0; i < 9; ++i) {
-      const double t0 = E.g0[i]; E.g0[i] = E.g0[9 + i]; E.g0[9 + i] = t0;
-      const double t1 = E.g1[i]; E.g1[i] = E.g1[9 + i]; E.g1[9 + i] = t1;
+      const C t0 = E.g0[i]; E.g0[i] = E.g0[9 + i]; E.g0[9 + i] = t0;
+      const C t1 = E.g1[i]; E.g1[i] = E.g1[9 + i]; E.g1[9 + i] = t1;
     }
   }
 }
@@ -1144,8 +1149,9 @@ __device__ __forceinline__ void eval_core(const double (&x)[18], unsigned pay, d
 // Brings the own half of J back to the triangle's own vertex order (selects on the recorded
 // permutation: no shared-memory round trip, the L1 data pipe is the kernel's busiest unit), and the
 // partner's block ranks into recorded order.
-__device__ __forceinline__ void unpermute_own(Entry& E, int (&er)[3]) {
-  double t0[9], t1[9];
+template <typename C>
+__device__ __forceinline__ void unpermute_own(Entry<C>& E, int (&er)[3]) {
+  C t0[9], t1[9];
 #pragma unroll
   for (int i = 0; i < 9; ++i) {
     t0[i] = E.g0[i];
@@ -1163,6 +1169,34 @@ __device__ __forceinline__ void unpermute_own(Entry& E, int (&er)[3]) {
   const int e0 = er[0], e1 = er[1], e2 = er[2];
 #pragma unroll
   for (int r = 0; r < 3; ++r) er[r] = (E.pp[r] == 0) ? e0 : ((E.pp[r] == 1) ? e1 : e2);
+}
+
+// Brings the partner half of J into COLUMN order (ascending block rank) and sorts the ranks with it.  The
+// lanes of a warp then all store their lowest-ranked block with the same instruction, the next with the
+// next: with the recorded order each lane's instruction hit a different one of its three blocks (offsets
+// 0, 9 or 18 words apart) and every tile store took 5 shared-memory wavefronts instead of 2 (ncu, round 2).
+// Selects only: no shared-memory round trip.
+template <typename C>
+__device__ __forceinline__ void sort_partner_by_rank(Entry<C>& E, int (&er)[3]) {
+  const int o0 = (er[0] > er[1]) + (er[0] > er[2]);  // position of recorded vertex r among the three ranks
+  const int o1 = (er[1] > er[0]) + (er[1] > er[2]);
+  C t0[9], t1[9];
+#pragma unroll
+  for (int i = 0; i < 9; ++i) {
+    t0[i] = E.g0[9 + i];
+    t1[i] = E.g1[9 + i];
+  }
+  const int e0 = er[0], e1 = er[1], e2 = er[2];
+#pragma unroll
+  for (int n = 0; n < 3; ++n) {
+    const bool a = (o0 == n), b = (o1 == n);
+    er[n] = a ? e0 : (b ? e1 : e2);
+#pragma unroll
+    for (int j = 0; j < 3; ++j) {
+      E.g0[9 + 3 * n + j] = a ? t0[j] : (b ? t0[3 + j] : t0[6 + j]);
+      E.g1[9 + 3 * n + j] = a ? t1[j] : (b ? t1[3 + j] : t1[6 + j]);
+    }
+  }
 }
 
 __device__ __forceinline__ void bulk_s2g(void* gdst, const void* ssrc, uint32_t bytes) {
@@ -1203,11 +1237,16 @@ constexpr int STG_PASS = NSTG / 2;        // the 54 per-entry values are staged 
 constexpr int STG_STRIDE = STG_PASS;      // 27 doubles: odd, so lane = entry writes are conflict-free
 constexpr int LONG_STRIDE = 31;           // k_assemble_long: 27 + 3 staged values per entry, odd stride
 
+#ifdef TT_BANK_PLACE
+constexpr int BANK_SLACK = 128;
+#else
+constexpr int BANK_SLACK = 0;
+#endif
 template <typename T>
 struct TileCfg {
   static constexpr int RUN_UNIT = 27 * (int)sizeof(T);  // bytes one entry (or the diagonal) adds to a row run
-  static constexpr int TILE_BYTES = RUN_UNIT * (RND_MAX_ENT + RND_MAX_TRI) + 32 * RND_MAX_TRI;
-  static constexpr int STAGE_BYTES = 32 * STG_STRIDE * (int)sizeof(double);
+  static constexpr int TILE_BYTES = RUN_UNIT * (RND_MAX_ENT + RND_MAX_TRI) + (32 + BANK_SLACK) * RND_MAX_TRI;
+  static constexpr int STAGE_BYTES = 32 * STG_STRIDE * (int)sizeof(T);
   static constexpr int UNION_BYTES = TILE_BYTES > STAGE_BYTES ? TILE_BYTES : STAGE_BYTES;
 };
 
@@ -1290,7 +1329,7 @@ k_assemble_tile(const AsmParams<T> P) {
   constexpr int RUN_UNIT = TileCfg<T>::RUN_UNIT;
   const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
   TileWarpSmem<T>& S = reinterpret_cast<TileWarpSmem<T>*>(s_raw)[warp];
-  double* const stage = reinterpret_cast<double*>(S.tile);
+  T* const stage = reinterpret_cast<T*>(S.tile);
   const int64_t G = (int64_t)gridDim.x * TILE_WARPS;
   int64_t c = (int64_t)blockIdx.x * TILE_WARPS + warp;
   if (c >= P.n_chunks) return;
@@ -1304,7 +1343,7 @@ k_assemble_tile(const AsmParams<T> P) {
   RoundOps cur;
   load_round_ops(P, d_cur, lane, cur);
   int ids_nxt[6];
-  double x[18];
+  double x[18];  // J and the coefficients always in fp64 (reading A12; measured: fp32 J misses the 1e-4 bar on config 3)
   {
     int ids_cur[6];
     load_round_ids(P, d_cur, lane, ids_cur);
@@ -1325,13 +1364,13 @@ k_assemble_tile(const AsmParams<T> P) {
     if (lane < round_entries(d_nxt)) prefetch_pos_l2(P.pos, ids_nxt);
 
     // ---- lane = entry: J, coefficients ----
-    Entry E;
+    Entry<double> E;
 #pragma unroll
     for (int i = 0; i < 18; ++i) { E.g0[i] = 0.0; E.g1[i] = 0.0; }
-    E.cf = {0, 0, 0, 0, 0};
+    E.cf = {0.0, 0.0, 0.0, 0.0, 0.0};
     E.en = 0.0;
     int er[3] = {cur.er[0], cur.er[1], cur.er[2]};
-    if (valid) eval_core<PROJ>(x, cur.pay, P.sigma, P.hess_mode, E);
+    if (valid) eval_core<double, PROJ>(x, cur.pay, P.sigma, P.hess_mode, E);
     // ---- operands of round c + G, vertex ids of c + 2G, descriptor of c + 3G: requested after the
     //      register peak of the derivative code, consumed a round later ----
     RoundOps nxt;
@@ -1342,7 +1381,10 @@ k_assemble_tile(const AsmParams<T> P) {
     // the staging area aliases the row tile: the copy engine must have read the previous round's last row
     bulk_wait_read();
     __syncwarp();
-    if (valid) unpermute_own(E, er);
+    if (valid) {
+      unpermute_own(E, er);
+      sort_partner_by_rank(E, er);
+    }
 
     if (!is_long) {
       // lane = triangle: tile slots (16-byte slots, prefix sum over the round's triangles)
@@ -1350,7 +1392,7 @@ k_assemble_tile(const AsmParams<T> P) {
       const int run_bytes = RUN_UNIT * (cur.e1 - cur.e0 + (part_slot ? 0 : 1));
       int slot_off;
       {
-        int incl = (lane < ntri) ? (((run_bytes + 15) & ~15) + 16) : 0;
+        int incl = (lane < ntri) ? (((run_bytes + 15) & ~15) + 16 + BANK_SLACK) : 0;
         const int mine = incl;
 #pragma unroll
         for (int o = 1; o < RND_MAX_TRI; o <<= 1) {
@@ -1374,17 +1416,17 @@ k_assemble_tile(const AsmParams<T> P) {
 #pragma unroll
       for (int h = 0; h < 2; ++h) {
         if (valid) {
-          double* st = stage + lane * STG_STRIDE - h * STG_PASS;
+          T* st = stage + lane * STG_STRIDE - h * STG_PASS;
           int k = 0;
 #pragma unroll
           for (int r = 0; r < 9; ++r)
 #pragma unroll
             for (int q = r; q < 9; ++q, ++k)
-              if (k >= h * STG_PASS && k < (h + 1) * STG_PASS) st[k] = E.g0[r] * d0[q] + E.g1[r] * d1[q];
+              if (k >= h * STG_PASS && k < (h + 1) * STG_PASS) st[k] = (T)(E.g0[r] * d0[q] + E.g1[r] * d1[q]);
 #pragma unroll
           for (int i = 0; i < 9; ++i)
             if (NDIAG + i >= h * STG_PASS && NDIAG + i < (h + 1) * STG_PASS)
-              st[NDIAG + i] = E.cf.cg0 * E.g0[i] + E.cf.cg1 * E.g1[i];
+              st[NDIAG + i] = (T)(E.cf.cg0 * E.g0[i] + E.cf.cg1 * E.g1[i]);
         }
         __syncwarp();
         // per-triangle sums, lane = component, entries in ascending order (deterministic); two
@@ -1395,15 +1437,15 @@ k_assemble_tile(const AsmParams<T> P) {
           const int b1 = __shfl_sync(FULL, my_first, tt + 2);
           const int dA = a1 - a0, dB = b1 - a1, dn = max(dA, dB);
           if (lane < STG_PASS) {
-            const double* pA = stage + a0 * STG_STRIDE + lane;
-            const double* pB = stage + a1 * STG_STRIDE + lane;
+            const T* pA = stage + a0 * STG_STRIDE + lane;   // products in T, sums over a triangle's entries in fp64
+            const T* pB = stage + a1 * STG_STRIDE + lane;
             // the first RED_UNR entries of both triangles are loaded before any add (one shared-memory
             // latency per pair of triangles, not one per entry); longer triangles finish in a loop
             double vA[RED_UNR], vB[RED_UNR];
 #pragma unroll
             for (int j = 0; j < RED_UNR; ++j) {
-              vA[j] = (j < dA) ? pA[j * STG_STRIDE] : 0.0;
-              vB[j] = (j < dB) ? pB[j * STG_STRIDE] : 0.0;
+              vA[j] = (j < dA) ? (double)pA[j * STG_STRIDE] : 0.0;
+              vB[j] = (j < dB) ? (double)pB[j * STG_STRIDE] : 0.0;
             }
             double accA = vA[0], accB = vB[0];
 #pragma unroll
@@ -1413,8 +1455,8 @@ k_assemble_tile(const AsmParams<T> P) {
             }
 #pragma unroll 2
             for (int j = RED_UNR; j < dn; ++j) {
-              if (j < dA) accA += pA[j * STG_STRIDE];
-              if (j < dB) accB += pB[j * STG_STRIDE];
+              if (j < dA) accA += (double)pA[j * STG_STRIDE];
+              if (j < dB) accB += (double)pB[j * STG_STRIDE];
             }
             S.dsum[tt][h * STG_PASS + lane] = accA;
             if (dB > 0) S.dsum[tt + 1][h * STG_PASS + lane] = accB;
@@ -1442,7 +1484,15 @@ k_assemble_tile(const AsmParams<T> P) {
       for (int m = 0; m < 3; ++m) {
         const unsigned long long g =
             (unsigned long long)((cur.rb[m] >= 0) ? (P.vals + 9 * cur.rb[m]) : (P.tvals + 9 * (-cur.rb[m] - 1)));
+#ifdef TT_BANK_PLACE
+        // Bank placement: shift every run (16-byte steps, inside BANK_SLACK spare bytes) so that its first entry
+        // lands on bank 27 * (its first lane): the 32 lanes of the round then follow one arithmetic progression.
+        constexpr int BANKW = 128 / (int)sizeof(T), STEPW = 16 / (int)sizeof(T);
+        const int base_off = slot_off + (int)(g & 15ull);
+        const int my_off = base_off + ((((27 * (cur.e0 - e_lo)) - base_off / (int)sizeof(T)) & (BANKW - 1)) & ~(STEPW - 1)) * (int)sizeof(T);
+#else
         const int my_off = slot_off + (int)(g & 15ull);
+#endif
         // the tile is single-buffered: the copy engine must have read the previous row's runs
         if (m > 0) {
           bulk_wait_read();
@@ -1455,22 +1505,16 @@ k_assemble_tile(const AsmParams<T> P) {
         }
         __syncwarp();
         if (valid) {
-          double a[3], b[3];
-#pragma unroll
-          for (int i = 0; i < 3; ++i) {
-            a[i] = E.cf.c00 * E.g0[3 * m + i] + E.cf.c01 * E.g1[3 * m + i];
-            b[i] = E.cf.c01 * E.g0[3 * m + i] + E.cf.c11 * E.g1[3 * m + i];
-          }
-          T* run = reinterpret_cast<T*>(S.tile + S.run_off[my_ti]);
-          // The two outer products of a block run in the OUTPUT precision (fp32 variant: FFMA on the
-          // rounded J, 1e-7 relative per block against a 1e-3 tolerance; J, the coefficients and every
-          // sum over pairs stay fp64 -- reading A12).
+          // The staged diagonal / gradient products and the two outer products of a block run in the OUTPUT
+          // precision (fp32 variant: rounded J, 1e-7 relative per product against 1e-4 / 1e-3); J, the
+          // coefficients and every sum over pairs stay fp64 -- reading A12.
           T at[3], bt[3];
 #pragma unroll
           for (int i = 0; i < 3; ++i) {
-            at[i] = (T)a[i];
-            bt[i] = (T)b[i];
+            at[i] = (T)(E.cf.c00 * E.g0[3 * m + i] + E.cf.c01 * E.g1[3 * m + i]);
+            bt[i] = (T)(E.cf.c01 * E.g0[3 * m + i] + E.cf.c11 * E.g1[3 * m + i]);
           }
+          T* run = reinterpret_cast<T*>(S.tile + S.run_off[my_ti]);
 #pragma unroll
           for (int n = 0; n < 3; ++n) {
             T* blk = run + 9 * er[n];
@@ -1528,7 +1572,7 @@ k_assemble_tile(const AsmParams<T> P) {
       }
     }
     if (is_long && lane < round_entries(d_nxt)) load_pos18(P.pos, ids_nxt, x);
-    double e_acc = E.en;
+    double e_acc = (double)E.en;
 #pragma unroll
     for (int o = 16; o > 0; o >>= 1) e_acc += __shfl_down_sync(FULL, e_acc, o);
     if (lane == 0) P.chunk_energy[c] = e_acc;  // 0 for a long round: k_assemble_long overwrites it
@@ -1615,7 +1659,7 @@ k_assemble_long_tile(const AsmParams<T> P) {
         int er[3];
 #pragma unroll
         for (int n = 0; n < 3; ++n) er[n] = __ldg(P.erank + 3 * e + n);
-        Entry E;
+        Entry<double> E;
         double* const jc = S.jc + gi * JC_N * 32 + lane;
         if (!CACHE || m == 0) {
           int ids[6];
@@ -1730,7 +1774,7 @@ k_assemble_long_direct(const AsmParams<T> P) {
   for (int base = e_lo; base < e_hi; base += 32) {
     const int nvalid = min(32, e_hi - base);
     const bool valid = lane < nvalid;
-    Entry E;
+    Entry<double> E;
     int er[3] = {0, 0, 0};
     if (valid) {
       const int64_t e = (int64_t)base + lane;
@@ -1837,7 +1881,7 @@ k_entry_reduce(const AsmParams<T> P, const int* __restrict__ round_list, int64_t
       double x[18];
       load_pos18(P.pos, ids, x);
       const unsigned pay = (unsigned)__ldg(P.dvals + e);
-      Entry E;
+      Entry<double> E;
       eval_core(x, pay, P.sigma, P.hess_mode, E);
       e_acc += E.en;
       double u0 = E.cf.cg0, u1 = E.cf.cg1;  // MODE 1: Eq. 3
@@ -2049,7 +2093,7 @@ k_entry_pipe(const AsmParams<T> P) {
 #pragma unroll
     for (int k = 0; k < 9; ++k) v[k] = 0.0;
     double e_acc = 0.0;
-    Entry E;
+    Entry<double> E;
     if (valid) {
       double xf[18], x[18];
       read_round_gather(S.xp[buf], S.xo[buf], m_cur, lane, xf);

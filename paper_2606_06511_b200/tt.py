@@ -8,12 +8,13 @@ library or without a CUDA device raises.
 from __future__ import annotations
 
 import ctypes
+import os
 from pathlib import Path
 
 import torch
 
 _HERE = Path(__file__).resolve().parent
-LIB_PATH = _HERE / "libtt.so"
+LIB_PATH = Path(os.environ["TT_LIB_PATH"]) if os.environ.get("TT_LIB_PATH") else _HERE / "libtt.so"   # override: A/B builds
 
 TT_OK = 0
 TT_F64, TT_F32 = 0, 1
