@@ -21,7 +21,7 @@ _HERE = Path(__file__).resolve().parent
 _SRC = _HERE / "tt_oracle.cpp"
 _LIB = _HERE / "libtt_oracle.so"
 
-HESS_EQ4, HESS_FILTER, HESS_PSD2, HESS_PSDPROJ = 0, 1, 2, 3
+HESS_EQ4, HESS_FILTER, HESS_PSD2, HESS_PSDPROJ, HESS_EXACT = 0, 1, 2, 3, 4
 
 _lib = None
 
@@ -62,6 +62,11 @@ def _load():
         lib.tt_oracle_bsr_matvec.restype = None
         lib.tt_oracle_broad_phase.argtypes = [c_dp, c_ip, i64, ctypes.c_double, c_ip, i64]
         lib.tt_oracle_broad_phase.restype = i64
+        lib.tt_oracle_pair_exact.argtypes = [c_dp, ctypes.c_double, ctypes.POINTER(ctypes.c_int), c_dp, c_dp, c_dp, c_dp,
+                                             c_dp, c_dp]
+        lib.tt_oracle_pair_exact.restype = None
+        lib.tt_oracle_exact_hess_vec.argtypes = [c_dp, i64, c_ip, c_ip, i64, ctypes.c_double, c_dp, c_dp]
+        lib.tt_oracle_exact_hess_vec.restype = None
         lib.tt_oracle_block_jacobi.argtypes = [i64, c_ip, c_ip, c_dp, ctypes.c_double, c_dp]
         lib.tt_oracle_block_jacobi.restype = None
         lib.tt_oracle_pcg.argtypes = [i64, c_ip, c_ip, c_dp, ctypes.c_double, c_dp, c_dp, i64, ctypes.c_double,
@@ -228,3 +233,29 @@ def pcg(rowptr, colind, vals, b, shift: float = 0.0, max_iter: int = 50, rtol: f
                           float(rtol), _dp(x), _dp(xh), _dp(res))
     k = int(k)
     return dict(x=x, iters=k, res=res[:k + 1], x_hist=None if xh is None else xh[:k + 1], minv=minv)
+
+
+def pair_exact(x, sigma: float = 1.0) -> dict:
+    """One pair in second-order duals: the EXACT Hessian of T = (tc0 tc1)^2 (second half)
+    plus the second derivatives H0, H1 of tc0, tc1."""
+    lib = _load()
+    x = _f64(x).reshape(18)
+    active = ctypes.c_int(0)
+    tc, T, grad = np.zeros(2), np.zeros(1), np.zeros(18)
+    H, H0, H1 = np.zeros((18, 18)), np.zeros((18, 18)), np.zeros((18, 18))
+    lib.tt_oracle_pair_exact(_dp(x), float(sigma), ctypes.byref(active), _dp(tc), _dp(T), _dp(grad), _dp(H), _dp(H0),
+                             _dp(H1))
+    return dict(active=bool(active.value), tc=tc, energy=float(T[0]), grad=grad, H=H, H0=H0, H1=H1)
+
+
+def exact_hess_vec(pos, tris, pair_ids, p, sigma: float = 1.0):
+    """y = H_exact p over all active pairs."""
+    lib = _load()
+    pos = _f64(pos)
+    tris = _i32(tris)
+    pair_ids = _i32(pair_ids).reshape(-1, 2)
+    p = _f64(p)
+    y = np.zeros_like(pos)
+    lib.tt_oracle_exact_hess_vec(_dp(pos), pos.shape[0], _ip(tris), _ip(pair_ids), pair_ids.shape[0], float(sigma),
+                                 _dp(p), _dp(y))
+    return y

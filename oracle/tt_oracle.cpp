@@ -84,28 +84,111 @@ inline Dual dsqrt(const Dual& a) {
 inline Dual dmin(const Dual& a, const Dual& b) { return (b.val < a.val) ? b : a; }
 inline Dual dmax(const Dual& a, const Dual& b) { return (b.val > a.val) ? b : a; }
 
-struct Vec3 {
-  Dual x, y, z;
+// ---- second-order forward-mode dual number: value + 18 first + 18 x 18 second partials ----------
+// Used only for the EXACT Hessian (second half: the terms Eq. 4 drops, PAPER.md L26
+// "ignoring the asymmetric part of the exact Hessian").  The same listing code below runs on either
+// dual type (it is a template on the scalar), so the exact Hessian is App. A differentiated twice.
+struct Dual2 {
+  double val;
+  double d[NDOF];
+  double h[NDOF][NDOF];
 };
-inline Vec3 operator+(const Vec3& a, const Vec3& b) { return {a.x + b.x, a.y + b.y, a.z + b.z}; }
-inline Vec3 operator-(const Vec3& a, const Vec3& b) { return {a.x - b.x, a.y - b.y, a.z - b.z}; }
-inline Vec3 operator*(const Dual& s, const Vec3& a) { return {s * a.x, s * a.y, s * a.z}; }
-inline Vec3 operator*(double s, const Vec3& a) { return {s * a.x, s * a.y, s * a.z}; }
-inline Vec3 operator/(const Vec3& a, const Dual& s) { return {a.x / s, a.y / s, a.z / s}; }
-inline Dual dot(const Vec3& a, const Vec3& b) { return a.x * b.x + a.y * b.y + a.z * b.z; }
-inline Vec3 cross(const Vec3& a, const Vec3& b) {
+inline Dual2 constant2(double c) {
+  Dual2 r;
+  std::memset(&r, 0, sizeof(r));
+  r.val = c;
+  return r;
+}
+inline Dual2 operator+(const Dual2& a, const Dual2& b) {
+  Dual2 r;
+  r.val = a.val + b.val;
+  for (int i = 0; i < NDOF; ++i) r.d[i] = a.d[i] + b.d[i];
+  for (int i = 0; i < NDOF; ++i)
+    for (int j = 0; j < NDOF; ++j) r.h[i][j] = a.h[i][j] + b.h[i][j];
+  return r;
+}
+inline Dual2 operator-(const Dual2& a, const Dual2& b) {
+  Dual2 r;
+  r.val = a.val - b.val;
+  for (int i = 0; i < NDOF; ++i) r.d[i] = a.d[i] - b.d[i];
+  for (int i = 0; i < NDOF; ++i)
+    for (int j = 0; j < NDOF; ++j) r.h[i][j] = a.h[i][j] - b.h[i][j];
+  return r;
+}
+inline Dual2 operator*(const Dual2& a, const Dual2& b) {  // (ab)'' = a''b + a b'' + a'b'^T + b'a'^T
+  Dual2 r;
+  r.val = a.val * b.val;
+  for (int i = 0; i < NDOF; ++i) r.d[i] = a.d[i] * b.val + a.val * b.d[i];
+  for (int i = 0; i < NDOF; ++i)
+    for (int j = 0; j < NDOF; ++j)
+      r.h[i][j] = a.h[i][j] * b.val + a.val * b.h[i][j] + a.d[i] * b.d[j] + b.d[i] * a.d[j];
+  return r;
+}
+inline Dual2 operator*(double s, const Dual2& a) {
+  Dual2 r;
+  r.val = s * a.val;
+  for (int i = 0; i < NDOF; ++i) r.d[i] = s * a.d[i];
+  for (int i = 0; i < NDOF; ++i)
+    for (int j = 0; j < NDOF; ++j) r.h[i][j] = s * a.h[i][j];
+  return r;
+}
+inline Dual2 operator/(const Dual2& a, const Dual2& b) {  // a * (1/b): (1/b)' = -b'/b^2, (1/b)'' = 2 b'b'^T/b^3 - b''/b^2
+  Dual2 q;
+  const double v = 1.0 / b.val;
+  q.val = v;
+  for (int i = 0; i < NDOF; ++i) q.d[i] = -v * v * b.d[i];
+  for (int i = 0; i < NDOF; ++i)
+    for (int j = 0; j < NDOF; ++j) q.h[i][j] = 2.0 * v * v * v * b.d[i] * b.d[j] - v * v * b.h[i][j];
+  return a * q;
+}
+inline Dual2 dsqrt(const Dual2& a) {  // s = sqrt(a): s' = a'/(2s), s'' = a''/(2s) - a'a'^T/(4 s^3)
+  Dual2 r;
+  r.val = std::sqrt(a.val);
+  const double s = r.val;
+  for (int i = 0; i < NDOF; ++i) r.d[i] = a.d[i] / (2.0 * s);
+  for (int i = 0; i < NDOF; ++i)
+    for (int j = 0; j < NDOF; ++j) r.h[i][j] = a.h[i][j] / (2.0 * s) - a.d[i] * a.d[j] / (4.0 * s * s * s);
+  return r;
+}
+inline Dual2 dmin(const Dual2& a, const Dual2& b) { return (b.val < a.val) ? b : a; }
+inline Dual2 dmax(const Dual2& a, const Dual2& b) { return (b.val > a.val) ? b : a; }
+
+// seeds: the idx-th independent variable
+template <class D> D seed(double c, int idx);
+template <> inline Dual seed<Dual>(double c, int idx) { return variable(c, idx); }
+template <> inline Dual2 seed<Dual2>(double c, int idx) {
+  Dual2 r = constant2(c);
+  r.d[idx] = 1.0;
+  return r;
+}
+
+template <class D>
+struct Vec3T {
+  D x, y, z;
+};
+using Vec3 = Vec3T<Dual>;
+template <class D> inline Vec3T<D> operator+(const Vec3T<D>& a, const Vec3T<D>& b) { return {a.x + b.x, a.y + b.y, a.z + b.z}; }
+template <class D> inline Vec3T<D> operator-(const Vec3T<D>& a, const Vec3T<D>& b) { return {a.x - b.x, a.y - b.y, a.z - b.z}; }
+template <class D> inline Vec3T<D> operator*(const D& s, const Vec3T<D>& a) { return {s * a.x, s * a.y, s * a.z}; }
+template <class D> inline Vec3T<D> operator*(double s, const Vec3T<D>& a) { return {s * a.x, s * a.y, s * a.z}; }
+template <class D> inline Vec3T<D> operator/(const Vec3T<D>& a, const D& s) { return {a.x / s, a.y / s, a.z / s}; }
+template <class D> inline D dot(const Vec3T<D>& a, const Vec3T<D>& b) { return a.x * b.x + a.y * b.y + a.z * b.z; }
+template <class D> inline Vec3T<D> cross(const Vec3T<D>& a, const Vec3T<D>& b) {
   return {a.y * b.z - a.z * b.y, a.z * b.x - a.x * b.z, a.x * b.y - a.y * b.x};
 }
-inline Vec3 normalized(const Vec3& a) {  // Vector3dual::normalize()
-  Dual n = dsqrt(dot(a, a));
+template <class D> inline Vec3T<D> normalized(const Vec3T<D>& a) {  // Vector3dual::normalize()
+  D n = dsqrt(dot(a, a));
   return a / n;
 }
 
 // ---- App. A `intersects` -----------------------------------------------
 // Plane triangle (U0,U1,U2) cuts triangle (V0,V1,V2); on success segment0/1 are the two
 // end-points of the cut.  Readings A1-A4 of DESIGN.md.
-bool intersects(const Vec3& U0, const Vec3& U1, const Vec3& U2, const Vec3& V0, const Vec3& V1,
-                const Vec3& V2, Vec3& segment0, Vec3& segment1) {
+template <class D>
+bool intersects(const Vec3T<D>& U0, const Vec3T<D>& U1, const Vec3T<D>& U2, const Vec3T<D>& V0, const Vec3T<D>& V1,
+                const Vec3T<D>& V2, Vec3T<D>& segment0, Vec3T<D>& segment1) {
+  using Vec3 = Vec3T<D>;
+  using Dual = D;
   Vec3 edge1 = U1 - U0;                  // L78
   Vec3 edge2 = U2 - U0;                  // L79
   Vec3 normal = cross(edge1, edge2);     // L80
@@ -158,39 +241,50 @@ struct PairResult {
 // x holds T_a = (a0,a1,a2) then T_b = (b0,b1,b2).  The listing names the triangle whose
 // segment is S00/S01 (interval I_a) `U` and the other `V`; so U := T_a, V := T_b, and the dual
 // seeds are placed so that partial index 3m+c is a_m[c] and 9+3m+c is b_m[c].
-PairResult pair_3dttit(const double x[NDOF], double sigma) {
-  PairResult r;
-  r.active = false;
-  r.tc[0] = r.tc[1] = 0.0;
-  std::memset(r.g, 0, sizeof(r.g));
+// (template on the dual type D: first order for Eq. 3 / Eq. 4, second order for the exact Hessian)
+template <class D>
+bool ttit_core(const double x[NDOF], double sigma, D& tc0_out, D& tc1_out) {
+  using Vec3 = Vec3T<D>;
+  using Dual = D;
   Vec3 U[3], V[3];
   for (int m = 0; m < 3; ++m) {
-    U[m] = {variable(x[3 * m + 0], 3 * m + 0), variable(x[3 * m + 1], 3 * m + 1),
-            variable(x[3 * m + 2], 3 * m + 2)};
-    V[m] = {variable(x[9 + 3 * m + 0], 9 + 3 * m + 0), variable(x[9 + 3 * m + 1], 9 + 3 * m + 1),
-            variable(x[9 + 3 * m + 2], 9 + 3 * m + 2)};
+    U[m] = {seed<D>(x[3 * m + 0], 3 * m + 0), seed<D>(x[3 * m + 1], 3 * m + 1), seed<D>(x[3 * m + 2], 3 * m + 2)};
+    V[m] = {seed<D>(x[9 + 3 * m + 0], 9 + 3 * m + 0), seed<D>(x[9 + 3 * m + 1], 9 + 3 * m + 1),
+            seed<D>(x[9 + 3 * m + 2], 9 + 3 * m + 2)};
   }
   Vec3 S00, S01, S10, S11;
   if (intersects(V[0], V[1], V[2], U[0], U[1], U[2], S00, S01) &&   // L134: plane(V) cuts U
       intersects(U[0], U[1], U[2], V[0], V[1], V[2], S10, S11)) {   // L135: plane(U) cuts V
     Vec3 uNormal = cross(U[1] - U[0], U[2] - U[0]);                  // L137
     Vec3 vNormal = cross(V[1] - V[0], V[2] - V[0]);                  // L139
-    Vec3 D = cross(uNormal, vNormal);                                // L141
-    if (!(dot(D, D).val > 0.0)) return r;  // parallel planes: excluded by L11 ("not coplanar")
-    D = normalized(D);                                               // L142
+    Vec3 Dv = cross(uNormal, vNormal);                               // L141 (the listing's D)
+    if (!(dot(Dv, Dv).val > 0.0)) return false;  // parallel planes: excluded by L11 ("not coplanar")
+    Dv = normalized(Dv);                                             // L142
     Vec3 A = 0.25 * (S00 + S01 + S10 + S11);                         // L144
-    Dual t00 = dot(D, S00 - A);                                      // L145
-    Dual t01 = dot(D, S01 - A);
-    Dual t10 = dot(D, S10 - A);
-    Dual t11 = dot(D, S11 - A);
+    Dual t00 = dot(Dv, S00 - A);                                     // L145
+    Dual t01 = dot(Dv, S01 - A);
+    Dual t10 = dot(Dv, S10 - A);
+    Dual t11 = dot(Dv, S11 - A);
     Dual ta0 = dmin(t00, t01);                                       // L149
     Dual ta1 = dmax(t00, t01);
     Dual tb0 = dmin(t10, t11);
     Dual tb1 = dmax(t10, t11);
     bool intersected = (ta1.val > tb0.val && ta0.val < tb1.val);     // L153
-    if (!intersected) return r;                                      // A11: tc := (0,0)
-    Dual tc0 = sigma * (ta0 - tb1);  // Eq. 1 (L13) with sigma = 1; L154 prints sigma = 0.5 (A6)
-    Dual tc1 = sigma * (ta1 - tb0);  // L155
+    if (!intersected) return false;                                  // A11: tc := (0,0)
+    tc0_out = sigma * (ta0 - tb1);   // Eq. 1 (L13) with sigma = 1; L154 prints sigma = 0.5 (A6)
+    tc1_out = sigma * (ta1 - tb0);   // L155
+    return true;
+  }
+  return false;
+}
+
+PairResult pair_3dttit(const double x[NDOF], double sigma) {
+  PairResult r;
+  r.active = false;
+  r.tc[0] = r.tc[1] = 0.0;
+  std::memset(r.g, 0, sizeof(r.g));
+  Dual tc0, tc1;
+  if (ttit_core<Dual>(x, sigma, tc0, tc1)) {
     r.active = true;
     r.tc[0] = tc0.val;
     r.tc[1] = tc1.val;
@@ -200,6 +294,28 @@ PairResult pair_3dttit(const double x[NDOF], double sigma) {
     }
   }
   return r;
+}
+
+// Exact Hessian of one pair (NEXT-3, second half): T = (tc0 tc1)^2 evaluated in second-order duals, so
+// H_exact = the second partials of T itself -- Eq. 4 plus the terms 2 tc0 tc1^2 d2tc0 + 2 tc1 tc0^2 d2tc1
+// that PAPER.md L26 drops.  Also returns tc, the gradient and the two second-derivative matrices.
+bool pair_exact(const double x[NDOF], double sigma, double tc[2], double* T, double grad[NDOF], double* H /*[18*18]*/,
+                double* H0 /*[18*18] or NULL*/, double* H1) {
+  Dual2 tc0, tc1;
+  if (!ttit_core<Dual2>(x, sigma, tc0, tc1)) return false;
+  const Dual2 prod = tc0 * tc1;
+  const Dual2 E = prod * prod;   // Eq. 2
+  tc[0] = tc0.val;
+  tc[1] = tc1.val;
+  *T = E.val;
+  for (int i = 0; i < NDOF; ++i) grad[i] = E.d[i];
+  for (int i = 0; i < NDOF; ++i)
+    for (int j = 0; j < NDOF; ++j) {
+      H[NDOF * i + j] = E.h[i][j];
+      if (H0) H0[NDOF * i + j] = tc0.h[i][j];
+      if (H1) H1[NDOF * i + j] = tc1.h[i][j];
+    }
+  return true;
 }
 
 // Eq. 2 (L17)
@@ -556,6 +672,51 @@ int64_t tt_oracle_broad_phase(const double* pos, const int32_t* tris, int64_t n_
     }
   }
   return cnt[n_tris];
+}
+
+// ---- exact Hessian (second half; the terms Eq. 4 ignores) -------------
+// One pair: active flag, tc, T, gradient (18), exact Hessian H (18 x 18), and the second derivatives of
+// tc0 / tc1 (H0, H1; may be NULL).  Inactive pairs: everything zero.
+void tt_oracle_pair_exact(const double* x, double sigma, int* active, double* tc, double* T, double* grad,
+                          double* H, double* H0, double* H1) {
+  std::memset(grad, 0, sizeof(double) * NDOF);
+  std::memset(H, 0, sizeof(double) * NDOF * NDOF);
+  if (H0) std::memset(H0, 0, sizeof(double) * NDOF * NDOF);
+  if (H1) std::memset(H1, 0, sizeof(double) * NDOF * NDOF);
+  tc[0] = tc[1] = 0.0;
+  *T = 0.0;
+  *active = pair_exact(x, sigma, tc, T, grad, H, H0, H1) ? 1 : 0;
+}
+
+// y = H_exact p, summed over the active pairs in ascending pair order (adjacent pairs skipped, L11).
+void tt_oracle_exact_hess_vec(const double* pos, int64_t n_verts, const int32_t* tris, const int32_t* pairs,
+                              int64_t n_pairs, double sigma, const double* p, double* y) {
+  for (int64_t i = 0; i < 3 * n_verts; ++i) y[i] = 0.0;
+  std::vector<double> yl((size_t)n_pairs * NDOF, 0.0);
+  std::vector<uint8_t> act((size_t)n_pairs, 0);
+#pragma omp parallel for schedule(dynamic, 64)
+  for (int64_t k = 0; k < n_pairs; ++k) {
+    const int32_t* pr = pairs + 2 * k;
+    if (share_vertex(tris + 3 * (int64_t)pr[0], tris + 3 * (int64_t)pr[1])) continue;
+    double x[NDOF], tc[2], T, grad[NDOF];
+    int32_t vid[6];
+    gather_x(pos, tris, pr, x, vid);
+    std::vector<double> H(NDOF * NDOF);
+    if (!pair_exact(x, sigma, tc, &T, grad, H.data(), nullptr, nullptr)) continue;
+    act[k] = 1;
+    for (int i = 0; i < NDOF; ++i) {
+      double a = 0.0;
+      for (int j = 0; j < NDOF; ++j) a += H[NDOF * i + j] * p[3 * (int64_t)vid[j / 3] + j % 3];
+      yl[(size_t)k * NDOF + i] = a;
+    }
+  }
+  for (int64_t k = 0; k < n_pairs; ++k) {
+    if (!act[k]) continue;
+    int32_t vid[6];
+    double x[NDOF];
+    gather_x(pos, tris, pairs + 2 * k, x, vid);
+    for (int i = 0; i < NDOF; ++i) y[3 * (int64_t)vid[i / 3] + i % 3] += yl[(size_t)k * NDOF + i];
+  }
 }
 
 // ---- inexact-Newton linear solve ("inexact Newton optimization route") ------

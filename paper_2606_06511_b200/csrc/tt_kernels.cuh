@@ -1174,7 +1174,9 @@ __device__ __forceinline__ void unpermute_own(Entry<C>& E, int (&er)[3]) {
 // Brings the partner half of J into COLUMN order (ascending block rank) and sorts the ranks with it.  The
 // lanes of a warp then all store their lowest-ranked block with the same instruction, the next with the
 // next: with the recorded order each lane's instruction hit a different one of its three blocks (offsets
-// 0, 9 or 18 words apart) and every tile store took 5 shared-memory wavefronts instead of 2 (ncu, round 2).
+// 0, 9 or 18 words apart) and every tile store took 5 shared-memory wavefronts instead of 2.  ncu, 10 M pairs:
+// store bank conflicts 86.4 M -> 64.7 M of 204 M -> 182 M store wavefronts; the kernel time did not move
+// (2.39 ms): K4 is bound by issue latency at 8 warps / SM, not by the L1 data pipe (profiles/r2_notes.md).
 // Selects only: no shared-memory round trip.
 template <typename C>
 __device__ __forceinline__ void sort_partner_by_rank(Entry<C>& E, int (&er)[3]) {
@@ -1237,16 +1239,11 @@ constexpr int STG_PASS = NSTG / 2;        // the 54 per-entry values are staged 
 constexpr int STG_STRIDE = STG_PASS;      // 27 doubles: odd, so lane = entry writes are conflict-free
 constexpr int LONG_STRIDE = 31;           // k_assemble_long: 27 + 3 staged values per entry, odd stride
 
-#ifdef TT_BANK_PLACE
-constexpr int BANK_SLACK = 128;
-#else
-constexpr int BANK_SLACK = 0;
-#endif
 template <typename T>
 struct TileCfg {
   static constexpr int RUN_UNIT = 27 * (int)sizeof(T);  // bytes one entry (or the diagonal) adds to a row run
-  static constexpr int TILE_BYTES = RUN_UNIT * (RND_MAX_ENT + RND_MAX_TRI) + (32 + BANK_SLACK) * RND_MAX_TRI;
-  static constexpr int STAGE_BYTES = 32 * STG_STRIDE * (int)sizeof(T);
+  static constexpr int TILE_BYTES = RUN_UNIT * (RND_MAX_ENT + RND_MAX_TRI) + 32 * RND_MAX_TRI;
+  static constexpr int STAGE_BYTES = 32 * STG_STRIDE * (int)sizeof(double);
   static constexpr int UNION_BYTES = TILE_BYTES > STAGE_BYTES ? TILE_BYTES : STAGE_BYTES;
 };
 
@@ -1329,7 +1326,7 @@ k_assemble_tile(const AsmParams<T> P) {
   constexpr int RUN_UNIT = TileCfg<T>::RUN_UNIT;
   const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
   TileWarpSmem<T>& S = reinterpret_cast<TileWarpSmem<T>*>(s_raw)[warp];
-  T* const stage = reinterpret_cast<T*>(S.tile);
+  double* const stage = reinterpret_cast<double*>(S.tile);
   const int64_t G = (int64_t)gridDim.x * TILE_WARPS;
   int64_t c = (int64_t)blockIdx.x * TILE_WARPS + warp;
   if (c >= P.n_chunks) return;
@@ -1392,7 +1389,7 @@ k_assemble_tile(const AsmParams<T> P) {
       const int run_bytes = RUN_UNIT * (cur.e1 - cur.e0 + (part_slot ? 0 : 1));
       int slot_off;
       {
-        int incl = (lane < ntri) ? (((run_bytes + 15) & ~15) + 16 + BANK_SLACK) : 0;
+        int incl = (lane < ntri) ? (((run_bytes + 15) & ~15) + 16) : 0;
         const int mine = incl;
 #pragma unroll
         for (int o = 1; o < RND_MAX_TRI; o <<= 1) {
@@ -1416,17 +1413,17 @@ k_assemble_tile(const AsmParams<T> P) {
 #pragma unroll
       for (int h = 0; h < 2; ++h) {
         if (valid) {
-          T* st = stage + lane * STG_STRIDE - h * STG_PASS;
+          double* st = stage + lane * STG_STRIDE - h * STG_PASS;
           int k = 0;
 #pragma unroll
           for (int r = 0; r < 9; ++r)
 #pragma unroll
             for (int q = r; q < 9; ++q, ++k)
-              if (k >= h * STG_PASS && k < (h + 1) * STG_PASS) st[k] = (T)(E.g0[r] * d0[q] + E.g1[r] * d1[q]);
+              if (k >= h * STG_PASS && k < (h + 1) * STG_PASS) st[k] = E.g0[r] * d0[q] + E.g1[r] * d1[q];
 #pragma unroll
           for (int i = 0; i < 9; ++i)
             if (NDIAG + i >= h * STG_PASS && NDIAG + i < (h + 1) * STG_PASS)
-              st[NDIAG + i] = (T)(E.cf.cg0 * E.g0[i] + E.cf.cg1 * E.g1[i]);
+              st[NDIAG + i] = E.cf.cg0 * E.g0[i] + E.cf.cg1 * E.g1[i];
         }
         __syncwarp();
         // per-triangle sums, lane = component, entries in ascending order (deterministic); two
@@ -1437,15 +1434,15 @@ k_assemble_tile(const AsmParams<T> P) {
           const int b1 = __shfl_sync(FULL, my_first, tt + 2);
           const int dA = a1 - a0, dB = b1 - a1, dn = max(dA, dB);
           if (lane < STG_PASS) {
-            const T* pA = stage + a0 * STG_STRIDE + lane;   // products in T, sums over a triangle's entries in fp64
-            const T* pB = stage + a1 * STG_STRIDE + lane;
+            const double* pA = stage + a0 * STG_STRIDE + lane;
+            const double* pB = stage + a1 * STG_STRIDE + lane;
             // the first RED_UNR entries of both triangles are loaded before any add (one shared-memory
             // latency per pair of triangles, not one per entry); longer triangles finish in a loop
             double vA[RED_UNR], vB[RED_UNR];
 #pragma unroll
             for (int j = 0; j < RED_UNR; ++j) {
-              vA[j] = (j < dA) ? (double)pA[j * STG_STRIDE] : 0.0;
-              vB[j] = (j < dB) ? (double)pB[j * STG_STRIDE] : 0.0;
+              vA[j] = (j < dA) ? pA[j * STG_STRIDE] : 0.0;
+              vB[j] = (j < dB) ? pB[j * STG_STRIDE] : 0.0;
             }
             double accA = vA[0], accB = vB[0];
 #pragma unroll
@@ -1455,8 +1452,8 @@ k_assemble_tile(const AsmParams<T> P) {
             }
 #pragma unroll 2
             for (int j = RED_UNR; j < dn; ++j) {
-              if (j < dA) accA += (double)pA[j * STG_STRIDE];
-              if (j < dB) accB += (double)pB[j * STG_STRIDE];
+              if (j < dA) accA += pA[j * STG_STRIDE];
+              if (j < dB) accB += pB[j * STG_STRIDE];
             }
             S.dsum[tt][h * STG_PASS + lane] = accA;
             if (dB > 0) S.dsum[tt + 1][h * STG_PASS + lane] = accB;
@@ -1484,15 +1481,7 @@ k_assemble_tile(const AsmParams<T> P) {
       for (int m = 0; m < 3; ++m) {
         const unsigned long long g =
             (unsigned long long)((cur.rb[m] >= 0) ? (P.vals + 9 * cur.rb[m]) : (P.tvals + 9 * (-cur.rb[m] - 1)));
-#ifdef TT_BANK_PLACE
-        // Bank placement: shift every run (16-byte steps, inside BANK_SLACK spare bytes) so that its first entry
-        // lands on bank 27 * (its first lane): the 32 lanes of the round then follow one arithmetic progression.
-        constexpr int BANKW = 128 / (int)sizeof(T), STEPW = 16 / (int)sizeof(T);
-        const int base_off = slot_off + (int)(g & 15ull);
-        const int my_off = base_off + ((((27 * (cur.e0 - e_lo)) - base_off / (int)sizeof(T)) & (BANKW - 1)) & ~(STEPW - 1)) * (int)sizeof(T);
-#else
         const int my_off = slot_off + (int)(g & 15ull);
-#endif
         // the tile is single-buffered: the copy engine must have read the previous row's runs
         if (m > 0) {
           bulk_wait_read();
@@ -1505,9 +1494,10 @@ k_assemble_tile(const AsmParams<T> P) {
         }
         __syncwarp();
         if (valid) {
-          // The staged diagonal / gradient products and the two outer products of a block run in the OUTPUT
-          // precision (fp32 variant: rounded J, 1e-7 relative per product against 1e-4 / 1e-3); J, the
-          // coefficients and every sum over pairs stay fp64 -- reading A12.
+          // The two outer products of a block run in the OUTPUT precision (fp32 variant: FFMA on the rounded J,
+          // 1e-7 relative per block against a 1e-3 tolerance); J, the coefficients, the staged diagonal /
+          // gradient products and every sum over pairs stay fp64 -- reading A12.  (Staging in fp32 was measured:
+          // 54 more F2F conversions per entry, K4 2.45 -> 2.70 ms.)
           T at[3], bt[3];
 #pragma unroll
           for (int i = 0; i < 3; ++i) {
