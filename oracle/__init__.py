@@ -67,6 +67,8 @@ def _load():
         lib.tt_oracle_pair_exact.restype = None
         lib.tt_oracle_exact_hess_vec.argtypes = [c_dp, i64, c_ip, c_ip, i64, ctypes.c_double, c_dp, c_dp]
         lib.tt_oracle_exact_hess_vec.restype = None
+        lib.tt_oracle_assemble_exact.argtypes = [c_dp, i64, c_ip, c_ip, i64, c_bp, ctypes.c_double, c_ip, c_ip, c_dp]
+        lib.tt_oracle_assemble_exact.restype = None
         lib.tt_oracle_block_jacobi.argtypes = [i64, c_ip, c_ip, c_dp, ctypes.c_double, c_dp]
         lib.tt_oracle_block_jacobi.restype = None
         lib.tt_oracle_pcg.argtypes = [i64, c_ip, c_ip, c_dp, ctypes.c_double, c_dp, c_dp, i64, ctypes.c_double,
@@ -156,7 +158,11 @@ def assemble(pos, tris, pair_ids, sigma: float = 1.0, hess_mode: int = HESS_FILT
                                   _ip(colind))
         vals = np.zeros((max(int(nnzb), 1), 3, 3))
         lib.tt_oracle_assemble(nV, _ip(tris), _ip(pair_ids), P, _bp(r["active"]), _dp(r["tc"]),
-                               _dp(r["J"]), int(hess_mode), _ip(rowptr), _ip(colind), _dp(grad), _dp(vals))
+                               _dp(r["J"]), HESS_EQ4 if hess_mode == HESS_EXACT else int(hess_mode), _ip(rowptr), _ip(colind),
+                               _dp(grad), _dp(vals))
+        if hess_mode == HESS_EXACT:   # same pattern, same gradient; the values from second-order duals
+            lib.tt_oracle_assemble_exact(_dp(pos), nV, _ip(tris), _ip(pair_ids), P, _bp(r["active"]), float(sigma),
+                                         _ip(rowptr), _ip(colind), _dp(vals))
         out.update(rowptr=rowptr, colind=colind[:nnzb], vals=vals[:nnzb], nnzb=int(nnzb))
     else:
         lib.tt_oracle_assemble(nV, _ip(tris), _ip(pair_ids), P, _bp(r["active"]), _dp(r["tc"]),

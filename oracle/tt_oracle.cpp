@@ -719,6 +719,32 @@ void tt_oracle_exact_hess_vec(const double* pos, int64_t n_verts, const int32_t*
   }
 }
 
+// BSR values of the EXACT Hessian: vals[nnzb,3,3] accumulated in ASCENDING PAIR ORDER from pair_exact's 18 x 18
+// matrices, on the pattern tt_oracle_bsr_pattern built for the same active set (the pattern does not depend on
+// the Hessian variant: every active pair fills its 6 x 6 vertex blocks).
+void tt_oracle_assemble_exact(const double* pos, int64_t n_verts, const int32_t* tris, const int32_t* pairs,
+                              int64_t n_pairs, const uint8_t* active, double sigma, const int32_t* rowptr,
+                              const int32_t* colind, double* vals) {
+  std::memset(vals, 0, sizeof(double) * 9 * (size_t)rowptr[n_verts]);
+  std::vector<double> H(NDOF * NDOF);
+  for (int64_t k = 0; k < n_pairs; ++k) {
+    if (!active[k]) continue;
+    double x[NDOF], tc[2], T, grad[NDOF];
+    int32_t vid[6];
+    gather_x(pos, tris, pairs + 2 * k, x, vid);
+    if (!pair_exact(x, sigma, tc, &T, grad, H.data(), nullptr, nullptr)) continue;
+    for (int p = 0; p < 6; ++p)
+      for (int q = 0; q < 6; ++q) {
+        const int32_t* lo = colind + rowptr[vid[p]];
+        const int32_t* hi = colind + rowptr[vid[p] + 1];
+        const int32_t* it = std::lower_bound(lo, hi, vid[q]);
+        double* blk = vals + 9 * (int64_t)(it - colind);
+        for (int a = 0; a < 3; ++a)
+          for (int b = 0; b < 3; ++b) blk[3 * a + b] += H[(3 * p + a) * NDOF + 3 * q + b];
+      }
+  }
+}
+
 // ---- inexact-Newton linear solve ("inexact Newton optimization route") ------
 // The paper names the route and gives no detail, so the operations are their textbook definitions:
 //   * block-Jacobi preconditioner: the inverse of every 3x3 diagonal block of (H + shift I)

@@ -100,3 +100,40 @@ def test_exact_hess_vec_sums_the_pairs(oracle_mod):
     g = oracle_mod.assemble(pb.pos, pb.tris, pb.pairs, 1.0, 0, want_hess=False)["grad"]
     yx = oracle_mod.exact_hess_vec(pb.pos, pb.tris, pb.pairs, pb.pos)
     assert np.linalg.norm(yx - 3 * g) <= 1e-9 * np.linalg.norm(3 * g)
+
+
+def test_exact_assembly_against_dense(oracle_mod):
+    """assemble(hess_mode=HESS_EXACT): the BSR equals a dense 576 x 576 accumulation of pair_exact's matrices written in
+    the test (shared-vertex variant included), the pattern is the Eq. 4 pattern, BSR.p == exact_hess_vec(p), and Euler's
+    identity H x = 3 grad holds for the assembled matrix."""
+    from paper_2606_06511_b200 import inputs
+    for pb in (inputs.config0_soup(), inputs.config0_soup(n_tris=48, pool=40, seed=5)):
+        nV = pb.pos.shape[0]
+        r = oracle_mod.assemble(pb.pos, pb.tris, pb.pairs, 1.0, oracle_mod.HESS_EXACT)
+        r0 = oracle_mod.assemble(pb.pos, pb.tris, pb.pairs, 1.0, oracle_mod.HESS_EQ4)
+        assert (r["rowptr"] == r0["rowptr"]).all() and (r["colind"] == r0["colind"]).all()
+        np.testing.assert_array_equal(r["grad"], r0["grad"])
+        D = np.zeros((3 * nV, 3 * nV))
+        for pr in pb.pairs:
+            vid = np.concatenate([pb.tris[pr[0]], pb.tris[pr[1]]])
+            if len(set(vid.tolist())) < 6:
+                continue
+            e = oracle_mod.pair_exact(pb.pos[vid].ravel())
+            if e["active"]:
+                idx = (3 * vid[:, None] + np.arange(3)[None, :]).ravel()
+                D[np.ix_(idx, idx)] += e["H"]
+        B = np.zeros_like(D)
+        for v in range(nV):
+            for k in range(r["rowptr"][v], r["rowptr"][v + 1]):
+                c = r["colind"][k]
+                B[3 * v:3 * v + 3, 3 * c:3 * c + 3] = r["vals"][k]
+        assert np.abs(B - D).max() <= 1e-12 * np.abs(D).max()
+        assert np.abs(B - B.T).max() <= 1e-11 * np.abs(B).max()
+        p = np.random.default_rng(6).normal(size=pb.pos.shape)
+        y = oracle_mod.bsr_matvec(r["rowptr"], r["colind"], r["vals"], p)
+        ye = oracle_mod.exact_hess_vec(pb.pos, pb.tris, pb.pairs, p)
+        assert np.linalg.norm(y - ye) <= 1e-12 * np.linalg.norm(ye)
+        yx = oracle_mod.bsr_matvec(r["rowptr"], r["colind"], r["vals"], pb.pos)
+        assert np.linalg.norm(yx - 3 * r["grad"]) <= 1e-9 * np.linalg.norm(3 * r["grad"])
+        # the exact matrix really differs from Eq. 4 (the dropped terms are not small)
+        assert np.linalg.norm(r["vals"] - r0["vals"]) > 1e-2 * np.linalg.norm(r0["vals"])
