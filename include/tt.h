@@ -33,7 +33,8 @@
  *     not only the upper triangle).
  *   - All work is enqueued on `stream` (a cudaStream_t passed as void*, NULL = default stream).
  *     tt_energy, tt_energy_grad_hess and tt_hess_vec are asynchronous; tt_hess_symbolic blocks
- *     until the sizes it hands to the host are known (three host round trips on `stream`; its last
+ *     until the sizes it hands to the host are known (one host round trip on `stream`, a second one when
+ *     some vertex is shared by several touched triangles; its last
  *     kernels may still be running on return, later calls on the same stream are ordered after
  *     them); the *_host call synchronises the stream before returning.
  *   - Outputs are OVERWRITTEN, never accumulated into: grad / y / vals are fully defined on
@@ -70,8 +71,13 @@ typedef enum { TT_F64 = 0, TT_F32 = 1 } tt_dtype;
  *   TT_HESS_FILTER third part kept iff L47's quantity 8 t_c^0 t_c^1 (g0.g1) >= 0   (default)
  *   TT_HESS_PSD2   first two parts only (always positive semi-definite)
  *   TT_HESS_PSDPROJ the projection of Eq. 4's per-pair matrix onto the positive semi-definite cone
- *                  (its negative eigenvalue removed): the closest PSD matrix to the pair's Eq. 4     */
-typedef enum { TT_HESS_EQ4 = 0, TT_HESS_FILTER = 1, TT_HESS_PSD2 = 2, TT_HESS_PSDPROJ = 3 } tt_hess_mode;
+ *                  (its negative eigenvalue removed): the closest PSD matrix to the pair's Eq. 4
+ *   TT_HESS_EXACT  the exact Hessian of T (Eq. 4 "ignores" part of it): Eq. 4, all three parts, plus
+ *                  2 t_c^0 (t_c^1)^2 d2 t_c^0 + 2 t_c^1 (t_c^0)^2 d2 t_c^1 -- the second derivatives of the end-points.
+ *                  Same BSR pattern; symmetric, in general indefinite.  A variant for Newton's method proper and for
+ *                  checking Eq. 4 against it: its kernels are plain (about 9 gradient evaluations per directed
+ *                  entry for the assembly, one for H p), not tuned like the Eq. 4 path.                       */
+typedef enum { TT_HESS_EQ4 = 0, TT_HESS_FILTER = 1, TT_HESS_PSD2 = 2, TT_HESS_PSDPROJ = 3, TT_HESS_EXACT = 4 } tt_hess_mode;
 
 typedef struct {
   int32_t dtype;      /* tt_dtype                                                                   */

@@ -170,16 +170,23 @@ __device__ __forceinline__ unsigned pair_config(const PairGeom& g) {
 template <typename S>
 struct EndPoint {
   S t;                            // D . E
+  v3<S> E;                        // the end-point itself (used by the exact Hessian only)
   v3<S> ownk, owne, yk, yp, yq;   // blocks of s D^T dE
 };
+// tau of an end-point that IS a vertex (zmask == 0, App. A): the vertex does not slide along its edge, so
+// tau is the constant 1 -- which is what d_k / (d_k - 0) evaluates to; types that carry derivatives overload this
+// to drop tau's (tt_exact.cuh).
+__device__ __forceinline__ double vertex_tau(double tau, double) { return tau; }
+__device__ __forceinline__ float vertex_tau(float tau, float) { return tau; }
 template <typename S>
 __device__ __forceinline__ EndPoint<S> end_point(S s, const v3<S> Dh, const v3<S> xk, const v3<S> ex, S dk,
                                                  S de, S zmask, const v3<S> yk, const v3<S> eyp,
                                                  const v3<S> eyq, const v3<S> nY) {
   EndPoint<S> r;
   const S inv = S(1) / (dk - de);  // opposite signs: |dk - de| = |dk| + |de|, no cancellation
-  const S tau = dk * inv;
+  const S tau = vertex_tau(dk * inv, zmask);
   const v3<S> E = axpy(tau, ex, xk);
+  r.E = E;
   r.t = dot(Dh, E);
   const S w = s * zmask * dot(Dh, ex) * inv;  // s c / den
   const S wn = w * inv;                       // s c / den^2
@@ -197,18 +204,26 @@ __device__ __forceinline__ EndPoint<S> end_point(S s, const v3<S> Dh, const v3<S
 //   x = [a_k, a_p, a_q, b_k, b_p, b_q].  The line direction is taken from the PERMUTED normals, so
 //   (tc0, tc1, g0, g1) may come out as (-tc0, -tc1, -g0, -g1): Eq. 2-4 and L47's third quantity are
 //   even in that sign (every term pairs two of them), so energy, gradient and Hessian are unchanged.
+// What the exact Hessian (tt_exact.cuh) needs beyond g0, g1: the two interval differences as VECTORS (c0 = P_a - Q_b,
+// c1 = Q_a - P_b; both parallel to D at any regular point), the normals, the edge vectors and 1 / |n_a x n_b|.
 template <typename S>
-__device__ __forceinline__ void pair_derivs_recorded(const v3<S> ak, const v3<S> ap, const v3<S> aq, const v3<S> bk,
-                                                     const v3<S> bp, const v3<S> bq, S sigma, unsigned za,
-                                                     unsigned zb, S& tc0, S& tc1,
-                                                     S (&g0)[18], S (&g1)[18]) {
+struct PairAux {
+  v3<S> c0, c1, na, nb, eap, eaq, ebp, ebq, Dh;
+  S rinv;
+};
+template <typename S>
+__device__ __forceinline__ void pair_derivs_core(const v3<S> ak, const v3<S> ap, const v3<S> aq, const v3<S> bk,
+                                                 const v3<S> bp, const v3<S> bq, S sigma, unsigned za,
+                                                 unsigned zb, S& tc0, S& tc1,
+                                                 S (&g0)[18], S (&g1)[18], PairAux<S>& aux) {
   const v3<S> eap = ap - ak, eaq = aq - ak, ebp = bp - bk, ebq = bq - bk;
   const v3<S> na = cross(eap, eaq), nb = cross(ebp, ebq);
   const v3<S> ab = ak - bk;
   const S dak = dot(nb, ab), dap = dot(nb, ap - bk), daq = dot(nb, aq - bk);
   const S dbk = -dot(na, ab), dbp = dot(na, bp - ak), dbq = dot(na, bq - ak);
   const v3<S> D = cross(na, nb);
-  const v3<S> Dh = inv_sqrt(dot(D, D)) * D;
+  const S rinv = inv_sqrt(dot(D, D));
+  const v3<S> Dh = rinv * D;
   const EndPoint<S> Pa = end_point<S>(sigma, Dh, ak, eap, dak, dap, za == 1u ? S(0) : S(1), bk, ebp, ebq, nb);
   const EndPoint<S> Qa = end_point<S>(sigma, Dh, ak, eaq, dak, daq, za == 2u ? S(0) : S(1), bk, ebp, ebq, nb);
   const EndPoint<S> Pb = end_point<S>(-sigma, Dh, bk, ebp, dbk, dbp, zb == 1u ? S(0) : S(1), ak, eap, eaq, na);
@@ -220,6 +235,16 @@ __device__ __forceinline__ void pair_derivs_recorded(const v3<S> ak, const v3<S>
   put(g0, 9, Pa.yk + Qb.ownk);   put(g0, 12, Pa.yp);            put(g0, 15, Pa.yq + Qb.owne);
   put(g1, 0, Qa.ownk + Pb.yk);   put(g1, 3, Pb.yp);             put(g1, 6, Qa.owne + Pb.yq);
   put(g1, 9, Qa.yk + Pb.ownk);   put(g1, 12, Qa.yp + Pb.owne);  put(g1, 15, Qa.yq);
+  aux.c0 = Pa.E - Qb.E;  aux.c1 = Qa.E - Pb.E;
+  aux.na = na;  aux.nb = nb;  aux.eap = eap;  aux.eaq = eaq;  aux.ebp = ebp;  aux.ebq = ebq;  aux.Dh = Dh;  aux.rinv = rinv;
+}
+template <typename S>
+__device__ __forceinline__ void pair_derivs_recorded(const v3<S> ak, const v3<S> ap, const v3<S> aq, const v3<S> bk,
+                                                     const v3<S> bp, const v3<S> bq, S sigma, unsigned za,
+                                                     unsigned zb, S& tc0, S& tc1,
+                                                     S (&g0)[18], S (&g1)[18]) {
+  PairAux<S> aux;  // never read here: the compiler drops it
+  pair_derivs_core<S>(ak, ap, aq, bk, bp, bq, sigma, za, zb, tc0, tc1, g0, g1, aux);
 }
 
 // Step a3, second half: Eq. 3 and Eq. 4 coefficients.  keep = tt_hess_mode's treatment of the

@@ -15,6 +15,7 @@
 #include "tt_kernels.cuh"
 #include "tt_probe.cuh"
 #include "tt_solve.cuh"
+#include "tt_exact.cuh"
 
 namespace {
 
@@ -690,7 +691,13 @@ tt_status numeric_impl(tt_ctx* ctx, const tt_problem* q, void* energy_sum, void*
   if (ctx->n_chunks > 0) {
     cudaEvent_t* ev_k4 = ctx->evr[1][ctx->ev_n[1] % tt_ctx::EV_RING];
     TT_CUDA(cudaEventRecord(ev_k4[0], st));
-    if (want_h) {
+    if (want_h && ctx->opt.hess_mode == TT_HESS_EXACT) {
+      // the exact Hessian (tt_exact.cuh): one kernel over every round, same partition, ranks and row bases
+      k_assemble_exact<T><<<grid_for(ctx->n_chunks, EX_WARPS), 32 * EX_WARPS, 0, st>>>(p);
+      TT_LAUNCH_CHECK();
+      tt_status s2 = launch_split_finish<T, true>(ctx, q, (T*)vals, st);
+      if (s2 != TT_OK) return s2;
+    } else if (want_h) {
       const size_t smem = sizeof(TileWarpSmem<T>) * TILE_WARPS;
       const int64_t full = (ctx->n_chunks + TILE_WARPS - 1) / TILE_WARPS;
       const int64_t pers = ctx->tile_grid[sizeof(T) == 8 ? 0 : 1];
@@ -739,7 +746,13 @@ tt_status hessvec_impl(tt_ctx* ctx, const tt_problem* q, const void* pvec, void*
   if (ctx->n_chunks > 0) {
     cudaEvent_t* ev_k6 = ctx->evr[2][ctx->ev_n[2] % tt_ctx::EV_RING];
     TT_CUDA(cudaEventRecord(ev_k6[0], st));
-    tt_status s1 = launch_entry_reduce<T, 2>(ctx, p, st);
+    tt_status s1 = TT_OK;
+    if (ctx->opt.hess_mode == TT_HESS_EXACT) {
+      k_hess_vec_exact<T><<<grid_for(ctx->n_chunks, RED_THREADS / 32), RED_THREADS, 0, st>>>(p);
+      TT_LAUNCH_CHECK();
+    } else {
+      s1 = launch_entry_reduce<T, 2>(ctx, p, st);
+    }
     if (s1 != TT_OK) return s1;
     s1 = launch_split_finish<T, false>(ctx, q, (T*)nullptr, st);
     if (s1 != TT_OK) return s1;
@@ -921,7 +934,7 @@ tt_status tt_create(const tt_options* opt, tt_ctx** out) {
   if (!opt || !out) return TT_ERR_INVALID_ARG;
   *out = nullptr;
   if (opt->dtype != TT_F64 && opt->dtype != TT_F32) return TT_ERR_INVALID_ARG;
-  if (opt->hess_mode < TT_HESS_EQ4 || opt->hess_mode > TT_HESS_PSDPROJ) return TT_ERR_INVALID_ARG;
+  if (opt->hess_mode < TT_HESS_EQ4 || opt->hess_mode > TT_HESS_EXACT) return TT_ERR_INVALID_ARG;
   if (!(opt->tc_scale > 0.0)) return TT_ERR_INVALID_ARG;
   int ndev = 0;
   if (cudaGetDeviceCount(&ndev) != cudaSuccess || opt->device < 0 || opt->device >= ndev) {

@@ -18,7 +18,7 @@ LIB_PATH = Path(os.environ["TT_LIB_PATH"]) if os.environ.get("TT_LIB_PATH") else
 
 TT_OK = 0
 TT_F64, TT_F32 = 0, 1
-TT_HESS_EQ4, TT_HESS_FILTER, TT_HESS_PSD2, TT_HESS_PSDPROJ = 0, 1, 2, 3
+TT_HESS_EQ4, TT_HESS_FILTER, TT_HESS_PSD2, TT_HESS_PSDPROJ, TT_HESS_EXACT = 0, 1, 2, 3, 4
 TT_FLAG_FORCE_GENERAL_ROWS = 1
 TT_FLAG_VALIDATE_INDICES = 2
 TT_FLAG_NO_STATE_CHECK = 4

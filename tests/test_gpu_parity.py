@@ -91,7 +91,10 @@ def run_case(oracle, pb, dtype="f64", hess_mode=1, sigma=1.0, flags=0, check_val
     y = torch.full_like(p, float("nan"))
     ctx.tt_hess_vec(out["prob"], p, y)
     torch.cuda.synchronize()
-    y_ref = oracle.hess_vec_pairs(pos_np.shape[0], pb.tris, pairs, ref["active"], ref["tc"], ref["J"], p_np, hess_mode)
+    if hess_mode == 4:   # exact Hessian: the oracle's second-order duals, pair by pair
+        y_ref = oracle.exact_hess_vec(pos_np, pb.tris, pairs, p_np, sigma)
+    else:
+        y_ref = oracle.hess_vec_pairs(pos_np.shape[0], pb.tris, pairs, ref["active"], ref["tc"], ref["J"], p_np, hess_mode)
     assert rel(y.cpu().numpy(), y_ref) <= tol["y"]
     assert max_row_err(y.cpu().numpy(), y_ref, hp_row_scale(ref["rowptr"], ref["colind"], ref["vals"], p_np)) <= rt["y"]
     y_bsr = oracle.bsr_matvec(out["rowptr"].cpu().numpy(), out["colind"].cpu().numpy(),
