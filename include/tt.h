@@ -221,6 +221,43 @@ tt_status tt_pcg_solve(tt_ctx* ctx, const tt_problem* prob, const int32_t* rowpt
                        const void* vals, const void* minv, const void* b, void* x,
                        const tt_pcg_options* opt, int32_t* iters_host, double* relres_host, void* stream);
 
+/* ---- One damped inexact-Newton step on E(x) = sum of T over a fixed candidate list, and the untangling loop around
+ * it ("inexact Newton optimization route", L41-43 / Fig. 2; SURVEY.md 8(f) NEXT-2 "line search on
+ * tt_energy", NEXT-4).  The paper gives no formula, tolerance or step rule; reading A16 fixes the textbook
+ * choice (line-search Newton-CG with a Levenberg-Marquardt shift):
+ *     E0, g, H  at x (this ctx's hess_mode: use a PSD one, TT_HESS_PSD2 or TT_HESS_PSDPROJ, so that H + mu I is SPD)
+ *     d         = pcg.max_iter / pcg.rtol steps of block-Jacobi PCG on (H + mu I) d = g from 0   (tt_pcg_solve)
+ *     alpha     = first of 1, 1/2, 1/4, ... (at most max_backtrack halvings) with
+ *                 E(x - alpha d) <= E0 - armijo_c1 alpha g.d                                      (tt_energy)
+ *     x        <- x - alpha d, IN PLACE; x is left unchanged when no alpha is accepted (accepted = 0).
+ * Everything runs on the device; the host sees the scalars of `report` (one round trip per trial step length).
+ *   pos DEVICE [nV,3] dtype, read AND written; tris, pairs DEVICE as in tt_problem; report HOST [1].
+ * The call invalidates the state cached by tt_hess_symbolic (the positions have moved).
+ * tt_untangle: repeat { candidates = tt_broad_phase(pos, inflate); tt_newton_step } until no pair is active, a step
+ * is rejected, or max_steps steps were taken.  history HOST [max_steps] (one report per step taken), steps_host HOST [1]. */
+typedef struct {
+  double mu;              /* > 0: Levenberg-Marquardt shift added to the diagonal                                  */
+  double armijo_c1;       /* in (0, 1), e.g. 1e-4                                                                   */
+  int32_t max_backtrack;  /* >= 0: halvings of alpha after the full step                                            */
+  int32_t matrix_free;    /* 0: assemble the BSR, block-Jacobi PCG; 1: CG on tt_hess_vec, no BSR, no preconditioner */
+  tt_pcg_options pcg;     /* max_iter, rtol, check_every of the inner solve (its shift is ignored: mu is used)      */
+} tt_newton_options;
+typedef struct {
+  double energy0, energy1;  /* E at x before / after the step (equal if rejected)                                   */
+  double grad_norm;         /* |g|_2 at x                                                                           */
+  double gd;                /* g . d  (> 0 for a descent step x - alpha d)                                          */
+  double alpha;             /* accepted step length, 0 if rejected or nothing is active                             */
+  double pcg_relres;        /* |r|_2 / |g|_2 of the inner solve                                                     */
+  int64_t n_pairs, n_active, nnzb;
+  int32_t pcg_iters, backtracks, accepted, reserved;
+} tt_newton_report;
+tt_status tt_newton_step(tt_ctx* ctx, void* pos, int64_t n_verts, const int32_t* tris, int64_t n_tris,
+                         const int32_t* pairs, int64_t n_pairs, const tt_newton_options* opt,
+                         tt_newton_report* report_host, void* stream);
+tt_status tt_untangle(tt_ctx* ctx, void* pos, int64_t n_verts, const int32_t* tris, int64_t n_tris, double inflate,
+                      int32_t max_steps, const tt_newton_options* opt, tt_newton_report* history_host,
+                      int32_t* steps_host, void* stream);
+
 /* Counters of the last tt_hess_symbolic: what[0]=n_active, [1]=directed entries (2*n_active),
  * [2]=touched triangles, [3]=blocks written directly (exclusive rows), [4]=blocks produced by the
  * general-row merge, [5]=merge records, [6]=nnzb, [7]=kernels launched by this ctx so far (CUB calls

@@ -60,7 +60,7 @@ def untangle(pos, tris, inflate: float = 0.0, max_steps: int = 20, **kw) -> dict
         cand = broad_phase(x, tris, inflate)
         s = newton_step(x, tris, cand, **kw)
         hist.append(dict(E0=s["E0"], E1=s["E1"], alpha=s["alpha"], n_active=s["n_active"], n_pairs=int(cand.shape[0]),
-                         accepted=s["accepted"]))
+                         accepted=s["accepted"], x0=x, x1=s["x"]))
         if s["n_active"] == 0 or not s["accepted"]:
             break
         x = s["x"]

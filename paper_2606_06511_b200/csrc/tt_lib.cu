@@ -80,6 +80,7 @@ struct tt_ctx {
   DevBuf everts, rdesc, tfirst, sfirst, sinfo, tsplit, split_list, dpart, bucket_cnt, bucket_off, long_list, asm_energy, tvals, tslot, vkeys[2], vvals[2], vptr, vslot1;
   DevBuf cub_tmp;
   DevBuf pcg_r, pcg_p, pcg_q, pcg_part[2], pcg_sc, pcg_hist;  // tt_pcg_solve workspace
+  DevBuf nw_g, nw_d, nw_x, nw_vals, nw_minv, nw_sc;            // tt_newton_step workspace
   DevBuf possig;  // [2] u64: checksum of pos at tt_hess_symbolic, and at the last numeric / H.p call
   // broad phase (tt_broad_phase): boxes, grid, (cell, triangle) records, pair keys, result
   DevBuf bp_box, bp_part, bp_grid, bp_cnt, bp_off, bp_keys[2], bp_vals[2], bp_pcnt, bp_poff, bp_pkeys[2], bp_pairs;
@@ -925,6 +926,109 @@ tt_status broad_impl(tt_ctx* ctx, const void* pos, int64_t nV, const int32_t* tr
   return TT_OK;
 }
 
+
+// ---- one Levenberg-Marquardt inexact-Newton step with Armijo backtracking (reading A16) -------------
+template <typename T>
+tt_status newton_impl(tt_ctx* ctx, void* pos, int64_t nV, const int32_t* tris, int64_t nT, const int32_t* pairs, int64_t P,
+                      const tt_newton_options* o, tt_newton_report* rep, cudaStream_t st) {
+  using namespace tts;
+  std::memset(rep, 0, sizeof(*rep));
+  rep->n_pairs = P;
+  tt_problem q{pos, nV, tris, nT, pairs, P};
+  int64_t nnzb = 0, A = 0;
+  tt_status s = symbolic_impl<T>(ctx, &q, &nnzb, &A, st);
+  if (s != TT_OK) return s;
+  rep->n_active = A;
+  rep->nnzb = nnzb;
+  if (A == 0 || nV == 0) {  // nothing intersects: E = 0 is the minimum
+    rep->accepted = 1;
+    return TT_OK;
+  }
+  const int64_t n = 3 * nV;
+  const bool mf = o->matrix_free != 0;
+  TT_CUDA(ctx->nw_g.ensure(sizeof(T) * (size_t)n));
+  TT_CUDA(ctx->nw_d.ensure(sizeof(T) * (size_t)n));
+  TT_CUDA(ctx->nw_x.ensure(sizeof(T) * (size_t)n));
+  TT_CUDA(ctx->nw_sc.ensure(sizeof(double) * 8));
+  if (!mf) {
+    TT_CUDA(ctx->nw_vals.ensure(sizeof(T) * 9 * (size_t)(nnzb + 1)));
+    TT_CUDA(ctx->nw_minv.ensure(sizeof(T) * 9 * (size_t)nV));
+  }
+  T* g = ctx->nw_g.as<T>();
+  T* d = ctx->nw_d.as<T>();
+  T* x_try = ctx->nw_x.as<T>();
+  double* sc = ctx->nw_sc.as<double>();        // [0] g.d  [1] g.g
+  T* e_dev = reinterpret_cast<T*>(sc + 2);      // [0] E0   [1] E(x_try)
+  int* rowptr = ctx->rowptr.as<int>();
+  int* colind = ctx->colind.as<int>();
+  T* vals = mf ? nullptr : ctx->nw_vals.as<T>();
+  s = numeric_impl<T>(ctx, &q, e_dev, g, mf ? nullptr : rowptr, mf ? nullptr : colind, vals, nnzb, st);
+  if (s != TT_OK) return s;
+  T* minv = nullptr;
+  if (!mf) {
+    minv = ctx->nw_minv.as<T>();
+    k_block_jacobi<T><<<grid_for(nV, VEC_THREADS), VEC_THREADS, 0, st>>>(rowptr, colind, vals, nV, o->mu, minv);
+    TT_LAUNCH_CHECK();
+  }
+  tt_pcg_options po = o->pcg;
+  po.shift = o->mu;
+  int32_t iters = 0;
+  double relres = 0.0;
+  s = pcg_impl<T>(ctx, &q, rowptr, colind, vals, minv, g, d, &po, &iters, &relres, st);
+  if (s != TT_OK) return s;
+  rep->pcg_iters = iters;
+  rep->pcg_relres = relres;
+  const unsigned gn = grid_for(n, VEC_THREADS);
+  double* part0 = ctx->pcg_part[0].as<double>();
+  double* part1 = ctx->pcg_part[1].as<double>();
+  k_dot2<T><<<gn, VEC_THREADS, 0, st>>>(g, d, n, part0, part1);
+  TT_LAUNCH_CHECK();
+  k_dot2_final<<<1, 1024, 0, st>>>(part0, part1, (int64_t)gn, sc);
+  TT_LAUNCH_CHECK();
+  double h_sc[2] = {0.0, 0.0};
+  T h_e[2] = {(T)0, (T)0};
+  TT_CUDA(cudaMemcpyAsync(h_sc, sc, sizeof(h_sc), cudaMemcpyDeviceToHost, st));
+  TT_CUDA(cudaMemcpyAsync(h_e, e_dev, sizeof(T), cudaMemcpyDeviceToHost, st));
+  TT_CUDA(cudaStreamSynchronize(st));
+  const double E0 = (double)h_e[0], gd = h_sc[0];
+  rep->energy0 = rep->energy1 = E0;
+  rep->gd = gd;
+  rep->grad_norm = sqrt(h_sc[1]);
+  // ---- Armijo backtracking on the energy of the SAME candidate list ----
+  tt_problem qt{x_try, nV, tris, nT, pairs, P};
+  double alpha = 1.0;
+  for (int j = 0; j <= o->max_backtrack; ++j) {
+    k_step<T><<<gn, VEC_THREADS, 0, st>>>((const T*)pos, d, alpha, n, x_try);
+    TT_LAUNCH_CHECK();
+    s = energy_impl<T>(ctx, &qt, e_dev + 1, nullptr, nullptr, nullptr, nullptr, st);
+    if (s != TT_OK) return s;
+    TT_CUDA(cudaMemcpyAsync(h_e + 1, e_dev + 1, sizeof(T), cudaMemcpyDeviceToHost, st));
+    TT_CUDA(cudaStreamSynchronize(st));
+    const double Et = (double)h_e[1];
+    if (Et <= E0 - o->armijo_c1 * alpha * gd) {
+      TT_CUDA(cudaMemcpyAsync(pos, x_try, sizeof(T) * (size_t)n, cudaMemcpyDeviceToDevice, st));
+      rep->energy1 = Et;
+      rep->alpha = alpha;
+      rep->backtracks = j;
+      rep->accepted = 1;
+      ctx->sig.valid = false;  // the positions have moved: the cached active set and branch decisions are stale
+      return TT_OK;
+    }
+    alpha *= 0.5;
+  }
+  rep->backtracks = o->max_backtrack + 1;
+  return TT_OK;
+}
+
+tt_status check_newton_args(tt_ctx* ctx, const void* pos, int64_t nV, const int32_t* tris, int64_t nT, const tt_newton_options* o) {
+  if (!ctx) return TT_ERR_INVALID_ARG;
+  if (!o || !(o->mu > 0.0) || !(o->armijo_c1 > 0.0 && o->armijo_c1 < 1.0) || o->max_backtrack < 0 || o->pcg.max_iter < 0 ||
+      !(o->pcg.rtol >= 0.0))
+    return fail(ctx, TT_ERR_INVALID_ARG, "newton options: need mu > 0, 0 < armijo_c1 < 1, max_backtrack >= 0, pcg.max_iter >= 0, pcg.rtol >= 0");
+  if (nV < 0 || nT < 0 || (nV > 0 && !pos) || (nT > 0 && !tris)) return fail(ctx, TT_ERR_INVALID_ARG, "NULL array or negative size");
+  return TT_OK;
+}
+
 }  // namespace
 
 // =================================================================================== C ABI
@@ -1230,6 +1334,46 @@ tt_status tt_pcg_solve(tt_ctx* ctx, const tt_problem* prob, const int32_t* rowpt
   }
   return ctx->opt.dtype == TT_F64 ? pcg_impl<double>(ctx, prob, rowptr, colind, vals, minv, b, x, opt, iters_host, relres_host, st)
                                   : pcg_impl<float>(ctx, prob, rowptr, colind, vals, minv, b, x, opt, iters_host, relres_host, st);
+}
+
+tt_status tt_newton_step(tt_ctx* ctx, void* pos, int64_t n_verts, const int32_t* tris, int64_t n_tris, const int32_t* pairs,
+                         int64_t n_pairs, const tt_newton_options* opt, tt_newton_report* report_host, void* stream) {
+  tt_status s = check_newton_args(ctx, pos, n_verts, tris, n_tris, opt);
+  if (s != TT_OK) return s;
+  if (!report_host) return fail(ctx, TT_ERR_INVALID_ARG, "tt_newton_step: report_host is NULL");
+  tt_problem q{pos, n_verts, tris, n_tris, pairs, n_pairs};
+  s = check_problem(ctx, &q);
+  if (s != TT_OK) return s;
+  TT_CUDA(cudaSetDevice(ctx->opt.device));
+  cudaStream_t st = (cudaStream_t)stream;
+  return ctx->opt.dtype == TT_F64 ? newton_impl<double>(ctx, pos, n_verts, tris, n_tris, pairs, n_pairs, opt, report_host, st)
+                                  : newton_impl<float>(ctx, pos, n_verts, tris, n_tris, pairs, n_pairs, opt, report_host, st);
+}
+
+tt_status tt_untangle(tt_ctx* ctx, void* pos, int64_t n_verts, const int32_t* tris, int64_t n_tris, double inflate,
+                      int32_t max_steps, const tt_newton_options* opt, tt_newton_report* history_host, int32_t* steps_host,
+                      void* stream) {
+  tt_status s = check_newton_args(ctx, pos, n_verts, tris, n_tris, opt);
+  if (s != TT_OK) return s;
+  if (max_steps < 0 || (max_steps > 0 && !history_host) || !steps_host || !(inflate >= 0.0))
+    return fail(ctx, TT_ERR_INVALID_ARG, "tt_untangle: max_steps / inflate negative, or history_host / steps_host NULL");
+  TT_CUDA(cudaSetDevice(ctx->opt.device));
+  cudaStream_t st = (cudaStream_t)stream;
+  *steps_host = 0;
+  for (int it = 0; it < max_steps; ++it) {
+    int64_t n_pairs = 0;
+    s = ctx->opt.dtype == TT_F64 ? broad_impl<double>(ctx, pos, n_verts, tris, n_tris, inflate, &n_pairs, st)
+                                 : broad_impl<float>(ctx, pos, n_verts, tris, n_tris, inflate, &n_pairs, st);
+    if (s != TT_OK) return s;
+    const int32_t* pairs = n_pairs > 0 ? ctx->bp_pairs.as<int32_t>() : nullptr;
+    tt_newton_report* rep = history_host + it;
+    s = ctx->opt.dtype == TT_F64 ? newton_impl<double>(ctx, pos, n_verts, tris, n_tris, pairs, n_pairs, opt, rep, st)
+                                 : newton_impl<float>(ctx, pos, n_verts, tris, n_tris, pairs, n_pairs, opt, rep, st);
+    if (s != TT_OK) return s;
+    *steps_host = it + 1;
+    if (rep->n_active == 0 || !rep->accepted) break;
+  }
+  return TT_OK;
 }
 
 tt_status tt_bsr_device(tt_ctx* ctx, const int32_t** rowptr, const int32_t** colind, const void** vals, int64_t* nnzb) {

@@ -278,4 +278,36 @@ k_pcg_dir(const T* __restrict__ z, T* __restrict__ p, int64_t n, const PcgScalar
   if (i < n && !sc->done) p[i] = (T)((double)z[i] + sc->beta * (double)p[i]);
 }
 
+// ---- the Newton step around the solve (tt_newton_step; reading A16) ----------------------------------
+// partials of g.d and g.g (fixed order), then both sums in one CTA
+template <typename T>
+__global__ void __launch_bounds__(VEC_THREADS)
+k_dot2(const T* __restrict__ g, const T* __restrict__ d, int64_t n, double* __restrict__ part_gd, double* __restrict__ part_gg) {
+  const int64_t i = (int64_t)blockIdx.x * VEC_THREADS + threadIdx.x;
+  double a = 0.0, b = 0.0;
+  if (i < n) {
+    const double gi = (double)g[i];
+    a = gi * (double)d[i];
+    b = gi * gi;
+  }
+  cta_sum2(a, b, part_gd, part_gg);
+}
+__global__ void __launch_bounds__(1024) k_dot2_final(const double* __restrict__ part_gd, const double* __restrict__ part_gg,
+                                                     int64_t n, double* __restrict__ out /*[2]*/) {
+  __shared__ double s[32];
+  const double gd = final_sum(part_gd, n, s);
+  const double gg = final_sum(part_gg, n, s);
+  if (threadIdx.x == 0) {
+    out[0] = gd;
+    out[1] = gg;
+  }
+}
+// x_try = x - alpha d
+template <typename T>
+__global__ void __launch_bounds__(VEC_THREADS)
+k_step(const T* __restrict__ x, const T* __restrict__ d, double alpha, int64_t n, T* __restrict__ x_try) {
+  const int64_t i = (int64_t)blockIdx.x * VEC_THREADS + threadIdx.x;
+  if (i < n) x_try[i] = (T)((double)x[i] - alpha * (double)d[i]);
+}
+
 }  // namespace tts

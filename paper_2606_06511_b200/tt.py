@@ -24,7 +24,7 @@ TT_FLAG_VALIDATE_INDICES = 2
 TT_FLAG_NO_STATE_CHECK = 4
 
 EXPORTS = ["tt_create", "tt_destroy", "tt_energy", "tt_hess_symbolic", "tt_energy_grad_hess", "tt_hess_vec",
-           "tt_energy_grad_hess_host", "tt_broad_phase", "tt_broad_phase_pairs", "tt_broad_phase_copy", "tt_bsr_device", "tt_bsr_spmv", "tt_block_jacobi", "tt_pcg_solve", "tt_stats", "tt_kernel_ms", "tt_kernel_ms_mean", "tt_probe_peaks", "tt_status_string", "tt_last_error"]
+           "tt_energy_grad_hess_host", "tt_broad_phase", "tt_broad_phase_pairs", "tt_broad_phase_copy", "tt_bsr_device", "tt_bsr_spmv", "tt_block_jacobi", "tt_pcg_solve", "tt_newton_step", "tt_untangle", "tt_stats", "tt_kernel_ms", "tt_kernel_ms_mean", "tt_probe_peaks", "tt_status_string", "tt_last_error"]
 
 
 class TTOptions(ctypes.Structure):
@@ -40,6 +40,22 @@ class TTProblem(ctypes.Structure):
 class TTPcgOptions(ctypes.Structure):
     _fields_ = [("max_iter", ctypes.c_int32), ("check_every", ctypes.c_int32), ("rtol", ctypes.c_double),
                 ("shift", ctypes.c_double)]
+
+
+class TTNewtonOptions(ctypes.Structure):
+    _fields_ = [("mu", ctypes.c_double), ("armijo_c1", ctypes.c_double), ("max_backtrack", ctypes.c_int32),
+                ("matrix_free", ctypes.c_int32), ("pcg", TTPcgOptions)]
+
+
+class TTNewtonReport(ctypes.Structure):
+    _fields_ = [("energy0", ctypes.c_double), ("energy1", ctypes.c_double), ("grad_norm", ctypes.c_double),
+                ("gd", ctypes.c_double), ("alpha", ctypes.c_double), ("pcg_relres", ctypes.c_double),
+                ("n_pairs", ctypes.c_int64), ("n_active", ctypes.c_int64), ("nnzb", ctypes.c_int64),
+                ("pcg_iters", ctypes.c_int32), ("backtracks", ctypes.c_int32), ("accepted", ctypes.c_int32),
+                ("reserved", ctypes.c_int32)]
+
+    def as_dict(self):
+        return {k: getattr(self, k) for k, _ in self._fields_ if k != "reserved"}
 
 
 class TTError(RuntimeError):
@@ -91,6 +107,12 @@ def load_library():
     lib.tt_pcg_solve.argtypes = [vp, ctypes.POINTER(TTProblem), vp, vp, vp, vp, vp, vp, ctypes.POINTER(TTPcgOptions),
                                  ctypes.POINTER(ctypes.c_int32), ctypes.POINTER(ctypes.c_double), vp]
     lib.tt_pcg_solve.restype = ctypes.c_int
+    lib.tt_newton_step.argtypes = [vp, vp, i64, vp, i64, vp, i64, ctypes.POINTER(TTNewtonOptions),
+                                   ctypes.POINTER(TTNewtonReport), vp]
+    lib.tt_newton_step.restype = ctypes.c_int
+    lib.tt_untangle.argtypes = [vp, vp, i64, vp, i64, ctypes.c_double, ctypes.c_int32, ctypes.POINTER(TTNewtonOptions),
+                                ctypes.POINTER(TTNewtonReport), ctypes.POINTER(ctypes.c_int32), vp]
+    lib.tt_untangle.restype = ctypes.c_int
     lib.tt_stats.argtypes = [vp, ctypes.POINTER(i64), ctypes.c_int32]
     lib.tt_stats.restype = ctypes.c_int
     lib.tt_kernel_ms.argtypes = [vp, ctypes.POINTER(ctypes.c_float), ctypes.c_int32]
@@ -226,6 +248,32 @@ class Context:
                                           _ptr(b), _ptr(x), ctypes.byref(opt), ctypes.byref(it) if want_stats else None,
                                           ctypes.byref(rr) if want_stats else None, _stream_ptr(stream)))
         return (it.value, rr.value) if want_stats else None
+
+    @staticmethod
+    def _newton_options(mu, c1, max_backtrack, matrix_free, pcg_iter, pcg_rtol):
+        return TTNewtonOptions(float(mu), float(c1), int(max_backtrack), 1 if matrix_free else 0,
+                               TTPcgOptions(int(pcg_iter), 0, float(pcg_rtol), 0.0))
+
+    def tt_newton_step(self, pos, tris, pairs, mu=1e-3, c1=1e-4, max_backtrack=20, matrix_free=False, pcg_iter=20,
+                       pcg_rtol=0.0, stream=None):
+        """One damped inexact-Newton step; `pos` is updated IN PLACE.  Returns the report as a dict."""
+        assert pos.is_cuda and pos.dtype == self.dtype and pos.is_contiguous()
+        opt = self._newton_options(mu, c1, max_backtrack, matrix_free, pcg_iter, pcg_rtol)
+        rep = TTNewtonReport()
+        self._check(self.lib.tt_newton_step(self.h, _ptr(pos), pos.shape[0], _ptr(tris), tris.shape[0], _ptr(pairs),
+                                            pairs.shape[0], ctypes.byref(opt), ctypes.byref(rep), _stream_ptr(stream)))
+        return rep.as_dict()
+
+    def tt_untangle(self, pos, tris, inflate=0.0, max_steps=20, mu=1e-3, c1=1e-4, max_backtrack=20, matrix_free=False,
+                    pcg_iter=20, pcg_rtol=0.0, stream=None):
+        """Broad phase + Newton step until nothing intersects; `pos` is updated IN PLACE.  Returns the list of reports."""
+        assert pos.is_cuda and pos.dtype == self.dtype and pos.is_contiguous()
+        opt = self._newton_options(mu, c1, max_backtrack, matrix_free, pcg_iter, pcg_rtol)
+        hist = (TTNewtonReport * max(int(max_steps), 1))()
+        n = ctypes.c_int32(0)
+        self._check(self.lib.tt_untangle(self.h, _ptr(pos), pos.shape[0], _ptr(tris), tris.shape[0], float(inflate),
+                                         int(max_steps), ctypes.byref(opt), hist, ctypes.byref(n), _stream_ptr(stream)))
+        return [hist[i].as_dict() for i in range(n.value)]
 
     def tt_kernel_ms(self):
         arr = (ctypes.c_float * 3)()
