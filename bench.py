@@ -267,8 +267,9 @@ def measure(ctx, pb, args, dev, steps, warmup, world=1, rank=0, sampler_rank0=Fa
     nnzb, n_active = ctx.tt_hess_symbolic(prob)
     energy = torch.zeros(1, dtype=tdt, device=dev)
     grad = torch.empty((nV, 3), dtype=tdt, device=dev)
-    rowptr = torch.empty(nV + 1, dtype=torch.int32, device=dev)
-    colind = torch.empty(max(nnzb, 1), dtype=torch.int32, device=dev)
+    # the BSR pattern stays where tt_hess_symbolic builds it (ctx-owned views, tt_hess_pattern): the numeric call
+    # then writes the values only and does not duplicate rowptr / colind into a second pair of arrays
+    rowptr, colind, _ = ctx.tt_hess_pattern(nV)
     vals = torch.empty((max(nnzb, 1), 3, 3), dtype=tdt, device=dev)
     pvec = torch.randn((nV, 3), dtype=tdt, device=dev)
     yvec = torch.empty_like(pvec)
@@ -282,7 +283,8 @@ def measure(ctx, pb, args, dev, steps, warmup, world=1, rank=0, sampler_rank0=Fa
         ctx.tt_hess_symbolic(prob)
         if record:
             ev[1].record(stream)
-        ctx.tt_energy_grad_hess(prob, energy, grad, rowptr, colind, vals, max(nnzb, 1))
+        rp_addr, ci_addr, _ = ctx.tt_hess_pattern_ptrs()   # re-read: a symbolic call may re-allocate its workspace
+        ctx.tt_energy_grad_hess(prob, energy, grad, rp_addr, ci_addr, vals, max(nnzb, 1))
         if record:
             ev[2].record(stream)
         ctx.tt_hess_vec(prob, pvec, yvec)
@@ -322,6 +324,7 @@ def measure(ctx, pb, args, dev, steps, warmup, world=1, rank=0, sampler_rank0=Fa
     hbm, peak_src = peaks()
     st = ctx.tt_stats()
     n_touch = st["n_touched_tris"]                                    # triangles of ACTIVE pairs
+    rowptr, colind, _ = ctx.tt_hess_pattern(nV)                       # the views of the LAST symbolic call
     rows_touched = int((rowptr[1:] != rowptr[:-1]).sum().item())      # their vertices (= non-empty rows)
     cand_tris = int(torch.unique(pairs).numel())                      # triangles any CANDIDATE refers to
     cand_verts = int(torch.unique(tris[torch.unique(pairs).long()]).numel()) if P else 0

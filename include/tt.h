@@ -130,6 +130,12 @@ tt_status tt_energy(tt_ctx* ctx, const tt_problem* prob, void* energy_sum, void*
 tt_status tt_hess_symbolic(tt_ctx* ctx, const tt_problem* prob, int64_t* nnzb_host,
                            int64_t* n_active_host, void* stream);
 
+/* Device views of the pattern built by the last tt_hess_symbolic (owned by ctx, valid until the next
+ * tt_hess_symbolic / *_host call or tt_destroy): rowptr [nV+1], colind [nnzb].  Passing exactly these pointers as
+ * bsr_rowptr / bsr_colind to tt_energy_grad_hess makes that call skip its copy of the pattern into caller memory
+ * (the pattern is then shared, not duplicated: 4 (nV + 1 + nnzb) bytes less to move per numeric call).        */
+tt_status tt_hess_pattern(tt_ctx* ctx, const int32_t** rowptr, const int32_t** colind, int64_t* nnzb);
+
 /* Steps 2-4 (Eq. 2-4), numeric phase, on the active set cached by tt_hess_symbolic for
  * the same problem (same pointers and sizes, and unchanged positions: TT_ERR_STATE otherwise --
  * the positions are verified by checksum unless TT_FLAG_NO_STATE_CHECK, which makes this call block

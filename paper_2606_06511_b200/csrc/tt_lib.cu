@@ -1376,6 +1376,15 @@ tt_status tt_untangle(tt_ctx* ctx, void* pos, int64_t n_verts, const int32_t* tr
   return TT_OK;
 }
 
+tt_status tt_hess_pattern(tt_ctx* ctx, const int32_t** rowptr, const int32_t** colind, int64_t* nnzb) {
+  if (!ctx) return TT_ERR_INVALID_ARG;
+  if (!ctx->sig.valid) return fail(ctx, TT_ERR_STATE, "tt_hess_pattern: no tt_hess_symbolic result");
+  if (rowptr) *rowptr = ctx->rowptr.as<int32_t>();
+  if (colind) *colind = ctx->colind.as<int32_t>();
+  if (nnzb) *nnzb = ctx->nnzb;
+  return TT_OK;
+}
+
 tt_status tt_bsr_device(tt_ctx* ctx, const int32_t** rowptr, const int32_t** colind, const void** vals, int64_t* nnzb) {
   if (!ctx) return TT_ERR_INVALID_ARG;
   if (!ctx->o_vals.p) return fail(ctx, TT_ERR_STATE, "tt_bsr_device: no tt_energy_grad_hess_host result");

@@ -24,7 +24,7 @@ TT_FLAG_VALIDATE_INDICES = 2
 TT_FLAG_NO_STATE_CHECK = 4
 
 EXPORTS = ["tt_create", "tt_destroy", "tt_energy", "tt_hess_symbolic", "tt_energy_grad_hess", "tt_hess_vec",
-           "tt_energy_grad_hess_host", "tt_broad_phase", "tt_broad_phase_pairs", "tt_broad_phase_copy", "tt_bsr_device", "tt_bsr_spmv", "tt_block_jacobi", "tt_pcg_solve", "tt_newton_step", "tt_untangle", "tt_stats", "tt_kernel_ms", "tt_kernel_ms_mean", "tt_probe_peaks", "tt_status_string", "tt_last_error"]
+           "tt_energy_grad_hess_host", "tt_hess_pattern", "tt_broad_phase", "tt_broad_phase_pairs", "tt_broad_phase_copy", "tt_bsr_device", "tt_bsr_spmv", "tt_block_jacobi", "tt_pcg_solve", "tt_newton_step", "tt_untangle", "tt_stats", "tt_kernel_ms", "tt_kernel_ms_mean", "tt_probe_peaks", "tt_status_string", "tt_last_error"]
 
 
 class TTOptions(ctypes.Structure):
@@ -98,6 +98,8 @@ def load_library():
     lib.tt_broad_phase_pairs.restype = ctypes.c_int
     lib.tt_broad_phase_copy.argtypes = [vp, vp, i64, vp]
     lib.tt_broad_phase_copy.restype = ctypes.c_int
+    lib.tt_hess_pattern.argtypes = [vp, ctypes.POINTER(vp), ctypes.POINTER(vp), ctypes.POINTER(i64)]
+    lib.tt_hess_pattern.restype = ctypes.c_int
     lib.tt_bsr_device.argtypes = [vp, ctypes.POINTER(vp), ctypes.POINTER(vp), ctypes.POINTER(vp), ctypes.POINTER(i64)]
     lib.tt_bsr_device.restype = ctypes.c_int
     lib.tt_bsr_spmv.argtypes = [vp, i64, vp, vp, vp, ctypes.c_double, vp, vp, vp]
@@ -131,7 +133,12 @@ def load_library():
 
 
 def _ptr(t):
-    return None if t is None else ctypes.c_void_p(t.data_ptr())
+    """Device pointer of a tensor; raw addresses (int / c_void_p, e.g. from tt_hess_pattern_ptrs) pass through."""
+    if t is None or isinstance(t, ctypes.c_void_p):
+        return t
+    if isinstance(t, int):
+        return ctypes.c_void_p(t)
+    return ctypes.c_void_p(t.data_ptr())
 
 
 def _stream_ptr(stream):
@@ -197,6 +204,29 @@ class Context:
         self._check(self.lib.tt_energy_grad_hess(self.h, ctypes.byref(prob[0]), _ptr(energy_sum), _ptr(grad),
                                                  _ptr(bsr_rowptr), _ptr(bsr_colind), _ptr(bsr_vals),
                                                  int(nnzb_capacity), _stream_ptr(stream)))
+
+    # ---- tt_hess_pattern ----
+    def tt_hess_pattern_ptrs(self):
+        """(rowptr address, colind address, nnzb) of the ctx-owned pattern -- re-read after every tt_hess_symbolic (the
+        workspace may have been re-allocated)."""
+        rp, ci, n = ctypes.c_void_p(), ctypes.c_void_p(), ctypes.c_int64(0)
+        self._check(self.lib.tt_hess_pattern(self.h, ctypes.byref(rp), ctypes.byref(ci), ctypes.byref(n)))
+        return rp.value, ci.value, int(n.value)
+
+    def tt_hess_pattern(self, n_verts):
+        """Zero-copy int32 tensor views (rowptr [nV+1], colind [nnzb]) of the ctx-owned pattern of the last
+        tt_hess_symbolic; valid until the next symbolic / host call.  Passing them to tt_energy_grad_hess skips its
+        pattern copy."""
+        rp, ci, n = ctypes.c_void_p(), ctypes.c_void_p(), ctypes.c_int64(0)
+        self._check(self.lib.tt_hess_pattern(self.h, ctypes.byref(rp), ctypes.byref(ci), ctypes.byref(n)))
+
+        class _View:
+            def __init__(self, ptr, count):
+                self.__cuda_array_interface__ = dict(shape=(count,), typestr="<i4", data=(ptr, False), version=2)
+
+        rowptr = torch.as_tensor(_View(rp.value, int(n_verts) + 1), device=self.device)
+        colind = torch.as_tensor(_View(ci.value, max(int(n.value), 1)), device=self.device)
+        return rowptr, colind, int(n.value)
 
     # ---- tt_hess_vec ----
     def tt_hess_vec(self, prob, p, y, stream=None):

@@ -446,3 +446,30 @@ def test_properties_on_gpu_outputs(oracle_mod):
     assert float(z.norm().cpu()) <= 1e-9 * float(out["vals"].norm().cpu())
     assert float(g.sum(0).abs().max().cpu()) <= 1e-9 * float(g.abs().max().cpu()) * 100
     ctx.close()
+
+
+def test_hess_pattern_views(oracle_mod):
+    """tt_hess_pattern: the ctx-owned pattern views equal the pattern tt_energy_grad_hess copies out, and a numeric call
+    that is handed the views (no copy) writes the same values."""
+    from paper_2606_06511_b200 import inputs, tt
+    dev = _dev()
+    pb = inputs.config0_soup(n_tris=64, pool=48, seed=77)
+    ctx = tt.Context(torch.float64, 1, 1.0, 0)
+    pos, tris, prs = (torch.from_numpy(a).to(dev) for a in (pb.pos, pb.tris, pb.pairs))
+    out = tt.assemble(ctx, pos, tris, prs)
+    rp, ci, nnzb = ctx.tt_hess_pattern(pb.n_verts)
+    assert nnzb == out["nnzb"] and torch.equal(rp, out["rowptr"]) and torch.equal(ci[:nnzb], out["colind"])
+    vals2 = torch.full_like(out["vals"], float("nan"))
+    e2 = torch.zeros(1, dtype=torch.float64, device=dev)
+    g2 = torch.empty_like(out["grad"])
+    a_rp, a_ci, _ = ctx.tt_hess_pattern_ptrs()
+    assert a_rp == rp.data_ptr() and a_ci == ci.data_ptr()
+    ctx.tt_energy_grad_hess(out["prob"], e2, g2, a_rp, a_ci, vals2, nnzb)
+    torch.cuda.synchronize()
+    assert torch.equal(vals2, out["vals"]) and torch.equal(g2, out["grad"])
+    ctx.close()
+    ctx3 = tt.Context(torch.float64, 1, 1.0, 0)
+    with pytest.raises(tt.TTError) as ei:
+        ctx3.tt_hess_pattern_ptrs()
+    assert ei.value.status == -5
+    ctx3.close()
