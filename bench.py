@@ -490,6 +490,22 @@ def main():
                 "kernel_ms": dom["ms"], "share_of_step": dom["ms"] / ms_step,
                 "kernel_launches_averaged": m["kernel_launches"]}
 
+    # ---- what random gathers can reach on this memory system (tt_probe_gather), beside the copy bandwidth: K1 gathers
+    #      6 vertices per candidate, K6 3 partner vertices + 3 partner p per directed entry ----
+    gather = None
+    try:
+        gp = tt.tt_probe_gather(local_rank)
+        k1_useful = 6 * 3 * w * P                      # bytes of vertex data K1 gathers (ids and pair list not counted)
+        k6_useful = 2 * 3 * 3 * w * 2 * n_active       # partner positions + partner p per directed entry
+        gather = {"vertex_items_gbs": gp["vertex_gbs"], "triangle_items_gbs": gp["triangle_gbs"], "unit": "GB/s of useful bytes",
+                  "what": "random 24-byte / 72-byte fp64 items from a 144 MB array, one per thread (tt_probe_gather)",
+                  "k_classify": {"useful_gather_bytes": int(k1_useful), "achieved_gbs": k1_useful / (m["kernel_ms"]["classify"] * 1e-3) / 1e9,
+                                 "frac_of_vertex_gather": k1_useful / (m["kernel_ms"]["classify"] * 1e-3) / 1e9 / gp["vertex_gbs"]},
+                  "k_entry_pipe": {"useful_gather_bytes": int(k6_useful), "achieved_gbs": k6_useful / (m["kernel_ms"]["hess_vec"] * 1e-3) / 1e9,
+                                   "frac_of_triangle_gather": k6_useful / (m["kernel_ms"]["hess_vec"] * 1e-3) / 1e9 / gp["triangle_gbs"]}}
+    except Exception as e:   # diagnostic only
+        gather = {"error": str(e)}
+
     cpu = None
     if world == 1 and not args.no_cpu_baseline:
         cpu = cpu_baseline(pb, args.hess_mode)
@@ -510,7 +526,7 @@ def main():
            "cpu_baseline": cpu, "e2e": e2e, "gpu_launches": m["launches"],
            "clocks": m["clocks"], "kernel_ms": m["kernel_ms"],
            "kernel_roofline": {k: {"frac": m[k]["frac"], "algorithmic_bytes": m[k]["algorithmic_bytes"]} for k in ("k1", "k4", "k6")},
-           "phase_ms": m["phase_ms"], "sweep": sweep,
+           "phase_ms": m["phase_ms"], "sweep": sweep, "gather_probe": gather,
            "active_pairs_per_s": n_active * world / (ms_step * 1e-3)}
     print(json.dumps(out), flush=True)
     if world > 1:

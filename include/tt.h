@@ -288,6 +288,13 @@ tt_status tt_kernel_ms_mean(tt_ctx* ctx, float* ms, int32_t* launches, int32_t n
  *   ALU peak.                                                              */
 tt_status tt_probe_peaks(int32_t device, double* tflops);
 
+/* Diagnostic (not on the hot path): useful bytes per second of RANDOM gathers from a 144 MB array (the size of the
+ * 6 M-vertex fp64 position array of BASELINE configs[4]; larger than the L2), one item per thread:
+ *   gbs HOST [2]: [0] = 24-byte items (one vertex), [1] = 72-byte items (the three vertices of a soup triangle), GB/s.
+ * This is the ceiling that the access pattern of the classification (K1) and H.p (K6) kernels can reach on this
+ * memory system -- sector granularity and DRAM row locality included; bench.py reports it beside the copy bandwidth. */
+tt_status tt_probe_gather(int32_t device, double* gbs);
+
 const char* tt_status_string(tt_status s);
 const char* tt_last_error(const tt_ctx* ctx);
 

@@ -1444,6 +1444,16 @@ tt_status tt_probe_peaks(int32_t device, double* tflops) {
   return (tflops[0] > 0.0 && tflops[1] > 0.0) ? TT_OK : TT_ERR_CUDA;
 }
 
+tt_status tt_probe_gather(int32_t device, double* gbs) {
+  if (!gbs) return TT_ERR_INVALID_ARG;
+  if (cudaSetDevice(device) != cudaSuccess) { (void)cudaGetLastError(); return TT_ERR_CUDA; }
+  const size_t bytes = (size_t)144 << 20;       // the size of config 4's position array (6 M vertices, fp64)
+  const long long items = 60ll * 1000 * 1000;   // K1 gathers 60 M vertices per 10 M candidates
+  gbs[0] = ttp::gather_gbs<3>(bytes, items, nullptr);
+  gbs[1] = ttp::gather_gbs<9>(bytes, items / 3, nullptr);
+  return (gbs[0] > 0.0 && gbs[1] > 0.0) ? TT_OK : TT_ERR_CUDA;
+}
+
 const char* tt_status_string(tt_status s) {
   switch (s) {
     case TT_OK: return "TT_OK";

@@ -24,7 +24,7 @@ TT_FLAG_VALIDATE_INDICES = 2
 TT_FLAG_NO_STATE_CHECK = 4
 
 EXPORTS = ["tt_create", "tt_destroy", "tt_energy", "tt_hess_symbolic", "tt_energy_grad_hess", "tt_hess_vec",
-           "tt_energy_grad_hess_host", "tt_hess_pattern", "tt_broad_phase", "tt_broad_phase_pairs", "tt_broad_phase_copy", "tt_bsr_device", "tt_bsr_spmv", "tt_block_jacobi", "tt_pcg_solve", "tt_newton_step", "tt_untangle", "tt_stats", "tt_kernel_ms", "tt_kernel_ms_mean", "tt_probe_peaks", "tt_status_string", "tt_last_error"]
+           "tt_energy_grad_hess_host", "tt_hess_pattern", "tt_broad_phase", "tt_broad_phase_pairs", "tt_broad_phase_copy", "tt_bsr_device", "tt_bsr_spmv", "tt_block_jacobi", "tt_pcg_solve", "tt_newton_step", "tt_untangle", "tt_stats", "tt_kernel_ms", "tt_kernel_ms_mean", "tt_probe_peaks", "tt_probe_gather", "tt_status_string", "tt_last_error"]
 
 
 class TTOptions(ctypes.Structure):
@@ -124,6 +124,8 @@ def load_library():
     lib.tt_kernel_ms_mean.restype = ctypes.c_int
     lib.tt_probe_peaks.argtypes = [ctypes.c_int32, ctypes.POINTER(ctypes.c_double)]
     lib.tt_probe_peaks.restype = ctypes.c_int
+    lib.tt_probe_gather.argtypes = [ctypes.c_int32, ctypes.POINTER(ctypes.c_double)]
+    lib.tt_probe_gather.restype = ctypes.c_int
     lib.tt_status_string.argtypes = [ctypes.c_int]
     lib.tt_status_string.restype = ctypes.c_char_p
     lib.tt_last_error.argtypes = [vp]
@@ -336,6 +338,18 @@ def tt_probe_peaks(device=0):
     if st != TT_OK:
         raise TTError(st, lib.tt_status_string(st).decode(), "tt_probe_peaks failed")
     return dict(fp64_tflops=float(arr[0]), fp32_tflops=float(arr[1]))
+
+
+def tt_probe_gather(device=0):
+    """Useful GB/s of random 24-byte / 72-byte gathers from a 144 MB array (diagnostic)."""
+    if not torch.cuda.is_available():
+        raise RuntimeError("paper_2606_06511_b200 needs a CUDA device (no CPU fallback)")
+    lib = load_library()
+    arr = (ctypes.c_double * 2)()
+    st = lib.tt_probe_gather(int(device), arr)
+    if st != TT_OK:
+        raise TTError(st, lib.tt_status_string(st).decode(), "tt_probe_gather failed")
+    return dict(vertex_gbs=float(arr[0]), triangle_gbs=float(arr[1]))
 
 
 def assemble(ctx: Context, pos, tris, pairs, want_hess=True, stream=None):
