@@ -1171,36 +1171,6 @@ __device__ __forceinline__ void unpermute_own(Entry<C>& E, int (&er)[3]) {
   for (int r = 0; r < 3; ++r) er[r] = (E.pp[r] == 0) ? e0 : ((E.pp[r] == 1) ? e1 : e2);
 }
 
-// Brings the partner half of J into COLUMN order (ascending block rank) and sorts the ranks with it.  The
-// lanes of a warp then all store their lowest-ranked block with the same instruction, the next with the
-// next: with the recorded order each lane's instruction hit a different one of its three blocks (offsets
-// 0, 9 or 18 words apart) and every tile store took 5 shared-memory wavefronts instead of 2.  ncu, 10 M pairs:
-// store bank conflicts 86.4 M -> 64.7 M of 204 M -> 182 M store wavefronts; the kernel time did not move
-// (2.39 ms): K4 is bound by issue latency at 8 warps / SM, not by the L1 data pipe (profiles/r2_notes.md).
-// Selects only: no shared-memory round trip.
-template <typename C>
-__device__ __forceinline__ void sort_partner_by_rank(Entry<C>& E, int (&er)[3]) {
-  const int o0 = (er[0] > er[1]) + (er[0] > er[2]);  // position of recorded vertex r among the three ranks
-  const int o1 = (er[1] > er[0]) + (er[1] > er[2]);
-  C t0[9], t1[9];
-#pragma unroll
-  for (int i = 0; i < 9; ++i) {
-    t0[i] = E.g0[9 + i];
-    t1[i] = E.g1[9 + i];
-  }
-  const int e0 = er[0], e1 = er[1], e2 = er[2];
-#pragma unroll
-  for (int n = 0; n < 3; ++n) {
-    const bool a = (o0 == n), b = (o1 == n);
-    er[n] = a ? e0 : (b ? e1 : e2);
-#pragma unroll
-    for (int j = 0; j < 3; ++j) {
-      E.g0[9 + 3 * n + j] = a ? t0[j] : (b ? t0[3 + j] : t0[6 + j]);
-      E.g1[9 + 3 * n + j] = a ? t1[j] : (b ? t1[3 + j] : t1[6 + j]);
-    }
-  }
-}
-
 __device__ __forceinline__ void bulk_s2g(void* gdst, const void* ssrc, uint32_t bytes) {
   asm volatile("cp.async.bulk.global.shared::cta.bulk_group [%0], [%1], %2;" ::"l"(gdst),
                "r"((uint32_t)__cvta_generic_to_shared(ssrc)), "r"(bytes)
@@ -1318,7 +1288,11 @@ __device__ __forceinline__ void load_round_ops(const AsmParams<T>& P, const int4
   }
 }
 
-template <typename T, bool PROJ>  // PROJ: TT_HESS_PSDPROJ compiled in (the other modes run the leaner instantiation)
+// PROJ: TT_HESS_PSDPROJ compiled in (the other modes run the leaner instantiation).  PARTS: some slots are parts of
+// split triangles (more than 32 partners); without any -- up to ~15 M pairs on BASELINE's 2 M-triangle soup -- the
+// instantiation without their code runs: the kernel sits at 254 of 255 registers and the few selects and the ballot
+// of the part path cost it 3 % (measured, profiles/r2_step_breakdown.md).
+template <typename T, bool PROJ, bool PARTS>
 __global__ void __maxnreg__(TT_TILE_MAXNREG)
 k_assemble_tile(const AsmParams<T> P) {
   extern __shared__ __align__(16) unsigned char s_raw[];
@@ -1380,12 +1354,11 @@ k_assemble_tile(const AsmParams<T> P) {
     __syncwarp();
     if (valid) {
       unpermute_own(E, er);
-      sort_partner_by_rank(E, er);
     }
 
     if (!is_long) {
       // lane = triangle: tile slots (16-byte slots, prefix sum over the round's triangles)
-      const bool part_slot = cur.dr[0] < 0;  // a part of a split triangle: no diagonal blocks in its runs
+      const bool part_slot = PARTS && cur.dr[0] < 0;  // a part of a split triangle: no diagonal blocks in its runs
       const int run_bytes = RUN_UNIT * (cur.e1 - cur.e0 + (part_slot ? 0 : 1));
       int slot_off;
       {
@@ -1467,7 +1440,7 @@ k_assemble_tile(const AsmParams<T> P) {
         __syncwarp();
       }
 
-      {  // parts hand their diagonal partial sums to k_split_finish
+      if (PARTS) {  // parts hand their diagonal partial sums to k_split_finish
         const int pidx = (lane < ntri && part_slot) ? (-1 - cur.dr[0]) : -1;
         if (__ballot_sync(FULL, pidx >= 0)) {
           for (int tt = 0; tt < ntri; ++tt) {
@@ -1534,7 +1507,7 @@ k_assemble_tile(const AsmParams<T> P) {
           }
 #pragma unroll
           for (int tt = 0; tt < RND_MAX_TRI; ++tt)
-            if (tt < ntri && off[tt] >= 0) *reinterpret_cast<T*>(S.tile + off[tt] + cq * (int)sizeof(T)) = val[tt];
+            if (tt < ntri && (!PARTS || off[tt] >= 0)) *reinterpret_cast<T*>(S.tile + off[tt] + cq * (int)sizeof(T)) = val[tt];
         }
         // positions of the next round (L2 hits): requested as soon as this round's J is dead
         if (m == 2 && lane < round_entries(d_nxt)) load_pos18(P.pos, ids_nxt, x);

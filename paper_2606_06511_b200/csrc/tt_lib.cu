@@ -702,10 +702,12 @@ tt_status numeric_impl(tt_ctx* ctx, const tt_problem* q, void* energy_sum, void*
       const size_t smem = sizeof(TileWarpSmem<T>) * TILE_WARPS;
       const int64_t full = (ctx->n_chunks + TILE_WARPS - 1) / TILE_WARPS;
       const int64_t pers = ctx->tile_grid[sizeof(T) == 8 ? 0 : 1];
-      if (ctx->opt.hess_mode == TT_HESS_PSDPROJ)
-        k_assemble_tile<T, true><<<(unsigned)(full < pers ? full : pers), 32 * TILE_WARPS, smem, st>>>(p);
-      else
-        k_assemble_tile<T, false><<<(unsigned)(full < pers ? full : pers), 32 * TILE_WARPS, smem, st>>>(p);
+      const unsigned grid = (unsigned)(full < pers ? full : pers);
+      const bool proj = ctx->opt.hess_mode == TT_HESS_PSDPROJ, parts = ctx->n_parts > 0;
+      if (proj && parts) k_assemble_tile<T, true, true><<<grid, 32 * TILE_WARPS, smem, st>>>(p);
+      else if (proj) k_assemble_tile<T, true, false><<<grid, 32 * TILE_WARPS, smem, st>>>(p);
+      else if (parts) k_assemble_tile<T, false, true><<<grid, 32 * TILE_WARPS, smem, st>>>(p);
+      else k_assemble_tile<T, false, false><<<grid, 32 * TILE_WARPS, smem, st>>>(p);
       if (ctx->n_long > 0) {
         TT_LAUNCH_CHECK();
         k_assemble_long_tile<T, true><<<(unsigned)ctx->n_long, 32, sizeof(LongTileSmem<T, true>), st>>>(p);
@@ -1065,18 +1067,22 @@ tt_status tt_create(const tt_options* opt, tt_ctx** out) {
   {
     cudaError_t e = cudaSuccess;
     auto opt_in = [&](const void* f, size_t smem) { if (e == cudaSuccess) e = cudaFuncSetAttribute(f, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem); };
-    opt_in((const void*)ttk::k_assemble_tile<double, false>, sizeof(ttk::TileWarpSmem<double>) * ttk::TILE_WARPS);
-    opt_in((const void*)ttk::k_assemble_tile<double, true>, sizeof(ttk::TileWarpSmem<double>) * ttk::TILE_WARPS);
-    opt_in((const void*)ttk::k_assemble_tile<float, false>, sizeof(ttk::TileWarpSmem<float>) * ttk::TILE_WARPS);
-    opt_in((const void*)ttk::k_assemble_tile<float, true>, sizeof(ttk::TileWarpSmem<float>) * ttk::TILE_WARPS);
+    opt_in((const void*)ttk::k_assemble_tile<double, false, false>, sizeof(ttk::TileWarpSmem<double>) * ttk::TILE_WARPS);
+    opt_in((const void*)ttk::k_assemble_tile<double, false, true>, sizeof(ttk::TileWarpSmem<double>) * ttk::TILE_WARPS);
+    opt_in((const void*)ttk::k_assemble_tile<double, true, false>, sizeof(ttk::TileWarpSmem<double>) * ttk::TILE_WARPS);
+    opt_in((const void*)ttk::k_assemble_tile<double, true, true>, sizeof(ttk::TileWarpSmem<double>) * ttk::TILE_WARPS);
+    opt_in((const void*)ttk::k_assemble_tile<float, false, false>, sizeof(ttk::TileWarpSmem<float>) * ttk::TILE_WARPS);
+    opt_in((const void*)ttk::k_assemble_tile<float, false, true>, sizeof(ttk::TileWarpSmem<float>) * ttk::TILE_WARPS);
+    opt_in((const void*)ttk::k_assemble_tile<float, true, false>, sizeof(ttk::TileWarpSmem<float>) * ttk::TILE_WARPS);
+    opt_in((const void*)ttk::k_assemble_tile<float, true, true>, sizeof(ttk::TileWarpSmem<float>) * ttk::TILE_WARPS);
     opt_in((const void*)ttk::k_assemble_long_tile<double, true>, sizeof(ttk::LongTileSmem<double, true>));
     opt_in((const void*)ttk::k_assemble_long_tile<double, false>, sizeof(ttk::LongTileSmem<double, false>));
     opt_in((const void*)ttk::k_assemble_long_tile<float, true>, sizeof(ttk::LongTileSmem<float, true>));
     opt_in((const void*)ttk::k_assemble_long_tile<float, false>, sizeof(ttk::LongTileSmem<float, false>));
         int sms = 0, nb0 = 0, nb1 = 0;
     if (e == cudaSuccess) e = cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, opt->device);
-    if (e == cudaSuccess) e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&nb0, ttk::k_assemble_tile<double, true>, 32 * ttk::TILE_WARPS, sizeof(ttk::TileWarpSmem<double>) * ttk::TILE_WARPS);
-    if (e == cudaSuccess) e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&nb1, ttk::k_assemble_tile<float, true>, 32 * ttk::TILE_WARPS, sizeof(ttk::TileWarpSmem<float>) * ttk::TILE_WARPS);
+    if (e == cudaSuccess) e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&nb0, ttk::k_assemble_tile<double, true, true>, 32 * ttk::TILE_WARPS, sizeof(ttk::TileWarpSmem<double>) * ttk::TILE_WARPS);
+    if (e == cudaSuccess) e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&nb1, ttk::k_assemble_tile<float, true, true>, 32 * ttk::TILE_WARPS, sizeof(ttk::TileWarpSmem<float>) * ttk::TILE_WARPS);
     if (e != cudaSuccess) { (void)cudaGetLastError(); delete c; return TT_ERR_CUDA; }
     auto pipe_setup = [&](const void* f, size_t smem, int& grid) {
       int nb = 0;
