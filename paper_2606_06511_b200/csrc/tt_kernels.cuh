@@ -107,22 +107,19 @@ __device__ __forceinline__ double block_sum(double v, double* smem /*[THREADS/32
 #ifndef TT_CLS_MIN_CTAS
 #define TT_CLS_MIN_CTAS 3   // 85 registers, 24 warps / SM: 0.755 -> 0.69 ms at 10M candidates (4: 0.73)
 #endif
-// Per-candidate record written by K1 for the symbolic phase: recorded branch decisions (ttg::pair_config,
-// 12 bits) | place of the entry a -> b in a's segment (26 bits) | place of b -> a in b's segment (26 bits).
-constexpr int REC_P0_SHIFT = 12, REC_P1_SHIFT = 38;
-constexpr unsigned long long REC_CFG_MASK = 0xfffull, REC_P_MASK = 0x3ffffffull;
+// Per-candidate record written by K1 for the symbolic phase: the recorded branch decisions (ttg::pair_config, 12 bits).
 template <typename T>
 __global__ void __launch_bounds__(CLS_THREADS, TT_CLS_MIN_CTAS)
 k_classify(const T* __restrict__ pos, const int* __restrict__ tris, const int2* __restrict__ pairs,
            int64_t P, double sigma, uint32_t* __restrict__ mask, int* __restrict__ blk_count,
            double* __restrict__ blk_energy, T* __restrict__ e_pp, T* __restrict__ tc_out,
-           uint64_t* __restrict__ rec_out, int* __restrict__ deg) {
+           uint16_t* __restrict__ rec_out, int* __restrict__ deg) {
   __shared__ double s_e[CLS_THREADS / 32];
   __shared__ int s_c[CLS_THREADS / 32];
   const int64_t k = (int64_t)blockIdx.x * CLS_THREADS + threadIdx.x;
   bool active = false;
   double tc0 = 0.0, tc1 = 0.0, en = 0.0;
-  unsigned long long cfg = 0ull;
+  unsigned cfg = 0u;
   if (k < P) {
     const int2 pr = __ldg(pairs + k);
     int va[3], vb[3];
@@ -137,17 +134,16 @@ k_classify(const T* __restrict__ pos, const int* __restrict__ tris, const int2* 
         en = pr2 * pr2;  // Eq. 2
         cfg = ttg::pair_config(g);
         if (deg) {
-          // Counting sort of the directed entries by source triangle, first half: the histogram, and -- the
-          // value the atomic returns -- this entry's place inside its triangle's segment.  (Integer atomics:
-          // WHICH place an entry gets depends on the schedule, the segment's CONTENT does not, and every
-          // segment is sorted before anything depends on its order.)
-          const unsigned long long p0 = (unsigned)atomicAdd(deg + pr.x, 1);
-          const unsigned long long p1 = (unsigned)atomicAdd(deg + pr.y, 1);
-          cfg |= (p0 << REC_P0_SHIFT) | (p1 << REC_P1_SHIFT);
+          // Counting sort of the directed entries by source triangle, first half: the histogram (integer
+          // reductions without a return value: the RESULT does not depend on the schedule).  The place of an entry
+          // inside its triangle's segment is taken by k_compact; K1 runs at 35 % occupancy on a chain of dependent
+          // gathers and an atomic whose value it has to wait for costs it 10 % (measured).
+          atomicAdd(deg + pr.x, 1);
+          atomicAdd(deg + pr.y, 1);
         }
       }
     }
-    if (rec_out) rec_out[k] = cfg;
+    if (rec_out) rec_out[k] = (uint16_t)cfg;
     if (e_pp) e_pp[k] = (T)en;
     if (tc_out) {
       tc_out[2 * k] = (T)tc0;
@@ -205,15 +201,15 @@ __global__ void k_set_count(const int* __restrict__ blk_off, const int* __restri
 // Order-preserving compaction of the active pair ids (ballot / popc positions + per-CTA offsets) and, in
 // the same pass, the COUNTING SORT of the directed entries by source triangle: active pair (s, t) becomes
 // the entries s -> t (side 0) and t -> s (side 1); K1 has counted the entries of every triangle (deg), the
-// scan of deg is tptr, and an entry goes to the place inside its triangle's segment that K1's atomic returned.
-// The order INSIDE a segment is whatever the atomics gave; the symbolic kernels sort every segment by
-// (partner, side) before anything depends on it, so all results are deterministic (two entries with the
-// same key are the same pair listed twice: bit-identical contributions).
+// scan of deg is tptr, and an entry takes the next free place of its triangle's segment (integer atomic on
+// `fill`, zeroed by the caller).  The order INSIDE a segment is whatever the atomics give; the symbolic
+// kernels sort every segment by (partner, side) before anything depends on it, so all results are
+// deterministic (two entries with the same key are the same pair listed twice: bit-identical contributions).
 //   ent[slot] = (partner triangle, side | recorded config of the canonical pair << 1)
 __global__ void __launch_bounds__(CLS_THREADS)
 k_compact(const uint32_t* __restrict__ mask, const int* __restrict__ blk_off, int64_t P,
-          int* __restrict__ active_ids, const int2* __restrict__ pairs, const uint64_t* __restrict__ rec,
-          const int* __restrict__ tptr, uint2* __restrict__ ent) {
+          int* __restrict__ active_ids, const int2* __restrict__ pairs, const uint16_t* __restrict__ rec,
+          const int* __restrict__ tptr, uint2* __restrict__ ent, int* __restrict__ fill) {
   const int64_t k = (int64_t)blockIdx.x * CLS_THREADS + threadIdx.x;
   const int w = threadIdx.x >> 5, l = threadIdx.x & 31;
   const int64_t word0 = (int64_t)blockIdx.x * (CLS_THREADS / 32);
@@ -232,10 +228,9 @@ k_compact(const uint32_t* __restrict__ mask, const int* __restrict__ blk_off, in
       // streaming loads / stores for everything that is touched once, so that the 8-byte scattered
       // stores of the entries find their lines still in L2 when the line's other entries arrive
       const int2 pr = __ldcs(pairs + k);
-      const unsigned long long r = __ldcs(rec + k);
-      const unsigned c = (unsigned)(r & REC_CFG_MASK) << 1;
-      const int sa = __ldg(tptr + pr.x) + (int)((r >> REC_P0_SHIFT) & REC_P_MASK);
-      const int sb = __ldg(tptr + pr.y) + (int)((r >> REC_P1_SHIFT) & REC_P_MASK);
+      const unsigned c = (unsigned)__ldcs(rec + k) << 1;
+      const int sa = __ldg(tptr + pr.x) + atomicAdd(fill + pr.x, 1);
+      const int sb = __ldg(tptr + pr.y) + atomicAdd(fill + pr.y, 1);
       ent[sa] = make_uint2((unsigned)pr.y, c);
       ent[sb] = make_uint2((unsigned)pr.x, c | 1u);
     }

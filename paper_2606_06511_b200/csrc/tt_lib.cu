@@ -270,14 +270,14 @@ tt_status run_classify(tt_ctx* ctx, const tt_problem* q, T* e_pp, T* tc, bool re
   TT_CUDA(ctx->blk_energy.ensure(sizeof(double) * (size_t)(nblk + 1)));
   TT_CUDA(ctx->counts.ensure(sizeof(int64_t) * 16));
   TT_CUDA(ctx->energy.ensure(sizeof(double) * 2));
-  if (record) TT_CUDA(ctx->rec.ensure(sizeof(uint64_t) * (size_t)(P + 1)));
+  if (record) TT_CUDA(ctx->rec.ensure(sizeof(uint16_t) * (size_t)(P + 2)));
   TT_CUDA(cudaMemsetAsync(ctx->blk_count.as<int>() + nblk, 0, sizeof(int), st));
   if (nblk > 0) {
     cudaEvent_t* ev_k1 = ctx->evr[0][ctx->ev_n[0] % tt_ctx::EV_RING];
     TT_CUDA(cudaEventRecord(ev_k1[0], st));
     ttk::k_classify<T><<<(unsigned)nblk, ttk::CLS_THREADS, 0, st>>>(
         (const T*)q->pos, q->tris, (const int2*)q->pairs, P, ctx->opt.tc_scale, ctx->mask.as<uint32_t>(),
-        ctx->blk_count.as<int>(), ctx->blk_energy.as<double>(), e_pp, tc, record ? ctx->rec.as<uint64_t>() : nullptr, deg);
+        ctx->blk_count.as<int>(), ctx->blk_energy.as<double>(), e_pp, tc, record ? ctx->rec.as<uint16_t>() : nullptr, deg);
     TT_LAUNCH_CHECK();
     TT_CUDA(cudaEventRecord(ev_k1[1], st));
     ctx->ev_n[0]++;
@@ -356,16 +356,17 @@ tt_status symbolic_impl(tt_ctx* ctx, const tt_problem* q, int64_t* nnzb_host, in
   const int64_t n_ub = 2 * P;
   const int64_t touched_ub = nT < n_ub ? nT : n_ub;
   const int64_t slots_ub = touched_ub + n_ub / 8 + 8;
-  // ---- one zeroed block: deg [nT+1], vcnt [nV+1], rowlen [nV+1] ----
-  const size_t zints = (size_t)(nT + 1) + 2 * (size_t)(nV + 1);
+  // ---- one zeroed block: deg [nT+1], vcnt [nV+1], rowlen [nV+1], fill [nT+1] ----
+  const size_t zints = (size_t)(nT + 1) + 2 * (size_t)(nV + 1) + (size_t)(nT + 1);
   TT_CUDA(ctx->zero_blk.ensure(sizeof(int) * zints));
   TT_CUDA(cudaMemsetAsync(ctx->zero_blk.p, 0, sizeof(int) * zints, st));
   int* deg = ctx->zero_blk.as<int>();
   int* vcnt = deg + (nT + 1);
   int* rowlen = vcnt + (nV + 1);
+  int* fill = rowlen + (nV + 1);
   ctx->vcnt_p = vcnt;
   ctx->rowlen_p = rowlen;
-  // ---- K1: classification, recorded decisions, degree histogram + place of every entry in its segment ----
+  // ---- K1: classification, recorded decisions, degree histogram ----
   s = run_classify<T>(ctx, q, nullptr, nullptr, true, deg, st, &nblk);
   if (s != TT_OK) return s;
   int64_t* d_counts = ctx->counts.as<int64_t>();
@@ -381,8 +382,8 @@ tt_status symbolic_impl(tt_ctx* ctx, const tt_problem* q, int64_t* nnzb_host, in
   TT_CUDA(ctx->dvals.ensure(sizeof(uint16_t) * (size_t)(n_ub + 2)));
   if (nblk > 0) {
     k_compact<<<(unsigned)nblk, CLS_THREADS, 0, st>>>(ctx->mask.as<uint32_t>(), ctx->blk_off.as<int>(), P, ctx->active_ids.as<int>(),
-                                                      (const int2*)q->pairs, ctx->rec.as<uint64_t>(), ctx->tptr.as<int>(),
-                                                      ctx->ent_in.as<uint2>());
+                                                      (const int2*)q->pairs, ctx->rec.as<uint16_t>(), ctx->tptr.as<int>(),
+                                                      ctx->ent_in.as<uint2>(), fill);
     TT_LAUNCH_CHECK();
   }
   // ---- touched triangles, vertex use counts, the work partition (slots, rounds) shared by the symbolic
