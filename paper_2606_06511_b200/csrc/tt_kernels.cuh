@@ -509,7 +509,7 @@ struct PackAdd {
   }
 };
 // sinfo[slot] = (touched index | SLOT_PART, unit offset of the part inside its triangle's row run, part ordinal
-// or -1, unused).  A unit is a group of 3 columns: entry j of a split triangle is unit j + (j >= pos_d), the
+// or -1, the triangle's id).  A unit is a group of 3 columns: entry j of a split triangle is unit j + (j >= pos_d), the
 // diagonal columns are unit pos_d.
 
 // tfirst[i] = first directed entry of touched triangle i; tfirst[n_touched] = n_dir
@@ -582,7 +582,7 @@ k_long_prep(const int* __restrict__ tris, const int* __restrict__ touched, const
 // FILL = true : round descriptors (first entry, entries, first slot, slots), slot tables, the list of
 //               long (unsplittable) rounds and the list of split triangles, at the offsets bucket_off[b].
 template <bool FILL>
-__global__ void k_chunk_pack(const int* __restrict__ tfirst, const int* __restrict__ n_touched_dev,
+__global__ void k_chunk_pack(const int* __restrict__ touched, const int* __restrict__ tfirst, const int* __restrict__ n_touched_dev,
                              const int* __restrict__ tsplit, PackCount* __restrict__ bucket_cnt,
                              const PackCount* __restrict__ bucket_off, int4* __restrict__ rdesc,
                              int* __restrict__ long_list, int* __restrict__ sfirst, int4* __restrict__ sinfo,
@@ -611,7 +611,7 @@ __global__ void k_chunk_pack(const int* __restrict__ tfirst, const int* __restri
   auto add_slot = [&](int e_begin, int cnt, int ti_flag, int u0, int pidx) {
     if (FILL) {
       sfirst[base.slots + nslot] = e_begin;
-      sinfo[base.slots + nslot] = make_int4(ti_flag, u0, pidx, 0);
+      sinfo[base.slots + nslot] = make_int4(ti_flag, u0, pidx, touched[ti_flag & ~SLOT_PART]);
     }
     ++nslot;
     ent += cnt;
@@ -785,19 +785,40 @@ k_round_symbolic(const int* __restrict__ tris, const int* __restrict__ touched, 
   unsigned long long* skey = s_key[warp];
   uint2* sent = s_ent[warp];
   const int64_t n_chunks = *n_chunks_dev;
-  for (int64_t c = (int64_t)blockIdx.x * RSYM_WARPS + warp; c < n_chunks; c += (int64_t)gridDim.x * RSYM_WARPS) {
-    const int4 d = __ldg(rdesc + c);
+  const int64_t stride = (int64_t)gridDim.x * RSYM_WARPS;
+  // The head of a round is a chain of dependent loads (descriptor -> slot table -> vertex ids); the descriptor
+  // and the slot rows of the NEXT round are requested while this one is worked on, so that a round starts
+  // one load (the triangles' vertex ids) away from its data instead of three.
+  const int4 dzero = make_int4(0, 0, 0, 0);
+  int64_t c = (int64_t)blockIdx.x * RSYM_WARPS + warp;
+  int4 d = (c < n_chunks) ? __ldg(rdesc + c) : dzero;
+  int4 psi = make_int4(0, 0, -1, 0);
+  int pf = 0, pl = 0;
+  auto fetch_slots = [&](const int4 dd) {  // slot rows of a round (lane = slot); nothing for a long round
+    psi = make_int4(0, 0, -1, 0);
+    pf = pl = 0;
+    if (dd.y <= RND_MAX_ENT && lane < dd.w) {
+      psi = __ldg(sinfo + dd.z + lane);
+      pf = __ldg(sfirst + dd.z + lane);
+      pl = __ldg(sfirst + dd.z + lane + 1);
+    }
+  };
+  fetch_slots(d);
+  for (; c < n_chunks; c += stride) {
+    const int4 d_next = (c + stride < n_chunks) ? __ldg(rdesc + c + stride) : dzero;
     const int e_lo = d.x, nent = d.y, s_lo = d.z, nsl = d.w;
-    if (nent > RND_MAX_ENT) continue;  // long triangle: k_tri_symbolic
+    if (nent > RND_MAX_ENT) {  // long triangle: k_tri_symbolic
+      d = d_next;
+      fetch_slots(d);
+      continue;
+    }
     // ---- lane = slot ----
     int f = 0, l = 0, ov[3] = {0, 0, 0};
-    int4 si = make_int4(0, 0, -1, 0);
+    const int4 si = psi;
     if (lane < nsl) {
-      si = __ldg(sinfo + s_lo + lane);
-      const int s = __ldg(touched + (si.x & ~SLOT_PART));
-      f = __ldg(sfirst + s_lo + lane) - e_lo;
-      l = __ldg(sfirst + s_lo + lane + 1) - e_lo;
-      load3i(tris + 3 * (int64_t)s, ov);
+      f = pf - e_lo;
+      l = pl - e_lo;
+      load3i(tris + 3 * (int64_t)si.w, ov);
 #pragma unroll
       for (int n = 0; n < 3; ++n) own[3 * lane + n] = ov[n];
       first[lane] = f;
@@ -985,6 +1006,8 @@ k_round_symbolic(const int* __restrict__ tris, const int* __restrict__ touched, 
       }
     }
     __syncwarp();  // shared memory is reused by the next round
+    d = d_next;
+    fetch_slots(d);
   }
 }
 
@@ -1041,9 +1064,8 @@ k_round_fill(const int* __restrict__ tris, const int* __restrict__ touched, cons
   if (lane < nsl) {
     const int64_t sl = (int64_t)s_lo + lane;
     const int ti = si.x & ~SLOT_PART;
-    const int s = __ldg(touched + ti);
     int ov[3];
-    load3i(tris + 3 * (int64_t)s, ov);
+    load3i(tris + 3 * (int64_t)si.w, ov);  // sinfo carries the triangle's id: one load less in the chain
     ubase[lane] = ub;
     if (!is_part) {
       utt[ub + (l - f)] = (unsigned char)lane;  // the diagonal's unit closes the run

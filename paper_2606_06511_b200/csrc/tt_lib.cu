@@ -435,7 +435,7 @@ tt_status symbolic_impl(tt_ctx* ctx, const tt_problem* q, int64_t* nnzb_host, in
           ctx->partner.as<int>(), ctx->dvals.as<uint16_t>(), ctx->tsplit.as<int>());
       TT_LAUNCH_CHECK();
     }
-    k_chunk_pack<false><<<grid_for(buckets_ub, 128), 128, 0, st>>>(ctx->tfirst.as<int>(), d_num, ctx->tsplit.as<int>(),
+    k_chunk_pack<false><<<grid_for(buckets_ub, 128), 128, 0, st>>>(ctx->touched.as<int>(), ctx->tfirst.as<int>(), d_num, ctx->tsplit.as<int>(),
                                                                   ctx->bucket_cnt.as<PackCount>(), nullptr, nullptr, nullptr,
                                                                   nullptr, nullptr, nullptr);
     TT_LAUNCH_CHECK();
@@ -449,7 +449,7 @@ tt_status symbolic_impl(tt_ctx* ctx, const tt_problem* q, int64_t* nnzb_host, in
                                              PackAdd(), zero, buckets_ub + 1, st));
       ctx->launches += 2;
     }
-    k_chunk_pack<true><<<grid_for(buckets_ub, 128), 128, 0, st>>>(ctx->tfirst.as<int>(), d_num, ctx->tsplit.as<int>(), nullptr,
+    k_chunk_pack<true><<<grid_for(buckets_ub, 128), 128, 0, st>>>(ctx->touched.as<int>(), ctx->tfirst.as<int>(), d_num, ctx->tsplit.as<int>(), nullptr,
                                                                  ctx->bucket_off.as<PackCount>(), ctx->rdesc.as<int4>(),
                                                                  ctx->long_list.as<int>(), ctx->sfirst.as<int>(),
                                                                  ctx->sinfo.as<int4>(), ctx->split_list.as<int4>());
