@@ -97,9 +97,10 @@ typedef struct {
 #define TT_FLAG_VALIDATE_INDICES 2
 /* tt_energy_grad_hess and tt_hess_vec replay the branch decisions (lone vertex, min/max order,
  * on-plane flag, active mask) that tt_hess_symbolic recorded at the positions it saw.  By default
- * both calls re-take a 64-bit checksum of `pos` (one read of the array, ~0.03 ms per 6 M vertices,
- * plus one short host round trip) and return TT_ERR_STATE if the positions have changed since
- * tt_hess_symbolic.  This flag skips the check: the caller then guarantees unchanged positions
+ * both calls re-take a 64-bit checksum of `pos` (one read of the array, ~0.03 ms per 6 M vertices;
+ * the call enqueues its kernels and then waits for the checksum only, so the GPU does not idle) and
+ * return TT_ERR_STATE if the positions have changed since tt_hess_symbolic -- the outputs of such a
+ * call are not valid.  This flag skips the check: the caller then guarantees unchanged positions
  * (tt_pcg_solve checks once per solve, not per product).                                          */
 #define TT_FLAG_NO_STATE_CHECK 4
 
@@ -138,8 +139,8 @@ tt_status tt_hess_pattern(tt_ctx* ctx, const int32_t** rowptr, const int32_t** c
 
 /* Steps 2-4 (Eq. 2-4), numeric phase, on the active set cached by tt_hess_symbolic for
  * the same problem (same pointers and sizes, and unchanged positions: TT_ERR_STATE otherwise --
- * the positions are verified by checksum unless TT_FLAG_NO_STATE_CHECK, which makes this call block
- * for one short host round trip before its kernels are enqueued).
+ * the positions are verified by checksum unless TT_FLAG_NO_STATE_CHECK: the call returns once the
+ * checksum, enqueued ahead of its kernels, has been read back).
  *   energy_sum [1] dtype; grad [nV,3] dtype or NULL;
  *   bsr_rowptr [nV+1], bsr_colind [nnzb_capacity], bsr_vals [nnzb_capacity,3,3] dtype -- all
  *   three NULL to skip the Hessian.  TT_ERR_CAPACITY if nnzb_capacity < nnzb.                     */

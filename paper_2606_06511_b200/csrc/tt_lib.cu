@@ -105,7 +105,8 @@ struct tt_ctx {
   int64_t ev_n[3] = {0, 0, 0};   // launches recorded since the last reset
   // host-buffer entry point: copies that do not feed the next kernel travel on a second stream
   cudaStream_t side = nullptr;
-  cudaEvent_t ev_in = nullptr, ev_p = nullptr, ev_num = nullptr, ev_side = nullptr;
+  cudaEvent_t ev_in = nullptr, ev_p = nullptr, ev_num = nullptr, ev_side = nullptr, ev_sig = nullptr;
+  unsigned long long* h_sig = nullptr;  // pinned [2]: the two position checksums, read back without stalling the stream
 };
 
 namespace {
@@ -195,17 +196,33 @@ tt_status pos_checksum(tt_ctx* ctx, const tt_problem* q, int slot, cudaStream_t 
   }
   return TT_OK;
 }
-// TT_ERR_STATE unless pos still has the checksum tt_hess_symbolic took (one short host round trip)
-tt_status check_positions(tt_ctx* ctx, const tt_problem* q, const char* who, cudaStream_t st) {
+// The position check of the numeric / H.p calls, in two halves so that the GPU never waits for the host:
+//   begin: enqueue the checksum of the current positions and its read-back into pinned memory, record an event;
+//   (the caller then enqueues its kernels)
+//   end:   wait for THAT EVENT only and compare with the checksum tt_hess_symbolic took -> TT_ERR_STATE.
+// If the positions have moved, the kernels that were enqueued in between replay stale branch decisions: they
+// cannot fault (every index is fixed by the symbolic phase) and the call returns the error, so its outputs are
+// simply not valid -- as for any failed call.
+tt_status check_positions_begin(tt_ctx* ctx, const tt_problem* q, cudaStream_t st) {
   if (ctx->opt.flags & TT_FLAG_NO_STATE_CHECK) return TT_OK;
   tt_status s = pos_checksum(ctx, q, 1, st);
   if (s != TT_OK) return s;
-  unsigned long long sig[2] = {0ull, 0ull};
-  TT_CUDA(cudaMemcpyAsync(sig, ctx->possig.p, sizeof(sig), cudaMemcpyDeviceToHost, st));
-  TT_CUDA(cudaStreamSynchronize(st));
-  if (sig[0] != sig[1])
+  TT_CUDA(cudaMemcpyAsync(ctx->h_sig, ctx->possig.p, 2 * sizeof(unsigned long long), cudaMemcpyDeviceToHost, st));
+  TT_CUDA(cudaEventRecord(ctx->ev_sig, st));
+  return TT_OK;
+}
+tt_status check_positions_end(tt_ctx* ctx, const char* who) {
+  if (ctx->opt.flags & TT_FLAG_NO_STATE_CHECK) return TT_OK;
+  TT_CUDA(cudaEventSynchronize(ctx->ev_sig));
+  if (ctx->h_sig[0] != ctx->h_sig[1])
     return fail(ctx, TT_ERR_STATE, "%s: positions changed since tt_hess_symbolic (the cached active set and branch decisions are stale): call tt_hess_symbolic again", who);
   return TT_OK;
+}
+// the same in one piece, for callers that must know before they enqueue anything (tt_pcg_solve)
+tt_status check_positions(tt_ctx* ctx, const tt_problem* q, const char* who, cudaStream_t st) {
+  tt_status s = check_positions_begin(ctx, q, st);
+  if (s != TT_OK) return s;
+  return check_positions_end(ctx, who);
 }
 
 // exclusive sum of n ints (+ grand total in out[n]); `in` must have n+1 entries with in[n] == 0
@@ -1060,7 +1077,9 @@ tt_status tt_create(const tt_options* opt, tt_ctx** out) {
       cudaEventCreateWithFlags(&c->ev_in, cudaEventDisableTiming) != cudaSuccess ||
       cudaEventCreateWithFlags(&c->ev_p, cudaEventDisableTiming) != cudaSuccess ||
       cudaEventCreateWithFlags(&c->ev_num, cudaEventDisableTiming) != cudaSuccess ||
-      cudaEventCreateWithFlags(&c->ev_side, cudaEventDisableTiming) != cudaSuccess) {
+      cudaEventCreateWithFlags(&c->ev_side, cudaEventDisableTiming) != cudaSuccess ||
+      cudaEventCreateWithFlags(&c->ev_sig, cudaEventDisableTiming) != cudaSuccess ||
+      cudaMallocHost((void**)&c->h_sig, 2 * sizeof(unsigned long long)) != cudaSuccess) {
     (void)cudaGetLastError();
     tt_destroy(c);
     return TT_ERR_CUDA;
@@ -1111,8 +1130,9 @@ void tt_destroy(tt_ctx* ctx) {
     for (int r = 0; r < tt_ctx::EV_RING; ++r)
       for (int j = 0; j < 2; ++j)
         if (ctx->evr[i][r][j]) cudaEventDestroy(ctx->evr[i][r][j]);
-  for (cudaEvent_t e : {ctx->ev_in, ctx->ev_p, ctx->ev_num, ctx->ev_side})
+  for (cudaEvent_t e : {ctx->ev_in, ctx->ev_p, ctx->ev_num, ctx->ev_side, ctx->ev_sig})
     if (e) cudaEventDestroy(e);
+  if (ctx->h_sig) cudaFreeHost(ctx->h_sig);
   if (ctx->side) cudaStreamDestroy(ctx->side);
   delete ctx;
 }
@@ -1148,11 +1168,13 @@ tt_status tt_energy_grad_hess(tt_ctx* ctx, const tt_problem* prob, void* energy_
   if (!ctx->sig.matches(prob)) return fail(ctx, TT_ERR_STATE, "tt_energy_grad_hess: no matching tt_hess_symbolic for this problem");
   TT_CUDA(cudaSetDevice(ctx->opt.device));
   cudaStream_t st = (cudaStream_t)stream;
-  s = check_positions(ctx, prob, "tt_energy_grad_hess", st);
+  s = check_positions_begin(ctx, prob, st);
   if (s != TT_OK) return s;
-  return ctx->opt.dtype == TT_F64
-             ? numeric_impl<double>(ctx, prob, energy_sum, grad, bsr_rowptr, bsr_colind, bsr_vals, nnzb_capacity, st)
-             : numeric_impl<float>(ctx, prob, energy_sum, grad, bsr_rowptr, bsr_colind, bsr_vals, nnzb_capacity, st);
+  s = ctx->opt.dtype == TT_F64
+          ? numeric_impl<double>(ctx, prob, energy_sum, grad, bsr_rowptr, bsr_colind, bsr_vals, nnzb_capacity, st)
+          : numeric_impl<float>(ctx, prob, energy_sum, grad, bsr_rowptr, bsr_colind, bsr_vals, nnzb_capacity, st);
+  const tt_status s_pos = check_positions_end(ctx, "tt_energy_grad_hess");
+  return s_pos != TT_OK ? s_pos : s;
 }
 
 tt_status tt_hess_vec(tt_ctx* ctx, const tt_problem* prob, const void* p, void* y, void* stream) {
@@ -1162,9 +1184,11 @@ tt_status tt_hess_vec(tt_ctx* ctx, const tt_problem* prob, const void* p, void* 
   if (!ctx->sig.matches(prob)) return fail(ctx, TT_ERR_STATE, "tt_hess_vec: no matching tt_hess_symbolic for this problem");
   TT_CUDA(cudaSetDevice(ctx->opt.device));
   cudaStream_t st = (cudaStream_t)stream;
-  s = check_positions(ctx, prob, "tt_hess_vec", st);
+  s = check_positions_begin(ctx, prob, st);
   if (s != TT_OK) return s;
-  return ctx->opt.dtype == TT_F64 ? hessvec_impl<double>(ctx, prob, p, y, st) : hessvec_impl<float>(ctx, prob, p, y, st);
+  s = ctx->opt.dtype == TT_F64 ? hessvec_impl<double>(ctx, prob, p, y, st) : hessvec_impl<float>(ctx, prob, p, y, st);
+  const tt_status s_pos = check_positions_end(ctx, "tt_hess_vec");
+  return s_pos != TT_OK ? s_pos : s;
 }
 
 namespace {
