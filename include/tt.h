@@ -270,7 +270,8 @@ tt_status tt_untangle(tt_ctx* ctx, void* pos, int64_t n_verts, const int32_t* tr
  * general-row merge, [5]=merge records, [6]=nnzb, [7]=kernels launched by this ctx so far (CUB calls
  * counted by the kernels they launch), [8]=slots of the work partition, [9]=triangles with more than 32
  * partners that were split into parts, [10]=parts, [11]=such triangles that could not be split (rounds of
- * their own, long-triangle kernels).                                                                 */
+ * their own, long-triangle kernels), [12]=rounds of the work partition (one warp each in K4 / K6: a round holds at
+ * most 32 directed entries, so [1] / (32 [12]) is the lane fill).                                     */
 tt_status tt_stats(const tt_ctx* ctx, int64_t* what, int32_t n);
 
 /* Device durations (CUDA events on the caller's stream) of the most recent launch of the three

@@ -101,7 +101,7 @@ __device__ __noinline__ void pair_second_dir(const double (&x)[18], const double
 // entry order.
 namespace ttk {
 
-constexpr int EX_WARPS = 4;
+constexpr int EX_WARPS = (RND_MAX_TRI > 12) ? 2 : 4;
 constexpr int EX_NACC = 90;  // 9 own rows x 9 own columns (diagonal blocks) + 9 gradient values
 struct ExactWarpSmem {
   double stage[32 * 9];                // per entry: the 9 own-column values of the current row (or the gradient)

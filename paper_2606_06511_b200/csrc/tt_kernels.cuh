@@ -494,10 +494,20 @@ k_fill_rows(const int* __restrict__ tris, const int* __restrict__ touched, int64
 // Packing is greedy in touched order, restarted at every bucket of CHK_BUCKET touched triangles so that
 // buckets pack in parallel (one thread per bucket; count pass, scan, fill pass).
 constexpr int RND_MAX_ENT = 32;
+// Slots per round: at most RND_MAX_TRI (the capacity every per-round array is sized for).  The packing LIMIT of one
+// symbolic call is 16 or 8, chosen on the device from the mean number of entries per touched triangle: with one or
+// two partners per triangle (1-5 M pairs on BASELINE's 2 M-triangle soup) 8 slots fill a third of a round's 32
+// lanes; with five or more, rounds fill anyway and K4 runs 8 % faster with its per-slot loops unrolled 8 deep
+// (measured; K4 is instantiated for both, K6 and the symbolic kernels do not care).
 #ifndef TT_RND_MAX_TRI
-#define TT_RND_MAX_TRI 8
+#define TT_RND_MAX_TRI 16
 #endif
 constexpr int RND_MAX_TRI = TT_RND_MAX_TRI;
+constexpr int RND_TRI_LOW = 8;
+// limit = 16 iff  entries / touched < 3.5
+__host__ __device__ inline int round_tri_limit(int64_t n_entries, int64_t n_touched) {
+  return (RND_MAX_TRI > RND_TRI_LOW && 2 * n_entries < 7 * n_touched) ? RND_MAX_TRI : RND_TRI_LOW;
+}
 constexpr int CHK_BUCKET = 128;
 
 struct PackCount {  // per-bucket counts, scanned together
@@ -592,6 +602,7 @@ __global__ void k_chunk_pack(const int* __restrict__ touched, const int* __restr
   const int64_t n_buckets = (n_touched + CHK_BUCKET - 1) / CHK_BUCKET;
   if (b >= n_buckets) return;             // the counts of the buckets beyond stay zero
   const int64_t i0 = b * CHK_BUCKET, i1 = min(i0 + (int64_t)CHK_BUCKET, n_touched);
+  const int max_tri = round_tri_limit((int64_t)tfirst[n_touched], n_touched);
   PackCount base = PackCount{0, 0, 0, 0, 0};
   if (FILL) base = bucket_off[b];
   int nch = 0, nlong = 0, nslot = 0, nsplit = 0, npart = 0, ent = 0, tri = 0;
@@ -621,7 +632,7 @@ __global__ void k_chunk_pack(const int* __restrict__ touched, const int* __restr
     const int e_next = tfirst[i + 1];
     const int d = e_next - e_i;
     if (d <= RND_MAX_ENT) {
-      if (tri == 0 || ent + d > RND_MAX_ENT || tri + 1 > RND_MAX_TRI) open_round(e_i);
+      if (tri == 0 || ent + d > RND_MAX_ENT || tri + 1 > max_tri) open_round(e_i);
       add_slot(e_i, d, (int)i, 0, -1);
     } else {
       const int sp = tsplit[i];
@@ -630,7 +641,7 @@ __global__ void k_chunk_pack(const int* __restrict__ touched, const int* __restr
         if (FILL) long_list[base.longs + nlong] = base.rounds + nch - 1;
         ++nlong;
         add_slot(e_i, d, (int)i, 0, -1);
-        tri = RND_MAX_TRI;  // closes the round: the next slot opens a new one
+        tri = max_tri;  // closes the round: the next slot opens a new one
       } else {
         const int first_slot = nslot;
         if (FILL) split_list[base.splits + nsplit] = make_int4(base.slots + nslot, 0, (int)i, base.parts + npart);
@@ -639,7 +650,7 @@ __global__ void k_chunk_pack(const int* __restrict__ touched, const int* __restr
           int j = seg ? sp : 0;
           const int j1 = seg ? d : sp;
           while (j < j1) {
-            if (tri == 0 || ent >= RND_MAX_ENT || tri + 1 > RND_MAX_TRI) open_round(e_i + j);
+            if (tri == 0 || ent >= RND_MAX_ENT || tri + 1 > max_tri) open_round(e_i + j);
             const int take = min(j1 - j, RND_MAX_ENT - ent);
             add_slot(e_i + j, take, (int)i | SLOT_PART, j + seg, base.parts + npart);
             ++npart;
@@ -1226,10 +1237,10 @@ constexpr int STG_PASS = NSTG / 2;        // the 54 per-entry values are staged 
 constexpr int STG_STRIDE = STG_PASS;      // 27 doubles: odd, so lane = entry writes are conflict-free
 constexpr int LONG_STRIDE = 31;           // k_assemble_long: 27 + 3 staged values per entry, odd stride
 
-template <typename T>
+template <typename T, int MT>  // MT: slots per round this instantiation of K4 is built for
 struct TileCfg {
   static constexpr int RUN_UNIT = 27 * (int)sizeof(T);  // bytes one entry (or the diagonal) adds to a row run
-  static constexpr int TILE_BYTES = RUN_UNIT * (RND_MAX_ENT + RND_MAX_TRI) + 32 * RND_MAX_TRI;
+  static constexpr int TILE_BYTES = RUN_UNIT * (RND_MAX_ENT + MT) + 32 * MT;
   static constexpr int STAGE_BYTES = 32 * STG_STRIDE * (int)sizeof(double);
   static constexpr int UNION_BYTES = TILE_BYTES > STAGE_BYTES ? TILE_BYTES : STAGE_BYTES;
 };
@@ -1237,12 +1248,12 @@ struct TileCfg {
 // Shared memory of one warp.  `tile` holds, in turn, (1) the per-entry staging area of the
 // diagonal / gradient products and (2) the row tile the copy engine reads: the two never live at
 // the same time (the per-triangle sums move to `dsum` in between).
-template <typename T>
+template <typename T, int MT>
 struct alignas(16) TileWarpSmem {
-  unsigned char tile[TileCfg<T>::UNION_BYTES];
-  double dsum[RND_MAX_TRI][NSTG];         // per-triangle sums: 45 diagonal-block values + 9 gradient values
-  int run_off[RND_MAX_TRI];               // byte offset of the triangle's run in the tile (current row)
-  int diag_off[RND_MAX_TRI][3];           // byte offset of its diagonal block n in the tile (current row)
+  unsigned char tile[TileCfg<T, MT>::UNION_BYTES];
+  double dsum[MT][NSTG];                  // per-triangle sums: 45 diagonal-block values + 9 gradient values
+  int run_off[MT];                        // byte offset of the triangle's run in the tile (current row)
+  int diag_off[MT][3];                    // byte offset of its diagonal block n in the tile (current row)
 };
 // Pulls the (at most two) 32-byte sectors of each of six vertices into L2.
 template <typename T>
@@ -1309,14 +1320,14 @@ __device__ __forceinline__ void load_round_ops(const AsmParams<T>& P, const int4
 // split triangles (more than 32 partners); without any -- up to ~15 M pairs on BASELINE's 2 M-triangle soup -- the
 // instantiation without their code runs: the kernel sits at 254 of 255 registers and the few selects and the ballot
 // of the part path cost it 3 % (measured, profiles/r2_step_breakdown.md).
-template <typename T, bool PROJ, bool PARTS>
+template <typename T, bool PROJ, bool PARTS, int MT>
 __global__ void __maxnreg__(TT_TILE_MAXNREG)
 k_assemble_tile(const AsmParams<T> P) {
   extern __shared__ __align__(16) unsigned char s_raw[];
   constexpr unsigned FULL = 0xffffffffu;
-  constexpr int RUN_UNIT = TileCfg<T>::RUN_UNIT;
+  constexpr int RUN_UNIT = TileCfg<T, MT>::RUN_UNIT;
   const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-  TileWarpSmem<T>& S = reinterpret_cast<TileWarpSmem<T>*>(s_raw)[warp];
+  TileWarpSmem<T, MT>& S = reinterpret_cast<TileWarpSmem<T, MT>*>(s_raw)[warp];
   double* const stage = reinterpret_cast<double*>(S.tile);
   const int64_t G = (int64_t)gridDim.x * TILE_WARPS;
   int64_t c = (int64_t)blockIdx.x * TILE_WARPS + warp;
@@ -1382,7 +1393,7 @@ k_assemble_tile(const AsmParams<T> P) {
         int incl = (lane < ntri) ? (((run_bytes + 15) & ~15) + 16) : 0;
         const int mine = incl;
 #pragma unroll
-        for (int o = 1; o < RND_MAX_TRI; o <<= 1) {
+        for (int o = 1; o < MT; o <<= 1) {
           const int v = __shfl_up_sync(FULL, incl, o);
           if (lane >= o) incl += v;
         }
@@ -1515,15 +1526,15 @@ k_assemble_tile(const AsmParams<T> P) {
           const int r_ = 3 * m + cq / 3, c_ = 3 * cn + cq % 3;
           const int lo = min(r_, c_), hi = max(r_, c_);
           const int uidx = lo * 9 - (lo * (lo - 1)) / 2 + (hi - lo);
-          int off[RND_MAX_TRI];
-          T val[RND_MAX_TRI];
+          int off[MT];
+          T val[MT];
 #pragma unroll
-          for (int tt = 0; tt < RND_MAX_TRI; ++tt) {  // slots past ntri hold stale but readable data
+          for (int tt = 0; tt < MT; ++tt) {  // slots past ntri hold stale but readable data
             off[tt] = S.diag_off[tt][cn];
             val[tt] = (T)S.dsum[tt][uidx];
           }
 #pragma unroll
-          for (int tt = 0; tt < RND_MAX_TRI; ++tt)
+          for (int tt = 0; tt < MT; ++tt)
             if (tt < ntri && (!PARTS || off[tt] >= 0)) *reinterpret_cast<T*>(S.tile + off[tt] + cq * (int)sizeof(T)) = val[tt];
         }
         // positions of the next round (L2 hits): requested as soon as this round's J is dead

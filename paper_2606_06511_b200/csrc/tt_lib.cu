@@ -92,7 +92,8 @@ struct tt_ctx {
   int64_t A = 0, n_dir = 0, n_touched = 0, R = 0, U = 0, nnzb = 0, n_chunks = 0, n_long = 0, rows_excl = 0, rows_gen = 0;
   int64_t n_slots = 0, n_split = 0, n_parts = 0;
   int bitsT = 1, bitsV = 1, sms = 148;
-  int tile_grid[2] = {0, 0};  // persistent grid of k_assemble_tile<double / float>
+  int tile_grid[2][2] = {{0, 0}, {0, 0}};  // persistent grid of k_assemble_tile<double / float, MT = 8 / 16>
+  int tri_limit = 8;          // slots-per-round limit the last symbolic call packed with (ttk::round_tri_limit)
   int pipe_grid[2][2] = {{0, 0}, {0, 0}};  // persistent grid of k_entry_pipe<double / float, MODE 1 / 2>
   uint64_t* rkeys_sorted = nullptr;
   uint32_t* rvals_sorted = nullptr;
@@ -526,6 +527,7 @@ tt_status symbolic_impl(tt_ctx* ctx, const tt_problem* q, int64_t* nnzb_host, in
   ctx->n_touched = n_touched;
   ctx->n_chunks = n_chunks;
   ctx->n_long = n_long;
+  ctx->tri_limit = round_tri_limit(n, n_touched);  // what k_chunk_pack packed with (same rule, same integers)
   if (R >= (int64_t(1) << 31)) return fail(ctx, TT_ERR_INVALID_ARG, "general-row workspace exceeds 2^31 blocks");
   ctx->R = R;
   const unsigned tri_grid = grid_for(n_slots, SYM_WARPS);
@@ -717,15 +719,23 @@ tt_status numeric_impl(tt_ctx* ctx, const tt_problem* q, void* energy_sum, void*
       tt_status s2 = launch_split_finish<T, true>(ctx, q, (T*)vals, st);
       if (s2 != TT_OK) return s2;
     } else if (want_h) {
-      const size_t smem = sizeof(TileWarpSmem<T>) * TILE_WARPS;
+      const bool wide = ctx->tri_limit > RND_TRI_LOW;  // which instantiation: per-slot loops unrolled 16 or 8 deep
+      const size_t smem = (wide ? sizeof(TileWarpSmem<T, RND_MAX_TRI>) : sizeof(TileWarpSmem<T, RND_TRI_LOW>)) * TILE_WARPS;
       const int64_t full = (ctx->n_chunks + TILE_WARPS - 1) / TILE_WARPS;
-      const int64_t pers = ctx->tile_grid[sizeof(T) == 8 ? 0 : 1];
+      const int64_t pers = ctx->tile_grid[sizeof(T) == 8 ? 0 : 1][wide ? 1 : 0];
       const unsigned grid = (unsigned)(full < pers ? full : pers);
       const bool proj = ctx->opt.hess_mode == TT_HESS_PSDPROJ, parts = ctx->n_parts > 0;
-      if (proj && parts) k_assemble_tile<T, true, true><<<grid, 32 * TILE_WARPS, smem, st>>>(p);
-      else if (proj) k_assemble_tile<T, true, false><<<grid, 32 * TILE_WARPS, smem, st>>>(p);
-      else if (parts) k_assemble_tile<T, false, true><<<grid, 32 * TILE_WARPS, smem, st>>>(p);
-      else k_assemble_tile<T, false, false><<<grid, 32 * TILE_WARPS, smem, st>>>(p);
+      const int which = (proj ? 4 : 0) | (parts ? 2 : 0) | (wide ? 1 : 0);
+      switch (which) {
+        case 0: k_assemble_tile<T, false, false, RND_TRI_LOW><<<grid, 32 * TILE_WARPS, smem, st>>>(p); break;
+        case 1: k_assemble_tile<T, false, false, RND_MAX_TRI><<<grid, 32 * TILE_WARPS, smem, st>>>(p); break;
+        case 2: k_assemble_tile<T, false, true, RND_TRI_LOW><<<grid, 32 * TILE_WARPS, smem, st>>>(p); break;
+        case 3: k_assemble_tile<T, false, true, RND_MAX_TRI><<<grid, 32 * TILE_WARPS, smem, st>>>(p); break;
+        case 4: k_assemble_tile<T, true, false, RND_TRI_LOW><<<grid, 32 * TILE_WARPS, smem, st>>>(p); break;
+        case 5: k_assemble_tile<T, true, false, RND_MAX_TRI><<<grid, 32 * TILE_WARPS, smem, st>>>(p); break;
+        case 6: k_assemble_tile<T, true, true, RND_TRI_LOW><<<grid, 32 * TILE_WARPS, smem, st>>>(p); break;
+        default: k_assemble_tile<T, true, true, RND_MAX_TRI><<<grid, 32 * TILE_WARPS, smem, st>>>(p); break;
+      }
       if (ctx->n_long > 0) {
         TT_LAUNCH_CHECK();
         k_assemble_long_tile<T, true><<<(unsigned)ctx->n_long, 32, sizeof(LongTileSmem<T, true>), st>>>(p);
@@ -1087,22 +1097,30 @@ tt_status tt_create(const tt_options* opt, tt_ctx** out) {
   {
     cudaError_t e = cudaSuccess;
     auto opt_in = [&](const void* f, size_t smem) { if (e == cudaSuccess) e = cudaFuncSetAttribute(f, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem); };
-    opt_in((const void*)ttk::k_assemble_tile<double, false, false>, sizeof(ttk::TileWarpSmem<double>) * ttk::TILE_WARPS);
-    opt_in((const void*)ttk::k_assemble_tile<double, false, true>, sizeof(ttk::TileWarpSmem<double>) * ttk::TILE_WARPS);
-    opt_in((const void*)ttk::k_assemble_tile<double, true, false>, sizeof(ttk::TileWarpSmem<double>) * ttk::TILE_WARPS);
-    opt_in((const void*)ttk::k_assemble_tile<double, true, true>, sizeof(ttk::TileWarpSmem<double>) * ttk::TILE_WARPS);
-    opt_in((const void*)ttk::k_assemble_tile<float, false, false>, sizeof(ttk::TileWarpSmem<float>) * ttk::TILE_WARPS);
-    opt_in((const void*)ttk::k_assemble_tile<float, false, true>, sizeof(ttk::TileWarpSmem<float>) * ttk::TILE_WARPS);
-    opt_in((const void*)ttk::k_assemble_tile<float, true, false>, sizeof(ttk::TileWarpSmem<float>) * ttk::TILE_WARPS);
-    opt_in((const void*)ttk::k_assemble_tile<float, true, true>, sizeof(ttk::TileWarpSmem<float>) * ttk::TILE_WARPS);
+    int sms = 0;
+    if (e == cudaSuccess) e = cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, opt->device);
+    auto tile_setup = [&](const void* f, size_t smem, int* grid) {  // opt in; persistent grid = one wave of resident CTAs
+      int nb = 0;
+      opt_in(f, smem);
+      if (grid && e == cudaSuccess) {
+        e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&nb, f, 32 * ttk::TILE_WARPS, smem);
+        *grid = sms * (nb > 0 ? nb : 1);
+      }
+    };
+#define TT_TILE_SETUP(T, DI, MT, MI)                                                                                        \
+    tile_setup((const void*)ttk::k_assemble_tile<T, false, false, MT>, sizeof(ttk::TileWarpSmem<T, MT>) * ttk::TILE_WARPS, nullptr); \
+    tile_setup((const void*)ttk::k_assemble_tile<T, false, true, MT>, sizeof(ttk::TileWarpSmem<T, MT>) * ttk::TILE_WARPS, nullptr);  \
+    tile_setup((const void*)ttk::k_assemble_tile<T, true, false, MT>, sizeof(ttk::TileWarpSmem<T, MT>) * ttk::TILE_WARPS, nullptr);  \
+    tile_setup((const void*)ttk::k_assemble_tile<T, true, true, MT>, sizeof(ttk::TileWarpSmem<T, MT>) * ttk::TILE_WARPS, &c->tile_grid[DI][MI]);
+    TT_TILE_SETUP(double, 0, ttk::RND_TRI_LOW, 0)
+    TT_TILE_SETUP(double, 0, ttk::RND_MAX_TRI, 1)
+    TT_TILE_SETUP(float, 1, ttk::RND_TRI_LOW, 0)
+    TT_TILE_SETUP(float, 1, ttk::RND_MAX_TRI, 1)
+#undef TT_TILE_SETUP
     opt_in((const void*)ttk::k_assemble_long_tile<double, true>, sizeof(ttk::LongTileSmem<double, true>));
     opt_in((const void*)ttk::k_assemble_long_tile<double, false>, sizeof(ttk::LongTileSmem<double, false>));
     opt_in((const void*)ttk::k_assemble_long_tile<float, true>, sizeof(ttk::LongTileSmem<float, true>));
     opt_in((const void*)ttk::k_assemble_long_tile<float, false>, sizeof(ttk::LongTileSmem<float, false>));
-        int sms = 0, nb0 = 0, nb1 = 0;
-    if (e == cudaSuccess) e = cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, opt->device);
-    if (e == cudaSuccess) e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&nb0, ttk::k_assemble_tile<double, true, true>, 32 * ttk::TILE_WARPS, sizeof(ttk::TileWarpSmem<double>) * ttk::TILE_WARPS);
-    if (e == cudaSuccess) e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&nb1, ttk::k_assemble_tile<float, true, true>, 32 * ttk::TILE_WARPS, sizeof(ttk::TileWarpSmem<float>) * ttk::TILE_WARPS);
     if (e != cudaSuccess) { (void)cudaGetLastError(); delete c; return TT_ERR_CUDA; }
     auto pipe_setup = [&](const void* f, size_t smem, int& grid) {
       int nb = 0;
@@ -1116,8 +1134,6 @@ tt_status tt_create(const tt_options* opt, tt_ctx** out) {
     pipe_setup((const void*)ttk::k_entry_pipe<float, 2>, sizeof(ttk::PipeWarpSmem<float, 2>) * ttk::PIPE_WARPS, c->pipe_grid[1][1]);
     if (e != cudaSuccess) { (void)cudaGetLastError(); delete c; return TT_ERR_CUDA; }
     c->sms = sms;
-    c->tile_grid[0] = sms * (nb0 > 0 ? nb0 : 1);  // one wave of resident CTAs: the kernel is persistent
-    c->tile_grid[1] = sms * (nb1 > 0 ? nb1 : 1);
   }
   *out = c;
   return TT_OK;
@@ -1428,9 +1444,9 @@ tt_status tt_bsr_device(tt_ctx* ctx, const int32_t** rowptr, const int32_t** col
 
 tt_status tt_stats(const tt_ctx* ctx, int64_t* what, int32_t n) {
   if (!ctx || !what || n < 0) return TT_ERR_INVALID_ARG;
-  const int64_t v[12] = {ctx->A, ctx->n_dir, ctx->n_touched, ctx->nnzb - ctx->U, ctx->U, ctx->R, ctx->nnzb, ctx->launches,
-                         ctx->n_slots, ctx->n_split, ctx->n_parts, ctx->n_long};
-  for (int i = 0; i < n && i < 12; ++i) what[i] = v[i];
+  const int64_t v[13] = {ctx->A, ctx->n_dir, ctx->n_touched, ctx->nnzb - ctx->U, ctx->U, ctx->R, ctx->nnzb, ctx->launches,
+                         ctx->n_slots, ctx->n_split, ctx->n_parts, ctx->n_long, ctx->n_chunks};
+  for (int i = 0; i < n && i < 13; ++i) what[i] = v[i];
   return TT_OK;
 }
 

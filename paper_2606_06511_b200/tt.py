@@ -321,10 +321,10 @@ class Context:
         return {k: float(arr[i]) for i, k in enumerate(names)}, {k: int(cnt[i]) for i, k in enumerate(names)}
 
     def tt_stats(self):
-        arr = (ctypes.c_int64 * 12)()
-        self._check(self.lib.tt_stats(self.h, arr, 12))
+        arr = (ctypes.c_int64 * 13)()
+        self._check(self.lib.tt_stats(self.h, arr, 13))
         keys = ["n_active", "n_directed", "n_touched_tris", "blocks_direct", "blocks_merged", "merge_records", "nnzb",
-                "launches", "n_slots", "split_triangles", "parts", "long_rounds"]
+                "launches", "n_slots", "split_triangles", "parts", "long_rounds", "rounds"]
         return dict(zip(keys, [int(v) for v in arr]))
 
 
