@@ -243,14 +243,20 @@ __device__ __forceinline__ unsigned long long entry_key(const uint2 e) {
 }
 
 // ------------------------------------------------------------------------------------------ K3
-// Segment pointers from sorted keys: ptr[g] = first entry whose (key >> shift) >= g, g = 0..G.
+// Segment pointers from sorted keys: ptr[g] = first entry whose (key >> shift) >= g, g = 0..G.  One thread per
+// GROUP, binary search (a thread per ENTRY that fills the groups between its key and its predecessor's walks
+// up to G groups alone when the keys are sparse: 147 us on the 1 M-triangle torus, measured, against 10 here).
 __global__ void k_segment_ptr(const uint64_t* __restrict__ keys, int64_t n, int shift, int64_t G,
                               int* __restrict__ ptr) {
-  const int64_t e = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
-  if (e > n) return;
-  const int64_t cur = (e < n) ? (int64_t)(keys[e] >> shift) : G;
-  const int64_t prev = (e > 0) ? (int64_t)(keys[e - 1] >> shift) : -1;
-  for (int64_t g = prev + 1; g <= cur; ++g) ptr[g] = (int)e;
+  const int64_t g = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (g > G) return;
+  int64_t lo = 0, hi = n;  // first e in [0, n] with (keys[e] >> shift) >= g
+  while (lo < hi) {
+    const int64_t mid = (lo + hi) >> 1;
+    if ((int64_t)(__ldg(keys + mid) >> shift) < g) lo = mid + 1;
+    else hi = mid;
+  }
+  ptr[g] = (int)lo;
 }
 
 // Touched triangles count their vertices (integer atomics: the RESULT is order independent).

@@ -623,7 +623,7 @@ tt_status symbolic_impl(tt_ctx* ctx, const tt_problem* q, int64_t* nnzb_host, in
     TT_LAUNCH_CHECK();
     s = sort_pairs(ctx, ctx->vkeys, ctx->vvals, nvs, 0, ceil_log2(nV + 1), &vkeys_sorted, &ctx->vvals_sorted, st);
     if (s != TT_OK) return s;
-    k_segment_ptr<<<grid_for(nvs + 1, 256), 256, 0, st>>>(vkeys_sorted, nvs, 0, nV, ctx->vptr.as<int>());
+    k_segment_ptr<<<grid_for(nV + 1, 256), 256, 0, st>>>(vkeys_sorted, nvs, 0, nV, ctx->vptr.as<int>());
     TT_LAUNCH_CHECK();
   }
 
