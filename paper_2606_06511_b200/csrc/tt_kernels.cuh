@@ -516,6 +516,113 @@ __host__ __device__ inline int round_tri_limit(int64_t n_entries, int64_t n_touc
 }
 constexpr int CHK_BUCKET = 128;
 
+// Layout order of the triangles' entry segments.  K4 / K6 give one warp to a ROUND of consecutive slots with at most
+// 32 directed entries, and a round costs the same whether 20 or 32 of its lanes work: what counts is the NUMBER of
+// rounds.  Packing the triangles in id order fills 80-85 % of the lanes once triangles have 10-25 partners (two
+// neighbours of 20 do not fit one round); nothing ties the segments to id order, though -- rows are addressed
+// through rowbase -- so every bucket of ORD_BUCKET consecutive triangle ids is re-ordered here by best-fit-decreasing
+// bin packing of the degrees into rounds of 32 (one thread per bucket), and the segments, the touched list, the
+// slots and the rounds follow that order.  Simulated on the soup's measured degrees: 18 % fewer rounds at 20 M
+// pairs, 11 % at 50 M, none below a mean degree of ~7 (there the 8-slot limit binds, not the 32 entries): such
+// buckets keep their id order.  Triangles with more than 32 partners go first (their parts fill rounds anyway).
+//   order[pos] = triangle id at layout position pos;  degp[pos] = its degree (degp[nT] = 0)
+constexpr int ORD_BUCKET = 128;
+__global__ void __launch_bounds__(64)
+k_bucket_order(const int* __restrict__ deg, int64_t nT, const int64_t* __restrict__ n_active_dev, int* __restrict__ order,
+               int* __restrict__ degp) {
+  const int64_t b = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  const int64_t n_buckets = (nT + ORD_BUCKET - 1) / ORD_BUCKET;
+  if (b == n_buckets) degp[nT] = 0;  // closes the scan (one extra thread)
+  if (2 * *n_active_dev < 7 * nT) {  // fewer than 7 entries per triangle overall: id order, as a coalesced copy
+    for (int64_t t = b; t < nT; t += (int64_t)gridDim.x * blockDim.x) {
+      order[t] = (int)t;
+      degp[t] = deg[t];
+    }
+    return;
+  }
+  if (b >= n_buckets) return;
+  const int64_t t0 = b * ORD_BUCKET;
+  const int n = (int)min((int64_t)ORD_BUCKET, nT - t0);
+  short d[ORD_BUCKET];
+  int sum = 0, touched = 0;
+  for (int i = 0; i < n; ++i) {
+    const int v = deg[t0 + i];
+    d[i] = (short)min(v, 32767);
+    sum += v;
+    touched += v > 0;
+  }
+  if (sum < 7 * touched || n < 4) {  // few partners per triangle (or nothing to pack): id order
+    for (int i = 0; i < n; ++i) {
+      order[t0 + i] = (int)(t0 + i);
+      degp[t0 + i] = deg[t0 + i];
+    }
+    return;
+  }
+  // stable counting sort by degree class (long first, then 32 .. 0)
+  unsigned char srt[ORD_BUCKET];
+  {
+    int cnt[34];
+    for (int k = 0; k < 34; ++k) cnt[k] = 0;
+    for (int i = 0; i < n; ++i) cnt[33 - min((int)d[i], 33)]++;   // class 0 = long, 1 = 32, ..., 33 = 0
+    int acc = 0;
+    for (int k = 0; k < 34; ++k) { const int c = cnt[k]; cnt[k] = acc; acc += c; }
+    for (int i = 0; i < n; ++i) srt[cnt[33 - min((int)d[i], 33)]++] = (unsigned char)i;
+  }
+  // best fit decreasing into rounds of RND_MAX_ENT entries and RND_TRI_LOW slots
+  unsigned char rnd_of[ORD_BUCKET], room[ORD_BUCKET], cnt_r[ORD_BUCKET];
+  short head[RND_MAX_ENT], nxt[ORD_BUCKET];   // open rounds by remaining room (singly linked)
+  for (int r = 0; r < RND_MAX_ENT; ++r) head[r] = -1;
+  int n_rounds = 0;
+  for (int k = 0; k < n; ++k) {
+    const int i = srt[k], di = d[i];
+    if (di > RND_MAX_ENT || di == 0) {  // long triangles first, untouched ones last: rounds of their own in this order
+      rnd_of[i] = (unsigned char)n_rounds;
+      room[n_rounds] = 0;
+      cnt_r[n_rounds] = RND_TRI_LOW;
+      ++n_rounds;
+      continue;
+    }
+    int r = di;
+    while (r < RND_MAX_ENT && head[r] < 0) ++r;
+    int q;
+    if (r < RND_MAX_ENT) {  // the open round with the least room that still takes it
+      q = head[r];
+      head[r] = nxt[q];
+    } else {
+      q = n_rounds++;
+      room[q] = RND_MAX_ENT;
+      cnt_r[q] = 0;
+    }
+    rnd_of[i] = (unsigned char)q;
+    room[q] = (unsigned char)(room[q] - di);
+    cnt_r[q]++;
+    if (room[q] > 0 && cnt_r[q] < RND_TRI_LOW) {
+      nxt[q] = head[room[q]];
+      head[room[q]] = (short)q;
+    }
+  }
+  // emit: rounds in creation order, members in placement order (stable counting sort by round)
+  {
+    short start[ORD_BUCKET];
+    for (int q = 0; q < n_rounds; ++q) start[q] = 0;
+    for (int i = 0; i < n; ++i) start[rnd_of[i]]++;
+    short acc = 0;
+    for (int q = 0; q < n_rounds; ++q) { const short c = start[q]; start[q] = acc; acc += c; }
+    for (int k = 0; k < n; ++k) {
+      const int i = srt[k];
+      const int pos = start[rnd_of[i]]++;
+      order[t0 + pos] = (int)(t0 + i);
+      degp[t0 + pos] = deg[t0 + i];
+    }
+  }
+}
+// segment starts by triangle id from the scan in layout order
+__global__ void k_scatter_tptr(const int* __restrict__ tptrp, const int* __restrict__ order, int64_t nT, int* __restrict__ tptr) {
+  const int64_t pos = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (pos < nT) tptr[order[pos]] = tptrp[pos];
+  if (pos == nT) tptr[nT] = tptrp[nT];
+}
+
 struct PackCount {  // per-bucket counts, scanned together
   int rounds, longs, slots, splits, parts;
 };

@@ -67,7 +67,7 @@ struct tt_ctx {
   // classification
   DevBuf mask, blk_count, blk_off, blk_energy, counts, energy, rec, sum_stage;
   // active set + directed entries
-  DevBuf active_ids, ent_in, partner, dvals, tptr, zero_blk, touched;
+  DevBuf active_ids, ent_in, partner, dvals, tptr, zero_blk, touched, order, degp, tptrp;
   // per-triangle symbolic
   DevBuf erank, drank, tlen, toff, slot_excl, rowbase;
   int* vcnt_p = nullptr;    // views into zero_blk (one memset per symbolic call)
@@ -390,9 +390,20 @@ tt_status symbolic_impl(tt_ctx* ctx, const tt_problem* q, int64_t* nnzb_host, in
   int64_t* d_counts = ctx->counts.as<int64_t>();
   k_set_count<<<1, 32, 0, st>>>(ctx->blk_off.as<int>(), ctx->blk_count.as<int>(), nblk, d_counts, nullptr);
   TT_LAUNCH_CHECK();
+  // ---- layout order of the entry segments (k_bucket_order), segment starts in that order, then by triangle id ----
   TT_CUDA(ctx->tptr.ensure(sizeof(int) * (size_t)(nT + 2)));
-  s = scan_i32(ctx, deg, ctx->tptr.as<int>(), nT + 1, st);  // tptr[nT] = directed entries = 2 A
+  TT_CUDA(ctx->order.ensure(sizeof(int) * (size_t)(nT + 2)));
+  TT_CUDA(ctx->degp.ensure(sizeof(int) * (size_t)(nT + 2)));
+  TT_CUDA(ctx->tptrp.ensure(sizeof(int) * (size_t)(nT + 2)));
+  {
+    const int64_t n_ord = (nT + ORD_BUCKET - 1) / ORD_BUCKET + 1;   // + the thread that closes degp
+    k_bucket_order<<<grid_for(n_ord, 64), 64, 0, st>>>(deg, nT, d_counts, ctx->order.as<int>(), ctx->degp.as<int>());
+    TT_LAUNCH_CHECK();
+  }
+  s = scan_i32(ctx, ctx->degp.as<int>(), ctx->tptrp.as<int>(), nT + 1, st);  // tptrp[nT] = directed entries = 2 A
   if (s != TT_OK) return s;
+  k_scatter_tptr<<<grid_for(nT + 1, 256), 256, 0, st>>>(ctx->tptrp.as<int>(), ctx->order.as<int>(), nT, ctx->tptr.as<int>());
+  TT_LAUNCH_CHECK();
   // ---- K2: compaction + counting-sort scatter of the directed entries by source triangle ----
   TT_CUDA(ctx->active_ids.ensure(sizeof(int) * (size_t)(P + 1)));
   TT_CUDA(ctx->ent_in.ensure(sizeof(uint2) * (size_t)(n_ub + 1)));
@@ -435,12 +446,14 @@ tt_status symbolic_impl(tt_ctx* ctx, const tt_problem* q, int64_t* nnzb_host, in
   if (touched_ub > 0) {
     k_vertex_touch<<<grid_for(nT, 256), 256, 0, st>>>(q->tris, deg, nT, vcnt);
     TT_LAUNCH_CHECK();
+    // touched triangles in LAYOUT order: the ids at the positions whose degree is not zero
     cub::CountingInputIterator<int> iota(0);
-    cub::TransformInputIterator<int, DegFlag, cub::CountingInputIterator<int>> flags(iota, DegFlag{deg});
+    cub::TransformInputIterator<int, DegFlag, cub::CountingInputIterator<int>> flags(iota, DegFlag{ctx->degp.as<int>()});
+    const int* ord = ctx->order.as<int>();
     size_t tmp = 0;
-    TT_CUDA(cub::DeviceSelect::Flagged(nullptr, tmp, iota, flags, ctx->touched.as<int>(), d_num, (int)nT, st));
+    TT_CUDA(cub::DeviceSelect::Flagged(nullptr, tmp, ord, flags, ctx->touched.as<int>(), d_num, (int)nT, st));
     TT_CUDA(ctx->cub_tmp.ensure(tmp));
-    TT_CUDA(cub::DeviceSelect::Flagged(ctx->cub_tmp.p, tmp, iota, flags, ctx->touched.as<int>(), d_num, (int)nT, st));
+    TT_CUDA(cub::DeviceSelect::Flagged(ctx->cub_tmp.p, tmp, ord, flags, ctx->touched.as<int>(), d_num, (int)nT, st));
     ctx->launches += 2;  // CUB select: init + sweep kernel
     k_touched_first<<<grid_for(touched_ub + 1, 256), 256, 0, st>>>(ctx->touched.as<int>(), d_num, ctx->tptr.as<int>(), nT,
                                                                    ctx->tfirst.as<int>());
