@@ -57,6 +57,9 @@ def parse():
     ap.add_argument("--hess-mode", type=int, default=1)
     ap.add_argument("--broad-phase", default=None, choices=["config2", "config3"],
                     help="time tt_broad_phase (SURVEY 8(f) NEXT-1) on that mesh instead of the hot path; prints its own JSON line")
+    ap.add_argument("--solver", action="store_true",
+                    help="time the consumer (SURVEY 8(f) NEXT-2) on the same workload instead of the hot path: tt_bsr_spmv "
+                         "against its HBM roofline, tt_pcg_solve iterations/s (assembled and matrix-free); prints its own JSON line")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     return ap.parse_args()
@@ -243,6 +246,58 @@ def run_broad_phase(args):
     ctx.close()
 
 
+def run_solver(args):
+    """Side measurement, not the headline: the consumer of the assembly on config 4 (or --config), inputs resident, CUDA events."""
+    import torch
+    from paper_2606_06511_b200 import tt
+    dev = torch.device("cuda", 0)
+    tdt = torch.float64 if args.dtype == "f64" else torch.float32
+    w = 8 if args.dtype == "f64" else 4
+    pb = make_problem(args, 0, "cuda:0")
+    ctx = tt.Context(tdt, 2, 1.0, 0)     # PSD2: H + mu I is SPD
+    pos_np = pb.pos if w == 8 else pb.pos.astype(np.float32)
+    out = tt.assemble(ctx, torch.from_numpy(pos_np).to(dev), torch.from_numpy(pb.tris).to(dev), torch.from_numpy(pb.pairs).to(dev))
+    nV, nnzb = pb.n_verts, out["nnzb"]
+    x = torch.randn((nV, 3), dtype=tdt, device=dev)
+    y = torch.empty_like(x)
+    stream = torch.cuda.current_stream()
+    hbm, peak_src = peaks()
+
+    def timed(fn, reps):
+        for _ in range(args.warmup):
+            fn()
+        torch.cuda.synchronize()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record(stream)
+        for _ in range(reps):
+            fn()
+        e1.record(stream)
+        torch.cuda.synchronize()
+        return e0.elapsed_time(e1) / reps
+
+    ms_spmv = timed(lambda: ctx.tt_bsr_spmv(out["rowptr"], out["colind"], out["vals"], x, y, 0.0), args.steps)
+    b_spmv = (9 * w + 4) * nnzb + 4 * (nV + 1) + 6 * w * nV          # values + colind, rowptr, x gathered once + y
+    diag = out["vals"][out["colind"] == torch.repeat_interleave(torch.arange(nV, device=dev), (out["rowptr"][1:] - out["rowptr"][:-1]).long())]
+    mu = float(diag.double().diagonal(dim1=1, dim2=2).sum(1).mean().item()) / 3 * 1e-2     # 1 % of the mean diagonal
+    minv = torch.empty((nV, 3, 3), dtype=tdt, device=dev)
+    ms_jac = timed(lambda: ctx.tt_block_jacobi(out["rowptr"], out["colind"], out["vals"], minv, mu), args.steps)
+    iters = 20
+    ms_pcg = timed(lambda: ctx.tt_pcg_solve(out["prob"], out["grad"], y, rowptr=out["rowptr"], colind=out["colind"], vals=out["vals"],
+                                            minv=minv, max_iter=iters, rtol=0.0, shift=mu, want_stats=False), max(2, args.steps // 4))
+    ms_pcg_mf = timed(lambda: ctx.tt_pcg_solve(out["prob"], out["grad"], y, max_iter=iters, rtol=0.0, shift=mu, want_stats=False),
+                      max(2, args.steps // 4))
+    print(json.dumps({"metric": "consumer: tt_bsr_spmv GB/s against the HBM roofline; tt_pcg_solve iterations/s", "n_gpus": 1,
+                      "dtype": args.dtype, "data": "synthetic", "steps": args.steps, "warmup": args.warmup,
+                      "config": {"workload": "BASELINE %s: %d triangles, %d candidate pairs, nnzb %d, PSD2 Hessian, shift %.3g" % (
+                          WORKLOADS[args.config], pb.n_tris, pb.n_pairs, nnzb, mu)},
+                      "spmv": {"ms": ms_spmv, "algorithmic_bytes": int(b_spmv), "achieved": b_spmv / (ms_spmv * 1e-3) / 1e9, "peak": hbm,
+                               "unit": "GB/s", "frac": b_spmv / (ms_spmv * 1e-3) / 1e9 / hbm, "peak_source": peak_src, "bound": "hbm"},
+                      "block_jacobi_ms": ms_jac,
+                      "pcg_assembled": {"iters": iters, "ms_per_solve": ms_pcg, "iters_per_s": iters / (ms_pcg * 1e-3)},
+                      "pcg_matrix_free": {"iters": iters, "ms_per_solve": ms_pcg_mf, "iters_per_s": iters / (ms_pcg_mf * 1e-3)}}), flush=True)
+    ctx.close()
+
+
 WORKLOADS = {0: "configs[0] 64-triangle soup, all pairs", 1: "configs[1] two icospheres, inflated-AABB candidates",
              2: "configs[2] folded cloth 256x256, inflated-AABB candidates", 3: "configs[3] twisted torus 1M triangles, AABB candidates",
              4: "configs[4] throughput sweep: random soup, seeded random candidate pairs"}
@@ -387,6 +442,9 @@ def main():
         return
     if args.broad_phase:
         run_broad_phase(args)
+        return
+    if args.solver:
+        run_solver(args)
         return
     if args.gpus > 1 and "WORLD_SIZE" not in os.environ:
         self_spawn(args)

@@ -29,7 +29,7 @@ struct PcgScalars {
 // One warp per block row; the lanes stride over the row's VALUES (9 per block), so the reads of `vals`
 // -- 9w of the (9w + 4) bytes a block costs -- are perfectly coalesced whatever the row length.  Value i
 // of the row belongs to block i / 9, element (r, c) = ((i % 9) / 3, i % 3), and adds vals[i] * x[3 col + c]
-// to component r.  Accumulation in fp64, fixed shuffle tree: deterministic.
+// to component r.  Accumulation in fp64, fixed order: deterministic.
 template <typename T>
 __global__ void __launch_bounds__(VEC_THREADS)
 k_bsr_spmv(const int* __restrict__ rowptr, const int* __restrict__ colind, const T* __restrict__ vals,
@@ -39,25 +39,34 @@ k_bsr_spmv(const int* __restrict__ rowptr, const int* __restrict__ colind, const
   const int64_t row = ((int64_t)blockIdx.x * VEC_THREADS + threadIdx.x) >> 5;
   if (row >= n_rows) return;
   const int64_t b0 = __ldg(rowptr + row), b1 = __ldg(rowptr + row + 1);
-  double a0 = 0.0, a1 = 0.0, a2 = 0.0;
-  for (int64_t i = 9 * b0 + lane; i < 9 * b1; i += 32) {
-    const int64_t blk = i / 9;
-    const int e = (int)(i - 9 * blk);
-    const int r = e / 3, c = e - 3 * r;
-    const double v = (double)__ldg(vals + i) * (double)__ldg(x + 3 * (int64_t)__ldg(colind + blk) + c);
-    a0 += (r == 0) ? v : 0.0;
-    a1 += (r == 1) ? v : 0.0;
-    a2 += (r == 2) ? v : 0.0;
+  // Lanes 0..26 walk the row THREE BLOCKS at a time: lane l always holds element (r, c) = ((l % 9) / 3, l % 3) of block
+  // 3 k + l / 9, so nothing about a value's place has to be computed inside the loop (a 32-wide stride needs a division by
+  // 9 and three predicated adds per value: with 64-bit indices that made 87 instructions per 32 values and the kernel was
+  // bound by instruction issue at 34 % of the HBM roofline -- ncu, profiles/r2_step_breakdown.md).  Reads of `vals` stay
+  // contiguous (27 consecutive values per trip) and are streamed (ld.global.cs): what is read once should not push x out
+  // of the L2.  Lanes 27..31 idle.
+  const int nb = (int)(b1 - b0);
+  const int bo = lane / 9, e = lane - 9 * bo, c = e % 3;
+  const T* __restrict__ vp = vals + 9 * b0 + lane;
+  const int* __restrict__ cp = colind + b0 + bo;
+  double acc = 0.0;
+  if (lane < 27) {
+#pragma unroll 2
+    for (int k = bo; k < nb; k += 3) {
+      acc = fma((double)__ldcs(vp), (double)__ldg(x + 3 * (int64_t)__ldg(cp) + c), acc);
+      vp += 27;
+      cp += 3;
+    }
   }
-#pragma unroll
-  for (int o = 16; o > 0; o >>= 1) {
-    a0 += __shfl_xor_sync(FULL, a0, o);
-    a1 += __shfl_xor_sync(FULL, a1, o);
-    a2 += __shfl_xor_sync(FULL, a2, o);
-  }
-  if (lane < 3) {
-    const double a = (lane == 0) ? a0 : ((lane == 1) ? a1 : a2);
-    y[3 * row + lane] = (T)(a + shift * (double)__ldg(x + 3 * row + lane));
+  // lane l < 9 collects element l of the three block slots (lanes l, l + 9, l + 18), then lanes 0, 3, 6 the three columns of
+  // rows 0, 1, 2: four shuffles in a fixed order (deterministic)
+  const double t1 = __shfl_down_sync(FULL, acc, 9), t2 = __shfl_down_sync(FULL, acc, 18);
+  const double s9 = acc + t1 + t2;
+  const double u1 = __shfl_down_sync(FULL, s9, 1), u2 = __shfl_down_sync(FULL, s9, 2);
+  const double tot = s9 + u1 + u2;
+  if (lane < 9 && e == 3 * (lane / 3)) {
+    const int rr = lane / 3;
+    y[3 * row + rr] = (T)(tot + shift * (double)__ldg(x + 3 * row + rr));
   }
 }
 
