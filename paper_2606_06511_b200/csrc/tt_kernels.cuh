@@ -2051,11 +2051,14 @@ k_entry_reduce(const AsmParams<T> P, const int* __restrict__ round_list, int64_t
 // cp.async (LDGSTS: no registers held while in flight) into lane-private slots, vertex ids one
 // round further ahead and descriptors two, so that the three dependent gathers of a round
 // (descriptor -> vertex ids -> positions) are all off the critical path.
+// One-warp CTAs: the kernel needs ~216 registers, and 9 x 32 x 216 fit the register file where 2 CTAs of 4 warps stop
+// at 8 warps (0.942 -> 0.893 ms at 10 M pairs, measured; asking ptxas for 9 CTAs makes it cap the kernel at 168
+// registers and spill: 1.30 ms -- so the bound below stays at 8 and the occupancy query finds the ninth).
 #ifndef TT_PIPE_WARPS
-#define TT_PIPE_WARPS 4
+#define TT_PIPE_WARPS 1
 #endif
 #ifndef TT_PIPE_MIN_CTAS
-#define TT_PIPE_MIN_CTAS 2
+#define TT_PIPE_MIN_CTAS 8
 #endif
 constexpr int PIPE_WARPS = TT_PIPE_WARPS;
 template <typename T, int MODE>
