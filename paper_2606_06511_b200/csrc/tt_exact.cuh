@@ -70,7 +70,10 @@ struct PairDir {
   double tc0, tc1, dtc0, dtc1;  // dtc_r = g_r . v
   double g0[18], g1[18], h0[18], h1[18];
 };
-__device__ __noinline__ void pair_second_dir(const double (&x)[18], const double (&v)[18], unsigned za, unsigned zb,
+// (inlined: the callers' loops are not unrolled, so there is one copy per kernel; assembly 47.7 -> 35.0 ms and H.p 4.7 ->
+// 4.0 ms at 10 M pairs against the out-of-line call, measured.  Folding the gradient pass into the first row pass was also
+// measured and is slower: 44 ms.)
+__device__ __forceinline__ void pair_second_dir(const double (&x)[18], const double (&v)[18], unsigned za, unsigned zb,
                                              double sigma, PairDir& o) {
   // local frame: translate by -a_k (the direction of a_k is subtracted with it)
   auto pt = [&](int i) {

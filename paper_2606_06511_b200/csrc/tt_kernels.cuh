@@ -514,7 +514,10 @@ constexpr int RND_TRI_LOW = 8;
 __host__ __device__ inline int round_tri_limit(int64_t n_entries, int64_t n_touched) {
   return (RND_MAX_TRI > RND_TRI_LOW && 2 * n_entries < 7 * n_touched) ? RND_MAX_TRI : RND_TRI_LOW;
 }
-constexpr int CHK_BUCKET = 128;
+#ifndef TT_CHK_BUCKET
+#define TT_CHK_BUCKET 128
+#endif
+constexpr int CHK_BUCKET = TT_CHK_BUCKET;
 
 // Layout order of the triangles' entry segments.  K4 / K6 give one warp to a ROUND of consecutive slots with at most
 // 32 directed entries, and a round costs the same whether 20 or 32 of its lanes work: what counts is the NUMBER of
