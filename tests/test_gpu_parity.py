@@ -191,6 +191,20 @@ def test_config4_sweep_reduced(oracle_mod, dtype):
     assert abs(out["n_active"] / pb.n_pairs - 0.5) < 0.01
 
 
+@pytest.mark.parametrize("n_tris,n_pairs,dtype", [(6000, 60_000, "f64"), (6000, 60_000, "f32"), (3000, 70_000, "f64")])
+def test_bin_packed_segment_order(oracle_mod, n_tris, n_pairs, dtype):
+    """10 and 23 partners per triangle on average: the entry segments are laid out in best-fit-decreasing order inside
+    buckets of 128 triangles (k_bucket_order) and, in the second case, mixed with triangles that are split into parts; the
+    matrix must not change (rows are addressed through rowbase) and the rounds must fill better than id order would."""
+    from paper_2606_06511_b200 import inputs
+    pb = inputs.config4_sweep(n_tris=n_tris, n_pairs=n_pairs, seed=777)
+    ref, out, st = run_case(oracle_mod, pb, dtype, 1)
+    assert st["blocks_merged"] == 0
+    assert st["n_directed"] / (32.0 * st["rounds"]) > 0.9          # lane fill (id order: ~0.80 at these degrees)
+    if n_tris == 3000:
+        assert st["split_triangles"] > 50
+
+
 @pytest.mark.parametrize("n_pairs,dtype", [(24_000, "f64"), (24_000, "f32"), (60_000, "f64")])
 @pytest.mark.parametrize("layout", ["soup", "shuffled"])
 def test_long_triangles(oracle_mod, n_pairs, dtype, layout):
