@@ -60,6 +60,9 @@ def parse():
     ap.add_argument("--solver", action="store_true",
                     help="time the consumer (SURVEY 8(f) NEXT-2) on the same workload instead of the hot path: tt_bsr_spmv "
                          "against its HBM roofline, tt_pcg_solve iterations/s (assembled and matrix-free); prints its own JSON line")
+    ap.add_argument("--untangle", action="store_true",
+                    help="run tt_untangle (broad phase + Newton step with line search, SURVEY 8(f) NEXT-2 / NEXT-4) on the mesh "
+                         "given by --config (1, 2 or 3) for --steps steps; prints its own JSON line")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     return ap.parse_args()
@@ -298,6 +301,39 @@ def run_solver(args):
     ctx.close()
 
 
+def run_untangle(args):
+    """Side measurement, not the headline: the untangling loop on a mesh config -- per step one tt_broad_phase, one symbolic +
+    numeric call, a block-Jacobi PCG solve and the Armijo line search on tt_energy.  Wall time per step (the loop synchronises
+    once per trial step length), energy and active-pair count along the way."""
+    import torch
+    from paper_2606_06511_b200 import inputs, tt
+    dev = torch.device("cuda", 0)
+    cfg = args.config if args.config in (1, 2, 3) else 1
+    pb = inputs.by_name("config%d" % cfg)
+    inflate = {1: 0.02, 2: 0.002, 3: 0.0}[cfg]
+    ctx = tt.Context(torch.float64, 2, 1.0, 0)     # PSD2
+    tris = torch.from_numpy(pb.tris).to(dev)
+    mu, iters = 1e-3, 30
+    pos = torch.from_numpy(pb.pos).to(dev).clone()
+    ctx.tt_untangle(pos, tris, inflate=inflate, max_steps=2, mu=mu, pcg_iter=iters)       # warm-up (workspace allocation)
+    pos = torch.from_numpy(pb.pos).to(dev).clone()
+    torch.cuda.synchronize()
+    t0 = time.perf_counter()
+    hist = ctx.tt_untangle(pos, tris, inflate=inflate, max_steps=args.steps, mu=mu, pcg_iter=iters)
+    torch.cuda.synchronize()
+    dt = time.perf_counter() - t0
+    disp = float((pos - torch.from_numpy(pb.pos).to(dev)).norm(dim=1).max())
+    print(json.dumps({"metric": "untangling loop (tt_untangle): ms per step, energy and active pairs along the way", "n_gpus": 1,
+                      "dtype": "f64", "data": "synthetic", "steps": len(hist),
+                      "config": {"workload": "BASELINE %s: %d triangles; inflate %g, PSD2, mu %g, %d PCG steps per Newton step" % (
+                          WORKLOADS[cfg], pb.n_tris, inflate, mu, iters)},
+                      "ms_per_step": 1e3 * dt / max(len(hist), 1), "all_accepted": all(h["accepted"] for h in hist),
+                      "n_pairs": [hist[0]["n_pairs"], hist[-1]["n_pairs"]], "n_active": [h["n_active"] for h in hist][::max(1, len(hist) // 10)],
+                      "energy": [hist[0]["energy0"]] + [h["energy1"] for h in hist][::max(1, len(hist) // 10)],
+                      "max_vertex_displacement": disp}), flush=True)
+    ctx.close()
+
+
 WORKLOADS = {0: "configs[0] 64-triangle soup, all pairs", 1: "configs[1] two icospheres, inflated-AABB candidates",
              2: "configs[2] folded cloth 256x256, inflated-AABB candidates", 3: "configs[3] twisted torus 1M triangles, AABB candidates",
              4: "configs[4] throughput sweep: random soup, seeded random candidate pairs"}
@@ -445,6 +481,9 @@ def main():
         return
     if args.solver:
         run_solver(args)
+        return
+    if args.untangle:
+        run_untangle(args)
         return
     if args.gpus > 1 and "WORLD_SIZE" not in os.environ:
         self_spawn(args)
