@@ -21,7 +21,7 @@ from __future__ import annotations
 
 import numpy as np
 
-from . import HESS_PSD2, assemble, pairs as _pairs
+from . import HESS_PSD2, assemble, broad_phase, pairs as _pairs
 
 
 def edges_of(tris) -> np.ndarray:
@@ -144,6 +144,9 @@ def newton_step(pos, rest, tris, pair_ids, k: float, hess_mode: int = HESS_PSD2,
     gd = float(np.sum(g * d))
     out = dict(x=pos.copy(), E0=E0, E1=E0, gnorm=float(np.linalg.norm(g)), gd=gd, alpha=0.0, backtracks=0, accepted=False,
                n_active=int(r["active"].sum()), d=d, E_membrane=Em)
+    if out["n_active"] == 0:        # reading A16: the loop's goal is "no pair is active"; nothing to do
+        out.update(accepted=True, d=np.zeros_like(pos), gd=0.0)
+        return out
     alpha = 1.0
     for j in range(max_backtrack + 1):
         x_try = pos - alpha * d
@@ -154,3 +157,18 @@ def newton_step(pos, rest, tris, pair_ids, k: float, hess_mode: int = HESS_PSD2,
         alpha *= 0.5
     out["backtracks"] = max_backtrack + 1
     return out
+
+
+def untangle(pos, rest, tris, k: float, inflate: float = 0.0, max_steps: int = 20, **kw) -> dict:
+    """oracle/newton.py's untangle with the membrane term in every step."""
+    x = np.ascontiguousarray(pos, dtype=np.float64).copy()
+    hist = []
+    for _ in range(max_steps):
+        cand = broad_phase(x, tris, inflate)
+        s = newton_step(x, rest, tris, cand, k, **kw)
+        hist.append(dict(E0=s["E0"], E1=s["E1"], alpha=s["alpha"], n_active=s["n_active"], n_pairs=int(cand.shape[0]),
+                         accepted=s["accepted"], x0=x, x1=s["x"]))
+        if s["n_active"] == 0 or not s["accepted"]:
+            break
+        x = s["x"]
+    return dict(x=x, history=hist)

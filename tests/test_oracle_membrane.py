@@ -109,3 +109,15 @@ def test_newton_step_with_membrane(oracle_mod):
     soft = mb.newton_step(pb.pos, pb.pos, pb.tris, pb.pairs, 1e-3, mu=1e-2, pcg_iter=50)
     stiff = mb.newton_step(pb.pos, pb.pos, pb.tris, pb.pairs, 1e3, mu=1e-2, pcg_iter=50)
     assert strain(stiff["x"]) < 0.05 * strain(soft["x"])
+
+
+def test_no_active_pair_is_a_fixed_point_and_untangle_stops(oracle_mod):
+    """Reading A16 (the loop ends when no pair is active) carried over to the membrane step: with an empty candidate list, or
+    one whose pairs are all apart, x is returned unchanged and accepted -- even when the membrane itself is strained."""
+    from oracle import membrane as mb
+    rest, tris, rng = mesh()
+    pos = 1.2 * rest
+    s = mb.newton_step(pos, rest, tris, np.zeros((0, 2), dtype=np.int32), 3.0)
+    assert s["accepted"] and s["n_active"] == 0 and s["alpha"] == 0.0 and (s["x"] == pos).all() and s["E_membrane"] > 0
+    r = mb.untangle(pos, rest, tris, 3.0, inflate=0.0, max_steps=5)
+    assert len(r["history"]) == 1 and (r["x"] == pos).all()
