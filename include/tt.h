@@ -248,6 +248,8 @@ typedef struct {
   int32_t max_backtrack;  /* >= 0: halvings of alpha after the full step                                            */
   int32_t matrix_free;    /* 0: assemble the BSR, block-Jacobi PCG; 1: CG on tt_hess_vec, no BSR, no preconditioner */
   tt_pcg_options pcg;     /* max_iter, rtol, check_every of the inner solve (its shift is ignored: mu is used)      */
+  int32_t membrane;       /* 0: E = E_T;  1: E = E_T + E_m, the mesh of the last tt_membrane_build (see below)      */
+  int32_t reserved;       /* 0                                                                                       */
 } tt_newton_options;
 typedef struct {
   double energy0, energy1;  /* E at x before / after the step (equal if rejected)                                   */
@@ -257,6 +259,7 @@ typedef struct {
   double pcg_relres;        /* |r|_2 / |g|_2 of the inner solve                                                     */
   int64_t n_pairs, n_active, nnzb;
   int32_t pcg_iters, backtracks, accepted, reserved;
+  double energy_membrane;   /* E_m's share of energy1 (0 without the membrane term)                                 */
 } tt_newton_report;
 tt_status tt_newton_step(tt_ctx* ctx, void* pos, int64_t n_verts, const int32_t* tris, int64_t n_tris,
                          const int32_t* pairs, int64_t n_pairs, const tt_newton_options* opt,
@@ -264,6 +267,32 @@ tt_status tt_newton_step(tt_ctx* ctx, void* pos, int64_t n_verts, const int32_t*
 tt_status tt_untangle(tt_ctx* ctx, void* pos, int64_t n_verts, const int32_t* tris, int64_t n_tris, double inflate,
                       int32_t max_steps, const tt_newton_options* opt, tt_newton_report* history_host,
                       int32_t* steps_host, void* stream);
+
+/* ---- The membrane term of the untangling demo (Fig. 2: the paper optimises
+ * meshes "from an invalid to a valid state" inside a simulation whose elastic model it does not give; DESIGN.md
+ * reading A18 takes the simplest textbook one, springs on the mesh's own edges):
+ *     E_m(x) = k/2 sum over the mesh's unique edges (i, j) of (|x_i - x_j| - L_ij)^2,   L_ij = |r_i - r_j| at rest,
+ *     grad_i = k sum_j (|d| - L) n,       d = x_i - x_j,  n = d / |d|,
+ *     H_m p  at i = sum_j K (p_i - p_j),  K = k [ n n^T + max(0, 1 - L / |d|) (I - n n^T) ]
+ * (K = the edge's exact Hessian block with the negative part of a compressed spring clamped to zero, so H_m is PSD).
+ * An edge whose two ends coincide (|d| = 0) has no direction and contributes nothing.
+ *
+ * tt_membrane_build:       builds the vertex -> neighbour adjacency of `tris` (sort + unique of the half-edges; an
+ *                          edge shared by several triangles counts once, a degenerate edge i == i is dropped) and the
+ *                          rest lengths from rest_pos.  rest_pos DEVICE [n_verts,3] dtype, tris DEVICE [n_tris,3]
+ *                          int32; both are only read during the call.  The result is owned by ctx and replaces the
+ *                          previous one; one host round trip on `stream` (the number of unique half-edges).
+ * tt_membrane_energy_grad: energy DEVICE [1] DOUBLE (whatever the dtype), grad DEVICE [n_verts,3] dtype or NULL.
+ * tt_membrane_hess_vec:    y = H_m(pos) p;  pos, p, y DEVICE [n_verts,3] dtype, p != y.
+ * Both need a preceding tt_membrane_build (TT_ERR_STATE otherwise) and use ITS n_verts.  One thread per vertex walks
+ * the neighbours in ascending order: no atomics, results bit-reproducible; arithmetic in fp64 for both dtypes.
+ * With tt_newton_options.membrane = 1, tt_newton_step / tt_untangle minimise E_T + E_m: g = g_T + g_m, the inner
+ * solve applies H_T p (assembled or matrix-free) + H_m p + mu p, and the preconditioner is the inverse of the
+ * MEMBRANE's diagonal blocks + mu I in both back ends (TT_ERR_STATE if the built mesh has another n_verts).         */
+tt_status tt_membrane_build(tt_ctx* ctx, const void* rest_pos, int64_t n_verts, const int32_t* tris, int64_t n_tris,
+                            double stiffness, void* stream);
+tt_status tt_membrane_energy_grad(tt_ctx* ctx, const void* pos, double* energy, void* grad, void* stream);
+tt_status tt_membrane_hess_vec(tt_ctx* ctx, const void* pos, const void* p, void* y, void* stream);
 
 /* Counters of the last tt_hess_symbolic: what[0]=n_active, [1]=directed entries (2*n_active),
  * [2]=touched triangles, [3]=blocks written directly (exclusive rows), [4]=blocks produced by the

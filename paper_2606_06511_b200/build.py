@@ -8,7 +8,7 @@ from pathlib import Path
 
 HERE = Path(__file__).resolve().parent
 SRC = HERE / "csrc" / "tt_lib.cu"
-DEPS = [SRC, HERE / "csrc" / "tt_kernels.cuh", HERE / "csrc" / "tt_geom.cuh", HERE / "csrc" / "tt_probe.cuh", HERE / "csrc" / "tt_broad.cuh", HERE / "csrc" / "tt_solve.cuh", HERE / "csrc" / "tt_exact.cuh", HERE.parent / "include" / "tt.h"]
+DEPS = [SRC, HERE / "csrc" / "tt_kernels.cuh", HERE / "csrc" / "tt_geom.cuh", HERE / "csrc" / "tt_probe.cuh", HERE / "csrc" / "tt_broad.cuh", HERE / "csrc" / "tt_solve.cuh", HERE / "csrc" / "tt_exact.cuh", HERE / "csrc" / "tt_membrane.cuh", HERE.parent / "include" / "tt.h"]
 LIB = HERE / "libtt.so"
 
 NVCC_FLAGS = ["-O3", "-std=c++17", "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo",

@@ -16,6 +16,7 @@
 #include "tt_probe.cuh"
 #include "tt_solve.cuh"
 #include "tt_exact.cuh"
+#include "tt_membrane.cuh"
 
 namespace {
 
@@ -81,6 +82,10 @@ struct tt_ctx {
   DevBuf cub_tmp;
   DevBuf pcg_r, pcg_p, pcg_q, pcg_part[2], pcg_sc, pcg_hist;  // tt_pcg_solve workspace
   DevBuf nw_g, nw_d, nw_x, nw_vals, nw_minv, nw_sc;            // tt_newton_step workspace
+  // membrane (tt_membrane_build): vertex -> neighbour adjacency, rest lengths
+  DevBuf mb_keys[2], mb_ptr, mb_adj, mb_rest, mb_part, mb_num;
+  int64_t mb_nV = -1, mb_half = 0;
+  double mb_k = 0.0;
   DevBuf possig;  // [2] u64: checksum of pos at tt_hess_symbolic, and at the last numeric / H.p call
   // broad phase (tt_broad_phase): boxes, grid, (cell, triangle) records, pair keys, result
   DevBuf bp_box, bp_part, bp_grid, bp_cnt, bp_off, bp_keys[2], bp_vals[2], bp_pcnt, bp_poff, bp_pkeys[2], bp_pairs;
@@ -822,10 +827,80 @@ tt_status spmv_impl(tt_ctx* ctx, int64_t nV, const int32_t* rowptr, const int32_
   return TT_OK;
 }
 
+// ---- the membrane term (tt_membrane.cuh, reading A18) ----------------------------------
+template <typename T>
+tt_status membrane_build_impl(tt_ctx* ctx, const void* rest_pos, int64_t nV, const int32_t* tris, int64_t nT, double k, cudaStream_t st) {
+  using namespace ttm;
+  ctx->mb_nV = -1;
+  const int64_t n6 = 6 * nT;
+  TT_CUDA(ctx->mb_ptr.ensure(sizeof(int) * (size_t)(nV + 2)));
+  TT_CUDA(ctx->mb_num.ensure(sizeof(int64_t) * 2));
+  int64_t n_uniq = 0;
+  if (n6 > 0) {
+    for (int i = 0; i < 2; ++i) TT_CUDA(ctx->mb_keys[i].ensure(sizeof(unsigned long long) * (size_t)n6));
+    k_half_edges<<<grid_for(nT, MB_THREADS), MB_THREADS, 0, st>>>(tris, nT, nV, ctx->mb_keys[0].as<unsigned long long>());
+    TT_LAUNCH_CHECK();
+    cub::DoubleBuffer<unsigned long long> dk(ctx->mb_keys[0].as<unsigned long long>(), ctx->mb_keys[1].as<unsigned long long>());
+    const int end_bit = 32 + ceil_log2(nV + 2);
+    size_t tmp = 0;
+    TT_CUDA(cub::DeviceRadixSort::SortKeys(nullptr, tmp, dk, n6, 0, end_bit, st));
+    TT_CUDA(ctx->cub_tmp.ensure(tmp));
+    TT_CUDA(cub::DeviceRadixSort::SortKeys(ctx->cub_tmp.p, tmp, dk, n6, 0, end_bit, st));
+    ctx->launches += 2 + (end_bit + 7) / 8;
+    unsigned long long* sorted = dk.Current();
+    unsigned long long* uniq = dk.Alternate();
+    tmp = 0;
+    TT_CUDA(cub::DeviceSelect::Unique(nullptr, tmp, sorted, uniq, ctx->mb_num.as<int64_t>(), n6, st));
+    TT_CUDA(ctx->cub_tmp.ensure(tmp));
+    TT_CUDA(cub::DeviceSelect::Unique(ctx->cub_tmp.p, tmp, sorted, uniq, ctx->mb_num.as<int64_t>(), n6, st));
+    ctx->launches += 2;
+    TT_CUDA(cudaMemcpyAsync(&n_uniq, ctx->mb_num.p, sizeof(int64_t), cudaMemcpyDeviceToHost, st));
+    TT_CUDA(cudaStreamSynchronize(st));
+    TT_CUDA(ctx->mb_adj.ensure(sizeof(int) * (size_t)(n_uniq + 1)));
+    TT_CUDA(ctx->mb_rest.ensure(sizeof(double) * (size_t)(n_uniq + 1)));
+    k_adjacency<T><<<grid_for(n_uniq, MB_THREADS), MB_THREADS, 0, st>>>(uniq, n_uniq, nV, (const T*)rest_pos, ctx->mb_adj.as<int>(),
+                                                                          ctx->mb_rest.as<double>());
+    TT_LAUNCH_CHECK();
+    ttk::k_segment_ptr<<<grid_for(nV + 1, 256), 256, 0, st>>>((const uint64_t*)uniq, n_uniq, 32, nV, ctx->mb_ptr.as<int>());
+    TT_LAUNCH_CHECK();
+  } else {
+    TT_CUDA(cudaMemsetAsync(ctx->mb_ptr.p, 0, sizeof(int) * (size_t)(nV + 2), st));
+  }
+  TT_CUDA(ctx->mb_part.ensure(sizeof(double) * (size_t)(grid_for(nV > 0 ? nV : 1, MB_THREADS) + 2)));
+  ctx->mb_half = n_uniq;
+  ctx->mb_k = k;
+  ctx->mb_nV = nV;
+  return TT_OK;
+}
+// energy -> e_out[0] (double, device), gradient written or added to grad (may be NULL)
+template <typename T>
+tt_status membrane_energy_grad_impl(tt_ctx* ctx, const void* pos, double* e_out, void* grad, bool accumulate, cudaStream_t st) {
+  using namespace ttm;
+  const int64_t nV = ctx->mb_nV;
+  const unsigned g = grid_for(nV > 0 ? nV : 1, MB_THREADS);
+  k_membrane<T, 0><<<g, MB_THREADS, 0, st>>>((const T*)pos, ctx->mb_ptr.as<int>(), ctx->mb_adj.as<int>(), ctx->mb_rest.as<double>(), nV,
+                                             ctx->mb_k, nullptr, 0.0, accumulate ? 1 : 0, (T*)grad, ctx->mb_part.as<double>());
+  TT_LAUNCH_CHECK();
+  ttk::k_sum_partials<double><<<1, 1024, 0, st>>>(ctx->mb_part.as<double>(), (int64_t)g, 1.0, e_out);
+  TT_LAUNCH_CHECK();
+  return TT_OK;
+}
+template <typename T, int MODE>  // 1: y (+)= H_m p;  2: minv = (D + mu I)^-1
+tt_status membrane_apply_impl(tt_ctx* ctx, const void* pos, const void* p, double mu, bool accumulate, void* out, cudaStream_t st) {
+  using namespace ttm;
+  const int64_t nV = ctx->mb_nV;
+  if (nV <= 0) return TT_OK;
+  k_membrane<T, MODE><<<grid_for(nV, MB_THREADS), MB_THREADS, 0, st>>>((const T*)pos, ctx->mb_ptr.as<int>(), ctx->mb_adj.as<int>(),
+                                                                          ctx->mb_rest.as<double>(), nV, ctx->mb_k, (const T*)p, mu,
+                                                                          accumulate ? 1 : 0, (T*)out, nullptr);
+  TT_LAUNCH_CHECK();
+  return TT_OK;
+}
+
 template <typename T>
 tt_status pcg_impl(tt_ctx* ctx, const tt_problem* q, const int32_t* rowptr, const int32_t* colind, const void* vals,
                    const void* minv, const void* b, void* x, const tt_pcg_options* opt, int32_t* iters_host,
-                   double* relres_host, cudaStream_t st) {
+                   double* relres_host, cudaStream_t st, bool membrane = false) {
   using namespace tts;
   const int64_t nV = q->n_verts, n = 3 * nV;
   const bool matrix_free = (vals == nullptr);
@@ -855,6 +930,10 @@ tt_status pcg_impl(tt_ctx* ctx, const tt_problem* q, const int32_t* rowptr, cons
   for (int it = 0; it < opt->max_iter; ++it) {
     tt_status s = matrix_free ? hessvec_impl<T>(ctx, q, p, Ap, st) : spmv_impl<T>(ctx, nV, rowptr, colind, vals, opt->shift, p, Ap, st);
     if (s != TT_OK) return s;
+    if (membrane) {  // + H_m p (tt_membrane.cuh)
+      s = membrane_apply_impl<T, 1>(ctx, q->pos, p, 0.0, true, Ap, st);
+      if (s != TT_OK) return s;
+    }
     k_pcg_pq<T><<<gn, VEC_THREADS, 0, st>>>(p, Ap, n, opt->shift, matrix_free ? 1 : 0, part0);
     TT_LAUNCH_CHECK();
     k_pcg_alpha<<<1, 1024, 0, st>>>(part0, (int64_t)gn, sc);
@@ -983,32 +1062,38 @@ tt_status newton_impl(tt_ctx* ctx, void* pos, int64_t nV, const int32_t* tris, i
   if (s != TT_OK) return s;
   rep->n_active = A;
   rep->nnzb = nnzb;
-  if (A == 0 || nV == 0) {  // nothing intersects: E = 0 is the minimum
+  if (A == 0 || nV == 0) {  // nothing intersects: the loop's goal is reached (the membrane alone is not relaxed further)
     rep->accepted = 1;
     return TT_OK;
   }
   const int64_t n = 3 * nV;
   const bool mf = o->matrix_free != 0;
+  const bool mb = o->membrane != 0;  // E = E_T + E_m (tt_membrane.cuh, reading A18)
   TT_CUDA(ctx->nw_g.ensure(sizeof(T) * (size_t)n));
   TT_CUDA(ctx->nw_d.ensure(sizeof(T) * (size_t)n));
   TT_CUDA(ctx->nw_x.ensure(sizeof(T) * (size_t)n));
   TT_CUDA(ctx->nw_sc.ensure(sizeof(double) * 8));
-  if (!mf) {
-    TT_CUDA(ctx->nw_vals.ensure(sizeof(T) * 9 * (size_t)(nnzb + 1)));
-    TT_CUDA(ctx->nw_minv.ensure(sizeof(T) * 9 * (size_t)nV));
-  }
+  if (!mf) TT_CUDA(ctx->nw_vals.ensure(sizeof(T) * 9 * (size_t)(nnzb + 1)));
+  if (!mf || mb) TT_CUDA(ctx->nw_minv.ensure(sizeof(T) * 9 * (size_t)nV));
   T* g = ctx->nw_g.as<T>();
   T* d = ctx->nw_d.as<T>();
   T* x_try = ctx->nw_x.as<T>();
   double* sc = ctx->nw_sc.as<double>();        // [0] g.d  [1] g.g
   T* e_dev = reinterpret_cast<T*>(sc + 2);      // [0] E0   [1] E(x_try)
+  double* em_dev = sc + 4;                      // [0] E_m(x)  [1] E_m(x_try)   (membrane only)
   int* rowptr = ctx->rowptr.as<int>();
   int* colind = ctx->colind.as<int>();
   T* vals = mf ? nullptr : ctx->nw_vals.as<T>();
   s = numeric_impl<T>(ctx, &q, e_dev, g, mf ? nullptr : rowptr, mf ? nullptr : colind, vals, nnzb, st);
   if (s != TT_OK) return s;
   T* minv = nullptr;
-  if (!mf) {
+  if (mb) {  // g += g_m;  the preconditioner is the membrane's own diagonal blocks + mu I (in both back ends)
+    s = membrane_energy_grad_impl<T>(ctx, pos, em_dev, g, true, st);
+    if (s != TT_OK) return s;
+    minv = ctx->nw_minv.as<T>();
+    s = membrane_apply_impl<T, 2>(ctx, pos, nullptr, o->mu, false, minv, st);
+    if (s != TT_OK) return s;
+  } else if (!mf) {
     minv = ctx->nw_minv.as<T>();
     k_block_jacobi<T><<<grid_for(nV, VEC_THREADS), VEC_THREADS, 0, st>>>(rowptr, colind, vals, nV, o->mu, minv);
     TT_LAUNCH_CHECK();
@@ -1017,7 +1102,7 @@ tt_status newton_impl(tt_ctx* ctx, void* pos, int64_t nV, const int32_t* tris, i
   po.shift = o->mu;
   int32_t iters = 0;
   double relres = 0.0;
-  s = pcg_impl<T>(ctx, &q, rowptr, colind, vals, minv, g, d, &po, &iters, &relres, st);
+  s = pcg_impl<T>(ctx, &q, rowptr, colind, vals, minv, g, d, &po, &iters, &relres, st, mb);
   if (s != TT_OK) return s;
   rep->pcg_iters = iters;
   rep->pcg_relres = relres;
@@ -1028,12 +1113,14 @@ tt_status newton_impl(tt_ctx* ctx, void* pos, int64_t nV, const int32_t* tris, i
   TT_LAUNCH_CHECK();
   k_dot2_final<<<1, 1024, 0, st>>>(part0, part1, (int64_t)gn, sc);
   TT_LAUNCH_CHECK();
-  double h_sc[2] = {0.0, 0.0};
+  double h_sc[2] = {0.0, 0.0}, h_em[2] = {0.0, 0.0};
   T h_e[2] = {(T)0, (T)0};
   TT_CUDA(cudaMemcpyAsync(h_sc, sc, sizeof(h_sc), cudaMemcpyDeviceToHost, st));
   TT_CUDA(cudaMemcpyAsync(h_e, e_dev, sizeof(T), cudaMemcpyDeviceToHost, st));
+  if (mb) TT_CUDA(cudaMemcpyAsync(h_em, em_dev, sizeof(double), cudaMemcpyDeviceToHost, st));
   TT_CUDA(cudaStreamSynchronize(st));
-  const double E0 = (double)h_e[0], gd = h_sc[0];
+  const double E0 = (double)h_e[0] + h_em[0], gd = h_sc[0];
+  rep->energy_membrane = h_em[0];
   rep->energy0 = rep->energy1 = E0;
   rep->gd = gd;
   rep->grad_norm = sqrt(h_sc[1]);
@@ -1045,12 +1132,18 @@ tt_status newton_impl(tt_ctx* ctx, void* pos, int64_t nV, const int32_t* tris, i
     TT_LAUNCH_CHECK();
     s = energy_impl<T>(ctx, &qt, e_dev + 1, nullptr, nullptr, nullptr, nullptr, st);
     if (s != TT_OK) return s;
+    if (mb) {
+      s = membrane_energy_grad_impl<T>(ctx, x_try, em_dev + 1, nullptr, false, st);
+      if (s != TT_OK) return s;
+      TT_CUDA(cudaMemcpyAsync(h_em + 1, em_dev + 1, sizeof(double), cudaMemcpyDeviceToHost, st));
+    }
     TT_CUDA(cudaMemcpyAsync(h_e + 1, e_dev + 1, sizeof(T), cudaMemcpyDeviceToHost, st));
     TT_CUDA(cudaStreamSynchronize(st));
-    const double Et = (double)h_e[1];
+    const double Et = (double)h_e[1] + h_em[1];
     if (Et <= E0 - o->armijo_c1 * alpha * gd) {
       TT_CUDA(cudaMemcpyAsync(pos, x_try, sizeof(T) * (size_t)n, cudaMemcpyDeviceToDevice, st));
       rep->energy1 = Et;
+      rep->energy_membrane = h_em[1];
       rep->alpha = alpha;
       rep->backtracks = j;
       rep->accepted = 1;
@@ -1069,6 +1162,9 @@ tt_status check_newton_args(tt_ctx* ctx, const void* pos, int64_t nV, const int3
       !(o->pcg.rtol >= 0.0))
     return fail(ctx, TT_ERR_INVALID_ARG, "newton options: need mu > 0, 0 < armijo_c1 < 1, max_backtrack >= 0, pcg.max_iter >= 0, pcg.rtol >= 0");
   if (nV < 0 || nT < 0 || (nV > 0 && !pos) || (nT > 0 && !tris)) return fail(ctx, TT_ERR_INVALID_ARG, "NULL array or negative size");
+  if (o->membrane != 0 && ctx->mb_nV != nV)
+    return fail(ctx, TT_ERR_STATE, "newton options ask for the membrane term, but tt_membrane_build has not been called for a mesh of %lld vertices",
+                (long long)nV);
   return TT_OK;
 }
 
@@ -1394,6 +1490,43 @@ tt_status tt_pcg_solve(tt_ctx* ctx, const tt_problem* prob, const int32_t* rowpt
   }
   return ctx->opt.dtype == TT_F64 ? pcg_impl<double>(ctx, prob, rowptr, colind, vals, minv, b, x, opt, iters_host, relres_host, st)
                                   : pcg_impl<float>(ctx, prob, rowptr, colind, vals, minv, b, x, opt, iters_host, relres_host, st);
+}
+
+tt_status tt_membrane_build(tt_ctx* ctx, const void* rest_pos, int64_t n_verts, const int32_t* tris, int64_t n_tris,
+                            double stiffness, void* stream) {
+  if (!ctx) return TT_ERR_INVALID_ARG;
+  if (n_verts < 0 || n_tris < 0 || n_verts >= (int64_t(1) << 31) / 3 || n_tris >= (int64_t(1) << 31) / 6)
+    return fail(ctx, TT_ERR_INVALID_ARG, "tt_membrane_build: size out of range");
+  if ((n_verts > 0 && !rest_pos) || (n_tris > 0 && !tris)) return fail(ctx, TT_ERR_INVALID_ARG, "tt_membrane_build: NULL array");
+  if (!(stiffness >= 0.0)) return fail(ctx, TT_ERR_INVALID_ARG, "tt_membrane_build: stiffness must be >= 0");
+  TT_CUDA(cudaSetDevice(ctx->opt.device));
+  cudaStream_t st = (cudaStream_t)stream;
+  if (n_tris > 0) {
+    tt_status s = validate_indices(ctx, tris, n_tris, n_verts, nullptr, 0, st);
+    if (s != TT_OK) return s;
+  }
+  return ctx->opt.dtype == TT_F64 ? membrane_build_impl<double>(ctx, rest_pos, n_verts, tris, n_tris, stiffness, st)
+                                  : membrane_build_impl<float>(ctx, rest_pos, n_verts, tris, n_tris, stiffness, st);
+}
+
+tt_status tt_membrane_energy_grad(tt_ctx* ctx, const void* pos, double* energy, void* grad, void* stream) {
+  if (!ctx) return TT_ERR_INVALID_ARG;
+  if (ctx->mb_nV < 0) return fail(ctx, TT_ERR_STATE, "tt_membrane_energy_grad without tt_membrane_build");
+  if (!energy || (ctx->mb_nV > 0 && !pos)) return fail(ctx, TT_ERR_INVALID_ARG, "tt_membrane_energy_grad: NULL argument");
+  TT_CUDA(cudaSetDevice(ctx->opt.device));
+  cudaStream_t st = (cudaStream_t)stream;
+  return ctx->opt.dtype == TT_F64 ? membrane_energy_grad_impl<double>(ctx, pos, energy, grad, false, st)
+                                  : membrane_energy_grad_impl<float>(ctx, pos, energy, grad, false, st);
+}
+
+tt_status tt_membrane_hess_vec(tt_ctx* ctx, const void* pos, const void* p, void* y, void* stream) {
+  if (!ctx) return TT_ERR_INVALID_ARG;
+  if (ctx->mb_nV < 0) return fail(ctx, TT_ERR_STATE, "tt_membrane_hess_vec without tt_membrane_build");
+  if (ctx->mb_nV > 0 && (!pos || !p || !y || p == y)) return fail(ctx, TT_ERR_INVALID_ARG, "tt_membrane_hess_vec: NULL or aliased argument");
+  TT_CUDA(cudaSetDevice(ctx->opt.device));
+  cudaStream_t st = (cudaStream_t)stream;
+  return ctx->opt.dtype == TT_F64 ? membrane_apply_impl<double, 1>(ctx, pos, p, 0.0, false, y, st)
+                                  : membrane_apply_impl<float, 1>(ctx, pos, p, 0.0, false, y, st);
 }
 
 tt_status tt_newton_step(tt_ctx* ctx, void* pos, int64_t n_verts, const int32_t* tris, int64_t n_tris, const int32_t* pairs,

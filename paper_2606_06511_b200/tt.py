@@ -24,7 +24,7 @@ TT_FLAG_VALIDATE_INDICES = 2
 TT_FLAG_NO_STATE_CHECK = 4
 
 EXPORTS = ["tt_create", "tt_destroy", "tt_energy", "tt_hess_symbolic", "tt_energy_grad_hess", "tt_hess_vec",
-           "tt_energy_grad_hess_host", "tt_hess_pattern", "tt_broad_phase", "tt_broad_phase_pairs", "tt_broad_phase_copy", "tt_bsr_device", "tt_bsr_spmv", "tt_block_jacobi", "tt_pcg_solve", "tt_newton_step", "tt_untangle", "tt_stats", "tt_kernel_ms", "tt_kernel_ms_mean", "tt_probe_peaks", "tt_probe_gather", "tt_status_string", "tt_last_error"]
+           "tt_energy_grad_hess_host", "tt_hess_pattern", "tt_broad_phase", "tt_broad_phase_pairs", "tt_broad_phase_copy", "tt_bsr_device", "tt_bsr_spmv", "tt_block_jacobi", "tt_pcg_solve", "tt_newton_step", "tt_untangle", "tt_membrane_build", "tt_membrane_energy_grad", "tt_membrane_hess_vec", "tt_stats", "tt_kernel_ms", "tt_kernel_ms_mean", "tt_probe_peaks", "tt_probe_gather", "tt_status_string", "tt_last_error"]
 
 
 class TTOptions(ctypes.Structure):
@@ -44,7 +44,8 @@ class TTPcgOptions(ctypes.Structure):
 
 class TTNewtonOptions(ctypes.Structure):
     _fields_ = [("mu", ctypes.c_double), ("armijo_c1", ctypes.c_double), ("max_backtrack", ctypes.c_int32),
-                ("matrix_free", ctypes.c_int32), ("pcg", TTPcgOptions)]
+                ("matrix_free", ctypes.c_int32), ("pcg", TTPcgOptions), ("membrane", ctypes.c_int32),
+                ("reserved", ctypes.c_int32)]
 
 
 class TTNewtonReport(ctypes.Structure):
@@ -52,7 +53,7 @@ class TTNewtonReport(ctypes.Structure):
                 ("gd", ctypes.c_double), ("alpha", ctypes.c_double), ("pcg_relres", ctypes.c_double),
                 ("n_pairs", ctypes.c_int64), ("n_active", ctypes.c_int64), ("nnzb", ctypes.c_int64),
                 ("pcg_iters", ctypes.c_int32), ("backtracks", ctypes.c_int32), ("accepted", ctypes.c_int32),
-                ("reserved", ctypes.c_int32)]
+                ("reserved", ctypes.c_int32), ("energy_membrane", ctypes.c_double)]
 
     def as_dict(self):
         return {k: getattr(self, k) for k, _ in self._fields_ if k != "reserved"}
@@ -115,6 +116,12 @@ def load_library():
     lib.tt_untangle.argtypes = [vp, vp, i64, vp, i64, ctypes.c_double, ctypes.c_int32, ctypes.POINTER(TTNewtonOptions),
                                 ctypes.POINTER(TTNewtonReport), ctypes.POINTER(ctypes.c_int32), vp]
     lib.tt_untangle.restype = ctypes.c_int
+    lib.tt_membrane_build.argtypes = [vp, vp, i64, vp, i64, ctypes.c_double, vp]
+    lib.tt_membrane_build.restype = ctypes.c_int
+    lib.tt_membrane_energy_grad.argtypes = [vp, vp, vp, vp, vp]
+    lib.tt_membrane_energy_grad.restype = ctypes.c_int
+    lib.tt_membrane_hess_vec.argtypes = [vp, vp, vp, vp, vp]
+    lib.tt_membrane_hess_vec.restype = ctypes.c_int
     lib.tt_stats.argtypes = [vp, ctypes.POINTER(i64), ctypes.c_int32]
     lib.tt_stats.restype = ctypes.c_int
     lib.tt_kernel_ms.argtypes = [vp, ctypes.POINTER(ctypes.c_float), ctypes.c_int32]
@@ -282,25 +289,48 @@ class Context:
         return (it.value, rr.value) if want_stats else None
 
     @staticmethod
-    def _newton_options(mu, c1, max_backtrack, matrix_free, pcg_iter, pcg_rtol):
+    def _newton_options(mu, c1, max_backtrack, matrix_free, pcg_iter, pcg_rtol, membrane=False):
         return TTNewtonOptions(float(mu), float(c1), int(max_backtrack), 1 if matrix_free else 0,
-                               TTPcgOptions(int(pcg_iter), 0, float(pcg_rtol), 0.0))
+                               TTPcgOptions(int(pcg_iter), 0, float(pcg_rtol), 0.0), 1 if membrane else 0, 0)
+
+    def tt_membrane_build(self, rest_pos, tris, stiffness, stream=None):
+        """Adjacency + rest lengths of the edge-spring membrane of `tris` (owned by the context)."""
+        assert rest_pos.is_cuda and rest_pos.dtype == self.dtype and rest_pos.is_contiguous()
+        assert tris.is_cuda and tris.dtype == torch.int32 and tris.is_contiguous()
+        self._check(self.lib.tt_membrane_build(self.h, _ptr(rest_pos), rest_pos.shape[0], _ptr(tris), tris.shape[0],
+                                               float(stiffness), _stream_ptr(stream)))
+
+    def tt_membrane_energy_grad(self, pos, want_grad=True, stream=None):
+        """E_m (a 1-element fp64 device tensor) and its gradient ([nV,3] dtype, or None)."""
+        assert pos.is_cuda and pos.dtype == self.dtype and pos.is_contiguous()
+        e = torch.empty(1, dtype=torch.float64, device=pos.device)
+        g = torch.empty_like(pos) if want_grad else None
+        self._check(self.lib.tt_membrane_energy_grad(self.h, _ptr(pos), _ptr(e), _ptr(g) if want_grad else None,
+                                                     _stream_ptr(stream)))
+        return e, g
+
+    def tt_membrane_hess_vec(self, pos, p, stream=None):
+        assert pos.is_cuda and pos.dtype == self.dtype and pos.is_contiguous()
+        assert p.is_cuda and p.dtype == self.dtype and p.is_contiguous() and p.shape == pos.shape
+        y = torch.empty_like(p)
+        self._check(self.lib.tt_membrane_hess_vec(self.h, _ptr(pos), _ptr(p), _ptr(y), _stream_ptr(stream)))
+        return y
 
     def tt_newton_step(self, pos, tris, pairs, mu=1e-3, c1=1e-4, max_backtrack=20, matrix_free=False, pcg_iter=20,
-                       pcg_rtol=0.0, stream=None):
+                       pcg_rtol=0.0, membrane=False, stream=None):
         """One damped inexact-Newton step; `pos` is updated IN PLACE.  Returns the report as a dict."""
         assert pos.is_cuda and pos.dtype == self.dtype and pos.is_contiguous()
-        opt = self._newton_options(mu, c1, max_backtrack, matrix_free, pcg_iter, pcg_rtol)
+        opt = self._newton_options(mu, c1, max_backtrack, matrix_free, pcg_iter, pcg_rtol, membrane)
         rep = TTNewtonReport()
         self._check(self.lib.tt_newton_step(self.h, _ptr(pos), pos.shape[0], _ptr(tris), tris.shape[0], _ptr(pairs),
                                             pairs.shape[0], ctypes.byref(opt), ctypes.byref(rep), _stream_ptr(stream)))
         return rep.as_dict()
 
     def tt_untangle(self, pos, tris, inflate=0.0, max_steps=20, mu=1e-3, c1=1e-4, max_backtrack=20, matrix_free=False,
-                    pcg_iter=20, pcg_rtol=0.0, stream=None):
+                    pcg_iter=20, pcg_rtol=0.0, membrane=False, stream=None):
         """Broad phase + Newton step until nothing intersects; `pos` is updated IN PLACE.  Returns the list of reports."""
         assert pos.is_cuda and pos.dtype == self.dtype and pos.is_contiguous()
-        opt = self._newton_options(mu, c1, max_backtrack, matrix_free, pcg_iter, pcg_rtol)
+        opt = self._newton_options(mu, c1, max_backtrack, matrix_free, pcg_iter, pcg_rtol, membrane)
         hist = (TTNewtonReport * max(int(max_steps), 1))()
         n = ctypes.c_int32(0)
         self._check(self.lib.tt_untangle(self.h, _ptr(pos), pos.shape[0], _ptr(tris), tris.shape[0], float(inflate),
