@@ -63,6 +63,8 @@ def parse():
     ap.add_argument("--untangle", action="store_true",
                     help="run tt_untangle (broad phase + Newton step with line search, SURVEY 8(f) NEXT-2 / NEXT-4) on the mesh "
                          "given by --config (1, 2 or 3) for --steps steps; prints its own JSON line")
+    ap.add_argument("--membrane", type=float, default=0.0,
+                    help="with --untangle: stiffness k of the edge-spring membrane (SURVEY 8(f) NEXT-4, DESIGN.md A18); 0 = none")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     return ap.parse_args()
@@ -314,15 +316,27 @@ def run_untangle(args):
     ctx = tt.Context(torch.float64, 2, 1.0, 0)     # PSD2
     tris = torch.from_numpy(pb.tris).to(dev)
     mu, iters = 1e-3, 30
-    pos = torch.from_numpy(pb.pos).to(dev).clone()
-    ctx.tt_untangle(pos, tris, inflate=inflate, max_steps=2, mu=mu, pcg_iter=iters)       # warm-up (workspace allocation)
-    pos = torch.from_numpy(pb.pos).to(dev).clone()
+    mbk = float(args.membrane)
+    kw = dict(inflate=inflate, mu=mu, pcg_iter=iters, membrane=mbk > 0.0, matrix_free=mbk > 0.0)
+    rest = torch.from_numpy(pb.pos).to(dev)
+    if mbk > 0.0:
+        torch.cuda.synchronize()
+        t0 = time.perf_counter()
+        ctx.tt_membrane_build(rest, tris, mbk)
+        torch.cuda.synchronize()
+        ms_build = 1e3 * (time.perf_counter() - t0)
+    pos = rest.clone()
+    ctx.tt_untangle(pos, tris, max_steps=2, **kw)       # warm-up (workspace allocation)
+    pos = rest.clone()
     torch.cuda.synchronize()
     t0 = time.perf_counter()
-    hist = ctx.tt_untangle(pos, tris, inflate=inflate, max_steps=args.steps, mu=mu, pcg_iter=iters)
+    hist = ctx.tt_untangle(pos, tris, max_steps=args.steps, **kw)
     torch.cuda.synchronize()
     dt = time.perf_counter() - t0
-    disp = float((pos - torch.from_numpy(pb.pos).to(dev)).norm(dim=1).max())
+    disp = float((pos - rest).norm(dim=1).max())
+    t64 = tris.long()
+    ed = torch.cat([t64[:, [0, 1]], t64[:, [1, 2]], t64[:, [2, 0]]])
+    strain = float(((pos[ed[:, 0]] - pos[ed[:, 1]]).norm(dim=1) / (rest[ed[:, 0]] - rest[ed[:, 1]]).norm(dim=1) - 1).abs().max())
     print(json.dumps({"metric": "untangling loop (tt_untangle): ms per step, energy and active pairs along the way", "n_gpus": 1,
                       "dtype": "f64", "data": "synthetic", "steps": len(hist),
                       "config": {"workload": "BASELINE %s: %d triangles; inflate %g, PSD2, mu %g, %d PCG steps per Newton step" % (
@@ -330,7 +344,9 @@ def run_untangle(args):
                       "ms_per_step": 1e3 * dt / max(len(hist), 1), "all_accepted": all(h["accepted"] for h in hist),
                       "n_pairs": [hist[0]["n_pairs"], hist[-1]["n_pairs"]], "n_active": [h["n_active"] for h in hist][::max(1, len(hist) // 10)],
                       "energy": [hist[0]["energy0"]] + [h["energy1"] for h in hist][::max(1, len(hist) // 10)],
-                      "max_vertex_displacement": disp}), flush=True)
+                      "max_vertex_displacement": disp, "max_edge_strain": strain,
+                      "membrane": ({"stiffness": mbk, "build_ms": ms_build, "energy_membrane": hist[-1]["energy_membrane"],
+                                    "back_end": "matrix-free, membrane block-Jacobi"} if mbk > 0.0 else None)}), flush=True)
     ctx.close()
 
 

@@ -487,3 +487,32 @@ def test_hess_pattern_views(oracle_mod):
         ctx3.tt_hess_pattern_ptrs()
     assert ei.value.status == -5
     ctx3.close()
+
+
+@pytest.mark.parametrize("dtype", ["f64", "f32"])
+def test_bit_reproducible_run_to_run(oracle_mod, dtype):
+    """no floating-point atomics, every sum in a fixed order -- although the counting-sort scatter of K2 places
+    entries with integer atomics, the segments are sorted before anything depends on their order.  Two contexts and a repeated
+    call must give bit-identical energy, gradient, pattern, values and H.p (config 4 at 300 k pairs: ordinary rounds, split
+    and long triangles, general rows through shared vertices are all present in the soup with a small vertex pool)."""
+    from paper_2606_06511_b200 import inputs, tt
+    dev = _dev()
+    tdt = torch.float64 if dtype == "f64" else torch.float32
+    pb = inputs.config4_sweep(n_tris=20_000, n_pairs=300_000)
+    pos = torch.from_numpy(pb.pos).to(dev).to(tdt).contiguous()
+    tris = torch.from_numpy(pb.tris).to(dev)
+    prs = torch.from_numpy(pb.pairs).to(dev)
+    p = torch.from_numpy(np.random.default_rng(3).normal(size=pb.pos.shape)).to(dev).to(tdt).contiguous()
+    outs = []
+    for rep in range(3):
+        ctx = tt.Context(tdt, 1, 1.0, 0) if rep != 1 else ctx          # rep 1 reuses the first context
+        out = tt.assemble(ctx, pos, tris, prs, want_hess=True)
+        y = torch.empty_like(p)
+        ctx.tt_hess_vec(out["prob"], p, y)
+        torch.cuda.synchronize()
+        outs.append((out["energy"].clone(), out["grad"].clone(), out["rowptr"].clone(), out["colind"].clone(), out["vals"].clone(), y))
+    st = ctx.tt_stats()
+    assert st["split_triangles"] + st["long_rounds"] > 0
+    for o in outs[1:]:
+        for a, b in zip(outs[0], o):
+            assert a.shape == b.shape and torch.equal(a, b)
