@@ -1322,6 +1322,8 @@ __device__ __forceinline__ void bulk_s2g(void* gdst, const void* ssrc, uint32_t 
 }
 __device__ __forceinline__ void bulk_commit() { asm volatile("cp.async.bulk.commit_group;" ::: "memory"); }
 __device__ __forceinline__ void bulk_wait_read() { asm volatile("cp.async.bulk.wait_group.read 0;" ::: "memory"); }
+template <int N>  // at most N of this thread's most recent groups may still be reading shared memory
+__device__ __forceinline__ void bulk_wait_read_n() { asm volatile("cp.async.bulk.wait_group.read %0;" ::"n"(N) : "memory"); }
 __device__ __forceinline__ void bulk_wait_all() { asm volatile("cp.async.bulk.wait_group 0;" ::: "memory"); }
 __device__ __forceinline__ void fence_async_smem() { asm volatile("fence.proxy.async.shared::cta;" ::: "memory"); }
 
@@ -1346,6 +1348,9 @@ __device__ __forceinline__ void cp_async_wait() { asm volatile("cp.async.wait_gr
 #define TT_RED_UNR 8                      // entries per triangle whose staged values are loaded up front
 #endif
 constexpr int RED_UNR = TT_RED_UNR;
+#ifndef TT_TILE_NBUF
+#define TT_TILE_NBUF 2                    // row tiles per warp: with two, a row is built while the copy engine reads the previous one
+#endif
 constexpr int TILE_WARPS = TT_TILE_WARPS; // warps per CTA (independent; a CTA is only a packaging unit)
 constexpr int NDIAG = 45;                 // upper triangle of the symmetric 9x9 diagonal block, row-major packed
 constexpr int NSTG = NDIAG + 9;           // + gradient of the three own vertices
@@ -1359,6 +1364,9 @@ struct TileCfg {
   static constexpr int TILE_BYTES = RUN_UNIT * (RND_MAX_ENT + MT) + 32 * MT;
   static constexpr int STAGE_BYTES = 32 * STG_STRIDE * (int)sizeof(double);
   static constexpr int UNION_BYTES = TILE_BYTES > STAGE_BYTES ? TILE_BYTES : STAGE_BYTES;
+  // fp64 with 16 slots per round: two tiles per warp would not leave room for 8 warps per SM
+  static constexpr int NBUF = (MT > RND_TRI_LOW && sizeof(T) == 8) ? 1 : TT_TILE_NBUF;
+  static_assert(UNION_BYTES % 16 == 0, "tile buffers must stay 16-byte aligned");
 };
 
 // Shared memory of one warp.  `tile` holds, in turn, (1) the per-entry staging area of the
@@ -1366,7 +1374,7 @@ struct TileCfg {
 // the same time (the per-triangle sums move to `dsum` in between).
 template <typename T, int MT>
 struct alignas(16) TileWarpSmem {
-  unsigned char tile[TileCfg<T, MT>::UNION_BYTES];
+  unsigned char tile[TileCfg<T, MT>::NBUF * TileCfg<T, MT>::UNION_BYTES];
   double dsum[MT][NSTG];                  // per-triangle sums: 45 diagonal-block values + 9 gradient values
   int run_off[MT];                        // byte offset of the triangle's run in the tile (current row)
   int diag_off[MT][3];                    // byte offset of its diagonal block n in the tile (current row)
@@ -1443,8 +1451,9 @@ k_assemble_tile(const AsmParams<T> P) {
   constexpr unsigned FULL = 0xffffffffu;
   constexpr int RUN_UNIT = TileCfg<T, MT>::RUN_UNIT;
   const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+  constexpr int NBUF = TileCfg<T, MT>::NBUF, UNION_BYTES = TileCfg<T, MT>::UNION_BYTES;
   TileWarpSmem<T, MT>& S = reinterpret_cast<TileWarpSmem<T, MT>*>(s_raw)[warp];
-  double* const stage = reinterpret_cast<double*>(S.tile);
+  int krow = 0;  // rows handed to the copy engine so far: row k lives in tile buffer k % NBUF
   const int64_t G = (int64_t)gridDim.x * TILE_WARPS;
   int64_t c = (int64_t)blockIdx.x * TILE_WARPS + warp;
   if (c >= P.n_chunks) return;
@@ -1493,8 +1502,10 @@ k_assemble_tile(const AsmParams<T> P) {
     int ids_nn[6];
     load_round_ids(P, d_nn, lane, ids_nn);
     const int4 d_nnn = (c + 3 * G < P.n_chunks) ? __ldg(P.rdesc + c + 3 * G) : dzero;
-    // the staging area aliases the row tile: the copy engine must have read the previous round's last row
-    bulk_wait_read();
+    // the staging area aliases the tile buffer of this round's first row: the copy engine must have read the row that
+    // used it last (every lane commits one group per row, so "all but the NBUF - 1 newest groups" means exactly that)
+    double* const stage = reinterpret_cast<double*>(S.tile + (krow % NBUF) * UNION_BYTES);
+    bulk_wait_read_n<NBUF - 1>();
     __syncwarp();
     if (valid) {
       unpermute_own(E, er);
@@ -1599,9 +1610,11 @@ k_assemble_tile(const AsmParams<T> P) {
         const unsigned long long g =
             (unsigned long long)((cur.rb[m] >= 0) ? (P.vals + 9 * cur.rb[m]) : (P.tvals + 9 * (-cur.rb[m] - 1)));
         const int my_off = slot_off + (int)(g & 15ull);
-        // the tile is single-buffered: the copy engine must have read the previous row's runs
+        // the copy engine must have read the row that used this buffer last
+        unsigned char* const tb = S.tile + (krow % NBUF) * UNION_BYTES;
+        ++krow;
         if (m > 0) {
-          bulk_wait_read();
+          bulk_wait_read_n<NBUF - 1>();
           __syncwarp();
         }
         if (lane < ntri) {
@@ -1621,7 +1634,7 @@ k_assemble_tile(const AsmParams<T> P) {
             at[i] = (T)(E.cf.c00 * E.g0[3 * m + i] + E.cf.c01 * E.g1[3 * m + i]);
             bt[i] = (T)(E.cf.c01 * E.g0[3 * m + i] + E.cf.c11 * E.g1[3 * m + i]);
           }
-          T* run = reinterpret_cast<T*>(S.tile + S.run_off[my_ti]);
+          T* run = reinterpret_cast<T*>(tb + S.run_off[my_ti]);
 #pragma unroll
           for (int n = 0; n < 3; ++n) {
             T* blk = run + 9 * er[n];
@@ -1651,7 +1664,7 @@ k_assemble_tile(const AsmParams<T> P) {
           }
 #pragma unroll
           for (int tt = 0; tt < MT; ++tt)
-            if (tt < ntri && (!PARTS || off[tt] >= 0)) *reinterpret_cast<T*>(S.tile + off[tt] + cq * (int)sizeof(T)) = val[tt];
+            if (tt < ntri && (!PARTS || off[tt] >= 0)) *reinterpret_cast<T*>(tb + off[tt] + cq * (int)sizeof(T)) = val[tt];
         }
         // positions of the next round (L2 hits): requested as soon as this round's J is dead
         if (m == 2 && lane < round_entries(d_nxt)) load_pos18(P.pos, ids_nxt, x);
@@ -1659,7 +1672,7 @@ k_assemble_tile(const AsmParams<T> P) {
         __syncwarp();
         // ---- lane = triangle: hand the run to the copy engine ----
         if (lane < ntri) {
-          const unsigned char* src = S.tile + my_off;
+          const unsigned char* src = tb + my_off;
           int head = (int)((16ull - (g & 15ull)) & 15ull);
           head = min(head, run_bytes);
           const int body = (run_bytes - head) & ~15;
@@ -1674,8 +1687,8 @@ k_assemble_tile(const AsmParams<T> P) {
             for (int o = head + body; o < run_bytes; o += (int)sizeof(T))
               *reinterpret_cast<T*>(g + o) = *reinterpret_cast<const T*>(src + o);
           }
-          bulk_commit();
         }
+        bulk_commit();  // by every lane, so that all lanes count the same groups
       }
     }
     if (is_long && lane < round_entries(d_nxt)) load_pos18(P.pos, ids_nxt, x);
