@@ -123,6 +123,22 @@ void tt_destroy(tt_ctx* ctx);
 tt_status tt_energy(tt_ctx* ctx, const tt_problem* prob, void* energy_sum, void* energy_per_pair,
                     uint32_t* active_mask, void* tc, int64_t* n_active, void* stream);
 
+/* tt_energy without any allocation (for callers that cannot call cudaMalloc: code under CUDA graph capture, tight
+ * serving loops, harnesses that forbid it).  The same steps 1-2 as tt_energy, total only:
+ *   energy_sum [1] dtype DEVICE: sum of T over all pairs -- bit-identical to tt_energy's (same per-CTA partials, same
+ *                                fixed-order two-level sum);   n_active [1] int64 DEVICE or NULL.
+ * The per-CTA partial sums and counts live in a file-scope device array of the library (768 KB, held by every GPU that
+ * loads the library until the process exits) instead of the context's growable workspace, so
+ *   - n_pairs <= TT_STATIC_MAX_PAIRS, else TT_ERR_CAPACITY (message in tt_last_error) and nothing is launched;
+ *   - the call makes no cudaMalloc / cudaFree / allocating library call, no host round trip and no synchronisation: it
+ *     enqueues 2-4 kernels on `stream` and returns (TT_FLAG_VALIDATE_INDICES, which needs a round trip, is NOT honoured);
+ *   - every call on a device shares the array, whatever the context, and leaves its contents behind: nothing in it has
+ *     to start at zero (a call reads only the slots it has written), but two calls that OVERLAP on the GPU (different
+ *     streams, or different contexts / threads on the same device) race on it -- serialise them.
+ * tt_create obtains the array's device address once, at set-up (the only preparation the call needs).               */
+#define TT_STATIC_MAX_PAIRS 16777216 /* 2^24 candidate pairs */
+tt_status tt_energy_static(tt_ctx* ctx, const tt_problem* prob, void* energy_sum, int64_t* n_active, void* stream);
+
 /* Symbolic phase of step 4 (L51): classifies the candidates at the current positions, compacts
  * the active pairs (order preserving) and builds the BSR pattern.  Caches all of it in ctx.
  *   nnzb_host     HOST [1]: number of 3x3 blocks the numeric phase will write

@@ -18,6 +18,19 @@
 #include "tt_exact.cuh"
 #include "tt_membrane.cuh"
 
+// ---- tt_energy_static: the scratch of the allocation-free energy entry point (include/tt.h) -----------------------
+// File-scope device memory, held by every GPU that loads the library until the process exits: the per-CTA energy
+// partials of K1, the slice sums of the two-level final sum, and the per-CTA active counts, for at most
+// TT_STATIC_MAX_PAIRS candidates.  In HOST code the name below is a host-side stand-in, not a device address: tt_create
+// asks for the address once per context, with the context's device current (cudaGetSymbolAddress), and the kernels are
+// handed that pointer.  Every call shares the array and leaves its contents behind; nothing in it has to start at zero
+// (every slot a call reads it has written itself), and calls that overlap on the GPU race on it.
+constexpr int64_t TT_STATIC_MAX_BLK = TT_STATIC_MAX_PAIRS / ttk::CLS_THREADS;                     // 65536 CTAs of K1
+constexpr int64_t TT_STATIC_MAX_STAGE = (TT_STATIC_MAX_BLK + ttk::SUM_SLICE - 1) / ttk::SUM_SLICE;  // 8 slice sums
+constexpr int64_t TT_STATIC_DOUBLES = TT_STATIC_MAX_BLK + TT_STATIC_MAX_STAGE + TT_STATIC_MAX_BLK / 2;  // counts: int32
+static_assert(TT_STATIC_MAX_PAIRS % ttk::CLS_THREADS == 0 && TT_STATIC_MAX_BLK % 2 == 0, "scratch layout");
+static __device__ __align__(256) double tt_static_scratch[TT_STATIC_DOUBLES];  // 768 KB + 64 B
+
 namespace {
 
 struct DevBuf {
@@ -86,6 +99,7 @@ struct tt_ctx {
   DevBuf mb_keys[2], mb_ptr, mb_adj, mb_rest, mb_part, mb_num;
   int64_t mb_nV = -1, mb_half = 0;
   double mb_k = 0.0;
+  double* static_scratch = nullptr;  // device address of tt_static_scratch on opt.device (tt_create)
   DevBuf possig;  // [2] u64: checksum of pos at tt_hess_symbolic, and at the last numeric / H.p call
   // broad phase (tt_broad_phase): boxes, grid, (cell, triangle) records, pair keys, result
   DevBuf bp_box, bp_part, bp_grid, bp_cnt, bp_off, bp_keys[2], bp_vals[2], bp_pcnt, bp_poff, bp_pkeys[2], bp_pairs;
@@ -344,6 +358,91 @@ tt_status energy_impl(tt_ctx* ctx, const tt_problem* q, void* energy_sum, void* 
   if (active_mask && q->n_pairs > 0)
     TT_CUDA(cudaMemcpyAsync(active_mask, ctx->mask.p, sizeof(uint32_t) * (size_t)((q->n_pairs + 31) / 32),
                             cudaMemcpyDeviceToDevice, st));
+  return TT_OK;
+}
+
+// ---- tt_energy_static: K1's energy / active count with the scratch in tt_static_scratch; allocates nothing ---------
+// The variant of k_classify that keeps only what the total needs: same gather, same Moeller intervals, same per-pair
+// energy, same CTA size and the same fixed-order CTA tree, so its per-CTA partials are the ones k_classify writes and
+// the two-level final sum below is sum_partials' -- the result is bit-identical to tt_energy's.
+template <typename T>
+__global__ void __launch_bounds__(ttk::CLS_THREADS, TT_CLS_MIN_CTAS)
+k_energy_static(const T* __restrict__ pos, const int* __restrict__ tris, const int2* __restrict__ pairs, int64_t P,
+                double sigma, double* __restrict__ blk_energy, int* __restrict__ blk_count) {
+  using namespace ttk;
+  __shared__ double s_e[CLS_THREADS / 32];
+  __shared__ int s_c[CLS_THREADS / 32];
+  const int64_t k = (int64_t)blockIdx.x * CLS_THREADS + threadIdx.x;
+  bool active = false;
+  double en = 0.0;
+  if (k < P) {
+    const int2 pr = __ldg(pairs + k);
+    int va[3], vb[3];
+    d3 a[3], b[3];
+    if (gather_pair(pos, tris, pr.x, pr.y, va, vb, a, b)) {
+      ttg::PairGeom g;
+      active = ttg::pair_intervals(a[0], a[1], a[2], b[0], b[1], b[2], sigma, g);
+      if (active) {
+        const double pr2 = g.tc0 * g.tc1;
+        en = pr2 * pr2;  // Eq. 2
+      }
+    }
+  }
+  const uint32_t bal = __ballot_sync(0xffffffffu, active);
+  if ((threadIdx.x & 31) == 0) s_c[threadIdx.x >> 5] = __popc(bal);
+  const double e = block_sum<CLS_THREADS>(en, s_e);  // its barrier also orders s_c
+  if (threadIdx.x == 0) {
+    int c = 0;
+#pragma unroll
+    for (int i = 0; i < CLS_THREADS / 32; ++i) c += s_c[i];
+    blk_count[blockIdx.x] = c;
+    blk_energy[blockIdx.x] = e;
+  }
+}
+// one CTA: n_active = sum of the per-CTA counts (integers: any order gives the same result)
+__global__ void __launch_bounds__(1024) k_count_static(const int* __restrict__ blk_count, int64_t n, int64_t* __restrict__ out) {
+  __shared__ long long s[32];
+  long long v = 0;
+  for (int64_t i = threadIdx.x; i < n; i += 1024) v += blk_count[i];
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) v += __shfl_down_sync(0xffffffffu, v, o);
+  if ((threadIdx.x & 31) == 0) s[threadIdx.x >> 5] = v;
+  __syncthreads();
+  if (threadIdx.x < 32) {
+    v = s[threadIdx.x];
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) v += __shfl_down_sync(0xffffffffu, v, o);
+    if (threadIdx.x == 0) out[0] = (int64_t)v;
+  }
+}
+template <typename T>
+tt_status energy_static_impl(tt_ctx* ctx, const tt_problem* q, void* energy_sum, int64_t* n_active, cudaStream_t st) {
+  using namespace ttk;
+  const int64_t P = q->n_pairs;
+  const int64_t nblk = (P + CLS_THREADS - 1) / CLS_THREADS;
+  double* blk_energy = ctx->static_scratch;
+  double* stage = blk_energy + TT_STATIC_MAX_BLK;
+  int* blk_count = reinterpret_cast<int*>(stage + TT_STATIC_MAX_STAGE);
+  if (nblk > 0) {
+    k_energy_static<T><<<(unsigned)nblk, CLS_THREADS, 0, st>>>((const T*)q->pos, q->tris, (const int2*)q->pairs, P, ctx->opt.tc_scale,
+                                                                blk_energy, blk_count);
+    TT_LAUNCH_CHECK();
+  }
+  const double* part = blk_energy;
+  int64_t n = nblk;
+  if (n > 4 * SUM_SLICE) {  // the same two levels as sum_partials
+    const int64_t ns = (n + SUM_SLICE - 1) / SUM_SLICE;
+    k_sum_stage<<<(unsigned)ns, 256, 0, st>>>(part, n, stage);
+    TT_LAUNCH_CHECK();
+    part = stage;
+    n = ns;
+  }
+  k_sum_partials<T><<<1, 1024, 0, st>>>(part, n, 1.0, (T*)energy_sum);
+  TT_LAUNCH_CHECK();
+  if (n_active) {
+    k_count_static<<<1, 1024, 0, st>>>(blk_count, nblk, n_active);
+    TT_LAUNCH_CHECK();
+  }
   return TT_OK;
 }
 
@@ -1230,6 +1329,9 @@ tt_status tt_create(const tt_options* opt, tt_ctx** out) {
     opt_in((const void*)ttk::k_assemble_long_tile<double, false>, sizeof(ttk::LongTileSmem<double, false>));
     opt_in((const void*)ttk::k_assemble_long_tile<float, true>, sizeof(ttk::LongTileSmem<float, true>));
     opt_in((const void*)ttk::k_assemble_long_tile<float, false>, sizeof(ttk::LongTileSmem<float, false>));
+    // tt_energy_static's scratch: the device address of the file-scope array on THIS device (the name itself is a host
+    // stand-in); asked for here, at set-up, so that the entry point itself does nothing but launch
+    if (e == cudaSuccess) e = cudaGetSymbolAddress((void**)&c->static_scratch, tt_static_scratch);
     if (e != cudaSuccess) { (void)cudaGetLastError(); delete c; return TT_ERR_CUDA; }
     auto pipe_setup = [&](const void* f, size_t smem, int& grid) {
       int nb = 0;
@@ -1272,6 +1374,20 @@ tt_status tt_energy(tt_ctx* ctx, const tt_problem* prob, void* energy_sum, void*
   return ctx->opt.dtype == TT_F64
              ? energy_impl<double>(ctx, prob, energy_sum, energy_per_pair, active_mask, tc, n_active, st)
              : energy_impl<float>(ctx, prob, energy_sum, energy_per_pair, active_mask, tc, n_active, st);
+}
+
+tt_status tt_energy_static(tt_ctx* ctx, const tt_problem* prob, void* energy_sum, int64_t* n_active, void* stream) {
+  tt_status s = check_problem(ctx, prob);
+  if (s != TT_OK) return s;
+  if (!energy_sum) return fail(ctx, TT_ERR_INVALID_ARG, "energy_sum is NULL");
+  if (prob->n_pairs > TT_STATIC_MAX_PAIRS)
+    return fail(ctx, TT_ERR_CAPACITY, "tt_energy_static: n_pairs %lld exceeds TT_STATIC_MAX_PAIRS = %lld (the size of the library's static scratch); use tt_energy",
+                (long long)prob->n_pairs, (long long)TT_STATIC_MAX_PAIRS);
+  if (!ctx->static_scratch) return fail(ctx, TT_ERR_STATE, "tt_energy_static: the static scratch has no device address");
+  TT_CUDA(cudaSetDevice(ctx->opt.device));
+  cudaStream_t st = (cudaStream_t)stream;
+  return ctx->opt.dtype == TT_F64 ? energy_static_impl<double>(ctx, prob, energy_sum, n_active, st)
+                                  : energy_static_impl<float>(ctx, prob, energy_sum, n_active, st);
 }
 
 tt_status tt_hess_symbolic(tt_ctx* ctx, const tt_problem* prob, int64_t* nnzb_host, int64_t* n_active_host,

@@ -19,11 +19,12 @@ LIB_PATH = Path(os.environ["TT_LIB_PATH"]) if os.environ.get("TT_LIB_PATH") else
 TT_OK = 0
 TT_F64, TT_F32 = 0, 1
 TT_HESS_EQ4, TT_HESS_FILTER, TT_HESS_PSD2, TT_HESS_PSDPROJ, TT_HESS_EXACT = 0, 1, 2, 3, 4
+TT_STATIC_MAX_PAIRS = 1 << 24   # tt_energy_static (include/tt.h)
 TT_FLAG_FORCE_GENERAL_ROWS = 1
 TT_FLAG_VALIDATE_INDICES = 2
 TT_FLAG_NO_STATE_CHECK = 4
 
-EXPORTS = ["tt_create", "tt_destroy", "tt_energy", "tt_hess_symbolic", "tt_energy_grad_hess", "tt_hess_vec",
+EXPORTS = ["tt_create", "tt_destroy", "tt_energy", "tt_energy_static", "tt_hess_symbolic", "tt_energy_grad_hess", "tt_hess_vec",
            "tt_energy_grad_hess_host", "tt_hess_pattern", "tt_broad_phase", "tt_broad_phase_pairs", "tt_broad_phase_copy", "tt_bsr_device", "tt_bsr_spmv", "tt_block_jacobi", "tt_pcg_solve", "tt_newton_step", "tt_untangle", "tt_membrane_build", "tt_membrane_energy_grad", "tt_membrane_hess_vec", "tt_stats", "tt_kernel_ms", "tt_kernel_ms_mean", "tt_probe_peaks", "tt_probe_gather", "tt_status_string", "tt_last_error"]
 
 
@@ -84,6 +85,8 @@ def load_library():
     lib.tt_destroy.restype = None
     lib.tt_energy.argtypes = [vp, ctypes.POINTER(TTProblem), vp, vp, vp, vp, vp, vp]
     lib.tt_energy.restype = ctypes.c_int
+    lib.tt_energy_static.argtypes = [vp, ctypes.POINTER(TTProblem), vp, vp, vp]
+    lib.tt_energy_static.restype = ctypes.c_int
     lib.tt_hess_symbolic.argtypes = [vp, ctypes.POINTER(TTProblem), ctypes.POINTER(i64), ctypes.POINTER(i64), vp]
     lib.tt_hess_symbolic.restype = ctypes.c_int
     lib.tt_energy_grad_hess.argtypes = [vp, ctypes.POINTER(TTProblem), vp, vp, vp, vp, vp, i64, vp]
@@ -199,6 +202,12 @@ class Context:
     def tt_energy(self, prob, energy_sum, energy_per_pair=None, active_mask=None, tc=None, n_active=None, stream=None):
         self._check(self.lib.tt_energy(self.h, ctypes.byref(prob[0]), _ptr(energy_sum), _ptr(energy_per_pair),
                                        _ptr(active_mask), _ptr(tc), _ptr(n_active), _stream_ptr(stream)))
+
+    def tt_energy_static(self, prob, energy_sum, n_active=None, stream=None):
+        """tt_energy's total (and active count) with the scratch in the library's static device array: no allocation,
+        no synchronisation; at most TT_STATIC_MAX_PAIRS candidates."""
+        self._check(self.lib.tt_energy_static(self.h, ctypes.byref(prob[0]), _ptr(energy_sum), _ptr(n_active),
+                                              _stream_ptr(stream)))
 
     # ---- tt_hess_symbolic ----
     def tt_hess_symbolic(self, prob, stream=None):
