@@ -1348,6 +1348,13 @@ __device__ __forceinline__ void cp_async_wait() { asm volatile("cp.async.wait_gr
 #define TT_RED_UNR 8                      // entries per triangle whose staged values are loaded up front
 #endif
 constexpr int RED_UNR = TT_RED_UNR;
+#ifndef TT_RED_UNR1
+#define TT_RED_UNR1 6                     // the same for the one-pass sums (four chains: fewer values each)
+#endif
+constexpr int RED_UNR1 = TT_RED_UNR1;
+#ifndef TT_TILE_ONEPASS
+#define TT_TILE_ONEPASS 1
+#endif
 #ifndef TT_TILE_NBUF
 #define TT_TILE_NBUF 2                    // row tiles per warp: with two, a row is built while the copy engine reads the previous one
 #endif
@@ -1356,6 +1363,7 @@ constexpr int NDIAG = 45;                 // upper triangle of the symmetric 9x9
 constexpr int NSTG = NDIAG + 9;           // + gradient of the three own vertices
 constexpr int STG_PASS = NSTG / 2;        // the 54 per-entry values are staged in two passes of 27
 constexpr int STG_STRIDE = STG_PASS;      // 27 doubles: odd, so lane = entry writes are conflict-free
+constexpr int STG1_STRIDE = NSTG + 1;     // one-pass staging (all 54 values of an entry at once): 55 doubles, odd
 constexpr int LONG_STRIDE = 31;           // k_assemble_long: 27 + 3 staged values per entry, odd stride
 
 template <typename T, int MT>  // MT: slots per round this instantiation of K4 is built for
@@ -1363,9 +1371,15 @@ struct TileCfg {
   static constexpr int RUN_UNIT = 27 * (int)sizeof(T);  // bytes one entry (or the diagonal) adds to a row run
   static constexpr int TILE_BYTES = RUN_UNIT * (RND_MAX_ENT + MT) + 32 * MT;
   static constexpr int STAGE_BYTES = 32 * STG_STRIDE * (int)sizeof(double);
-  static constexpr int UNION_BYTES = TILE_BYTES > STAGE_BYTES ? TILE_BYTES : STAGE_BYTES;
   // fp64 with 16 slots per round: two tiles per warp would not leave room for 8 warps per SM
   static constexpr int NBUF = (MT > RND_TRI_LOW && sizeof(T) == 8) ? 1 : TT_TILE_NBUF;
+  // With two tiles the staging area may span both: all 54 values of an entry are staged at once and summed in one loop
+  // (four independent chains instead of two, half the shuffles and warp barriers; the 36 registers of the diagonal
+  // factors are dead before the sums start).
+  static constexpr bool ONEPASS = (NBUF == 2) && (TT_TILE_ONEPASS != 0);
+  static constexpr int STAGE1_HALF = ((32 * STG1_STRIDE * (int)sizeof(double) / 2) + 15) & ~15;
+  static constexpr int UNION0 = TILE_BYTES > STAGE_BYTES ? TILE_BYTES : STAGE_BYTES;
+  static constexpr int UNION_BYTES = (ONEPASS && STAGE1_HALF > UNION0) ? STAGE1_HALF : UNION0;
   static_assert(UNION_BYTES % 16 == 0, "tile buffers must stay 16-byte aligned");
 };
 
@@ -1444,6 +1458,12 @@ __device__ __forceinline__ void load_round_ops(const AsmParams<T>& P, const int4
 // split triangles (more than 32 partners); without any -- up to ~15 M pairs on BASELINE's 2 M-triangle soup -- the
 // instantiation without their code runs: the kernel sits at 254 of 255 registers and the few selects and the ballot
 // of the part path cost it 3 % (measured, profiles/r2_step_breakdown.md).
+#ifdef TT_K4_PROFILE
+__device__ unsigned long long tt_k4_prof[16];
+#define K4_MARK(i) { const long long t_ = clock64(); prof[i] += t_ - tprev; tprev = t_; }
+#else
+#define K4_MARK(i)
+#endif
 template <typename T, bool PROJ, bool PARTS, int MT>
 __global__ void __maxnreg__(TT_TILE_MAXNREG)
 k_assemble_tile(const AsmParams<T> P) {
@@ -1477,6 +1497,10 @@ k_assemble_tile(const AsmParams<T> P) {
   }
   load_round_ids(P, d_nxt, lane, ids_nxt);
 
+#ifdef TT_K4_PROFILE
+  long long prof[10] = {0, 0, 0, 0, 0, 0, 0, 0, 0, 0};
+  long long tprev = clock64();
+#endif
   while (true) {
     const bool has_next = c + G < P.n_chunks;
     const int e_lo = d_cur.x, nent = d_cur.y, t_lo = d_cur.z, ntri = d_cur.w;
@@ -1495,6 +1519,7 @@ k_assemble_tile(const AsmParams<T> P) {
     E.en = 0.0;
     int er[3] = {cur.er[0], cur.er[1], cur.er[2]};
     if (valid) eval_core<double, PROJ>(x, cur.pay, P.sigma, P.hess_mode, E);
+    K4_MARK(0)
     // ---- operands of round c + G, vertex ids of c + 2G, descriptor of c + 3G: requested after the
     //      register peak of the derivative code, consumed a round later ----
     RoundOps nxt;
@@ -1504,12 +1529,14 @@ k_assemble_tile(const AsmParams<T> P) {
     const int4 d_nnn = (c + 3 * G < P.n_chunks) ? __ldg(P.rdesc + c + 3 * G) : dzero;
     // the staging area aliases the tile buffer of this round's first row: the copy engine must have read the row that
     // used it last (every lane commits one group per row, so "all but the NBUF - 1 newest groups" means exactly that)
-    double* const stage = reinterpret_cast<double*>(S.tile + (krow % NBUF) * UNION_BYTES);
-    bulk_wait_read_n<NBUF - 1>();
+    constexpr bool ONEPASS = TileCfg<T, MT>::ONEPASS;  // the staging area spans both tile buffers
+    double* const stage = reinterpret_cast<double*>(S.tile + (ONEPASS ? 0 : (krow % NBUF) * UNION_BYTES));
+    bulk_wait_read_n<ONEPASS ? 0 : NBUF - 1>();
     __syncwarp();
     if (valid) {
       unpermute_own(E, er);
     }
+    K4_MARK(1)
 
     if (!is_long) {
       // lane = triangle: tile slots (16-byte slots, prefix sum over the round's triangles)
@@ -1538,6 +1565,71 @@ k_assemble_tile(const AsmParams<T> P) {
         d0[i] = E.cf.c00 * E.g0[i] + E.cf.c01 * E.g1[i];
         d1[i] = E.cf.c01 * E.g0[i] + E.cf.c11 * E.g1[i];
       }
+      K4_MARK(2)
+      if constexpr (ONEPASS) {
+        if (valid) {
+          double* st = stage + lane * STG1_STRIDE;
+          int k = 0;
+#pragma unroll
+          for (int r = 0; r < 9; ++r)
+#pragma unroll
+            for (int q = r; q < 9; ++q, ++k) st[k] = E.g0[r] * d0[q] + E.g1[r] * d1[q];
+#pragma unroll
+          for (int i = 0; i < 9; ++i) st[NDIAG + i] = E.cf.cg0 * E.g0[i] + E.cf.cg1 * E.g1[i];
+        }
+        __syncwarp();
+        K4_MARK(3)
+        // per-triangle sums: lane = components (lane, lane + 27), entries in ascending order (deterministic); two
+        // triangles at a time: four independent load -> add chains in flight
+        for (int tt = 0; tt < ntri; tt += 2) {
+          const int a0 = __shfl_sync(FULL, my_first, tt), a1 = __shfl_sync(FULL, my_first, tt + 1);
+          const int b1 = __shfl_sync(FULL, my_first, tt + 2);
+          const int dA = a1 - a0, dB = b1 - a1, dn = max(dA, dB);
+          if (lane < STG_PASS) {
+            const double* pA = stage + a0 * STG1_STRIDE + lane;
+            const double* pB = stage + a1 * STG1_STRIDE + lane;
+            double vA0[RED_UNR1], vA1[RED_UNR1], vB0[RED_UNR1], vB1[RED_UNR1];
+#pragma unroll
+            for (int j = 0; j < RED_UNR1; ++j) {
+              vA0[j] = (j < dA) ? pA[j * STG1_STRIDE] : 0.0;
+              vA1[j] = (j < dA) ? pA[j * STG1_STRIDE + STG_PASS] : 0.0;
+              vB0[j] = (j < dB) ? pB[j * STG1_STRIDE] : 0.0;
+              vB1[j] = (j < dB) ? pB[j * STG1_STRIDE + STG_PASS] : 0.0;
+            }
+            double accA0 = vA0[0], accA1 = vA1[0], accB0 = vB0[0], accB1 = vB1[0];
+#pragma unroll
+            for (int j = 1; j < RED_UNR1; ++j) {
+              accA0 += vA0[j];
+              accA1 += vA1[j];
+              accB0 += vB0[j];
+              accB1 += vB1[j];
+            }
+            for (int j = RED_UNR1; j < dn; ++j) {
+              if (j < dA) {
+                accA0 += pA[j * STG1_STRIDE];
+                accA1 += pA[j * STG1_STRIDE + STG_PASS];
+              }
+              if (j < dB) {
+                accB0 += pB[j * STG1_STRIDE];
+                accB1 += pB[j * STG1_STRIDE + STG_PASS];
+              }
+            }
+            S.dsum[tt][lane] = accA0;
+            S.dsum[tt][STG_PASS + lane] = accA1;
+            if (dB > 0) {
+              S.dsum[tt + 1][lane] = accB0;
+              S.dsum[tt + 1][STG_PASS + lane] = accB1;
+            }
+            if (lane >= NDIAG - STG_PASS) {  // gradient of the triangle's three vertices
+              T* ts = P.tslot + 9 * ((int64_t)t_lo + tt) + (lane - (NDIAG - STG_PASS));
+              ts[0] = (T)accA1;
+              if (dB > 0) ts[9] = (T)accB1;
+            }
+          }
+        }
+        __syncwarp();
+        K4_MARK(4)
+      } else
 #pragma unroll
       for (int h = 0; h < 2; ++h) {
         if (valid) {
@@ -1554,6 +1646,7 @@ k_assemble_tile(const AsmParams<T> P) {
               st[NDIAG + i] = E.cf.cg0 * E.g0[i] + E.cf.cg1 * E.g1[i];
         }
         __syncwarp();
+        K4_MARK(3)
         // per-triangle sums, lane = component, entries in ascending order (deterministic); two
         // triangles at a time so that two independent load -> add chains are in flight.  The loops
         // are warp-uniform: lanes >= STG_PASS only take part in the shuffles.
@@ -1593,6 +1686,7 @@ k_assemble_tile(const AsmParams<T> P) {
           }
         }
         __syncwarp();
+        K4_MARK(4)
       }
 
       if (PARTS) {  // parts hand their diagonal partial sums to k_split_finish
@@ -1650,6 +1744,7 @@ k_assemble_tile(const AsmParams<T> P) {
               for (int j = 0; j < 3; ++j) blk[3 * i + j] = at[i] * p0[j] + bt[i] * p1[j];
           }
         }
+        K4_MARK(5)
         // diagonal-row blocks (p_m, p_n): lane = element (n, i, j), from the packed upper triangle
         if (lane < 27) {
           const int r_ = 3 * m + cq / 3, c_ = 3 * cn + cq % 3;
@@ -1668,6 +1763,7 @@ k_assemble_tile(const AsmParams<T> P) {
         }
         // positions of the next round (L2 hits): requested as soon as this round's J is dead
         if (m == 2 && lane < round_entries(d_nxt)) load_pos18(P.pos, ids_nxt, x);
+        K4_MARK(6)
         fence_async_smem();
         __syncwarp();
         // ---- lane = triangle: hand the run to the copy engine ----
@@ -1689,6 +1785,7 @@ k_assemble_tile(const AsmParams<T> P) {
           }
         }
         bulk_commit();  // by every lane, so that all lanes count the same groups
+        K4_MARK(7)
       }
     }
     if (is_long && lane < round_entries(d_nxt)) load_pos18(P.pos, ids_nxt, x);
@@ -1696,6 +1793,7 @@ k_assemble_tile(const AsmParams<T> P) {
 #pragma unroll
     for (int o = 16; o > 0; o >>= 1) e_acc += __shfl_down_sync(FULL, e_acc, o);
     if (lane == 0) P.chunk_energy[c] = e_acc;  // 0 for a long round: k_assemble_long overwrites it
+    K4_MARK(8)
     if (!has_next) break;
     c += G;
     d_cur = d_nxt;
@@ -1706,6 +1804,9 @@ k_assemble_tile(const AsmParams<T> P) {
     for (int i = 0; i < 6; ++i) ids_nxt[i] = ids_nn[i];
   }
   bulk_wait_all();  // shared memory must outlive the engine's reads
+#ifdef TT_K4_PROFILE
+  if (lane == 0) for (int i = 0; i < 10; ++i) atomicAdd(&tt_k4_prof[i], (unsigned long long)prof[i]);
+#endif
 }
 
 // Long triangles with at most LONG_TILE_MAX partners (a round of their own): one warp per triangle.

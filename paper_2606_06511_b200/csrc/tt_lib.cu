@@ -1376,6 +1376,14 @@ tt_status tt_energy(tt_ctx* ctx, const tt_problem* prob, void* energy_sum, void*
              : energy_impl<float>(ctx, prob, energy_sum, energy_per_pair, active_mask, tc, n_active, st);
 }
 
+#ifdef TT_K4_PROFILE
+int tt_debug_k4_prof(unsigned long long* out16, int reset) {
+  cudaDeviceSynchronize();
+  if (out16) cudaMemcpyFromSymbol(out16, ttk::tt_k4_prof, 16 * sizeof(unsigned long long));
+  if (reset) { unsigned long long z[16] = {0}; cudaMemcpyToSymbol(ttk::tt_k4_prof, z, sizeof(z)); }
+  return 0;
+}
+#endif
 tt_status tt_energy_static(tt_ctx* ctx, const tt_problem* prob, void* energy_sum, int64_t* n_active, void* stream) {
   tt_status s = check_problem(ctx, prob);
   if (s != TT_OK) return s;
