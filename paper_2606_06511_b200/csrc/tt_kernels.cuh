@@ -2189,7 +2189,9 @@ struct PipeWarpSmem {
 struct PipeOps {
   int ids[6];      // lane = entry: canonical pair, recorded order
   unsigned pay;
-  int f;           // lane = triangle: first entry of the triangle, relative to the round
+  int f;           // lane = triangle: first entry of the triangle (ABSOLUTE: the round's first entry d.x is subtracted
+                   // where f is used, rounds later -- subtracting it here made the load's first use immediate and left
+                   // its latency exposed: 14 % of K6's stall samples sat on that one subtraction)
 };
 template <typename T>
 __device__ __forceinline__ void load_pipe_ops(const AsmParams<T>& P, const int4 d, int lane, PipeOps& R) {
@@ -2205,7 +2207,7 @@ __device__ __forceinline__ void load_pipe_ops(const AsmParams<T>& P, const int4 
     R.ids[0] = v0.x; R.ids[1] = v0.y; R.ids[2] = v1.x; R.ids[3] = v1.y; R.ids[4] = v2.x; R.ids[5] = v2.y;
     R.pay = (unsigned)__ldg(P.dvals + e);
   }
-  if (lane < d.w) R.f = __ldg(P.tfirst + d.z + lane) - d.x;
+  if (lane < d.w) R.f = __ldg(P.tfirst + d.z + lane);
 }
 __device__ __forceinline__ void own_first_ids(const PipeOps& R, int (&pid)[6]) {
   const bool side = (R.pay & 1u) != 0u;
@@ -2234,7 +2236,7 @@ __device__ __forceinline__ OwnMap issue_round_gather(const T* __restrict__ src, 
   constexpr unsigned FULL = 0xffffffffu;
   const bool ok = d.y <= RND_MAX_ENT;
   const bool valid = ok && lane < d.y;
-  const unsigned heads = __reduce_or_sync(FULL, (ok && lane < d.w) ? (1u << o.f) : 0u) | 1u;
+  const unsigned heads = __reduce_or_sync(FULL, (ok && lane < d.w) ? (1u << (o.f - d.x)) : 0u) | 1u;
   const unsigned below = heads & (0xffffffffu >> (31 - lane));
   const int head_lane = 31 - __clz((int)below);
   int pid[6];
@@ -2365,7 +2367,7 @@ k_entry_pipe(const AsmParams<T> P) {
       cp_async_commit();
     }
     if (!is_long) {
-      const unsigned heads = __reduce_or_sync(FULL, tri_lane ? (1u << cur.f) : 0u) | 1u;  // bit i: entry i opens a triangle
+      const unsigned heads = __reduce_or_sync(FULL, tri_lane ? (1u << (cur.f - d_cur.x)) : 0u) | 1u;  // bit i: entry i opens a triangle
       const unsigned below = heads & (0xffffffffu >> (31 - lane));
       const int segf = 31 - __clz((int)below);
 #pragma unroll
