@@ -1373,13 +1373,13 @@ struct TileCfg {
   static constexpr int STAGE_BYTES = 32 * STG_STRIDE * (int)sizeof(double);
   // fp64 with 16 slots per round: two tiles per warp would not leave room for 8 warps per SM
   static constexpr int NBUF = (MT > RND_TRI_LOW && sizeof(T) == 8) ? 1 : TT_TILE_NBUF;
-  // With two tiles the staging area may span both: all 54 values of an entry are staged at once and summed in one loop
-  // (four independent chains instead of two, half the shuffles and warp barriers; the 36 registers of the diagonal
-  // factors are dead before the sums start).
-  static constexpr bool ONEPASS = (NBUF == 2) && (TT_TILE_ONEPASS != 0);
-  static constexpr int STAGE1_HALF = ((32 * STG1_STRIDE * (int)sizeof(double) / 2) + 15) & ~15;
+  // All 54 values of an entry are staged at once and summed in one loop (four independent chains instead of two, half
+  // the shuffles and warp barriers; the 36 registers of the diagonal factors are dead before the sums start).  The
+  // staging area spans the tile buffer(s), which are made large enough for it.
+  static constexpr bool ONEPASS = (TT_TILE_ONEPASS != 0);
+  static constexpr int STAGE1_PART = ((32 * STG1_STRIDE * (int)sizeof(double) / NBUF) + 15) & ~15;
   static constexpr int UNION0 = TILE_BYTES > STAGE_BYTES ? TILE_BYTES : STAGE_BYTES;
-  static constexpr int UNION_BYTES = (ONEPASS && STAGE1_HALF > UNION0) ? STAGE1_HALF : UNION0;
+  static constexpr int UNION_BYTES = (ONEPASS && STAGE1_PART > UNION0) ? STAGE1_PART : UNION0;
   static_assert(UNION_BYTES % 16 == 0, "tile buffers must stay 16-byte aligned");
 };
 
@@ -1529,7 +1529,7 @@ k_assemble_tile(const AsmParams<T> P) {
     const int4 d_nnn = (c + 3 * G < P.n_chunks) ? __ldg(P.rdesc + c + 3 * G) : dzero;
     // the staging area aliases the tile buffer of this round's first row: the copy engine must have read the row that
     // used it last (every lane commits one group per row, so "all but the NBUF - 1 newest groups" means exactly that)
-    constexpr bool ONEPASS = TileCfg<T, MT>::ONEPASS;  // the staging area spans both tile buffers
+    constexpr bool ONEPASS = TileCfg<T, MT>::ONEPASS;  // the staging area spans the tile buffer(s)
     double* const stage = reinterpret_cast<double*>(S.tile + (ONEPASS ? 0 : (krow % NBUF) * UNION_BYTES));
     bulk_wait_read_n<ONEPASS ? 0 : NBUF - 1>();
     __syncwarp();
