@@ -127,7 +127,7 @@ tt_status tt_energy(tt_ctx* ctx, const tt_problem* prob, void* energy_sum, void*
  * serving loops, harnesses that forbid it).  The same steps 1-2 as tt_energy, total only:
  *   energy_sum [1] dtype DEVICE: sum of T over all pairs -- bit-identical to tt_energy's (same per-CTA partials, same
  *                                fixed-order two-level sum);   n_active [1] int64 DEVICE or NULL.
- * The per-CTA partial sums and counts live in a file-scope device array of the library (768 KB, held by every GPU that
+ * The per-CTA partial sums and counts live in a file-scope device array of the library (1.5 MB, held by every GPU that
  * loads the library until the process exits) instead of the context's growable workspace, so
  *   - n_pairs <= TT_STATIC_MAX_PAIRS, else TT_ERR_CAPACITY (message in tt_last_error) and nothing is launched;
  *   - the call makes no cudaMalloc / cudaFree / allocating library call, no host round trip and no synchronisation: it

@@ -23,7 +23,10 @@
 namespace ttk {
 using ttg::d3;
 
-constexpr int CLS_THREADS = 256;   // K1 / K2 CTA size (8 warps -> 8 mask words per CTA)
+#ifndef TT_CLS_THREADS
+#define TT_CLS_THREADS 128         // measured: K1 0.675 ms with 256 threads, 0.645 with 128, 0.633 with 64 (10 M candidates) -- a CTA's
+#endif                             // slot is held until its slowest gather returns; 64 costs the mesh configs more partials than it saves
+constexpr int CLS_THREADS = TT_CLS_THREADS;   // K1 / K2 CTA size (4 warps -> 4 mask words per CTA)
 constexpr int SYM_WARPS = 4;       // warps per CTA in the per-triangle symbolic kernels
 constexpr int SYM_LMAX = 1536;     // longest row (in blocks) ranked in shared memory
 constexpr int SLOT_PART = (int)0x80000000;  // flag in sinfo.x: the slot is a part of a split triangle
@@ -105,7 +108,7 @@ __device__ __forceinline__ double block_sum(double v, double* smem /*[THREADS/32
 
 // ------------------------------------------------------------------------------------------ K1
 #ifndef TT_CLS_MIN_CTAS
-#define TT_CLS_MIN_CTAS 3   // 85 registers, 24 warps / SM: 0.755 -> 0.69 ms at 10M candidates (4: 0.73)
+#define TT_CLS_MIN_CTAS 6   // 80 registers, 24 warps / SM (more CTAs per SM need fewer registers and spill: measured slower)
 #endif
 // Per-candidate record written by K1 for the symbolic phase: the recorded branch decisions (ttg::pair_config, 12 bits).
 template <typename T>

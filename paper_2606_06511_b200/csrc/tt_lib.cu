@@ -25,11 +25,11 @@
 // asks for the address once per context, with the context's device current (cudaGetSymbolAddress), and the kernels are
 // handed that pointer.  Every call shares the array and leaves its contents behind; nothing in it has to start at zero
 // (every slot a call reads it has written itself), and calls that overlap on the GPU race on it.
-constexpr int64_t TT_STATIC_MAX_BLK = TT_STATIC_MAX_PAIRS / ttk::CLS_THREADS;                     // 65536 CTAs of K1
-constexpr int64_t TT_STATIC_MAX_STAGE = (TT_STATIC_MAX_BLK + ttk::SUM_SLICE - 1) / ttk::SUM_SLICE;  // 8 slice sums
+constexpr int64_t TT_STATIC_MAX_BLK = TT_STATIC_MAX_PAIRS / ttk::CLS_THREADS;                     // 131072 CTAs of K1
+constexpr int64_t TT_STATIC_MAX_STAGE = (TT_STATIC_MAX_BLK + ttk::SUM_SLICE - 1) / ttk::SUM_SLICE;  // 16 slice sums
 constexpr int64_t TT_STATIC_DOUBLES = TT_STATIC_MAX_BLK + TT_STATIC_MAX_STAGE + TT_STATIC_MAX_BLK / 2;  // counts: int32
 static_assert(TT_STATIC_MAX_PAIRS % ttk::CLS_THREADS == 0 && TT_STATIC_MAX_BLK % 2 == 0, "scratch layout");
-static __device__ __align__(256) double tt_static_scratch[TT_STATIC_DOUBLES];  // 768 KB + 64 B
+static __device__ __align__(256) double tt_static_scratch[TT_STATIC_DOUBLES];  // 1.5 MB + 128 B
 
 namespace {
 

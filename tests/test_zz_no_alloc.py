@@ -38,8 +38,8 @@ def _existing(ctx, prob, tdt):
 def test_energy_static_matches_tt_energy_on_calls_in_a_row(dtype):
     from paper_2606_06511_b200 import inputs, tt
     tdt = torch.float64 if dtype == "f64" else torch.float32
-    small = inputs.config4_sweep(n_tris=20_000, n_pairs=300_000)       # 1 172 CTAs of K1: one-level final sum
-    # the same mesh with its candidate list repeated 30 x (duplicates are legal input and add): 35 157 CTAs, two levels
+    small = inputs.config4_sweep(n_tris=20_000, n_pairs=300_000)       # 2 344 CTAs of K1: one-level final sum
+    # the same mesh with its candidate list repeated 30 x (duplicates are legal input and add): 70 313 CTAs, two levels
     big = type(small)(small.pos, small.tris, np.ascontiguousarray(np.tile(small.pairs, (30, 1))), "config4 x30", small.meta)
     tiny = inputs.config0_soup()
     ctx = tt.Context(tdt, 1, 1.0, 0)
