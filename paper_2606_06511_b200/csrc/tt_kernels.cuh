@@ -2181,12 +2181,17 @@ k_entry_reduce(const AsmParams<T> P, const int* __restrict__ round_list, int64_t
 #define TT_PIPE_MIN_CTAS 8
 #endif
 constexpr int PIPE_WARPS = TT_PIPE_WARPS;
+#ifndef TT_K6_SMEM_SUM
+#define TT_K6_SMEM_SUM 1
+#endif
 template <typename T, int MODE>
 struct PipeWarpSmem {
   T xp[2][9 * 32];                          // partner triangle's positions, lane-private slots [k * 32 + lane]
   T xo[2][9 * RND_MAX_TRI];                 // own triangle's positions, ONE copy per triangle (head lane's order)
   T pp[MODE == 2 ? 9 * 32 : 1];             // p of the partner's vertices
   T po[MODE == 2 ? 9 * RND_MAX_TRI : 1];    // p of the own vertices, one copy per triangle
+  double stgf[sizeof(T) == 8 ? 1 : 9 * 32];  // staging of the per-entry results (fp64 aliases xp[buf], dead by then)
+  int fst[RND_MAX_TRI + 2];                 // first entry of every triangle of the round, nent behind the last
 };
 
 struct PipeOps {
@@ -2370,6 +2375,35 @@ k_entry_pipe(const AsmParams<T> P) {
       cp_async_commit();
     }
     if (!is_long) {
+#if TT_K6_SMEM_SUM
+      // per-triangle sums through shared memory: every entry stages its 9 values, then lane = (triangle, component)
+      // adds the triangle's entries in ascending order (a segmented shuffle scan of 9 doubles costs 5 x 9 x 3
+      // instructions per lane; this is a third of it)
+      double* const stg = (sizeof(T) == 8) ? reinterpret_cast<double*>(S.xp[buf]) : S.stgf;
+      const int ntri = d_cur.w;
+      __syncwarp();  // every lane has read its positions out of xp[buf]
+      if (tri_lane) S.fst[lane] = cur.f - d_cur.x;
+      if (lane == 0) S.fst[ntri] = nent;
+      if (valid) {
+#pragma unroll
+        for (int k = 0; k < 9; ++k) stg[9 * lane + k] = v[k];
+      }
+      __syncwarp();
+      for (int i = lane; i < 9 * ntri; i += 32) {
+        const int t = i / 9, k = i - 9 * t;
+        const int a = S.fst[t], b = S.fst[t + 1];
+        const double* q = stg + 9 * a + k;
+        double acc0 = 0.0, acc1 = 0.0;
+        int e = a;
+        for (; e + 1 < b; e += 2, q += 18) {
+          acc0 += q[0];
+          acc1 += q[9];
+        }
+        if (e < b) acc0 += q[0];
+        P.tslot[9 * ((int64_t)d_cur.z + t) + k] = (T)(acc0 + acc1);
+      }
+      __syncwarp();  // the next round's gathers land in xp[buf]
+#else
       const unsigned heads = __reduce_or_sync(FULL, tri_lane ? (1u << (cur.f - d_cur.x)) : 0u) | 1u;  // bit i: entry i opens a triangle
       const unsigned below = heads & (0xffffffffu >> (31 - lane));
       const int segf = 31 - __clz((int)below);
@@ -2388,6 +2422,7 @@ k_entry_pipe(const AsmParams<T> P) {
 #pragma unroll
         for (int k = 0; k < 9; ++k) P.tslot[9 * ti + k] = (T)v[k];
       }
+#endif
       if (MODE == 1) {
 #pragma unroll
         for (int o = 16; o > 0; o >>= 1) e_acc += __shfl_down_sync(FULL, e_acc, o);
