@@ -65,6 +65,9 @@ def parse():
                          "given by --config (1, 2 or 3) for --steps steps; prints its own JSON line")
     ap.add_argument("--membrane", type=float, default=0.0,
                     help="with --untangle: stiffness k of the edge-spring membrane (SURVEY 8(f) NEXT-4, DESIGN.md A18); 0 = none")
+    ap.add_argument("--k4-phases", action="store_true",
+                    help="phase timers of the assembly kernel on the headline workload: needs the profiling build "
+                         "(python -m paper_2606_06511_b200.build --profile); prints its own JSON line")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     return ap.parse_args()
@@ -303,6 +306,44 @@ def run_solver(args):
     ctx.close()
 
 
+def run_k4_phases(args):
+    """Diagnostic, not a bench value: where a round of k_assemble_tile spends its cycles.  Loads the profiling build
+    (-DTT_K4_PROFILE: clock64() marks summed per phase over every round of a launch, read through tt_debug_k4_prof);
+    the marks serialise the phases a little, so the kernel runs a few per cent slower than the product's."""
+    import ctypes
+    from paper_2606_06511_b200 import build as _b
+    os.environ["TT_LIB_PATH"] = str(_b.build_profile())
+    import torch
+    from paper_2606_06511_b200 import inputs, tt
+    dev = torch.device("cuda", 0)
+    pb = inputs.config4_sweep(n_tris=args.tris, n_pairs=args.pairs)
+    tdt = torch.float64 if args.dtype == "f64" else torch.float32
+    ctx = tt.Context(tdt, args.hess_mode, 1.0, 0)
+    pos = torch.from_numpy(pb.pos).to(dev).to(tdt).contiguous()
+    out = tt.assemble(ctx, pos, torch.from_numpy(pb.tris).to(dev), torch.from_numpy(pb.pairs).to(dev), want_hess=True)
+    torch.cuda.synchronize()
+    buf = (ctypes.c_ulonglong * 16)()
+    ctx.lib.tt_debug_k4_prof(buf, 1)
+    n = max(int(args.steps), 1)
+    for _ in range(n):
+        ctx.tt_energy_grad_hess(out["prob"], out["energy"], out["grad"], out["rowptr"], out["colind"], out["vals"], out["nnzb"])
+    torch.cuda.synchronize()
+    ms = ctx.tt_kernel_ms()["assemble"]
+    ctx.lib.tt_debug_k4_prof(buf, 0)
+    names = ["derivatives (eval_core)", "operand loads, wait for the copy engine, unpermute", "slot offsets, diagonal factors",
+             "staging + barrier", "per-triangle sums + barrier", "rows: waits, offsets, off-diagonal blocks",
+             "rows: diagonal blocks, next positions", "rows: proxy fence, barrier, bulk-copy issue", "energy, loop"]
+    v = [float(buf[i]) for i in range(9)]
+    tot = sum(v) or 1.0
+    st = ctx.tt_stats()
+    print(json.dumps({"metric": "k_assemble_tile phase timers (profiling build, -DTT_K4_PROFILE)", "n_gpus": 1, "dtype": args.dtype,
+                      "data": "synthetic", "config": {"workload": "BASELINE %s: %d triangles, %d candidate pairs" % (WORKLOADS[4], pb.n_tris, pb.n_pairs)},
+                      "launches": n, "kernel_ms_profiling_build": ms, "rounds": st["rounds"],
+                      "cycles_per_round_per_warp": tot / n / max(st["rounds"], 1),
+                      "share": {nm: x / tot for nm, x in zip(names, v)}}), flush=True)
+    ctx.close()
+
+
 def run_untangle(args):
     """Side measurement, not the headline: the untangling loop on a mesh config -- per step one tt_broad_phase, one symbolic +
     numeric call, a block-Jacobi PCG solve and the Armijo line search on tt_energy.  Wall time per step (the loop synchronises
@@ -497,6 +538,9 @@ def main():
         return
     if args.solver:
         run_solver(args)
+        return
+    if args.k4_phases:
+        run_k4_phases(args)
         return
     if args.untangle:
         run_untangle(args)

@@ -34,6 +34,21 @@ def build(force: bool = False, verbose: bool = False) -> Path:
     return LIB
 
 
+PROFILE_LIB = HERE / "libtt_prof.so"
+
+
+def build_profile() -> Path:
+    """A second library with the phase timers of K4 compiled in (-DTT_K4_PROFILE: clock64() marks summed per phase,
+    read through tt_debug_k4_prof).  A profiling build: `bench.py --k4-phases` loads it; nothing else does."""
+    if PROFILE_LIB.exists() and all(PROFILE_LIB.stat().st_mtime >= d.stat().st_mtime for d in DEPS):
+        return PROFILE_LIB
+    subprocess.run([nvcc_path(), *NVCC_FLAGS, "-DTT_K4_PROFILE", str(SRC), "-o", str(PROFILE_LIB)], check=True)
+    return PROFILE_LIB
+
+
 if __name__ == "__main__":
-    build(force="--force" in sys.argv, verbose="-v" in sys.argv)
-    print(LIB)
+    if "--profile" in sys.argv:
+        print(build_profile())
+    else:
+        build(force="--force" in sys.argv, verbose="-v" in sys.argv)
+        print(LIB)
