@@ -1355,6 +1355,9 @@ constexpr int RED_UNR = TT_RED_UNR;
 #define TT_RED_UNR1 6                     // the same for the one-pass sums (four chains: fewer values each)
 #endif
 constexpr int RED_UNR1 = TT_RED_UNR1;
+#ifndef TT_RED_UNR1_WIDE
+#define TT_RED_UNR1_WIDE 3             // measured at 1 / 2 / 5 M pairs: 6 -> 0.374 / 0.629 / 1.234 ms, 4 -> 0.364 / 0.615 / 1.231, 3 -> 0.359 / 0.609 / 1.231, 2 -> 0.355 / 0.609 / 1.239
+#endif
 #ifndef TT_TILE_ONEPASS
 #define TT_TILE_ONEPASS 1
 #endif
@@ -1591,9 +1594,10 @@ k_assemble_tile(const AsmParams<T> P) {
           if (lane < STG_PASS) {
             const double* pA = stage + a0 * STG1_STRIDE + lane;
             const double* pB = stage + a1 * STG1_STRIDE + lane;
-            double vA0[RED_UNR1], vA1[RED_UNR1], vB0[RED_UNR1], vB1[RED_UNR1];
+            constexpr int RU1 = (MT > RND_TRI_LOW) ? TT_RED_UNR1_WIDE : RED_UNR1;  // 16-slot rounds: triangles with few entries
+            double vA0[RU1], vA1[RU1], vB0[RU1], vB1[RU1];
 #pragma unroll
-            for (int j = 0; j < RED_UNR1; ++j) {
+            for (int j = 0; j < RU1; ++j) {
               vA0[j] = (j < dA) ? pA[j * STG1_STRIDE] : 0.0;
               vA1[j] = (j < dA) ? pA[j * STG1_STRIDE + STG_PASS] : 0.0;
               vB0[j] = (j < dB) ? pB[j * STG1_STRIDE] : 0.0;
@@ -1601,13 +1605,13 @@ k_assemble_tile(const AsmParams<T> P) {
             }
             double accA0 = vA0[0], accA1 = vA1[0], accB0 = vB0[0], accB1 = vB1[0];
 #pragma unroll
-            for (int j = 1; j < RED_UNR1; ++j) {
+            for (int j = 1; j < RU1; ++j) {
               accA0 += vA0[j];
               accA1 += vA1[j];
               accB0 += vB0[j];
               accB1 += vB1[j];
             }
-            for (int j = RED_UNR1; j < dn; ++j) {
+            for (int j = RU1; j < dn; ++j) {
               if (j < dA) {
                 accA0 += pA[j * STG1_STRIDE];
                 accA1 += pA[j * STG1_STRIDE + STG_PASS];
